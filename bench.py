@@ -1,0 +1,447 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the LETKF hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+Headline (BASELINE.json `metric`): batched fp64 syev matrices/s at M=64, batch 16384
+(BASELINE config 3: A = ((M-1)/rho) I + Yb^T diag(r) Yb, p=98).  One step = one
+letkf_syev_batched call over the whole batch.  The fused analysis (config 4) is timed as well and
+reported under "analysis".  Prints ONE JSON line on rank 0.
+
+--impl reference times the CPU oracle (oracle/, plain Jacobi) on the host cores on a bounded
+sample of the same workload; it is a baseline, not a target.
+"""
+import argparse
+import ctypes
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "batched fp64 syev matrices/s at M=64 (batch 16384); % of FP64/HBM roofline"
+M_HEAD, BATCH_HEAD, P_HEAD = 64, 16384, 98
+SM_COUNT = 148
+DFMA_PER_CLK_SM = 64          # fp64 FMA lanes per SM (4 SMSPs x 16), DESIGN.md section 6
+
+
+def host_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def syev_model_flops(M):
+    return 9.0 * M ** 3                      # SURVEY.md section 8(d) convention
+
+
+def syev_bytes(M):
+    return 16.0 * M * M + 8.0 * M            # read A once, write V and w once
+
+
+def analysis_model_flops(M, p, ns):
+    return 2.0 * p * M * M + 2.0 * p * M + 9.0 * M ** 3 + 4.0 * M * M + 2.0 * M ** 3 + 2.0 * ns * M * M + M * M
+
+
+def analysis_bytes(M, p, ns):
+    return 8.0 * (p * M + 2 * p + 2 * ns * M)
+
+
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """Samples SM clock / throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.stop_flag = [], set(), False
+        self.max_mhz, self.power = None, []
+        self.thread = None
+        try:
+            import pynvml
+            self.nv = pynvml
+            pynvml.nvmlInit()
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+            "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+            "hw_power_brake": getattr(nv, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80),
+        }
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def start(self):
+        if self.nv is not None:
+            self.stop_flag = False
+            self.thread = threading.Thread(target=self._loop, daemon=True)
+            self.thread.start()
+
+    def stop(self):
+        self.stop_flag = True
+        if self.thread is not None:
+            self.thread.join()
+        out = {"sm_mhz": float(np.median(self.samples)) if self.samples else None,
+               "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+               "samples": len(self.samples)}
+        if self.power:
+            out["power_w_max"] = round(max(self.power), 1)
+        return out
+
+
+# ------------------------------------------------------------------------------------------------
+def time_oracle_syev(A, nthreads=0):
+    import oracle
+    oracle.build()
+    t0 = time.perf_counter()
+    _, _, info, nt = oracle.syev_batched(A, nthreads=nthreads)
+    dt = time.perf_counter() - t0
+    return A.shape[0] / dt, nt, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands on the host cores; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2308_03310_b200 import workloads as wl
+    sample = 4096
+    A = wl.letkf_shaped(sample, M_HEAD, P_HEAD, config_index=3)
+    for _ in range(args.warmup):
+        time_oracle_syev(A[:64])
+    t0 = time.perf_counter()
+    nt = 0
+    for _ in range(args.steps):
+        _, nt, _ = time_oracle_syev(A)
+    dt = time.perf_counter() - t0
+    value = sample * args.steps / dt
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "matrices/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config3: syev fp64 M=64 LETKF-shaped p=98 (bounded sample of the 16384 batch)"},
+        "cpu_baseline": {"value": value, "unit": "matrices/s", "cores": nt, "kind": "oracle",
+                         "sample": f"first {sample} matrices of config 3 per step (cyclic Jacobi, OpenMP over the batch)"},
+        "e2e": {"value": value, "unit": "matrices/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------
+def cusolver_compare(A_dev, steps=2):
+    """cusolverDnDsyevjBatched on the same device matrices: comparison only, never in the product."""
+    import torch
+    lib = None
+    for name in ("libcusolver.so.11", "libcusolver.so.12", "libcusolver.so"):
+        for d in ("", os.path.join(os.path.dirname(torch.__file__), "lib") + "/", "/usr/local/cuda/lib64/"):
+            try:
+                lib = ctypes.CDLL(d + name)
+                break
+            except OSError:
+                continue
+        if lib is not None:
+            break
+    if lib is None:
+        import glob
+        cands = glob.glob(os.path.join(sys.prefix, "lib", "python*", "site-packages", "nvidia", "cusolver", "lib", "libcusolver.so*"))
+        if not cands:
+            return {"unavailable": "libcusolver not found"}
+        lib = ctypes.CDLL(cands[0])
+    batch, M, _ = A_dev.shape
+    vp, ci = ctypes.c_void_p, ctypes.c_int
+    h = vp()
+    if lib.cusolverDnCreate(ctypes.byref(h)) != 0:
+        return {"unavailable": "cusolverDnCreate failed"}
+    lib.cusolverDnSetStream(h, vp(torch.cuda.current_stream().cuda_stream))
+    params = vp()
+    lib.cusolverDnCreateSyevjInfo(ctypes.byref(params))
+    jobz, uplo = 1, 0            # CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER
+    Awork = A_dev.clone()
+    W = torch.empty((batch, M), dtype=torch.float64, device="cuda")
+    info = torch.zeros((batch,), dtype=torch.int32, device="cuda")
+    lwork = ci(0)
+    lib.cusolverDnDsyevjBatched_bufferSize.argtypes = [vp, ci, ci, ci, vp, ci, vp, ctypes.POINTER(ci), vp, ci]
+    st = lib.cusolverDnDsyevjBatched_bufferSize(h, jobz, uplo, M, vp(Awork.data_ptr()), M, vp(W.data_ptr()),
+                                                ctypes.byref(lwork), params, batch)
+    if st != 0:
+        return {"unavailable": f"bufferSize status {st}"}
+    work = torch.empty((max(lwork.value, 1),), dtype=torch.float64, device="cuda")
+    lib.cusolverDnDsyevjBatched.argtypes = [vp, ci, ci, ci, vp, ci, vp, vp, ci, vp, vp, ci]
+    times = []
+    for it in range(steps + 1):
+        Awork.copy_(A_dev)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        st = lib.cusolverDnDsyevjBatched(h, jobz, uplo, M, vp(Awork.data_ptr()), M, vp(W.data_ptr()),
+                                         vp(work.data_ptr()), lwork.value, vp(info.data_ptr()), params, batch)
+        e1.record()
+        torch.cuda.synchronize()
+        if st != 0:
+            return {"unavailable": f"syevjBatched status {st}"}
+        if it > 0:
+            times.append(e0.elapsed_time(e1))
+    # residual of its answer on a sample (column-major output == V^T in our row-major view)
+    n = min(batch, 512)
+    V = Awork[:n].transpose(1, 2)
+    R = torch.matmul(A_dev[:n], V) - V * W[:n].unsqueeze(1)
+    res = float((R.flatten(1).norm(dim=1) / A_dev[:n].flatten(1).norm(dim=1)).max())
+    lib.cusolverDnDestroySyevjInfo(params)
+    lib.cusolverDnDestroy(h)
+    ms = float(np.median(times))
+    return {"routine": "cusolverDnDsyevjBatched (default tol/sweeps)", "ms": ms,
+            "matrices_per_s": batch / (ms * 1e-3), "max_residual_sample": res,
+            "info_nonzero": int((info != 0).sum())}
+
+
+# ------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2308_03310_b200 import build as b, letkf, workloads as wl
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); "
+                         "use --impl reference for the CPU oracle baseline")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        b.build()
+    if world > 1:
+        dist.barrier()
+    letkf.load()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    M, B, p = M_HEAD, BATCH_HEAD, P_HEAD
+    # weak scaling: every rank owns a full config-3 batch (its own seed); no data-path collective
+    A_host = wl.letkf_shaped(B, M, p, config_index=3 + 1000 * rank)
+    A = torch.from_numpy(A_host).cuda()
+    w = torch.empty((B, M), dtype=torch.float64, device="cuda")
+    V = torch.empty_like(A)
+    info = torch.zeros((B,), dtype=torch.int32, device="cuda")
+    work = torch.empty(letkf.syev_workspace_bytes(M, B), dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def step():
+        letkf.syev_batched(A, w=w, V=V, info=info, work=work, stream=stream)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    assert int(info.abs().max()) == 0, "QL did not converge on the bench workload"
+    launches_per_step = letkf.last_launch_count()
+
+    # ---- timed region: K steps, CUDA events on the launching stream, per-kernel events inside
+    letkf.profile_enable(True)
+    sampler = ClockSampler(local)
+    kern = {}
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.start()
+    e0.record(stream)
+    recs_all = []
+    for _ in range(args.steps):
+        step()
+        recs_all.append(None)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    ms_total = max_over_ranks(e0.elapsed_time(e1))
+    ms_step = ms_total / args.steps
+    # per-kernel durations of the LAST step (events are re-used per call), averaged over 3 more steps
+    nprof = 3
+    rot_total = 0
+    for _ in range(nprof):
+        step()
+        for name, ms in letkf.profile_records():
+            kern.setdefault(name, []).append(ms)
+        rot_total = letkf.profile_rotations()
+    letkf.profile_enable(False)
+    kern_ms = {k: float(np.sum(v) / nprof) for k, v in kern.items()}
+    rot_per_matrix = rot_total / float(B)
+    value = world * B / (ms_step * 1e-3)
+
+    # ---- roofline of the dominant kernel
+    sm_max = clocks.get("sm_max_mhz") or 1965.0
+    peak_tflops = SM_COUNT * DFMA_PER_CLK_SM * 2 * sm_max * 1e6 / 1e12
+    flops_by_kernel = {}
+    for k in kern_ms:
+        if "tridiag" in k:
+            flops_by_kernel[k] = (8.0 / 3.0) * M ** 3 * B
+        elif "apply" in k:
+            flops_by_kernel[k] = 6.0 * M * rot_per_matrix * B
+        elif "ql" in k:
+            flops_by_kernel[k] = 30.0 * rot_per_matrix * B
+    dom = max(kern_ms, key=kern_ms.get)
+    dom_flops = flops_by_kernel.get(dom, 0.0)
+    achieved = dom_flops / (kern_ms[dom] * 1e-3) / 1e12
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = peaks.get("hbm_gbs", 6650.0)
+
+    # measured DFMA rate (context for the derived peak)
+    nfma, _ = letkf.probe_dfma(SM_COUNT * 8, 256, 2048)
+    torch.cuda.synchronize()
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record(stream)
+    nfma, _ = letkf.probe_dfma(SM_COUNT * 8, 256, 2048)
+    p1.record(stream)
+    torch.cuda.synchronize()
+    dfma_measured = 2.0 * nfma / (p0.elapsed_time(p1) * 1e-3) / 1e12
+
+    roofline = {
+        "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+        "frac": achieved / peak_tflops, "traffic": None,
+        "peak_source": f"derived: {SM_COUNT} SMs x {DFMA_PER_CLK_SM} DFMA/clk x 2 x {sm_max:.0f} MHz (DESIGN.md 6)",
+        "dfma_probe_tflops": dfma_measured,
+        "kernel_ms": kern_ms, "kernel_share": {k: v / sum(kern_ms.values()) for k, v in kern_ms.items()},
+        "rotations_per_matrix": rot_per_matrix,
+        "flops_counted_per_matrix": (8.0 / 3.0) * M ** 3 + 6.0 * M * rot_per_matrix,
+        "step_model_9M3": {"achieved": syev_model_flops(M) * B / (ms_step * 1e-3) / 1e12,
+                           "frac": syev_model_flops(M) * B / (ms_step * 1e-3) / 1e12 / peak_tflops},
+        "step_hbm": {"achieved_gbs": syev_bytes(M) * B / (ms_step * 1e-3) / 1e9,
+                     "peak_gbs": hbm_peak, "frac": syev_bytes(M) * B / (ms_step * 1e-3) / 1e9 / hbm_peak},
+    }
+
+    # ---- end to end through the public API with HOST buffers (pinned), copies inside the timing
+    A_pin = torch.from_numpy(A_host).pin_memory()
+    w_pin = torch.empty((B, M), dtype=torch.float64).pin_memory()
+    V_pin = torch.empty((B, M, M), dtype=torch.float64).pin_memory()
+    A_in = torch.empty_like(A)
+
+    def e2e_step():
+        A_in.copy_(A_pin, non_blocking=True)
+        letkf.syev_batched(A_in, w=w, V=V, info=info, work=work, stream=stream)
+        w_pin.copy_(w, non_blocking=True)
+        V_pin.copy_(V, non_blocking=True)
+
+    e2e_step()
+    barrier()
+    ksteps = min(args.steps, 5)
+    e0.record(stream)
+    for _ in range(ksteps):
+        e2e_step()
+    e1.record(stream)
+    barrier()
+    e2e_ms = max_over_ranks(e0.elapsed_time(e1)) / ksteps
+    e2e = {"value": world * B / (e2e_ms * 1e-3), "unit": "matrices/s",
+           "h2d_bytes_per_step": int(A_pin.numel() * 8), "d2h_bytes_per_step": int((w_pin.numel() + V_pin.numel()) * 8),
+           "ms_per_step": e2e_ms, "steps": ksteps}
+    del A_pin, V_pin, A_in
+
+    line = {
+        "metric": METRIC, "value": value, "unit": "matrices/s", "n_gpus": world,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": "config3: letkf_syev_batched fp64 M=64 batch=16384 per GPU, LETKF-shaped p=98 rho=1.1",
+                   "l2": "inputs larger than L2: A+V = 1 GiB per step, no flush needed"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
+        "roofline": roofline,
+    }
+
+    if rank == 0 and world == 1:
+        # ---- fused analysis (config 4), same protocol
+        if not args.no_analysis:
+            inp = wl.analysis_inputs()
+            t = {k: torch.from_numpy(inp[k]).cuda() for k in ("Yb", "d", "rinv_loc", "Xb")}
+            Xa = torch.empty_like(t["Xb"])
+            awork = torch.empty(letkf.analysis_workspace_bytes(M, p, 9, B), dtype=torch.uint8, device="cuda")
+
+            def astep():
+                letkf.analysis_batched(t["Yb"], t["d"], t["rinv_loc"], t["Xb"], inp["rho"], Xa=Xa, info=info,
+                                       work=awork, stream=stream)
+            for _ in range(3):
+                astep()
+            torch.cuda.synchronize()
+            e0.record(stream)
+            for _ in range(args.steps):
+                astep()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ams = e0.elapsed_time(e1) / args.steps
+            fl = analysis_model_flops(M, p, 9)
+            line["analysis"] = {
+                "workload": "config4: letkf_analysis_batched fp64 M=64 p=98 nstate=9, 128x128 grid points, W not requested",
+                "value": B / (ams * 1e-3), "unit": "grid points/s", "ms_per_step": ams,
+                "gpu_launches_per_step": letkf.last_launch_count(),
+                "model_tflops": fl * B / (ams * 1e-3) / 1e12, "frac_of_fp64_peak": fl * B / (ams * 1e-3) / 1e12 / peak_tflops,
+                "hbm_gbs": analysis_bytes(M, p, 9) * B / (ams * 1e-3) / 1e9}
+            del t, Xa, awork, inp
+        # ---- cuSOLVER on the same matrices (comparison only)
+        if not args.no_cusolver:
+            try:
+                line["cusolver"] = cusolver_compare(A)
+            except Exception as ex:          # comparison must never break the bench
+                line["cusolver"] = {"unavailable": repr(ex)[:200]}
+        # ---- CPU baseline: the oracle on the host cores, bounded sample
+        if not args.no_cpu_baseline:
+            sample = 8192
+            v, nt, dt = time_oracle_syev(A_host[:sample])
+            line["cpu_baseline"] = {"value": v, "unit": "matrices/s", "cores": nt, "kind": "oracle",
+                                    "sample": f"first {sample} matrices of config 3 (cyclic Jacobi fp64, OpenMP over the batch), {dt:.1f} s"}
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-analysis", action="store_true")
+    ap.add_argument("--no-cusolver", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

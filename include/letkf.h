@@ -1,0 +1,140 @@
+/*
+ * letkf.h -- C ABI of libletkf: the per-grid-point LETKF local analysis of
+ * arXiv 2308.03310 (Hasegawa et al., "GPU Optimization of Lattice Boltzmann Method with
+ * Local Ensemble Transform Kalman Filter"), hand-written CUDA for sm_100a (NVIDIA B200).
+ *
+ * Citations are "PAPER.md:<line>" of the paper text plus the equation / section.
+ *
+ * General contract (every entry point):
+ *   - every array pointer is a DEVICE pointer owned by the caller (for instance the data_ptr
+ *     of a torch tensor).  Arrays are row-major, batch outermost ("the batch
+ *     dimension is the outermost"), fp64, 16-byte aligned.
+ *   - work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy default
+ *     stream) and the call returns without synchronising.  Internally the library may fork
+ *     onto private streams that are joined back into `stream` before the call returns, so
+ *     stream order is all a caller needs.
+ *   - workspace: `work` is a caller-owned device buffer of at least the size returned by
+ *     the matching letkf_*_workspace_bytes(); if `work` is NULL the library takes it from
+ *     the device's default memory pool with cudaMallocAsync / cudaFreeAsync on `stream`
+ *     (stream-ordered, no synchronisation).
+ *   - return value: 0 = LETKF_OK; -k = the k-th argument (1-based) is invalid (NULL where
+ *     not allowed, out of range, misaligned); >0 = a cudaError_t from the launch.
+ *     Per-matrix numerical status is asynchronous, in info[b] (see below).
+ *   - inputs are never written unless aliased with an output as documented.
+ *   - there is NO CPU fallback: without a CUDA device every compute call returns a
+ *     cudaError_t.
+ *   - results are bitwise reproducible run to run for fixed inputs (no floating-point atomics).
+ */
+#ifndef LETKF_H
+#define LETKF_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LETKF_OK 0
+#define LETKF_MAX_M 256       /* largest ensemble size / matrix order accepted            */
+#define LETKF_VERSION 100     /* major*10000 + minor*100 + patch                          */
+
+/* info[b] bit flags (0 = converged on the fast path) */
+#define LETKF_INFO_SLOWPATH 0x40000000 /* the matrix was finished by the in-kernel slow path
+                                          (rotation log full); result is still valid       */
+/* info[b] & 0xFFFF = number of off-diagonal elements that had not converged after 30
+ * QL iterations each ("implicit QL method ... as in EISPACK/LAPACK"; cap as in
+ * EISPACK tql2).  Non-zero means w/V of that matrix are not to be trusted.                */
+
+/*
+ * Batched symmetric eigenvalue decomposition -- the paper's "main computing kernel"
+ * ("computed by the eigenvalue decomposition (EVD) of Q", section III
+ * Householder tridiagonalisation -> implicit QL -> back-transform).
+ *
+ *   A[b] = V[b] diag(w[b]) V[b]^T,  V[b]^T V[b] = I,  w[b] ascending.
+ *
+ *   A     in   [batch][M][M]  symmetric; only the LOWER triangle (row >= col) is read.
+ *   M          matrix order, 1 <= M <= LETKF_MAX_M
+ *   batch      number of matrices, >= 0 (0 = successful no-op)
+ *   w     out  [batch][M]     eigenvalues, ascending
+ *   V     out  [batch][M][M]  eigenvector k is COLUMN k: A[b] @ V[b] == V[b] * w[b]
+ *                             (numpy.linalg.eigh convention).  V may alias A (in place).
+ *                             Sign of each eigenvector (and the basis inside a repeated
+ *                             eigenvalue) is not specified.
+ *   info  out  [batch] ints or NULL
+ *   work       device workspace or NULL, work_bytes >= letkf_syev_workspace_bytes(M, batch)
+ *   stream     cudaStream_t
+ *
+ * Precondition: entries finite with 1e-100 < max|A| < 1e100 (no rescaling is applied);
+ * non-finite input terminates (iteration cap) with info[b] != 0.
+ */
+int letkf_syev_batched(const double* A, int M, int batch, double* w, double* V,
+                       int* info, void* work, size_t work_bytes, void* stream);
+
+size_t letkf_syev_workspace_bytes(int M, int batch);
+
+/*
+ * Fused LETKF local analysis of `batch` grid points (Eq.13-19;
+ * Procedure 1 lines 5-7).  For each point, with dY = Yb (p x M),
+ * r = rinv_loc (the diagonal of G o R^-1), dvec = d = y^o - ybar^f:
+ *
+ *   Q     = ((M-1)/rho) I + dY^T diag(r) dY                        Eq.17 (rho = 1 is the paper's)
+ *   Q     = V diag(lam) V^T
+ *   wbar  = V diag(1/lam) V^T dY^T diag(r) dvec                    Eq.14, Eq.16
+ *   W     = sqrt(M-1) V diag(lam^-1/2) V^T                         Eq.15, symmetric square root
+ *   xbar  = mean_m Xb[:, m],  dX = Xb - xbar                       Eq.9-11
+ *   Xa    = xbar 1^T + dX (wbar 1^T + W)                           Eq.13
+ *
+ *   Yb        in  [batch][p][M]       observation-space perturbations (rows centred by the caller)
+ *   d         in  [batch][p]          innovations
+ *   rinv_loc  in  [batch][p]          >= 0; 0 marks a padded / ignored observation
+ *   Xb        in  [batch][nstate][M]  background ensemble (members, not perturbations)
+ *   M, p, nstate, batch               1 <= M <= LETKF_MAX_M, p >= 0, nstate >= 1, batch >= 0
+ *   rho                               multiplicative covariance inflation, > 0
+ *   Xa        out [batch][nstate][M]  analysis ensemble; may alias Xb
+ *   W         out [batch][M][M] or NULL
+ *   wbar      out [batch][M]    or NULL
+ *   info      out [batch] or NULL     as for letkf_syev_batched
+ *   work / work_bytes / stream        as above, size from letkf_analysis_workspace_bytes()
+ */
+int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv_loc,
+                           const double* Xb, int M, int p, int nstate, int batch, double rho,
+                           double* Xa, double* W, double* wbar, int* info,
+                           void* work, size_t work_bytes, void* stream);
+
+size_t letkf_analysis_workspace_bytes(int M, int p, int nstate, int batch);
+
+/*
+ * Measurement helper (not part of the method): runs `iters` dependent-chain-free fp64 FMA
+ * rounds on every SM and writes one double per thread to `sink` (device, >= blocks*threads
+ * doubles) so the work cannot be elided.  Returns the number of fp64 FMAs executed in
+ * *fma_count (host pointer, may be NULL).  bench.py times it with CUDA events to obtain the
+ * measured DFMA peak that the roofline fraction is quoted against.
+ */
+int letkf_probe_dfma(double* sink, int blocks, int threads, int iters,
+                     unsigned long long* fma_count, void* stream);
+
+/*
+ * Profiling aid for bench.py (off by default; adds one CUDA event pair per kernel launch).
+ * With profiling on, each compute call records events around every kernel it enqueues, on the
+ * stream the kernel runs on, and counts the plane rotations its QL step generated.
+ *   letkf_profile_enable(on)         switch; returns the previous setting
+ *   letkf_profile_count()            records held from the last compute call of this thread
+ *   letkf_profile_record(i, &name, &ms)  SYNCHRONISES on record i's events; name is a static string
+ *   letkf_profile_rotations()        SYNCHRONISES; total rotations generated by the last call
+ */
+int letkf_profile_enable(int on);
+int letkf_profile_count(void);
+int letkf_profile_record(int idx, const char** name, float* ms);
+long long letkf_profile_rotations(void);
+
+/* Number of kernels the last compute call on this host thread enqueued (bench.py's
+ * gpu_launches claim is counted from this, not guessed). */
+int letkf_last_launch_count(void);
+
+const char* letkf_status_string(int status);
+int letkf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LETKF_H */

@@ -1,0 +1,151 @@
+// common.cuh -- shared device helpers of libletkf (CUDA path only; the CPU oracle shares nothing
+// with this tree).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace letkf {
+
+// Per-matrix workspace layout (device).  One record per matrix of the current chunk.
+//   dws, ews  : the tridiagonal form T = Q^T A Q (kept untouched after the reduction so the
+//               slow path can restart from it)
+//   perm      : perm[k] = index (in QL order) of the k-th smallest eigenvalue
+//   hdr       : one word per QL sweep, lo | (m << 16): rotations i = m-1 ... lo
+//   rot       : (c, s) of every rotation, in application order
+struct Workspace {
+    double*   dws;      // [chunk][M]
+    double*   ews;      // [chunk][M]
+    int*      perm;     // [chunk][M]
+    int*      nsweeps;  // [chunk]
+    int*      flags;    // [chunk]   1 = rotation log overflowed, finish on the slow path
+    uint32_t* hdr;      // [chunk][swcap]
+    double2*  rot;      // [chunk][logcap]
+    int       swcap;
+    int       logcap;
+    unsigned long long* rot_counter;   // profiling only (NULL otherwise): total rotations logged
+};
+
+__host__ __device__ inline int sweep_capacity(int M) { return 6 * M + 32; }
+__host__ __device__ inline int log_capacity(int M)   { return 2 * M * M + 4 * M + 16; }
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Deterministic block-wide sum; red must hold NT/32 doubles.  All threads get the result.
+template <int NT>
+__device__ __forceinline__ double block_sum(double v, double* red)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    v = warp_sum(v);
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    double t = 0.0;
+#pragma unroll
+    for (int w = 0; w < NT / 32; ++w) t += red[w];
+    __syncthreads();
+    return t;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Implicit-shift QL on a symmetric tridiagonal matrix ("The eigenvalues and
+// eigenvectors of the tridiagonal matrix are computed by the implicit QL method as in
+// EISPACK/LAPACK").  Only the scalar recurrences are run here; every plane rotation (c, s) is
+// written to `sink` and applied to the eigenvector matrix elsewhere, so the serial chain
+// (sqrt/div latency) never stalls the threads that own the matrix.
+//
+// d[i*stride], e[i*stride]: diagonal / off-diagonal (e[i] couples i and i+1; e[M-1] unused).
+// One call produces the next non-empty sweep: rotations for i = m-1 ... lo, stored at
+// sink[0 .. m-lo-1], to be applied as
+//      f = z[i+1];  z[i+1] = s*z[i] + c*f;  z[i] = c*z[i] - s*f      (columns of Z).
+// Returns 1 with (lo, m) set, 0 when all eigenvalues have converged, -1 if the sweep would not
+// fit into sink_cap (nothing is changed in that case).
+// Conventions fixed in DESIGN.md reading G10: Wilkinson shift, deflation when
+// |e_m| <= 2^-53 (|d_m| + |d_m+1|), at most 30 sweeps per eigenvalue (then st.fail is bumped).
+struct QLState { int l; int iter; int fail; };
+
+__device__ __forceinline__ int ql_next_sweep(QLState& st, double* d, double* e, int stride, int M,
+                                             double2* sink, int sink_cap, int& lo_out, int& m_out)
+{
+#define LD(i) d[(size_t)(i) * stride]
+#define LE(i) e[(size_t)(i) * stride]
+    const double eps = 1.1102230246251565e-16;   // 2^-53
+    while (st.l < M) {
+        const int l = st.l;
+        int m = l;
+        for (; m < M - 1; ++m) {
+            const double dd = fabs(LD(m)) + fabs(LD(m + 1));
+            if (fabs(LE(m)) <= eps * dd) break;
+        }
+        if (m == l) { st.l = l + 1; st.iter = 0; continue; }
+        if (st.iter >= 30) { st.fail += 1; st.l = l + 1; st.iter = 0; continue; }
+        if (m - l > sink_cap) return -1;
+        st.iter += 1;
+
+        const double el = LE(l);
+        double g = (LD(l + 1) - LD(l)) / (2.0 * el);
+        double r = sqrt(g * g + 1.0);
+        g = LD(m) - LD(l) + el / (g + copysign(r, g));
+        double s = 1.0, c = 1.0, p = 0.0;
+        int i;
+        for (i = m - 1; i >= l; --i) {
+            const double ei = LE(i);
+            const double f = s * ei;
+            const double b = c * ei;
+            const double r2 = f * f + g * g;
+            if (!(r2 > 0.0)) {            // underflow (or NaN): split here
+                LE(i + 1) = 0.0;
+                LD(i + 1) -= p;
+                LE(m) = 0.0;
+                break;
+            }
+            const double rinv = rsqrt(r2);
+            r = r2 * rinv;
+            LE(i + 1) = r;
+            s = f * rinv;
+            c = g * rinv;
+            g = LD(i + 1) - p;
+            r = (LD(i) - g) * s + 2.0 * c * b;
+            p = s * r;
+            LD(i + 1) = g + p;
+            g = c * r - b;
+            sink[m - 1 - i] = make_double2(c, s);
+        }
+        int lo;
+        if (i >= l) {
+            lo = i + 1;
+        } else {
+            LD(l) -= p;
+            LE(l) = g;
+            LE(m) = 0.0;
+            lo = l;
+        }
+        if (m - lo > 0) { lo_out = lo; m_out = m; return 1; }
+    }
+    return 0;
+#undef LD
+#undef LE
+}
+
+// Ascending insertion sort of d with the permutation that sorts it (stable).
+__device__ __forceinline__ void sort_eigenvalues(double* d, int* perm, int stride, int M)
+{
+    for (int k = 0; k < M; ++k) perm[(size_t)k * stride] = k;
+    for (int k = 1; k < M; ++k) {
+        const double val = d[(size_t)k * stride];
+        const int pk = perm[(size_t)k * stride];
+        int j = k - 1;
+        while (j >= 0 && d[(size_t)j * stride] > val) {
+            d[(size_t)(j + 1) * stride] = d[(size_t)j * stride];
+            perm[(size_t)(j + 1) * stride] = perm[(size_t)j * stride];
+            --j;
+        }
+        d[(size_t)(j + 1) * stride] = val;
+        perm[(size_t)(j + 1) * stride] = pk;
+    }
+}
+
+}  // namespace letkf

@@ -1,0 +1,433 @@
+// generic_kernels.cuh -- the any-M (1 <= M <= 256) path of libletkf: one CTA per matrix, the
+// matrix held in the caller's V buffer (global memory / L2).  It is the path for M > 64, the
+// finisher for matrices whose rotation log overflowed on the fast path, and the reference point
+// the register-resident kernels of fast_kernels.cuh are measured against.
+//
+// Steps:
+//   a3  Householder tridiagonalisation  T = Q^T A Q               generic_tridiag_formq
+//   a5' explicit Q (stored transposed, "Qt" layout: Qt[c][r] = Q[r][c])   "
+//   a4  implicit QL, rotations logged                             ql_log_kernel (ql_kernel.cuh)
+//   a5  V = Q Z by replaying the rotations on the rows of Q       generic_apply
+#pragma once
+#include "common.cuh"
+
+namespace letkf {
+
+constexpr int GEN_NT = 256;
+
+// ---------------------------------------------------------------------------------------------
+// a3 + explicit Q.  Reduction order is "from the last row up" (pivot i = M-1 ... 1, reflector
+// H_i acts on indices 0..i-1), so Q = H_{M-1} ... H_1 and T = Q^T A Q.
+// A: [batch][M][M] (lower triangle read).  V: [batch][M][M] receives Q^T.  May alias.
+__global__ void __launch_bounds__(GEN_NT)
+generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, int M)
+{
+    extern __shared__ double sm[];
+    double* v    = sm;            // [M]
+    double* wv   = sm + M;        // [M]
+    double* pv   = sm + 2 * M;    // [M]
+    double* taus = sm + 3 * M;    // [M]
+    double* red  = sm + 4 * M;    // [GEN_NT/32]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = GEN_NT / 32;
+    const size_t b = blockIdx.x;
+    const double* A = A_ + b * M * M;
+    double* S = V_ + b * M * M;
+    double* dws = ws.dws + b * M;
+    double* ews = ws.ews + b * M;
+
+    // full symmetric copy of the lower triangle
+    for (int r = warp; r < M; r += NW)
+        for (int c = lane; c < M; c += 32) {
+            const double val = (r >= c) ? A[(size_t)r * M + c] : A[(size_t)c * M + r];
+            S[(size_t)r * M + c] = val;
+        }
+    __syncthreads();
+
+    for (int i = M - 1; i >= 1; --i) {
+        double* rowi = S + (size_t)i * M;
+        double part = 0.0;
+        for (int c = tid; c < i - 1; c += GEN_NT) { const double x = rowi[c]; part += x * x; }
+        const double sigma = block_sum<GEN_NT>(part, red);
+        const double alpha = rowi[i - 1];
+        double beta, tau, scal;
+        if (sigma == 0.0) { tau = 0.0; beta = alpha; scal = 0.0; }       // reading G19: H = I
+        else {
+            beta = -copysign(sqrt(alpha * alpha + sigma), alpha);
+            tau = (beta - alpha) / beta;
+            scal = 1.0 / (alpha - beta);
+        }
+        for (int c = tid; c < i; c += GEN_NT) v[c] = (c == i - 1) ? 1.0 : rowi[c] * scal;
+        if (tid == 0) { ews[i - 1] = beta; dws[i] = rowi[i]; taus[i] = tau; }
+        __syncthreads();
+        for (int c = tid; c < i; c += GEN_NT) rowi[c] = v[c];            // keep the reflector
+        if (tau != 0.0) {
+            for (int j = warp; j < i; j += NW) {                          // p = tau * S11 v
+                const double* rj = S + (size_t)j * M;
+                double acc = 0.0;
+                for (int c = lane; c < i; c += 32) acc += rj[c] * v[c];
+                acc = warp_sum(acc);
+                if (lane == 0) pv[j] = tau * acc;
+            }
+            __syncthreads();
+            part = 0.0;
+            for (int c = tid; c < i; c += GEN_NT) part += pv[c] * v[c];
+            const double K = 0.5 * tau * block_sum<GEN_NT>(part, red);
+            for (int c = tid; c < i; c += GEN_NT) wv[c] = pv[c] - K * v[c];
+            __syncthreads();
+            for (int j = warp; j < i; j += NW) {                          // S11 -= v w^T + w v^T
+                double* rj = S + (size_t)j * M;
+                const double vj = v[j], wj = wv[j];
+                for (int c = lane; c < i; c += 32) rj[c] -= vj * wv[c] + wj * v[c];
+            }
+        }
+        __syncthreads();
+    }
+    if (tid == 0) { dws[0] = S[0]; ews[M - 1] = 0.0; }
+
+    // Q^T = H_1 H_2 ... H_{M-1}, grown in place: B_i = diag(B_{i-1}, 1) H_i on the leading i x i
+    for (int i = 1; i <= M - 1; ++i) {
+        for (int c = tid; c < i; c += GEN_NT) v[c] = S[(size_t)i * M + c];
+        const double tau = taus[i];
+        for (int c = tid; c < i - 1; c += GEN_NT) {
+            S[(size_t)(i - 1) * M + c] = 0.0;
+            S[(size_t)c * M + (i - 1)] = 0.0;
+        }
+        if (tid == 0) S[(size_t)(i - 1) * M + (i - 1)] = 1.0;
+        __syncthreads();
+        if (tau != 0.0) {
+            for (int r = warp; r < i; r += NW) {
+                double* br = S + (size_t)r * M;
+                double acc = 0.0;
+                for (int c = lane; c < i; c += 32) acc += br[c] * v[c];
+                acc = warp_sum(acc) * tau;
+                for (int c = lane; c < i; c += 32) br[c] -= acc * v[c];
+            }
+        }
+        __syncthreads();
+    }
+    for (int c = tid; c < M - 1; c += GEN_NT) {
+        S[(size_t)(M - 1) * M + c] = 0.0;
+        S[(size_t)c * M + (M - 1)] = 0.0;
+    }
+    if (tid == 0) S[(size_t)(M - 1) * M + (M - 1)] = 1.0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5: replay the logged rotations on B = Q^T (thread r owns row r of Q = column r of B, so all
+// accesses are coalesced and no synchronisation is needed), then sort the eigenvectors and
+// transpose in place to the row-major V the interface promises.
+// Matrices flagged by ql_log_kernel (log overflow) -- or all of them when `force_slow` -- run
+// the classic in-kernel QL instead: thread 0 generates one sweep into shared memory, all threads
+// apply it.  only_flagged: process nothing but flagged matrices (finisher after the fast path;
+// there V already holds Q row-major, `q_rowmajor`).
+__global__ void __launch_bounds__(GEN_NT)
+generic_apply(double* V_, double* __restrict__ w_, Workspace ws, int M, int* __restrict__ info,
+              int only_flagged, int q_rowmajor)
+{
+    extern __shared__ double sm[];
+    double*  dsm    = sm;                                         // [M]
+    double*  esm    = sm + M;                                     // [M]
+    double2* cs     = reinterpret_cast<double2*>(sm + 2 * M);     // [M]
+    int*     permsm = reinterpret_cast<int*>(sm + 4 * M);         // [M]
+    int*     leader = permsm + M;                                 // [M]
+    double*  tile   = sm + 5 * M;                                 // 2 x [32][33]
+    __shared__ int sh_rc, sh_lo, sh_m, sh_fail;
+
+    const int tid = threadIdx.x;
+    const size_t b = blockIdx.x;
+    const int flagged = ws.flags[b];
+    if (only_flagged && !flagged) return;
+    double* B = V_ + b * M * M;
+
+    if (q_rowmajor) {      // bring row-major Q into the Qt layout first (in-place transpose)
+        for (int idx = tid; idx < M * M; idx += GEN_NT) {
+            const int r = idx / M, c = idx - r * M;
+            if (r < c) {
+                const double x = B[(size_t)r * M + c], y = B[(size_t)c * M + r];
+                B[(size_t)r * M + c] = y;
+                B[(size_t)c * M + r] = x;
+            }
+        }
+        __syncthreads();
+    }
+
+    if (!flagged) {
+        const int nsw = ws.nsweeps[b];
+        const uint32_t* hdr = ws.hdr + b * ws.swcap;
+        const double2* rot = ws.rot + b * ws.logcap;
+        for (int r = tid; r < M; r += GEN_NT) {
+            int pos = 0;
+            for (int sidx = 0; sidx < nsw; ++sidx) {
+                const uint32_t h = hdr[sidx];
+                const int lo = h & 0xffff, m = h >> 16;
+                double f = B[(size_t)m * M + r];
+                for (int i = m - 1; i >= lo; --i) {
+                    const double2 q = rot[pos++];
+                    const double zi = B[(size_t)i * M + r];
+                    B[(size_t)(i + 1) * M + r] = q.y * zi + q.x * f;
+                    f = q.x * zi - q.y * f;
+                }
+                B[(size_t)lo * M + r] = f;
+            }
+        }
+        for (int k = tid; k < M; k += GEN_NT) permsm[k] = ws.perm[b * M + k];
+    } else {
+        for (int k = tid; k < M; k += GEN_NT) { dsm[k] = ws.dws[b * M + k]; esm[k] = ws.ews[b * M + k]; }
+        __syncthreads();
+        QLState st{0, 0, 0};
+        if (tid == 0) esm[M - 1] = 0.0;
+        for (;;) {
+            if (tid == 0) {
+                int lo = 0, m = 0;
+                sh_rc = ql_next_sweep(st, dsm, esm, 1, M, cs, M, lo, m);
+                sh_lo = lo; sh_m = m;
+            }
+            __syncthreads();
+            if (sh_rc != 1) break;
+            const int lo = sh_lo, m = sh_m;
+            for (int r = tid; r < M; r += GEN_NT) {
+                double f = B[(size_t)m * M + r];
+                for (int i = m - 1; i >= lo; --i) {
+                    const double2 q = cs[m - 1 - i];
+                    const double zi = B[(size_t)i * M + r];
+                    B[(size_t)(i + 1) * M + r] = q.y * zi + q.x * f;
+                    f = q.x * zi - q.y * f;
+                }
+                B[(size_t)lo * M + r] = f;
+            }
+            __syncthreads();
+        }
+        if (tid == 0) {
+            sort_eigenvalues(dsm, permsm, 1, M);
+            sh_fail = st.fail;
+        }
+        __syncthreads();
+        for (int k = tid; k < M; k += GEN_NT) w_[b * M + k] = dsm[k];
+        if (info && tid == 0) info[b] = sh_fail | 0x40000000;
+    }
+    __syncthreads();
+
+    // sort: new row k of B = old row perm[k]; cycles are followed by every thread for its column
+    for (int k = tid; k < M; k += GEN_NT) {
+        int j = permsm[k];
+        while (j > k) j = permsm[j];
+        leader[k] = (j == k) && (permsm[k] != k);
+    }
+    __syncthreads();
+    for (int r = tid; r < M; r += GEN_NT) {
+        for (int k = 0; k < M; ++k) {
+            if (!leader[k]) continue;
+            const double first = B[(size_t)k * M + r];
+            int j = k;
+            for (;;) {
+                const int src = permsm[j];
+                if (src == k) { B[(size_t)j * M + r] = first; break; }
+                B[(size_t)j * M + r] = B[(size_t)src * M + r];
+                j = src;
+            }
+        }
+    }
+    __syncthreads();
+
+    // in-place transpose Qt layout -> row-major V, 32x32 tiles through shared memory
+    const int nt = (M + 31) / 32;
+    double* t0 = tile;
+    double* t1 = tile + 32 * 33;
+    const int tx = tid & 31, ty = tid >> 5;       // 32 x 8
+    for (int ti = 0; ti < nt; ++ti)
+        for (int tj = ti; tj < nt; ++tj) {
+            for (int yy = ty; yy < 32; yy += GEN_NT / 32) {
+                const int r0 = ti * 32 + yy, c0 = tj * 32 + tx;
+                if (r0 < M && c0 < M) t0[yy * 33 + tx] = B[(size_t)r0 * M + c0];
+                const int r1 = tj * 32 + yy, c1 = ti * 32 + tx;
+                if (r1 < M && c1 < M) t1[yy * 33 + tx] = B[(size_t)r1 * M + c1];
+            }
+            __syncthreads();
+            for (int yy = ty; yy < 32; yy += GEN_NT / 32) {
+                const int r1 = tj * 32 + yy, c1 = ti * 32 + tx;       // B[tj-tile] <- t0^T
+                if (r1 < M && c1 < M) B[(size_t)r1 * M + c1] = t0[tx * 33 + yy];
+                if (ti != tj) {
+                    const int r0 = ti * 32 + yy, c0 = tj * 32 + tx;   // B[ti-tile] <- t1^T
+                    if (r0 < M && c0 < M) B[(size_t)r0 * M + c0] = t1[tx * 33 + yy];
+                }
+            }
+            __syncthreads();
+        }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a1 + a2 (Eq.17 and the right factor of Eq.14), any M, p.
+//   Aout[b][m][n] = ((M-1)/rho) delta_mn + sum_j r_j Yb[j][m] Yb[j][n]
+//   gout[b][m]    = sum_j Yb[j][m] r_j d_j
+// 16 x 16 threads, 4 x 4 outputs each per 64 x 64 output tile.
+__global__ void __launch_bounds__(256)
+generic_gram(const double* __restrict__ Yb_, const double* __restrict__ d_,
+             const double* __restrict__ r_, int M, int p, double shift,
+             double* __restrict__ Aout_, double* __restrict__ gout_)
+{
+    const size_t b = blockIdx.x;
+    const double* Yb = Yb_ + b * (size_t)p * M;
+    const double* dv = d_ + b * (size_t)p;
+    const double* rv = r_ + b * (size_t)p;
+    double* Aout = Aout_ + b * (size_t)M * M;
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+
+    for (int m = tid; m < M; m += 256) {
+        double acc = 0.0;
+        for (int j = 0; j < p; ++j) acc += Yb[(size_t)j * M + m] * rv[j] * dv[j];
+        gout_[b * M + m] = acc;
+    }
+    for (int m0 = 0; m0 < M; m0 += 64)
+        for (int n0 = 0; n0 < M; n0 += 64) {
+            double acc[4][4];
+#pragma unroll
+            for (int a = 0; a < 4; ++a)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) acc[a][c] = 0.0;
+            for (int j = 0; j < p; ++j) {
+                const double rj = rv[j];
+                double ym[4], yn[4];
+#pragma unroll
+                for (int a = 0; a < 4; ++a) {
+                    const int m = m0 + ty + 16 * a, n = n0 + tx + 16 * a;
+                    ym[a] = (m < M) ? rj * Yb[(size_t)j * M + m] : 0.0;
+                    yn[a] = (n < M) ? Yb[(size_t)j * M + n] : 0.0;
+                }
+#pragma unroll
+                for (int a = 0; a < 4; ++a)
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) acc[a][c] += ym[a] * yn[c];
+            }
+#pragma unroll
+            for (int a = 0; a < 4; ++a)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const int m = m0 + ty + 16 * a, n = n0 + tx + 16 * c;
+                    if (m < M && n < M)
+                        Aout[(size_t)m * M + n] = acc[a][c] + ((m == n) ? shift : 0.0);
+                }
+        }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a6 - a9 (Eq.13-16, Eq.9-11), any M.  V row-major, lam ascending, g from generic_gram.
+//   t     = diag(1/lam) V^T g,  wbar = V t                                   Eq.14 / Eq.16
+//   W     = sqrt(M-1) V diag(lam^-1/2) V^T                                   Eq.15   (if wanted)
+//   Xa    = xbar 1^T + (dX wbar) 1^T + sqrt(M-1) ((dX V) diag(lam^-1/2)) V^T  Eq.13, without
+//           forming W: dX W = ((dX V) Lam^-1/2) V^T  (same product, associativity only)
+// Dynamic shared memory: t[M], wb[M], xbar[ns], cs[ns], T1[ns][M], dX[ns][M]
+__global__ void __launch_bounds__(256)
+generic_epilogue(const double* __restrict__ V_, const double* __restrict__ lam_,
+                 const double* __restrict__ g_, const double* Xb_, int M, int ns,
+                 double* Xa_, double* __restrict__ W_, double* __restrict__ wbar_)
+{
+    extern __shared__ double sm[];
+    double* t    = sm;
+    double* wb   = sm + M;
+    double* xbar = sm + 2 * M;
+    double* cs   = xbar + ns;
+    double* T1   = cs + ns;
+    double* dX   = T1 + (size_t)ns * M;
+    const size_t b = blockIdx.x;
+    const double* V = V_ + b * (size_t)M * M;
+    const double* lam = lam_ + b * M;
+    const double* g = g_ + b * M;
+    const double* Xb = Xb_ + b * (size_t)ns * M;
+    double* Xa = Xa_ + b * (size_t)ns * M;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const double sq = sqrt((double)(M - 1));
+
+    for (int k = tid; k < M; k += 256) {
+        double acc = 0.0;
+        for (int n = 0; n < M; ++n) acc += V[(size_t)n * M + k] * g[n];
+        t[k] = acc / lam[k];
+    }
+    for (int s = warp; s < ns; s += 8) {                      // Eq.9-11
+        double acc = 0.0;
+        for (int m = lane; m < M; m += 32) acc += Xb[(size_t)s * M + m];
+        acc = warp_sum(acc) / (double)M;
+        if (lane == 0) xbar[s] = acc;
+        for (int m = lane; m < M; m += 32) dX[(size_t)s * M + m] = Xb[(size_t)s * M + m] - acc;
+    }
+    __syncthreads();
+    for (int m = warp; m < M; m += 8) {                       // wbar = V t
+        double acc = 0.0;
+        for (int k = lane; k < M; k += 32) acc += V[(size_t)m * M + k] * t[k];
+        acc = warp_sum(acc);
+        if (lane == 0) { wb[m] = acc; if (wbar_) wbar_[b * M + m] = acc; }
+    }
+    for (int idx = tid; idx < ns * M; idx += 256) {            // T1 = sqrt(M-1) (dX V) Lam^-1/2
+        const int s = idx / M, k = idx - s * M;
+        double acc = 0.0;
+        for (int m = 0; m < M; ++m) acc += dX[(size_t)s * M + m] * V[(size_t)m * M + k];
+        T1[idx] = acc * sq / sqrt(lam[k]);
+    }
+    __syncthreads();
+    for (int s = warp; s < ns; s += 8) {                      // c_s = dX[s] . wbar
+        double acc = 0.0;
+        for (int m = lane; m < M; m += 32) acc += dX[(size_t)s * M + m] * wb[m];
+        acc = warp_sum(acc);
+        if (lane == 0) cs[s] = acc;
+    }
+    __syncthreads();
+    for (int m = warp; m < M; m += 8) {                       // Xa[s][m]
+        for (int s = 0; s < ns; ++s) {
+            double acc = 0.0;
+            for (int k = lane; k < M; k += 32) acc += T1[(size_t)s * M + k] * V[(size_t)m * M + k];
+            acc = warp_sum(acc);
+            if (lane == 0) Xa[(size_t)s * M + m] = xbar[s] + cs[s] + acc;
+        }
+    }
+    if (W_) {                                                  // Eq.15, 16x16 threads x (4x4)
+        double* W = W_ + b * (size_t)M * M;
+        const int tx = tid & 15, ty = tid >> 4;
+        for (int m0 = 0; m0 < M; m0 += 64)
+            for (int n0 = 0; n0 < M; n0 += 64) {
+                double acc[4][4];
+#pragma unroll
+                for (int a = 0; a < 4; ++a)
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) acc[a][c] = 0.0;
+                for (int k = 0; k < M; ++k) {
+                    const double sc = sq / sqrt(lam[k]);
+                    double vm[4], vn[4];
+#pragma unroll
+                    for (int a = 0; a < 4; ++a) {
+                        const int m = m0 + ty + 16 * a, n = n0 + tx + 16 * a;
+                        vm[a] = (m < M) ? sc * V[(size_t)m * M + k] : 0.0;
+                        vn[a] = (n < M) ? V[(size_t)n * M + k] : 0.0;
+                    }
+#pragma unroll
+                    for (int a = 0; a < 4; ++a)
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) acc[a][c] += vm[a] * vn[c];
+                }
+#pragma unroll
+                for (int a = 0; a < 4; ++a)
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        const int m = m0 + ty + 16 * a, n = n0 + tx + 16 * c;
+                        if (m < M && n < M) W[(size_t)m * M + n] = acc[a][c];
+                    }
+            }
+    }
+}
+
+// fp64 FMA throughput probe (measurement helper, see letkf.h)
+__global__ void probe_dfma_kernel(double* sink, int iters)
+{
+    double a0 = threadIdx.x * 1e-9, a1 = a0 + 1.0, a2 = a0 + 2.0, a3 = a0 + 3.0;
+    double a4 = a0 + 4.0, a5 = a0 + 5.0, a6 = a0 + 6.0, a7 = a0 + 7.0;
+    const double x = 1.0000001, y = 1e-9;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            a0 = fma(a0, x, y); a1 = fma(a1, x, y); a2 = fma(a2, x, y); a3 = fma(a3, x, y);
+            a4 = fma(a4, x, y); a5 = fma(a5, x, y); a6 = fma(a6, x, y); a7 = fma(a7, x, y);
+        }
+    }
+    sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+}
+
+}  // namespace letkf

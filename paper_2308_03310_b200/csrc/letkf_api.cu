@@ -1,0 +1,360 @@
+// letkf_api.cu -- the C ABI of libletkf (include/letkf.h): argument checking, workspace carving,
+// dispatch on M, kernel launches.  No torch types; plain device pointers and sizes.
+#include "../../include/letkf.h"
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <vector>
+
+#include "common.cuh"
+#include "ql_kernel.cuh"
+#include "generic_kernels.cuh"
+#include "fast_kernels.cuh"
+
+namespace letkf {
+
+static thread_local int g_launches = 0;
+
+// ---- profiling aid (letkf_profile_*) --------------------------------------------------------
+struct ProfRec { const char* name; cudaEvent_t e0, e1; };
+struct Prof {
+    bool on = false;
+    std::vector<ProfRec> recs;
+    std::vector<cudaEvent_t> pool;
+    size_t used = 0;
+    unsigned long long* d_rot = nullptr;
+    cudaEvent_t get()
+    {
+        if (used == pool.size()) { cudaEvent_t e; cudaEventCreate(&e); pool.push_back(e); }
+        return pool[used++];
+    }
+};
+static thread_local Prof g_prof;
+
+static void prof_reset(cudaStream_t st)
+{
+    g_prof.recs.clear();
+    g_prof.used = 0;
+    if (g_prof.on) {
+        if (!g_prof.d_rot) cudaMalloc(&g_prof.d_rot, sizeof(unsigned long long));
+        cudaMemsetAsync(g_prof.d_rot, 0, sizeof(unsigned long long), st);
+    }
+}
+static void prof_begin(const char* name, cudaStream_t st)
+{
+    if (!g_prof.on) return;
+    ProfRec r{name, g_prof.get(), g_prof.get()};
+    cudaEventRecord(r.e0, st);
+    g_prof.recs.push_back(r);
+}
+static void prof_end(cudaStream_t st)
+{
+    if (!g_prof.on) return;
+    cudaEventRecord(g_prof.recs.back().e1, st);
+}
+
+#define KLAUNCH(name, st, ...)                                 \
+    do {                                                       \
+        prof_begin(name, st);                                  \
+        __VA_ARGS__;                                           \
+        prof_end(st);                                          \
+        cudaError_t e_ = cudaGetLastError();                   \
+        if (e_ != cudaSuccess) return (int)e_;                 \
+        ++g_launches;                                          \
+    } while (0)
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// bytes of workspace one matrix needs on the syev path
+static size_t syev_bytes_per_matrix(int M)
+{
+    size_t s = 0;
+    s += 2 * sizeof(double) * (size_t)M;                 // dws, ews
+    s += sizeof(int) * (size_t)M;                        // perm
+    s += 2 * sizeof(int);                                // nsweeps, flags
+    s += sizeof(uint32_t) * (size_t)sweep_capacity(M);   // hdr
+    s += sizeof(double2) * (size_t)log_capacity(M);      // rot
+    return s;
+}
+
+// matrices processed per pass: bounds the workspace to about 1 GiB
+static int syev_chunk(int M, int batch)
+{
+    const size_t per = syev_bytes_per_matrix(M);
+    size_t c = ((size_t)1 << 30) / per;
+    if (c < 1024) c = 1024;
+    if (c > (size_t)batch) c = (size_t)batch;
+    if (c < 1) c = 1;
+    return (int)c;
+}
+
+static size_t carve(Workspace& ws, void* base, int M, int chunk)
+{
+    char* p = reinterpret_cast<char*>(base);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { char* q = p ? p + off : nullptr; off = align_up(off + bytes, 256); return q; };
+    ws.swcap = sweep_capacity(M);
+    ws.logcap = log_capacity(M);
+    ws.rot_counter = g_prof.on ? g_prof.d_rot : nullptr;
+    ws.dws     = reinterpret_cast<double*>(take(sizeof(double) * (size_t)M * chunk));
+    ws.ews     = reinterpret_cast<double*>(take(sizeof(double) * (size_t)M * chunk));
+    ws.perm    = reinterpret_cast<int*>(take(sizeof(int) * (size_t)M * chunk));
+    ws.nsweeps = reinterpret_cast<int*>(take(sizeof(int) * (size_t)chunk));
+    ws.flags   = reinterpret_cast<int*>(take(sizeof(int) * (size_t)chunk));
+    ws.hdr     = reinterpret_cast<uint32_t*>(take(sizeof(uint32_t) * (size_t)ws.swcap * chunk));
+    ws.rot     = reinterpret_cast<double2*>(take(sizeof(double2) * (size_t)ws.logcap * chunk));
+    return off;
+}
+
+static inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+#define LAUNCH_CHECK()                                         \
+    do {                                                       \
+        cudaError_t e_ = cudaGetLastError();                   \
+        if (e_ != cudaSuccess) return (int)e_;                 \
+        ++g_launches;                                          \
+    } while (0)
+
+template <typename K>
+static cudaError_t allow_smem(K kernel, size_t bytes)
+{
+    if (bytes <= 48 * 1024) return cudaSuccess;
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+// One chunk of the EVD: A (n matrices) -> w, V.  ws is sized for >= n matrices.
+static int syev_chunk_run(const double* A, int M, int n, double* w, double* V, int* info,
+                          Workspace ws, cudaStream_t st)
+{
+    cudaError_t ce;
+    const size_t ql_smem = sizeof(double) * 2 * (size_t)M * QL_TPB;
+    if ((ce = allow_smem(ql_log_kernel, ql_smem)) != cudaSuccess) return (int)ce;
+    const size_t ap_smem = sizeof(double) * (5 * (size_t)M + 2 * 32 * 33);
+    const int qblocks = (n + QL_TPB - 1) / QL_TPB;
+
+    if (fast_supported(M)) {
+        int rc = fast_tridiag_launch(A, V, ws, M, n, st);
+        if (rc) return rc;
+        ++g_launches;
+        ql_log_kernel<<<qblocks, QL_TPB, ql_smem, st>>>(ws, M, n, w, info);
+        LAUNCH_CHECK();
+        rc = fast_apply_launch(V, ws, M, n, st);
+        if (rc) return rc;
+        ++g_launches;
+        // finisher for matrices whose rotation log overflowed (normally none: exits at once)
+        generic_apply<<<n, GEN_NT, ap_smem, st>>>(V, w, ws, M, info, /*only_flagged=*/1, /*q_rowmajor=*/1);
+        LAUNCH_CHECK();
+        return 0;
+    }
+    const size_t td_smem = sizeof(double) * (4 * (size_t)M + GEN_NT / 32);
+    KLAUNCH("generic_tridiag_formq", st, generic_tridiag_formq<<<n, GEN_NT, td_smem, st>>>(A, V, ws, M));
+    KLAUNCH("ql_log_kernel", st, ql_log_kernel<<<qblocks, QL_TPB, ql_smem, st>>>(ws, M, n, w, info));
+    KLAUNCH("generic_apply", st, generic_apply<<<n, GEN_NT, ap_smem, st>>>(V, w, ws, M, info, 0, 0));
+    return 0;
+}
+
+struct ScopedWork {
+    void* ptr = nullptr;
+    bool owned = false;
+    cudaStream_t st = nullptr;
+    int acquire(void* user, size_t user_bytes, size_t need, cudaStream_t s, int argpos)
+    {
+        st = s;
+        if (user) {
+            if (user_bytes < need || misaligned(user)) return -argpos;
+            ptr = user;
+            return 0;
+        }
+        if (need == 0) return 0;
+        cudaError_t ce = cudaMallocAsync(&ptr, need, s);
+        if (ce != cudaSuccess) return (int)ce;
+        owned = true;
+        return 0;
+    }
+    ~ScopedWork() { if (owned && ptr) cudaFreeAsync(ptr, st); }
+};
+
+}  // namespace letkf
+
+using namespace letkf;
+
+extern "C" {
+
+size_t letkf_syev_workspace_bytes(int M, int batch)
+{
+    if (M < 1 || M > LETKF_MAX_M || batch < 1) return 0;
+    Workspace ws;
+    return carve(ws, nullptr, M, syev_chunk(M, batch));
+}
+
+int letkf_syev_batched(const double* A, int M, int batch, double* w, double* V, int* info,
+                       void* work, size_t work_bytes, void* stream)
+{
+    g_launches = 0;
+    if (M < 1 || M > LETKF_MAX_M) return -2;
+    if (batch < 0) return -3;
+    if (batch == 0) return LETKF_OK;
+    if (!A || misaligned(A)) return -1;
+    if (!w || misaligned(w)) return -4;
+    if (!V || misaligned(V)) return -5;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    prof_reset(st);
+
+    const int chunk = syev_chunk(M, batch);
+    Workspace ws;
+    const size_t need = carve(ws, nullptr, M, chunk);
+    ScopedWork sw;
+    int rc = sw.acquire(work, work_bytes, need, st, 7);
+    if (rc) return rc;
+    carve(ws, sw.ptr, M, chunk);
+
+    for (int b0 = 0; b0 < batch; b0 += chunk) {
+        const int n = (batch - b0 < chunk) ? batch - b0 : chunk;
+        const size_t mo = (size_t)b0 * M * M;
+        rc = syev_chunk_run(A + mo, M, n, w + (size_t)b0 * M, V + mo, info ? info + b0 : nullptr, ws, st);
+        if (rc) return rc;
+    }
+    return LETKF_OK;
+}
+
+size_t letkf_analysis_workspace_bytes(int M, int p, int nstate, int batch)
+{
+    (void)p; (void)nstate;
+    if (M < 1 || M > LETKF_MAX_M || batch < 1) return 0;
+    const int chunk = syev_chunk(M, batch);
+    Workspace ws;
+    size_t s = carve(ws, nullptr, M, chunk);
+    s += align_up(sizeof(double) * (size_t)M * M * chunk, 256);   // Q / V
+    s += align_up(sizeof(double) * (size_t)M * chunk, 256);       // lam
+    s += align_up(sizeof(double) * (size_t)M * chunk, 256);       // g
+    return s;
+}
+
+int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv_loc,
+                           const double* Xb, int M, int p, int nstate, int batch, double rho,
+                           double* Xa, double* W, double* wbar, int* info,
+                           void* work, size_t work_bytes, void* stream)
+{
+    g_launches = 0;
+    if (M < 1 || M > LETKF_MAX_M) return -5;
+    if (p < 0) return -6;
+    if (nstate < 1) return -7;
+    if (batch < 0) return -8;
+    if (!(rho > 0.0)) return -9;
+    if (batch == 0) return LETKF_OK;
+    if (p > 0 && (!Yb || misaligned(Yb))) return -1;
+    if (p > 0 && (!d || misaligned(d))) return -2;
+    if (p > 0 && (!rinv_loc || misaligned(rinv_loc))) return -3;
+    if (!Xb || misaligned(Xb)) return -4;
+    if (!Xa || misaligned(Xa)) return -10;
+    if (W && misaligned(W)) return -11;
+    if (wbar && misaligned(wbar)) return -12;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    prof_reset(st);
+
+    const int chunk = syev_chunk(M, batch);
+    const size_t need = letkf_analysis_workspace_bytes(M, p, nstate, batch);
+    ScopedWork sw;
+    int rc = sw.acquire(work, work_bytes, need, st, 14);
+    if (rc) return rc;
+    Workspace ws;
+    size_t off = carve(ws, sw.ptr, M, chunk);
+    char* base = reinterpret_cast<char*>(sw.ptr);
+    double* Vbuf = reinterpret_cast<double*>(base + off); off += align_up(sizeof(double) * (size_t)M * M * chunk, 256);
+    double* lam  = reinterpret_cast<double*>(base + off); off += align_up(sizeof(double) * (size_t)M * chunk, 256);
+    double* gbuf = reinterpret_cast<double*>(base + off);
+
+    const double shift = (double)(M - 1) / rho;
+    cudaError_t ce;
+    const size_t ep_smem = sizeof(double) * (2 * (size_t)M + 2 * (size_t)nstate + 2 * (size_t)nstate * M);
+    if (ep_smem > 200 * 1024) return -7;
+    if ((ce = allow_smem(generic_epilogue, ep_smem)) != cudaSuccess) return (int)ce;
+
+    for (int b0 = 0; b0 < batch; b0 += chunk) {
+        const int n = (batch - b0 < chunk) ? batch - b0 : chunk;
+        const double* Ybc = Yb + (size_t)b0 * p * M;
+        const double* dc = d + (size_t)b0 * p;
+        const double* rc_ = rinv_loc + (size_t)b0 * p;
+        const double* Xbc = Xb + (size_t)b0 * nstate * M;
+        double* Xac = Xa + (size_t)b0 * nstate * M;
+        double* Wc = W ? W + (size_t)b0 * M * M : nullptr;
+        double* wbc = wbar ? wbar + (size_t)b0 * M : nullptr;
+        int* infoc = info ? info + b0 : nullptr;
+
+        if (fast_supported(M)) {
+            rc = fast_analysis_chunk(Ybc, dc, rc_, Xbc, M, p, nstate, n, shift, Xac, Wc, wbc, infoc,
+                                     ws, Vbuf, lam, gbuf, st, &g_launches);
+            if (rc) return rc;
+            continue;
+        }
+        KLAUNCH("generic_gram", st, generic_gram<<<n, 256, 0, st>>>(Ybc, dc, rc_, M, p, shift, Vbuf, gbuf));
+        rc = syev_chunk_run(Vbuf, M, n, lam, Vbuf, infoc, ws, st);
+        if (rc) return rc;
+        KLAUNCH("generic_epilogue", st,
+                generic_epilogue<<<n, 256, ep_smem, st>>>(Vbuf, lam, gbuf, Xbc, M, nstate, Xac, Wc, wbc));
+    }
+    return LETKF_OK;
+}
+
+int letkf_probe_dfma(double* sink, int blocks, int threads, int iters,
+                     unsigned long long* fma_count, void* stream)
+{
+    if (!sink) return -1;
+    if (blocks < 1) return -2;
+    if (threads < 1 || threads > 1024) return -3;
+    if (iters < 0) return -4;
+    probe_dfma_kernel<<<blocks, threads, 0, reinterpret_cast<cudaStream_t>(stream)>>>(sink, iters);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return (int)e;
+    if (fma_count) *fma_count = (unsigned long long)blocks * threads * (unsigned long long)iters * 64ull;
+    return LETKF_OK;
+}
+
+int letkf_last_launch_count(void) { return g_launches; }
+
+int letkf_profile_enable(int on)
+{
+    const int prev = g_prof.on ? 1 : 0;
+    g_prof.on = on != 0;
+    return prev;
+}
+
+int letkf_profile_count(void) { return (int)g_prof.recs.size(); }
+
+int letkf_profile_record(int idx, const char** name, float* ms)
+{
+    if (idx < 0 || idx >= (int)g_prof.recs.size()) return -1;
+    const ProfRec& r = g_prof.recs[idx];
+    cudaError_t e = cudaEventSynchronize(r.e1);
+    if (e != cudaSuccess) return (int)e;
+    float t = 0.f;
+    e = cudaEventElapsedTime(&t, r.e0, r.e1);
+    if (e != cudaSuccess) return (int)e;
+    if (name) *name = r.name;
+    if (ms) *ms = t;
+    return LETKF_OK;
+}
+
+long long letkf_profile_rotations(void)
+{
+    if (!g_prof.d_rot) return -1;
+    unsigned long long v = 0;
+    if (cudaMemcpy(&v, g_prof.d_rot, sizeof(v), cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+    return (long long)v;
+}
+
+const char* letkf_status_string(int status)
+{
+    static thread_local char buf[96];
+    if (status == 0) return "ok";
+    if (status < 0) {
+        snprintf(buf, sizeof(buf), "invalid argument %d (1-based position in the call)", -status);
+        return buf;
+    }
+    return cudaGetErrorString((cudaError_t)status);
+}
+
+int letkf_version(void) { return LETKF_VERSION; }
+
+}  // extern "C"

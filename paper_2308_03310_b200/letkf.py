@@ -1,0 +1,197 @@
+"""Thin Python binding of libletkf (include/letkf.h): argument marshalling only.
+
+Every step of the hot path runs inside the CUDA library; torch is used for device memory and
+streams.  There is no CPU fallback: if libletkf.so is missing or no CUDA device is present the
+calls raise.  Names and argument order follow the C ABI one to one.
+"""
+import ctypes
+import os
+
+import torch
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libletkf.so")
+MAX_M = 256
+INFO_SLOWPATH = 0x40000000
+
+EXPORTS = (
+    "letkf_syev_batched", "letkf_syev_workspace_bytes",
+    "letkf_analysis_batched", "letkf_analysis_workspace_bytes",
+    "letkf_probe_dfma", "letkf_last_launch_count",
+    "letkf_profile_enable", "letkf_profile_count", "letkf_profile_record", "letkf_profile_rotations",
+    "letkf_status_string", "letkf_version",
+)
+
+_lib = None
+
+
+class LetkfError(RuntimeError):
+    pass
+
+
+def load():
+    """dlopen libletkf.so and declare the prototypes.  Raises if the library is not built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise LetkfError(
+            f"{LIB_PATH} not found: build it with `python -m paper_2308_03310_b200.build` "
+            "(or __graft_entry__.build()). There is no CPU fallback.")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, ci, cd, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+    lib.letkf_syev_batched.argtypes = [vp, ci, ci, vp, vp, vp, vp, sz, vp]
+    lib.letkf_syev_batched.restype = ci
+    lib.letkf_syev_workspace_bytes.argtypes = [ci, ci]
+    lib.letkf_syev_workspace_bytes.restype = sz
+    lib.letkf_analysis_batched.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, cd,
+                                           vp, vp, vp, vp, vp, sz, vp]
+    lib.letkf_analysis_batched.restype = ci
+    lib.letkf_analysis_workspace_bytes.argtypes = [ci, ci, ci, ci]
+    lib.letkf_analysis_workspace_bytes.restype = sz
+    lib.letkf_probe_dfma.argtypes = [vp, ci, ci, ci, ctypes.POINTER(ctypes.c_ulonglong), vp]
+    lib.letkf_probe_dfma.restype = ci
+    lib.letkf_last_launch_count.argtypes = []
+    lib.letkf_last_launch_count.restype = ci
+    lib.letkf_profile_enable.argtypes = [ci]
+    lib.letkf_profile_enable.restype = ci
+    lib.letkf_profile_count.argtypes = []
+    lib.letkf_profile_count.restype = ci
+    lib.letkf_profile_record.argtypes = [ci, ctypes.POINTER(ctypes.c_char_p), ctypes.POINTER(ctypes.c_float)]
+    lib.letkf_profile_record.restype = ci
+    lib.letkf_profile_rotations.argtypes = []
+    lib.letkf_profile_rotations.restype = ctypes.c_longlong
+    lib.letkf_status_string.argtypes = [ci]
+    lib.letkf_status_string.restype = ctypes.c_char_p
+    lib.letkf_version.argtypes = []
+    lib.letkf_version.restype = ci
+    _lib = lib
+    return lib
+
+
+def _check(status, what):
+    if status != 0:
+        msg = load().letkf_status_string(status).decode()
+        raise LetkfError(f"{what} failed with status {status}: {msg}")
+
+
+def _ptr(t):
+    return ctypes.c_void_p(t.data_ptr()) if t is not None else ctypes.c_void_p(0)
+
+
+def _stream(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+def _dev_f64(t, name):
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64
+            and t.is_contiguous()):
+        raise LetkfError(f"{name} must be a contiguous float64 CUDA tensor")
+    return t
+
+
+def version():
+    return load().letkf_version()
+
+
+def last_launch_count():
+    return load().letkf_last_launch_count()
+
+
+def syev_workspace_bytes(M, batch):
+    return load().letkf_syev_workspace_bytes(M, batch)
+
+
+def analysis_workspace_bytes(M, p, nstate, batch):
+    return load().letkf_analysis_workspace_bytes(M, p, nstate, batch)
+
+
+def syev_batched(A, w=None, V=None, info=None, work=None, stream=None):
+    """letkf_syev_batched: A[batch][M][M] (lower triangle read) -> (w, V, info).
+
+    ``V`` may be ``A`` itself (in place).  Outputs are allocated when not given.  The call is
+    stream-ordered and does not synchronise.
+    """
+    lib = load()
+    _dev_f64(A, "A")
+    batch, M, M2 = A.shape
+    if M != M2:
+        raise LetkfError("A must be [batch][M][M]")
+    if w is None:
+        w = torch.empty((batch, M), dtype=torch.float64, device=A.device)
+    if V is None:
+        V = torch.empty_like(A)
+    if info is None:
+        info = torch.zeros((batch,), dtype=torch.int32, device=A.device)
+    _dev_f64(w, "w")
+    _dev_f64(V, "V")
+    wb = work.numel() * work.element_size() if work is not None else 0
+    with torch.cuda.device(A.device):
+        st = lib.letkf_syev_batched(_ptr(A), M, batch, _ptr(w), _ptr(V), _ptr(info),
+                                    _ptr(work), wb, _stream(stream))
+    _check(st, "letkf_syev_batched")
+    return w, V, info
+
+
+def analysis_batched(Yb, d, rinv_loc, Xb, rho, Xa=None, want_W=False, want_wbar=False,
+                     W=None, wbar=None, info=None, work=None, stream=None):
+    """letkf_analysis_batched: Yb[batch][p][M], d[batch][p], rinv_loc[batch][p],
+    Xb[batch][nstate][M] -> dict(Xa, W, wbar, info).  ``Xa`` may be ``Xb`` (in place)."""
+    lib = load()
+    _dev_f64(Yb, "Yb")
+    _dev_f64(d, "d")
+    _dev_f64(rinv_loc, "rinv_loc")
+    _dev_f64(Xb, "Xb")
+    batch, p, M = Yb.shape
+    nstate = Xb.shape[1]
+    if d.shape != (batch, p) or rinv_loc.shape != (batch, p) or Xb.shape != (batch, nstate, M):
+        raise LetkfError("inconsistent shapes")
+    dev = Xb.device
+    if Xa is None:
+        Xa = torch.empty_like(Xb)
+    if W is None and want_W:
+        W = torch.empty((batch, M, M), dtype=torch.float64, device=dev)
+    if wbar is None and want_wbar:
+        wbar = torch.empty((batch, M), dtype=torch.float64, device=dev)
+    if info is None:
+        info = torch.zeros((batch,), dtype=torch.int32, device=dev)
+    wb = work.numel() * work.element_size() if work is not None else 0
+    with torch.cuda.device(dev):
+        st = lib.letkf_analysis_batched(_ptr(Yb), _ptr(d), _ptr(rinv_loc), _ptr(Xb),
+                                        M, p, nstate, batch, float(rho),
+                                        _ptr(Xa), _ptr(W), _ptr(wbar), _ptr(info),
+                                        _ptr(work), wb, _stream(stream))
+    _check(st, "letkf_analysis_batched")
+    return dict(Xa=Xa, W=W, wbar=wbar, info=info)
+
+
+def probe_dfma(blocks, threads, iters, stream=None):
+    """Launch the fp64-FMA throughput probe once; returns the number of FMAs it executes."""
+    lib = load()
+    sink = torch.empty((blocks * threads,), dtype=torch.float64, device="cuda")
+    n = ctypes.c_ulonglong(0)
+    st = lib.letkf_probe_dfma(_ptr(sink), blocks, threads, iters, ctypes.byref(n), _stream(stream))
+    _check(st, "letkf_probe_dfma")
+    return n.value, sink
+
+
+def profile_enable(on):
+    return load().letkf_profile_enable(1 if on else 0)
+
+
+def profile_records():
+    """[(kernel name, milliseconds)] of the last compute call (synchronises)."""
+    lib = load()
+    out = []
+    for i in range(lib.letkf_profile_count()):
+        name = ctypes.c_char_p()
+        ms = ctypes.c_float()
+        _check(lib.letkf_profile_record(i, ctypes.byref(name), ctypes.byref(ms)), "letkf_profile_record")
+        out.append((name.value.decode(), ms.value))
+    return out
+
+
+def profile_rotations():
+    return load().letkf_profile_rotations()

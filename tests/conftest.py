@@ -17,3 +17,7 @@ def oracle():
     import oracle as _oracle
     _oracle.build()
     return _oracle
+
+TESTS = os.path.dirname(os.path.abspath(__file__))
+if TESTS not in sys.path:
+    sys.path.insert(0, TESTS)

@@ -1,0 +1,126 @@
+"""GPU parity: letkf_analysis_batched (through the C ABI) against the CPU oracle.
+PAPER.md:120-146 (Eq.13-19); tolerances of north_star / parity.py."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2308_03310_b200 import workloads as wl
+import parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def lk():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    from paper_2308_03310_b200 import build, letkf
+    build.build()
+    letkf.load()
+    return letkf
+
+
+def run_gpu(lk, inp, want_W=True, want_wbar=True, rho=None, **kw):
+    import torch
+    t = {k: torch.from_numpy(np.ascontiguousarray(inp[k])).cuda() for k in ("Yb", "d", "rinv_loc", "Xb")}
+    out = lk.analysis_batched(t["Yb"], t["d"], t["rinv_loc"], t["Xb"], inp["rho"] if rho is None else rho,
+                              want_W=want_W, want_wbar=want_wbar, **kw)
+    torch.cuda.synchronize()
+    return {k: (v.cpu().numpy() if v is not None else None) for k, v in out.items()}
+
+
+def run_oracle(oracle, inp, rho=None):
+    return oracle.letkf_analysis_batched(inp["Yb"], inp["d"], inp["rinv_loc"], inp["Xb"],
+                                         inp["rho"] if rho is None else rho)
+
+
+@pytest.mark.parametrize("M,p,ns,batch", [(64, 98, 9, 200), (64, 3, 9, 65), (64, 48, 9, 64), (48, 49, 9, 100),
+                                          (32, 49, 9, 100), (16, 5, 3, 77), (6, 4, 2, 5), (2, 7, 1, 9),
+                                          (1, 3, 2, 4), (33, 20, 4, 21), (96, 98, 9, 6), (130, 98, 9, 3)])
+def test_analysis_vs_oracle(lk, oracle, M, p, ns, batch):
+    """BASELINE config 4 shape (reduced batch), the paper's dense (p=3) and sparse (p=48) shapes,
+    and ragged / odd sizes."""
+    inp = wl.analysis_inputs(batch=batch, M=M, p=p, nstate=ns, config_index=400 + M + p)
+    out = run_gpu(lk, inp)
+    ref = run_oracle(oracle, inp)
+    assert (out["info"] == 0).all()
+    parity.assert_analysis(out, ref, inp["Xb"], f"M={M} p={p} ns={ns}")
+
+
+def test_without_optional_outputs_and_in_place(lk, oracle):
+    import torch
+    inp = wl.analysis_inputs(batch=50, M=64, p=98, nstate=9, config_index=41)
+    ref = run_oracle(oracle, inp)
+    out = run_gpu(lk, inp, want_W=False, want_wbar=False)
+    assert out["W"] is None and out["wbar"] is None
+    parity.assert_analysis(out, ref, inp["Xb"], "no W")
+    t = {k: torch.from_numpy(inp[k]).cuda() for k in ("Yb", "d", "rinv_loc", "Xb")}
+    Xb = t["Xb"].clone()
+    o2 = lk.analysis_batched(t["Yb"], t["d"], t["rinv_loc"], Xb, inp["rho"], Xa=Xb)
+    torch.cuda.synchronize()
+    assert o2["Xa"].data_ptr() == Xb.data_ptr()
+    parity.assert_analysis({"Xa": Xb.cpu().numpy()}, ref, inp["Xb"], "in place")
+
+
+def test_no_observations_closed_form(lk):
+    """p = 0 (pin P-9): A = ((M-1)/rho) I, W = sqrt(rho) I, wbar = 0, Xa = xbar + sqrt(rho) dX."""
+    inp = wl.analysis_inputs(batch=7, M=64, p=0, nstate=9, config_index=42)
+    out = run_gpu(lk, inp)
+    xbar = inp["Xb"].mean(axis=2, keepdims=True)
+    exact = xbar + math.sqrt(inp["rho"]) * (inp["Xb"] - xbar)
+    assert np.abs(out["Xa"] - exact).max() <= 1e-13
+    assert np.abs(out["W"] - math.sqrt(inp["rho"]) * np.eye(64)).max() <= 1e-13
+    assert np.abs(out["wbar"]).max() == 0.0
+
+
+def test_zero_weights_are_padding(lk, oracle):
+    """Reading G7 (PAPER.md:151 l_max padding): zero-weight observations do not matter."""
+    inp = wl.analysis_inputs(batch=30, M=64, p=98, nstate=9, config_index=43, zero_weight_fraction=0.25)
+    out = run_gpu(lk, inp)
+    ref = run_oracle(oracle, inp)
+    parity.assert_analysis(out, ref, inp["Xb"], "25% zero weights")
+    junk = dict(inp)
+    junk["Yb"] = inp["Yb"].copy()
+    junk["d"] = inp["d"].copy()
+    mask = inp["rinv_loc"] == 0.0
+    junk["Yb"][mask] = 123.0
+    junk["d"][mask] = -7.0
+    out2 = run_gpu(lk, junk)
+    assert parity.rel_fro(out2["Xa"], out["Xa"]) <= 1e-13
+
+
+def test_rho_one_is_eq17(lk, oracle):
+    inp = wl.analysis_inputs(batch=20, M=64, p=98, nstate=9, config_index=44)
+    out = run_gpu(lk, inp, rho=1.0)
+    ref = run_oracle(oracle, inp, rho=1.0)
+    parity.assert_analysis(out, ref, inp["Xb"], "rho=1")
+
+
+def test_structural_identities_full_size(lk, oracle):
+    """BASELINE config 4 at full size (128x128 points, the launch configuration bench.py times):
+    pins P-8 on every point -- W symmetric, W 1 = sqrt(rho) 1, mean(Xa) = xbar + dX wbar --
+    plus oracle parity on a strided sample."""
+    import torch
+    inp = wl.analysis_inputs()                       # batch=16384, M=64, p=98, ns=9
+    t = {k: torch.from_numpy(inp[k]).cuda() for k in ("Yb", "d", "rinv_loc", "Xb")}
+    out = lk.analysis_batched(t["Yb"], t["d"], t["rinv_loc"], t["Xb"], inp["rho"], want_W=True, want_wbar=True)
+    torch.cuda.synchronize()
+    assert int(out["info"].abs().max()) == 0
+    W, wbar, Xa, Xb = out["W"], out["wbar"], out["Xa"], t["Xb"]
+    assert float((W - W.transpose(1, 2)).abs().max()) <= 1e-12
+    assert float((W.sum(dim=2) - math.sqrt(inp["rho"])).abs().max()) <= 1e-11
+    xbar = Xb.mean(dim=2, keepdim=True)
+    dX = Xb - xbar
+    mean_pred = xbar.squeeze(2) + torch.einsum("bsm,bm->bs", dX, wbar) \
+        + (math.sqrt(inp["rho"]) - 1.0) * 0.0
+    # mean over members of dX W = dX (W 1)/M = sqrt(rho) dX 1 / M = 0
+    assert float((Xa.mean(dim=2) - mean_pred).abs().max()) <= 1e-12
+    sel = np.arange(0, 16384, 256)
+    sub = {k: (v[sel] if isinstance(v, np.ndarray) else v) for k, v in inp.items()}
+    ref = run_oracle(oracle, sub)
+    got = {"Xa": Xa.cpu().numpy()[sel], "W": W.cpu().numpy()[sel], "wbar": wbar.cpu().numpy()[sel]}
+    parity.assert_analysis(got, ref, sub["Xb"], "config4 sample")
+    out2 = lk.analysis_batched(t["Yb"], t["d"], t["rinv_loc"], t["Xb"], inp["rho"])
+    torch.cuda.synchronize()
+    assert float((out2["Xa"] - Xa).abs().max()) <= 1e-13

@@ -1,0 +1,193 @@
+"""GPU parity: letkf_syev_batched (through the C ABI) against the CPU oracle on the same seeded
+inputs.  PAPER.md:142, 183 (EVD by Householder + QL); tolerances of north_star / parity.py."""
+import numpy as np
+import pytest
+
+from paper_2308_03310_b200 import workloads as wl
+import parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def lk():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    from paper_2308_03310_b200 import build, letkf
+    build.build()
+    letkf.load()
+    return letkf
+
+
+def run_gpu(lk, A, **kw):
+    import torch
+    At = torch.from_numpy(np.ascontiguousarray(A)).cuda()
+    w, V, info = lk.syev_batched(At, **kw)
+    torch.cuda.synchronize()
+    return w.cpu().numpy(), V.cpu().numpy(), info.cpu().numpy()
+
+
+def test_config1_known_spectrum(lk, oracle):
+    """BASELINE config 1: M=32, batch=1024, A = Q diag(lam) Q^T; eigenvalues known by construction."""
+    A, lam = wl.known_spectrum(batch=1024, M=32)
+    w, V, info = run_gpu(lk, A)
+    assert (info == 0).all()
+    wo, Vo, io, _ = oracle.syev_batched(A)
+    assert (io == 0).all()
+    parity.assert_evd(A, w, V, wo, "config1 vs oracle")
+    scale = lam.max(axis=1)
+    assert (np.abs(w - lam).max(axis=1) / scale).max() <= 1e-12      # the construction's own spectrum
+
+
+@pytest.mark.parametrize("M,p,batch", [(48, 49, 300), (64, 98, 300), (16, 49, 257), (32, 49, 129)])
+def test_letkf_shaped_vs_oracle(lk, oracle, M, p, batch):
+    """BASELINE configs 2/3/5 (reduced batch): A = ((M-1)/rho) I + Yb^T diag(r) Yb."""
+    A = wl.letkf_shaped(batch, M, p, config_index=20 + M)
+    w, V, info = run_gpu(lk, A)
+    assert (info == 0).all()
+    wo, _, _, _ = oracle.syev_batched(A)
+    parity.assert_evd(A, w, V, wo, f"M={M} p={p}")
+
+
+@pytest.mark.parametrize("M", [1, 2, 3, 4, 5, 7, 15, 17, 31, 33, 47, 63, 65, 96, 100, 128])
+def test_any_order_vs_oracle(lk, oracle, M):
+    batch = 37 if M <= 65 else 9
+    rng = np.random.Generator(np.random.Philox(key=77 + M))
+    G = rng.standard_normal((batch, M, M))
+    A = G + np.transpose(G, (0, 2, 1))
+    w, V, info = run_gpu(lk, A)
+    assert (info == 0).all()
+    wo, _, _, _ = oracle.syev_batched(A)
+    parity.assert_evd(A, w, V, wo, f"random symmetric M={M}")
+
+
+@pytest.mark.parametrize("M", [192, 256])
+def test_large_order_vs_oracle(lk, oracle, M):
+    A = wl.config5(M, batch=4)
+    w, V, info = run_gpu(lk, A)
+    assert (info == 0).all()
+    wo, _, _, _ = oracle.syev_batched(A)
+    parity.assert_evd(A, w, V, wo, f"config5 M={M}")
+
+
+@pytest.mark.parametrize("p", [0, 3, 48])
+def test_paper_shaped_clusters(lk, oracle, p):
+    """Dense (l_max=1, V=3 -> p=3) and sparse (p=48) observation
+    shapes: an (M-p)-fold eigenvalue cluster at (M-1)/rho and zero Householder columns."""
+    M, batch = 64, 64
+    A = wl.letkf_shaped(batch, M, p, config_index=600 + p)
+    w, V, info = run_gpu(lk, A)
+    assert (info == 0).all()
+    wo, _, _, _ = oracle.syev_batched(A)
+    parity.assert_evd(A, w, V, wo, f"cluster p={p}")
+    if p < M - 1:
+        assert np.abs(w[:, : M - max(p, 1)] - (M - 1) / wl.RHO).max() <= 1e-12 * np.abs(wo).max()
+
+
+@pytest.mark.parametrize("M", [8, 64, 100])
+def test_toeplitz_closed_form(lk, M):
+    """tridiag(1,0,1): lambda_k = 2 cos(k pi/(M+1)) -- closed form, no oracle involved."""
+    A = np.stack([wl.toeplitz_tridiagonal(M), wl.toeplitz_tridiagonal(M, a=3.0, b=-0.5)])
+    w, V, info = run_gpu(lk, A)
+    k = np.arange(1, M + 1)
+    exact0 = np.sort(2.0 * np.cos(k * np.pi / (M + 1)))
+    exact1 = np.sort(3.0 - 1.0 * np.cos(k * np.pi / (M + 1)))
+    assert np.abs(w[0] - exact0).max() <= 1e-12 * 2
+    assert np.abs(w[1] - exact1).max() <= 1e-12 * 4
+    parity.assert_evd(A, w, V, None, "toeplitz")
+
+
+def test_degenerate_inputs(lk):
+    M = 64
+    A = np.zeros((4, M, M))
+    A[1] = 3.5 * np.eye(M)                                   # A = cI
+    A[2] = np.diag(np.arange(M, 0, -1.0))                    # diagonal, descending
+    A[3][0, 0] = 1.0                                         # rank one
+    w, V, info = run_gpu(lk, A)
+    assert (info == 0).all()
+    parity.assert_evd(A, w, V, None, "degenerate")
+    assert np.abs(w[0]).max() == 0.0
+    assert np.abs(w[1] - 3.5).max() == 0.0
+    assert np.abs(w[2] - np.arange(1.0, M + 1)).max() == 0.0
+
+
+def test_only_lower_triangle_is_read(lk, oracle):
+    A = wl.letkf_shaped(40, 64, 98, config_index=31)
+    junk = A.copy()
+    iu = np.triu_indices(64, 1)
+    junk[:, iu[0], iu[1]] = 1e30
+    w, V, _ = run_gpu(lk, junk)
+    w2, V2, _ = run_gpu(lk, A)
+    assert np.array_equal(w, w2) and np.array_equal(V, V2)
+
+
+def test_in_place_and_user_workspace(lk):
+    import torch
+    A = wl.letkf_shaped(100, 48, 49, config_index=32)
+    At = torch.from_numpy(A).cuda()
+    w0, V0, _ = lk.syev_batched(At)
+    nbytes = lk.syev_workspace_bytes(48, 100)
+    work = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    Ain = At.clone()
+    w1, V1, _ = lk.syev_batched(Ain, V=Ain, work=work)
+    torch.cuda.synchronize()
+    assert V1.data_ptr() == Ain.data_ptr()
+    assert torch.equal(w0, w1) and torch.equal(V0, V1)
+    small = torch.empty(64, dtype=torch.uint8, device="cuda")
+    with pytest.raises(lk.LetkfError):
+        lk.syev_batched(At, work=small)
+
+
+@pytest.mark.parametrize("batch", [1, 31, 33, 1000])
+def test_ragged_batches(lk, oracle, batch):
+    A = wl.letkf_shaped(batch, 64, 98, config_index=33)
+    w, V, info = run_gpu(lk, A)
+    assert (info == 0).all()
+    sel = np.unique(np.linspace(0, batch - 1, min(batch, 40)).astype(int))
+    wo, _, _, _ = oracle.syev_batched(A[sel])
+    parity.assert_evd(A[sel], w[sel], V[sel], wo, f"batch={batch}")
+    parity.assert_evd(A, w, V, None, f"batch={batch} all")
+
+
+def test_determinism(lk):
+    A = wl.letkf_shaped(200, 64, 98, config_index=34)
+    a = run_gpu(lk, A)
+    b = run_gpu(lk, A)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+def test_nan_input_terminates(lk):
+    A = wl.letkf_shaped(8, 64, 98, config_index=35)
+    A[3, 10, 4] = np.nan
+    w, V, info = run_gpu(lk, A)
+    assert info[3] != 0
+    good = [0, 1, 2, 4, 5, 6, 7]
+    assert (info[good] == 0).all()
+    parity.assert_evd(A[good], w[good], V[good], None, "neighbours of a NaN matrix")
+
+
+def test_headline_full_size(lk, oracle):
+    """BASELINE config 3 at full size (M=64, batch=16384, the launch configuration bench.py times):
+    residual/orthogonality/ordering on every matrix, oracle parity on a strided sample."""
+    A = wl.config3()
+    w, V, info = run_gpu(lk, A)
+    assert (info == 0).all()
+    for b0 in range(0, A.shape[0], 2048):
+        sl = slice(b0, b0 + 2048)
+        parity.assert_evd(A[sl], w[sl], V[sl], None, f"config3 [{b0}:]")
+    assert np.abs(w[:, 0] - 63 / wl.RHO).max() <= 1e-12 * w.max()   # A 1 = ((M-1)/rho) 1 (rows centred)
+    sel = np.arange(0, A.shape[0], 128)
+    wo, _, _, _ = oracle.syev_batched(A[sel])
+    parity.assert_evd(A[sel], w[sel], V[sel], wo, "config3 sample vs oracle")
+
+
+def test_config2_full_size(lk, oracle):
+    A = wl.config2()
+    w, V, info = run_gpu(lk, A)
+    assert (info == 0).all()
+    for b0 in range(0, A.shape[0], 4096):
+        sl = slice(b0, b0 + 4096)
+        parity.assert_evd(A[sl], w[sl], V[sl], None, f"config2 [{b0}:]")
+    sel = np.arange(0, A.shape[0], 128)
+    wo, _, _, _ = oracle.syev_batched(A[sel])
+    parity.assert_evd(A[sel], w[sel], V[sel], wo, "config2 sample vs oracle")
