@@ -131,6 +131,10 @@ long long letkf_profile_rotations(void);
  * gpu_launches claim is counted from this, not guessed). */
 int letkf_last_launch_count(void);
 
+/* Test/diagnostic options.  "force_generic" = 1 routes every M through the any-M kernels
+ * (otherwise only M > 64 and overflowed matrices use them).  Returns 0, or -1 for an unknown name. */
+int letkf_set_option(const char* name, int value);
+
 const char* letkf_status_string(int status);
 int letkf_version(void);
 

@@ -131,20 +131,20 @@ __device__ __forceinline__ int ql_next_sweep(QLState& st, double* d, double* e, 
 }
 
 // Ascending insertion sort of d with the permutation that sorts it (stable).
-__device__ __forceinline__ void sort_eigenvalues(double* d, int* perm, int stride, int M)
+__device__ __forceinline__ void sort_eigenvalues(double* d, int dstride, int* perm, int pstride, int M)
 {
-    for (int k = 0; k < M; ++k) perm[(size_t)k * stride] = k;
+    for (int k = 0; k < M; ++k) perm[(size_t)k * pstride] = k;
     for (int k = 1; k < M; ++k) {
-        const double val = d[(size_t)k * stride];
-        const int pk = perm[(size_t)k * stride];
+        const double val = d[(size_t)k * dstride];
+        const int pk = perm[(size_t)k * pstride];
         int j = k - 1;
-        while (j >= 0 && d[(size_t)j * stride] > val) {
-            d[(size_t)(j + 1) * stride] = d[(size_t)j * stride];
-            perm[(size_t)(j + 1) * stride] = perm[(size_t)j * stride];
+        while (j >= 0 && d[(size_t)j * dstride] > val) {
+            d[(size_t)(j + 1) * dstride] = d[(size_t)j * dstride];
+            perm[(size_t)(j + 1) * pstride] = perm[(size_t)j * pstride];
             --j;
         }
-        d[(size_t)(j + 1) * stride] = val;
-        perm[(size_t)(j + 1) * stride] = pk;
+        d[(size_t)(j + 1) * dstride] = val;
+        perm[(size_t)(j + 1) * pstride] = pk;
     }
 }
 

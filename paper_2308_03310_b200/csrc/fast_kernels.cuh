@@ -1,11 +1,375 @@
-// fast_kernels.cuh -- register-resident path for M <= 64 (stub: not enabled yet).
+// fast_kernels.cuh -- register-resident path for M <= 64 (the paper's sizes, Table I,
+// and the headline M = 64).
+//
+// Design: a matrix lives in the REGISTERS of MT threads, one row (or, while
+// Q is formed, one column) per thread, for its whole life inside a kernel.  An SM issues 64 fp64
+// FMAs per clock but shared memory delivers only 16 doubles per clock, so BLAS-2 work fed from
+// shared memory cannot pass 25% of the fp64 peak; here shared memory only carries the
+// broadcast vectors (one LDS.128 feeds two FMAs in every lane).  Register arrays need
+// compile-time indices, so every loop whose bounds move with the reduction step is a fully
+// unrolled block entered through a jump table (a switch with fall-through cases).
+//
+//   fast_tridiag_formq<MT>   a3 + explicit Q  : thread j = row j of A, then column r of Q
+//   ql_log_kernel            a4               : ql_kernel.cuh, one thread per matrix
+//   fast_apply<MT>           a5 (+ a6-a9)     : thread r = row r of Q; replays the rotation log
 #pragma once
 #include "common.cuh"
+
 namespace letkf {
-static inline bool fast_supported(int) { return false; }
-static inline int fast_tridiag_launch(const double*, double*, Workspace, int, int, cudaStream_t) { return -1; }
-static inline int fast_apply_launch(double*, Workspace, int, int, cudaStream_t) { return -1; }
-static inline int fast_analysis_chunk(const double*, const double*, const double*, const double*, int, int, int,
-                                      int, double, double*, double*, double*, int*, Workspace, double*, double*,
-                                      double*, cudaStream_t, int*) { return -1; }
+
+// X(31) X(30) ... X(0)
+#define LETKF_REP32_DESC(X) \
+    X(31) X(30) X(29) X(28) X(27) X(26) X(25) X(24) X(23) X(22) X(21) X(20) X(19) X(18) X(17) X(16) \
+    X(15) X(14) X(13) X(12) X(11) X(10) X(9) X(8) X(7) X(6) X(5) X(4) X(3) X(2) X(1) X(0)
+#define LETKF_REP64_DESC(X) \
+    X(63) X(62) X(61) X(60) X(59) X(58) X(57) X(56) X(55) X(54) X(53) X(52) X(51) X(50) X(49) X(48) \
+    X(47) X(46) X(45) X(44) X(43) X(42) X(41) X(40) X(39) X(38) X(37) X(36) X(35) X(34) X(33) X(32) \
+    X(31) X(30) X(29) X(28) X(27) X(26) X(25) X(24) X(23) X(22) X(21) X(20) X(19) X(18) X(17) X(16) \
+    X(15) X(14) X(13) X(12) X(11) X(10) X(9) X(8) X(7) X(6) X(5) X(4) X(3) X(2) X(1) X(0)
+
+// register-array read with a run-time index (jump table; indices stay compile-time constants)
+template <int MT>
+__device__ __forceinline__ double pick(const double (&a)[MT], int i)
+{
+    double x = 0.0;
+    switch (i) {
+#define LETKF_PICK(c) case c: if constexpr (c < MT) x = a[c]; break;
+        LETKF_REP64_DESC(LETKF_PICK)
+#undef LETKF_PICK
+    }
+    return x;
 }
+
+// acc = sum_{c < 2*(qtop+1)} a[c] * vec[c]          (vec in shared memory, 16-byte aligned)
+template <int MT>
+__device__ __forceinline__ double dot_desc(const double (&a)[MT], const double* vec, int qtop)
+{
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    const double2* v2 = reinterpret_cast<const double2*>(vec);
+    switch (qtop) {
+#define LETKF_DOT(q)                                                          \
+    case q:                                                                   \
+        if constexpr (2 * (q) + 1 < MT) {                                     \
+            const double2 t = v2[q];                                          \
+            if ((q) & 1) { s2 = fma(a[2 * (q)], t.x, s2); s3 = fma(a[2 * (q) + 1], t.y, s3); } \
+            else         { s0 = fma(a[2 * (q)], t.x, s0); s1 = fma(a[2 * (q) + 1], t.y, s1); } \
+        }
+        LETKF_REP32_DESC(LETKF_DOT)
+#undef LETKF_DOT
+    }
+    return (s0 + s1) + (s2 + s3);
+}
+
+// a[c] -= alpha * vec[c]   for c < 2*(qtop+1)
+template <int MT>
+__device__ __forceinline__ void axpy_desc(double (&a)[MT], const double* vec, double alpha, int qtop)
+{
+    const double2* v2 = reinterpret_cast<const double2*>(vec);
+    switch (qtop) {
+#define LETKF_AXPY(q)                                                         \
+    case q:                                                                   \
+        if constexpr (2 * (q) + 1 < MT) {                                     \
+            const double2 t = v2[q];                                          \
+            a[2 * (q)]     = fma(-alpha, t.x, a[2 * (q)]);                    \
+            a[2 * (q) + 1] = fma(-alpha, t.y, a[2 * (q) + 1]);                \
+        }
+        LETKF_REP32_DESC(LETKF_AXPY)
+#undef LETKF_AXPY
+    }
+}
+
+// a[c] -= vj * w[c] + wj * v[c]   for c < 2*(qtop+1);  vw[c] = (v_c, w_c)
+template <int MT>
+__device__ __forceinline__ void rank2_desc(double (&a)[MT], const double2* vw, double vj, double wj, int qtop)
+{
+    switch (qtop) {
+#define LETKF_R2(q)                                                           \
+    case q:                                                                   \
+        if constexpr (2 * (q) + 1 < MT) {                                     \
+            const double2 t0 = vw[2 * (q)];                                   \
+            const double2 t1 = vw[2 * (q) + 1];                               \
+            a[2 * (q)]     = fma(-vj, t0.y, fma(-wj, t0.x, a[2 * (q)]));      \
+            a[2 * (q) + 1] = fma(-vj, t1.y, fma(-wj, t1.x, a[2 * (q) + 1]));  \
+        }
+        LETKF_REP32_DESC(LETKF_R2)
+#undef LETKF_R2
+    }
+}
+
+template <int MT> struct FastCfg {
+    static constexpr int NT = (MT + 31) / 32 * 32;      // threads per matrix = threads per CTA
+    static constexpr int NW = NT / 32;
+    static constexpr int LDT = MT + 1;                  // padded tile stride (doubles)
+};
+
+// Sum over the CTA of one double per thread, MT <= 64: warp shuffle + one shared slot per warp.
+// Costs one __syncthreads; `slot` is a 2-double scratch that must not be reused before the next
+// barrier of the caller.
+template <int NW>
+__device__ __forceinline__ double cta_sum(double v, double* slot)
+{
+    v = warp_sum(v);
+    if constexpr (NW == 1) return v;
+    if ((threadIdx.x & 31) == 0) slot[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double t = 0.0;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) t += slot[w];
+    return t;
+}
+
+// Barrier over the first `nwarps` warps of the CTA (named barrier 1; __syncwarp when one warp).
+__device__ __forceinline__ void part_barrier(int nwarps)
+{
+    if (nwarps <= 1) __syncwarp();
+    else asm volatile("bar.sync 1, %0;" ::"r"(nwarps * 32) : "memory");
+}
+
+// Dynamic shared memory of fast_tridiag_formq<MT>:
+//   tile[MT*(MT+1)]  staging of A (padded), later the reflectors R[i][c] (stride MT)
+//   vs[MT]  v;  vw[MT] (v,w) pairs;  taus[MT];  red[8]
+template <int MT> constexpr size_t fast_tridiag_smem()
+{
+    return sizeof(double) * ((size_t)MT * (MT + 1) + MT + 2 * MT + MT + 8);
+}
+
+// ---------------------------------------------------------------------------------------------
+// a3 + explicit Q for one matrix per CTA.  gram == true: the matrix is not read from A but formed
+// from the LETKF inputs (a1, a2: Eq.17 and the right factor of Eq.14) straight into the registers.
+template <int MT, bool GRAM>
+__global__ void __launch_bounds__(FastCfg<MT>::NT, (MT == 64) ? 6 : (MT == 48 ? 8 : 16))
+fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Workspace ws, int M,
+                   const double* __restrict__ Yb_, const double* __restrict__ d_,
+                   const double* __restrict__ r_, int p, double shift, double* __restrict__ gout_)
+{
+    using C = FastCfg<MT>;
+    extern __shared__ __align__(16) double sm[];
+    double*  tile = sm;
+    double*  vs   = sm + MT * (MT + 1);
+    double2* vw   = reinterpret_cast<double2*>(vs + MT);
+    double*  taus = vs + 3 * MT;
+    double*  red  = taus + MT;
+    const int j = threadIdx.x, lane = j & 31, warp = j >> 5;
+    const size_t b = blockIdx.x;
+    double a[MT];
+
+    if constexpr (!GRAM) {
+        const double* A = A_ + b * M * M;
+        for (int idx = j; idx < M * M; idx += C::NT) {
+            const int r = idx / M, c = idx - r * M;
+            tile[r * C::LDT + c] = A[idx];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int c = 0; c < MT; ++c) {
+            double v = 0.0;
+            if (j < M && c < M) v = (c <= j) ? tile[j * C::LDT + c] : tile[c * C::LDT + j];
+            a[c] = v;
+        }
+        __syncthreads();
+    } else {
+        // a_j[c] = shift*delta + sum_i r_i Yb[i][j] Yb[i][c];  Yb rows staged through the tile
+        const double* Yb = Yb_ + b * (size_t)p * M;
+        const double* dv = d_ + b * (size_t)p;
+        const double* rv = r_ + b * (size_t)p;
+#pragma unroll
+        for (int c = 0; c < MT; ++c) a[c] = (c == j && j < M) ? shift : 0.0;
+        double gj = 0.0;
+        constexpr int RB = MT;                    // observation rows per stage (tile holds MT rows of MT)
+        for (int i0 = 0; i0 < p; i0 += RB) {
+            const int nr = min(RB, p - i0);
+            for (int idx = j; idx < nr * MT; idx += C::NT) {
+                const int r = idx / MT, c = idx - r * MT;
+                tile[idx] = (c < M) ? Yb[(size_t)(i0 + r) * M + c] : 0.0;
+            }
+            __syncthreads();
+            for (int r = 0; r < nr; ++r) {
+                const double ri = rv[i0 + r];
+                const double yj = tile[r * MT + j];
+                const double yr = yj * ri;
+                gj = fma(yr, dv[i0 + r], gj);
+                const double2* row = reinterpret_cast<const double2*>(tile + r * MT);
+#pragma unroll
+                for (int q = 0; q < MT / 2; ++q) {
+                    const double2 t = row[q];
+                    a[2 * q]     = fma(yr, t.x, a[2 * q]);
+                    a[2 * q + 1] = fma(yr, t.y, a[2 * q + 1]);
+                }
+            }
+            __syncthreads();
+        }
+        if (j < M) gout_[b * M + j] = gj;
+    }
+
+    double* dws = ws.dws + b * M;
+    double* ews = ws.ews + b * M;
+    double* R = tile;                              // reflector i at R[i*MT + c]
+
+    // ---- a3: Householder tridiagonalisation, pivot i = M-1 ... 1, H_i acts on indices 0..i-1
+    for (int i = M - 1; i >= 1; --i) {
+        // warps 0 .. np-1 hold rows <= i and take part in this step; the others are done and
+        // wait at the barrier after the loop (part_barrier counts only the participants)
+        const int np = min(C::NW, (i >> 5) + 1);
+        if (warp >= np) break;
+        const double x = pick<MT>(a, i);           // x_j = A[j][i]; for j == i this is d_i
+        if (j == i) dws[i] = x;
+        if (j == i - 1) red[4] = x;                // alpha
+        double part = (j < i - 1) ? x * x : 0.0;
+        part = warp_sum(part);
+        if (lane == 0) red[warp] = part;
+        part_barrier(np);
+        double sigma = 0.0;
+#pragma unroll
+        for (int w2 = 0; w2 < C::NW; ++w2) sigma += (w2 < np) ? red[w2] : 0.0;
+        const double alpha = red[4];
+        double tau, scal, beta;
+        if (sigma == 0.0) { tau = 0.0; beta = alpha; scal = 0.0; }      // reading G19: H_i = I
+        else {
+            const double nrm2 = fma(alpha, alpha, sigma);
+            const double rinv = rsqrt(nrm2);
+            const double nrm = nrm2 * rinv;
+            beta = -copysign(nrm, alpha);
+            tau = fma(fabs(alpha), rinv, 1.0);                            // (beta - alpha)/beta
+            scal = 1.0 / (alpha - beta);
+        }
+        const double vj = (j < i - 1) ? x * scal : ((j == i - 1) ? 1.0 : 0.0);
+        vs[j] = vj;
+        R[i * MT + j] = vj;
+        if (j == 0) { ews[i - 1] = beta; taus[i] = tau; }
+        part_barrier(np);
+        if (tau != 0.0) {
+            const int qtop = (i - 1) >> 1;
+            double pj = tau * dot_desc<MT>(a, vs, qtop);                  // p = tau A v
+            if (j >= i) pj = 0.0;
+            double pv = warp_sum(pj * vj);
+            if (lane == 0) red[2 + warp] = pv;
+            part_barrier(np);
+            double ptv = 0.0;
+#pragma unroll
+            for (int w2 = 0; w2 < C::NW; ++w2) ptv += (w2 < np) ? red[2 + w2] : 0.0;
+            const double wj = pj - (0.5 * tau * ptv) * vj;                // w = p - (tau/2)(p.v) v
+            vw[j] = make_double2(vj, wj);
+            part_barrier(np);
+            if (j < i) rank2_desc<MT>(a, vw, vj, wj, qtop);              // A -= v w^T + w v^T
+        }
+    }
+    if (j == 0) { dws[0] = a[0]; ews[M - 1] = 0.0; }
+    __syncthreads();
+
+    // ---- explicit Q = H_{M-1} ... H_1: thread r owns column r of Q; no synchronisation needed
+    double (&q)[MT] = a;
+#pragma unroll
+    for (int c = 0; c < MT; ++c) q[c] = (c == j) ? 1.0 : 0.0;
+    for (int i = warp * 32 + 1; i <= M - 1; ++i) {
+        const double tau = taus[i];
+        if (tau == 0.0) continue;
+        const int qtop = (i - 1) >> 1;
+        const double* v = R + i * MT;
+        const double s = tau * dot_desc<MT>(q, v, qtop);
+        axpy_desc<MT>(q, v, s, qtop);
+    }
+    if (j < M) {
+        double* Q = Q_ + b * M * M;
+#pragma unroll
+        for (int c = 0; c < MT; ++c)
+            if (c < M) Q[(size_t)c * M + j] = q[c];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5: V = Q Z by replaying the logged rotations; thread r owns row r of Q in registers.
+// Dynamic shared memory: tile[MT*(MT+1)], cs[2][MT] double2, hdr[swcap] u32, inv[MT] int
+template <int MT> size_t fast_apply_smem(int swcap)
+{
+    return sizeof(double) * ((size_t)MT * (MT + 1) + 4 * MT) + sizeof(uint32_t) * (size_t)swcap + sizeof(int) * MT + 16;
+}
+
+template <int MT>
+__device__ __forceinline__ void apply_sweep(double (&z)[MT], const double2* cs, int lo, int m)
+{
+    // rotations i = m-1 ... lo on columns (i, i+1):  f = z[i+1]; z[i+1] = s z[i] + c f; z[i] = c z[i] - s f
+    switch (m - 1) {
+#define LETKF_ROT(i)                                                          \
+    case i:                                                                   \
+        if constexpr ((i) + 1 < MT) {                                         \
+            const double2 t = cs[i];                                          \
+            const double f = z[(i) + 1];                                      \
+            const double zi = z[i];                                           \
+            z[(i) + 1] = fma(t.y, zi, t.x * f);                               \
+            z[i] = fma(t.x, zi, -(t.y * f));                                  \
+            if ((i) == lo) break;                                             \
+        }
+        LETKF_REP64_DESC(LETKF_ROT)
+#undef LETKF_ROT
+    }
+}
+
+template <int MT>
+__global__ void __launch_bounds__(FastCfg<MT>::NT, (MT == 64) ? 6 : (MT == 48 ? 8 : 16))
+fast_apply(double* __restrict__ V_, Workspace ws, int M)
+{
+    using C = FastCfg<MT>;
+    extern __shared__ __align__(16) double sm[];
+    double*   tile = sm;
+    double2*  cs   = reinterpret_cast<double2*>(sm + MT * (MT + 1) + (MT & 1));
+    uint32_t* hdr  = reinterpret_cast<uint32_t*>(cs + 2 * MT);
+    int*      inv  = reinterpret_cast<int*>(hdr + ws.swcap);
+    const int r = threadIdx.x;
+    const size_t b = blockIdx.x;
+    if (ws.flags[b]) return;                       // finished by generic_apply (slow path)
+    double* V = V_ + b * M * M;
+    const int nsw = ws.nsweeps[b];
+    const double2* rot = ws.rot + b * ws.logcap;
+
+    for (int idx = r; idx < M * M; idx += C::NT) {
+        const int rr = idx / M, c = idx - rr * M;
+        tile[rr * C::LDT + c] = V[idx];
+    }
+    for (int s = r; s < nsw; s += C::NT) hdr[s] = ws.hdr[b * ws.swcap + s];
+    if (r < M) inv[ws.perm[b * M + r]] = r;        // output column of QL-order column c
+    __syncthreads();
+    double z[MT];
+#pragma unroll
+    for (int c = 0; c < MT; ++c) z[c] = (r < M && c < M) ? tile[r * C::LDT + c] : 0.0;
+
+    int pos = 0;
+    if (nsw > 0) {
+        const uint32_t h = hdr[0];
+        const int lo = h & 0xffff, m = h >> 16;
+        if (r >= lo && r < m) cs[r] = rot[pos + (m - 1 - r)];
+    }
+    __syncthreads();
+    for (int s = 0; s < nsw; ++s) {
+        const uint32_t h = hdr[s];
+        const int lo = h & 0xffff, m = h >> 16;
+        pos += m - lo;
+        double2 nxt = make_double2(1.0, 0.0);
+        bool have = false;
+        if (s + 1 < nsw) {
+            const uint32_t h2 = hdr[s + 1];
+            const int lo2 = h2 & 0xffff, m2 = h2 >> 16;
+            have = (r >= lo2 && r < m2);
+            if (have) nxt = rot[pos + (m2 - 1 - r)];
+        }
+        apply_sweep<MT>(z, cs + (s & 1) * MT, lo, m);
+        if (have) cs[((s + 1) & 1) * MT + r] = nxt;
+        __syncthreads();
+    }
+
+    // sorted, row-major V through the tile
+    if (r < M) {
+#pragma unroll
+        for (int c = 0; c < MT; ++c)
+            if (c < M) tile[r * C::LDT + inv[c]] = z[c];
+    }
+    __syncthreads();
+    for (int idx = r; idx < M * M; idx += C::NT) {
+        const int rr = idx / M, c = idx - rr * M;
+        V[idx] = tile[rr * C::LDT + c];
+    }
+}
+
+static inline bool fast_supported(int M) { return M >= 2 && M <= 64; }
+static inline int fast_bucket(int M) { return M <= 16 ? 16 : (M <= 32 ? 32 : (M <= 48 ? 48 : 64)); }
+
+}  // namespace letkf

@@ -199,7 +199,7 @@ generic_apply(double* V_, double* __restrict__ w_, Workspace ws, int M, int* __r
             __syncthreads();
         }
         if (tid == 0) {
-            sort_eigenvalues(dsm, permsm, 1, M);
+            sort_eigenvalues(dsm, 1, permsm, 1, M);
             sh_fail = st.fail;
         }
         __syncthreads();

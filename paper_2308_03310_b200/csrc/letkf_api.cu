@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <string.h>
 #include <vector>
 
 #include "common.cuh"
@@ -123,9 +124,45 @@ static cudaError_t allow_smem(K kernel, size_t bytes)
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
-// One chunk of the EVD: A (n matrices) -> w, V.  ws is sized for >= n matrices.
+static bool g_force_generic = false;     // letkf_set_option("force_generic", 1): tests only
+
+// a1/a2 inputs when the matrix is to be formed from the LETKF observations instead of read
+struct GramArgs { const double* Yb; const double* d; const double* r; int p; double shift; double* gout; };
+
+template <int MT>
+static int fast_tridiag_run(const double* A, double* V, Workspace ws, int M, int n, cudaStream_t st,
+                            const GramArgs* gram)
+{
+    const size_t smem = fast_tridiag_smem<MT>();
+    cudaError_t ce;
+    if (gram) {
+        if ((ce = allow_smem(fast_tridiag_formq<MT, true>, smem)) != cudaSuccess) return (int)ce;
+        KLAUNCH("fast_tridiag_formq<gram>", st,
+                fast_tridiag_formq<MT, true><<<n, FastCfg<MT>::NT, smem, st>>>(
+                    nullptr, V, ws, M, gram->Yb, gram->d, gram->r, gram->p, gram->shift, gram->gout));
+    } else {
+        if ((ce = allow_smem(fast_tridiag_formq<MT, false>, smem)) != cudaSuccess) return (int)ce;
+        KLAUNCH("fast_tridiag_formq", st,
+                fast_tridiag_formq<MT, false><<<n, FastCfg<MT>::NT, smem, st>>>(
+                    A, V, ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr));
+    }
+    return 0;
+}
+
+template <int MT>
+static int fast_apply_run(double* V, Workspace ws, int M, int n, cudaStream_t st)
+{
+    const size_t smem = fast_apply_smem<MT>(ws.swcap);
+    cudaError_t ce;
+    if ((ce = allow_smem(fast_apply<MT>, smem)) != cudaSuccess) return (int)ce;
+    KLAUNCH("fast_apply", st, fast_apply<MT><<<n, FastCfg<MT>::NT, smem, st>>>(V, ws, M));
+    return 0;
+}
+
+// One chunk of the EVD: A (n matrices) -> w, V.  ws is sized for >= n matrices.  With `gram` the
+// matrix is formed from the observations (A is ignored).
 static int syev_chunk_run(const double* A, int M, int n, double* w, double* V, int* info,
-                          Workspace ws, cudaStream_t st)
+                          Workspace ws, cudaStream_t st, const GramArgs* gram = nullptr)
 {
     cudaError_t ce;
     const size_t ql_smem = sizeof(double) * 2 * (size_t)M * QL_TPB;
@@ -133,19 +170,32 @@ static int syev_chunk_run(const double* A, int M, int n, double* w, double* V, i
     const size_t ap_smem = sizeof(double) * (5 * (size_t)M + 2 * 32 * 33);
     const int qblocks = (n + QL_TPB - 1) / QL_TPB;
 
-    if (fast_supported(M)) {
-        int rc = fast_tridiag_launch(A, V, ws, M, n, st);
+    if (fast_supported(M) && !g_force_generic) {
+        int rc = 0;
+        switch (fast_bucket(M)) {
+            case 16: rc = fast_tridiag_run<16>(A, V, ws, M, n, st, gram); break;
+            case 32: rc = fast_tridiag_run<32>(A, V, ws, M, n, st, gram); break;
+            case 48: rc = fast_tridiag_run<48>(A, V, ws, M, n, st, gram); break;
+            default: rc = fast_tridiag_run<64>(A, V, ws, M, n, st, gram); break;
+        }
         if (rc) return rc;
-        ++g_launches;
-        ql_log_kernel<<<qblocks, QL_TPB, ql_smem, st>>>(ws, M, n, w, info);
-        LAUNCH_CHECK();
-        rc = fast_apply_launch(V, ws, M, n, st);
+        KLAUNCH("ql_log_kernel", st, ql_log_kernel<<<qblocks, QL_TPB, ql_smem, st>>>(ws, M, n, w, info));
+        switch (fast_bucket(M)) {
+            case 16: rc = fast_apply_run<16>(V, ws, M, n, st); break;
+            case 32: rc = fast_apply_run<32>(V, ws, M, n, st); break;
+            case 48: rc = fast_apply_run<48>(V, ws, M, n, st); break;
+            default: rc = fast_apply_run<64>(V, ws, M, n, st); break;
+        }
         if (rc) return rc;
-        ++g_launches;
         // finisher for matrices whose rotation log overflowed (normally none: exits at once)
-        generic_apply<<<n, GEN_NT, ap_smem, st>>>(V, w, ws, M, info, /*only_flagged=*/1, /*q_rowmajor=*/1);
-        LAUNCH_CHECK();
+        KLAUNCH("generic_apply(flagged)", st,
+                generic_apply<<<n, GEN_NT, ap_smem, st>>>(V, w, ws, M, info, /*only_flagged=*/1, /*q_rowmajor=*/1));
         return 0;
+    }
+    if (gram) {
+        KLAUNCH("generic_gram", st,
+                generic_gram<<<n, 256, 0, st>>>(gram->Yb, gram->d, gram->r, M, gram->p, gram->shift, V, gram->gout));
+        A = V;
     }
     const size_t td_smem = sizeof(double) * (4 * (size_t)M + GEN_NT / 32);
     KLAUNCH("generic_tridiag_formq", st, generic_tridiag_formq<<<n, GEN_NT, td_smem, st>>>(A, V, ws, M));
@@ -282,14 +332,8 @@ int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv
         double* wbc = wbar ? wbar + (size_t)b0 * M : nullptr;
         int* infoc = info ? info + b0 : nullptr;
 
-        if (fast_supported(M)) {
-            rc = fast_analysis_chunk(Ybc, dc, rc_, Xbc, M, p, nstate, n, shift, Xac, Wc, wbc, infoc,
-                                     ws, Vbuf, lam, gbuf, st, &g_launches);
-            if (rc) return rc;
-            continue;
-        }
-        KLAUNCH("generic_gram", st, generic_gram<<<n, 256, 0, st>>>(Ybc, dc, rc_, M, p, shift, Vbuf, gbuf));
-        rc = syev_chunk_run(Vbuf, M, n, lam, Vbuf, infoc, ws, st);
+        GramArgs ga{Ybc, dc, rc_, p, shift, gbuf};
+        rc = syev_chunk_run(Vbuf, M, n, lam, Vbuf, infoc, ws, st, &ga);
         if (rc) return rc;
         KLAUNCH("generic_epilogue", st,
                 generic_epilogue<<<n, 256, ep_smem, st>>>(Vbuf, lam, gbuf, Xbc, M, nstate, Xac, Wc, wbc));
@@ -312,6 +356,13 @@ int letkf_probe_dfma(double* sink, int blocks, int threads, int iters,
 }
 
 int letkf_last_launch_count(void) { return g_launches; }
+
+int letkf_set_option(const char* name, int value)
+{
+    if (!name) return -1;
+    if (strcmp(name, "force_generic") == 0) { g_force_generic = value != 0; return LETKF_OK; }
+    return -1;
+}
 
 int letkf_profile_enable(int on)
 {

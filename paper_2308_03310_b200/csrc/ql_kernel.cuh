@@ -53,7 +53,7 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
             hdr[nsw++] = (uint32_t)lo | ((uint32_t)m << 16);
             pos += m - lo;
         }
-        if (!overflow) sort_eigenvalues(d, reinterpret_cast<int*>(e), QL_TPB * 2, M);
+        if (!overflow) sort_eigenvalues(d, QL_TPB, reinterpret_cast<int*>(e), QL_TPB * 2, M);
         ws.nsweeps[b] = nsw;
         ws.flags[b] = overflow;
         if (info && !overflow) info[b] = st.fail;

@@ -19,7 +19,7 @@ EXPORTS = (
     "letkf_analysis_batched", "letkf_analysis_workspace_bytes",
     "letkf_probe_dfma", "letkf_last_launch_count",
     "letkf_profile_enable", "letkf_profile_count", "letkf_profile_record", "letkf_profile_rotations",
-    "letkf_status_string", "letkf_version",
+    "letkf_set_option", "letkf_status_string", "letkf_version",
 )
 
 _lib = None
@@ -61,6 +61,8 @@ def load():
     lib.letkf_profile_record.restype = ci
     lib.letkf_profile_rotations.argtypes = []
     lib.letkf_profile_rotations.restype = ctypes.c_longlong
+    lib.letkf_set_option.argtypes = [ctypes.c_char_p, ci]
+    lib.letkf_set_option.restype = ci
     lib.letkf_status_string.argtypes = [ci]
     lib.letkf_status_string.restype = ctypes.c_char_p
     lib.letkf_version.argtypes = []
@@ -195,3 +197,7 @@ def profile_records():
 
 def profile_rotations():
     return load().letkf_profile_rotations()
+
+
+def set_option(name, value):
+    _check(load().letkf_set_option(name.encode(), int(value)), f"letkf_set_option({name})")

@@ -191,3 +191,17 @@ def test_config2_full_size(lk, oracle):
     sel = np.arange(0, A.shape[0], 128)
     wo, _, _, _ = oracle.syev_batched(A[sel])
     parity.assert_evd(A[sel], w[sel], V[sel], wo, "config2 sample vs oracle")
+
+
+@pytest.mark.parametrize("M", [3, 16, 48, 64])
+def test_generic_kernels_at_small_order(lk, oracle, M):
+    """The any-M kernels (normally M > 64 and the overflow finisher) forced onto small M."""
+    A = wl.letkf_shaped(33, M, 49, config_index=70 + M)
+    lk.set_option("force_generic", 1)
+    try:
+        w, V, info = run_gpu(lk, A)
+    finally:
+        lk.set_option("force_generic", 0)
+    assert (info == 0).all()
+    wo, _, _, _ = oracle.syev_batched(A)
+    parity.assert_evd(A, w, V, wo, f"generic M={M}")
