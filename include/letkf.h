@@ -88,7 +88,7 @@ size_t letkf_syev_workspace_bytes(int M, int batch);
  *   d         in  [batch][p]          innovations
  *   rinv_loc  in  [batch][p]          >= 0; 0 marks a padded / ignored observation
  *   Xb        in  [batch][nstate][M]  background ensemble (members, not perturbations)
- *   M, p, nstate, batch               1 <= M <= LETKF_MAX_M, p >= 0, nstate >= 1, batch >= 0
+ *   M, p, nstate, batch               2 <= M <= LETKF_MAX_M (one member has no spread), p >= 0, nstate >= 1, batch >= 0
  *   rho                               multiplicative covariance inflation, > 0
  *   Xa        out [batch][nstate][M]  analysis ensemble; may alias Xb
  *   W         out [batch][M][M] or NULL

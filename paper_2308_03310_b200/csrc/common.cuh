@@ -67,67 +67,97 @@ __device__ __forceinline__ double block_sum(double v, double* red)
 // |e_m| <= 2^-53 (|d_m| + |d_m+1|), at most 30 sweeps per eigenvalue (then st.fail is bumped).
 struct QLState { int l; int iter; int fail; };
 
-__device__ __forceinline__ int ql_next_sweep(QLState& st, double* d, double* e, int stride, int M,
-                                             double2* sink, int sink_cap, int& lo_out, int& m_out)
+#define LETKF_LD(i) d[(size_t)(i) * stride]
+#define LETKF_LE(i) e[(size_t)(i) * stride]
+
+// Advance past converged eigenvalues; returns true with (l = st.l, m) when the block [l, m] needs
+// another sweep, false when everything has converged.
+__device__ __forceinline__ bool ql_find_block(QLState& st, const double* d, const double* e, int stride,
+                                              int M, int& m_out)
 {
-#define LD(i) d[(size_t)(i) * stride]
-#define LE(i) e[(size_t)(i) * stride]
     const double eps = 1.1102230246251565e-16;   // 2^-53
     while (st.l < M) {
         const int l = st.l;
         int m = l;
         for (; m < M - 1; ++m) {
-            const double dd = fabs(LD(m)) + fabs(LD(m + 1));
-            if (fabs(LE(m)) <= eps * dd) break;
+            const double dd = fabs(LETKF_LD(m)) + fabs(LETKF_LD(m + 1));
+            if (fabs(LETKF_LE(m)) <= eps * dd) break;
         }
         if (m == l) { st.l = l + 1; st.iter = 0; continue; }
         if (st.iter >= 30) { st.fail += 1; st.l = l + 1; st.iter = 0; continue; }
-        if (m - l > sink_cap) return -1;
         st.iter += 1;
+        m_out = m;
+        return true;
+    }
+    return false;
+}
 
-        const double el = LE(l);
-        double g = (LD(l + 1) - LD(l)) / (2.0 * el);
-        double r = sqrt(g * g + 1.0);
-        g = LD(m) - LD(l) + el / (g + copysign(r, g));
+// Wilkinson shift for the block [l, m]: returns the starting value of g.
+__device__ __forceinline__ double ql_shift(const double* d, const double* e, int stride, int l, int m)
+{
+    const double el = LETKF_LE(l);
+    double g = (LETKF_LD(l + 1) - LETKF_LD(l)) / (2.0 * el);
+    const double r = sqrt(g * g + 1.0);
+    return LETKF_LD(m) - LETKF_LD(l) + el / (g + copysign(r, g));
+}
+
+// One plane rotation of the sweep (index i).  Returns false if the sweep must stop here
+// (underflow / NaN: the block is split at i+1 and no rotation is produced).
+__device__ __forceinline__ bool ql_rot_step(double* d, double* e, int stride, int i, int m,
+                                            double& s, double& c, double& p, double& g, double2& cs_out)
+{
+    const double ei = LETKF_LE(i);
+    const double f = s * ei;
+    const double b = c * ei;
+    const double r2 = f * f + g * g;
+    if (!(r2 > 0.0)) {
+        LETKF_LE(i + 1) = 0.0;
+        LETKF_LD(i + 1) -= p;
+        LETKF_LE(m) = 0.0;
+        return false;
+    }
+    const double rinv = rsqrt(r2);
+    LETKF_LE(i + 1) = r2 * rinv;
+    s = f * rinv;
+    c = g * rinv;
+    g = LETKF_LD(i + 1) - p;
+    const double r = (LETKF_LD(i) - g) * s + 2.0 * c * b;
+    p = s * r;
+    LETKF_LD(i + 1) = g + p;
+    g = c * r - b;
+    cs_out = make_double2(c, s);
+    return true;
+}
+
+__device__ __forceinline__ void ql_finish_sweep(double* d, double* e, int stride, int l, int m, double p, double g)
+{
+    LETKF_LD(l) -= p;
+    LETKF_LE(l) = g;
+    LETKF_LE(m) = 0.0;
+}
+
+// Single-thread form: produces the next non-empty sweep (see the header comment above).
+__device__ __forceinline__ int ql_next_sweep(QLState& st, double* d, double* e, int stride, int M,
+                                             double2* sink, int sink_cap, int& lo_out, int& m_out)
+{
+    for (;;) {
+        int m;
+        if (!ql_find_block(st, d, e, stride, M, m)) return 0;
+        const int l = st.l;
+        if (m - l > sink_cap) { st.iter -= 1; return -1; }
+        double g = ql_shift(d, e, stride, l, m);
         double s = 1.0, c = 1.0, p = 0.0;
         int i;
         for (i = m - 1; i >= l; --i) {
-            const double ei = LE(i);
-            const double f = s * ei;
-            const double b = c * ei;
-            const double r2 = f * f + g * g;
-            if (!(r2 > 0.0)) {            // underflow (or NaN): split here
-                LE(i + 1) = 0.0;
-                LD(i + 1) -= p;
-                LE(m) = 0.0;
-                break;
-            }
-            const double rinv = rsqrt(r2);
-            r = r2 * rinv;
-            LE(i + 1) = r;
-            s = f * rinv;
-            c = g * rinv;
-            g = LD(i + 1) - p;
-            r = (LD(i) - g) * s + 2.0 * c * b;
-            p = s * r;
-            LD(i + 1) = g + p;
-            g = c * r - b;
-            sink[m - 1 - i] = make_double2(c, s);
+            double2 cs;
+            if (!ql_rot_step(d, e, stride, i, m, s, c, p, g, cs)) break;
+            sink[m - 1 - i] = cs;
         }
         int lo;
-        if (i >= l) {
-            lo = i + 1;
-        } else {
-            LD(l) -= p;
-            LE(l) = g;
-            LE(m) = 0.0;
-            lo = l;
-        }
+        if (i >= l) lo = i + 1;
+        else { ql_finish_sweep(d, e, stride, l, m, p, g); lo = l; }
         if (m - lo > 0) { lo_out = lo; m_out = m; return 1; }
     }
-    return 0;
-#undef LD
-#undef LE
 }
 
 // Ascending insertion sort of d with the permutation that sorts it (stable).
@@ -147,5 +177,8 @@ __device__ __forceinline__ void sort_eigenvalues(double* d, int dstride, int* pe
         perm[(size_t)(j + 1) * pstride] = pk;
     }
 }
+
+#undef LETKF_LD
+#undef LETKF_LE
 
 }  // namespace letkf

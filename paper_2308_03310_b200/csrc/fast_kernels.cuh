@@ -40,59 +40,82 @@ __device__ __forceinline__ double pick(const double (&a)[MT], int i)
     return x;
 }
 
-// acc = sum_{c < 2*(qtop+1)} a[c] * vec[c]          (vec in shared memory, 16-byte aligned)
+// The three BLAS-1 shapes below run over c < 8*(gtop+1) in blocks of 8 columns, entered at block
+// gtop through a jump table and falling through to block 0.  Entry only at block granularity: a
+// load may not be hoisted above its own case label, so with one label per element every LDS sat
+// directly in front of the FMA that needs it (measured: short-scoreboard stall 4.2 per issue,
+// profiles/).  With 8-column blocks the 4-8 LDS.128 of a block are issued back to back.  The
+// callers keep the shared vectors ZERO beyond the active length, so the overhang is harmless.
+#define LETKF_REP8_DESC(X) X(7) X(6) X(5) X(4) X(3) X(2) X(1) X(0)
+
+// acc = sum_{c < 8*(gtop+1)} a[c] * vec[c]          (vec in shared memory, 16-byte aligned)
 template <int MT>
-__device__ __forceinline__ double dot_desc(const double (&a)[MT], const double* vec, int qtop)
+__device__ __forceinline__ double dot_desc(const double (&a)[MT], const double* vec, int gtop)
 {
     double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
     const double2* v2 = reinterpret_cast<const double2*>(vec);
-    switch (qtop) {
-#define LETKF_DOT(q)                                                          \
-    case q:                                                                   \
-        if constexpr (2 * (q) + 1 < MT) {                                     \
-            const double2 t = v2[q];                                          \
-            if ((q) & 1) { s2 = fma(a[2 * (q)], t.x, s2); s3 = fma(a[2 * (q) + 1], t.y, s3); } \
-            else         { s0 = fma(a[2 * (q)], t.x, s0); s1 = fma(a[2 * (q) + 1], t.y, s1); } \
+    switch (gtop) {
+#define LETKF_DOT(g)                                                          \
+    case g:                                                                   \
+        if constexpr (8 * (g) + 7 < MT) {                                     \
+            const double2 t0 = v2[4 * (g)], t1 = v2[4 * (g) + 1];             \
+            const double2 t2 = v2[4 * (g) + 2], t3 = v2[4 * (g) + 3];         \
+            s0 = fma(a[8 * (g)],     t0.x, s0); s1 = fma(a[8 * (g) + 1], t0.y, s1); \
+            s2 = fma(a[8 * (g) + 2], t1.x, s2); s3 = fma(a[8 * (g) + 3], t1.y, s3); \
+            s0 = fma(a[8 * (g) + 4], t2.x, s0); s1 = fma(a[8 * (g) + 5], t2.y, s1); \
+            s2 = fma(a[8 * (g) + 6], t3.x, s2); s3 = fma(a[8 * (g) + 7], t3.y, s3); \
         }
-        LETKF_REP32_DESC(LETKF_DOT)
+        LETKF_REP8_DESC(LETKF_DOT)
 #undef LETKF_DOT
     }
     return (s0 + s1) + (s2 + s3);
 }
 
-// a[c] -= alpha * vec[c]   for c < 2*(qtop+1)
+// a[c] -= alpha * vec[c]   for c < 8*(gtop+1)
 template <int MT>
-__device__ __forceinline__ void axpy_desc(double (&a)[MT], const double* vec, double alpha, int qtop)
+__device__ __forceinline__ void axpy_desc(double (&a)[MT], const double* vec, double alpha, int gtop)
 {
     const double2* v2 = reinterpret_cast<const double2*>(vec);
-    switch (qtop) {
-#define LETKF_AXPY(q)                                                         \
-    case q:                                                                   \
-        if constexpr (2 * (q) + 1 < MT) {                                     \
-            const double2 t = v2[q];                                          \
-            a[2 * (q)]     = fma(-alpha, t.x, a[2 * (q)]);                    \
-            a[2 * (q) + 1] = fma(-alpha, t.y, a[2 * (q) + 1]);                \
+    const double na = -alpha;
+    switch (gtop) {
+#define LETKF_AXPY(g)                                                         \
+    case g:                                                                   \
+        if constexpr (8 * (g) + 7 < MT) {                                     \
+            const double2 t0 = v2[4 * (g)], t1 = v2[4 * (g) + 1];             \
+            const double2 t2 = v2[4 * (g) + 2], t3 = v2[4 * (g) + 3];         \
+            a[8 * (g)]     = fma(na, t0.x, a[8 * (g)]);     a[8 * (g) + 1] = fma(na, t0.y, a[8 * (g) + 1]); \
+            a[8 * (g) + 2] = fma(na, t1.x, a[8 * (g) + 2]); a[8 * (g) + 3] = fma(na, t1.y, a[8 * (g) + 3]); \
+            a[8 * (g) + 4] = fma(na, t2.x, a[8 * (g) + 4]); a[8 * (g) + 5] = fma(na, t2.y, a[8 * (g) + 5]); \
+            a[8 * (g) + 6] = fma(na, t3.x, a[8 * (g) + 6]); a[8 * (g) + 7] = fma(na, t3.y, a[8 * (g) + 7]); \
         }
-        LETKF_REP32_DESC(LETKF_AXPY)
+        LETKF_REP8_DESC(LETKF_AXPY)
 #undef LETKF_AXPY
     }
 }
 
-// a[c] -= vj * w[c] + wj * v[c]   for c < 2*(qtop+1);  vw[c] = (v_c, w_c)
+// a[c] -= vj * p[c] + wj * v[c]   for c < 8*(gtop+1);  vp[c] = (v_c, p_c)
 template <int MT>
-__device__ __forceinline__ void rank2_desc(double (&a)[MT], const double2* vw, double vj, double wj, int qtop)
+__device__ __forceinline__ void rank2_desc(double (&a)[MT], const double2* vp, double vj, double wj, int gtop)
 {
-    switch (qtop) {
-#define LETKF_R2(q)                                                           \
-    case q:                                                                   \
-        if constexpr (2 * (q) + 1 < MT) {                                     \
-            const double2 t0 = vw[2 * (q)];                                   \
-            const double2 t1 = vw[2 * (q) + 1];                               \
-            a[2 * (q)]     = fma(-vj, t0.y, fma(-wj, t0.x, a[2 * (q)]));      \
-            a[2 * (q) + 1] = fma(-vj, t1.y, fma(-wj, t1.x, a[2 * (q) + 1]));  \
+    const double nv = -vj, nw = -wj;
+    switch (gtop) {
+#define LETKF_R2E(c) a[c] = fma(nv, vp_##c.y, fma(nw, vp_##c.x, a[c]));
+#define LETKF_R2(g)                                                           \
+    case g:                                                                   \
+        if constexpr (8 * (g) + 7 < MT) {                                     \
+            _Pragma("unroll")                                                 \
+            for (int h = 0; h < 2; ++h) {                                     \
+                const double2 u0 = vp[8 * (g) + 4 * h],     u1 = vp[8 * (g) + 4 * h + 1]; \
+                const double2 u2 = vp[8 * (g) + 4 * h + 2], u3 = vp[8 * (g) + 4 * h + 3]; \
+                a[8 * (g) + 4 * h]     = fma(nv, u0.y, fma(nw, u0.x, a[8 * (g) + 4 * h]));     \
+                a[8 * (g) + 4 * h + 1] = fma(nv, u1.y, fma(nw, u1.x, a[8 * (g) + 4 * h + 1])); \
+                a[8 * (g) + 4 * h + 2] = fma(nv, u2.y, fma(nw, u2.x, a[8 * (g) + 4 * h + 2])); \
+                a[8 * (g) + 4 * h + 3] = fma(nv, u3.y, fma(nw, u3.x, a[8 * (g) + 4 * h + 3])); \
+            }                                                                 \
         }
-        LETKF_REP32_DESC(LETKF_R2)
+        LETKF_REP8_DESC(LETKF_R2)
 #undef LETKF_R2
+#undef LETKF_R2E
     }
 }
 
@@ -137,7 +160,7 @@ template <int MT> constexpr size_t fast_tridiag_smem()
 // a3 + explicit Q for one matrix per CTA.  gram == true: the matrix is not read from A but formed
 // from the LETKF inputs (a1, a2: Eq.17 and the right factor of Eq.14) straight into the registers.
 template <int MT, bool GRAM>
-__global__ void __launch_bounds__(FastCfg<MT>::NT, (MT == 64) ? 6 : (MT == 48 ? 8 : 16))
+__global__ void __launch_bounds__(FastCfg<MT>::NT, (MT == 64) ? 4 : (MT == 48 ? 7 : 16))
 fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Workspace ws, int M,
                    const double* __restrict__ Yb_, const double* __restrict__ d_,
                    const double* __restrict__ r_, int p, double shift, double* __restrict__ gout_)
@@ -233,24 +256,27 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
             scal = 1.0 / (alpha - beta);
         }
         const double vj = (j < i - 1) ? x * scal : ((j == i - 1) ? 1.0 : 0.0);
-        vs[j] = vj;
-        R[i * MT + j] = vj;
+        if (j < MT) {                                   // NT may exceed MT (MT = 16, 48)
+            vs[j] = vj;
+            R[i * MT + j] = vj;
+        }
         if (j == 0) { ews[i - 1] = beta; taus[i] = tau; }
         part_barrier(np);
         if (tau != 0.0) {
-            const int qtop = (i - 1) >> 1;
-            double pj = tau * dot_desc<MT>(a, vs, qtop);                  // p = tau A v
+            const int gtop = (i - 1) >> 3;
+            double pj = tau * dot_desc<MT>(a, vs, gtop);                  // p = tau A v
             if (j >= i) pj = 0.0;
             double pv = warp_sum(pj * vj);
             if (lane == 0) red[2 + warp] = pv;
+            if (j < MT) vw[j] = make_double2(vj, pj);                     // (v_c, p_c) broadcast pairs
             part_barrier(np);
             double ptv = 0.0;
 #pragma unroll
             for (int w2 = 0; w2 < C::NW; ++w2) ptv += (w2 < np) ? red[2 + w2] : 0.0;
-            const double wj = pj - (0.5 * tau * ptv) * vj;                // w = p - (tau/2)(p.v) v
-            vw[j] = make_double2(vj, wj);
-            part_barrier(np);
-            if (j < i) rank2_desc<MT>(a, vw, vj, wj, qtop);              // A -= v w^T + w v^T
+            // A -= v w^T + w v^T with w = p - K v, K = (tau/2) p.v, written on the broadcast
+            // pairs (v_c, p_c):  a_jc -= v_j p_c + (p_j - 2 K v_j) v_c   (one barrier fewer)
+            const double wj = pj - (tau * ptv) * vj;
+            if (j < i) rank2_desc<MT>(a, vw, vj, wj, gtop);
         }
     }
     if (j == 0) { dws[0] = a[0]; ews[M - 1] = 0.0; }
@@ -263,10 +289,10 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
     for (int i = warp * 32 + 1; i <= M - 1; ++i) {
         const double tau = taus[i];
         if (tau == 0.0) continue;
-        const int qtop = (i - 1) >> 1;
+        const int gtop = (i - 1) >> 3;
         const double* v = R + i * MT;
-        const double s = tau * dot_desc<MT>(q, v, qtop);
-        axpy_desc<MT>(q, v, s, qtop);
+        const double s = tau * dot_desc<MT>(q, v, gtop);
+        axpy_desc<MT>(q, v, s, gtop);
     }
     if (j < M) {
         double* Q = Q_ + b * M * M;
@@ -284,23 +310,35 @@ template <int MT> size_t fast_apply_smem(int swcap)
     return sizeof(double) * ((size_t)MT * (MT + 1) + 4 * MT) + sizeof(uint32_t) * (size_t)swcap + sizeof(int) * MT + 16;
 }
 
+// Rotations i = m-1 ... lo on columns (i, i+1):  f = z[i+1]; z[i+1] = s z[i] + c f; z[i] = c z[i] - s f.
+// Blocks of 4 rotations, entered at the block of m-1 and left after the block of lo; cs[] holds
+// the identity (1, 0) outside [lo, m), so the overhang at both ends changes nothing.  The only
+// dependent chain from one rotation to the next is the single FMA that produces z[i].
 template <int MT>
 __device__ __forceinline__ void apply_sweep(double (&z)[MT], const double2* cs, int lo, int m)
 {
-    // rotations i = m-1 ... lo on columns (i, i+1):  f = z[i+1]; z[i+1] = s z[i] + c f; z[i] = c z[i] - s f
-    switch (m - 1) {
-#define LETKF_ROT(i)                                                          \
-    case i:                                                                   \
+    switch ((m - 1) >> 2) {
+#define LETKF_ROT1(i, t)                                                      \
         if constexpr ((i) + 1 < MT) {                                         \
-            const double2 t = cs[i];                                          \
             const double f = z[(i) + 1];                                      \
             const double zi = z[i];                                           \
             z[(i) + 1] = fma(t.y, zi, t.x * f);                               \
-            z[i] = fma(t.x, zi, -(t.y * f));                                  \
-            if ((i) == lo) break;                                             \
+            z[i] = fma(-t.y, f, t.x * zi);                                    \
         }
-        LETKF_REP64_DESC(LETKF_ROT)
+#define LETKF_ROT(g)                                                          \
+    case g:                                                                   \
+        if constexpr (4 * (g) + 3 < MT) {                                     \
+            const double2 t3 = cs[4 * (g) + 3], t2 = cs[4 * (g) + 2];         \
+            const double2 t1 = cs[4 * (g) + 1], t0 = cs[4 * (g)];             \
+            LETKF_ROT1(4 * (g) + 3, t3) LETKF_ROT1(4 * (g) + 2, t2)           \
+            LETKF_ROT1(4 * (g) + 1, t1) LETKF_ROT1(4 * (g), t0)               \
+            if (4 * (g) <= lo) break;                                         \
+        }
+        LETKF_ROT(15) LETKF_ROT(14) LETKF_ROT(13) LETKF_ROT(12) LETKF_ROT(11) LETKF_ROT(10) LETKF_ROT(9)
+        LETKF_ROT(8) LETKF_ROT(7) LETKF_ROT(6) LETKF_ROT(5) LETKF_ROT(4) LETKF_ROT(3) LETKF_ROT(2)
+        LETKF_ROT(1) LETKF_ROT(0)
 #undef LETKF_ROT
+#undef LETKF_ROT1
     }
 }
 
@@ -336,7 +374,7 @@ fast_apply(double* __restrict__ V_, Workspace ws, int M)
     if (nsw > 0) {
         const uint32_t h = hdr[0];
         const int lo = h & 0xffff, m = h >> 16;
-        if (r >= lo && r < m) cs[r] = rot[pos + (m - 1 - r)];
+        if (r < MT) cs[r] = (r >= lo && r < m) ? rot[pos + (m - 1 - r)] : make_double2(1.0, 0.0);
     }
     __syncthreads();
     for (int s = 0; s < nsw; ++s) {
@@ -352,7 +390,7 @@ fast_apply(double* __restrict__ V_, Workspace ws, int M)
             if (have) nxt = rot[pos + (m2 - 1 - r)];
         }
         apply_sweep<MT>(z, cs + (s & 1) * MT, lo, m);
-        if (have) cs[((s + 1) & 1) * MT + r] = nxt;
+        if (r < MT) cs[((s + 1) & 1) * MT + r] = nxt;       // identity outside [lo2, m2)
         __syncthreads();
     }
 

@@ -287,7 +287,7 @@ int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv
                            void* work, size_t work_bytes, void* stream)
 {
     g_launches = 0;
-    if (M < 1 || M > LETKF_MAX_M) return -5;
+    if (M < 2 || M > LETKF_MAX_M) return -5;   // M = 1 has no ensemble spread: Eq.15 is 0/0
     if (p < 0) return -6;
     if (nstate < 1) return -7;
     if (batch < 0) return -8;

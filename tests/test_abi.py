@@ -61,6 +61,7 @@ def test_argument_validation_needs_no_device(lib):
                         k.get("ns", 2), k.get("batch", 4), k.get("rho", 1.1), k.get("Xa", fake),
                         null, null, null, null, 0, null]
     assert ana(*args(M=0)) == -5
+    assert ana(*args(M=1)) == -5
     assert ana(*args(p=-1)) == -6
     assert ana(*args(ns=0)) == -7
     assert ana(*args(batch=-2)) == -8

@@ -37,7 +37,7 @@ def run_oracle(oracle, inp, rho=None):
 
 @pytest.mark.parametrize("M,p,ns,batch", [(64, 98, 9, 200), (64, 3, 9, 65), (64, 48, 9, 64), (48, 49, 9, 100),
                                           (32, 49, 9, 100), (16, 5, 3, 77), (6, 4, 2, 5), (2, 7, 1, 9),
-                                          (1, 3, 2, 4), (33, 20, 4, 21), (96, 98, 9, 6), (130, 98, 9, 3)])
+                                          (33, 20, 4, 21), (96, 98, 9, 6), (130, 98, 9, 3)])
 def test_analysis_vs_oracle(lk, oracle, M, p, ns, batch):
     """BASELINE config 4 shape (reduced batch), the paper's dense (p=3) and sparse (p=48) shapes,
     and ragged / odd sizes."""
