@@ -52,7 +52,7 @@ __device__ __forceinline__ double pick(const double (&a)[MT], int i)
 template <int MT>
 __device__ __forceinline__ double dot_desc(const double (&a)[MT], const double* vec, int gtop)
 {
-    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0, s4 = 0.0, s5 = 0.0, s6 = 0.0, s7 = 0.0;
     const double2* v2 = reinterpret_cast<const double2*>(vec);
     switch (gtop) {
 #define LETKF_DOT(g)                                                          \
@@ -62,13 +62,13 @@ __device__ __forceinline__ double dot_desc(const double (&a)[MT], const double* 
             const double2 t2 = v2[4 * (g) + 2], t3 = v2[4 * (g) + 3];         \
             s0 = fma(a[8 * (g)],     t0.x, s0); s1 = fma(a[8 * (g) + 1], t0.y, s1); \
             s2 = fma(a[8 * (g) + 2], t1.x, s2); s3 = fma(a[8 * (g) + 3], t1.y, s3); \
-            s0 = fma(a[8 * (g) + 4], t2.x, s0); s1 = fma(a[8 * (g) + 5], t2.y, s1); \
-            s2 = fma(a[8 * (g) + 6], t3.x, s2); s3 = fma(a[8 * (g) + 7], t3.y, s3); \
+            s4 = fma(a[8 * (g) + 4], t2.x, s4); s5 = fma(a[8 * (g) + 5], t2.y, s5); \
+            s6 = fma(a[8 * (g) + 6], t3.x, s6); s7 = fma(a[8 * (g) + 7], t3.y, s7); \
         }
         LETKF_REP8_DESC(LETKF_DOT)
 #undef LETKF_DOT
     }
-    return (s0 + s1) + (s2 + s3);
+    return ((s0 + s1) + (s2 + s3)) + ((s4 + s5) + (s6 + s7));
 }
 
 // a[c] -= alpha * vec[c]   for c < 8*(gtop+1)
@@ -148,6 +148,31 @@ __device__ __forceinline__ void part_barrier(int nwarps)
     else asm volatile("bar.sync 1, %0;" ::"r"(nwarps * 32) : "memory");
 }
 
+// Coalesced copy of a row-major M x M matrix into the padded shared tile; 8 loads in flight per
+// thread (a plain load->store loop exposed the full DRAM latency 64 times, profiles/).
+template <int MT>
+__device__ __forceinline__ void load_tile(double* tile, const double* __restrict__ G, int M)
+{
+    using C = FastCfg<MT>;
+    const int n = M * M;
+    for (int base = threadIdx.x; base < n; base += 8 * C::NT) {
+        double tmp[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int idx = base + u * C::NT;
+            tmp[u] = (idx < n) ? G[idx] : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int idx = base + u * C::NT;
+            if (idx < n) {
+                const int r = idx / M, c = idx - r * M;
+                tile[r * C::LDT + c] = tmp[u];
+            }
+        }
+    }
+}
+
 // Dynamic shared memory of fast_tridiag_formq<MT>:
 //   tile[MT*(MT+1)]  staging of A (padded), later the reflectors R[i][c] (stride MT)
 //   vs[MT]  v;  vw[MT] (v,w) pairs;  taus[MT];  red[8]
@@ -177,11 +202,7 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
     double a[MT];
 
     if constexpr (!GRAM) {
-        const double* A = A_ + b * M * M;
-        for (int idx = j; idx < M * M; idx += C::NT) {
-            const int r = idx / M, c = idx - r * M;
-            tile[r * C::LDT + c] = A[idx];
-        }
+        load_tile<MT>(tile, A_ + b * M * M, M);
         __syncthreads();
 #pragma unroll
         for (int c = 0; c < MT; ++c) {
@@ -280,9 +301,12 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
         }
     }
     if (j == 0) { dws[0] = a[0]; ews[M - 1] = 0.0; }
-    __syncthreads();
+    __syncwarp();
 
-    // ---- explicit Q = H_{M-1} ... H_1: thread r owns column r of Q; no synchronisation needed
+    // ---- explicit Q = H_{M-1} ... H_1: thread r owns column r of Q; no synchronisation needed.
+    // Column r only needs H_i with i > r, and a warp leaves the loop above exactly when all
+    // reflectors with i >= its first row have been stored (barrier 2 of those steps included it),
+    // so the upper warps form their columns of Q while warp 0 is still reducing the last 32 rows.
     double (&q)[MT] = a;
 #pragma unroll
     for (int c = 0; c < MT; ++c) q[c] = (c == j) ? 1.0 : 0.0;
@@ -359,10 +383,7 @@ fast_apply(double* __restrict__ V_, Workspace ws, int M)
     const int nsw = ws.nsweeps[b];
     const double2* rot = ws.rot + b * ws.logcap;
 
-    for (int idx = r; idx < M * M; idx += C::NT) {
-        const int rr = idx / M, c = idx - rr * M;
-        tile[rr * C::LDT + c] = V[idx];
-    }
+    load_tile<MT>(tile, V, M);
     for (int s = r; s < nsw; s += C::NT) hdr[s] = ws.hdr[b * ws.swcap + s];
     if (r < M) inv[ws.perm[b * M + r]] = r;        // output column of QL-order column c
     __syncthreads();

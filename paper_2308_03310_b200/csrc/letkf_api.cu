@@ -120,6 +120,7 @@ static inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_
 template <typename K>
 static cudaError_t allow_smem(K kernel, size_t bytes)
 {
+    cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (bytes <= 48 * 1024) return cudaSuccess;
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
