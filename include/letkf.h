@@ -117,7 +117,12 @@ int letkf_probe_dfma(double* sink, int blocks, int threads, int iters,
  * Profiling aid for bench.py (off by default; adds one CUDA event pair per kernel launch).
  * With profiling on, each compute call records events around every kernel it enqueues, on the
  * stream the kernel runs on, and counts the plane rotations its QL step generated.
- *   letkf_profile_enable(on)         switch; returns the previous setting
+ *   letkf_profile_enable(on)         switch; returns the previous setting.  on = 1: the call runs
+ *                                    as ONE chunk on the caller's stream, so each record is a kernel
+ *                                    timed alone; on = 2: the sub-chunk pipeline is kept and each
+ *                                    record is taken on the private stream the kernel runs on (a
+ *                                    timeline: records of different streams overlap)
+ *   letkf_profile_record_start(i, &ms)   SYNCHRONISES; start of record i relative to record 0
  *   letkf_profile_count()            records held from the last compute call of this thread
  *   letkf_profile_record(i, &name, &ms)  SYNCHRONISES on record i's events; name is a static string
  *   letkf_profile_rotations()        SYNCHRONISES; total rotations generated by the last call
@@ -125,6 +130,7 @@ int letkf_probe_dfma(double* sink, int blocks, int threads, int iters,
 int letkf_profile_enable(int on);
 int letkf_profile_count(void);
 int letkf_profile_record(int idx, const char** name, float* ms);
+int letkf_profile_record_start(int idx, float* ms_from_first);
 long long letkf_profile_rotations(void);
 
 /* Number of kernels the last compute call on this host thread enqueued (bench.py's
@@ -132,7 +138,8 @@ long long letkf_profile_rotations(void);
 int letkf_last_launch_count(void);
 
 /* Test/diagnostic options.  "force_generic" = 1 routes every M through the any-M kernels
- * (otherwise only M > 64 and overflowed matrices use them).  Returns 0, or -1 for an unknown name. */
+ * (otherwise only M > 64 and overflowed matrices use them); "pipeline" = 0 runs every pass as one
+ * chunk on the caller's stream instead of the sub-chunk pipeline over private streams (default 1).  Returns 0, or -1 for an unknown name. */
 int letkf_set_option(const char* name, int value);
 
 const char* letkf_status_string(int status);

@@ -121,9 +121,9 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
 // the classic in-kernel QL instead: thread 0 generates one sweep into shared memory, all threads
 // apply it.  only_flagged: process nothing but flagged matrices (finisher after the fast path;
 // there V already holds Q row-major, `q_rowmajor`).
-__global__ void __launch_bounds__(GEN_NT)
-generic_apply(double* V_, double* __restrict__ w_, Workspace ws, int M, int* __restrict__ info,
-              int only_flagged, int q_rowmajor)
+__device__ __forceinline__ void
+generic_apply_one(double* V_, double* __restrict__ w_, const Workspace& ws, int M, int* __restrict__ info,
+                  int only_flagged, int q_rowmajor, size_t b)
 {
     extern __shared__ double sm[];
     double*  dsm    = sm;                                         // [M]
@@ -135,7 +135,6 @@ generic_apply(double* V_, double* __restrict__ w_, Workspace ws, int M, int* __r
     __shared__ int sh_rc, sh_lo, sh_m, sh_fail;
 
     const int tid = threadIdx.x;
-    const size_t b = blockIdx.x;
     const int flagged = ws.flags[b];
     if (only_flagged && !flagged) return;
     double* B = V_ + b * M * M;
@@ -254,6 +253,18 @@ generic_apply(double* V_, double* __restrict__ w_, Workspace ws, int M, int* __r
             }
             __syncthreads();
         }
+}
+
+// Grid-stride over the n matrices of the pass (gridDim.x = n for the any-M path; a small
+// persistent grid for the flagged-only finisher, which normally finds nothing to do).
+__global__ void __launch_bounds__(GEN_NT)
+generic_apply(double* V_, double* __restrict__ w_, Workspace ws, int M, int n, int* __restrict__ info,
+              int only_flagged, int q_rowmajor)
+{
+    for (size_t b = blockIdx.x; b < (size_t)n; b += gridDim.x) {
+        generic_apply_one(V_, w_, ws, M, info, only_flagged, q_rowmajor, b);
+        __syncthreads();
+    }
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -21,6 +21,7 @@ static thread_local int g_launches = 0;
 struct ProfRec { const char* name; cudaEvent_t e0, e1; };
 struct Prof {
     bool on = false;
+    bool keep_pipeline = false;   // letkf_profile_enable(2): time the kernels where they run
     std::vector<ProfRec> recs;
     std::vector<cudaEvent_t> pool;
     size_t used = 0;
@@ -79,11 +80,15 @@ static size_t syev_bytes_per_matrix(int M)
     return s;
 }
 
-// matrices processed per pass: bounds the workspace to about 1 GiB
+// matrices processed per pass.  The workspace (dominated by the rotation log, 16*log_capacity(M)
+// bytes per matrix) is sized for the whole batch up to WORK_CAP: ql_log_kernel costs the serial
+// latency of one matrix's QL iteration whatever the batch (profiles/r01a), so passes are kept as
+// few as the 180 GB of HBM allow.
+static const size_t WORK_CAP = (size_t)8 << 30;
 static int syev_chunk(int M, int batch)
 {
     const size_t per = syev_bytes_per_matrix(M);
-    size_t c = ((size_t)1 << 30) / per;
+    size_t c = WORK_CAP / per;
     if (c < 1024) c = 1024;
     if (c > (size_t)batch) c = (size_t)batch;
     if (c < 1) c = 1;
@@ -106,6 +111,20 @@ static size_t carve(Workspace& ws, void* base, int M, int chunk)
     ws.hdr     = reinterpret_cast<uint32_t*>(take(sizeof(uint32_t) * (size_t)ws.swcap * chunk));
     ws.rot     = reinterpret_cast<double2*>(take(sizeof(double2) * (size_t)ws.logcap * chunk));
     return off;
+}
+
+// the records of matrices b0 ... of a carved workspace
+static Workspace ws_slice(const Workspace& w, int M, int b0)
+{
+    Workspace s = w;
+    s.dws += (size_t)b0 * M;
+    s.ews += (size_t)b0 * M;
+    s.perm += (size_t)b0 * M;
+    s.nsweeps += b0;
+    s.flags += b0;
+    s.hdr += (size_t)b0 * w.swcap;
+    s.rot += (size_t)b0 * w.logcap;
+    return s;
 }
 
 static inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
@@ -160,27 +179,46 @@ static int fast_apply_run(double* V, Workspace ws, int M, int n, cudaStream_t st
     return 0;
 }
 
-// One chunk of the EVD: A (n matrices) -> w, V.  ws is sized for >= n matrices.  With `gram` the
-// matrix is formed from the observations (A is ignored).
-static int syev_chunk_run(const double* A, int M, int n, double* w, double* V, int* info,
-                          Workspace ws, cudaStream_t st, const GramArgs* gram = nullptr)
+// ---------------------------------------------------------------------------------------------
+// The EVD of n matrices as three stages.  stage_T: a3 (+ a1, a2 with `gram`) and the explicit Q;
+// stage_QL: a4, the logged QL iteration; stage_AP: a5, replay of the log on Q, eigenvalue sort.
+// ws is the workspace slice of these n matrices.
+static int stage_T(const double* A, int M, int n, double* V, Workspace ws, cudaStream_t st,
+                   const GramArgs* gram)
+{
+    if (fast_supported(M) && !g_force_generic) {
+        switch (fast_bucket(M)) {
+            case 16: return fast_tridiag_run<16>(A, V, ws, M, n, st, gram);
+            case 32: return fast_tridiag_run<32>(A, V, ws, M, n, st, gram);
+            case 48: return fast_tridiag_run<48>(A, V, ws, M, n, st, gram);
+            default: return fast_tridiag_run<64>(A, V, ws, M, n, st, gram);
+        }
+    }
+    if (gram) {
+        KLAUNCH("generic_gram", st,
+                generic_gram<<<n, 256, 0, st>>>(gram->Yb, gram->d, gram->r, M, gram->p, gram->shift, V, gram->gout));
+        A = V;
+    }
+    const size_t td_smem = sizeof(double) * (4 * (size_t)M + GEN_NT / 32);
+    KLAUNCH("generic_tridiag_formq", st, generic_tridiag_formq<<<n, GEN_NT, td_smem, st>>>(A, V, ws, M));
+    return 0;
+}
+
+static int stage_QL(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st)
 {
     cudaError_t ce;
     const size_t ql_smem = sizeof(double) * 2 * (size_t)M * QL_TPB;
     if ((ce = allow_smem(ql_log_kernel, ql_smem)) != cudaSuccess) return (int)ce;
-    const size_t ap_smem = sizeof(double) * (5 * (size_t)M + 2 * 32 * 33);
     const int qblocks = (n + QL_TPB - 1) / QL_TPB;
+    KLAUNCH("ql_log_kernel", st, ql_log_kernel<<<qblocks, QL_TPB, ql_smem, st>>>(ws, M, n, w, info));
+    return 0;
+}
 
+static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws, cudaStream_t st)
+{
+    const size_t ap_smem = sizeof(double) * (5 * (size_t)M + 2 * 32 * 33);
     if (fast_supported(M) && !g_force_generic) {
         int rc = 0;
-        switch (fast_bucket(M)) {
-            case 16: rc = fast_tridiag_run<16>(A, V, ws, M, n, st, gram); break;
-            case 32: rc = fast_tridiag_run<32>(A, V, ws, M, n, st, gram); break;
-            case 48: rc = fast_tridiag_run<48>(A, V, ws, M, n, st, gram); break;
-            default: rc = fast_tridiag_run<64>(A, V, ws, M, n, st, gram); break;
-        }
-        if (rc) return rc;
-        KLAUNCH("ql_log_kernel", st, ql_log_kernel<<<qblocks, QL_TPB, ql_smem, st>>>(ws, M, n, w, info));
         switch (fast_bucket(M)) {
             case 16: rc = fast_apply_run<16>(V, ws, M, n, st); break;
             case 32: rc = fast_apply_run<32>(V, ws, M, n, st); break;
@@ -190,18 +228,107 @@ static int syev_chunk_run(const double* A, int M, int n, double* w, double* V, i
         if (rc) return rc;
         // finisher for matrices whose rotation log overflowed (normally none: exits at once)
         KLAUNCH("generic_apply(flagged)", st,
-                generic_apply<<<n, GEN_NT, ap_smem, st>>>(V, w, ws, M, info, /*only_flagged=*/1, /*q_rowmajor=*/1));
+                generic_apply<<<(n < 296 ? n : 296), GEN_NT, ap_smem, st>>>(V, w, ws, M, n, info, /*only_flagged=*/1, /*q_rowmajor=*/1));
         return 0;
     }
-    if (gram) {
-        KLAUNCH("generic_gram", st,
-                generic_gram<<<n, 256, 0, st>>>(gram->Yb, gram->d, gram->r, M, gram->p, gram->shift, V, gram->gout));
-        A = V;
+    KLAUNCH("generic_apply", st, generic_apply<<<n, GEN_NT, ap_smem, st>>>(V, w, ws, M, n, info, 0, 0));
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Private streams of the calling host thread.  A pass over n matrices is cut into sub-chunks that
+// flow through three stages on separate streams: ql_log_kernel is bound by the serial latency of
+// one matrix's iteration and keeps one warp per SM sub-partition busy at most, so it runs beside
+// the ALU-bound stage_T / stage_AP kernels of the neighbouring sub-chunks (highest priority, so a
+// ready QL block takes the first free slot).  stage_T outranks stage_AP: every QL kernel should
+// start as early as possible, the apply kernels fill the machine behind them.  Everything is forked from and joined back into the
+// caller's stream with events: the caller sees plain stream order.
+struct Pipe {
+    int dev = -1;
+    cudaStream_t sT[2] = {nullptr, nullptr}, sA[2] = {nullptr, nullptr};
+    cudaStream_t sQ[8] = {};          // one per sub-chunk: all QL kernels of a pass run side by side
+    std::vector<cudaEvent_t> ev;
+    size_t used = 0;
+    int init()
+    {
+        int d = 0;
+        cudaError_t ce = cudaGetDevice(&d);
+        if (ce != cudaSuccess) return (int)ce;
+        if (d == dev) return 0;
+        int least = 0, greatest = 0;
+        cudaDeviceGetStreamPriorityRange(&least, &greatest);
+        const int mid = (greatest < least) ? greatest + 1 : greatest;
+        for (int k = 0; k < 2; ++k) {
+            if ((ce = cudaStreamCreateWithPriority(&sT[k], cudaStreamNonBlocking, mid)) != cudaSuccess) return (int)ce;
+            if ((ce = cudaStreamCreateWithPriority(&sA[k], cudaStreamNonBlocking, least)) != cudaSuccess) return (int)ce;
+        }
+        for (int k = 0; k < 8; ++k)
+            if ((ce = cudaStreamCreateWithPriority(&sQ[k], cudaStreamNonBlocking, greatest)) != cudaSuccess) return (int)ce;
+        ev.clear();
+        used = 0;
+        dev = d;
+        return 0;
     }
-    const size_t td_smem = sizeof(double) * (4 * (size_t)M + GEN_NT / 32);
-    KLAUNCH("generic_tridiag_formq", st, generic_tridiag_formq<<<n, GEN_NT, td_smem, st>>>(A, V, ws, M));
-    KLAUNCH("ql_log_kernel", st, ql_log_kernel<<<qblocks, QL_TPB, ql_smem, st>>>(ws, M, n, w, info));
-    KLAUNCH("generic_apply", st, generic_apply<<<n, GEN_NT, ap_smem, st>>>(V, w, ws, M, info, 0, 0));
+    cudaEvent_t event()
+    {
+        if (used == ev.size()) {
+            cudaEvent_t e;
+            cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+            ev.push_back(e);
+        }
+        return ev[used++];
+    }
+    // `to` waits for everything enqueued on `from` so far
+    void link(cudaStream_t from, cudaStream_t to)
+    {
+        cudaEvent_t e = event();
+        cudaEventRecord(e, from);
+        cudaStreamWaitEvent(to, e, 0);
+    }
+};
+static thread_local Pipe g_pipe;
+
+static int g_pipeline = 1;               // letkf_set_option("pipeline", 0): one stream, one chunk
+static const int PIPE_MIN_SUB = 1024;    // smallest sub-chunk worth a launch of its own
+static const int PIPE_MAX_SUB = 8;       // = number of QL streams
+
+// One pass: n matrices whose workspace records are ws[0..n).  stageT(b0, nk, stream) enqueues the
+// first stage of matrices [b0, b0+nk); post(b0, nk, stream) whatever follows stage_AP (the
+// analysis epilogue) or nothing.
+template <class FT, class FP>
+static int run_pass(int M, int n, double* w, double* V, int* info, const Workspace& ws,
+                    cudaStream_t st, FT stageT, FP post)
+{
+    int nsub = (g_pipeline && (!g_prof.on || g_prof.keep_pipeline)) ? n / PIPE_MIN_SUB : 1;
+    if (nsub > PIPE_MAX_SUB) nsub = PIPE_MAX_SUB;
+    if (nsub < 2) {
+        int rc = stageT(0, n, st);
+        if (rc) return rc;
+        if ((rc = stage_QL(M, n, w, info, ws, st))) return rc;
+        if ((rc = stage_AP(M, n, w, V, info, ws, st))) return rc;
+        return post(0, n, st);
+    }
+    Pipe& P = g_pipe;
+    int rc = P.init();
+    if (rc) return rc;
+    P.used = 0;
+    for (int k = 0; k < 2; ++k) { P.link(st, P.sT[k]); P.link(st, P.sA[k]); }
+    for (int k = 0; k < nsub; ++k) P.link(st, P.sQ[k]);
+    const int per = (n + nsub - 1) / nsub;
+    for (int k = 0, b0 = 0; b0 < n; ++k, b0 += per) {
+        const int nk = (n - b0 < per) ? n - b0 : per;
+        const int s = k & 1;
+        const Workspace wk = ws_slice(ws, M, b0);
+        int* infok = info ? info + b0 : nullptr;
+        if ((rc = stageT(b0, nk, P.sT[s]))) return rc;
+        P.link(P.sT[s], P.sQ[k]);
+        if ((rc = stage_QL(M, nk, w + (size_t)b0 * M, infok, wk, P.sQ[k]))) return rc;
+        P.link(P.sQ[k], P.sA[s]);
+        if ((rc = stage_AP(M, nk, w + (size_t)b0 * M, V + (size_t)b0 * M * M, infok, wk, P.sA[s]))) return rc;
+        if ((rc = post(b0, nk, P.sA[s]))) return rc;
+    }
+    for (int k = 0; k < 2; ++k) { P.link(P.sT[k], st); P.link(P.sA[k], st); }
+    for (int k = 0; k < nsub; ++k) P.link(P.sQ[k], st);
     return 0;
 }
 
@@ -262,8 +389,13 @@ int letkf_syev_batched(const double* A, int M, int batch, double* w, double* V, 
 
     for (int b0 = 0; b0 < batch; b0 += chunk) {
         const int n = (batch - b0 < chunk) ? batch - b0 : chunk;
-        const size_t mo = (size_t)b0 * M * M;
-        rc = syev_chunk_run(A + mo, M, n, w + (size_t)b0 * M, V + mo, info ? info + b0 : nullptr, ws, st);
+        const double* Ac = A + (size_t)b0 * M * M;
+        double* Vc = V + (size_t)b0 * M * M;
+        auto stageT = [&](int c0, int nk, cudaStream_t s) {
+            return stage_T(Ac + (size_t)c0 * M * M, M, nk, Vc + (size_t)c0 * M * M, ws_slice(ws, M, c0), s, nullptr);
+        };
+        auto post = [](int, int, cudaStream_t) { return 0; };
+        rc = run_pass(M, n, w + (size_t)b0 * M, Vc, info ? info + b0 : nullptr, ws, st, stageT, post);
         if (rc) return rc;
     }
     return LETKF_OK;
@@ -333,11 +465,22 @@ int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv
         double* wbc = wbar ? wbar + (size_t)b0 * M : nullptr;
         int* infoc = info ? info + b0 : nullptr;
 
-        GramArgs ga{Ybc, dc, rc_, p, shift, gbuf};
-        rc = syev_chunk_run(Vbuf, M, n, lam, Vbuf, infoc, ws, st, &ga);
+        auto stageT = [&](int c0, int nk, cudaStream_t s) {
+            GramArgs ga{Ybc + (size_t)c0 * p * M, dc + (size_t)c0 * p, rc_ + (size_t)c0 * p, p, shift,
+                        gbuf + (size_t)c0 * M};
+            double* Vk = Vbuf + (size_t)c0 * M * M;
+            return stage_T(Vk, M, nk, Vk, ws_slice(ws, M, c0), s, &ga);
+        };
+        auto post = [&](int c0, int nk, cudaStream_t s) -> int {
+            KLAUNCH("generic_epilogue", s,
+                    generic_epilogue<<<nk, 256, ep_smem, s>>>(
+                        Vbuf + (size_t)c0 * M * M, lam + (size_t)c0 * M, gbuf + (size_t)c0 * M,
+                        Xbc + (size_t)c0 * nstate * M, M, nstate, Xac + (size_t)c0 * nstate * M,
+                        Wc ? Wc + (size_t)c0 * M * M : nullptr, wbc ? wbc + (size_t)c0 * M : nullptr));
+            return 0;
+        };
+        rc = run_pass(M, n, lam, Vbuf, infoc, ws, st, stageT, post);
         if (rc) return rc;
-        KLAUNCH("generic_epilogue", st,
-                generic_epilogue<<<n, 256, ep_smem, st>>>(Vbuf, lam, gbuf, Xbc, M, nstate, Xac, Wc, wbc));
     }
     return LETKF_OK;
 }
@@ -362,6 +505,7 @@ int letkf_set_option(const char* name, int value)
 {
     if (!name) return -1;
     if (strcmp(name, "force_generic") == 0) { g_force_generic = value != 0; return LETKF_OK; }
+    if (strcmp(name, "pipeline") == 0) { g_pipeline = value != 0; return LETKF_OK; }
     return -1;
 }
 
@@ -369,6 +513,7 @@ int letkf_profile_enable(int on)
 {
     const int prev = g_prof.on ? 1 : 0;
     g_prof.on = on != 0;
+    g_prof.keep_pipeline = on == 2;
     return prev;
 }
 
@@ -386,6 +531,15 @@ int letkf_profile_record(int idx, const char** name, float* ms)
     if (name) *name = r.name;
     if (ms) *ms = t;
     return LETKF_OK;
+}
+
+int letkf_profile_record_start(int idx, float* ms_from_first)
+{
+    if (idx < 0 || idx >= (int)g_prof.recs.size() || !ms_from_first) return -1;
+    cudaError_t e = cudaEventSynchronize(g_prof.recs[idx].e0);
+    if (e != cudaSuccess) return (int)e;
+    e = cudaEventElapsedTime(ms_from_first, g_prof.recs[0].e0, g_prof.recs[idx].e0);
+    return e == cudaSuccess ? LETKF_OK : (int)e;
 }
 
 long long letkf_profile_rotations(void)

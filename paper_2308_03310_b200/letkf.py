@@ -18,7 +18,7 @@ EXPORTS = (
     "letkf_syev_batched", "letkf_syev_workspace_bytes",
     "letkf_analysis_batched", "letkf_analysis_workspace_bytes",
     "letkf_probe_dfma", "letkf_last_launch_count",
-    "letkf_profile_enable", "letkf_profile_count", "letkf_profile_record", "letkf_profile_rotations",
+    "letkf_profile_enable", "letkf_profile_count", "letkf_profile_record", "letkf_profile_record_start", "letkf_profile_rotations",
     "letkf_set_option", "letkf_status_string", "letkf_version",
 )
 
@@ -59,6 +59,8 @@ def load():
     lib.letkf_profile_count.restype = ci
     lib.letkf_profile_record.argtypes = [ci, ctypes.POINTER(ctypes.c_char_p), ctypes.POINTER(ctypes.c_float)]
     lib.letkf_profile_record.restype = ci
+    lib.letkf_profile_record_start.argtypes = [ci, ctypes.POINTER(ctypes.c_float)]
+    lib.letkf_profile_record_start.restype = ci
     lib.letkf_profile_rotations.argtypes = []
     lib.letkf_profile_rotations.restype = ctypes.c_longlong
     lib.letkf_set_option.argtypes = [ctypes.c_char_p, ci]
@@ -180,7 +182,19 @@ def probe_dfma(blocks, threads, iters, stream=None):
 
 
 def profile_enable(on):
-    return load().letkf_profile_enable(1 if on else 0)
+    """0/False off; 1/True each kernel timed alone (one chunk, caller's stream); 2 timeline of the pipeline."""
+    return load().letkf_profile_enable(int(on))
+
+
+def profile_timeline():
+    """[(kernel name, start ms relative to the first record, duration ms)] of the last compute call."""
+    lib = load()
+    out = []
+    for i, (name, ms) in enumerate(profile_records()):
+        t0 = ctypes.c_float()
+        _check(lib.letkf_profile_record_start(i, ctypes.byref(t0)), "letkf_profile_record_start")
+        out.append((name, t0.value, ms))
+    return out
 
 
 def profile_records():

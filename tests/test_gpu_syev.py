@@ -205,3 +205,27 @@ def test_generic_kernels_at_small_order(lk, oracle, M):
     assert (info == 0).all()
     wo, _, _, _ = oracle.syev_batched(A)
     parity.assert_evd(A, w, V, wo, f"generic M={M}")
+
+
+def test_pipelined_equals_single_stream(lk):
+    """The sub-chunk pipeline over private streams (Streams) only reorders
+    launches: its results are bitwise those of the one-stream, one-chunk run, also in place and
+    when the call follows other work on a user stream."""
+    import torch
+    A = wl.letkf_shaped(4096 + 37, 64, 98, config_index=901)
+    At = torch.from_numpy(A).cuda()
+    try:
+        lk.set_option("pipeline", 0)
+        w0, V0, i0 = lk.syev_batched(At)
+        torch.cuda.synchronize()
+    finally:
+        lk.set_option("pipeline", 1)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        B = At.clone()                                   # produced on the user stream just before
+        w1, V1, i1 = lk.syev_batched(B, V=B, stream=st)  # in place
+        s = V1.sum()                                     # consumed on the user stream just after
+    st.synchronize()
+    assert torch.equal(w0, w1) and torch.equal(V0, V1) and torch.equal(i0, i1)
+    assert torch.isfinite(s)
+    assert lk.last_launch_count() >= 4 * 4               # >= 4 sub-chunks x 4 kernels
