@@ -119,6 +119,53 @@ __device__ __forceinline__ void rank2_desc(double (&a)[MT], const double2* vp, d
     }
 }
 
+// ---- statically shaped BLAS-1 pieces of the reduction (pivot group G: columns 0 .. 8G+7) -----
+// Inside a group of 8 pivots the active column range rounds up to the same 8-column block, so
+// every loop below has compile-time bounds: straight-line code, no jump table, and the compiler is
+// free to hoist the shared-memory loads of a whole pass.
+
+// sum_{c < 8(G+1)} a[c] * vec[c]
+template <int MT, int G>
+__device__ __forceinline__ double dot_blocks(const double (&a)[MT], const double* vec)
+{
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0, s4 = 0.0, s5 = 0.0, s6 = 0.0, s7 = 0.0;
+    const double2* v2 = reinterpret_cast<const double2*>(vec);
+#pragma unroll
+    for (int g = G; g >= 0; --g) {
+        const double2 t0 = v2[4 * g], t1 = v2[4 * g + 1], t2 = v2[4 * g + 2], t3 = v2[4 * g + 3];
+        s0 = fma(a[8 * g],     t0.x, s0); s1 = fma(a[8 * g + 1], t0.y, s1);
+        s2 = fma(a[8 * g + 2], t1.x, s2); s3 = fma(a[8 * g + 3], t1.y, s3);
+        s4 = fma(a[8 * g + 4], t2.x, s4); s5 = fma(a[8 * g + 5], t2.y, s5);
+        s6 = fma(a[8 * g + 6], t3.x, s6); s7 = fma(a[8 * g + 7], t3.y, s7);
+    }
+    return ((s0 + s1) + (s2 + s3)) + ((s4 + s5) + (s6 + s7));
+}
+
+// a[c] -= alpha * vec[c] for the 8 columns of block g
+template <int MT>
+__device__ __forceinline__ void axpy_block(double (&a)[MT], const double* vec, double nalpha, int g)
+{
+    const double2* v2 = reinterpret_cast<const double2*>(vec);
+    const double2 t0 = v2[4 * g], t1 = v2[4 * g + 1], t2 = v2[4 * g + 2], t3 = v2[4 * g + 3];
+    a[8 * g]     = fma(nalpha, t0.x, a[8 * g]);     a[8 * g + 1] = fma(nalpha, t0.y, a[8 * g + 1]);
+    a[8 * g + 2] = fma(nalpha, t1.x, a[8 * g + 2]); a[8 * g + 3] = fma(nalpha, t1.y, a[8 * g + 3]);
+    a[8 * g + 4] = fma(nalpha, t2.x, a[8 * g + 4]); a[8 * g + 5] = fma(nalpha, t2.y, a[8 * g + 5]);
+    a[8 * g + 6] = fma(nalpha, t3.x, a[8 * g + 6]); a[8 * g + 7] = fma(nalpha, t3.y, a[8 * g + 7]);
+}
+
+// a[8G + k], k = 0..7 at run time (select chain; the block is compile-time)
+template <int MT, int G>
+__device__ __forceinline__ double block_pick(const double (&a)[MT], int k)
+{
+    double x = a[8 * G];
+#pragma unroll
+    for (int t = 1; t < 8; ++t) x = (k == t) ? a[8 * G + t] : x;
+    return x;
+}
+
+#ifndef LETKF_TRI_REGS64
+#define LETKF_TRI_REGS64 168
+#endif
 template <int MT> struct FastCfg {
     static constexpr int NT = (MT + 31) / 32 * 32;      // threads per matrix = threads per CTA
     static constexpr int NW = NT / 32;
@@ -175,28 +222,123 @@ __device__ __forceinline__ void load_tile(double* tile, const double* __restrict
 
 // Dynamic shared memory of fast_tridiag_formq<MT>:
 //   tile[MT*(MT+1)]  staging of A (padded), later the reflectors R[i][c] (stride MT)
-//   vs[MT]  v;  vw[MT] (v,w) pairs;  taus[MT];  red[8]
+//   xs[NT] raw pivot column;  vbuf[NT] v;  pbuf[NT] p;  pv[NT] p_j v_j;  taus[NT];  red[8]
 template <int MT> constexpr size_t fast_tridiag_smem()
 {
-    return sizeof(double) * ((size_t)MT * (MT + 1) + MT + 2 * MT + MT + 8);
+    return sizeof(double) * ((size_t)MT * (MT + 1) + 5 * FastCfg<MT>::NT + 8);
+}
+
+struct TriShared {
+    double* R;      // reflector i at R[i*MT + c]
+    double* xs;     // x_c = A[c][i] for c < i-1, zero from i-1 on
+    double* vbuf;   // v_c (v_{i-1} = 1, zero from i on)
+    double* pbuf;   // p_c = tau (A v)_c, zero from i on
+    double* pv;     // p_c v_c
+    double* taus;
+    double* red;    // [0..1] per-warp partial of sigma, [4] alpha
+};
+
+// Pivots i = min(8G+8, M-1) ... 8G+1 of the Householder reduction (H_i acts on indices 0..i-1, the
+// active columns all lie in blocks 0..G).  Two barriers per pivot:
+//   B1  the raw pivot column x and the partial sums of sigma are visible (both were produced by
+//       the look-ahead at the end of the previous pivot)
+//       -> every thread forms the scalars (tau, beta, 1/(alpha-beta)) redundantly WHILE it runs the
+//          raw product sum_c a_jc x_c; then p_j, v_j
+//   B2  v, p and the products p_c v_c are visible
+//       -> pass A  a_jc -= v_j p_c  overlaps the shuffle tree of p.v
+//       -> pass B  a_jc -= (p_j - tau (p.v) v_j) v_c, top block first: column i-1 is then final, it
+//          is the next pivot's x, whose norm tree overlaps the rest of pass B.
+// Entered and left with B1 done (by the NP warps that hold rows < 8G+8).
+template <int MT, int G>
+__device__ __forceinline__ void pivot_group(double (&a)[MT], const TriShared& sh, int M,
+                                            double* __restrict__ dws, double* __restrict__ ews)
+{
+    using C = FastCfg<MT>;
+    constexpr int NPR = (8 * G + 8 + 31) / 32;
+    constexpr int NP = NPR < C::NW ? NPR : C::NW;
+    constexpr unsigned FULL = 0xffffffffu;
+    const int j = threadIdx.x, lane = j & 31, warp = j >> 5;
+    if (warp >= NP) return;
+    const int ihi = (8 * G + 8 < M - 1) ? 8 * G + 8 : M - 1;
+    for (int i = ihi; i >= 8 * G + 1; --i) {
+        const int k = i - 1 - 8 * G;
+        double sigma = sh.red[0];
+        if constexpr (NP > 1) sigma += sh.red[1];
+        const double alpha = sh.red[4];
+        const double xj = sh.xs[j];
+        const double praw = dot_blocks<MT, G>(a, sh.xs);
+        const double acol = block_pick<MT, G>(a, k);          // A[j][i-1] before the update
+        double tau = 0.0, scal = 0.0, beta = alpha;            // sigma == 0: H_i = I (reading G19)
+        if (sigma != 0.0) {
+            const double nrm2 = fma(alpha, alpha, sigma);
+            const double rinv = rsqrt(nrm2);
+            beta = -copysign(nrm2 * rinv, alpha);
+            tau = fma(fabs(alpha), rinv, 1.0);                 // (beta - alpha) / beta
+            scal = 1.0 / (alpha - beta);
+        }
+        const double vj = (j < i - 1) ? xj * scal : ((j == i - 1) ? 1.0 : 0.0);
+        const double pj = (j < i) ? tau * fma(scal, praw, acol) : 0.0;
+        sh.vbuf[j] = vj;
+        sh.pbuf[j] = pj;
+        sh.pv[j] = pj * vj;
+        if (j < MT) sh.R[i * MT + j] = vj;
+        if (j == 0) { ews[i - 1] = beta; sh.taus[i] = tau; }
+        part_barrier(NP);                                      // ---- B2
+        double t = sh.pv[lane];
+        if constexpr (NP > 1) t += sh.pv[lane + 32];
+        const double nvj = -vj;
+#pragma unroll
+        for (int step = 0; step < (G + 1 > 5 ? G + 1 : 5); ++step) {
+            if (step < 5) t += __shfl_xor_sync(FULL, t, 16 >> step);
+            if (step <= G) axpy_block<MT>(a, sh.pbuf, nvj, G - step);
+        }
+        const double nwj = fma(tau * t, vj, -pj);              // -(p_j - tau (p.v) v_j)
+        axpy_block<MT>(a, sh.vbuf, nwj, G);
+        const double xn = block_pick<MT, G>(a, k);             // A[j][i-1], final: next pivot's x_j
+        if (j == i - 1) dws[i - 1] = xn;
+        sh.xs[j] = (j < i - 2) ? xn : 0.0;
+        if (j == i - 2) sh.red[4] = xn;
+        double part = (j < i - 2) ? xn * xn : 0.0;
+#pragma unroll
+        for (int step = 0; step < (G > 5 ? G : 5); ++step) {
+            if (step < 5) part += __shfl_xor_sync(FULL, part, 16 >> step);
+            if (step < G) axpy_block<MT>(a, sh.vbuf, nwj, G - 1 - step);
+        }
+        if (lane == 0) sh.red[warp] = part;
+        part_barrier(NP);                                      // ---- B1 of the next pivot
+    }
+}
+
+template <int MT, int G>
+__device__ __forceinline__ void pivot_groups_down(double (&a)[MT], const TriShared& sh, int M,
+                                                  double* __restrict__ dws, double* __restrict__ ews)
+{
+    pivot_group<MT, G>(a, sh, M, dws, ews);
+    if constexpr (G > 0) pivot_groups_down<MT, G - 1>(a, sh, M, dws, ews);
 }
 
 // ---------------------------------------------------------------------------------------------
 // a3 + explicit Q for one matrix per CTA.  gram == true: the matrix is not read from A but formed
 // from the LETKF inputs (a1, a2: Eq.17 and the right factor of Eq.14) straight into the registers.
 template <int MT, bool GRAM>
-__global__ void __launch_bounds__(FastCfg<MT>::NT, (MT == 64) ? 4 : (MT == 48 ? 7 : 16))
+__global__ void __launch_bounds__(FastCfg<MT>::NT) __maxnreg__((MT == 64) ? LETKF_TRI_REGS64 : (MT == 48 ? 168 : (MT == 32 ? 168 : 128)))
 fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Workspace ws, int M,
                    const double* __restrict__ Yb_, const double* __restrict__ d_,
                    const double* __restrict__ r_, int p, double shift, double* __restrict__ gout_)
 {
     using C = FastCfg<MT>;
     extern __shared__ __align__(16) double sm[];
-    double*  tile = sm;
-    double*  vs   = sm + MT * (MT + 1);
-    double2* vw   = reinterpret_cast<double2*>(vs + MT);
-    double*  taus = vs + 3 * MT;
-    double*  red  = taus + MT;
+    double* tile = sm;
+    double* small = sm + MT * (MT + 1);
+    TriShared sh;
+    sh.R = tile;
+    sh.xs = small;
+    sh.vbuf = small + C::NT;
+    sh.pbuf = small + 2 * C::NT;
+    sh.pv = small + 3 * C::NT;
+    sh.taus = small + 4 * C::NT;
+    sh.red = small + 5 * C::NT;
+    double* taus = sh.taus;
     const int j = threadIdx.x, lane = j & 31, warp = j >> 5;
     const size_t b = blockIdx.x;
     double a[MT];
@@ -249,58 +391,25 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
     double* ews = ws.ews + b * M;
     double* R = tile;                              // reflector i at R[i*MT + c]
 
-    // ---- a3: Householder tridiagonalisation, pivot i = M-1 ... 1, H_i acts on indices 0..i-1
-    for (int i = M - 1; i >= 1; --i) {
-        // warps 0 .. np-1 hold rows <= i and take part in this step; the others are done and
-        // wait at the barrier after the loop (part_barrier counts only the participants)
-        const int np = min(C::NW, (i >> 5) + 1);
-        if (warp >= np) break;
-        const double x = pick<MT>(a, i);           // x_j = A[j][i]; for j == i this is d_i
-        if (j == i) dws[i] = x;
-        if (j == i - 1) red[4] = x;                // alpha
-        double part = (j < i - 1) ? x * x : 0.0;
+    // ---- a3: Householder tridiagonalisation, pivot i = M-1 ... 1, H_i acts on indices 0..i-1.
+    // Prologue = the look-ahead of a fictitious pivot M: publish column M-1 and its partial norms.
+    {
+        const int i0 = M - 1;
+        const double x = pick<MT>(a, i0);              // x_j = A[j][i0]; for j == i0 this is d_i0
+        if (j == i0) dws[i0] = x;
+        sh.xs[j] = (j < i0 - 1) ? x : 0.0;
+        if (j == i0 - 1) sh.red[4] = x;
+        double part = (j < i0 - 1) ? x * x : 0.0;
         part = warp_sum(part);
-        if (lane == 0) red[warp] = part;
-        part_barrier(np);
-        double sigma = 0.0;
-#pragma unroll
-        for (int w2 = 0; w2 < C::NW; ++w2) sigma += (w2 < np) ? red[w2] : 0.0;
-        const double alpha = red[4];
-        double tau, scal, beta;
-        if (sigma == 0.0) { tau = 0.0; beta = alpha; scal = 0.0; }      // reading G19: H_i = I
-        else {
-            const double nrm2 = fma(alpha, alpha, sigma);
-            const double rinv = rsqrt(nrm2);
-            const double nrm = nrm2 * rinv;
-            beta = -copysign(nrm, alpha);
-            tau = fma(fabs(alpha), rinv, 1.0);                            // (beta - alpha)/beta
-            scal = 1.0 / (alpha - beta);
-        }
-        const double vj = (j < i - 1) ? x * scal : ((j == i - 1) ? 1.0 : 0.0);
-        if (j < MT) {                                   // NT may exceed MT (MT = 16, 48)
-            vs[j] = vj;
-            R[i * MT + j] = vj;
-        }
-        if (j == 0) { ews[i - 1] = beta; taus[i] = tau; }
-        part_barrier(np);
-        if (tau != 0.0) {
-            const int gtop = (i - 1) >> 3;
-            double pj = tau * dot_desc<MT>(a, vs, gtop);                  // p = tau A v
-            if (j >= i) pj = 0.0;
-            double pv = warp_sum(pj * vj);
-            if (lane == 0) red[2 + warp] = pv;
-            if (j < MT) vw[j] = make_double2(vj, pj);                     // (v_c, p_c) broadcast pairs
-            part_barrier(np);
-            double ptv = 0.0;
-#pragma unroll
-            for (int w2 = 0; w2 < C::NW; ++w2) ptv += (w2 < np) ? red[2 + w2] : 0.0;
-            // A -= v w^T + w v^T with w = p - K v, K = (tau/2) p.v, written on the broadcast
-            // pairs (v_c, p_c):  a_jc -= v_j p_c + (p_j - 2 K v_j) v_c   (one barrier fewer)
-            const double wj = pj - (tau * ptv) * vj;
-            if (j < i) rank2_desc<MT>(a, vw, vj, wj, gtop);
-        }
+        if (lane == 0) sh.red[warp] = part;
+        if (j == 0) ews[M - 1] = 0.0;
+        __syncthreads();
     }
-    if (j == 0) { dws[0] = a[0]; ews[M - 1] = 0.0; }
+    // a warp leaves pivot_groups_down when the rows it holds are done (after the B1 that closes
+    // the last pivot it took part in), the others carry on with barriers that no longer count it
+#ifndef LETKF_DBG_SKIPRED
+    pivot_groups_down<MT, (MT - 2) / 8>(a, sh, M, dws, ews);
+#endif
     __syncwarp();
 
     // ---- explicit Q = H_{M-1} ... H_1: thread r owns column r of Q; no synchronisation needed.
@@ -310,6 +419,7 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
     double (&q)[MT] = a;
 #pragma unroll
     for (int c = 0; c < MT; ++c) q[c] = (c == j) ? 1.0 : 0.0;
+#ifndef LETKF_DBG_SKIPQ
     for (int i = warp * 32 + 1; i <= M - 1; ++i) {
         const double tau = taus[i];
         if (tau == 0.0) continue;
@@ -318,6 +428,7 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
         const double s = tau * dot_desc<MT>(q, v, gtop);
         axpy_desc<MT>(q, v, s, gtop);
     }
+#endif
     if (j < M) {
         double* Q = Q_ + b * M * M;
 #pragma unroll

@@ -49,48 +49,113 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
     double2* rot = ws.rot + (size_t)(valid ? b : b0) * ws.logcap;
     uint32_t* hdr = ws.hdr + (size_t)(valid ? b : b0) * ws.swcap;
 
-    QLState st{0, 0, 0};
+    // Per-lane state: the unreduced block [l, m] (e[m] == 0), the sweeps spent on eigenvalue l,
+    // the failures.  The deflation test of the classic algorithm ("first m >= l with negligible
+    // e[m]", rescanned before every sweep) is evaluated INSIDE the sweep on the values it has
+    // just produced, so the per-sweep rescan disappears (it was 30% of this kernel, profiles/r01a);
+    // a scan is needed only when l enters a part of the matrix no sweep of this block has seen.
+    const double eps = 1.1102230246251565e-16;   // 2^-53 (reading G10)
+#define QL_D(i) d[(i) * stride]
+#define QL_E(i) e[(i) * stride]
+    auto scan_end = [&](int from) {
+        int k = from;
+        for (; k < M - 1; ++k)
+            if (fabs(QL_E(k)) <= eps * (fabs(QL_D(k)) + fabs(QL_D(k + 1)))) break;
+        QL_E(k) = 0.0;
+        return k;
+    };
+    int l = 0, m = 0, iter = 0, fail = 0;
     int overflow = 0, nsw = 0, pos = 0;
     bool done = !valid;
+    if (!done) m = scan_end(0);
     for (;;) {
         // ---- per-lane sweep set-up (divergent inside, reconverges at the vote)
-        int l = 0, m = 0, i = -1;
-        double g = 0.0, s = 1.0, c = 1.0, p = 0.0;
         bool sweeping = false;
-        if (!done) {
-            if (ql_find_block(st, d, e, stride, M, m)) {
-                l = st.l;
-                if (pos + (m - l) > ws.logcap || nsw >= ws.swcap) { overflow = 1; done = true; }
-                else { g = ql_shift(d, e, stride, l, m); i = m - 1; sweeping = true; }
-            } else {
-                done = true;
+        while (!done) {
+            if (m == l) {                              // eigenvalue l has converged
+                l += 1; iter = 0;
+                if (l >= M) { done = true; break; }
+                m = scan_end(l);
+                continue;
             }
+            if (iter >= 30) {                          // give up on this one (info counts it)
+                fail += 1; QL_E(l) = 0.0; m = l;
+                continue;
+            }
+            if (pos + (m - l) > ws.logcap || nsw >= ws.swcap) { overflow = 1; done = true; break; }
+            iter += 1;
+            sweeping = true;
+            break;
         }
         if (!__any_sync(FULL, sweeping)) break;
+        int i = -1, mlow = m;
+        double g = 0.0, s = 1.0, c = 1.0, p = 0.0, dprev = 0.0;
+        if (sweeping) {
+            // Wilkinson shift
+            const double el = QL_E(l), dl = QL_D(l);
+            const double gg = (QL_D(l + 1) - dl) / (2.0 * el);
+            const double rr = sqrt(gg * gg + 1.0);
+            g = QL_D(m) - dl + el / (gg + copysign(rr, gg));
+            i = m - 1;
+        }
         const int maxlen = __reduce_max_sync(FULL, sweeping ? m - l : 0);
         // ---- lockstep rotation steps
         bool broke = false;
+        double2* out = rot + pos;
         for (int k = 0; k < maxlen; ++k) {
             if (sweeping && !broke && i >= l) {
-                double2 cs;
-                if (ql_rot_step(d, e, stride, i, m, s, c, p, g, cs)) {
-                    rot[pos + (m - 1 - i)] = cs;
-                    --i;
-                } else {
+                const double ei = QL_E(i), di = QL_D(i), di1 = QL_D(i + 1);
+                const double f = s * ei;
+                const double b2 = c * ei;
+                const double r2 = fma(f, f, g * g);
+                if (!(r2 > 0.0)) {                     // underflow / NaN: split the block at i+1
+                    QL_E(i + 1) = 0.0;
+                    QL_D(i + 1) = di1 - p;
+                    QL_E(m) = 0.0;
                     broke = true;
+                } else {
+                    const double rinv = rsqrt(r2);
+                    const double enew = r2 * rinv;
+                    s = f * rinv;
+                    c = g * rinv;
+                    g = di1 - p;
+                    const double r = fma(di - g, s, 2.0 * c * b2);
+                    p = s * r;
+                    const double dnew = g + p;
+                    QL_E(i + 1) = enew;
+                    QL_D(i + 1) = dnew;
+                    g = fma(c, r, -b2);
+                    out[m - 1 - i] = make_double2(c, s);
+                    // deflation test of index i+1 on this sweep's values (d[i+2] = dprev)
+                    if (i + 1 < m && fabs(enew) <= eps * (fabs(dnew) + fabs(dprev))) mlow = i + 1;
+                    dprev = dnew;
+                    --i;
                 }
             }
         }
         if (sweeping) {
             int lo;
-            if (broke) lo = i + 1;
-            else { ql_finish_sweep(d, e, stride, l, m, p, g); lo = l; }
-            if (m - lo > 0) {
-                hdr[nsw++] = (uint32_t)lo | ((uint32_t)m << 16);
-                pos += m - lo;
+            if (broke) {
+                lo = i + 1;
+                // the block was split by hand: what is left of it below i+1 is rescanned
+                if (m - lo > 0) { hdr[nsw++] = (uint32_t)lo | ((uint32_t)m << 16); pos += m - lo; }
+                m = scan_end(l);
+            } else {
+                const double dl = QL_D(l) - p;
+                QL_D(l) = dl;
+                QL_E(l) = g;
+                QL_E(m) = 0.0;
+                hdr[nsw++] = (uint32_t)l | ((uint32_t)m << 16);
+                pos += m - l;
+                if (mlow < m) QL_E(mlow) = 0.0;
+                m = mlow;
+                if (fabs(g) <= eps * (fabs(dl) + fabs(dprev))) { QL_E(l) = 0.0; m = l; }
             }
         }
     }
+#undef QL_D
+#undef QL_E
+    QLState st{0, 0, fail};
     if (valid) {
         if (!overflow) sort_eigenvalues(d, QL_TPB, reinterpret_cast<int*>(e), QL_TPB * 2, M);
         ws.nsweeps[b] = nsw;
