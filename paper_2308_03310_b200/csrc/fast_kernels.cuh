@@ -125,7 +125,7 @@ __device__ __forceinline__ void rank2_desc(double (&a)[MT], const double2* vp, d
 // free to hoist the shared-memory loads of a whole pass.
 
 // sum_{c < 8(G+1)} a[c] * vec[c]
-template <int MT, int G>
+template <int MT, int G, bool FENCED = false>
 __device__ __forceinline__ double dot_blocks(const double (&a)[MT], const double* vec)
 {
     double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0, s4 = 0.0, s5 = 0.0, s6 = 0.0, s7 = 0.0;
@@ -137,6 +137,7 @@ __device__ __forceinline__ double dot_blocks(const double (&a)[MT], const double
         s2 = fma(a[8 * g + 2], t1.x, s2); s3 = fma(a[8 * g + 3], t1.y, s3);
         s4 = fma(a[8 * g + 4], t2.x, s4); s5 = fma(a[8 * g + 5], t2.y, s5);
         s6 = fma(a[8 * g + 6], t3.x, s6); s7 = fma(a[8 * g + 7], t3.y, s7);
+        if constexpr (FENCED) __syncwarp();     // ptxas does not move shared loads across it
     }
     return ((s0 + s1) + (s2 + s3)) + ((s4 + s5) + (s6 + s7));
 }
@@ -218,6 +219,31 @@ __device__ __forceinline__ void load_tile(double* tile, const double* __restrict
             }
         }
     }
+}
+
+// Explicit Q: reflectors i = 8G+1 ... 8G+8 applied to the column q held by this thread.  The
+// __syncwarp() after every 8-column block is a scheduling fence: ptxas does not move shared-memory
+// loads across it, and without it the loads of a whole pass are hoisted and the matrix spills.
+template <int MT, int G>
+__device__ __forceinline__ void q_group(double (&q)[MT], const double* R, const double* taus, int M)
+{
+#pragma unroll 1
+    for (int i = 8 * G + 1; i <= 8 * G + 8 && i <= M - 1; ++i) {
+        const double tau1 = taus[i];
+        if (tau1 == 0.0) continue;
+        const double* v1 = R + i * MT;
+        const double ns1 = -tau1 * dot_blocks<MT, G, true>(q, v1);
+#pragma unroll
+        for (int g = G; g >= 0; --g) { axpy_block<MT>(q, v1, ns1, g); __syncwarp(); }
+    }
+}
+
+template <int MT, int G, int GMAX>
+__device__ __forceinline__ void q_groups_up(double (&q)[MT], const double* R, const double* taus,
+                                            int M, int gstart)
+{
+    if (G >= gstart) q_group<MT, G>(q, R, taus, M);
+    if constexpr (G < GMAX) q_groups_up<MT, G + 1, GMAX>(q, R, taus, M, gstart);
 }
 
 // Dynamic shared memory of fast_tridiag_formq<MT>:
@@ -420,14 +446,7 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
 #pragma unroll
     for (int c = 0; c < MT; ++c) q[c] = (c == j) ? 1.0 : 0.0;
 #ifndef LETKF_DBG_SKIPQ
-    for (int i = warp * 32 + 1; i <= M - 1; ++i) {
-        const double tau = taus[i];
-        if (tau == 0.0) continue;
-        const int gtop = (i - 1) >> 3;
-        const double* v = R + i * MT;
-        const double s = tau * dot_desc<MT>(q, v, gtop);
-        axpy_desc<MT>(q, v, s, gtop);
-    }
+    q_groups_up<MT, 0, (MT - 2) / 8>(q, R, taus, M, warp * 4);
 #endif
     if (j < M) {
         double* Q = Q_ + b * M * M;
