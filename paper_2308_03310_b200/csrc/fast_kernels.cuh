@@ -459,9 +459,22 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
 // ---------------------------------------------------------------------------------------------
 // a5: V = Q Z by replaying the logged rotations; thread r owns row r of Q in registers.
 // Dynamic shared memory: tile[MT*(MT+1)], cs[2][MT] double2, hdr[swcap] u32, inv[MT] int
+constexpr int AP_S = 4;      // sweeps staged per barrier round
+template <int MT> __host__ __device__ constexpr int ap_tile_doubles() { return (MT * (MT + 1) + 3) & ~1; }
 template <int MT> size_t fast_apply_smem(int swcap)
 {
-    return sizeof(double) * ((size_t)MT * (MT + 1) + 4 * MT) + sizeof(uint32_t) * (size_t)swcap + sizeof(int) * MT + 16;
+    static_assert(4 * AP_S * MT <= MT * (MT + 1), "the staged rotations alias the tile");
+    return sizeof(double) * (size_t)ap_tile_doubles<MT>() + sizeof(uint32_t) * (size_t)swcap + sizeof(int) * MT + 16;
+}
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
+{
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all()
+{
+    asm volatile("cp.async.wait_all;" ::: "memory");
 }
 
 // Rotations i = m-1 ... lo on columns (i, i+1):  f = z[i+1]; z[i+1] = s z[i] + c f; z[i] = c z[i] - s f.
@@ -503,8 +516,8 @@ fast_apply(double* __restrict__ V_, Workspace ws, int M)
     using C = FastCfg<MT>;
     extern __shared__ __align__(16) double sm[];
     double*   tile = sm;
-    double2*  cs   = reinterpret_cast<double2*>(sm + MT * (MT + 1) + (MT & 1));
-    uint32_t* hdr  = reinterpret_cast<uint32_t*>(cs + 2 * MT);
+    double2*  cs   = reinterpret_cast<double2*>(sm);   // [2][AP_S][MT], aliases the tile while rotating
+    uint32_t* hdr  = reinterpret_cast<uint32_t*>(sm + ap_tile_doubles<MT>());
     int*      inv  = reinterpret_cast<int*>(hdr + ws.swcap);
     const int r = threadIdx.x;
     const size_t b = blockIdx.x;
@@ -521,27 +534,42 @@ fast_apply(double* __restrict__ V_, Workspace ws, int M)
 #pragma unroll
     for (int c = 0; c < MT; ++c) z[c] = (r < M && c < M) ? tile[r * C::LDT + c] : 0.0;
 
-    int pos = 0;
-    if (nsw > 0) {
-        const uint32_t h = hdr[0];
-        const int lo = h & 0xffff, m = h >> 16;
-        if (r < MT) cs[r] = (r >= lo && r < m) ? rot[pos + (m - 1 - r)] : make_double2(1.0, 0.0);
-    }
-    __syncthreads();
-    for (int s = 0; s < nsw; ++s) {
-        const uint32_t h = hdr[s];
-        const int lo = h & 0xffff, m = h >> 16;
-        pos += m - lo;
-        double2 nxt = make_double2(1.0, 0.0);
-        bool have = false;
-        if (s + 1 < nsw) {
-            const uint32_t h2 = hdr[s + 1];
-            const int lo2 = h2 & 0xffff, m2 = h2 >> 16;
-            have = (r >= lo2 && r < m2);
-            if (have) nxt = rot[pos + (m2 - 1 - r)];
+    // The (c, s) of AP_S sweeps are staged per barrier round, double-buffered: thread r copies the
+    // rotation that acts on columns (r, r+1) of each sweep straight from the log into shared
+    // memory (cp.async, no registers), identity outside [lo, m); the copies of round k+1 fly
+    // while round k is applied.
+    int spos = 0;                                   // log position of the next sweep to stage
+    auto stage = [&](int round) {
+        double2* dst = cs + (round & 1) * AP_S * MT;
+#pragma unroll
+        for (int t = 0; t < AP_S; ++t) {
+            const int s = round * AP_S + t;
+            if (s < nsw) {
+                const uint32_t h = hdr[s];
+                const int lo = h & 0xffff, m = h >> 16;
+                if (r < MT) {
+                    if (r >= lo && r < m) cp_async16(dst + t * MT + r, rot + spos + (m - 1 - r));
+                    else dst[t * MT + r] = make_double2(1.0, 0.0);
+                }
+                spos += m - lo;
+            }
         }
-        apply_sweep<MT>(z, cs + (s & 1) * MT, lo, m);
-        if (r < MT) cs[((s + 1) & 1) * MT + r] = nxt;       // identity outside [lo2, m2)
+    };
+    const int nrounds = (nsw + AP_S - 1) / AP_S;
+    __syncthreads();                                // every row has left the tile: reuse it for cs
+    if (nrounds > 0) stage(0);
+    cp_async_wait_all();
+    __syncthreads();
+    for (int k = 0; k < nrounds; ++k) {
+        if (k + 1 < nrounds) stage(k + 1);
+        const double2* cur = cs + (k & 1) * AP_S * MT;
+        const int send = min(nsw, (k + 1) * AP_S);
+#pragma unroll 1
+        for (int s = k * AP_S; s < send; ++s) {
+            const uint32_t h = hdr[s];
+            apply_sweep<MT>(z, cur + (s - k * AP_S) * MT, h & 0xffff, h >> 16);
+        }
+        cp_async_wait_all();
         __syncthreads();
     }
 
