@@ -196,19 +196,21 @@ __device__ __forceinline__ void part_barrier(int nwarps)
     else asm volatile("bar.sync 1, %0;" ::"r"(nwarps * 32) : "memory");
 }
 
-// Coalesced copy of a row-major M x M matrix into the padded shared tile; 8 loads in flight per
-// thread (a plain load->store loop exposed the full DRAM latency 64 times, profiles/).
+// Coalesced copy of rows [r0, r0+nr) of a row-major M x M matrix into the padded shared tile
+// (tile row = matrix row - r0); 8 loads in flight per thread (a plain load->store loop exposed
+// the full DRAM latency once per element, profiles/r01a).
 template <int MT>
-__device__ __forceinline__ void load_tile(double* tile, const double* __restrict__ G, int M)
+__device__ __forceinline__ void load_rows(double* tile, const double* __restrict__ G, int M, int r0, int nr)
 {
     using C = FastCfg<MT>;
-    const int n = M * M;
+    const int n = nr * M;
+    const double* src = G + (size_t)r0 * M;
     for (int base = threadIdx.x; base < n; base += 8 * C::NT) {
         double tmp[8];
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
             const int idx = base + u * C::NT;
-            tmp[u] = (idx < n) ? G[idx] : 0.0;
+            tmp[u] = (idx < n) ? src[idx] : 0.0;
         }
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
@@ -221,6 +223,18 @@ __device__ __forceinline__ void load_tile(double* tile, const double* __restrict
     }
 }
 
+// Reflector storage: H_i (i-1 in [8G, 8G+7]) is only ever read over the 8(G+1) columns of its
+// pivot group, so its row is that long: group G starts at 32 G (G+1) doubles.
+template <int MT> struct RefLayout {
+    static constexpr int GMAX = (MT - 2) / 8;
+    static constexpr int TOTAL = 32 * (GMAX + 1) * (GMAX + 2);
+    static constexpr int HT = MT < 32 ? MT : 32;                 // rows of A staged per pass
+    static constexpr int STAGE = HT * (MT + 1);
+    static constexpr int REGION = ((TOTAL > STAGE ? TOTAL : STAGE) + 1) & ~1;   // doubles
+    __device__ static constexpr int base(int G) { return 32 * G * (G + 1); }
+    __device__ static constexpr int len(int G) { return 8 * (G + 1); }
+};
+
 // Explicit Q: reflectors i = 8G+1 ... 8G+8 applied to the column q held by this thread.  The
 // __syncwarp() after every 8-column block is a scheduling fence: ptxas does not move shared-memory
 // loads across it, and without it the loads of a whole pass are hoisted and the matrix spills.
@@ -231,7 +245,7 @@ __device__ __forceinline__ void q_group(double (&q)[MT], const double* R, const 
     for (int i = 8 * G + 1; i <= 8 * G + 8 && i <= M - 1; ++i) {
         const double tau1 = taus[i];
         if (tau1 == 0.0) continue;
-        const double* v1 = R + i * MT;
+        const double* v1 = R + RefLayout<MT>::base(G) + (i - 1 - 8 * G) * RefLayout<MT>::len(G);
         const double ns1 = -tau1 * dot_blocks<MT, G, true>(q, v1);
 #pragma unroll
         for (int g = G; g >= 0; --g) { axpy_block<MT>(q, v1, ns1, g); __syncwarp(); }
@@ -247,15 +261,15 @@ __device__ __forceinline__ void q_groups_up(double (&q)[MT], const double* R, co
 }
 
 // Dynamic shared memory of fast_tridiag_formq<MT>:
-//   tile[MT*(MT+1)]  staging of A (padded), later the reflectors R[i][c] (stride MT)
+//   region[RefLayout::REGION]  staging of A, 32 padded rows per pass, later the reflectors
 //   xs[NT] raw pivot column;  vbuf[NT] v;  pbuf[NT] p;  pv[NT] p_j v_j;  taus[NT];  red[8]
 template <int MT> constexpr size_t fast_tridiag_smem()
 {
-    return sizeof(double) * ((size_t)MT * (MT + 1) + 5 * FastCfg<MT>::NT + 8);
+    return sizeof(double) * ((size_t)RefLayout<MT>::REGION + 5 * FastCfg<MT>::NT + 8);
 }
 
 struct TriShared {
-    double* R;      // reflector i at R[i*MT + c]
+    double* R;      // reflector storage, RefLayout<MT>
     double* xs;     // x_c = A[c][i] for c < i-1, zero from i-1 on
     double* vbuf;   // v_c (v_{i-1} = 1, zero from i on)
     double* pbuf;   // p_c = tau (A v)_c, zero from i on
@@ -307,7 +321,7 @@ __device__ __forceinline__ void pivot_group(double (&a)[MT], const TriShared& sh
         sh.vbuf[j] = vj;
         sh.pbuf[j] = pj;
         sh.pv[j] = pj * vj;
-        if (j < MT) sh.R[i * MT + j] = vj;
+        if (j < RefLayout<MT>::len(G)) sh.R[RefLayout<MT>::base(G) + k * RefLayout<MT>::len(G) + j] = vj;
         if (j == 0) { ews[i - 1] = beta; sh.taus[i] = tau; }
         part_barrier(NP);                                      // ---- B2
         double t = sh.pv[lane];
@@ -355,7 +369,7 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
     using C = FastCfg<MT>;
     extern __shared__ __align__(16) double sm[];
     double* tile = sm;
-    double* small = sm + MT * (MT + 1);
+    double* small = sm + RefLayout<MT>::REGION;
     TriShared sh;
     sh.R = tile;
     sh.xs = small;
@@ -370,15 +384,25 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
     double a[MT];
 
     if constexpr (!GRAM) {
-        load_tile<MT>(tile, A_ + b * M * M, M);
-        __syncthreads();
+        // a_j[c] = A[max(j,c)][min(j,c)] (only the lower triangle is read), 32 rows per pass
+        constexpr int HT = RefLayout<MT>::HT;
 #pragma unroll
-        for (int c = 0; c < MT; ++c) {
-            double v = 0.0;
-            if (j < M && c < M) v = (c <= j) ? tile[j * C::LDT + c] : tile[c * C::LDT + j];
-            a[c] = v;
+        for (int c = 0; c < MT; ++c) a[c] = 0.0;
+#pragma unroll
+        for (int r0 = 0; r0 < MT; r0 += HT) {
+            if (r0 < M) {
+                load_rows<MT>(tile, A_ + b * M * M, M, r0, min(HT, M - r0));
+                __syncthreads();
+#pragma unroll
+                for (int c = 0; c < MT; ++c) {
+                    if (c < r0 + HT) {                                   // rows beyond this pass: later
+                        const int hi = max(j, c), lo = min(j, c);
+                        if (hi >= r0 && hi < r0 + HT && hi < M) a[c] = tile[(hi - r0) * C::LDT + lo];
+                    }
+                }
+                __syncthreads();
+            }
         }
-        __syncthreads();
     } else {
         // a_j[c] = shift*delta + sum_i r_i Yb[i][j] Yb[i][c];  Yb rows staged through the tile
         const double* Yb = Yb_ + b * (size_t)p * M;
@@ -387,7 +411,7 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
 #pragma unroll
         for (int c = 0; c < MT; ++c) a[c] = (c == j && j < M) ? shift : 0.0;
         double gj = 0.0;
-        constexpr int RB = MT;                    // observation rows per stage (tile holds MT rows of MT)
+        constexpr int RB = RefLayout<MT>::HT;      // observation rows per stage (the region holds HT rows of MT+1)
         for (int i0 = 0; i0 < p; i0 += RB) {
             const int nr = min(RB, p - i0);
             for (int idx = j; idx < nr * MT; idx += C::NT) {
@@ -526,7 +550,7 @@ fast_apply(double* __restrict__ V_, Workspace ws, int M)
     const int nsw = ws.nsweeps[b];
     const double2* rot = ws.rot + b * ws.logcap;
 
-    load_tile<MT>(tile, V, M);
+    load_rows<MT>(tile, V, M, 0, M);
     for (int s = r; s < nsw; s += C::NT) hdr[s] = ws.hdr[b * ws.swcap + s];
     if (r < M) inv[ws.perm[b * M + r]] = r;        // output column of QL-order column c
     __syncthreads();

@@ -204,14 +204,28 @@ static int stage_T(const double* A, int M, int n, double* V, Workspace ws, cudaS
     return 0;
 }
 
-static int stage_QL(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st)
+static int g_ql_tpb = 0;                 // letkf_set_option("ql_tpb", 32/64/96): 0 = by size
+
+template <int TPB>
+static int ql_run(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st)
 {
     cudaError_t ce;
-    const size_t ql_smem = sizeof(double) * 2 * (size_t)M * QL_TPB;
-    if ((ce = allow_smem(ql_log_kernel, ql_smem)) != cudaSuccess) return (int)ce;
-    const int qblocks = (n + QL_TPB - 1) / QL_TPB;
-    KLAUNCH("ql_log_kernel", st, ql_log_kernel<<<qblocks, QL_TPB, ql_smem, st>>>(ws, M, n, w, info));
+    const size_t ql_smem = sizeof(double) * 2 * (size_t)M * TPB;
+    if ((ce = allow_smem(ql_log_kernel<TPB>, ql_smem)) != cudaSuccess) return (int)ce;
+    const int qblocks = (n + TPB - 1) / TPB;
+    KLAUNCH("ql_log_kernel", st, ql_log_kernel<TPB><<<qblocks, TPB, ql_smem, st>>>(ws, M, n, w, info));
     return 0;
+}
+
+static int stage_QL(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st)
+{
+    int tpb = g_ql_tpb ? g_ql_tpb : (M <= 64 ? 96 : 32);
+    while (tpb > 32 && sizeof(double) * 2 * (size_t)M * tpb > 200 * 1024) tpb -= 32;
+    switch (tpb) {
+        case 96: return ql_run<96>(M, n, w, info, ws, st);
+        case 64: return ql_run<64>(M, n, w, info, ws, st);
+        default: return ql_run<32>(M, n, w, info, ws, st);
+    }
 }
 
 static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws, cudaStream_t st)
@@ -245,7 +259,7 @@ static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws,
 // caller's stream with events: the caller sees plain stream order.
 struct Pipe {
     int dev = -1;
-    cudaStream_t sT[2] = {nullptr, nullptr}, sA[2] = {nullptr, nullptr};
+    cudaStream_t sT[2] = {nullptr, nullptr}, sA[4] = {};
     cudaStream_t sQ[8] = {};          // one per sub-chunk: all QL kernels of a pass run side by side
     std::vector<cudaEvent_t> ev;
     size_t used = 0;
@@ -260,8 +274,9 @@ struct Pipe {
         const int mid = (greatest < least) ? greatest + 1 : greatest;
         for (int k = 0; k < 2; ++k) {
             if ((ce = cudaStreamCreateWithPriority(&sT[k], cudaStreamNonBlocking, mid)) != cudaSuccess) return (int)ce;
-            if ((ce = cudaStreamCreateWithPriority(&sA[k], cudaStreamNonBlocking, least)) != cudaSuccess) return (int)ce;
         }
+        for (int k = 0; k < 4; ++k)
+            if ((ce = cudaStreamCreateWithPriority(&sA[k], cudaStreamNonBlocking, least)) != cudaSuccess) return (int)ce;
         for (int k = 0; k < 8; ++k)
             if ((ce = cudaStreamCreateWithPriority(&sQ[k], cudaStreamNonBlocking, greatest)) != cudaSuccess) return (int)ce;
         ev.clear();
@@ -312,7 +327,8 @@ static int run_pass(int M, int n, double* w, double* V, int* info, const Workspa
     int rc = P.init();
     if (rc) return rc;
     P.used = 0;
-    for (int k = 0; k < 2; ++k) { P.link(st, P.sT[k]); P.link(st, P.sA[k]); }
+    for (int k = 0; k < 2; ++k) P.link(st, P.sT[k]);
+    for (int k = 0; k < 4; ++k) P.link(st, P.sA[k]);
     for (int k = 0; k < nsub; ++k) P.link(st, P.sQ[k]);
     const int per = (n + nsub - 1) / nsub;
     for (int k = 0, b0 = 0; b0 < n; ++k, b0 += per) {
@@ -323,11 +339,13 @@ static int run_pass(int M, int n, double* w, double* V, int* info, const Workspa
         if ((rc = stageT(b0, nk, P.sT[s]))) return rc;
         P.link(P.sT[s], P.sQ[k]);
         if ((rc = stage_QL(M, nk, w + (size_t)b0 * M, infok, wk, P.sQ[k]))) return rc;
-        P.link(P.sQ[k], P.sA[s]);
-        if ((rc = stage_AP(M, nk, w + (size_t)b0 * M, V + (size_t)b0 * M * M, infok, wk, P.sA[s]))) return rc;
-        if ((rc = post(b0, nk, P.sA[s]))) return rc;
+        cudaStream_t sa = P.sA[k & 3];
+        P.link(P.sQ[k], sa);
+        if ((rc = stage_AP(M, nk, w + (size_t)b0 * M, V + (size_t)b0 * M * M, infok, wk, sa))) return rc;
+        if ((rc = post(b0, nk, sa))) return rc;
     }
-    for (int k = 0; k < 2; ++k) { P.link(P.sT[k], st); P.link(P.sA[k], st); }
+    for (int k = 0; k < 2; ++k) P.link(P.sT[k], st);
+    for (int k = 0; k < 4; ++k) P.link(P.sA[k], st);
     for (int k = 0; k < nsub; ++k) P.link(P.sQ[k], st);
     return 0;
 }
@@ -506,6 +524,7 @@ int letkf_set_option(const char* name, int value)
     if (!name) return -1;
     if (strcmp(name, "force_generic") == 0) { g_force_generic = value != 0; return LETKF_OK; }
     if (strcmp(name, "pipeline") == 0) { g_pipeline = value != 0; return LETKF_OK; }
+    if (strcmp(name, "ql_tpb") == 0) { g_ql_tpb = (value == 32 || value == 64 || value == 96) ? value : 0; return LETKF_OK; }
     return -1;
 }
 

@@ -14,8 +14,11 @@
 
 namespace letkf {
 
-constexpr int QL_TPB = 32;   // one warp per CTA: shared memory is 2*M*32 doubles
-
+// QL_TPB matrices per CTA (a multiple of 32; each warp is its own lockstep group): shared memory is
+// 2*M*QL_TPB doubles.  Several warps per CTA do not make the kernel faster -- they make the CTAs
+// fewer and larger, so that a QL CTA arriving on an SM full of tridiag / apply CTAs evicts ONE of
+// them for up to three warps of QL work instead of one per warp (Streams).
+template <int QL_TPB>
 __global__ void __launch_bounds__(QL_TPB)
 ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __restrict__ info)
 {
@@ -23,7 +26,7 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
     double* dsm = sm;                         // [M][32]
     double* esm = sm + (size_t)M * QL_TPB;    // [M][32]
     const unsigned FULL = 0xffffffffu;
-    const int lane = threadIdx.x;
+    const int lane = threadIdx.x;              // column of the [M][QL_TPB] arrays
     const int b0 = blockIdx.x * QL_TPB;
     const int nb = min(QL_TPB, batch - b0);
 
@@ -38,7 +41,7 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
         dsm[ii * QL_TPB + bb] = dv;
         esm[ii * QL_TPB + bb] = ev;
     }
-    __syncwarp();
+    __syncthreads();
 
     const int b = b0 + lane;
     const bool valid = lane < nb;
@@ -162,10 +165,10 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
         ws.flags[b] = overflow;
         if (info && !overflow) info[b] = st.fail;
     }
-    __syncwarp();
+    __syncthreads();
     if (ws.rot_counter) {
         const int tot = __reduce_add_sync(FULL, valid ? pos : 0);
-        if (lane == 0) atomicAdd(ws.rot_counter, (unsigned long long)tot);
+        if ((lane & 31) == 0) atomicAdd(ws.rot_counter, (unsigned long long)tot);
     }
     // coalesced store of w and perm (matrices that overflowed are rewritten by the slow path)
     const int* psm = reinterpret_cast<const int*>(esm);
