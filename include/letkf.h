@@ -104,6 +104,28 @@ int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv
 size_t letkf_analysis_workspace_bytes(int M, int p, int nstate, int batch);
 
 /*
+ * The same two operations on HOST buffers (the end-to-end form: this is what bench.py's "e2e"
+ * times).  Every array pointer is a HOST pointer with the layouts above; page-locked (pinned)
+ * memory lets the copies run asynchronously at full PCIe rate, pageable memory works but
+ * serialises them.  The library cuts the batch into chunks and pipelines host-to-device copy,
+ * kernels and device-to-host copy of neighbouring chunks on its own streams.  The device staging
+ * arena (two chunks of inputs, outputs and workspace) is allocated on first use and KEPT by the
+ * calling host thread for its next call, grown when a larger one is needed; letkf_host_release()
+ * frees it.  The call BLOCKS
+ * until the outputs are in the host buffers.  Return values as for the device forms (argument
+ * positions are those of this signature); alignment of host pointers is not required.
+ * V may alias A, Xa may alias Xb.  info / W / wbar may be NULL.
+ */
+int letkf_syev_batched_host(const double* A, int M, int batch, double* w, double* V, int* info);
+
+int letkf_analysis_batched_host(const double* Yb, const double* d, const double* rinv_loc,
+                                const double* Xb, int M, int p, int nstate, int batch, double rho,
+                                double* Xa, double* W, double* wbar, int* info);
+
+/* Frees the staging arena the host entry points keep for the calling host thread (no-op if none). */
+void letkf_host_release(void);
+
+/*
  * Measurement helper (not part of the method): runs `iters` dependent-chain-free fp64 FMA
  * rounds on every SM and writes one double per thread to `sink` (device, >= blocks*threads
  * doubles) so the work cannot be elided.  Returns the number of fp64 FMAs executed in

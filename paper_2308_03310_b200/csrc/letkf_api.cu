@@ -503,6 +503,168 @@ int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv
     return LETKF_OK;
 }
 
+// ---- host-buffer entry points -----------------------------------------------------------------
+// The batch is cut into chunks that travel H2D -> compute -> D2H on two alternating streams, so
+// the copy of chunk c+1 and the read-back of chunk c-1 overlap the kernels of chunk c (PCIe is
+// full duplex).  The device staging arena is kept by the calling host thread between calls
+// (letkf_host_release() frees it); the call returns after the last byte has reached the host.
+struct HostPipe {
+    int dev = -1;
+    cudaStream_t s[2] = {nullptr, nullptr};
+    char* arena = nullptr;        // device staging memory, grown on demand and kept between calls
+    size_t arena_bytes = 0;       // (re-allocating > 1 GB per call costs more than the whole EVD)
+    int reserve(size_t bytes)
+    {
+        if (bytes <= arena_bytes) return 0;
+        if (arena) cudaFree(arena);
+        arena = nullptr;
+        arena_bytes = 0;
+        cudaError_t ce = cudaMalloc(reinterpret_cast<void**>(&arena), bytes);
+        if (ce != cudaSuccess) return (int)ce;
+        arena_bytes = bytes;
+        return 0;
+    }
+    void release()
+    {
+        if (arena) cudaFree(arena);
+        arena = nullptr;
+        arena_bytes = 0;
+    }
+    int init()
+    {
+        int d = 0;
+        cudaError_t ce = cudaGetDevice(&d);
+        if (ce != cudaSuccess) return (int)ce;
+        if (d == dev) return 0;
+        arena = nullptr;            // memory of another device is left to that device's context
+        arena_bytes = 0;
+        for (int k = 0; k < 2; ++k)
+            if ((ce = cudaStreamCreateWithFlags(&s[k], cudaStreamNonBlocking)) != cudaSuccess) return (int)ce;
+        dev = d;
+        return 0;
+    }
+};
+static thread_local HostPipe g_hpipe;
+
+static int host_chunk(int batch)
+{
+    int c = (batch + 7) / 8;                 // eight chunks when the batch is large: the first
+                                             // copy in and the last copy out are not overlapped
+    if (c < 2048) c = 2048;                  // keep every chunk worth the inner pipeline
+    if (c > batch) c = batch;
+    return c;
+}
+
+#define CUDA_TRY(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { rc = (int)e_; goto done; } } while (0)
+
+int letkf_syev_batched_host(const double* A, int M, int batch, double* w, double* V, int* info)
+{
+    if (M < 1 || M > LETKF_MAX_M) return -2;
+    if (batch < 0) return -3;
+    if (batch == 0) return LETKF_OK;
+    if (!A) return -1;
+    if (!w) return -4;
+    if (!V) return -5;
+    int rc = g_hpipe.init();
+    if (rc) return rc;
+    const int chunk = host_chunk(batch);
+    const size_t mat = sizeof(double) * (size_t)M * M, vec = sizeof(double) * (size_t)M;
+    const size_t wsb = align_up(letkf_syev_workspace_bytes(M, chunk), 256);
+    const size_t per = align_up(mat * chunk, 256) + align_up(vec * chunk, 256) + align_up(sizeof(int) * (size_t)chunk, 256) + wsb;
+    int launches = 0;
+    if ((rc = g_hpipe.reserve(2 * per))) return rc;
+    char* arena = g_hpipe.arena;
+    for (int b0 = 0, c = 0; b0 < batch; b0 += chunk, ++c) {
+        const int n = (batch - b0 < chunk) ? batch - b0 : chunk;
+        cudaStream_t st = g_hpipe.s[c & 1];
+        char* base = arena + (size_t)(c & 1) * per;
+        double* dV = reinterpret_cast<double*>(base);
+        double* dw = reinterpret_cast<double*>(base + align_up(mat * chunk, 256));
+        int* dinfo = reinterpret_cast<int*>(reinterpret_cast<char*>(dw) + align_up(vec * chunk, 256));
+        void* dwork = reinterpret_cast<char*>(dinfo) + align_up(sizeof(int) * (size_t)chunk, 256);
+        CUDA_TRY(cudaMemcpyAsync(dV, A + (size_t)b0 * M * M, mat * n, cudaMemcpyHostToDevice, st));
+        CUDA_TRY(cudaMemsetAsync(dinfo, 0, sizeof(int) * (size_t)n, st));
+        rc = letkf_syev_batched(dV, M, n, dw, dV, dinfo, dwork, wsb, st);     // in place
+        if (rc) goto done;
+        launches += g_launches;
+        CUDA_TRY(cudaMemcpyAsync(V + (size_t)b0 * M * M, dV, mat * n, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaMemcpyAsync(w + (size_t)b0 * M, dw, vec * n, cudaMemcpyDeviceToHost, st));
+        if (info) CUDA_TRY(cudaMemcpyAsync(info + b0, dinfo, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost, st));
+    }
+done:
+    cudaStreamSynchronize(g_hpipe.s[0]);
+    cudaStreamSynchronize(g_hpipe.s[1]);
+    g_launches = launches;
+    return rc;
+}
+
+int letkf_analysis_batched_host(const double* Yb, const double* d, const double* rinv_loc,
+                                const double* Xb, int M, int p, int nstate, int batch, double rho,
+                                double* Xa, double* W, double* wbar, int* info)
+{
+    if (M < 2 || M > LETKF_MAX_M) return -5;
+    if (p < 0) return -6;
+    if (nstate < 1) return -7;
+    if (batch < 0) return -8;
+    if (!(rho > 0.0)) return -9;
+    if (batch == 0) return LETKF_OK;
+    if (p > 0 && !Yb) return -1;
+    if (p > 0 && !d) return -2;
+    if (p > 0 && !rinv_loc) return -3;
+    if (!Xb) return -4;
+    if (!Xa) return -10;
+    int rc = g_hpipe.init();
+    if (rc) return rc;
+    const int chunk = host_chunk(batch);
+    const size_t sYb = sizeof(double) * (size_t)p * M, sd = sizeof(double) * (size_t)p;
+    const size_t sX = sizeof(double) * (size_t)nstate * M, sW = sizeof(double) * (size_t)M * M;
+    const size_t sw = sizeof(double) * (size_t)M;
+    const size_t wsb = align_up(letkf_analysis_workspace_bytes(M, p, nstate, chunk), 256);
+    size_t off[8], per = 0;
+    const size_t sizes[8] = {sYb * chunk, sd * chunk, sd * chunk, sX * chunk, W ? sW * chunk : 0,
+                             wbar ? sw * chunk : 0, sizeof(int) * (size_t)chunk, wsb};
+    for (int k = 0; k < 8; ++k) { off[k] = per; per += align_up(sizes[k] ? sizes[k] : 16, 256); }
+    int launches = 0;
+    if ((rc = g_hpipe.reserve(2 * per))) return rc;
+    char* arena = g_hpipe.arena;
+    for (int b0 = 0, c = 0; b0 < batch; b0 += chunk, ++c) {
+        const int n = (batch - b0 < chunk) ? batch - b0 : chunk;
+        cudaStream_t st = g_hpipe.s[c & 1];
+        char* base = arena + (size_t)(c & 1) * per;
+        double* dYb = reinterpret_cast<double*>(base + off[0]);
+        double* dd = reinterpret_cast<double*>(base + off[1]);
+        double* dr = reinterpret_cast<double*>(base + off[2]);
+        double* dX = reinterpret_cast<double*>(base + off[3]);
+        double* dW = W ? reinterpret_cast<double*>(base + off[4]) : nullptr;
+        double* dwb = wbar ? reinterpret_cast<double*>(base + off[5]) : nullptr;
+        int* dinfo = reinterpret_cast<int*>(base + off[6]);
+        void* dwork = base + off[7];
+        if (p > 0) {
+            CUDA_TRY(cudaMemcpyAsync(dYb, Yb + (size_t)b0 * p * M, sYb * n, cudaMemcpyHostToDevice, st));
+            CUDA_TRY(cudaMemcpyAsync(dd, d + (size_t)b0 * p, sd * n, cudaMemcpyHostToDevice, st));
+            CUDA_TRY(cudaMemcpyAsync(dr, rinv_loc + (size_t)b0 * p, sd * n, cudaMemcpyHostToDevice, st));
+        }
+        CUDA_TRY(cudaMemcpyAsync(dX, Xb + (size_t)b0 * nstate * M, sX * n, cudaMemcpyHostToDevice, st));
+        CUDA_TRY(cudaMemsetAsync(dinfo, 0, sizeof(int) * (size_t)n, st));
+        rc = letkf_analysis_batched(dYb, dd, dr, dX, M, p, nstate, n, rho, dX, dW, dwb, dinfo, dwork, wsb, st);
+        if (rc) goto done;
+        launches += g_launches;
+        CUDA_TRY(cudaMemcpyAsync(Xa + (size_t)b0 * nstate * M, dX, sX * n, cudaMemcpyDeviceToHost, st));
+        if (W) CUDA_TRY(cudaMemcpyAsync(W + (size_t)b0 * M * M, dW, sW * n, cudaMemcpyDeviceToHost, st));
+        if (wbar) CUDA_TRY(cudaMemcpyAsync(wbar + (size_t)b0 * M, dwb, sw * n, cudaMemcpyDeviceToHost, st));
+        if (info) CUDA_TRY(cudaMemcpyAsync(info + b0, dinfo, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost, st));
+    }
+done:
+    cudaStreamSynchronize(g_hpipe.s[0]);
+    cudaStreamSynchronize(g_hpipe.s[1]);
+    g_launches = launches;
+    return rc;
+}
+
+#undef CUDA_TRY
+
+void letkf_host_release(void) { g_hpipe.release(); }
+
 int letkf_probe_dfma(double* sink, int blocks, int threads, int iters,
                      unsigned long long* fma_count, void* stream)
 {

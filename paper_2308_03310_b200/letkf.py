@@ -17,6 +17,7 @@ INFO_SLOWPATH = 0x40000000
 EXPORTS = (
     "letkf_syev_batched", "letkf_syev_workspace_bytes",
     "letkf_analysis_batched", "letkf_analysis_workspace_bytes",
+    "letkf_syev_batched_host", "letkf_analysis_batched_host", "letkf_host_release",
     "letkf_probe_dfma", "letkf_last_launch_count",
     "letkf_profile_enable", "letkf_profile_count", "letkf_profile_record", "letkf_profile_record_start", "letkf_profile_rotations",
     "letkf_set_option", "letkf_status_string", "letkf_version",
@@ -49,6 +50,12 @@ def load():
     lib.letkf_analysis_batched.restype = ci
     lib.letkf_analysis_workspace_bytes.argtypes = [ci, ci, ci, ci]
     lib.letkf_analysis_workspace_bytes.restype = sz
+    lib.letkf_syev_batched_host.argtypes = [vp, ci, ci, vp, vp, vp]
+    lib.letkf_syev_batched_host.restype = ci
+    lib.letkf_analysis_batched_host.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, cd, vp, vp, vp, vp]
+    lib.letkf_analysis_batched_host.restype = ci
+    lib.letkf_host_release.argtypes = []
+    lib.letkf_host_release.restype = None
     lib.letkf_probe_dfma.argtypes = [vp, ci, ci, ci, ctypes.POINTER(ctypes.c_ulonglong), vp]
     lib.letkf_probe_dfma.restype = ci
     lib.letkf_last_launch_count.argtypes = []
@@ -169,6 +176,60 @@ def analysis_batched(Yb, d, rinv_loc, Xb, rho, Xa=None, want_W=False, want_wbar=
                                         _ptr(work), wb, _stream(stream))
     _check(st, "letkf_analysis_batched")
     return dict(Xa=Xa, W=W, wbar=wbar, info=info)
+
+
+def _host_f64(t, name):
+    if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
+        raise LetkfError(f"{name} must be a contiguous float64 CPU tensor (pinned for full copy speed)")
+    return t
+
+
+def syev_batched_host(A, w=None, V=None, info=None):
+    """letkf_syev_batched_host: the EVD on HOST tensors (pinned memory recommended).  The library
+    pipelines H2D copy, kernels and D2H copy; the call blocks until w, V, info are on the host."""
+    lib = load()
+    _host_f64(A, "A")
+    batch, M, M2 = A.shape
+    if M != M2:
+        raise LetkfError("A must be [batch][M][M]")
+    pin = A.is_pinned()
+    if w is None:
+        w = torch.empty((batch, M), dtype=torch.float64, pin_memory=pin)
+    if V is None:
+        V = torch.empty((batch, M, M), dtype=torch.float64, pin_memory=pin)
+    if info is None:
+        info = torch.zeros((batch,), dtype=torch.int32, pin_memory=pin)
+    _host_f64(w, "w")
+    _host_f64(V, "V")
+    st = lib.letkf_syev_batched_host(_ptr(A), M, batch, _ptr(w), _ptr(V), _ptr(info))
+    _check(st, "letkf_syev_batched_host")
+    return w, V, info
+
+
+def analysis_batched_host(Yb, d, rinv_loc, Xb, rho, Xa=None, want_W=False, want_wbar=False, info=None):
+    """letkf_analysis_batched_host: the fused analysis on HOST tensors; blocks until done."""
+    lib = load()
+    for t, n in ((Yb, "Yb"), (d, "d"), (rinv_loc, "rinv_loc"), (Xb, "Xb")):
+        _host_f64(t, n)
+    batch, nstate, M = Xb.shape
+    p = Yb.shape[1]
+    if Yb.shape != (batch, p, M) or d.shape != (batch, p) or rinv_loc.shape != (batch, p):
+        raise LetkfError("shape mismatch: Yb[batch][p][M], d[batch][p], rinv_loc[batch][p], Xb[batch][nstate][M]")
+    pin = Xb.is_pinned()
+    if Xa is None:
+        Xa = torch.empty_like(Xb, pin_memory=pin)
+    W = torch.empty((batch, M, M), dtype=torch.float64, pin_memory=pin) if want_W else None
+    wbar = torch.empty((batch, M), dtype=torch.float64, pin_memory=pin) if want_wbar else None
+    if info is None:
+        info = torch.zeros((batch,), dtype=torch.int32, pin_memory=pin)
+    st = lib.letkf_analysis_batched_host(_ptr(Yb), _ptr(d), _ptr(rinv_loc), _ptr(Xb), M, p, nstate, batch,
+                                         float(rho), _ptr(Xa), _ptr(W), _ptr(wbar), _ptr(info))
+    _check(st, "letkf_analysis_batched_host")
+    return {"Xa": Xa, "W": W, "wbar": wbar, "info": info}
+
+
+def host_release():
+    load().letkf_host_release()
 
 
 def probe_dfma(blocks, threads, iters, stream=None):

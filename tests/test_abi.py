@@ -96,3 +96,24 @@ def test_product_never_imports_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in src and "from oracle" not in src, f
                 assert "oracle.h" not in src and "liboracle" not in src, f
+
+
+def test_host_entry_points_validate_before_touching_a_device(lib):
+    null = ctypes.c_void_p(0)
+    fake = ctypes.c_void_p(0x1000)
+    hs = lib.letkf_syev_batched_host
+    assert hs(fake, 0, 4, fake, fake, null) == -2
+    assert hs(fake, 8, -1, fake, fake, null) == -3
+    assert hs(null, 8, 0, null, null, null) == 0
+    assert hs(null, 8, 4, fake, fake, null) == -1
+    assert hs(fake, 8, 4, null, fake, null) == -4
+    assert hs(fake, 8, 4, fake, null, null) == -5
+    ha = lib.letkf_analysis_batched_host
+    assert ha(fake, fake, fake, fake, 1, 3, 2, 4, 1.1, fake, null, null, null) == -5
+    assert ha(fake, fake, fake, fake, 8, -1, 2, 4, 1.1, fake, null, null, null) == -6
+    assert ha(fake, fake, fake, fake, 8, 3, 0, 4, 1.1, fake, null, null, null) == -7
+    assert ha(fake, fake, fake, fake, 8, 3, 2, 4, 0.0, fake, null, null, null) == -9
+    assert ha(null, fake, fake, fake, 8, 3, 2, 4, 1.1, fake, null, null, null) == -1
+    assert ha(fake, fake, fake, null, 8, 3, 2, 4, 1.1, fake, null, null, null) == -4
+    assert ha(fake, fake, fake, fake, 8, 3, 2, 4, 1.1, null, null, null, null) == -10
+    assert ha(null, null, null, null, 8, 3, 2, 0, 1.1, null, null, null, null) == 0

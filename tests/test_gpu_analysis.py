@@ -124,3 +124,18 @@ def test_structural_identities_full_size(lk, oracle):
     out2 = lk.analysis_batched(t["Yb"], t["d"], t["rinv_loc"], t["Xb"], inp["rho"])
     torch.cuda.synchronize()
     assert float((out2["Xa"] - Xa).abs().max()) <= 1e-13
+
+
+def test_host_entry_point_equals_device_call(lk):
+    import torch
+    inp = wl.analysis_inputs(batch=2048 + 77, M=64, p=98, nstate=9)
+    t = {k: torch.from_numpy(inp[k]) for k in ("Yb", "d", "rinv_loc", "Xb")}
+    dev = lk.analysis_batched(t["Yb"].cuda(), t["d"].cuda(), t["rinv_loc"].cuda(), t["Xb"].cuda(),
+                              inp["rho"], want_W=True, want_wbar=True)
+    torch.cuda.synchronize()
+    host = lk.analysis_batched_host(t["Yb"].pin_memory(), t["d"].pin_memory(), t["rinv_loc"].pin_memory(),
+                                    t["Xb"].pin_memory(), inp["rho"], want_W=True, want_wbar=True)
+    for k in ("Xa", "W", "wbar", "info"):
+        assert torch.equal(host[k], dev[k].cpu()), k
+    lean = lk.analysis_batched_host(t["Yb"], t["d"], t["rinv_loc"], t["Xb"], inp["rho"])   # pageable, no W
+    assert lean["W"] is None and torch.equal(lean["Xa"], host["Xa"])

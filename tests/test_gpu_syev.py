@@ -229,3 +229,18 @@ def test_pipelined_equals_single_stream(lk):
     assert torch.equal(w0, w1) and torch.equal(V0, V1) and torch.equal(i0, i1)
     assert torch.isfinite(s)
     assert lk.last_launch_count() >= 4 * 4               # >= 4 sub-chunks x 4 kernels
+
+
+@pytest.mark.parametrize("pinned", [True, False])
+def test_host_entry_point_equals_device_call(lk, pinned):
+    """letkf_syev_batched_host (chunked H2D -> kernels -> D2H inside the library) returns bitwise
+    what the device call returns, from pinned and from pageable host memory, ragged last chunk."""
+    import torch
+    A = torch.from_numpy(wl.letkf_shaped(2 * 2048 + 300, 64, 98, config_index=902))
+    wd, Vd, idv = lk.syev_batched(A.cuda())
+    torch.cuda.synchronize()
+    Ah = A.pin_memory() if pinned else A
+    w, V, info = lk.syev_batched_host(Ah)
+    assert torch.equal(w, wd.cpu()) and torch.equal(V, Vd.cpu()) and torch.equal(info, idv.cpu())
+    w2, V2, _ = lk.syev_batched_host(Ah.clone(), V=None)          # second call reuses the streams
+    assert torch.equal(V2, V)
