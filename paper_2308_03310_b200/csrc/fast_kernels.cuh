@@ -197,30 +197,26 @@ __device__ __forceinline__ void part_barrier(int nwarps)
 }
 
 // Coalesced copy of rows [r0, r0+nr) of a row-major M x M matrix into the padded shared tile
-// (tile row = matrix row - r0); 8 loads in flight per thread (a plain load->store loop exposed
-// the full DRAM latency once per element, profiles/r01a).
+// (tile row = matrix row - r0).  Thread t owns column t: no index arithmetic beyond one add per
+// row (a flat index split by a run-time M cost an integer division per element and 17% of the
+// tridiagonalisation kernel, profiles/r01b), 8 loads in flight per thread.
 template <int MT>
 __device__ __forceinline__ void load_rows(double* tile, const double* __restrict__ G, int M, int r0, int nr)
 {
     using C = FastCfg<MT>;
-    const int n = nr * M;
-    const double* src = G + (size_t)r0 * M;
-    for (int base = threadIdx.x; base < n; base += 8 * C::NT) {
+    const int t = threadIdx.x;
+    if (t >= M) return;
+    const double* src = G + (size_t)r0 * M + t;
+    double* dst = tile + t;
+    int r = 0;
+    for (; r + 8 <= nr; r += 8) {
         double tmp[8];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
-            const int idx = base + u * C::NT;
-            tmp[u] = (idx < n) ? src[idx] : 0.0;
-        }
+        for (int u = 0; u < 8; ++u) tmp[u] = src[(size_t)(r + u) * M];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
-            const int idx = base + u * C::NT;
-            if (idx < n) {
-                const int r = idx / M, c = idx - r * M;
-                tile[r * C::LDT + c] = tmp[u];
-            }
-        }
+        for (int u = 0; u < 8; ++u) dst[(r + u) * C::LDT] = tmp[u];
     }
+    for (; r < nr; ++r) dst[r * C::LDT] = src[(size_t)r * M];
 }
 
 // Reflector storage: H_i (i-1 in [8G, 8G+7]) is only ever read over the 8(G+1) columns of its
@@ -414,9 +410,17 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
         constexpr int RB = RefLayout<MT>::HT;      // observation rows per stage (the region holds HT rows of MT+1)
         for (int i0 = 0; i0 < p; i0 += RB) {
             const int nr = min(RB, p - i0);
-            for (int idx = j; idx < nr * MT; idx += C::NT) {
-                const int r = idx / MT, c = idx - r * MT;
-                tile[idx] = (c < M) ? Yb[(size_t)(i0 + r) * M + c] : 0.0;
+            if (j < MT) {                          // thread j stages column j of every row, 8 in flight
+                const double* src = Yb + (size_t)i0 * M + j;
+                int r = 0;
+                for (; r + 8 <= nr; r += 8) {
+                    double tmp[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) tmp[u] = (j < M) ? src[(size_t)(r + u) * M] : 0.0;
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) tile[(r + u) * MT + j] = tmp[u];
+                }
+                for (; r < nr; ++r) tile[r * MT + j] = (j < M) ? src[(size_t)r * M] : 0.0;
             }
             __syncthreads();
             for (int r = 0; r < nr; ++r) {
@@ -604,9 +608,9 @@ fast_apply(double* __restrict__ V_, Workspace ws, int M)
             if (c < M) tile[r * C::LDT + inv[c]] = z[c];
     }
     __syncthreads();
-    for (int idx = r; idx < M * M; idx += C::NT) {
-        const int rr = idx / M, c = idx - rr * M;
-        V[idx] = tile[rr * C::LDT + c];
+    if (r < M) {                                   // thread r writes column r of every row: coalesced
+#pragma unroll 8
+        for (int rr = 0; rr < M; ++rr) V[(size_t)rr * M + r] = tile[rr * C::LDT + r];
     }
 }
 
