@@ -488,10 +488,11 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
 // a5: V = Q Z by replaying the logged rotations; thread r owns row r of Q in registers.
 // Dynamic shared memory: tile[MT*(MT+1)], cs[2][MT] double2, hdr[swcap] u32, inv[MT] int
 constexpr int AP_S = 4;      // sweeps staged per barrier round
-template <int MT> __host__ __device__ constexpr int ap_tile_doubles() { return (MT * (MT + 1) + 3) & ~1; }
+// tile of fast_apply: HT = min(MT, 32) padded rows (the matrix passes through it 32 rows at a time)
+template <int MT> __host__ __device__ constexpr int ap_tile_doubles() { return ((MT < 32 ? MT : 32) * (MT + 1) + 3) & ~1; }
 template <int MT> size_t fast_apply_smem(int swcap)
 {
-    static_assert(4 * AP_S * MT <= MT * (MT + 1), "the staged rotations alias the tile");
+    static_assert(4 * AP_S * MT <= ap_tile_doubles<MT>(), "the staged rotations alias the tile");
     return sizeof(double) * (size_t)ap_tile_doubles<MT>() + sizeof(uint32_t) * (size_t)swcap + sizeof(int) * MT + 16;
 }
 
@@ -554,13 +555,24 @@ fast_apply(double* __restrict__ V_, Workspace ws, int M)
     const int nsw = ws.nsweeps[b];
     const double2* rot = ws.rot + b * ws.logcap;
 
-    load_rows<MT>(tile, V, M, 0, M);
+    constexpr int HT = MT < 32 ? MT : 32;          // rows per pass through the tile
     for (int s = r; s < nsw; s += C::NT) hdr[s] = ws.hdr[b * ws.swcap + s];
     if (r < M) inv[ws.perm[b * M + r]] = r;        // output column of QL-order column c
-    __syncthreads();
     double z[MT];
 #pragma unroll
-    for (int c = 0; c < MT; ++c) z[c] = (r < M && c < M) ? tile[r * C::LDT + c] : 0.0;
+    for (int c = 0; c < MT; ++c) z[c] = 0.0;
+#pragma unroll
+    for (int r0 = 0; r0 < MT; r0 += HT) {
+        if (r0 < M) {
+            load_rows<MT>(tile, V, M, r0, min(HT, M - r0));
+            __syncthreads();
+            if (r >= r0 && r < r0 + HT && r < M) {
+#pragma unroll
+                for (int c = 0; c < MT; ++c) z[c] = (c < M) ? tile[(r - r0) * C::LDT + c] : 0.0;
+            }
+            __syncthreads();
+        }
+    }
 
     // The (c, s) of AP_S sweeps are staged per barrier round, double-buffered: thread r copies the
     // rotation that acts on columns (r, r+1) of each sweep straight from the log into shared
@@ -584,8 +596,7 @@ fast_apply(double* __restrict__ V_, Workspace ws, int M)
         }
     };
     const int nrounds = (nsw + AP_S - 1) / AP_S;
-    __syncthreads();                                // every row has left the tile: reuse it for cs
-    if (nrounds > 0) stage(0);
+    if (nrounds > 0) stage(0);                      // every row has left the tile: it now holds cs
     cp_async_wait_all();
     __syncthreads();
     for (int k = 0; k < nrounds; ++k) {
@@ -601,16 +612,23 @@ fast_apply(double* __restrict__ V_, Workspace ws, int M)
         __syncthreads();
     }
 
-    // sorted, row-major V through the tile
-    if (r < M) {
+    // sorted, row-major V through the tile, HT rows per pass
 #pragma unroll
-        for (int c = 0; c < MT; ++c)
-            if (c < M) tile[r * C::LDT + inv[c]] = z[c];
-    }
-    __syncthreads();
-    if (r < M) {                                   // thread r writes column r of every row: coalesced
+    for (int r0 = 0; r0 < MT; r0 += HT) {
+        if (r0 < M) {
+            if (r >= r0 && r < r0 + HT && r < M) {
+#pragma unroll
+                for (int c = 0; c < MT; ++c)
+                    if (c < M) tile[(r - r0) * C::LDT + inv[c]] = z[c];
+            }
+            __syncthreads();
+            if (r < M) {                           // thread r writes column r of every row: coalesced
+                const int nr = min(HT, M - r0);
 #pragma unroll 8
-        for (int rr = 0; rr < M; ++rr) V[(size_t)rr * M + r] = tile[rr * C::LDT + r];
+                for (int rr = 0; rr < nr; ++rr) V[(size_t)(r0 + rr) * M + r] = tile[rr * C::LDT + r];
+            }
+            __syncthreads();
+        }
     }
 }
 

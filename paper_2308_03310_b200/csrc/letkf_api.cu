@@ -219,7 +219,7 @@ static int ql_run(int M, int n, double* w, int* info, Workspace ws, cudaStream_t
 
 static int stage_QL(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st)
 {
-    int tpb = g_ql_tpb ? g_ql_tpb : (M <= 64 ? 96 : 32);
+    int tpb = g_ql_tpb ? g_ql_tpb : (M <= 64 ? 64 : 32);
     while (tpb > 32 && sizeof(double) * 2 * (size_t)M * tpb > 200 * 1024) tpb -= 32;
     switch (tpb) {
         case 96: return ql_run<96>(M, n, w, info, ws, st);
