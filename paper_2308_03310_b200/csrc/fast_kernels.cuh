@@ -490,6 +490,24 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
 constexpr int AP_S = 4;      // sweeps staged per barrier round
 // tile of fast_apply: HT = min(MT, 32) padded rows (the matrix passes through it 32 rows at a time)
 template <int MT> __host__ __device__ constexpr int ap_tile_doubles() { return ((MT < 32 ? MT : 32) * (MT + 1) + 3) & ~1; }
+// a6-a9 fused into the tail of fast_apply (the analysis call when W is not wanted): V never
+// goes to HBM.  lam = eigenvalues ascending (output order), g = Yb^T (r o d), Eq.14.
+struct EpiArgs {
+    const double* lam;    // [n][M]
+    const double* g;      // [n][M]
+    const double* Xb;     // [n][ns][M]
+    double*       Xa;     // [n][ns][M]
+    double*       wbar;   // [n][M] or NULL
+    int           ns;
+};
+constexpr int EPI_QC = 5;          // right-hand sides accumulated per pass over V
+constexpr int EPI_NS_MAX = 15;     // fused epilogue for nstate <= 15, generic_epilogue beyond
+// extra doubles of dynamic shared memory: Bm[MT][ns+1], Tm[ns+1][MT], xbar[ns], cvec[ns]
+template <int MT> size_t fast_epi_smem(int ns)
+{
+    return sizeof(double) * (2 * (size_t)MT * (ns + 1) + 2 * (size_t)ns + 4);
+}
+
 template <int MT> size_t fast_apply_smem(int swcap)
 {
     static_assert(4 * AP_S * MT <= ap_tile_doubles<MT>(), "the staged rotations alias the tile");
@@ -538,9 +556,9 @@ __device__ __forceinline__ void apply_sweep(double (&z)[MT], const double2* cs, 
     }
 }
 
-template <int MT>
+template <int MT, bool EPI>
 __global__ void __launch_bounds__(FastCfg<MT>::NT, (MT == 64) ? 6 : (MT == 48 ? 8 : 16))
-fast_apply(double* __restrict__ V_, Workspace ws, int M)
+fast_apply(double* __restrict__ V_, Workspace ws, int M, EpiArgs ep)
 {
     using C = FastCfg<MT>;
     extern __shared__ __align__(16) double sm[];
@@ -612,22 +630,129 @@ fast_apply(double* __restrict__ V_, Workspace ws, int M)
         __syncthreads();
     }
 
-    // sorted, row-major V through the tile, HT rows per pass
+    if constexpr (!EPI) {
+        // sorted, row-major V through the tile, HT rows per pass
 #pragma unroll
-    for (int r0 = 0; r0 < MT; r0 += HT) {
-        if (r0 < M) {
-            if (r >= r0 && r < r0 + HT && r < M) {
+        for (int r0 = 0; r0 < MT; r0 += HT) {
+            if (r0 < M) {
+                if (r >= r0 && r < r0 + HT && r < M) {
 #pragma unroll
-                for (int c = 0; c < MT; ++c)
-                    if (c < M) tile[(r - r0) * C::LDT + inv[c]] = z[c];
-            }
-            __syncthreads();
-            if (r < M) {                           // thread r writes column r of every row: coalesced
-                const int nr = min(HT, M - r0);
+                    for (int c = 0; c < MT; ++c)
+                        if (c < M) tile[(r - r0) * C::LDT + inv[c]] = z[c];
+                }
+                __syncthreads();
+                if (r < M) {                       // thread r writes column r of every row: coalesced
+                    const int nr = min(HT, M - r0);
 #pragma unroll 8
-                for (int rr = 0; rr < nr; ++rr) V[(size_t)(r0 + rr) * M + r] = tile[rr * C::LDT + r];
+                    for (int rr = 0; rr < nr; ++rr) V[(size_t)(r0 + rr) * M + r] = tile[rr * C::LDT + r];
+                }
+                __syncthreads();
             }
-            __syncthreads();
+        }
+    } else {
+        // ---- a6-a9 on the V held in registers (row r of V in QL column order; the order of the
+        // columns is irrelevant to sums over k as long as lam_k follows it: lam_k = lam[inv[k]]).
+        //   T[q][k] = sum_r V[r][k] B[r][q],  B = [g | dX^T]               (reduction over rows:
+        //             through the tile, thread k owns column k)
+        //   t'_k = T[0][k]/lam_k,  U'[s][k] = sqrt(M-1) T[1+s][k]/sqrt(lam_k)
+        //   c_s = sum_k T[1+s][k] t'_k  (= dX_s . wbar),  wbar_m = sum_k V[m][k] t'_k
+        //   Xa[s][m] = xbar_s + c_s + sum_k U'[s][k] V[m][k]                 (thread m owns row m)
+        const int ns = ep.ns, nq = ns + 1;
+        double* Bm   = reinterpret_cast<double*>(                            // [MT][nq], 16-byte aligned
+            (reinterpret_cast<uintptr_t>(inv + MT) + 15) & ~static_cast<uintptr_t>(15));
+        double* Tm   = Bm + (size_t)MT * nq;                                // [nq][MT]
+        double* xbar = Tm + (size_t)MT * nq;                                // [ns]
+        double* cvec = xbar + ns;                                           // [ns]
+        const double* Xb = ep.Xb + b * (size_t)ns * M;
+        const int lane = r & 31, warp = r >> 5;
+        for (int s = warp; s < ns; s += C::NW) {                            // Eq.9-11
+            double acc = 0.0;
+            for (int m = lane; m < M; m += 32) acc += Xb[(size_t)s * M + m];
+            acc = warp_sum(acc) / (double)M;
+            if (lane == 0) xbar[s] = acc;
+            for (int m = lane; m < MT; m += 32) Bm[m * nq + 1 + s] = (m < M) ? Xb[(size_t)s * M + m] - acc : 0.0;
+        }
+        if (r < MT) Bm[r * nq] = (r < M) ? ep.g[b * M + r] : 0.0;
+        const double lamk = (r < M) ? ep.lam[b * M + inv[r]] : 1.0;
+        for (int q0 = 0; q0 < nq; q0 += EPI_QC) {
+            double acc[EPI_QC];
+#pragma unroll
+            for (int u = 0; u < EPI_QC; ++u) acc[u] = 0.0;
+#pragma unroll
+            for (int r0 = 0; r0 < MT; r0 += HT) {
+                if (r0 < M) {
+                    __syncthreads();                                        // tile free, Bm visible
+                    if (r >= r0 && r < r0 + HT) {
+#pragma unroll
+                        for (int c = 0; c < MT; ++c) tile[(r - r0) * C::LDT + c] = z[c];
+                    }
+                    __syncthreads();
+                    if (r < MT) {
+                        const int nr = min(HT, M - r0);
+                        for (int rr = 0; rr < nr; ++rr) {
+                            const double v = tile[rr * C::LDT + r];
+                            const double* brow = Bm + (r0 + rr) * nq + q0;
+#pragma unroll
+                            for (int u = 0; u < EPI_QC; ++u)
+                                if (q0 + u < nq) acc[u] = fma(v, brow[u], acc[u]);
+                        }
+                    }
+                }
+            }
+            if (r < MT) {
+#pragma unroll
+                for (int u = 0; u < EPI_QC; ++u)
+                    if (q0 + u < nq) Tm[(q0 + u) * MT + r] = acc[u];            // raw T[q][k]
+            }
+        }
+        __syncthreads();
+        // c_s = sum_k T[1+s][k] T[0][k] / lam_k : thread s sums its row (four partial sums)
+        const double tk = (r < M) ? Tm[r] / lamk : 0.0;
+        const double sk = (r < M) ? sqrt((double)(M - 1)) * rsqrt(lamk) : 0.0;
+        __syncthreads();
+        if (r < MT) {
+            Tm[r] = tk;                                                     // t'_k
+            // products for c_s go to the tile (free again), scaled rows stay in Tm
+            for (int s = 0; s < ns; ++s) {
+                const double raw = Tm[(1 + s) * MT + r];
+                tile[s * C::LDT + r] = raw * tk;
+                Tm[(1 + s) * MT + r] = raw * sk;                            // U'[s][k]
+            }
+        }
+        __syncthreads();
+        if (r < ns) {
+            double c0 = 0.0, c1 = 0.0, c2 = 0.0, c3 = 0.0;
+            for (int k = 0; k + 3 < MT; k += 4) {
+                c0 += tile[r * C::LDT + k];     c1 += tile[r * C::LDT + k + 1];
+                c2 += tile[r * C::LDT + k + 2]; c3 += tile[r * C::LDT + k + 3];
+            }
+            cvec[r] = (c0 + c1) + (c2 + c3);
+        }
+        __syncthreads();
+        if (r < M) {
+            double* Xa = ep.Xa + b * (size_t)ns * M;
+            if (ep.wbar) {
+                double a0 = 0.0, a1 = 0.0;
+                const double2* t2 = reinterpret_cast<const double2*>(Tm);
+#pragma unroll
+                for (int k = 0; k < MT; k += 2) {
+                    const double2 t = t2[k >> 1];
+                    a0 = fma(z[k], t.x, a0);
+                    if (k + 1 < MT) a1 = fma(z[k + 1], t.y, a1);
+                }
+                ep.wbar[b * M + r] = a0 + a1;
+            }
+            for (int s = 0; s < ns; ++s) {
+                double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+                const double2* u2 = reinterpret_cast<const double2*>(Tm + (1 + s) * MT);
+#pragma unroll
+                for (int k = 0; k < MT; k += 4) {
+                    const double2 t = u2[k >> 1], u = u2[(k >> 1) + 1];
+                    a0 = fma(z[k], t.x, a0);     a1 = fma(z[k + 1], t.y, a1);
+                    a2 = fma(z[k + 2], u.x, a2); a3 = fma(z[k + 3], u.y, a3);
+                }
+                Xa[(size_t)s * M + r] = xbar[s] + cvec[s] + ((a0 + a1) + (a2 + a3));
+            }
         }
     }
 }

@@ -328,10 +328,10 @@ generic_gram(const double* __restrict__ Yb_, const double* __restrict__ d_,
 //   Xa    = xbar 1^T + (dX wbar) 1^T + sqrt(M-1) ((dX V) diag(lam^-1/2)) V^T  Eq.13, without
 //           forming W: dX W = ((dX V) Lam^-1/2) V^T  (same product, associativity only)
 // Dynamic shared memory: t[M], wb[M], xbar[ns], cs[ns], T1[ns][M], dX[ns][M]
-__global__ void __launch_bounds__(256)
-generic_epilogue(const double* __restrict__ V_, const double* __restrict__ lam_,
-                 const double* __restrict__ g_, const double* Xb_, int M, int ns,
-                 double* Xa_, double* __restrict__ W_, double* __restrict__ wbar_)
+__device__ __forceinline__ void
+generic_epilogue_one(const double* __restrict__ V_, const double* __restrict__ lam_,
+                     const double* __restrict__ g_, const double* Xb_, int M, int ns,
+                     double* Xa_, double* __restrict__ W_, double* __restrict__ wbar_, size_t b)
 {
     extern __shared__ double sm[];
     double* t    = sm;
@@ -340,7 +340,6 @@ generic_epilogue(const double* __restrict__ V_, const double* __restrict__ lam_,
     double* cs   = xbar + ns;
     double* T1   = cs + ns;
     double* dX   = T1 + (size_t)ns * M;
-    const size_t b = blockIdx.x;
     const double* V = V_ + b * (size_t)M * M;
     const double* lam = lam_ + b * M;
     const double* g = g_ + b * M;
@@ -422,6 +421,21 @@ generic_epilogue(const double* __restrict__ V_, const double* __restrict__ lam_,
                         if (m < M && n < M) W[(size_t)m * M + n] = acc[a][c];
                     }
             }
+    }
+}
+
+// Grid-stride over the n grid points of the pass.  flags != NULL: only the points whose EVD was
+// finished by the slow path (the others had a6-a9 fused into fast_apply).
+__global__ void __launch_bounds__(256)
+generic_epilogue(const double* __restrict__ V_, const double* __restrict__ lam_,
+                 const double* __restrict__ g_, const double* Xb_, int M, int ns, int n,
+                 double* Xa_, double* __restrict__ W_, double* __restrict__ wbar_,
+                 const int* __restrict__ flags)
+{
+    for (size_t b = blockIdx.x; b < (size_t)n; b += gridDim.x) {
+        if (flags && !flags[b]) continue;
+        generic_epilogue_one(V_, lam_, g_, Xb_, M, ns, Xa_, W_, wbar_, b);
+        __syncthreads();
     }
 }
 

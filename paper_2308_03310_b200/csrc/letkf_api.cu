@@ -170,12 +170,18 @@ static int fast_tridiag_run(const double* A, double* V, Workspace ws, int M, int
 }
 
 template <int MT>
-static int fast_apply_run(double* V, Workspace ws, int M, int n, cudaStream_t st)
+static int fast_apply_run(double* V, Workspace ws, int M, int n, cudaStream_t st, const EpiArgs* ep)
 {
-    const size_t smem = fast_apply_smem<MT>(ws.swcap);
     cudaError_t ce;
-    if ((ce = allow_smem(fast_apply<MT>, smem)) != cudaSuccess) return (int)ce;
-    KLAUNCH("fast_apply", st, fast_apply<MT><<<n, FastCfg<MT>::NT, smem, st>>>(V, ws, M));
+    if (ep) {
+        const size_t smem = fast_apply_smem<MT>(ws.swcap) + fast_epi_smem<MT>(ep->ns);
+        if ((ce = allow_smem(fast_apply<MT, true>, smem)) != cudaSuccess) return (int)ce;
+        KLAUNCH("fast_apply<epilogue>", st, fast_apply<MT, true><<<n, FastCfg<MT>::NT, smem, st>>>(V, ws, M, *ep));
+    } else {
+        const size_t smem = fast_apply_smem<MT>(ws.swcap);
+        if ((ce = allow_smem(fast_apply<MT, false>, smem)) != cudaSuccess) return (int)ce;
+        KLAUNCH("fast_apply", st, fast_apply<MT, false><<<n, FastCfg<MT>::NT, smem, st>>>(V, ws, M, EpiArgs{}));
+    }
     return 0;
 }
 
@@ -228,16 +234,17 @@ static int stage_QL(int M, int n, double* w, int* info, Workspace ws, cudaStream
     }
 }
 
-static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws, cudaStream_t st)
+static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws, cudaStream_t st,
+                    const EpiArgs* ep = nullptr)
 {
     const size_t ap_smem = sizeof(double) * (5 * (size_t)M + 2 * 32 * 33);
     if (fast_supported(M) && !g_force_generic) {
         int rc = 0;
         switch (fast_bucket(M)) {
-            case 16: rc = fast_apply_run<16>(V, ws, M, n, st); break;
-            case 32: rc = fast_apply_run<32>(V, ws, M, n, st); break;
-            case 48: rc = fast_apply_run<48>(V, ws, M, n, st); break;
-            default: rc = fast_apply_run<64>(V, ws, M, n, st); break;
+            case 16: rc = fast_apply_run<16>(V, ws, M, n, st, ep); break;
+            case 32: rc = fast_apply_run<32>(V, ws, M, n, st, ep); break;
+            case 48: rc = fast_apply_run<48>(V, ws, M, n, st, ep); break;
+            default: rc = fast_apply_run<64>(V, ws, M, n, st, ep); break;
         }
         if (rc) return rc;
         // finisher for matrices whose rotation log overflowed (normally none: exits at once)
@@ -310,9 +317,21 @@ static const int PIPE_MAX_SUB = 8;       // = number of QL streams
 // One pass: n matrices whose workspace records are ws[0..n).  stageT(b0, nk, stream) enqueues the
 // first stage of matrices [b0, b0+nk); post(b0, nk, stream) whatever follows stage_AP (the
 // analysis epilogue) or nothing.
+static EpiArgs epi_slice(const EpiArgs& e, int M, int b0)
+{
+    EpiArgs s = e;
+    s.lam += (size_t)b0 * M;
+    s.g += (size_t)b0 * M;
+    s.Xb += (size_t)b0 * e.ns * M;
+    s.Xa += (size_t)b0 * e.ns * M;
+    if (s.wbar) s.wbar += (size_t)b0 * M;
+    return s;
+}
+
+// ep0: a6-a9 fused into the apply kernel (pointers of matrix 0 of the pass), or NULL.
 template <class FT, class FP>
 static int run_pass(int M, int n, double* w, double* V, int* info, const Workspace& ws,
-                    cudaStream_t st, FT stageT, FP post)
+                    cudaStream_t st, FT stageT, FP post, const EpiArgs* ep0 = nullptr)
 {
     int nsub = (g_pipeline && (!g_prof.on || g_prof.keep_pipeline)) ? n / PIPE_MIN_SUB : 1;
     if (nsub > PIPE_MAX_SUB) nsub = PIPE_MAX_SUB;
@@ -320,7 +339,7 @@ static int run_pass(int M, int n, double* w, double* V, int* info, const Workspa
         int rc = stageT(0, n, st);
         if (rc) return rc;
         if ((rc = stage_QL(M, n, w, info, ws, st))) return rc;
-        if ((rc = stage_AP(M, n, w, V, info, ws, st))) return rc;
+        if ((rc = stage_AP(M, n, w, V, info, ws, st, ep0))) return rc;
         return post(0, n, st);
     }
     Pipe& P = g_pipe;
@@ -341,7 +360,9 @@ static int run_pass(int M, int n, double* w, double* V, int* info, const Workspa
         if ((rc = stage_QL(M, nk, w + (size_t)b0 * M, infok, wk, P.sQ[k]))) return rc;
         cudaStream_t sa = P.sA[k & 3];
         P.link(P.sQ[k], sa);
-        if ((rc = stage_AP(M, nk, w + (size_t)b0 * M, V + (size_t)b0 * M * M, infok, wk, sa))) return rc;
+        EpiArgs epk;
+        if (ep0) epk = epi_slice(*ep0, M, b0);
+        if ((rc = stage_AP(M, nk, w + (size_t)b0 * M, V + (size_t)b0 * M * M, infok, wk, sa, ep0 ? &epk : nullptr))) return rc;
         if ((rc = post(b0, nk, sa))) return rc;
     }
     for (int k = 0; k < 2; ++k) P.link(P.sT[k], st);
@@ -489,15 +510,21 @@ int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv
             double* Vk = Vbuf + (size_t)c0 * M * M;
             return stage_T(Vk, M, nk, Vk, ws_slice(ws, M, c0), s, &ga);
         };
+        // a6-a9: fused into fast_apply when W is not wanted (V then never leaves the SM); the
+        // any-M kernel otherwise, and for the grid points the slow path finished.
+        const bool fused = !Wc && fast_supported(M) && !g_force_generic && nstate <= EPI_NS_MAX;
         auto post = [&](int c0, int nk, cudaStream_t s) -> int {
-            KLAUNCH("generic_epilogue", s,
-                    generic_epilogue<<<nk, 256, ep_smem, s>>>(
+            const int grid = fused ? (nk < 296 ? nk : 296) : nk;
+            KLAUNCH(fused ? "generic_epilogue(flagged)" : "generic_epilogue", s,
+                    generic_epilogue<<<grid, 256, ep_smem, s>>>(
                         Vbuf + (size_t)c0 * M * M, lam + (size_t)c0 * M, gbuf + (size_t)c0 * M,
-                        Xbc + (size_t)c0 * nstate * M, M, nstate, Xac + (size_t)c0 * nstate * M,
-                        Wc ? Wc + (size_t)c0 * M * M : nullptr, wbc ? wbc + (size_t)c0 * M : nullptr));
+                        Xbc + (size_t)c0 * nstate * M, M, nstate, nk, Xac + (size_t)c0 * nstate * M,
+                        Wc ? Wc + (size_t)c0 * M * M : nullptr, wbc ? wbc + (size_t)c0 * M : nullptr,
+                        fused ? ws.flags + c0 : nullptr));
             return 0;
         };
-        rc = run_pass(M, n, lam, Vbuf, infoc, ws, st, stageT, post);
+        EpiArgs ep{lam, gbuf, Xbc, Xac, wbc, nstate};
+        rc = run_pass(M, n, lam, Vbuf, infoc, ws, st, stageT, post, fused ? &ep : nullptr);
         if (rc) return rc;
     }
     return LETKF_OK;

@@ -137,5 +137,29 @@ def test_host_entry_point_equals_device_call(lk):
                                     t["Xb"].pin_memory(), inp["rho"], want_W=True, want_wbar=True)
     for k in ("Xa", "W", "wbar", "info"):
         assert torch.equal(host[k], dev[k].cpu()), k
+    # without W the epilogue is fused into the apply kernel (another summation order): bitwise
+    # equal to the device call of the same form, and within tolerance of the W form
     lean = lk.analysis_batched_host(t["Yb"], t["d"], t["rinv_loc"], t["Xb"], inp["rho"])   # pageable, no W
-    assert lean["W"] is None and torch.equal(lean["Xa"], host["Xa"])
+    dev_lean = lk.analysis_batched(t["Yb"].cuda(), t["d"].cuda(), t["rinv_loc"].cuda(), t["Xb"].cuda(), inp["rho"])
+    torch.cuda.synchronize()
+    assert lean["W"] is None and torch.equal(lean["Xa"], dev_lean["Xa"].cpu())
+    num = (lean["Xa"] - host["Xa"]).flatten(1).norm(dim=1)
+    den = (host["Xa"] - t["Xb"].mean(dim=2, keepdim=True)).flatten(1).norm(dim=1)
+    assert float((num / den).max()) <= parity.TOL_ANALYSIS
+
+
+@pytest.mark.parametrize("M,p,ns,batch", [(64, 98, 9, 200), (64, 3, 9, 65), (64, 48, 9, 64), (64, 0, 9, 8),
+                                          (48, 49, 9, 100), (47, 49, 5, 33), (32, 49, 9, 100), (33, 20, 4, 21),
+                                          (16, 5, 3, 77), (17, 5, 15, 9), (6, 4, 2, 5), (2, 7, 1, 9),
+                                          (64, 98, 16, 7)])
+def test_fused_epilogue_vs_oracle(lk, oracle, M, p, ns, batch):
+    """Without W the steps a6-a9 run inside the apply kernel on the V held in registers
+    (nstate <= 15; nstate = 16 falls back to the any-M epilogue): same tolerances vs the oracle,
+    wbar included, and the same answer as the unfused form to rounding."""
+    inp = wl.analysis_inputs(batch=batch, M=M, p=p, nstate=ns, config_index=500 + M + p)
+    ref = run_oracle(oracle, inp)
+    out = run_gpu(lk, inp, want_W=False, want_wbar=True)
+    assert (out["info"] == 0).all() and out["W"] is None
+    parity.assert_analysis(out, ref, inp["Xb"], f"fused M={M} p={p} ns={ns}")
+    full = run_gpu(lk, inp, want_W=True, want_wbar=True)
+    parity.assert_analysis(out, full, inp["Xb"], f"fused vs unfused M={M} p={p} ns={ns}")
