@@ -27,6 +27,10 @@ if ROOT not in sys.path:
 
 METRIC = "batched fp64 syev matrices/s at M=64 (batch 16384); % of FP64/HBM roofline"
 M_HEAD, BATCH_HEAD, P_HEAD = 64, 16384, 98
+# dram__bytes_read.sum + dram__bytes_write.sum per whole-batch launch (config 3) from the ncu --set full
+# capture kept in profiles/r01b_ncu_key_metrics.txt (bytes; ncu runs are never timed)
+NCU_DRAM_BYTES = {"fast_tridiag_formq": 0.537065e9 + 0.503918e9, "ql_log_kernel": 0.026824e9 + 1.110788e9,
+                  "fast_apply": 1.693477e9 + 0.502282e9}
 SM_COUNT = 148
 DFMA_PER_CLK_SM = 64          # fp64 FMA lanes per SM (4 SMSPs x 16), DESIGN.md section 6
 
@@ -334,7 +338,10 @@ def run_ours(args):
 
     roofline = {
         "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-        "frac": achieved / peak_tflops, "traffic": None,
+        "frac": achieved / peak_tflops, "traffic": NCU_DRAM_BYTES.get(dom),
+        "traffic_unit": "bytes per launch (whole batch), ncu dram read+write, profiles/r01b_ncu_key_metrics.txt",
+        "algorithmic_bytes": {"fast_tridiag_formq": 16.0 * M * M * B, "ql_log_kernel": 16.0 * rot_per_matrix * B,
+                              "fast_apply": (16.0 * M * M + 16.0 * rot_per_matrix) * B}.get(dom),
         "peak_source": f"derived: {SM_COUNT} SMs x {DFMA_PER_CLK_SM} DFMA/clk x 2 x {sm_max:.0f} MHz (DESIGN.md 6)",
         "dfma_probe_tflops": dfma_measured,
         "kernel_ms": kern_ms, "kernel_share": {k: v / sum(kern_ms.values()) for k, v in kern_ms.items()},
@@ -413,7 +420,41 @@ def run_ours(args):
                 "gpu_launches_per_step": letkf.last_launch_count(),
                 "model_tflops": fl * B / (ams * 1e-3) / 1e12, "frac_of_fp64_peak": fl * B / (ams * 1e-3) / 1e12 / peak_tflops,
                 "hbm_gbs": analysis_bytes(M, p, 9) * B / (ams * 1e-3) / 1e9}
+            letkf.profile_enable(True)
+            astep()
+            line["analysis"]["kernel_ms"] = {k: round(v, 4) for k, v in letkf.profile_records()}
+            letkf.profile_enable(False)
             del t, Xa, awork, inp
+        # ---- config 5: EVD size sweep, batch = floor(2^26 / M^2), LETKF-shaped
+        if not args.no_sweep:
+            sweep = []
+            del A, V, w, work
+            torch.cuda.empty_cache()
+            for Ms in (16, 32, 48, 64, 96, 128, 192, 256):
+                Bs = (1 << 26) // (Ms * Ms)
+                As = torch.from_numpy(wl.config5(Ms, batch=Bs)).cuda()
+                ws_ = torch.empty((Bs, Ms), dtype=torch.float64, device="cuda")
+                Vs = torch.empty_like(As)
+                infos = torch.zeros((Bs,), dtype=torch.int32, device="cuda")
+                wk = torch.empty(letkf.syev_workspace_bytes(Ms, Bs), dtype=torch.uint8, device="cuda")
+                for _ in range(3):
+                    letkf.syev_batched(As, w=ws_, V=Vs, info=infos, work=wk, stream=stream)
+                torch.cuda.synchronize()
+                nrep = 3
+                e0.record(stream)
+                for _ in range(nrep):
+                    letkf.syev_batched(As, w=ws_, V=Vs, info=infos, work=wk, stream=stream)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                sms = e0.elapsed_time(e1) / nrep
+                tf = syev_model_flops(Ms) * Bs / (sms * 1e-3) / 1e12
+                sweep.append({"M": Ms, "batch": Bs, "ms": round(sms, 4), "matrices_per_s": Bs / (sms * 1e-3),
+                              "model_9M3_tflops": round(tf, 3), "frac_of_fp64_peak": round(tf / peak_tflops, 4),
+                              "path": "registers (fast_*)" if Ms <= 64 else "any-M (generic_*)",
+                              "info_nonzero": int((infos != 0).sum())})
+                del As, Vs, ws_, wk, infos
+            line["sweep"] = sweep
+            A = torch.from_numpy(A_host).cuda()
         # ---- cuSOLVER on the same matrices (comparison only)
         if not args.no_cusolver:
             try:
@@ -440,6 +481,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-analysis", action="store_true")
     ap.add_argument("--no-cusolver", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

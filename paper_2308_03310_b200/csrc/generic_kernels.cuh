@@ -261,9 +261,23 @@ __global__ void __launch_bounds__(GEN_NT)
 generic_apply(double* V_, double* __restrict__ w_, Workspace ws, int M, int n, int* __restrict__ info,
               int only_flagged, int q_rowmajor)
 {
-    for (size_t b = blockIdx.x; b < (size_t)n; b += gridDim.x) {
-        generic_apply_one(V_, w_, ws, M, info, only_flagged, q_rowmajor, b);
-        __syncthreads();
+    if (!only_flagged) {
+        for (size_t b = blockIdx.x; b < (size_t)n; b += gridDim.x) {
+            generic_apply_one(V_, w_, ws, M, info, 0, q_rowmajor, b);
+            __syncthreads();
+        }
+        return;
+    }
+    // finisher: scan the flags GEN_NT at a time, work only where one is set (normally nowhere)
+    for (size_t base = (size_t)blockIdx.x * GEN_NT; base < (size_t)n; base += (size_t)gridDim.x * GEN_NT) {
+        const size_t mine = base + threadIdx.x;
+        const int f = (mine < (size_t)n) ? ws.flags[mine] : 0;
+        if (!__syncthreads_or(f)) continue;
+        const size_t end = (base + GEN_NT < (size_t)n) ? base + GEN_NT : (size_t)n;
+        for (size_t b = base; b < end; ++b) {
+            generic_apply_one(V_, w_, ws, M, info, 1, q_rowmajor, b);
+            __syncthreads();
+        }
     }
 }
 
@@ -432,10 +446,23 @@ generic_epilogue(const double* __restrict__ V_, const double* __restrict__ lam_,
                  double* Xa_, double* __restrict__ W_, double* __restrict__ wbar_,
                  const int* __restrict__ flags)
 {
-    for (size_t b = blockIdx.x; b < (size_t)n; b += gridDim.x) {
-        if (flags && !flags[b]) continue;
-        generic_epilogue_one(V_, lam_, g_, Xb_, M, ns, Xa_, W_, wbar_, b);
-        __syncthreads();
+    if (!flags) {
+        for (size_t b = blockIdx.x; b < (size_t)n; b += gridDim.x) {
+            generic_epilogue_one(V_, lam_, g_, Xb_, M, ns, Xa_, W_, wbar_, b);
+            __syncthreads();
+        }
+        return;
+    }
+    for (size_t base = (size_t)blockIdx.x * 256; base < (size_t)n; base += (size_t)gridDim.x * 256) {
+        const size_t mine = base + threadIdx.x;
+        const int f = (mine < (size_t)n) ? flags[mine] : 0;
+        if (!__syncthreads_or(f)) continue;
+        const size_t end = (base + 256 < (size_t)n) ? base + 256 : (size_t)n;
+        for (size_t b = base; b < end; ++b) {
+            if (!flags[b]) continue;
+            generic_epilogue_one(V_, lam_, g_, Xb_, M, ns, Xa_, W_, wbar_, b);
+            __syncthreads();
+        }
     }
 }
 

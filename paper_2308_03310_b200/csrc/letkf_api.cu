@@ -575,8 +575,8 @@ static thread_local HostPipe g_hpipe;
 
 static int host_chunk(int batch)
 {
-    int c = (batch + 7) / 8;                 // eight chunks when the batch is large: the first
-                                             // copy in and the last copy out are not overlapped
+    int c = (batch + 3) / 4;                 // four chunks when the batch is large (more, smaller
+                                             // chunks starve the inner sub-chunk pipeline: measured)
     if (c < 2048) c = 2048;                  // keep every chunk worth the inner pipeline
     if (c > batch) c = batch;
     return c;
