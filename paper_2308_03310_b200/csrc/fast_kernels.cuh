@@ -164,6 +164,12 @@ __device__ __forceinline__ double block_pick(const double (&a)[MT], int k)
     return x;
 }
 
+#ifndef LETKF_PIVOT_FENCE
+#define LETKF_PIVOT_FENCE(MT) false
+#endif
+#ifndef LETKF_TRI_REGS48
+#define LETKF_TRI_REGS48 168
+#endif
 #ifndef LETKF_TRI_REGS64
 #define LETKF_TRI_REGS64 168
 #endif
@@ -302,7 +308,7 @@ __device__ __forceinline__ void pivot_group(double (&a)[MT], const TriShared& sh
         if constexpr (NP > 1) sigma += sh.red[1];
         const double alpha = sh.red[4];
         const double xj = sh.xs[j];
-        const double praw = dot_blocks<MT, G>(a, sh.xs);
+        const double praw = dot_blocks<MT, G, LETKF_PIVOT_FENCE(MT)>(a, sh.xs);
         const double acol = block_pick<MT, G>(a, k);          // A[j][i-1] before the update
         double tau = 0.0, scal = 0.0, beta = alpha;            // sigma == 0: H_i = I (reading G19)
         if (sigma != 0.0) {
@@ -326,7 +332,7 @@ __device__ __forceinline__ void pivot_group(double (&a)[MT], const TriShared& sh
 #pragma unroll
         for (int step = 0; step < (G + 1 > 5 ? G + 1 : 5); ++step) {
             if (step < 5) t += __shfl_xor_sync(FULL, t, 16 >> step);
-            if (step <= G) axpy_block<MT>(a, sh.pbuf, nvj, G - step);
+            if (step <= G) { axpy_block<MT>(a, sh.pbuf, nvj, G - step); if constexpr (LETKF_PIVOT_FENCE(MT)) __syncwarp(); }
         }
         const double nwj = fma(tau * t, vj, -pj);              // -(p_j - tau (p.v) v_j)
         axpy_block<MT>(a, sh.vbuf, nwj, G);
@@ -338,7 +344,7 @@ __device__ __forceinline__ void pivot_group(double (&a)[MT], const TriShared& sh
 #pragma unroll
         for (int step = 0; step < (G > 5 ? G : 5); ++step) {
             if (step < 5) part += __shfl_xor_sync(FULL, part, 16 >> step);
-            if (step < G) axpy_block<MT>(a, sh.vbuf, nwj, G - 1 - step);
+            if (step < G) { axpy_block<MT>(a, sh.vbuf, nwj, G - 1 - step); if constexpr (LETKF_PIVOT_FENCE(MT)) __syncwarp(); }
         }
         if (lane == 0) sh.red[warp] = part;
         part_barrier(NP);                                      // ---- B1 of the next pivot
@@ -357,7 +363,7 @@ __device__ __forceinline__ void pivot_groups_down(double (&a)[MT], const TriShar
 // a3 + explicit Q for one matrix per CTA.  gram == true: the matrix is not read from A but formed
 // from the LETKF inputs (a1, a2: Eq.17 and the right factor of Eq.14) straight into the registers.
 template <int MT, bool GRAM>
-__global__ void __launch_bounds__(FastCfg<MT>::NT) __maxnreg__((MT == 64) ? LETKF_TRI_REGS64 : (MT == 48 ? 168 : (MT == 32 ? 128 : 80)))
+__global__ void __launch_bounds__(FastCfg<MT>::NT) __maxnreg__((MT == 64) ? LETKF_TRI_REGS64 : (MT == 48 ? LETKF_TRI_REGS48 : (MT == 32 ? 128 : 80)))
 fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Workspace ws, int M,
                    const double* __restrict__ Yb_, const double* __restrict__ d_,
                    const double* __restrict__ r_, int p, double shift, double* __restrict__ gout_)

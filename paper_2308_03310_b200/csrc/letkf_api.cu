@@ -12,6 +12,7 @@
 #include "ql_kernel.cuh"
 #include "generic_kernels.cuh"
 #include "fast_kernels.cuh"
+#include "mid_kernels.cuh"
 
 namespace letkf {
 
@@ -205,6 +206,13 @@ static int stage_T(const double* A, int M, int n, double* V, Workspace ws, cudaS
                 generic_gram<<<n, 256, 0, st>>>(gram->Yb, gram->d, gram->r, M, gram->p, gram->shift, V, gram->gout));
         A = V;
     }
+    if (mid_supported(M) && !g_force_generic) {          // matrix resident in shared memory
+        cudaError_t ce;
+        const size_t smem = mid_tridiag_smem(M);
+        if ((ce = allow_smem(mid_tridiag_formq, smem)) != cudaSuccess) return (int)ce;
+        KLAUNCH("mid_tridiag_formq", st, mid_tridiag_formq<<<n, MID_TPR * mid_threads(M), smem, st>>>(A, V, ws, M));
+        return 0;
+    }
     const size_t td_smem = sizeof(double) * (4 * (size_t)M + GEN_NT / 32);
     KLAUNCH("generic_tridiag_formq", st, generic_tridiag_formq<<<n, GEN_NT, td_smem, st>>>(A, V, ws, M));
     return 0;
@@ -250,6 +258,15 @@ static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws,
         // finisher for matrices whose rotation log overflowed (normally none: exits at once)
         KLAUNCH("generic_apply(flagged)", st,
                 generic_apply<<<(n < 296 ? n : 296), GEN_NT, ap_smem, st>>>(V, w, ws, M, n, info, /*only_flagged=*/1, /*q_rowmajor=*/1));
+        return 0;
+    }
+    if (mid_supported(M) && !g_force_generic) {
+        cudaError_t ce;
+        const size_t smem = mid_apply_smem(M, ws.swcap);
+        if ((ce = allow_smem(mid_apply, smem)) != cudaSuccess) return (int)ce;
+        KLAUNCH("mid_apply", st, mid_apply<<<n, mid_threads(M), smem, st>>>(V, ws, M));
+        KLAUNCH("generic_apply(flagged)", st,
+                generic_apply<<<(n < 296 ? n : 296), GEN_NT, ap_smem, st>>>(V, w, ws, M, n, info, /*only_flagged=*/1, /*q_rowmajor=*/0));
         return 0;
     }
     KLAUNCH("generic_apply", st, generic_apply<<<n, GEN_NT, ap_smem, st>>>(V, w, ws, M, n, info, 0, 0));
