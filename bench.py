@@ -424,6 +424,24 @@ def run_ours(args):
             astep()
             line["analysis"]["kernel_ms"] = {k: round(v, 4) for k, v in letkf.profile_records()}
             letkf.profile_enable(False)
+            # end to end through letkf_analysis_batched_host (pinned host buffers, PCIe inside)
+            hp = {k: torch.from_numpy(inp[k]).pin_memory() for k in ("Yb", "d", "rinv_loc", "Xb")}
+            Xa_pin = torch.empty_like(hp["Xb"]).pin_memory()
+            letkf.analysis_batched_host(hp["Yb"], hp["d"], hp["rinv_loc"], hp["Xb"], inp["rho"], Xa=Xa_pin)
+            ksteps = min(args.steps, 3)
+            e0.record(stream)
+            for _ in range(ksteps):
+                letkf.analysis_batched_host(hp["Yb"], hp["d"], hp["rinv_loc"], hp["Xb"], inp["rho"], Xa=Xa_pin)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            hms = e0.elapsed_time(e1) / ksteps
+            assert torch.equal(Xa_pin, Xa.cpu()), "analysis e2e result differs from the device call"
+            line["analysis"]["e2e"] = {
+                "value": B / (hms * 1e-3), "unit": "grid points/s", "ms_per_step": hms,
+                "h2d_bytes_per_step": int(sum(v.numel() for v in hp.values()) * 8),
+                "d2h_bytes_per_step": int(Xa_pin.numel() * 8 + B * 4), "api": "letkf_analysis_batched_host"}
+            del hp, Xa_pin
+            letkf.host_release()
             del t, Xa, awork, inp
         # ---- config 5: EVD size sweep, batch = floor(2^26 / M^2), LETKF-shaped
         if not args.no_sweep:

@@ -107,9 +107,10 @@ size_t letkf_analysis_workspace_bytes(int M, int p, int nstate, int batch);
  * The same two operations on HOST buffers (the end-to-end form: this is what bench.py's "e2e"
  * times).  Every array pointer is a HOST pointer with the layouts above; page-locked (pinned)
  * memory lets the copies run asynchronously at full PCIe rate, pageable memory works but
- * serialises them.  The library cuts the batch into chunks and pipelines host-to-device copy,
- * kernels and device-to-host copy of neighbouring chunks on its own streams.  The device staging
- * arena (two chunks of inputs, outputs and workspace) is allocated on first use and KEPT by the
+ * serialises them.  The library copies the batch in sub-chunk by sub-chunk on a copy-in stream,
+ * starts each sub-chunk's kernels as soon as its own inputs have arrived, and reads each
+ * sub-chunk's outputs back on a copy-out stream as soon as its last kernel is done.  The device staging
+ * arena (inputs, outputs and workspace of one pass) is allocated on first use and KEPT by the
  * calling host thread for its next call, grown when a larger one is needed; letkf_host_release()
  * frees it.  The call BLOCKS
  * until the outputs are in the host buffers.  Return values as for the device forms (argument

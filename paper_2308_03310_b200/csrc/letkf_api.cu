@@ -345,13 +345,22 @@ static EpiArgs epi_slice(const EpiArgs& e, int M, int b0)
     return s;
 }
 
+// Sub-chunks of a pass of n matrices: nsub pieces of `per` matrices (the last one shorter).
+static void pass_partition(int n, int& nsub, int& per)
+{
+    nsub = (g_pipeline && (!g_prof.on || g_prof.keep_pipeline)) ? n / PIPE_MIN_SUB : 1;
+    if (nsub > PIPE_MAX_SUB) nsub = PIPE_MAX_SUB;
+    if (nsub < 1) nsub = 1;
+    per = (n + nsub - 1) / nsub;
+}
+
 // ep0: a6-a9 fused into the apply kernel (pointers of matrix 0 of the pass), or NULL.
 template <class FT, class FP>
 static int run_pass(int M, int n, double* w, double* V, int* info, const Workspace& ws,
                     cudaStream_t st, FT stageT, FP post, const EpiArgs* ep0 = nullptr)
 {
-    int nsub = (g_pipeline && (!g_prof.on || g_prof.keep_pipeline)) ? n / PIPE_MIN_SUB : 1;
-    if (nsub > PIPE_MAX_SUB) nsub = PIPE_MAX_SUB;
+    int nsub, per;
+    pass_partition(n, nsub, per);
     if (nsub < 2) {
         int rc = stageT(0, n, st);
         if (rc) return rc;
@@ -366,7 +375,6 @@ static int run_pass(int M, int n, double* w, double* V, int* info, const Workspa
     for (int k = 0; k < 2; ++k) P.link(st, P.sT[k]);
     for (int k = 0; k < 4; ++k) P.link(st, P.sA[k]);
     for (int k = 0; k < nsub; ++k) P.link(st, P.sQ[k]);
-    const int per = (n + nsub - 1) / nsub;
     for (int k = 0, b0 = 0; b0 < n; ++k, b0 += per) {
         const int nk = (n - b0 < per) ? n - b0 : per;
         const int s = k & 1;
@@ -422,6 +430,29 @@ size_t letkf_syev_workspace_bytes(int M, int batch)
     return carve(ws, nullptr, M, syev_chunk(M, batch));
 }
 
+// Hooks of the host-buffer entry points: pre(b0, nk, s) is enqueued on the stream of a sub-chunk's
+// first kernel before it (wait for the sub-chunk's inputs), post(b0, nk, s) after its last kernel
+// (start the read-back).  b0 counts from the start of the pass.
+struct PassHooks {
+    int (*pre)(void* ctx, int b0, int nk, cudaStream_t s);
+    int (*post)(void* ctx, int b0, int nk, cudaStream_t s);
+    void* ctx;
+};
+
+static thread_local const PassHooks* g_analysis_hooks = nullptr;   // set by the host entry point only
+
+// one pass (n <= syev_chunk matrices, workspace carved for them) of the EVD on device buffers
+static int syev_pass(const double* A, int M, int n, double* w, double* V, int* info, const Workspace& ws,
+                     cudaStream_t st, const PassHooks* hooks)
+{
+    auto stageT = [&](int c0, int nk, cudaStream_t s) {
+        if (hooks) { const int rc = hooks->pre(hooks->ctx, c0, nk, s); if (rc) return rc; }
+        return stage_T(A + (size_t)c0 * M * M, M, nk, V + (size_t)c0 * M * M, ws_slice(ws, M, c0), s, nullptr);
+    };
+    auto post = [&](int c0, int nk, cudaStream_t s) { return hooks ? hooks->post(hooks->ctx, c0, nk, s) : 0; };
+    return run_pass(M, n, w, V, info, ws, st, stageT, post);
+}
+
 int letkf_syev_batched(const double* A, int M, int batch, double* w, double* V, int* info,
                        void* work, size_t work_bytes, void* stream)
 {
@@ -445,13 +476,8 @@ int letkf_syev_batched(const double* A, int M, int batch, double* w, double* V, 
 
     for (int b0 = 0; b0 < batch; b0 += chunk) {
         const int n = (batch - b0 < chunk) ? batch - b0 : chunk;
-        const double* Ac = A + (size_t)b0 * M * M;
-        double* Vc = V + (size_t)b0 * M * M;
-        auto stageT = [&](int c0, int nk, cudaStream_t s) {
-            return stage_T(Ac + (size_t)c0 * M * M, M, nk, Vc + (size_t)c0 * M * M, ws_slice(ws, M, c0), s, nullptr);
-        };
-        auto post = [](int, int, cudaStream_t) { return 0; };
-        rc = run_pass(M, n, w + (size_t)b0 * M, Vc, info ? info + b0 : nullptr, ws, st, stageT, post);
+        rc = syev_pass(A + (size_t)b0 * M * M, M, n, w + (size_t)b0 * M, V + (size_t)b0 * M * M,
+                       info ? info + b0 : nullptr, ws, st, nullptr);
         if (rc) return rc;
     }
     return LETKF_OK;
@@ -522,6 +548,10 @@ int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv
         int* infoc = info ? info + b0 : nullptr;
 
         auto stageT = [&](int c0, int nk, cudaStream_t s) {
+            if (g_analysis_hooks) {
+                const int hrc = g_analysis_hooks->pre(g_analysis_hooks->ctx, b0 + c0, nk, s);
+                if (hrc) return hrc;
+            }
             GramArgs ga{Ybc + (size_t)c0 * p * M, dc + (size_t)c0 * p, rc_ + (size_t)c0 * p, p, shift,
                         gbuf + (size_t)c0 * M};
             double* Vk = Vbuf + (size_t)c0 * M * M;
@@ -538,7 +568,7 @@ int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv
                         Xbc + (size_t)c0 * nstate * M, M, nstate, nk, Xac + (size_t)c0 * nstate * M,
                         Wc ? Wc + (size_t)c0 * M * M : nullptr, wbc ? wbc + (size_t)c0 * M : nullptr,
                         fused ? ws.flags + c0 : nullptr));
-            return 0;
+            return g_analysis_hooks ? g_analysis_hooks->post(g_analysis_hooks->ctx, b0 + c0, nk, s) : 0;
         };
         EpiArgs ep{lam, gbuf, Xbc, Xac, wbc, nstate};
         rc = run_pass(M, n, lam, Vbuf, infoc, ws, st, stageT, post, fused ? &ep : nullptr);
@@ -548,13 +578,24 @@ int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv
 }
 
 // ---- host-buffer entry points -----------------------------------------------------------------
-// The batch is cut into chunks that travel H2D -> compute -> D2H on two alternating streams, so
-// the copy of chunk c+1 and the read-back of chunk c-1 overlap the kernels of chunk c (PCIe is
-// full duplex).  The device staging arena is kept by the calling host thread between calls
+// A pass of the batch lives on the device at a time; the sub-chunks of the kernel pipeline are
+// copied in one after the other on a copy-in stream, each sub-chunk's first kernel waits for its
+// own copy only, and its read-back starts on a copy-out stream as soon as its last kernel is done:
+// both copy engines and the SMs overlap (PCIe is full duplex).  The device staging arena is kept by the calling host thread between calls
 // (letkf_host_release() frees it); the call returns after the last byte has reached the host.
 struct HostPipe {
     int dev = -1;
     cudaStream_t s[2] = {nullptr, nullptr};
+    cudaStream_t sC = nullptr;    // the stream the kernels of a host call are forked from
+    std::vector<cudaEvent_t> ev;
+    void events(size_t n)
+    {
+        while (ev.size() < n) {
+            cudaEvent_t e;
+            cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+            ev.push_back(e);
+        }
+    }
     char* arena = nullptr;        // device staging memory, grown on demand and kept between calls
     size_t arena_bytes = 0;       // (re-allocating > 1 GB per call costs more than the whole EVD)
     int reserve(size_t bytes)
@@ -584,25 +625,49 @@ struct HostPipe {
         arena_bytes = 0;
         for (int k = 0; k < 2; ++k)
             if ((ce = cudaStreamCreateWithFlags(&s[k], cudaStreamNonBlocking)) != cudaSuccess) return (int)ce;
+        if ((ce = cudaStreamCreateWithFlags(&sC, cudaStreamNonBlocking)) != cudaSuccess) return (int)ce;
+        ev.clear();
         dev = d;
         return 0;
     }
 };
 static thread_local HostPipe g_hpipe;
 
-static int host_chunk(int batch)
+// context of the copy hooks of letkf_syev_batched_host
+struct SyevHostCtx {
+    int M, per;                       // sub-chunk size of the pass
+    const double* hA; double* hw; double* hV; int* hinfo;      // host, at the start of the pass
+    double* dV; double* dw; int* dinfo;                          // device, at the start of the pass
+    cudaStream_t sD;                  // read-back stream
+    std::vector<cudaEvent_t>* evH;    // evH[k]: inputs of sub-chunk k are on the device
+    std::vector<cudaEvent_t>* evC;    // evC[k]: outputs of sub-chunk k are final
+};
+static int syev_host_pre(void* c, int b0, int, cudaStream_t s)
 {
-    int c = (batch + 3) / 4;                 // four chunks when the batch is large (more, smaller
-                                             // chunks starve the inner sub-chunk pipeline: measured)
-    if (c < 2048) c = 2048;                  // keep every chunk worth the inner pipeline
-    if (c > batch) c = batch;
-    return c;
+    SyevHostCtx* x = static_cast<SyevHostCtx*>(c);
+    return (int)cudaStreamWaitEvent(s, (*x->evH)[b0 / x->per], 0);
 }
-
-#define CUDA_TRY(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { rc = (int)e_; goto done; } } while (0)
+static int syev_host_post(void* c, int b0, int nk, cudaStream_t s)
+{
+    SyevHostCtx* x = static_cast<SyevHostCtx*>(c);
+    const int M = x->M;
+    cudaEvent_t e = (*x->evC)[b0 / x->per];
+    cudaError_t ce;
+    if ((ce = cudaEventRecord(e, s)) != cudaSuccess) return (int)ce;
+    if ((ce = cudaStreamWaitEvent(x->sD, e, 0)) != cudaSuccess) return (int)ce;
+    if ((ce = cudaMemcpyAsync(x->hV + (size_t)b0 * M * M, x->dV + (size_t)b0 * M * M,
+                              sizeof(double) * (size_t)nk * M * M, cudaMemcpyDeviceToHost, x->sD)) != cudaSuccess) return (int)ce;
+    if ((ce = cudaMemcpyAsync(x->hw + (size_t)b0 * M, x->dw + (size_t)b0 * M,
+                              sizeof(double) * (size_t)nk * M, cudaMemcpyDeviceToHost, x->sD)) != cudaSuccess) return (int)ce;
+    if (x->hinfo &&
+        (ce = cudaMemcpyAsync(x->hinfo + b0, x->dinfo + b0, sizeof(int) * (size_t)nk, cudaMemcpyDeviceToHost, x->sD)) != cudaSuccess)
+        return (int)ce;
+    return 0;
+}
 
 int letkf_syev_batched_host(const double* A, int M, int batch, double* w, double* V, int* info)
 {
+    g_launches = 0;
     if (M < 1 || M > LETKF_MAX_M) return -2;
     if (batch < 0) return -3;
     if (batch == 0) return LETKF_OK;
@@ -611,41 +676,85 @@ int letkf_syev_batched_host(const double* A, int M, int batch, double* w, double
     if (!V) return -5;
     int rc = g_hpipe.init();
     if (rc) return rc;
-    const int chunk = host_chunk(batch);
+    // One pass of up to syev_chunk matrices lives on the device at a time.  Its sub-chunks (the
+    // ones the kernel pipeline uses) are copied in one after the other on the copy-in stream; each
+    // sub-chunk's first kernel waits for its own copy only, and its read-back starts on the
+    // copy-out stream as soon as its last kernel is done: both copy engines and the SMs overlap.
+    const int chunk = syev_chunk(M, batch);
     const size_t mat = sizeof(double) * (size_t)M * M, vec = sizeof(double) * (size_t)M;
-    const size_t wsb = align_up(letkf_syev_workspace_bytes(M, chunk), 256);
-    const size_t per = align_up(mat * chunk, 256) + align_up(vec * chunk, 256) + align_up(sizeof(int) * (size_t)chunk, 256) + wsb;
+    Workspace ws;
+    const size_t wsb = align_up(carve(ws, nullptr, M, chunk), 256);
+    const size_t oV = 0, ow = align_up(mat * chunk, 256), oi = ow + align_up(vec * chunk, 256);
+    const size_t owk = oi + align_up(sizeof(int) * (size_t)chunk, 256);
+    if ((rc = g_hpipe.reserve(owk + wsb))) return rc;
+    char* base = g_hpipe.arena;
+    double* dV = reinterpret_cast<double*>(base + oV);
+    double* dw = reinterpret_cast<double*>(base + ow);
+    int* dinfo = reinterpret_cast<int*>(base + oi);
+    carve(ws, base + owk, M, chunk);
+    cudaStream_t sH = g_hpipe.s[0], sD = g_hpipe.s[1], sC = g_hpipe.sC;
     int launches = 0;
-    if ((rc = g_hpipe.reserve(2 * per))) return rc;
-    char* arena = g_hpipe.arena;
-    for (int b0 = 0, c = 0; b0 < batch; b0 += chunk, ++c) {
+    for (int b0 = 0; b0 < batch && rc == 0; b0 += chunk) {
         const int n = (batch - b0 < chunk) ? batch - b0 : chunk;
-        cudaStream_t st = g_hpipe.s[c & 1];
-        char* base = arena + (size_t)(c & 1) * per;
-        double* dV = reinterpret_cast<double*>(base);
-        double* dw = reinterpret_cast<double*>(base + align_up(mat * chunk, 256));
-        int* dinfo = reinterpret_cast<int*>(reinterpret_cast<char*>(dw) + align_up(vec * chunk, 256));
-        void* dwork = reinterpret_cast<char*>(dinfo) + align_up(sizeof(int) * (size_t)chunk, 256);
-        CUDA_TRY(cudaMemcpyAsync(dV, A + (size_t)b0 * M * M, mat * n, cudaMemcpyHostToDevice, st));
-        CUDA_TRY(cudaMemsetAsync(dinfo, 0, sizeof(int) * (size_t)n, st));
-        rc = letkf_syev_batched(dV, M, n, dw, dV, dinfo, dwork, wsb, st);     // in place
-        if (rc) goto done;
+        int nsub, per;
+        prof_reset(sC);
+        pass_partition(n, nsub, per);
+        g_hpipe.events(2 * nsub);
+        std::vector<cudaEvent_t> evH(g_hpipe.ev.begin(), g_hpipe.ev.begin() + nsub);
+        std::vector<cudaEvent_t> evC(g_hpipe.ev.begin() + nsub, g_hpipe.ev.begin() + 2 * nsub);
+        for (int k = 0, c0 = 0; c0 < n; ++k, c0 += per) {
+            const int nk = (n - c0 < per) ? n - c0 : per;
+            cudaMemcpyAsync(dV + (size_t)c0 * M * M, A + (size_t)(b0 + c0) * M * M, mat * nk, cudaMemcpyHostToDevice, sH);
+            cudaEventRecord(evH[k], sH);
+        }
+        cudaMemsetAsync(dinfo, 0, sizeof(int) * (size_t)n, sC);
+        SyevHostCtx ctx{M, per, A + (size_t)b0 * M * M, w + (size_t)b0 * M, V + (size_t)b0 * M * M,
+                        info ? info + b0 : nullptr, dV, dw, dinfo, sD, &evH, &evC};
+        PassHooks hooks{syev_host_pre, syev_host_post, &ctx};
+        rc = syev_pass(dV, M, n, dw, dV, dinfo, ws, sC, &hooks);     // in place
         launches += g_launches;
-        CUDA_TRY(cudaMemcpyAsync(V + (size_t)b0 * M * M, dV, mat * n, cudaMemcpyDeviceToHost, st));
-        CUDA_TRY(cudaMemcpyAsync(w + (size_t)b0 * M, dw, vec * n, cudaMemcpyDeviceToHost, st));
-        if (info) CUDA_TRY(cudaMemcpyAsync(info + b0, dinfo, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost, st));
+        // the arena is reused by the next pass: everything of this one must have left it
+        cudaStreamSynchronize(sC);
+        cudaStreamSynchronize(sD);
+        cudaStreamSynchronize(sH);
     }
-done:
-    cudaStreamSynchronize(g_hpipe.s[0]);
-    cudaStreamSynchronize(g_hpipe.s[1]);
+    cudaError_t ce = cudaGetLastError();
+    if (rc == 0 && ce != cudaSuccess) rc = (int)ce;
     g_launches = launches;
     return rc;
+}
+
+// context of the copy hooks of letkf_analysis_batched_host: up to four output arrays
+struct AnaHostCtx {
+    int per, nout;
+    char* host[4]; const char* dev[4]; size_t bytes[4];       // per grid point, at the start of the pass
+    cudaStream_t sD;
+    std::vector<cudaEvent_t>* evH;
+    std::vector<cudaEvent_t>* evC;
+};
+static int ana_host_pre(void* c, int b0, int, cudaStream_t s)
+{
+    AnaHostCtx* x = static_cast<AnaHostCtx*>(c);
+    return (int)cudaStreamWaitEvent(s, (*x->evH)[b0 / x->per], 0);
+}
+static int ana_host_post(void* c, int b0, int nk, cudaStream_t s)
+{
+    AnaHostCtx* x = static_cast<AnaHostCtx*>(c);
+    cudaEvent_t e = (*x->evC)[b0 / x->per];
+    cudaError_t ce;
+    if ((ce = cudaEventRecord(e, s)) != cudaSuccess) return (int)ce;
+    if ((ce = cudaStreamWaitEvent(x->sD, e, 0)) != cudaSuccess) return (int)ce;
+    for (int q = 0; q < x->nout; ++q)
+        if ((ce = cudaMemcpyAsync(x->host[q] + (size_t)b0 * x->bytes[q], x->dev[q] + (size_t)b0 * x->bytes[q],
+                                  x->bytes[q] * (size_t)nk, cudaMemcpyDeviceToHost, x->sD)) != cudaSuccess) return (int)ce;
+    return 0;
 }
 
 int letkf_analysis_batched_host(const double* Yb, const double* d, const double* rinv_loc,
                                 const double* Xb, int M, int p, int nstate, int batch, double rho,
                                 double* Xa, double* W, double* wbar, int* info)
 {
+    g_launches = 0;
     if (M < 2 || M > LETKF_MAX_M) return -5;
     if (p < 0) return -6;
     if (nstate < 1) return -7;
@@ -659,53 +768,72 @@ int letkf_analysis_batched_host(const double* Yb, const double* d, const double*
     if (!Xa) return -10;
     int rc = g_hpipe.init();
     if (rc) return rc;
-    const int chunk = host_chunk(batch);
+    // as letkf_syev_batched_host: one pass on the device at a time, inputs copied in sub-chunk by
+    // sub-chunk, outputs read back as each sub-chunk's last kernel finishes
+    const int chunk = syev_chunk(M, batch);
     const size_t sYb = sizeof(double) * (size_t)p * M, sd = sizeof(double) * (size_t)p;
     const size_t sX = sizeof(double) * (size_t)nstate * M, sW = sizeof(double) * (size_t)M * M;
     const size_t sw = sizeof(double) * (size_t)M;
     const size_t wsb = align_up(letkf_analysis_workspace_bytes(M, p, nstate, chunk), 256);
-    size_t off[8], per = 0;
+    size_t off[8], total = 0;
     const size_t sizes[8] = {sYb * chunk, sd * chunk, sd * chunk, sX * chunk, W ? sW * chunk : 0,
                              wbar ? sw * chunk : 0, sizeof(int) * (size_t)chunk, wsb};
-    for (int k = 0; k < 8; ++k) { off[k] = per; per += align_up(sizes[k] ? sizes[k] : 16, 256); }
+    for (int k = 0; k < 8; ++k) { off[k] = total; total += align_up(sizes[k] ? sizes[k] : 16, 256); }
+    if ((rc = g_hpipe.reserve(total))) return rc;
+    char* base = g_hpipe.arena;
+    double* dYb = reinterpret_cast<double*>(base + off[0]);
+    double* dd = reinterpret_cast<double*>(base + off[1]);
+    double* dr = reinterpret_cast<double*>(base + off[2]);
+    double* dX = reinterpret_cast<double*>(base + off[3]);
+    double* dW = W ? reinterpret_cast<double*>(base + off[4]) : nullptr;
+    double* dwb = wbar ? reinterpret_cast<double*>(base + off[5]) : nullptr;
+    int* dinfo = reinterpret_cast<int*>(base + off[6]);
+    void* dwork = base + off[7];
+    cudaStream_t sH = g_hpipe.s[0], sD = g_hpipe.s[1], sC = g_hpipe.sC;
     int launches = 0;
-    if ((rc = g_hpipe.reserve(2 * per))) return rc;
-    char* arena = g_hpipe.arena;
-    for (int b0 = 0, c = 0; b0 < batch; b0 += chunk, ++c) {
+    for (int b0 = 0; b0 < batch && rc == 0; b0 += chunk) {
         const int n = (batch - b0 < chunk) ? batch - b0 : chunk;
-        cudaStream_t st = g_hpipe.s[c & 1];
-        char* base = arena + (size_t)(c & 1) * per;
-        double* dYb = reinterpret_cast<double*>(base + off[0]);
-        double* dd = reinterpret_cast<double*>(base + off[1]);
-        double* dr = reinterpret_cast<double*>(base + off[2]);
-        double* dX = reinterpret_cast<double*>(base + off[3]);
-        double* dW = W ? reinterpret_cast<double*>(base + off[4]) : nullptr;
-        double* dwb = wbar ? reinterpret_cast<double*>(base + off[5]) : nullptr;
-        int* dinfo = reinterpret_cast<int*>(base + off[6]);
-        void* dwork = base + off[7];
-        if (p > 0) {
-            CUDA_TRY(cudaMemcpyAsync(dYb, Yb + (size_t)b0 * p * M, sYb * n, cudaMemcpyHostToDevice, st));
-            CUDA_TRY(cudaMemcpyAsync(dd, d + (size_t)b0 * p, sd * n, cudaMemcpyHostToDevice, st));
-            CUDA_TRY(cudaMemcpyAsync(dr, rinv_loc + (size_t)b0 * p, sd * n, cudaMemcpyHostToDevice, st));
+        int nsub, per;
+        pass_partition(n, nsub, per);
+        g_hpipe.events(2 * nsub);
+        std::vector<cudaEvent_t> evH(g_hpipe.ev.begin(), g_hpipe.ev.begin() + nsub);
+        std::vector<cudaEvent_t> evC(g_hpipe.ev.begin() + nsub, g_hpipe.ev.begin() + 2 * nsub);
+        for (int k = 0, c0 = 0; c0 < n; ++k, c0 += per) {
+            const int nk = (n - c0 < per) ? n - c0 : per;
+            const size_t g0 = (size_t)(b0 + c0);
+            if (p > 0) {
+                cudaMemcpyAsync(dYb + (size_t)c0 * p * M, Yb + g0 * p * M, sYb * nk, cudaMemcpyHostToDevice, sH);
+                cudaMemcpyAsync(dd + (size_t)c0 * p, d + g0 * p, sd * nk, cudaMemcpyHostToDevice, sH);
+                cudaMemcpyAsync(dr + (size_t)c0 * p, rinv_loc + g0 * p, sd * nk, cudaMemcpyHostToDevice, sH);
+            }
+            cudaMemcpyAsync(dX + (size_t)c0 * nstate * M, Xb + g0 * nstate * M, sX * nk, cudaMemcpyHostToDevice, sH);
+            cudaEventRecord(evH[k], sH);
         }
-        CUDA_TRY(cudaMemcpyAsync(dX, Xb + (size_t)b0 * nstate * M, sX * n, cudaMemcpyHostToDevice, st));
-        CUDA_TRY(cudaMemsetAsync(dinfo, 0, sizeof(int) * (size_t)n, st));
-        rc = letkf_analysis_batched(dYb, dd, dr, dX, M, p, nstate, n, rho, dX, dW, dwb, dinfo, dwork, wsb, st);
-        if (rc) goto done;
+        cudaMemsetAsync(dinfo, 0, sizeof(int) * (size_t)n, sC);
+        AnaHostCtx ctx;
+        ctx.per = per; ctx.sD = sD; ctx.evH = &evH; ctx.evC = &evC; ctx.nout = 0;
+        auto add = [&](void* h, const void* dv, size_t bytes) {
+            ctx.host[ctx.nout] = static_cast<char*>(h); ctx.dev[ctx.nout] = static_cast<const char*>(dv);
+            ctx.bytes[ctx.nout] = bytes; ++ctx.nout;
+        };
+        add(Xa + (size_t)b0 * nstate * M, dX, sX);
+        if (W) add(W + (size_t)b0 * M * M, dW, sW);
+        if (wbar) add(wbar + (size_t)b0 * M, dwb, sw);
+        if (info) add(info + b0, dinfo, sizeof(int));
+        PassHooks hooks{ana_host_pre, ana_host_post, &ctx};
+        g_analysis_hooks = &hooks;
+        rc = letkf_analysis_batched(dYb, dd, dr, dX, M, p, nstate, n, rho, dX, dW, dwb, dinfo, dwork, wsb, sC);
+        g_analysis_hooks = nullptr;
         launches += g_launches;
-        CUDA_TRY(cudaMemcpyAsync(Xa + (size_t)b0 * nstate * M, dX, sX * n, cudaMemcpyDeviceToHost, st));
-        if (W) CUDA_TRY(cudaMemcpyAsync(W + (size_t)b0 * M * M, dW, sW * n, cudaMemcpyDeviceToHost, st));
-        if (wbar) CUDA_TRY(cudaMemcpyAsync(wbar + (size_t)b0 * M, dwb, sw * n, cudaMemcpyDeviceToHost, st));
-        if (info) CUDA_TRY(cudaMemcpyAsync(info + b0, dinfo, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost, st));
+        cudaStreamSynchronize(sC);
+        cudaStreamSynchronize(sD);
+        cudaStreamSynchronize(sH);
     }
-done:
-    cudaStreamSynchronize(g_hpipe.s[0]);
-    cudaStreamSynchronize(g_hpipe.s[1]);
+    cudaError_t ce = cudaGetLastError();
+    if (rc == 0 && ce != cudaSuccess) rc = (int)ce;
     g_launches = launches;
     return rc;
 }
-
-#undef CUDA_TRY
 
 void letkf_host_release(void) { g_hpipe.release(); }
 
