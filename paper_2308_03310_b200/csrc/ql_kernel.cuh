@@ -91,7 +91,7 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
             break;
         }
         if (!__any_sync(FULL, sweeping)) break;
-        int i = -1, mlow = m;
+        int i = -1, mlow = m, ibreak = 0;
         double g = 0.0, s = 1.0, c = 1.0, p = 0.0, dprev = 0.0;
         if (sweeping) {
             // Wilkinson shift
@@ -102,36 +102,59 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
             i = m - 1;
         }
         const int maxlen = __reduce_max_sync(FULL, sweeping ? m - l : 0);
-        // ---- lockstep rotation steps
+        // ---- lockstep rotation steps.  The kernel is bound by the dependent chain of one step
+        // (g -> r2 -> 1/sqrt -> c, s -> r -> g), so everything else is kept off it: the operands of
+        // step i-1 are loaded at the top of step i, pointers are bumped instead of recomputed, and
+        // 1/sqrt is the hardware seed plus two Newton steps whenever r2 is a normal number.
         bool broke = false;
-        double2* out = rot + pos;
+        double2* outp = rot + pos;
+        double* pd = d + (i > 0 ? i : 0) * stride;     // &d[i]
+        double* pe = e + (i > 0 ? i : 0) * stride;     // &e[i]
+        double ei = 0.0, di = 0.0, di1 = 0.0;
+        if (sweeping) { ei = pe[0]; di = pd[0]; di1 = pd[stride]; }
         for (int k = 0; k < maxlen; ++k) {
-            if (sweeping && !broke && i >= l) {
-                const double ei = QL_E(i), di = QL_D(i), di1 = QL_D(i + 1);
+            if (i >= l) {                              // (i = -1 when not sweeping, l - 1 when done or broken)
+                const int nxt = (i > l) ? -stride : 0;
+                const double ein = pe[nxt], din = pd[nxt];
                 const double f = s * ei;
                 const double b2 = c * ei;
+                const double tb = b2 + b2;
                 const double r2 = fma(f, f, g * g);
                 if (!(r2 > 0.0)) {                     // underflow / NaN: split the block at i+1
-                    QL_E(i + 1) = 0.0;
-                    QL_D(i + 1) = di1 - p;
+                    pe[stride] = 0.0;
+                    pd[stride] = di1 - p;
                     QL_E(m) = 0.0;
                     broke = true;
+                    ibreak = i;
+                    i = l - 1;
                 } else {
-                    const double rinv = rsqrt(r2);
+                    double rinv;
+                    if (r2 > 1e-280 && r2 < 1e280) {
+                        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(rinv) : "d"(r2));
+                        const double hx = 0.5 * r2;
+                        double t = fma(-hx * rinv, rinv, 0.5);
+                        rinv = fma(rinv, t, rinv);
+                        t = fma(-hx * rinv, rinv, 0.5);
+                        rinv = fma(rinv, t, rinv);
+                    } else {
+                        rinv = rsqrt(r2);
+                    }
                     const double enew = r2 * rinv;
                     s = f * rinv;
                     c = g * rinv;
-                    g = di1 - p;
-                    const double r = fma(di - g, s, 2.0 * c * b2);
+                    const double gt = di1 - p;
+                    const double r = fma(c, tb, (di - gt) * s);
                     p = s * r;
-                    const double dnew = g + p;
-                    QL_E(i + 1) = enew;
-                    QL_D(i + 1) = dnew;
+                    const double dnew = gt + p;
                     g = fma(c, r, -b2);
-                    out[m - 1 - i] = make_double2(c, s);
+                    pe[stride] = enew;
+                    pd[stride] = dnew;
+                    *outp++ = make_double2(c, s);
                     // deflation test of index i+1 on this sweep's values (d[i+2] = dprev)
                     if (i + 1 < m && fabs(enew) <= eps * (fabs(dnew) + fabs(dprev))) mlow = i + 1;
                     dprev = dnew;
+                    di1 = di; di = din; ei = ein;
+                    pd += nxt; pe += nxt;
                     --i;
                 }
             }
@@ -139,7 +162,7 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
         if (sweeping) {
             int lo;
             if (broke) {
-                lo = i + 1;
+                lo = ibreak + 1;
                 // the block was split by hand: what is left of it below i+1 is rescanned
                 if (m - lo > 0) { hdr[nsw++] = (uint32_t)lo | ((uint32_t)m << 16); pos += m - lo; }
                 m = scan_end(l);
@@ -152,7 +175,9 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
                 pos += m - l;
                 if (mlow < m) QL_E(mlow) = 0.0;
                 m = mlow;
-                if (fabs(g) <= eps * (fabs(dl) + fabs(dprev))) { QL_E(l) = 0.0; m = l; }
+                // eigenvalue l converged: the next block starts at l+1 and ends at mlow, the lowest
+                // negligible off-diagonal this sweep has seen above l -- no rescan
+                if (fabs(g) <= eps * (fabs(dl) + fabs(dprev))) { QL_E(l) = 0.0; l += 1; iter = 0; }
             }
         }
     }
