@@ -120,25 +120,28 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
                 const double b2 = c * ei;
                 const double tb = b2 + b2;
                 const double r2 = fma(f, f, g * g);
-                if (!(r2 > 0.0)) {                     // underflow / NaN: split the block at i+1
+                double rinv;
+                bool ok = true;
+                if (r2 > 1e-280 && r2 < 1e280) {       // the common case: seed + two Newton steps
+                    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(rinv) : "d"(r2));
+                    const double hx = 0.5 * r2;
+                    double t = fma(-hx * rinv, rinv, 0.5);
+                    rinv = fma(rinv, t, rinv);
+                    t = fma(-hx * rinv, rinv, 0.5);
+                    rinv = fma(rinv, t, rinv);
+                } else if (r2 > 0.0) {
+                    rinv = rsqrt(r2);
+                } else {                               // underflow / NaN: split the block at i+1
                     pe[stride] = 0.0;
                     pd[stride] = di1 - p;
                     QL_E(m) = 0.0;
                     broke = true;
                     ibreak = i;
                     i = l - 1;
-                } else {
-                    double rinv;
-                    if (r2 > 1e-280 && r2 < 1e280) {
-                        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(rinv) : "d"(r2));
-                        const double hx = 0.5 * r2;
-                        double t = fma(-hx * rinv, rinv, 0.5);
-                        rinv = fma(rinv, t, rinv);
-                        t = fma(-hx * rinv, rinv, 0.5);
-                        rinv = fma(rinv, t, rinv);
-                    } else {
-                        rinv = rsqrt(r2);
-                    }
+                    ok = false;
+                    rinv = 0.0;
+                }
+                if (ok) {
                     const double enew = r2 * rinv;
                     s = f * rinv;
                     c = g * rinv;
