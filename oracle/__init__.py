@@ -102,3 +102,38 @@ def letkf_analysis_batched(Yb, d, rinv_loc, Xb, rho, nthreads=0, want_W=True):
         _dp(Xa), _dp(W) if want_W else None, _dp(wbar),
         info.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), nthreads)
     return dict(Xa=Xa, W=W, wbar=wbar, info=info, threads=nt)
+
+
+def localisation(loc_kind, L, dist):
+    lib = _load()
+    lib.oracle_localisation.argtypes = [ctypes.c_int, ctypes.c_double, ctypes.c_double]
+    lib.oracle_localisation.restype = ctypes.c_double
+    return lib.oracle_localisation(int(loc_kind), float(L), float(dist))
+
+
+def letkf_analysis_grid(Yf, yo, Xb, hw, loc_kind, L, sigma_o, rho, mask=None, nthreads=0):
+    """Grid form: Yf[V][Ny][Nx][M], yo[V][Ny][Nx], Xb[Ny*Nx][nstate][M] -> dict(Xa, wbar, info)."""
+    lib = _load()
+    Yf, yo, Xb = _c(Yf), _c(yo), _c(Xb)
+    V, Ny, Nx, M = Yf.shape
+    ns = Xb.shape[1]
+    assert yo.shape == (V, Ny, Nx) and Xb.shape == (Ny * Nx, ns, M)
+    mk = None
+    if mask is not None:
+        mk = np.ascontiguousarray(mask, dtype=np.uint8)
+        assert mk.shape == (Ny, Nx)
+    Xa = np.empty_like(Xb)
+    wbar = np.empty((Ny * Nx, M))
+    info = np.zeros(Ny * Nx, dtype=np.int32)
+    lib.oracle_letkf_analysis_grid.argtypes = [
+        ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+        ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+        ctypes.c_double, ctypes.c_double, ctypes.c_double,
+        ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]
+    lib.oracle_letkf_analysis_grid.restype = ctypes.c_int
+    nt = lib.oracle_letkf_analysis_grid(
+        Yf.ctypes.data, yo.ctypes.data, mk.ctypes.data if mk is not None else None, Xb.ctypes.data,
+        M, V, Ny, Nx, ns, int(hw), int(loc_kind), float(L), float(sigma_o), float(rho),
+        Xa.ctypes.data, wbar.ctypes.data, info.ctypes.data, nthreads)
+    return dict(Xa=Xa, wbar=wbar, info=info, threads=nt)
+

@@ -188,3 +188,79 @@ int oracle_letkf_analysis_batched(const double* Yb, const double* d,
     }
     return nt;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Grid form (Procedure 1 lines 1-2, Eq.18-19).
+ * Every point of a periodic Ny x Nx grid is a local problem whose observations are the V
+ * observed variables at the (2 hw + 1)^2 points of the square patch around it:
+ *   local row j = v (2hw+1)^2 + (dy+hw)(2hw+1) + (dx+hw),  point (y+dy mod Ny, x+dx mod Nx)
+ *   ybar  = mean_m Yf[v][yy][xx][m]                     Eq.18
+ *   dY_j  = Yf[v][yy][xx][:] - ybar                     Eq.19
+ *   d_j   = yo[v][yy][xx] - ybar                        innovation of Eq.14
+ *   r_j   = G(dist) / sigma_o^2, 0 where mask[yy][xx] == 0 (unobserved point, reading G7)
+ * with dist = sqrt(dx^2 + dy^2) in grid units and the localisation function G:
+ *   loc_kind 0: Gaussian exp(-dist^2 / (2 L^2))                 (BASELINE.json configs)
+ *   loc_kind 1: Gaspari-Cohn 5th-order piecewise rational with half-width c = L, zero from
+ *               2c on (ref.[21] of the paper; the paper's cutoff 2(p-1) dx is 2c)
+ * The local problem itself is analysis_point() above, unchanged.
+ */
+double oracle_localisation(int loc_kind, double L, double dist)
+{
+    if (loc_kind == 0) return exp(-(dist * dist) / (2.0 * L * L));
+    {
+        const double z = dist / L;
+        if (z >= 2.0) return 0.0;
+        if (z <= 1.0)
+            return ((((-0.25 * z + 0.5) * z + 0.625) * z - 5.0 / 3.0) * z) * z + 1.0;
+        return (((((1.0 / 12.0) * z - 0.5) * z + 0.625) * z + 5.0 / 3.0) * z - 5.0) * z + 4.0
+               - (2.0 / 3.0) / z;
+    }
+}
+
+int oracle_letkf_analysis_grid(const double* Yf, const double* yo, const unsigned char* mask,
+                               const double* Xb, int M, int V, int Ny, int Nx, int nstate,
+                               int hw, int loc_kind, double L, double sigma_o, double rho,
+                               double* Xa, double* wbar, int* info, int nthreads)
+{
+    int nt = pick_threads(nthreads);
+    const int side = 2 * hw + 1, P2 = side * side, p = V * P2;
+    const long npts = (long)Ny * Nx;
+    if (M < 1 || V < 1 || Ny < 1 || Nx < 1 || nstate < 1 || hw < 0) return nt;
+#pragma omp parallel num_threads(nt)
+    {
+        size_t MM = (size_t)M * M;
+        double* buf = (double*)malloc(sizeof(double) * (4 * MM + 4 * (size_t)M + (size_t)p * M + 2 * (size_t)p));
+        double *Q = buf, *Vv = buf + MM, *S = buf + 2 * MM, *Wl = buf + 3 * MM;
+        double *g = buf + 4 * MM, *lam = g + M, *wb = lam + M, *dX = wb + M;
+        double *Yb = dX + M, *dv = Yb + (size_t)p * M, *rv = dv + p;
+        long b;
+#pragma omp for schedule(dynamic)
+        for (b = 0; b < npts; ++b) {
+            const int y = (int)(b / Nx), x = (int)(b % Nx);
+            int v, dy, dx, m, sweeps;
+            for (v = 0; v < V; ++v)
+                for (dy = -hw; dy <= hw; ++dy)
+                    for (dx = -hw; dx <= hw; ++dx) {
+                        const int j = v * P2 + (dy + hw) * side + (dx + hw);
+                        const int yy = ((y + dy) % Ny + Ny) % Ny, xx = ((x + dx) % Nx + Nx) % Nx;
+                        const double* src = Yf + (((long)v * Ny + yy) * Nx + xx) * M;
+                        double ybar = 0.0;
+                        for (m = 0; m < M; ++m) ybar += src[m];
+                        ybar /= (double)M;
+                        for (m = 0; m < M; ++m) Yb[(long)j * M + m] = src[m] - ybar;
+                        dv[j] = yo[((long)v * Ny + yy) * Nx + xx] - ybar;
+                        rv[j] = (mask && !mask[(long)yy * Nx + xx])
+                                    ? 0.0
+                                    : oracle_localisation(loc_kind, L, sqrt((double)(dx * dx + dy * dy)))
+                                          / (sigma_o * sigma_o);
+                    }
+            sweeps = analysis_point(Yb, dv, rv, Xb + b * (long)nstate * M, M, p, nstate, rho,
+                                    Xa + b * (long)nstate * M, NULL, wbar ? wbar + b * (long)M : NULL,
+                                    Q, g, lam, Vv, S, Wl, wb, dX);
+            if (info) info[b] = (sweeps < 0) ? 1 : 0;
+        }
+        free(buf);
+    }
+    return nt;
+}
+

@@ -57,6 +57,20 @@ int oracle_letkf_analysis_batched(const double* Yb, const double* d,
                                   double* Xa, double* W, double* wbar,
                                   int* info, int nthreads);
 
+/* Localisation function G(dist) of PAPER.md:144 (dist in grid units): loc_kind 0 = Gaussian
+ * exp(-dist^2/(2 L^2)) (BASELINE.json), 1 = Gaspari-Cohn with half-width L (zero from 2L on). */
+double oracle_localisation(int loc_kind, double L, double dist);
+
+/* Grid form: the local problems of a periodic Ny x Nx grid with the V observed variables of a
+ * (2hw+1)^2 patch as local observations (Procedure 1 lines 1-2, Eq.18-19);
+ * Yf[V][Ny][Nx][M], yo[V][Ny][Nx], mask[Ny][Nx] or NULL, Xb/Xa[Ny*Nx][nstate][M], wbar may be
+ * NULL.  Pinned against the batched form on an explicitly gathered Y_loc
+ * (tests/test_oracle_grid.py).  Returns threads used. */
+int oracle_letkf_analysis_grid(const double* Yf, const double* yo, const unsigned char* mask,
+                               const double* Xb, int M, int V, int Ny, int Nx, int nstate,
+                               int hw, int loc_kind, double L, double sigma_o, double rho,
+                               double* Xa, double* wbar, int* info, int nthreads);
+
 #ifdef __cplusplus
 }
 #endif

@@ -162,3 +162,18 @@ def shard_range(batch, rank, world_size):
     lo = (batch * rank) // world_size
     hi = (batch * (rank + 1)) // world_size
     return lo, hi
+
+
+def grid_inputs(Ny=128, Nx=128, M=64, V=2, nstate=9, config_index=6, obs_every=1):
+    """Grid form of config 4: instead of a materialised Y_loc the
+    forecast observations of the whole periodic grid, Yf[V][Ny][Nx][M] ~ 0.05 + N(0, 0.1^2) (NOT
+    centred: Eq.18-19 are part of the path), observations yo[V][Ny][Nx] ~ 0.05 + N(0, 0.1^2),
+    background ensemble Xb[Ny*Nx][nstate][M] ~ N(1/9, 0.01^2) and a mask of observed points (every
+    `obs_every`-th point in x and y, "spacing of observation points"; 1 = all)."""
+    rng = _rng(config_index)
+    Yf = 0.05 + 0.1 * rng.standard_normal(size=(V, Ny, Nx, M))
+    yo = 0.05 + 0.1 * rng.standard_normal(size=(V, Ny, Nx))
+    Xb = 1.0 / 9.0 + 0.01 * rng.standard_normal(size=(Ny * Nx, nstate, M))
+    mask = np.zeros((Ny, Nx), dtype=np.uint8)
+    mask[::obs_every, ::obs_every] = 1
+    return dict(Yf=Yf, yo=yo, Xb=Xb, mask=mask, rho=RHO, sigma_o=SIGMA_O, hw=3, loc_kind=0, L=2.0)
