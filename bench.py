@@ -442,6 +442,46 @@ def run_ours(args):
                 "d2h_bytes_per_step": int(Xa_pin.numel() * 8 + B * 4), "api": "letkf_analysis_batched_host"}
             del hp, Xa_pin
             letkf.host_release()
+            # ---- grid form: same 128 x 128 x 2 x 7x7 problem, the local
+            # observations gathered inside the library from the fields (Y_loc never materialised)
+            gi = wl.grid_inputs()
+            gt = {k: torch.from_numpy(gi[k]).cuda() for k in ("Yf", "yo", "Xb")}
+            gXa = torch.empty_like(gt["Xb"])
+            gwork = torch.empty(letkf.analysis_grid_workspace_bytes(M, 2, 128, 128, 3, 9), dtype=torch.uint8, device="cuda")
+
+            def gstep():
+                letkf.analysis_grid(gt["Yf"], gt["yo"], gt["Xb"], 3, 0, 2.0, gi["sigma_o"], gi["rho"], Xa=gXa,
+                                    info=info, work=gwork, stream=stream)
+            for _ in range(3):
+                gstep()
+            torch.cuda.synchronize()
+            e0.record(stream)
+            for _ in range(args.steps):
+                gstep()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            gms = e0.elapsed_time(e1) / args.steps
+            gl = letkf.last_launch_count()
+            hp = {k: torch.from_numpy(gi[k]).pin_memory() for k in ("Yf", "yo", "Xb")}
+            gXa_pin = torch.empty_like(hp["Xb"]).pin_memory()
+            letkf.analysis_grid_host(hp["Yf"], hp["yo"], hp["Xb"], 3, 0, 2.0, gi["sigma_o"], gi["rho"], Xa=gXa_pin)
+            ksteps = min(args.steps, 3)
+            e0.record(stream)
+            for _ in range(ksteps):
+                letkf.analysis_grid_host(hp["Yf"], hp["yo"], hp["Xb"], 3, 0, 2.0, gi["sigma_o"], gi["rho"], Xa=gXa_pin)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ghms = e0.elapsed_time(e1) / ksteps
+            assert torch.equal(gXa_pin, gXa.cpu()), "grid e2e result differs from the device call"
+            line["analysis_grid"] = {
+                "workload": "letkf_analysis_grid fp64 M=64 V=2 128x128 periodic grid, 7x7 patch (p=98), nstate=9, Gaussian localisation",
+                "value": B / (gms * 1e-3), "unit": "grid points/s", "ms_per_step": gms, "gpu_launches_per_step": gl,
+                "hbm_bytes_per_point_algorithmic": 8.0 * (2 * 65 + 2 * 9 * M),
+                "e2e": {"value": B / (ghms * 1e-3), "unit": "grid points/s", "ms_per_step": ghms,
+                        "h2d_bytes_per_step": int(sum(v.numel() for v in hp.values()) * 8),
+                        "d2h_bytes_per_step": int(gXa_pin.numel() * 8 + B * 4), "api": "letkf_analysis_grid_host"}}
+            del gi, gt, gXa, gwork, hp, gXa_pin
+            letkf.host_release()
             del t, Xa, awork, inp
         # ---- config 5: EVD size sweep, batch = floor(2^26 / M^2), LETKF-shaped
         if not args.no_sweep:

@@ -104,6 +104,42 @@ int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv
 size_t letkf_analysis_workspace_bytes(int M, int p, int nstate, int batch);
 
 /*
+ * Grid form of the fused analysis (PAPER.md:144-151 R-localisation,
+ * Procedure 1 lines 1-2 "Extract local observation data", Eq.18-19): the local observations of
+ * every point of a PERIODIC Ny x Nx grid are gathered inside the library from the forecast
+ * observations of the whole grid, so that Y_loc[M, Nx, l_max V] (5.3 times the state)
+ * is never materialised.  For grid point (y, x) the local observations are the V observed
+ * variables at the (2 hw + 1)^2 points of the square patch around it,
+ *   local row j = v (2hw+1)^2 + (dy+hw)(2hw+1) + (dx+hw),  observed point (y+dy mod Ny, x+dx mod Nx),
+ *   dY_j = Yf[v][yy][xx][:] - mean_m Yf[v][yy][xx][m]            Eq.18-19
+ *   d_j  = yo[v][yy][xx] - mean_m Yf[v][yy][xx][m]
+ *   r_j  = G(sqrt(dx^2+dy^2)) / sigma_o^2,  0 where obs_mask[yy][xx] == 0 (no observation there)
+ * followed by the local analysis exactly as letkf_analysis_batched (same rho, same outputs).
+ * G is the localisation function of PAPER.md:144 in grid units:
+ *   loc_kind 0: Gaussian exp(-dist^2 / (2 loc_scale^2))            (BASELINE.json configs)
+ *   loc_kind 1: Gaspari-Cohn (ref.[21]), half-width loc_scale, zero from 2 loc_scale on; the
+ *               paper's cutoff 2(p-1) dx corresponds to loc_scale = p-1
+ *
+ *   Yf        in  [V][Ny][Nx][M]  forecast observations y_m^f = H x_m^f at every grid point
+ *   yo        in  [V][Ny][Nx]     observations
+ *   obs_mask  in  [Ny][Nx] bytes or NULL (NULL = every point observed)
+ *   Xb        in  [Ny*Nx][nstate][M]   background ensemble, grid point index y*Nx + x
+ *   Xa        out [Ny*Nx][nstate][M]   may alias Xb
+ *   wbar      out [Ny*Nx][M] or NULL;  info out [Ny*Nx] or NULL
+ *   work      >= letkf_analysis_grid_workspace_bytes(M, V, Ny, Nx, hw, nstate), or NULL
+ * For M <= 64 and nstate <= 15 the gather runs inside the tridiagonalisation kernel (the field is
+ * read through L2, nothing is materialised); otherwise Y_loc is materialised pass by pass in the
+ * workspace and the any-M kernels are used.
+ */
+int letkf_analysis_grid(const double* Yf, const double* yo, const unsigned char* obs_mask,
+                        const double* Xb, int M, int V, int Ny, int Nx, int nstate, int hw,
+                        int loc_kind, double loc_scale, double sigma_o, double rho,
+                        double* Xa, double* wbar, int* info,
+                        void* work, size_t work_bytes, void* stream);
+
+size_t letkf_analysis_grid_workspace_bytes(int M, int V, int Ny, int Nx, int hw, int nstate);
+
+/*
  * The same two operations on HOST buffers (the end-to-end form: this is what bench.py's "e2e"
  * times).  Every array pointer is a HOST pointer with the layouts above; page-locked (pinned)
  * memory lets the copies run asynchronously at full PCIe rate, pageable memory works but
@@ -122,6 +158,13 @@ int letkf_syev_batched_host(const double* A, int M, int batch, double* w, double
 int letkf_analysis_batched_host(const double* Yb, const double* d, const double* rinv_loc,
                                 const double* Xb, int M, int p, int nstate, int batch, double rho,
                                 double* Xa, double* W, double* wbar, int* info);
+
+/* letkf_analysis_grid on HOST buffers: only the observation fields and the ensemble cross PCIe
+ * (Y_loc never exists anywhere).  Argument positions as in this signature. */
+int letkf_analysis_grid_host(const double* Yf, const double* yo, const unsigned char* obs_mask,
+                             const double* Xb, int M, int V, int Ny, int Nx, int nstate, int hw,
+                             int loc_kind, double loc_scale, double sigma_o, double rho,
+                             double* Xa, double* wbar, int* info);
 
 /* Frees the staging arena the host entry points keep for the calling host thread (no-op if none). */
 void letkf_host_release(void);

@@ -359,6 +359,75 @@ __device__ __forceinline__ void pivot_groups_down(double (&a)[MT], const TriShar
     if constexpr (G > 0) pivot_groups_down<MT, G - 1>(a, sh, M, dws, ews);
 }
 
+// Grid form of the analysis (Procedure 1 lines 1-2,
+// Eq.18-19): the local observations of grid point b are gathered from the forecast-observation
+// field of the whole periodic grid instead of being read from a materialised Y_loc.
+//   local row i = v side^2 + (dy+hw) side + (dx+hw), side = 2 hw + 1, point (y+dy mod Ny, x+dx mod Nx)
+//   dY_i = Yf[v][yy][xx][:] - ybar,  d_i = yo[v][yy][xx] - ybar,  r_i = G(dist)/sigma_o^2 (0 if masked)
+struct GridArgs {
+    const double* Yf;            // [V][Ny][Nx][M]; NULL = not the grid form
+    const double* ybar;          // [V][Ny][Nx]   ensemble mean of Yf (Eq.18), formed by grid_obs_mean
+    const double* yo;            // [V][Ny][Nx]
+    const unsigned char* mask;   // [Ny][Nx] or NULL
+    int V, Ny, Nx, hw, loc_kind;
+    double L, inv_sig2;
+    int point0;                  // grid point of CTA 0
+};
+
+// localisation function G of PAPER.md:144: 0 = Gaussian exp(-dist^2/(2 L^2)) (BASELINE.json),
+// 1 = Gaspari-Cohn, the 5th-order piecewise rational of ref.[21] with half-width L (zero from 2L)
+__host__ __device__ inline double localisation(int kind, double L, double dist)
+{
+    if (kind == 0) return exp(-(dist * dist) / (2.0 * L * L));
+    const double z = dist / L;
+    if (z >= 2.0) return 0.0;
+    if (z <= 1.0) return ((((-0.25 * z + 0.5) * z + 0.625) * z - 5.0 / 3.0) * z) * z + 1.0;
+    return (((((1.0 / 12.0) * z - 0.5) * z + 0.625) * z + 5.0 / 3.0) * z - 5.0) * z + 4.0 - (2.0 / 3.0) / z;
+}
+
+// descriptor of local observation row i of grid point (y, x): index of the observed point in the
+// [V][Ny][Nx] fields and its weight
+__device__ __forceinline__ void grid_row(const GridArgs& g, int y, int x, int i, long& off, double& rloc)
+{
+    const int side = 2 * g.hw + 1, P2 = side * side;
+    const int v = i / P2, rem = i - v * P2;
+    const int dy = rem / side - g.hw, dx = rem % side - g.hw;
+    int yy = (y + dy) % g.Ny, xx = (x + dx) % g.Nx;
+    if (yy < 0) yy += g.Ny;
+    if (xx < 0) xx += g.Nx;
+    off = ((long)v * g.Ny + yy) * g.Nx + xx;
+    const bool seen = !g.mask || g.mask[(long)yy * g.Nx + xx];
+    rloc = seen ? localisation(g.loc_kind, g.L, sqrt((double)(dx * dx + dy * dy))) * g.inv_sig2 : 0.0;
+}
+
+// Eq.18 for the whole grid: ybar[o] = mean_m Yf[o][m]; one warp per observed point
+__global__ void __launch_bounds__(256)
+grid_obs_mean(const double* __restrict__ Yf, double* __restrict__ ybar, long nobs, int M)
+{
+    const long o = (long)blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (o >= nobs) return;
+    double acc = 0.0;
+    for (int m = threadIdx.x & 31; m < M; m += 32) acc += Yf[o * M + m];
+    acc = warp_sum(acc);
+    if ((threadIdx.x & 31) == 0) ybar[o] = acc / (double)M;
+}
+
+// The materialising gather (any M; the path for M > 64 and the cross-check of the fused one):
+// Yb[n][p][M], d[n][p], r[n][p] of grid points point0 ... point0+n-1; one CTA per point
+__global__ void __launch_bounds__(256)
+grid_gather(GridArgs g, int M, int p, double* __restrict__ Yb, double* __restrict__ d, double* __restrict__ r)
+{
+    const long b = blockIdx.x;
+    const int pt = g.point0 + (int)b, y = pt / g.Nx, x = pt - y * g.Nx;
+    for (int i = threadIdx.x >> 5; i < p; i += 8) {
+        long off; double rl;
+        grid_row(g, y, x, i, off, rl);
+        const double mean = g.ybar[off];
+        for (int m = threadIdx.x & 31; m < M; m += 32) Yb[(b * p + i) * M + m] = g.Yf[off * M + m] - mean;
+        if ((threadIdx.x & 31) == 0) { d[b * p + i] = g.yo[off] - mean; r[b * p + i] = rl; }
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // a3 + explicit Q for one matrix per CTA.  gram == true: the matrix is not read from A but formed
 // from the LETKF inputs (a1, a2: Eq.17 and the right factor of Eq.14) straight into the registers.
@@ -366,7 +435,8 @@ template <int MT, bool GRAM>
 __global__ void __launch_bounds__(FastCfg<MT>::NT) __maxnreg__((MT == 64) ? LETKF_TRI_REGS64 : (MT == 48 ? LETKF_TRI_REGS48 : (MT == 32 ? 128 : 80)))
 fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Workspace ws, int M,
                    const double* __restrict__ Yb_, const double* __restrict__ d_,
-                   const double* __restrict__ r_, int p, double shift, double* __restrict__ gout_)
+                   const double* __restrict__ r_, int p, double shift, double* __restrict__ gout_,
+                   GridArgs grid)
 {
     using C = FastCfg<MT>;
     extern __shared__ __align__(16) double sm[];
@@ -407,33 +477,62 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
         }
     } else {
         // a_j[c] = shift*delta + sum_i r_i Yb[i][j] Yb[i][c];  Yb rows staged through the tile
-        const double* Yb = Yb_ + b * (size_t)p * M;
-        const double* dv = d_ + b * (size_t)p;
-        const double* rv = r_ + b * (size_t)p;
+        const bool gridded = grid.Yf != nullptr;
+        const double* Yb = gridded ? nullptr : Yb_ + b * (size_t)p * M;
+        const double* dv = gridded ? nullptr : d_ + b * (size_t)p;
+        const double* rv = gridded ? nullptr : r_ + b * (size_t)p;
+        const int pt = grid.point0 + (int)b, gy = gridded ? pt / grid.Nx : 0, gx = gridded ? pt - gy * grid.Nx : 0;
+        // per-row scalars of the staged rows (the small vectors are free until the reduction starts)
+        constexpr int RB = (RefLayout<MT>::HT < C::NT / 2) ? RefLayout<MT>::HT : C::NT / 2;   // rows per stage
+        double* rloc = sh.xs;                                   // [RB]
+        double* dloc = sh.xs + RB;                              // [RB]
+        double* mloc = sh.vbuf;                                 // [RB]  ensemble mean of the row (grid form)
+        long*   oloc = reinterpret_cast<long*>(sh.pbuf);        // [RB]  observed point of the row (grid form)
 #pragma unroll
         for (int c = 0; c < MT; ++c) a[c] = (c == j && j < M) ? shift : 0.0;
         double gj = 0.0;
-        constexpr int RB = RefLayout<MT>::HT;      // observation rows per stage (the region holds HT rows of MT+1)
         for (int i0 = 0; i0 < p; i0 += RB) {
             const int nr = min(RB, p - i0);
-            if (j < MT) {                          // thread j stages column j of every row, 8 in flight
-                const double* src = Yb + (size_t)i0 * M + j;
-                int r = 0;
-                for (; r + 8 <= nr; r += 8) {
-                    double tmp[8];
-#pragma unroll
-                    for (int u = 0; u < 8; ++u) tmp[u] = (j < M) ? src[(size_t)(r + u) * M] : 0.0;
-#pragma unroll
-                    for (int u = 0; u < 8; ++u) tile[(r + u) * MT + j] = tmp[u];
+            if (j < nr) {
+                if (gridded) {
+                    long off; double rl;
+                    grid_row(grid, gy, gx, i0 + j, off, rl);
+                    const double mean = grid.ybar[off];
+                    oloc[j] = off; mloc[j] = mean; rloc[j] = rl; dloc[j] = grid.yo[off] - mean;
+                } else {
+                    rloc[j] = rv[i0 + j]; dloc[j] = dv[i0 + j];
                 }
-                for (; r < nr; ++r) tile[r * MT + j] = (j < M) ? src[(size_t)r * M] : 0.0;
+            }
+            if (gridded) __syncthreads();
+            if (j < MT) {                          // thread j stages column j of every row, 8 in flight
+                int r = 0;
+                if (gridded) {
+                    for (; r + 8 <= nr; r += 8) {
+                        double tmp[8];
+#pragma unroll
+                        for (int u = 0; u < 8; ++u) tmp[u] = (j < M) ? grid.Yf[oloc[r + u] * M + j] - mloc[r + u] : 0.0;
+#pragma unroll
+                        for (int u = 0; u < 8; ++u) tile[(r + u) * MT + j] = tmp[u];
+                    }
+                    for (; r < nr; ++r) tile[r * MT + j] = (j < M) ? grid.Yf[oloc[r] * M + j] - mloc[r] : 0.0;
+                } else {
+                    const double* src = Yb + (size_t)i0 * M + j;
+                    for (; r + 8 <= nr; r += 8) {
+                        double tmp[8];
+#pragma unroll
+                        for (int u = 0; u < 8; ++u) tmp[u] = (j < M) ? src[(size_t)(r + u) * M] : 0.0;
+#pragma unroll
+                        for (int u = 0; u < 8; ++u) tile[(r + u) * MT + j] = tmp[u];
+                    }
+                    for (; r < nr; ++r) tile[r * MT + j] = (j < M) ? src[(size_t)r * M] : 0.0;
+                }
             }
             __syncthreads();
             for (int r = 0; r < nr; ++r) {
-                const double ri = rv[i0 + r];
+                const double ri = rloc[r];
                 const double yj = tile[r * MT + j];
                 const double yr = yj * ri;
-                gj = fma(yr, dv[i0 + r], gj);
+                gj = fma(yr, dloc[r], gj);
                 const double2* row = reinterpret_cast<const double2*>(tile + r * MT);
 #pragma unroll
                 for (int q = 0; q < MT / 2; ++q) {

@@ -148,7 +148,7 @@ static cudaError_t allow_smem(K kernel, size_t bytes)
 static bool g_force_generic = false;     // letkf_set_option("force_generic", 1): tests only
 
 // a1/a2 inputs when the matrix is to be formed from the LETKF observations instead of read
-struct GramArgs { const double* Yb; const double* d; const double* r; int p; double shift; double* gout; };
+struct GramArgs { const double* Yb; const double* d; const double* r; int p; double shift; double* gout; GridArgs grid; };
 
 template <int MT>
 static int fast_tridiag_run(const double* A, double* V, Workspace ws, int M, int n, cudaStream_t st,
@@ -160,12 +160,12 @@ static int fast_tridiag_run(const double* A, double* V, Workspace ws, int M, int
         if ((ce = allow_smem(fast_tridiag_formq<MT, true>, smem)) != cudaSuccess) return (int)ce;
         KLAUNCH("fast_tridiag_formq<gram>", st,
                 fast_tridiag_formq<MT, true><<<n, FastCfg<MT>::NT, smem, st>>>(
-                    nullptr, V, ws, M, gram->Yb, gram->d, gram->r, gram->p, gram->shift, gram->gout));
+                    nullptr, V, ws, M, gram->Yb, gram->d, gram->r, gram->p, gram->shift, gram->gout, gram->grid));
     } else {
         if ((ce = allow_smem(fast_tridiag_formq<MT, false>, smem)) != cudaSuccess) return (int)ce;
         KLAUNCH("fast_tridiag_formq", st,
                 fast_tridiag_formq<MT, false><<<n, FastCfg<MT>::NT, smem, st>>>(
-                    A, V, ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr));
+                    A, V, ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{}));
     }
     return 0;
 }
@@ -496,6 +496,102 @@ size_t letkf_analysis_workspace_bytes(int M, int p, int nstate, int batch)
     return s;
 }
 
+// does the grid form run with the gather fused into the tridiagonalisation kernel?
+static bool grid_fused(int M, int nstate) { return fast_supported(M) && !g_force_generic && nstate <= EPI_NS_MAX; }
+
+size_t letkf_analysis_grid_workspace_bytes(int M, int V, int Ny, int Nx, int hw, int nstate)
+{
+    if (M < 2 || M > LETKF_MAX_M || V < 1 || Ny < 1 || Nx < 1 || hw < 0 || nstate < 1) return 0;
+    const long npts = (long)Ny * Nx;
+    if (npts > 0x7fffffffL) return 0;
+    const int batch = (int)npts, p = V * (2 * hw + 1) * (2 * hw + 1);
+    size_t s = align_up(letkf_analysis_workspace_bytes(M, p, nstate, batch), 256);
+    s += align_up(sizeof(double) * (size_t)V * npts, 256);                                   // ybar
+    const int chunk = syev_chunk(M, batch);                                                  // materialised Y_loc
+    s += align_up(sizeof(double) * (size_t)p * M * chunk, 256) + 2 * align_up(sizeof(double) * (size_t)p * chunk, 256);
+    return s;
+}
+
+// a1-a9 for `batch` grid points.  Either (Yb, d, rinv_loc) or `grid` (then gYb/gd/gr are scratch
+// for the materialised local observations of one pass, used when the gather cannot be fused).
+static int analysis_core(const double* Yb, const double* d, const double* rinv_loc, const GridArgs* grid,
+                         double* gYb, double* gd, double* gr,
+                         const double* Xb, int M, int p, int nstate, int batch, double rho,
+                         double* Xa, double* W, double* wbar, int* info,
+                         void* work, size_t work_bytes, int work_argpos, cudaStream_t st)
+{
+    const int chunk = syev_chunk(M, batch);
+    const size_t need = letkf_analysis_workspace_bytes(M, p, nstate, batch);
+    ScopedWork sw;
+    int rc = sw.acquire(work, work_bytes, need, st, work_argpos);
+    if (rc) return rc;
+    Workspace ws;
+    size_t off = carve(ws, sw.ptr, M, chunk);
+    char* base = reinterpret_cast<char*>(sw.ptr);
+    double* Vbuf = reinterpret_cast<double*>(base + off); off += align_up(sizeof(double) * (size_t)M * M * chunk, 256);
+    double* lam  = reinterpret_cast<double*>(base + off); off += align_up(sizeof(double) * (size_t)M * chunk, 256);
+    double* gbuf = reinterpret_cast<double*>(base + off);
+
+    const double shift = (double)(M - 1) / rho;
+    cudaError_t ce;
+    const size_t ep_smem = sizeof(double) * (2 * (size_t)M + 2 * (size_t)nstate + 2 * (size_t)nstate * M);
+    if (ep_smem > 200 * 1024) return -7;
+    if ((ce = allow_smem(generic_epilogue, ep_smem)) != cudaSuccess) return (int)ce;
+    const bool fuse_gather = grid && !W && grid_fused(M, nstate);
+
+    for (int b0 = 0; b0 < batch; b0 += chunk) {
+        const int n = (batch - b0 < chunk) ? batch - b0 : chunk;
+        // local observations of this pass: the caller's arrays, or the scratch the gather fills
+        const double* Ybc = grid ? gYb : Yb + (size_t)b0 * p * M;
+        const double* dc = grid ? gd : d + (size_t)b0 * p;
+        const double* rc_ = grid ? gr : rinv_loc + (size_t)b0 * p;
+        const double* Xbc = Xb + (size_t)b0 * nstate * M;
+        double* Xac = Xa + (size_t)b0 * nstate * M;
+        double* Wc = W ? W + (size_t)b0 * M * M : nullptr;
+        double* wbc = wbar ? wbar + (size_t)b0 * M : nullptr;
+        int* infoc = info ? info + b0 : nullptr;
+
+        auto stageT = [&](int c0, int nk, cudaStream_t s) {
+            if (g_analysis_hooks) {
+                const int hrc = g_analysis_hooks->pre(g_analysis_hooks->ctx, b0 + c0, nk, s);
+                if (hrc) return hrc;
+            }
+            GramArgs ga{Ybc + (size_t)c0 * p * M, dc + (size_t)c0 * p, rc_ + (size_t)c0 * p, p, shift,
+                        gbuf + (size_t)c0 * M, GridArgs{}};
+            if (grid) {
+                GridArgs gk = *grid;
+                gk.point0 = grid->point0 + b0 + c0;
+                if (fuse_gather) {
+                    ga.grid = gk;
+                } else {
+                    KLAUNCH("grid_gather", s,
+                            grid_gather<<<nk, 256, 0, s>>>(gk, M, p, gYb + (size_t)c0 * p * M, gd + (size_t)c0 * p,
+                                                           gr + (size_t)c0 * p));
+                }
+            }
+            double* Vk = Vbuf + (size_t)c0 * M * M;
+            return stage_T(Vk, M, nk, Vk, ws_slice(ws, M, c0), s, &ga);
+        };
+        // a6-a9: fused into fast_apply when W is not wanted (V then never leaves the SM); the
+        // any-M kernel otherwise, and for the grid points the slow path finished.
+        const bool fused = !Wc && fast_supported(M) && !g_force_generic && nstate <= EPI_NS_MAX;
+        auto post = [&](int c0, int nk, cudaStream_t s) -> int {
+            const int gridsz = fused ? (nk < 296 ? nk : 296) : nk;
+            KLAUNCH(fused ? "generic_epilogue(flagged)" : "generic_epilogue", s,
+                    generic_epilogue<<<gridsz, 256, ep_smem, s>>>(
+                        Vbuf + (size_t)c0 * M * M, lam + (size_t)c0 * M, gbuf + (size_t)c0 * M,
+                        Xbc + (size_t)c0 * nstate * M, M, nstate, nk, Xac + (size_t)c0 * nstate * M,
+                        Wc ? Wc + (size_t)c0 * M * M : nullptr, wbc ? wbc + (size_t)c0 * M : nullptr,
+                        fused ? ws.flags + c0 : nullptr));
+            return g_analysis_hooks ? g_analysis_hooks->post(g_analysis_hooks->ctx, b0 + c0, nk, s) : 0;
+        };
+        EpiArgs ep{lam, gbuf, Xbc, Xac, wbc, nstate};
+        rc = run_pass(M, n, lam, Vbuf, infoc, ws, st, stageT, post, fused ? &ep : nullptr);
+        if (rc) return rc;
+    }
+    return LETKF_OK;
+}
+
 int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv_loc,
                            const double* Xb, int M, int p, int nstate, int batch, double rho,
                            double* Xa, double* W, double* wbar, int* info,
@@ -517,64 +613,53 @@ int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv
     if (wbar && misaligned(wbar)) return -12;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     prof_reset(st);
+    return analysis_core(Yb, d, rinv_loc, nullptr, nullptr, nullptr, nullptr, Xb, M, p, nstate, batch, rho,
+                         Xa, W, wbar, info, work, work_bytes, 14, st);
+}
 
-    const int chunk = syev_chunk(M, batch);
-    const size_t need = letkf_analysis_workspace_bytes(M, p, nstate, batch);
+int letkf_analysis_grid(const double* Yf, const double* yo, const unsigned char* obs_mask, const double* Xb,
+                        int M, int V, int Ny, int Nx, int nstate, int hw, int loc_kind, double loc_scale,
+                        double sigma_o, double rho, double* Xa, double* wbar, int* info,
+                        void* work, size_t work_bytes, void* stream)
+{
+    g_launches = 0;
+    if (M < 2 || M > LETKF_MAX_M) return -5;
+    if (V < 1) return -6;
+    if (Ny < 1) return -7;
+    if (Nx < 1 || (long)Ny * Nx > 0x7fffffffL) return -8;
+    if (nstate < 1) return -9;
+    if (hw < 0) return -10;
+    if (loc_kind != 0 && loc_kind != 1) return -11;
+    if (!(loc_scale > 0.0)) return -12;
+    if (!(sigma_o > 0.0)) return -13;
+    if (!(rho > 0.0)) return -14;
+    if (!Yf || misaligned(Yf)) return -1;
+    if (!yo || misaligned(yo)) return -2;
+    if (!Xb || misaligned(Xb)) return -4;
+    if (!Xa || misaligned(Xa)) return -15;
+    if (wbar && misaligned(wbar)) return -16;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    prof_reset(st);
+    const int batch = Ny * Nx, side = 2 * hw + 1, p = V * side * side;
+    const size_t need = letkf_analysis_grid_workspace_bytes(M, V, Ny, Nx, hw, nstate);
     ScopedWork sw;
-    int rc = sw.acquire(work, work_bytes, need, st, 14);
+    int rc = sw.acquire(work, work_bytes, need, st, 18);
     if (rc) return rc;
-    Workspace ws;
-    size_t off = carve(ws, sw.ptr, M, chunk);
+    // carve: [analysis workspace][ybar][materialised Y_loc of one pass]
+    const size_t wa = align_up(letkf_analysis_workspace_bytes(M, p, nstate, batch), 256);
     char* base = reinterpret_cast<char*>(sw.ptr);
-    double* Vbuf = reinterpret_cast<double*>(base + off); off += align_up(sizeof(double) * (size_t)M * M * chunk, 256);
-    double* lam  = reinterpret_cast<double*>(base + off); off += align_up(sizeof(double) * (size_t)M * chunk, 256);
-    double* gbuf = reinterpret_cast<double*>(base + off);
-
-    const double shift = (double)(M - 1) / rho;
-    cudaError_t ce;
-    const size_t ep_smem = sizeof(double) * (2 * (size_t)M + 2 * (size_t)nstate + 2 * (size_t)nstate * M);
-    if (ep_smem > 200 * 1024) return -7;
-    if ((ce = allow_smem(generic_epilogue, ep_smem)) != cudaSuccess) return (int)ce;
-
-    for (int b0 = 0; b0 < batch; b0 += chunk) {
-        const int n = (batch - b0 < chunk) ? batch - b0 : chunk;
-        const double* Ybc = Yb + (size_t)b0 * p * M;
-        const double* dc = d + (size_t)b0 * p;
-        const double* rc_ = rinv_loc + (size_t)b0 * p;
-        const double* Xbc = Xb + (size_t)b0 * nstate * M;
-        double* Xac = Xa + (size_t)b0 * nstate * M;
-        double* Wc = W ? W + (size_t)b0 * M * M : nullptr;
-        double* wbc = wbar ? wbar + (size_t)b0 * M : nullptr;
-        int* infoc = info ? info + b0 : nullptr;
-
-        auto stageT = [&](int c0, int nk, cudaStream_t s) {
-            if (g_analysis_hooks) {
-                const int hrc = g_analysis_hooks->pre(g_analysis_hooks->ctx, b0 + c0, nk, s);
-                if (hrc) return hrc;
-            }
-            GramArgs ga{Ybc + (size_t)c0 * p * M, dc + (size_t)c0 * p, rc_ + (size_t)c0 * p, p, shift,
-                        gbuf + (size_t)c0 * M};
-            double* Vk = Vbuf + (size_t)c0 * M * M;
-            return stage_T(Vk, M, nk, Vk, ws_slice(ws, M, c0), s, &ga);
-        };
-        // a6-a9: fused into fast_apply when W is not wanted (V then never leaves the SM); the
-        // any-M kernel otherwise, and for the grid points the slow path finished.
-        const bool fused = !Wc && fast_supported(M) && !g_force_generic && nstate <= EPI_NS_MAX;
-        auto post = [&](int c0, int nk, cudaStream_t s) -> int {
-            const int grid = fused ? (nk < 296 ? nk : 296) : nk;
-            KLAUNCH(fused ? "generic_epilogue(flagged)" : "generic_epilogue", s,
-                    generic_epilogue<<<grid, 256, ep_smem, s>>>(
-                        Vbuf + (size_t)c0 * M * M, lam + (size_t)c0 * M, gbuf + (size_t)c0 * M,
-                        Xbc + (size_t)c0 * nstate * M, M, nstate, nk, Xac + (size_t)c0 * nstate * M,
-                        Wc ? Wc + (size_t)c0 * M * M : nullptr, wbc ? wbc + (size_t)c0 * M : nullptr,
-                        fused ? ws.flags + c0 : nullptr));
-            return g_analysis_hooks ? g_analysis_hooks->post(g_analysis_hooks->ctx, b0 + c0, nk, s) : 0;
-        };
-        EpiArgs ep{lam, gbuf, Xbc, Xac, wbc, nstate};
-        rc = run_pass(M, n, lam, Vbuf, infoc, ws, st, stageT, post, fused ? &ep : nullptr);
-        if (rc) return rc;
-    }
-    return LETKF_OK;
+    double* ybar = reinterpret_cast<double*>(base + wa);
+    size_t off = wa + align_up(sizeof(double) * (size_t)V * batch, 256);
+    const int chunk = syev_chunk(M, batch);
+    double* gYb = reinterpret_cast<double*>(base + off); off += align_up(sizeof(double) * (size_t)p * M * chunk, 256);
+    double* gd = reinterpret_cast<double*>(base + off);  off += align_up(sizeof(double) * (size_t)p * chunk, 256);
+    double* gr = reinterpret_cast<double*>(base + off);
+    const long nobs = (long)V * batch;
+    KLAUNCH("grid_obs_mean", st, grid_obs_mean<<<(unsigned)((nobs + 7) / 8), 256, 0, st>>>(Yf, ybar, nobs, M));
+    GridArgs g{Yf, ybar, yo, obs_mask, V, Ny, Nx, hw, loc_kind, loc_scale, 1.0 / (sigma_o * sigma_o), 0};
+    rc = analysis_core(nullptr, nullptr, nullptr, &g, gYb, gd, gr, Xb, M, p, nstate, batch, rho,
+                       Xa, nullptr, wbar, info, base, wa, 18, st);
+    return rc;
 }
 
 // ---- host-buffer entry points -----------------------------------------------------------------
@@ -836,6 +921,92 @@ int letkf_analysis_batched_host(const double* Yb, const double* d, const double*
 }
 
 void letkf_host_release(void) { g_hpipe.release(); }
+
+int letkf_analysis_grid_host(const double* Yf, const double* yo, const unsigned char* obs_mask,
+                             const double* Xb, int M, int V, int Ny, int Nx, int nstate, int hw,
+                             int loc_kind, double loc_scale, double sigma_o, double rho,
+                             double* Xa, double* wbar, int* info)
+{
+    g_launches = 0;
+    if (M < 2 || M > LETKF_MAX_M) return -5;
+    if (V < 1) return -6;
+    if (Ny < 1) return -7;
+    if (Nx < 1 || (long)Ny * Nx > 0x7fffffffL) return -8;
+    if (nstate < 1) return -9;
+    if (hw < 0) return -10;
+    if (loc_kind != 0 && loc_kind != 1) return -11;
+    if (!(loc_scale > 0.0)) return -12;
+    if (!(sigma_o > 0.0)) return -13;
+    if (!(rho > 0.0)) return -14;
+    if (!Yf) return -1;
+    if (!yo) return -2;
+    if (!Xb) return -4;
+    if (!Xa) return -15;
+    int rc = g_hpipe.init();
+    if (rc) return rc;
+    // The observation fields (V Ny Nx (M+1) doubles: 17 MB at 128 x 128 x 2 x 64) go in first, whole;
+    // the background ensemble follows sub-chunk by sub-chunk and the analysis ensemble comes back
+    // the same way (hooks as in letkf_analysis_batched_host).
+    const int batch = Ny * Nx;
+    const size_t nobs = (size_t)V * batch;
+    const size_t sX = sizeof(double) * (size_t)nstate * M, sw = sizeof(double) * (size_t)M;
+    const size_t wsb = align_up(letkf_analysis_grid_workspace_bytes(M, V, Ny, Nx, hw, nstate), 256);
+    size_t off[7], total = 0;
+    const size_t sizes[7] = {sizeof(double) * nobs * M, sizeof(double) * nobs, obs_mask ? (size_t)batch : 0,
+                             sX * batch, wbar ? sw * batch : 0, sizeof(int) * (size_t)batch, wsb};
+    for (int k = 0; k < 7; ++k) { off[k] = total; total += align_up(sizes[k] ? sizes[k] : 16, 256); }
+    if ((rc = g_hpipe.reserve(total))) return rc;
+    char* base = g_hpipe.arena;
+    double* dYf = reinterpret_cast<double*>(base + off[0]);
+    double* dyo = reinterpret_cast<double*>(base + off[1]);
+    unsigned char* dmask = obs_mask ? reinterpret_cast<unsigned char*>(base + off[2]) : nullptr;
+    double* dX = reinterpret_cast<double*>(base + off[3]);
+    double* dwb = wbar ? reinterpret_cast<double*>(base + off[4]) : nullptr;
+    int* dinfo = reinterpret_cast<int*>(base + off[5]);
+    void* dwork = base + off[6];
+    cudaStream_t sH = g_hpipe.s[0], sD = g_hpipe.s[1], sC = g_hpipe.sC;
+    const int chunk = syev_chunk(M, batch);
+    if (chunk < batch) return -8;                      // one pass only (180 GB: > 10^6 points at M = 64)
+    int nsub, per;
+    pass_partition(batch, nsub, per);
+    g_hpipe.events(2 * nsub + 1);
+    std::vector<cudaEvent_t> evH(g_hpipe.ev.begin(), g_hpipe.ev.begin() + nsub);
+    std::vector<cudaEvent_t> evC(g_hpipe.ev.begin() + nsub, g_hpipe.ev.begin() + 2 * nsub);
+    cudaEvent_t evF = g_hpipe.ev[2 * nsub];
+    cudaMemcpyAsync(dYf, Yf, sizes[0], cudaMemcpyHostToDevice, sH);
+    cudaMemcpyAsync(dyo, yo, sizes[1], cudaMemcpyHostToDevice, sH);
+    if (obs_mask) cudaMemcpyAsync(dmask, obs_mask, sizes[2], cudaMemcpyHostToDevice, sH);
+    cudaEventRecord(evF, sH);
+    for (int k = 0, c0 = 0; c0 < batch; ++k, c0 += per) {
+        const int nk = (batch - c0 < per) ? batch - c0 : per;
+        cudaMemcpyAsync(dX + (size_t)c0 * nstate * M, Xb + (size_t)c0 * nstate * M, sX * nk, cudaMemcpyHostToDevice, sH);
+        cudaEventRecord(evH[k], sH);
+    }
+    cudaStreamWaitEvent(sC, evF, 0);                   // the fields before anything is gathered
+    cudaMemsetAsync(dinfo, 0, sizeof(int) * (size_t)batch, sC);
+    AnaHostCtx ctx;
+    ctx.per = per; ctx.sD = sD; ctx.evH = &evH; ctx.evC = &evC; ctx.nout = 0;
+    auto add = [&](void* h, const void* dv, size_t bytes) {
+        ctx.host[ctx.nout] = static_cast<char*>(h); ctx.dev[ctx.nout] = static_cast<const char*>(dv);
+        ctx.bytes[ctx.nout] = bytes; ++ctx.nout;
+    };
+    add(Xa, dX, sX);
+    if (wbar) add(wbar, dwb, sw);
+    if (info) add(info, dinfo, sizeof(int));
+    PassHooks hooks{ana_host_pre, ana_host_post, &ctx};
+    g_analysis_hooks = &hooks;
+    rc = letkf_analysis_grid(dYf, dyo, dmask, dX, M, V, Ny, Nx, nstate, hw, loc_kind, loc_scale, sigma_o, rho,
+                             dX, dwb, dinfo, dwork, wsb, sC);
+    g_analysis_hooks = nullptr;
+    const int launches = g_launches;
+    cudaStreamSynchronize(sC);
+    cudaStreamSynchronize(sD);
+    cudaStreamSynchronize(sH);
+    cudaError_t ce = cudaGetLastError();
+    if (rc == 0 && ce != cudaSuccess) rc = (int)ce;
+    g_launches = launches;
+    return rc;
+}
 
 int letkf_probe_dfma(double* sink, int blocks, int threads, int iters,
                      unsigned long long* fma_count, void* stream)

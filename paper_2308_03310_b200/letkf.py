@@ -18,6 +18,7 @@ EXPORTS = (
     "letkf_syev_batched", "letkf_syev_workspace_bytes",
     "letkf_analysis_batched", "letkf_analysis_workspace_bytes",
     "letkf_syev_batched_host", "letkf_analysis_batched_host", "letkf_host_release",
+    "letkf_analysis_grid", "letkf_analysis_grid_workspace_bytes", "letkf_analysis_grid_host",
     "letkf_probe_dfma", "letkf_last_launch_count",
     "letkf_profile_enable", "letkf_profile_count", "letkf_profile_record", "letkf_profile_record_start", "letkf_profile_rotations",
     "letkf_set_option", "letkf_status_string", "letkf_version",
@@ -54,6 +55,12 @@ def load():
     lib.letkf_syev_batched_host.restype = ci
     lib.letkf_analysis_batched_host.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, cd, vp, vp, vp, vp]
     lib.letkf_analysis_batched_host.restype = ci
+    lib.letkf_analysis_grid.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, ci, ci, ci, cd, cd, cd, vp, vp, vp, vp, sz, vp]
+    lib.letkf_analysis_grid.restype = ci
+    lib.letkf_analysis_grid_workspace_bytes.argtypes = [ci, ci, ci, ci, ci, ci]
+    lib.letkf_analysis_grid_workspace_bytes.restype = sz
+    lib.letkf_analysis_grid_host.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, ci, ci, ci, cd, cd, cd, vp, vp, vp]
+    lib.letkf_analysis_grid_host.restype = ci
     lib.letkf_host_release.argtypes = []
     lib.letkf_host_release.restype = None
     lib.letkf_probe_dfma.argtypes = [vp, ci, ci, ci, ctypes.POINTER(ctypes.c_ulonglong), vp]
@@ -178,6 +185,40 @@ def analysis_batched(Yb, d, rinv_loc, Xb, rho, Xa=None, want_W=False, want_wbar=
     return dict(Xa=Xa, W=W, wbar=wbar, info=info)
 
 
+def analysis_grid(Yf, yo, Xb, hw, loc_kind, loc_scale, sigma_o, rho, obs_mask=None, Xa=None,
+                  want_wbar=False, info=None, work=None, stream=None):
+    """letkf_analysis_grid: Yf[V][Ny][Nx][M], yo[V][Ny][Nx], Xb[Ny*Nx][nstate][M] (device tensors)
+    -> dict(Xa, wbar, info).  The local observations are gathered inside the library."""
+    lib = load()
+    _dev_f64(Yf, "Yf")
+    _dev_f64(yo, "yo")
+    _dev_f64(Xb, "Xb")
+    V, Ny, Nx, M = Yf.shape
+    nstate = Xb.shape[1]
+    if yo.shape != (V, Ny, Nx) or Xb.shape != (Ny * Nx, nstate, M):
+        raise LetkfError("inconsistent shapes")
+    if obs_mask is not None and (obs_mask.dtype != torch.uint8 or obs_mask.shape != (Ny, Nx)
+                                 or not obs_mask.is_cuda or not obs_mask.is_contiguous()):
+        raise LetkfError("obs_mask must be a contiguous uint8 CUDA tensor [Ny][Nx]")
+    dev = Xb.device
+    if Xa is None:
+        Xa = torch.empty_like(Xb)
+    wbar = torch.empty((Ny * Nx, M), dtype=torch.float64, device=dev) if want_wbar else None
+    if info is None:
+        info = torch.zeros((Ny * Nx,), dtype=torch.int32, device=dev)
+    wb = work.numel() * work.element_size() if work is not None else 0
+    with torch.cuda.device(dev):
+        st = lib.letkf_analysis_grid(_ptr(Yf), _ptr(yo), _ptr(obs_mask), _ptr(Xb), M, V, Ny, Nx, nstate, int(hw),
+                                     int(loc_kind), float(loc_scale), float(sigma_o), float(rho),
+                                     _ptr(Xa), _ptr(wbar), _ptr(info), _ptr(work), wb, _stream(stream))
+    _check(st, "letkf_analysis_grid")
+    return dict(Xa=Xa, wbar=wbar, info=info)
+
+
+def analysis_grid_workspace_bytes(M, V, Ny, Nx, hw, nstate):
+    return load().letkf_analysis_grid_workspace_bytes(M, V, Ny, Nx, hw, nstate)
+
+
 def _host_f64(t, name):
     if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
         raise LetkfError(f"{name} must be a contiguous float64 CPU tensor (pinned for full copy speed)")
@@ -226,6 +267,30 @@ def analysis_batched_host(Yb, d, rinv_loc, Xb, rho, Xa=None, want_W=False, want_
                                          float(rho), _ptr(Xa), _ptr(W), _ptr(wbar), _ptr(info))
     _check(st, "letkf_analysis_batched_host")
     return {"Xa": Xa, "W": W, "wbar": wbar, "info": info}
+
+
+def analysis_grid_host(Yf, yo, Xb, hw, loc_kind, loc_scale, sigma_o, rho, obs_mask=None, Xa=None, want_wbar=False):
+    """letkf_analysis_grid_host: the grid form on HOST tensors (pinned recommended); blocks until done."""
+    lib = load()
+    for t, n in ((Yf, "Yf"), (yo, "yo"), (Xb, "Xb")):
+        _host_f64(t, n)
+    V, Ny, Nx, M = Yf.shape
+    nstate = Xb.shape[1]
+    if yo.shape != (V, Ny, Nx) or Xb.shape != (Ny * Nx, nstate, M):
+        raise LetkfError("inconsistent shapes")
+    if obs_mask is not None and (obs_mask.dtype != torch.uint8 or obs_mask.shape != (Ny, Nx) or obs_mask.is_cuda
+                                 or not obs_mask.is_contiguous()):
+        raise LetkfError("obs_mask must be a contiguous uint8 CPU tensor [Ny][Nx]")
+    pin = Xb.is_pinned()
+    if Xa is None:
+        Xa = torch.empty_like(Xb, pin_memory=pin)
+    wbar = torch.empty((Ny * Nx, M), dtype=torch.float64, pin_memory=pin) if want_wbar else None
+    info = torch.zeros((Ny * Nx,), dtype=torch.int32, pin_memory=pin)
+    st = lib.letkf_analysis_grid_host(_ptr(Yf), _ptr(yo), _ptr(obs_mask), _ptr(Xb), M, V, Ny, Nx, nstate, int(hw),
+                                      int(loc_kind), float(loc_scale), float(sigma_o), float(rho),
+                                      _ptr(Xa), _ptr(wbar), _ptr(info))
+    _check(st, "letkf_analysis_grid_host")
+    return dict(Xa=Xa, wbar=wbar, info=info)
 
 
 def host_release():

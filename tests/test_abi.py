@@ -117,3 +117,24 @@ def test_host_entry_points_validate_before_touching_a_device(lib):
     assert ha(fake, fake, fake, null, 8, 3, 2, 4, 1.1, fake, null, null, null) == -4
     assert ha(fake, fake, fake, fake, 8, 3, 2, 4, 1.1, null, null, null, null) == -10
     assert ha(null, null, null, null, 8, 3, 2, 0, 1.1, null, null, null, null) == 0
+
+
+def test_grid_entry_points_validate_before_touching_a_device(lib):
+    null = ctypes.c_void_p(0)
+    fake = ctypes.c_void_p(0x1000)
+    g = lib.letkf_analysis_grid
+    ok = dict(M=8, V=2, Ny=4, Nx=4, ns=2, hw=1, kind=0, L=2.0, sig=0.1, rho=1.1)
+
+    def call(Yf=fake, yo=fake, Xb=fake, Xa=fake, **k):
+        a = dict(ok, **k)
+        return g(Yf, yo, null, Xb, a["M"], a["V"], a["Ny"], a["Nx"], a["ns"], a["hw"], a["kind"], a["L"], a["sig"],
+                 a["rho"], Xa, null, null, null, 0, null)
+    assert call(M=1) == -5 and call(V=0) == -6 and call(Ny=0) == -7 and call(Nx=0) == -8
+    assert call(ns=0) == -9 and call(hw=-1) == -10 and call(kind=2) == -11 and call(L=0.0) == -12
+    assert call(sig=0.0) == -13 and call(rho=-1.0) == -14
+    assert call(Yf=null) == -1 and call(yo=null) == -2 and call(Xb=null) == -4 and call(Xa=null) == -15
+    assert lib.letkf_analysis_grid_workspace_bytes(64, 2, 128, 128, 3, 9) > 0
+    assert lib.letkf_analysis_grid_workspace_bytes(1, 2, 128, 128, 3, 9) == 0
+    h = lib.letkf_analysis_grid_host
+    assert h(fake, fake, null, fake, 1, 2, 4, 4, 2, 1, 0, 2.0, 0.1, 1.1, fake, null, null) == -5
+    assert h(null, fake, null, fake, 8, 2, 4, 4, 2, 1, 0, 2.0, 0.1, 1.1, fake, null, null) == -1
