@@ -26,23 +26,25 @@ __host__ __device__ inline int mid_ld(int M) { return ((M + 1 + 13) / 16) * 16 +
 constexpr int MID_TPR = 4;     // threads per row in mid_tridiag_formq
 static inline size_t mid_tridiag_smem(int M)
 {
-    return sizeof(double) * ((size_t)M * mid_ld(M) + 3 * ((size_t)mid_ld(M)) + (size_t)MID_TPR * mid_threads(M) + 32);
+    return sizeof(double) * ((size_t)M * mid_ld(M) + 3 * ((size_t)mid_ld(M)) + (size_t)MID_TPR * mid_threads(M) + 64 + 8);
 }
 static inline size_t mid_apply_smem(int M, int swcap)
 {
     return sizeof(double) * ((size_t)M * (M + 1) + 4 * (size_t)M) + sizeof(uint32_t) * (size_t)swcap + sizeof(int) * (size_t)M + 32;
 }
 
-// Block-wide sum for a run-time number of warps (<= 20); two barriers; all threads get the result.
-__device__ __forceinline__ double mid_block_sum(double v, double* red, int nwarps)
+// Block-wide sum for a run-time number of warps (<= 20); ONE barrier: consecutive calls alternate
+// between two scratch rows (`which`), so a warp that runs ahead into the next call cannot
+// overwrite partial sums that a slower warp is still reading.  All threads get the result.
+__device__ __forceinline__ double mid_block_sum(double v, double* red, int nwarps, int which)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double* row = red + which * 32;
     v = warp_sum(v);
-    if (lane == 0) red[warp] = v;
+    if (lane == 0) row[warp] = v;
     __syncthreads();
     double t = 0.0;
-    for (int w = 0; w < nwarps; ++w) t += red[w];
-    __syncthreads();
+    for (int w = 0; w < nwarps; ++w) t += row[w];
     return t;
 }
 
@@ -61,7 +63,7 @@ mid_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, int M
     double* wsm  = vs + LD;                  // [LD]
     double* taus = wsm + LD;                 // [LD]
     double* pd   = taus + LD;                // [TPR][RP] partial products
-    double* red  = pd + MID_TPR * RP;        // [32]
+    double* red  = pd + MID_TPR * RP;        // [2][32]
     const int tid = threadIdx.x, j = tid % RP, h = tid / RP, nw = blockDim.x >> 5;
     const size_t b = blockIdx.x;
     const double* A = A_ + b * M * M;
@@ -85,7 +87,7 @@ mid_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, int M
 
     for (int i = M - 1; i >= 1; --i) {
         const double xj = (j < i) ? S[j * LD + i] : 0.0;
-        const double sigma = mid_block_sum((h == 0 && j < i - 1) ? xj * xj : 0.0, red, nw);
+        const double sigma = mid_block_sum((h == 0 && j < i - 1) ? xj * xj : 0.0, red, nw, 0);
         const double alpha = S[(i - 1) * LD + i];
         double tau = 0.0, scal = 0.0, beta = alpha;                // sigma == 0: H_i = I (reading G19)
         if (sigma != 0.0) {
@@ -106,6 +108,7 @@ mid_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, int M
         if (tau != 0.0) {
             double a0 = 0.0, a1 = 0.0;
             if (j < i) {
+#pragma unroll 4
                 for (int p = h; p < npair; p += MID_TPR) {
                     const double2 r = row2[p], v = v2[p];
                     a0 = fma(r.x, v.x, a0);
@@ -120,11 +123,12 @@ mid_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, int M
                 for (int hh = 0; hh < MID_TPR; ++hh) pj += pd[hh * RP + j];
                 pj *= tau;
             }
-            const double ptv = mid_block_sum(h == 0 ? pj * vj : 0.0, red, nw);
+            const double ptv = mid_block_sum(h == 0 ? pj * vj : 0.0, red, nw, 1);
             const double wj = pj - (0.5 * tau * ptv) * vj;        // w = p - (tau/2)(p.v) v
             if (h == 0 && j <= i && j < M) wsm[j] = (j < i) ? wj : 0.0;
             __syncthreads();
             if (j < i) {                                           // S11 -= v w^T + w v^T
+#pragma unroll 4
                 for (int p = h; p < npair; p += MID_TPR) {
                     double2 r = row2w[p];
                     const double2 v = v2[p], w = w2[p];
@@ -134,9 +138,8 @@ mid_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, int M
                 }
             }
         }
-        __syncthreads();                                           // updates done before row i is reused
-        if (h == 0 && j < i) S[i * LD + j] = vj;                   // keep the reflector in the dead row i
-        if (h == 1 && j == 0) S[i * LD + i] = 0.0;                 // (pair overhang of the reflector row)
+        if (h == 0 && j < i) S[i * LD + j] = vj;                   // keep the reflector in the dead row i (no
+        if (h == 1 && j == 0) S[i * LD + i] = 0.0;                 // update touches it); (pair overhang)
         __syncthreads();
     }
     if (tid == 0) { dws[0] = S[0]; ews[M - 1] = 0.0; }
@@ -156,6 +159,7 @@ mid_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, int M
         if (tau != 0.0) {
             double a0 = 0.0, a1 = 0.0;
             if (j < i) {
+#pragma unroll 4
                 for (int p = h; p < npair; p += MID_TPR) {
                     const double2 r = row2[p], v = v2[p];
                     a0 = fma(r.x, v.x, a0);
@@ -169,6 +173,7 @@ mid_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, int M
 #pragma unroll
                 for (int hh = 0; hh < MID_TPR; ++hh) acc += pd[hh * RP + j];
                 acc *= -tau;
+#pragma unroll 4
                 for (int p = h; p < npair; p += MID_TPR) {
                     double2 r = row2w[p];
                     const double2 v = v2[p];
