@@ -271,6 +271,20 @@ def run_ours(args):
         step()
     barrier()
     assert int(info.abs().max()) == 0, "QL did not converge on the bench workload"
+    if args.timeline:
+        # one pipelined step with CUDA events around every kernel on the private stream it runs on
+        # (letkf_profile_enable(2)): the evidence that QL overlaps the other two kernels
+        letkf.profile_enable(2)
+        step()
+        torch.cuda.synchronize()
+        if rank == 0:
+            print("# kernel, start ms (relative to the first launch), duration ms, end ms")
+            for name, t0, ms in letkf.profile_timeline():
+                print(f"{name:28s} {t0:8.3f} {ms:8.3f} {t0 + ms:8.3f}")
+        letkf.profile_enable(0)
+        if world > 1:
+            dist.destroy_process_group()
+        return
     launches_per_step = letkf.last_launch_count()
 
     # ---- timed region: K steps as a user runs them (sub-chunk pipeline on), CUDA events on the
@@ -540,6 +554,7 @@ def main():
     ap.add_argument("--no-analysis", action="store_true")
     ap.add_argument("--no-cusolver", action="store_true")
     ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--timeline", action="store_true", help="print the kernel timeline of one pipelined step and exit")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
