@@ -6,8 +6,9 @@
 // FMAs per clock but shared memory delivers only 16 doubles per clock, so BLAS-2 work fed from
 // shared memory cannot pass 25% of the fp64 peak; here shared memory only carries the
 // broadcast vectors (one LDS.128 feeds two FMAs in every lane).  Register arrays need
-// compile-time indices, so every loop whose bounds move with the reduction step is a fully
-// unrolled block entered through a jump table (a switch with fall-through cases).
+// compile-time indices: the reduction runs in groups of 8 pivots with statically shaped 8-column
+// block loops (pivot_group<G>), the rotation replay in blocks of 4 rotations entered through a
+// switch with fall-through cases (apply_sweep).
 //
 //   fast_tridiag_formq<MT>   a3 + explicit Q  : thread j = row j of A, then column r of Q
 //   ql_log_kernel            a4               : ql_kernel.cuh, one thread per matrix
@@ -38,85 +39,6 @@ __device__ __forceinline__ double pick(const double (&a)[MT], int i)
 #undef LETKF_PICK
     }
     return x;
-}
-
-// The three BLAS-1 shapes below run over c < 8*(gtop+1) in blocks of 8 columns, entered at block
-// gtop through a jump table and falling through to block 0.  Entry only at block granularity: a
-// load may not be hoisted above its own case label, so with one label per element every LDS sat
-// directly in front of the FMA that needs it (measured: short-scoreboard stall 4.2 per issue,
-// profiles/).  With 8-column blocks the 4-8 LDS.128 of a block are issued back to back.  The
-// callers keep the shared vectors ZERO beyond the active length, so the overhang is harmless.
-#define LETKF_REP8_DESC(X) X(7) X(6) X(5) X(4) X(3) X(2) X(1) X(0)
-
-// acc = sum_{c < 8*(gtop+1)} a[c] * vec[c]          (vec in shared memory, 16-byte aligned)
-template <int MT>
-__device__ __forceinline__ double dot_desc(const double (&a)[MT], const double* vec, int gtop)
-{
-    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0, s4 = 0.0, s5 = 0.0, s6 = 0.0, s7 = 0.0;
-    const double2* v2 = reinterpret_cast<const double2*>(vec);
-    switch (gtop) {
-#define LETKF_DOT(g)                                                          \
-    case g:                                                                   \
-        if constexpr (8 * (g) + 7 < MT) {                                     \
-            const double2 t0 = v2[4 * (g)], t1 = v2[4 * (g) + 1];             \
-            const double2 t2 = v2[4 * (g) + 2], t3 = v2[4 * (g) + 3];         \
-            s0 = fma(a[8 * (g)],     t0.x, s0); s1 = fma(a[8 * (g) + 1], t0.y, s1); \
-            s2 = fma(a[8 * (g) + 2], t1.x, s2); s3 = fma(a[8 * (g) + 3], t1.y, s3); \
-            s4 = fma(a[8 * (g) + 4], t2.x, s4); s5 = fma(a[8 * (g) + 5], t2.y, s5); \
-            s6 = fma(a[8 * (g) + 6], t3.x, s6); s7 = fma(a[8 * (g) + 7], t3.y, s7); \
-        }
-        LETKF_REP8_DESC(LETKF_DOT)
-#undef LETKF_DOT
-    }
-    return ((s0 + s1) + (s2 + s3)) + ((s4 + s5) + (s6 + s7));
-}
-
-// a[c] -= alpha * vec[c]   for c < 8*(gtop+1)
-template <int MT>
-__device__ __forceinline__ void axpy_desc(double (&a)[MT], const double* vec, double alpha, int gtop)
-{
-    const double2* v2 = reinterpret_cast<const double2*>(vec);
-    const double na = -alpha;
-    switch (gtop) {
-#define LETKF_AXPY(g)                                                         \
-    case g:                                                                   \
-        if constexpr (8 * (g) + 7 < MT) {                                     \
-            const double2 t0 = v2[4 * (g)], t1 = v2[4 * (g) + 1];             \
-            const double2 t2 = v2[4 * (g) + 2], t3 = v2[4 * (g) + 3];         \
-            a[8 * (g)]     = fma(na, t0.x, a[8 * (g)]);     a[8 * (g) + 1] = fma(na, t0.y, a[8 * (g) + 1]); \
-            a[8 * (g) + 2] = fma(na, t1.x, a[8 * (g) + 2]); a[8 * (g) + 3] = fma(na, t1.y, a[8 * (g) + 3]); \
-            a[8 * (g) + 4] = fma(na, t2.x, a[8 * (g) + 4]); a[8 * (g) + 5] = fma(na, t2.y, a[8 * (g) + 5]); \
-            a[8 * (g) + 6] = fma(na, t3.x, a[8 * (g) + 6]); a[8 * (g) + 7] = fma(na, t3.y, a[8 * (g) + 7]); \
-        }
-        LETKF_REP8_DESC(LETKF_AXPY)
-#undef LETKF_AXPY
-    }
-}
-
-// a[c] -= vj * p[c] + wj * v[c]   for c < 8*(gtop+1);  vp[c] = (v_c, p_c)
-template <int MT>
-__device__ __forceinline__ void rank2_desc(double (&a)[MT], const double2* vp, double vj, double wj, int gtop)
-{
-    const double nv = -vj, nw = -wj;
-    switch (gtop) {
-#define LETKF_R2E(c) a[c] = fma(nv, vp_##c.y, fma(nw, vp_##c.x, a[c]));
-#define LETKF_R2(g)                                                           \
-    case g:                                                                   \
-        if constexpr (8 * (g) + 7 < MT) {                                     \
-            _Pragma("unroll")                                                 \
-            for (int h = 0; h < 2; ++h) {                                     \
-                const double2 u0 = vp[8 * (g) + 4 * h],     u1 = vp[8 * (g) + 4 * h + 1]; \
-                const double2 u2 = vp[8 * (g) + 4 * h + 2], u3 = vp[8 * (g) + 4 * h + 3]; \
-                a[8 * (g) + 4 * h]     = fma(nv, u0.y, fma(nw, u0.x, a[8 * (g) + 4 * h]));     \
-                a[8 * (g) + 4 * h + 1] = fma(nv, u1.y, fma(nw, u1.x, a[8 * (g) + 4 * h + 1])); \
-                a[8 * (g) + 4 * h + 2] = fma(nv, u2.y, fma(nw, u2.x, a[8 * (g) + 4 * h + 2])); \
-                a[8 * (g) + 4 * h + 3] = fma(nv, u3.y, fma(nw, u3.x, a[8 * (g) + 4 * h + 3])); \
-            }                                                                 \
-        }
-        LETKF_REP8_DESC(LETKF_R2)
-#undef LETKF_R2
-#undef LETKF_R2E
-    }
 }
 
 // ---- statically shaped BLAS-1 pieces of the reduction (pivot group G: columns 0 .. 8G+7) -----
@@ -164,12 +86,6 @@ __device__ __forceinline__ double block_pick(const double (&a)[MT], int k)
     return x;
 }
 
-#ifndef LETKF_PIVOT_FENCE
-#define LETKF_PIVOT_FENCE(MT) false
-#endif
-#ifndef LETKF_TRI_REGS48
-#define LETKF_TRI_REGS48 168
-#endif
 #ifndef LETKF_TRI_REGS64
 #define LETKF_TRI_REGS64 168
 #endif
@@ -308,7 +224,7 @@ __device__ __forceinline__ void pivot_group(double (&a)[MT], const TriShared& sh
         if constexpr (NP > 1) sigma += sh.red[1];
         const double alpha = sh.red[4];
         const double xj = sh.xs[j];
-        const double praw = dot_blocks<MT, G, LETKF_PIVOT_FENCE(MT)>(a, sh.xs);
+        const double praw = dot_blocks<MT, G>(a, sh.xs);
         const double acol = block_pick<MT, G>(a, k);          // A[j][i-1] before the update
         double tau = 0.0, scal = 0.0, beta = alpha;            // sigma == 0: H_i = I (reading G19)
         if (sigma != 0.0) {
@@ -332,7 +248,7 @@ __device__ __forceinline__ void pivot_group(double (&a)[MT], const TriShared& sh
 #pragma unroll
         for (int step = 0; step < (G + 1 > 5 ? G + 1 : 5); ++step) {
             if (step < 5) t += __shfl_xor_sync(FULL, t, 16 >> step);
-            if (step <= G) { axpy_block<MT>(a, sh.pbuf, nvj, G - step); if constexpr (LETKF_PIVOT_FENCE(MT)) __syncwarp(); }
+            if (step <= G) axpy_block<MT>(a, sh.pbuf, nvj, G - step);
         }
         const double nwj = fma(tau * t, vj, -pj);              // -(p_j - tau (p.v) v_j)
         axpy_block<MT>(a, sh.vbuf, nwj, G);
@@ -344,7 +260,7 @@ __device__ __forceinline__ void pivot_group(double (&a)[MT], const TriShared& sh
 #pragma unroll
         for (int step = 0; step < (G > 5 ? G : 5); ++step) {
             if (step < 5) part += __shfl_xor_sync(FULL, part, 16 >> step);
-            if (step < G) { axpy_block<MT>(a, sh.vbuf, nwj, G - 1 - step); if constexpr (LETKF_PIVOT_FENCE(MT)) __syncwarp(); }
+            if (step < G) axpy_block<MT>(a, sh.vbuf, nwj, G - 1 - step);
         }
         if (lane == 0) sh.red[warp] = part;
         part_barrier(NP);                                      // ---- B1 of the next pivot
@@ -432,7 +348,7 @@ grid_gather(GridArgs g, int M, int p, double* __restrict__ Yb, double* __restric
 // a3 + explicit Q for one matrix per CTA.  gram == true: the matrix is not read from A but formed
 // from the LETKF inputs (a1, a2: Eq.17 and the right factor of Eq.14) straight into the registers.
 template <int MT, bool GRAM>
-__global__ void __launch_bounds__(FastCfg<MT>::NT) __maxnreg__((MT == 64) ? LETKF_TRI_REGS64 : (MT == 48 ? LETKF_TRI_REGS48 : (MT == 32 ? 128 : 80)))
+__global__ void __launch_bounds__(FastCfg<MT>::NT) __maxnreg__((MT == 64) ? LETKF_TRI_REGS64 : (MT == 48 ? 168 : (MT == 32 ? 128 : 80)))
 fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Workspace ws, int M,
                    const double* __restrict__ Yb_, const double* __restrict__ d_,
                    const double* __restrict__ r_, int p, double shift, double* __restrict__ gout_,
@@ -566,9 +482,7 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
     }
     // a warp leaves pivot_groups_down when the rows it holds are done (after the B1 that closes
     // the last pivot it took part in), the others carry on with barriers that no longer count it
-#ifndef LETKF_DBG_SKIPRED
     pivot_groups_down<MT, (MT - 2) / 8>(a, sh, M, dws, ews);
-#endif
     __syncwarp();
 
     // ---- explicit Q = H_{M-1} ... H_1: thread r owns column r of Q; no synchronisation needed.
@@ -578,9 +492,7 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
     double (&q)[MT] = a;
 #pragma unroll
     for (int c = 0; c < MT; ++c) q[c] = (c == j) ? 1.0 : 0.0;
-#ifndef LETKF_DBG_SKIPQ
     q_groups_up<MT, 0, (MT - 2) / 8>(q, R, taus, M, warp * 4);
-#endif
     if (j < M) {
         double* Q = Q_ + b * M * M;
 #pragma unroll
