@@ -526,6 +526,27 @@ def run_ours(args):
                               "info_nonzero": int((infos != 0).sum())})
                 del As, Vs, ws_, wk, infos
             line["sweep"] = sweep
+            # the paper's Table I shapes (batch 16384 at M = 16, 32, 48, 64, A100 FP32:
+            # 1.3 / 2.4 / 7.8 / 14.2 ms) and its 64-GPU share of 256 matrices per GPU
+            shapes = []
+            for Ms, ps in ((16, 49), (32, 49), (48, 49), (64, 98)):
+                for Bs in (16384, 256):
+                    As = torch.from_numpy(wl.letkf_shaped(Bs, Ms, ps, config_index=80 + Ms)).cuda()
+                    ws_ = torch.empty((Bs, Ms), dtype=torch.float64, device="cuda")
+                    Vs = torch.empty_like(As)
+                    wk = torch.empty(letkf.syev_workspace_bytes(Ms, Bs), dtype=torch.uint8, device="cuda")
+                    for _ in range(3):
+                        letkf.syev_batched(As, w=ws_, V=Vs, work=wk, stream=stream)
+                    torch.cuda.synchronize()
+                    e0.record(stream)
+                    for _ in range(10):
+                        letkf.syev_batched(As, w=ws_, V=Vs, work=wk, stream=stream)
+                    e1.record(stream)
+                    torch.cuda.synchronize()
+                    sms = e0.elapsed_time(e1) / 10
+                    shapes.append({"M": Ms, "batch": Bs, "ms": round(sms, 4), "matrices_per_s": Bs / (sms * 1e-3)})
+                    del As, Vs, ws_, wk
+            line["paper_shapes_fp64"] = shapes
             A = torch.from_numpy(A_host).cuda()
         # ---- cuSOLVER on the same matrices (comparison only)
         if not args.no_cusolver:
