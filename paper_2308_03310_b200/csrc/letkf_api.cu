@@ -96,13 +96,15 @@ static int syev_chunk(int M, int batch)
     return (int)c;
 }
 
+static int g_log_shrink = 1;             // letkf_set_option("log_shrink", k): tests force the slow path
+
 static size_t carve(Workspace& ws, void* base, int M, int chunk)
 {
     char* p = reinterpret_cast<char*>(base);
     size_t off = 0;
     auto take = [&](size_t bytes) { char* q = p ? p + off : nullptr; off = align_up(off + bytes, 256); return q; };
     ws.swcap = sweep_capacity(M);
-    ws.logcap = log_capacity(M);
+    ws.logcap = log_capacity(M) / g_log_shrink;       // (the memory is still sized for the full log)
     ws.rot_counter = g_prof.on ? g_prof.d_rot : nullptr;
     ws.dws     = reinterpret_cast<double*>(take(sizeof(double) * (size_t)M * chunk));
     ws.ews     = reinterpret_cast<double*>(take(sizeof(double) * (size_t)M * chunk));
@@ -1029,6 +1031,7 @@ int letkf_set_option(const char* name, int value)
     if (!name) return -1;
     if (strcmp(name, "force_generic") == 0) { g_force_generic = value != 0; return LETKF_OK; }
     if (strcmp(name, "pipeline") == 0) { g_pipeline = value != 0; return LETKF_OK; }
+    if (strcmp(name, "log_shrink") == 0) { g_log_shrink = value >= 1 ? value : 1; return LETKF_OK; }
     if (strcmp(name, "ql_tpb") == 0) { g_ql_tpb = (value == 32 || value == 64 || value == 96) ? value : 0; return LETKF_OK; }
     return -1;
 }

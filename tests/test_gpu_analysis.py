@@ -163,3 +163,17 @@ def test_fused_epilogue_vs_oracle(lk, oracle, M, p, ns, batch):
     parity.assert_analysis(out, ref, inp["Xb"], f"fused M={M} p={p} ns={ns}")
     full = run_gpu(lk, inp, want_W=True, want_wbar=True)
     parity.assert_analysis(out, full, inp["Xb"], f"fused vs unfused M={M} p={p} ns={ns}")
+
+
+def test_fused_analysis_on_the_slow_path(lk, oracle):
+    """Log overflow inside the fused analysis: fast_apply<epilogue> skips the flagged points, the
+    finisher completes their EVD and generic_epilogue(flagged) their a6-a9."""
+    inp = wl.analysis_inputs(batch=150, M=64, p=98, nstate=9, config_index=45)
+    ref = run_oracle(oracle, inp)
+    try:
+        lk.set_option("log_shrink", 3)
+        out = run_gpu(lk, inp, want_W=False, want_wbar=True)
+    finally:
+        lk.set_option("log_shrink", 1)
+    assert ((out["info"] & 0xFFFF) == 0).all() and (out["info"] & lk.INFO_SLOWPATH).astype(bool).all()
+    parity.assert_analysis(out, ref, inp["Xb"], "fused analysis, slow path")

@@ -244,3 +244,23 @@ def test_host_entry_point_equals_device_call(lk, pinned):
     assert torch.equal(w, wd.cpu()) and torch.equal(V, Vd.cpu()) and torch.equal(info, idv.cpu())
     w2, V2, _ = lk.syev_batched_host(Ah.clone(), V=None)          # second call reuses the streams
     assert torch.equal(V2, V)
+
+
+@pytest.mark.parametrize("M,batch", [(64, 2100), (48, 300), (100, 12)])
+def test_log_overflow_slow_path(lk, oracle, M, batch):
+    """With the rotation log shrunk the QL kernel flags matrices whose log would overflow and the
+    finisher (classic in-kernel QL on the stored Q) completes them: same tolerances, and info
+    carries LETKF_INFO_SLOWPATH for exactly those matrices."""
+    A = wl.letkf_shaped(batch, M, 98 if M >= 64 else 49, config_index=930 + M)
+    try:
+        lk.set_option("log_shrink", 3)
+        w, V, info = run_gpu(lk, A)
+    finally:
+        lk.set_option("log_shrink", 1)
+    assert ((info & 0xFFFF) == 0).all()
+    assert (info & lk.INFO_SLOWPATH).astype(bool).all(), "every matrix should have taken the slow path"
+    wo, _, _, _ = oracle.syev_batched(A[:64])
+    parity.assert_evd(A, w, V, None, f"slow path M={M}")
+    assert np.abs(w[:64] - wo).max() <= parity.TOL_W * np.abs(wo).max()
+    w2, V2, info2 = run_gpu(lk, A)
+    assert (info2 == 0).all() and np.abs(w2 - w).max() <= parity.TOL_W * np.abs(w).max()
