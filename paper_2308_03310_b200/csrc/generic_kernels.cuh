@@ -174,8 +174,8 @@ generic_apply_one(double* V_, double* __restrict__ w_, const Workspace& ws, int 
     } else {
         for (int k = tid; k < M; k += GEN_NT) { dsm[k] = ws.dws[b * M + k]; esm[k] = ws.ews[b * M + k]; }
         __syncthreads();
-        QLState st{0, 0, 0};
-        if (tid == 0) esm[M - 1] = 0.0;
+        QLState st{0, 0, 0, 0.0};
+        if (tid == 0) { esm[M - 1] = 0.0; st.thr = ql_threshold(dsm, esm, 1, M); }
         for (;;) {
             if (tid == 0) {
                 int lo = 0, m = 0;

@@ -58,12 +58,13 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
     // just produced, so the per-sweep rescan disappears (it was 30% of this kernel, profiles/r01a);
     // a scan is needed only when l enters a part of the matrix no sweep of this block has seen.
     const double eps = 1.1102230246251565e-16;   // 2^-53 (reading G10)
+    const double thr = valid ? ql_threshold(d, e, stride, M) : 0.0;   // 2^-53 max_i(|d_i| + |e_i|)
 #define QL_D(i) d[(i) * stride]
 #define QL_E(i) e[(i) * stride]
     auto scan_end = [&](int from) {
         int k = from;
         for (; k < M - 1; ++k)
-            if (fabs(QL_E(k)) <= eps * (fabs(QL_D(k)) + fabs(QL_D(k + 1)))) break;
+            if (fabs(QL_E(k)) <= fmax(eps * (fabs(QL_D(k)) + fabs(QL_D(k + 1))), thr)) break;
         QL_E(k) = 0.0;
         return k;
     };
@@ -81,7 +82,7 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
                 m = scan_end(l);
                 continue;
             }
-            if (iter >= 30) {                          // give up on this one (info counts it)
+            if (iter >= QL_MAX_SWEEPS) {               // give up on this one (info counts it)
                 fail += 1; QL_E(l) = 0.0; m = l;
                 continue;
             }
@@ -154,7 +155,7 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
                     pd[stride] = dnew;
                     *outp++ = make_double2(c, s);
                     // deflation test of index i+1 on this sweep's values (d[i+2] = dprev)
-                    if (i + 1 < m && fabs(enew) <= eps * (fabs(dnew) + fabs(dprev))) mlow = i + 1;
+                    if (i + 1 < m && fabs(enew) <= fmax(eps * (fabs(dnew) + fabs(dprev)), thr)) mlow = i + 1;
                     dprev = dnew;
                     di1 = di; di = din; ei = ein;
                     pd += nxt; pe += nxt;
@@ -180,13 +181,13 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
                 m = mlow;
                 // eigenvalue l converged: the next block starts at l+1 and ends at mlow, the lowest
                 // negligible off-diagonal this sweep has seen above l -- no rescan
-                if (fabs(g) <= eps * (fabs(dl) + fabs(dprev))) { QL_E(l) = 0.0; l += 1; iter = 0; }
+                if (fabs(g) <= fmax(eps * (fabs(dl) + fabs(dprev)), thr)) { QL_E(l) = 0.0; l += 1; iter = 0; }
             }
         }
     }
 #undef QL_D
 #undef QL_E
-    QLState st{0, 0, fail};
+    QLState st{0, 0, fail, thr};
     if (valid) {
         if (!overflow) sort_eigenvalues(d, QL_TPB, reinterpret_cast<int*>(e), QL_TPB * 2, M);
         ws.nsweeps[b] = nsw;

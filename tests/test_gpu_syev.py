@@ -264,3 +264,39 @@ def test_log_overflow_slow_path(lk, oracle, M, batch):
     assert np.abs(w[:64] - wo).max() <= parity.TOL_W * np.abs(wo).max()
     w2, V2, info2 = run_gpu(lk, A)
     assert (info2 == 0).all() and np.abs(w2 - w).max() <= parity.TOL_W * np.abs(w).max()
+
+
+@pytest.mark.parametrize("M", [21, 48, 64, 100])
+def test_hard_spectra(lk, oracle, M):
+    """Matrices that stress the tridiagonal eigensolver and the deflation logic: Wilkinson W+ (pairs of
+    eigenvalues agreeing to ~1e-14), two of them glued by a tiny coupling, graded matrices over
+    many orders of magnitude (up and down), a rank-one update of the identity (an (M-1)-fold
+    cluster), a negative-definite matrix, an arrowhead, and entries at both ends of the documented
+    range (1e-100 < max|A| < 1e100).  Residual / orthogonality at tolerance, eigenvalues against
+    the oracle."""
+    rng = np.random.Generator(np.random.Philox(key=4242 + M))
+    mats = []
+    k = (M - 1) // 2
+    Wk = np.diag(np.abs(np.arange(M) - k).astype(float)) + np.diag(np.ones(M - 1), 1) + np.diag(np.ones(M - 1), -1)
+    mats.append(Wk)                                                        # Wilkinson W+
+    G = Wk.copy(); G[M // 2, M // 2 - 1] = G[M // 2 - 1, M // 2] = 1e-9    # glued halves
+    mats.append(G)
+    Q, _ = np.linalg.qr(rng.standard_normal((M, M)))
+    mats.append(Q @ np.diag(10.0 ** np.linspace(-12, 6, M)) @ Q.T)         # wide spectrum, dense
+    s = 10.0 ** np.linspace(0, 8, M)
+    B = rng.standard_normal((M, M)); B = B + B.T
+    mats.append(B * np.outer(s, s) / s[-1] ** 2)                           # graded downwards
+    mats.append((B * np.outer(s, s) / s[-1] ** 2)[::-1, ::-1].copy())      # graded upwards
+    u = rng.standard_normal(M)
+    mats.append(np.eye(M) + np.outer(u, u))                                # (M-1)-fold cluster at 1
+    mats.append(-(B @ B.T) - np.eye(M))                                    # negative definite
+    Ar = np.diag(np.arange(1.0, M + 1)); Ar[-1, :-1] = Ar[:-1, -1] = 0.5   # arrowhead
+    mats.append(Ar)
+    mats.append(B * 1e-99)
+    mats.append(B * 1e98)
+    A = np.stack([0.5 * (X + X.T) for X in mats])
+    w, V, info = run_gpu(lk, A)
+    assert (info == 0).all()
+    wo, _, io, _ = oracle.syev_batched(A)
+    assert (io == 0).all()
+    parity.assert_evd(A, w, V, wo, f"hard spectra M={M}")
