@@ -42,8 +42,8 @@ extern "C" {
 #define LETKF_INFO_SLOWPATH 0x40000000 /* the matrix was finished by the in-kernel slow path
                                           (rotation log full); result is still valid       */
 /* info[b] & 0xFFFF = number of off-diagonal elements that had not converged after 60
- * QL iterations each ("implicit QL method ... as in EISPACK/LAPACK"; cap as in
- * EISPACK tql2).  Non-zero means w/V of that matrix are not to be trusted.                */
+ * QL iterations each ("implicit QL method ... as in EISPACK/LAPACK"; twice the
+ * cap of EISPACK tql2).  Non-zero means w/V of that matrix are not to be trusted.                */
 
 /*
  * Batched symmetric eigenvalue decomposition -- the paper's "main computing kernel"
