@@ -266,7 +266,7 @@ def test_log_overflow_slow_path(lk, oracle, M, batch):
     assert (info2 == 0).all() and np.abs(w2 - w).max() <= parity.TOL_W * np.abs(w).max()
 
 
-@pytest.mark.parametrize("M", [21, 48, 64, 100])
+@pytest.mark.parametrize("M", [21, 48, 64, 100, 160, 200])
 def test_hard_spectra(lk, oracle, M):
     """Matrices that stress the tridiagonal eigensolver and the deflation logic: Wilkinson W+ (pairs of
     eigenvalues agreeing to ~1e-14), two of them glued by a tiny coupling, graded matrices over
