@@ -504,9 +504,13 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
 // ---------------------------------------------------------------------------------------------
 // a5: V = Q Z by replaying the logged rotations; thread r owns row r of Q in registers.
 // Dynamic shared memory: tile[MT*(MT+1)], cs[2][MT] double2, hdr[swcap] u32, inv[MT] int
-constexpr int AP_S = 4;      // sweeps staged per barrier round
+constexpr int AP_S = 8;      // sweeps staged per barrier round (measured: 2 / 4 / 8 -> 2.05 / 1.99 / 1.93 ms)
 // tile of fast_apply: HT = min(MT, 32) padded rows (the matrix passes through it 32 rows at a time)
-template <int MT> __host__ __device__ constexpr int ap_tile_doubles() { return ((MT < 32 ? MT : 32) * (MT + 1) + 3) & ~1; }
+template <int MT> __host__ __device__ constexpr int ap_tile_doubles()
+{
+    constexpr int tile = (MT < 32 ? MT : 32) * (MT + 1), cs = 4 * AP_S * MT;    // the staged rotations alias the tile
+    return ((tile > cs ? tile : cs) + 3) & ~1;
+}
 // a6-a9 fused into the tail of fast_apply (the analysis call when W is not wanted): V never
 // goes to HBM.  lam = eigenvalues ascending (output order), g = Yb^T (r o d), Eq.14.
 struct EpiArgs {
