@@ -392,73 +392,137 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
             }
         }
     } else {
-        // a_j[c] = shift*delta + sum_i r_i Yb[i][j] Yb[i][c];  Yb rows staged through the tile
+        // a1/a2 on the FP64 tensor cores.  A = shift I + Yb^T diag(r) Yb is a dense contraction
+        // over the p local observations, so it runs as mma.sync.m8n8k4.f64 (DMMA): measured on this
+        // B200 the instruction reaches the full fp64 rate (37.2 TFLOP/s, the DFMA peak) with 8x fewer
+        // issue slots, and the rank-1 DFMA form of this step was issue bound at 35% of peak.
+        //   warp w owns rows 32w .. 32w+31 of A: up to 4 row tiles x MT/8 column tiles of 8x8,
+        //   64 accumulator doubles per lane (exactly the registers a[] needs afterwards);
+        //   the observations are staged 4-row-interleaved, Ys[kk][col][4], so that a fragment
+        //   (row i = lane%4 of the k-step, column = 8 tile + lane/4) is 32 consecutive doubles;
+        //   the A fragment of row tile rt is the B fragment of column tile rt times r_i.
         const bool gridded = grid.Yf != nullptr;
         const double* Yb = gridded ? nullptr : Yb_ + b * (size_t)p * M;
         const double* dv = gridded ? nullptr : d_ + b * (size_t)p;
         const double* rv = gridded ? nullptr : r_ + b * (size_t)p;
         const int pt = grid.point0 + (int)b, gy = gridded ? pt / grid.Nx : 0, gx = gridded ? pt - gy * grid.Nx : 0;
-        // per-row scalars of the staged rows (the small vectors are free until the reduction starts)
-        constexpr int RB = (RefLayout<MT>::HT < C::NT / 2) ? RefLayout<MT>::HT : C::NT / 2;   // rows per stage
-        double* rloc = sh.xs;                                   // [RB]
-        double* dloc = sh.xs + RB;                              // [RB]
-        double* mloc = sh.vbuf;                                 // [RB]  ensemble mean of the row (grid form)
-        long*   oloc = reinterpret_cast<long*>(sh.pbuf);        // [RB]  observed point of the row (grid form)
+        constexpr int CT = MT / 8;                                   // column tiles (= row tiles of A)
+        constexpr int KBR = (RefLayout<MT>::REGION / MT) / 4 * 4;    // rows the region can stage
+        constexpr int RB0 = KBR < 32 ? KBR : 32;
+        constexpr int RB = (RB0 < C::NT / 2) ? RB0 : C::NT / 2;      // observation rows per stage (multiple of 4)
+        static_assert(RB % 4 == 0 && RB >= 4, "stage size");
+        double* Ys = tile;                                           // [RB/4][MT][4]
+        double* rloc = sh.xs;                                        // [RB] weight of the staged row
+        double* dloc = sh.xs + RB;                                   // [RB] innovation
+        double* mloc = sh.vbuf;                                      // [RB] ensemble mean of the row (grid form)
+        long*   oloc = reinterpret_cast<long*>(sh.pbuf);             // [RB] observed point of the row (grid form)
+        double acc[4][CT][2];
 #pragma unroll
-        for (int c = 0; c < MT; ++c) a[c] = (c == j && j < M) ? shift : 0.0;
+        for (int t = 0; t < 4; ++t)
+#pragma unroll
+            for (int ct = 0; ct < CT; ++ct) { acc[t][ct][0] = 0.0; acc[t][ct][1] = 0.0; }
         double gj = 0.0;
+        const int rt0 = 4 * warp;                                    // first row tile of this warp
         for (int i0 = 0; i0 < p; i0 += RB) {
             const int nr = min(RB, p - i0);
-            if (j < nr) {
-                if (gridded) {
-                    long off; double rl;
-                    grid_row(grid, gy, gx, i0 + j, off, rl);
-                    const double mean = grid.ybar[off];
-                    oloc[j] = off; mloc[j] = mean; rloc[j] = rl; dloc[j] = grid.yo[off] - mean;
-                } else {
-                    rloc[j] = rv[i0 + j]; dloc[j] = dv[i0 + j];
+            const int nk = (nr + 3) >> 2;                            // k-steps staged (rows padded with r = 0)
+            if (j < 4 * nk) {
+                double rl = 0.0, dl = 0.0;
+                if (j < nr) {
+                    if (gridded) {
+                        long off;
+                        grid_row(grid, gy, gx, i0 + j, off, rl);
+                        const double mean = grid.ybar[off];
+                        oloc[j] = off; mloc[j] = mean; dl = grid.yo[off] - mean;
+                    } else {
+                        rl = rv[i0 + j]; dl = dv[i0 + j];
+                    }
                 }
+                rloc[j] = rl; dloc[j] = dl;
             }
             if (gridded) __syncthreads();
             if (j < MT) {                          // thread j stages column j of every row, 8 in flight
                 int r = 0;
-                if (gridded) {
-                    for (; r + 8 <= nr; r += 8) {
-                        double tmp[8];
+                for (; r + 8 <= nr; r += 8) {
+                    double tmp[8];
 #pragma unroll
-                        for (int u = 0; u < 8; ++u) tmp[u] = (j < M) ? grid.Yf[oloc[r + u] * M + j] - mloc[r + u] : 0.0;
-#pragma unroll
-                        for (int u = 0; u < 8; ++u) tile[(r + u) * MT + j] = tmp[u];
-                    }
-                    for (; r < nr; ++r) tile[r * MT + j] = (j < M) ? grid.Yf[oloc[r] * M + j] - mloc[r] : 0.0;
-                } else {
-                    const double* src = Yb + (size_t)i0 * M + j;
-                    for (; r + 8 <= nr; r += 8) {
-                        double tmp[8];
-#pragma unroll
-                        for (int u = 0; u < 8; ++u) tmp[u] = (j < M) ? src[(size_t)(r + u) * M] : 0.0;
-#pragma unroll
-                        for (int u = 0; u < 8; ++u) tile[(r + u) * MT + j] = tmp[u];
-                    }
-                    for (; r < nr; ++r) tile[r * MT + j] = (j < M) ? src[(size_t)r * M] : 0.0;
+                    for (int u = 0; u < 8; ++u)
+                        tmp[u] = (j < M) ? (gridded ? grid.Yf[oloc[r + u] * M + j] - mloc[r + u]
+                                                    : Yb[(size_t)(i0 + r + u) * M + j]) : 0.0;
+                    double2* y0 = reinterpret_cast<double2*>(Ys + (r >> 2) * (4 * MT) + j * 4);       // r is a multiple of 8:
+                    double2* y1 = reinterpret_cast<double2*>(Ys + ((r >> 2) + 1) * (4 * MT) + j * 4); // two whole k-steps
+                    y0[0] = make_double2(tmp[0], tmp[1]); y0[1] = make_double2(tmp[2], tmp[3]);
+                    y1[0] = make_double2(tmp[4], tmp[5]); y1[1] = make_double2(tmp[6], tmp[7]);
+                }
+                for (; r < 4 * nk; ++r) {
+                    double v = 0.0;
+                    if (r < nr && j < M) v = gridded ? grid.Yf[oloc[r] * M + j] - mloc[r] : Yb[(size_t)(i0 + r) * M + j];
+                    Ys[(r >> 2) * (4 * MT) + j * 4 + (r & 3)] = v;
                 }
             }
             __syncthreads();
-            for (int r = 0; r < nr; ++r) {
-                const double ri = rloc[r];
-                const double yj = tile[r * MT + j];
-                const double yr = yj * ri;
-                gj = fma(yr, dloc[r], gj);
-                const double2* row = reinterpret_cast<const double2*>(tile + r * MT);
+            if (j < MT) {                          // a2: g_j += sum_r Yb[r][j] r_r d_r
+                for (int kk = 0; kk < nk; ++kk) {
+                    const double2* y2 = reinterpret_cast<const double2*>(Ys + kk * (4 * MT) + j * 4);
+                    const double2 y01 = y2[0], y23 = y2[1];
+                    gj = fma(y01.x, rloc[4 * kk] * dloc[4 * kk], gj);
+                    gj = fma(y01.y, rloc[4 * kk + 1] * dloc[4 * kk + 1], gj);
+                    gj = fma(y23.x, rloc[4 * kk + 2] * dloc[4 * kk + 2], gj);
+                    gj = fma(y23.y, rloc[4 * kk + 3] * dloc[4 * kk + 3], gj);
+                }
+            }
+            if (8 * rt0 < MT) {                    // (a warp beyond the matrix has no tiles: MT = 16 in a 32-thread CTA never gets here)
+                for (int kk = 0; kk < nk; ++kk) {
+                    const double* base = Ys + kk * (4 * MT) + lane;
+                    const double rk = rloc[4 * kk + (lane & 3)];
+                    double bfr[CT];
 #pragma unroll
-                for (int q = 0; q < MT / 2; ++q) {
-                    const double2 t = row[q];
-                    a[2 * q]     = fma(yr, t.x, a[2 * q]);
-                    a[2 * q + 1] = fma(yr, t.y, a[2 * q + 1]);
+                    for (int ct = 0; ct < CT; ++ct) bfr[ct] = base[32 * ct];
+#pragma unroll
+                    for (int t = 0; t < 4; ++t) {
+                        if (8 * (rt0 + t) < MT) {
+                            const double afr = base[32 * (rt0 + t)] * rk;   // (= bfr[rt0 + t]; re-read: a run-time
+                                                                            // register index would go to local memory)
+#pragma unroll
+                            for (int ct = 0; ct < CT; ++ct)
+                                asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                                             : "+d"(acc[t][ct][0]), "+d"(acc[t][ct][1]) : "d"(afr), "d"(bfr[ct]));
+                        }
+                    }
                 }
             }
             __syncthreads();
         }
+        // accumulator fragments -> rows in registers: lane l holds A[32w + 8t + l/4][8ct + 2(l%4) + e];
+        // each warp passes ITS rows through shared memory, 32 columns at a time (so that no more than
+        // 64 doubles are live), and its thread j reads back row j: no block barrier needed.
+        constexpr int CH = MT < 32 ? MT : 32;                       // columns per pass
+        constexpr int LDC = (MT * (CH + 2) <= RefLayout<MT>::REGION) ? CH + 2 : CH;
+        double* cbuf = tile + warp * 32 * LDC;
+#pragma unroll
+        for (int c0 = 0; c0 < MT; c0 += CH) {
+            __syncwarp();
+#pragma unroll
+            for (int t = 0; t < 4; ++t)
+#pragma unroll
+                for (int ct = c0 / 8; ct < (c0 + CH) / 8; ++ct)
+                    if (8 * (rt0 + t) < MT)
+                        *reinterpret_cast<double2*>(cbuf + (8 * t + (lane >> 2)) * LDC + (8 * ct - c0) + 2 * (lane & 3)) =
+                            make_double2(acc[t][ct][0], acc[t][ct][1]);
+            __syncwarp();
+            if (j < MT) {
+                const double2* row2 = reinterpret_cast<const double2*>(cbuf + lane * LDC);
+#pragma unroll
+                for (int q = 0; q < CH / 2; ++q) {
+                    const double2 v = row2[q];
+                    a[c0 + 2 * q] = v.x;
+                    a[c0 + 2 * q + 1] = v.y;
+                }
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < MT; ++c) a[c] = (j < M && c < M) ? a[c] + ((c == j) ? shift : 0.0) : 0.0;
+        __syncthreads();
         if (j < M) gout_[b * M + j] = gj;
     }
 
