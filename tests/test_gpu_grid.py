@@ -36,7 +36,10 @@ def run_gpu(lk, g, hw, loc_kind, L, masked=True, **kw):
                           (5, 9, 16, 2, 15, 1, 1, 3.0, 1),
                           (3, 3, 8, 1, 2, 2, 0, 2.0, 1),        # patch wider than the grid: wraps twice
                           (6, 5, 96, 2, 4, 1, 1, 2.0, 2),       # M > 64: materialising gather + mid path
-                          (4, 4, 64, 2, 16, 1, 0, 2.0, 1)])     # nstate > 15: materialising gather
+                          (4, 4, 64, 2, 16, 1, 0, 2.0, 1),      # nstate > 15: materialising gather
+                          (5, 6, 32, 3, 2, 0, 0, 2.0, 1),       # hw = 0: only the point's own observations (p = V)
+                          (1, 9, 24, 1, 2, 2, 1, 2.5, 1),       # a single row: the patch wraps onto itself in y
+                          (7, 1, 64, 2, 9, 1, 0, 2.0, 1)])      # a single column
 def test_grid_vs_oracle(lk, oracle, Ny, Nx, M, V, ns, hw, loc_kind, L, every):
     g = wl.grid_inputs(Ny=Ny, Nx=Nx, M=M, V=V, nstate=ns, config_index=700 + M + Ny, obs_every=every)
     out = run_gpu(lk, g, hw, loc_kind, L)
