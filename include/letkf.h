@@ -207,7 +207,9 @@ int letkf_last_launch_count(void);
  * (otherwise only M > 64 and overflowed matrices use them); "pipeline" = 0 runs every pass as one
  * chunk on the caller's stream instead of the sub-chunk pipeline over private streams (default 1);
  * "ql_tpb" = 32/64/96 matrices per QL CTA (0 = by size); "log_shrink" = k divides the rotation-log
- * capacity by k so that tests can force the log-overflow slow path (default 1).  Returns 0, or -1 for an unknown name. */
+ * capacity by k so that tests can force the log-overflow slow path (default 1); "split" = 1 runs the
+ * tridiagonalisation of 48 < M <= 64 as three kernels (pivots down to 33 / trailing 32 x 32 problem /
+ * explicit Q; experimental, default 0: measured slower than the single kernel).  Returns 0, or -1 for an unknown name. */
 int letkf_set_option(const char* name, int value);
 
 const char* letkf_status_string(int status);

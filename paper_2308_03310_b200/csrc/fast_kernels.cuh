@@ -267,6 +267,15 @@ __device__ __forceinline__ void pivot_group(double (&a)[MT], const TriShared& sh
     }
 }
 
+// groups G ... GLO only
+template <int MT, int G, int GLO>
+__device__ __forceinline__ void pivot_groups_range(double (&a)[MT], const TriShared& sh, int M,
+                                                   double* __restrict__ dws, double* __restrict__ ews)
+{
+    pivot_group<MT, G>(a, sh, M, dws, ews);
+    if constexpr (G > GLO) pivot_groups_range<MT, G - 1, GLO>(a, sh, M, dws, ews);
+}
+
 template <int MT, int G>
 __device__ __forceinline__ void pivot_groups_down(double (&a)[MT], const TriShared& sh, int M,
                                                   double* __restrict__ dws, double* __restrict__ ews)
@@ -347,7 +356,16 @@ grid_gather(GridArgs g, int M, int p, double* __restrict__ Yb, double* __restric
 // ---------------------------------------------------------------------------------------------
 // a3 + explicit Q for one matrix per CTA.  gram == true: the matrix is not read from A but formed
 // from the LETKF inputs (a1, a2: Eq.17 and the right factor of Eq.14) straight into the registers.
-template <int MT, bool GRAM>
+// Split form of the M in (48, 64] reduction (template SPLIT): this kernel
+// stops after pivot 33; the trailing 32 x 32 problem (fast_tridiag_tail, one warp per matrix, 2.5x
+// the CTAs per SM) and the explicit Q (fast_formq, one warp per 32 columns) are kernels of their
+// own, so that no warp sits idle holding registers while another finishes.  Scratch per matrix
+// (aliased onto the matrix's rotation log, which is not written before the QL kernel): doubles
+//   [0, 2304) reflectors in RefLayout order | [2304, 2368) taus | [2368, 3392) trailing 32 x 32 rows
+//   | [3392, 3456) raw pivot column of pivot 32 | [3456, 3464) sigma partial, -, -, -, alpha
+constexpr int SPLIT_TAUS = 2304, SPLIT_TR = 2368, SPLIT_XS = 3392, SPLIT_RED = 3456, SPLIT_DOUBLES = 3464;
+
+template <int MT, bool GRAM, bool SPLIT = false>
 __global__ void __launch_bounds__(FastCfg<MT>::NT) __maxnreg__((MT == 64) ? LETKF_TRI_REGS64 : (MT == 48 ? 168 : (MT == 32 ? 128 : 80)))
 fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Workspace ws, int M,
                    const double* __restrict__ Yb_, const double* __restrict__ d_,
@@ -546,6 +564,22 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
     }
     // a warp leaves pivot_groups_down when the rows it holds are done (after the B1 that closes
     // the last pivot it took part in), the others carry on with barriers that no longer count it
+    if constexpr (SPLIT) {
+        static_assert(MT == 64, "the split form is for the MT = 64 bucket");
+        pivot_groups_range<MT, (MT - 2) / 8, 4>(a, sh, M, dws, ews);
+        __syncthreads();
+        double* sc = reinterpret_cast<double*>(ws.rot + b * ws.logcap);
+        for (int k = RefLayout<MT>::base(4) + j; k < RefLayout<MT>::TOTAL; k += C::NT) sc[k] = sh.R[k];
+        sc[SPLIT_TAUS + j] = (j >= 33) ? sh.taus[j] : 0.0;
+        if (j < 32) {
+            double2* tr = reinterpret_cast<double2*>(sc + SPLIT_TR + j * 32);
+#pragma unroll
+            for (int c = 0; c < 32; c += 2) tr[c >> 1] = make_double2(a[c], a[c + 1]);
+            sc[SPLIT_XS + j] = sh.xs[j];
+            if (j < 8) sc[SPLIT_RED + j] = sh.red[j];
+        }
+        return;
+    } else {
     pivot_groups_down<MT, (MT - 2) / 8>(a, sh, M, dws, ews);
     __syncwarp();
 
@@ -557,6 +591,66 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
 #pragma unroll
     for (int c = 0; c < MT; ++c) q[c] = (c == j) ? 1.0 : 0.0;
     q_groups_up<MT, 0, (MT - 2) / 8>(q, R, taus, M, warp * 4);
+    if (j < M) {
+        double* Q = Q_ + b * M * M;
+#pragma unroll
+        for (int c = 0; c < MT; ++c)
+            if (c < M) Q[(size_t)c * M + j] = q[c];
+    }
+    }
+}
+
+// Trailing 32 x 32 problem of the split form: pivots min(M-1, 32) ... 1, one warp per matrix.
+__global__ void __maxnreg__(128)
+fast_tridiag_tail(Workspace ws, int M)
+{
+    extern __shared__ __align__(16) double sm[];
+    TriShared sh;
+    sh.R = sm;                                   // groups 0..3: 640 doubles
+    double* small = sm + 640;
+    sh.xs = small; sh.vbuf = small + 32; sh.pbuf = small + 64; sh.pv = small + 96;
+    sh.taus = small + 128;                       // [40]
+    sh.red = small + 168;                        // [8]
+    const int j = threadIdx.x;
+    const size_t b = blockIdx.x;
+    double* sc = reinterpret_cast<double*>(ws.rot + b * ws.logcap);
+    double a[32];
+    {
+        const double2* tr = reinterpret_cast<const double2*>(sc + SPLIT_TR + j * 32);
+#pragma unroll
+        for (int c = 0; c < 32; c += 2) { const double2 t = tr[c >> 1]; a[c] = t.x; a[c + 1] = t.y; }
+    }
+    sh.xs[j] = sc[SPLIT_XS + j];
+    if (j < 8) sh.red[j] = sc[SPLIT_RED + j];
+    __syncwarp();
+    const int Mt = M < 33 ? M : 33;
+    pivot_groups_down<32, 3>(a, sh, Mt, ws.dws + b * M, ws.ews + b * M);
+    __syncwarp();
+    for (int k = j; k < 640; k += 32) sc[k] = sh.R[k];
+    sc[SPLIT_TAUS + j] = (j >= 1) ? sh.taus[j] : 0.0;
+    if (j == 0) sc[SPLIT_TAUS + 32] = sh.taus[32];
+}
+
+// Explicit Q of the split form: CTA 2b + h forms columns 32h ... 32h+31 of matrix b.
+__global__ void __maxnreg__(168)
+fast_formq(double* __restrict__ Q_, Workspace ws, int M)
+{
+    constexpr int MT = 64;
+    extern __shared__ __align__(16) double sm[];
+    double* R = sm;                              // [2304]
+    double* taus = sm + 2304;                    // [64]
+    const int lane = threadIdx.x, h = blockIdx.x & 1;
+    const size_t b = blockIdx.x >> 1;
+    const int j = 32 * h + lane;
+    const double* sc = reinterpret_cast<const double*>(ws.rot + b * ws.logcap);
+    for (int k = (h ? RefLayout<MT>::base(4) : 0) + lane; k < RefLayout<MT>::TOTAL; k += 32) R[k] = sc[k];
+    taus[lane] = sc[SPLIT_TAUS + lane];
+    taus[lane + 32] = sc[SPLIT_TAUS + 32 + lane];
+    __syncwarp();
+    double q[MT];
+#pragma unroll
+    for (int c = 0; c < MT; ++c) q[c] = (c == j) ? 1.0 : 0.0;
+    q_groups_up<MT, 0, (MT - 2) / 8>(q, R, taus, M, 4 * h);
     if (j < M) {
         double* Q = Q_ + b * M * M;
 #pragma unroll

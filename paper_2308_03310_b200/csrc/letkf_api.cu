@@ -152,12 +152,34 @@ static bool g_force_generic = false;     // letkf_set_option("force_generic", 1)
 // a1/a2 inputs when the matrix is to be formed from the LETKF observations instead of read
 struct GramArgs { const double* Yb; const double* d; const double* r; int p; double shift; double* gout; GridArgs grid; };
 
+static int g_split = 0;                  // letkf_set_option("split", 1): three-kernel tridiagonalisation for M in (48, 64] (slower so far)
+
 template <int MT>
 static int fast_tridiag_run(const double* A, double* V, Workspace ws, int M, int n, cudaStream_t st,
                             const GramArgs* gram)
 {
     const size_t smem = fast_tridiag_smem<MT>();
     cudaError_t ce;
+    if constexpr (MT == 64) {
+        if (g_split && M > 34 && sizeof(double2) * (size_t)ws.logcap >= sizeof(double) * SPLIT_DOUBLES) {
+            if (gram) {
+                if ((ce = allow_smem(fast_tridiag_formq<MT, true, true>, smem)) != cudaSuccess) return (int)ce;
+                KLAUNCH("fast_tridiag_head<gram>", st,
+                        fast_tridiag_formq<MT, true, true><<<n, FastCfg<MT>::NT, smem, st>>>(
+                            nullptr, V, ws, M, gram->Yb, gram->d, gram->r, gram->p, gram->shift, gram->gout, gram->grid));
+            } else {
+                if ((ce = allow_smem(fast_tridiag_formq<MT, false, true>, smem)) != cudaSuccess) return (int)ce;
+                KLAUNCH("fast_tridiag_head", st,
+                        fast_tridiag_formq<MT, false, true><<<n, FastCfg<MT>::NT, smem, st>>>(
+                            A, V, ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{}));
+            }
+            KLAUNCH("fast_tridiag_tail", st, fast_tridiag_tail<<<n, 32, sizeof(double) * (640 + 176), st>>>(ws, M));
+            const size_t qs = sizeof(double) * (2304 + 64);
+            if ((ce = allow_smem(fast_formq, qs)) != cudaSuccess) return (int)ce;
+            KLAUNCH("fast_formq", st, fast_formq<<<2 * n, 32, qs, st>>>(V, ws, M));
+            return 0;
+        }
+    }
     if (gram) {
         if ((ce = allow_smem(fast_tridiag_formq<MT, true>, smem)) != cudaSuccess) return (int)ce;
         KLAUNCH("fast_tridiag_formq<gram>", st,
@@ -1031,6 +1053,7 @@ int letkf_set_option(const char* name, int value)
     if (!name) return -1;
     if (strcmp(name, "force_generic") == 0) { g_force_generic = value != 0; return LETKF_OK; }
     if (strcmp(name, "pipeline") == 0) { g_pipeline = value != 0; return LETKF_OK; }
+    if (strcmp(name, "split") == 0) { g_split = value != 0; return LETKF_OK; }
     if (strcmp(name, "log_shrink") == 0) { g_log_shrink = value >= 1 ? value : 1; return LETKF_OK; }
     if (strcmp(name, "ql_tpb") == 0) { g_ql_tpb = (value == 32 || value == 64 || value == 96) ? value : 0; return LETKF_OK; }
     return -1;

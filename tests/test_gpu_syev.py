@@ -300,3 +300,18 @@ def test_hard_spectra(lk, oracle, M):
     wo, _, io, _ = oracle.syev_batched(A)
     assert (io == 0).all()
     parity.assert_evd(A, w, V, wo, f"hard spectra M={M}")
+
+
+@pytest.mark.parametrize("M", [64, 57, 49])
+def test_split_tridiagonalisation_option(lk, oracle, M):
+    """letkf_set_option("split", 1): pivots down to 33, the trailing 32 x 32 problem and the explicit
+    Q as three kernels (experimental) -- same tolerances."""
+    A = wl.letkf_shaped(300, M, 98, config_index=940 + M)
+    try:
+        lk.set_option("split", 1)
+        w, V, info = run_gpu(lk, A)
+    finally:
+        lk.set_option("split", 0)
+    assert (info == 0).all()
+    wo, _, _, _ = oracle.syev_batched(A)
+    parity.assert_evd(A, w, V, wo, f"split M={M}")
