@@ -308,7 +308,7 @@ static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws,
 struct Pipe {
     int dev = -1;
     cudaStream_t sT[2] = {nullptr, nullptr}, sA[4] = {};
-    cudaStream_t sQ[8] = {};          // one per sub-chunk: all QL kernels of a pass run side by side
+    cudaStream_t sQ[16] = {};          // one per sub-chunk: all QL kernels of a pass run side by side
     std::vector<cudaEvent_t> ev;
     size_t used = 0;
     int init()
@@ -325,7 +325,7 @@ struct Pipe {
         }
         for (int k = 0; k < 4; ++k)
             if ((ce = cudaStreamCreateWithPriority(&sA[k], cudaStreamNonBlocking, least)) != cudaSuccess) return (int)ce;
-        for (int k = 0; k < 8; ++k)
+        for (int k = 0; k < 16; ++k)
             if ((ce = cudaStreamCreateWithPriority(&sQ[k], cudaStreamNonBlocking, greatest)) != cudaSuccess) return (int)ce;
         ev.clear();
         used = 0;
@@ -353,7 +353,9 @@ static thread_local Pipe g_pipe;
 
 static int g_pipeline = 1;               // letkf_set_option("pipeline", 0): one stream, one chunk
 static const int PIPE_MIN_SUB = 1024;    // smallest sub-chunk worth a launch of its own
-static const int PIPE_MAX_SUB = 8;       // = number of QL streams
+static const int PIPE_MAX_SUB = 16;      // = number of QL streams
+static thread_local int g_max_sub = 8;   // sub-chunks per pass: 8 for device calls (measured best), 16 for the
+                                         // host entry points (finer copy/compute overlap: shorter head and tail)
 
 // One pass: n matrices whose workspace records are ws[0..n).  stageT(b0, nk, stream) enqueues the
 // first stage of matrices [b0, b0+nk); post(b0, nk, stream) whatever follows stage_AP (the
@@ -373,7 +375,7 @@ static EpiArgs epi_slice(const EpiArgs& e, int M, int b0)
 static void pass_partition(int n, int& nsub, int& per)
 {
     nsub = (g_pipeline && (!g_prof.on || g_prof.keep_pipeline)) ? n / PIPE_MIN_SUB : 1;
-    if (nsub > PIPE_MAX_SUB) nsub = PIPE_MAX_SUB;
+    if (nsub > g_max_sub) nsub = g_max_sub;
     if (nsub < 1) nsub = 1;
     per = (n + nsub - 1) / nsub;
 }
@@ -742,6 +744,13 @@ struct HostPipe {
 };
 static thread_local HostPipe g_hpipe;
 
+// the host entry points cut a pass into up to PIPE_MAX_SUB sub-chunks for the duration of the call
+struct HostSubChunks {
+    int old;
+    HostSubChunks() : old(g_max_sub) { g_max_sub = PIPE_MAX_SUB; }
+    ~HostSubChunks() { g_max_sub = old; }
+};
+
 // context of the copy hooks of letkf_syev_batched_host
 struct SyevHostCtx {
     int M, per;                       // sub-chunk size of the pass
@@ -803,6 +812,7 @@ int letkf_syev_batched_host(const double* A, int M, int batch, double* w, double
     carve(ws, base + owk, M, chunk);
     cudaStream_t sH = g_hpipe.s[0], sD = g_hpipe.s[1], sC = g_hpipe.sC;
     int launches = 0;
+    HostSubChunks max_sub_guard;
     for (int b0 = 0; b0 < batch && rc == 0; b0 += chunk) {
         const int n = (batch - b0 < chunk) ? batch - b0 : chunk;
         int nsub, per;
@@ -877,6 +887,7 @@ int letkf_analysis_batched_host(const double* Yb, const double* d, const double*
     if (!Xa) return -10;
     int rc = g_hpipe.init();
     if (rc) return rc;
+    HostSubChunks max_sub_guard;
     // as letkf_syev_batched_host: one pass on the device at a time, inputs copied in sub-chunk by
     // sub-chunk, outputs read back as each sub-chunk's last kernel finishes
     const int chunk = syev_chunk(M, batch);
@@ -968,6 +979,7 @@ int letkf_analysis_grid_host(const double* Yf, const double* yo, const unsigned 
     if (!Xa) return -15;
     int rc = g_hpipe.init();
     if (rc) return rc;
+    HostSubChunks max_sub_guard;
     // The observation fields (V Ny Nx (M+1) doubles: 17 MB at 128 x 128 x 2 x 64) go in first, whole;
     // the background ensemble follows sub-chunk by sub-chunk and the analysis ensemble comes back
     // the same way (hooks as in letkf_analysis_batched_host).
