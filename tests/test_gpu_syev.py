@@ -315,3 +315,35 @@ def test_split_tridiagonalisation_option(lk, oracle, M):
     assert (info == 0).all()
     wo, _, _, _ = oracle.syev_batched(A)
     parity.assert_evd(A, w, V, wo, f"split M={M}")
+
+
+@pytest.mark.parametrize("M", [16, 32, 96, 128, 192, 256])
+def test_config5_full_sizes(lk, oracle, M):
+    """BASELINE config 5 at the sizes bench.py's sweep times (batch = floor(2^26 / M^2)): residual,
+    orthogonality and ordering on EVERY matrix (evaluated on the GPU with torch fp64 batched
+    matmuls: properties that hold at any size), eigenvalues against the oracle on a strided sample.
+    M = 48 and 64 have their own full-size tests (configs 2 and 3)."""
+    import torch
+    B = (1 << 26) // (M * M)
+    A = wl.config5(M, batch=B)
+    At = torch.from_numpy(A).cuda()
+    w, V, info = lk.syev_batched(At)
+    torch.cuda.synchronize()
+    assert int(info.abs().max()) == 0
+    assert bool((w[:, 1:] >= w[:, :-1]).all())
+    L = torch.tril(At)
+    Af = L + torch.tril(At, -1).transpose(1, 2)
+    step = max(1, B // 16)
+    worst_res = worst_orth = 0.0
+    for b0 in range(0, B, step):
+        sl = slice(b0, min(B, b0 + step))
+        R = torch.matmul(Af[sl], V[sl]) - V[sl] * w[sl].unsqueeze(1)
+        worst_res = max(worst_res, float((R.flatten(1).norm(dim=1) / Af[sl].flatten(1).norm(dim=1)).max()))
+        G = torch.matmul(V[sl].transpose(1, 2), V[sl]) - torch.eye(M, dtype=torch.float64, device="cuda")
+        worst_orth = max(worst_orth, float(G.abs().max()))
+    assert worst_res <= parity.TOL_RES, f"residual {worst_res:.3e}"
+    assert worst_orth <= parity.TOL_ORTH, f"orthogonality {worst_orth:.3e}"
+    sel = np.unique(np.linspace(0, B - 1, 12 if M <= 128 else 4).astype(int))
+    wo, _, _, _ = oracle.syev_batched(A[sel])
+    wg = w[torch.from_numpy(sel).cuda()].cpu().numpy()
+    assert (np.abs(wg - wo).max(axis=1) / np.abs(wo).max(axis=1)).max() <= parity.TOL_W
