@@ -103,16 +103,21 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
             i = m - 1;
         }
         const int maxlen = __reduce_max_sync(FULL, sweeping ? m - l : 0);
-        // ---- lockstep rotation steps.  The kernel is bound by the dependent chain of one step
-        // (g -> r2 -> 1/sqrt -> c, s -> r -> g), so everything else is kept off it: the operands of
-        // step i-1 are loaded at the top of step i, pointers are bumped instead of recomputed, and
-        // 1/sqrt is the hardware seed plus two Newton steps whenever r2 is a normal number.
+        // ---- lockstep rotation steps.  The kernel is bound by the dependent chain of one step,
+        // g -> r2 = f^2 + g^2 -> 1/sqrt -> c -> g, and the SM issues in order, so whatever else a
+        // step computes must not stand between two links of that chain.  The step is therefore
+        // software-pipelined by hand: p, the new d, its store and the deflation test of step i+1
+        // are computed at the top of step i, in the shadow of the 1/sqrt of step i (they need
+        // nothing from it); r is formed as q/r with q = g tb + (d_i - gt) f known before 1/r is;
+        // the operands of step i-1 are loaded at the top of step i; 1/sqrt is the hardware seed
+        // plus two Newton steps, issued before the range test of the rare cases.
         bool broke = false;
         double2* outp = rot + pos;
         double* pd = d + (i > 0 ? i : 0) * stride;     // &d[i]
         double* pe = e + (i > 0 ? i : 0) * stride;     // &e[i]
         double ei = 0.0, di = 0.0, di1 = 0.0;
-        if (sweeping) { ei = pe[0]; di = pd[0]; di1 = pd[stride]; }
+        double rp = 0.0, gtp = 0.0, enp = 0.0;         // r, gt and new e of the step before (pending)
+        if (sweeping) { ei = pe[0]; di = pd[0]; di1 = pd[stride]; gtp = pd[2 * stride]; }
         for (int k = 0; k < maxlen; ++k) {
             if (i >= l) {                              // (i = -1 when not sweeping, l - 1 when done or broken)
                 const int nxt = (i > l) ? -stride : 0;
@@ -122,46 +127,65 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
                 const double tb = b2 + b2;
                 const double r2 = fma(f, f, g * g);
                 double rinv;
-                bool ok = true;
-                if (r2 > 1e-280 && r2 < 1e280) {       // the common case: seed + two Newton steps
-                    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(rinv) : "d"(r2));
+                asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(rinv) : "d"(r2));
+                // in the shadow: finish step i+1 (s is still its s) ...
+                // (at the first step of a sweep nothing is pending: rp = 0, gtp = the value at d[m+1]
+                // -- or, for m = M-1, at the word that follows the d array -- which is written back)
+                p = s * rp;
+                const double dnew = gtp + p;
+                pd[2 * stride] = dnew;
+                // ... its deflation test, on this sweep's values (d[i+3] = dprev) ...
+                const bool defl = i + 2 < m && fabs(enp) <= fmax(eps * (fabs(dnew) + fabs(dprev)), thr);
+                mlow = defl ? i + 2 : mlow;
+                dprev = dnew;
+                // ... and what this step can form without 1/r
+                const double gt = di1 - p;
+                const double q = fma(g, tb, (di - gt) * f);
+                {
                     const double hx = 0.5 * r2;
                     double t = fma(-hx * rinv, rinv, 0.5);
                     rinv = fma(rinv, t, rinv);
                     t = fma(-hx * rinv, rinv, 0.5);
                     rinv = fma(rinv, t, rinv);
-                } else if (r2 > 0.0) {
-                    rinv = rsqrt(r2);
-                } else {                               // underflow / NaN: split the block at i+1
-                    pe[stride] = 0.0;
-                    pd[stride] = di1 - p;
-                    QL_E(m) = 0.0;
-                    broke = true;
-                    ibreak = i;
-                    i = l - 1;
-                    ok = false;
-                    rinv = 0.0;
+                }
+                // (q != q belongs to the test only to make ptxas form q BEFORE the branch, beside
+                // the Newton steps, instead of sinking it into the tail behind 1/r; a NaN q with a
+                // normal r2 merely takes the library rsqrt and continues as it would have)
+                bool ok = true;
+                if (!(r2 > 1e-280 && r2 < 1e280) || q != q) {
+                    if (r2 > 0.0) {
+                        rinv = rsqrt(r2);
+                    } else {                           // underflow / NaN: split the block at i+1
+                        pe[stride] = 0.0;
+                        pd[stride] = gt;
+                        QL_E(m) = 0.0;
+                        broke = true;
+                        ibreak = i;
+                        i = l - 1;
+                        ok = false;
+                    }
                 }
                 if (ok) {
-                    const double enew = r2 * rinv;
                     s = f * rinv;
                     c = g * rinv;
-                    const double gt = di1 - p;
-                    const double r = fma(c, tb, (di - gt) * s);
-                    p = s * r;
-                    const double dnew = gt + p;
-                    g = fma(c, r, -b2);
-                    pe[stride] = enew;
-                    pd[stride] = dnew;
+                    rp = q * rinv;
+                    g = fma(c, rp, -b2);
+                    enp = r2 * rinv;
+                    gtp = gt;
+                    pe[stride] = enp;
                     *outp++ = make_double2(c, s);
-                    // deflation test of index i+1 on this sweep's values (d[i+2] = dprev)
-                    if (i + 1 < m && fabs(enew) <= fmax(eps * (fabs(dnew) + fabs(dprev)), thr)) mlow = i + 1;
-                    dprev = dnew;
                     di1 = di; di = din; ei = ein;
                     pd += nxt; pe += nxt;
                     --i;
                 }
             }
+        }
+        if (sweeping && !broke) {                      // the last step (i = l) is still pending
+            p = s * rp;
+            const double dnew = gtp + p;
+            QL_D(l + 1) = dnew;
+            if (l + 1 < m && fabs(enp) <= fmax(eps * (fabs(dnew) + fabs(dprev)), thr)) mlow = l + 1;
+            dprev = dnew;
         }
         if (sweeping) {
             int lo;
