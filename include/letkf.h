@@ -40,7 +40,8 @@ extern "C" {
 
 /* info[b] bit flags (0 = converged on the fast path) */
 #define LETKF_INFO_SLOWPATH 0x40000000 /* the matrix was finished by the in-kernel slow path
-                                          (rotation log full); result is still valid       */
+                                          (rotation log full, or a QL rotation with f^2 + g^2
+                                          outside [1e-280, 1e280]); result is still valid   */
 /* info[b] & 0xFFFF = number of off-diagonal elements that had not converged after 60
  * QL iterations each ("implicit QL method ... as in EISPACK/LAPACK"; twice the
  * cap of EISPACK tql2).  Non-zero means w/V of that matrix are not to be trusted.                */

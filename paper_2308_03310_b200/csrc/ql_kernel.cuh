@@ -92,7 +92,7 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
             break;
         }
         if (!__any_sync(FULL, sweeping)) break;
-        int i = -1, mlow = m, ibreak = 0;
+        int i = -1, mlow = m;
         double g = 0.0, s = 1.0, c = 1.0, p = 0.0, dprev = 0.0;
         if (sweeping) {
             // Wilkinson shift
@@ -105,21 +105,27 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
         const int maxlen = __reduce_max_sync(FULL, sweeping ? m - l : 0);
         // ---- lockstep rotation steps.  The kernel is bound by the dependent chain of one step,
         // g -> r2 = f^2 + g^2 -> 1/sqrt -> c -> g, and the SM issues in order, so whatever else a
-        // step computes must not stand between two links of that chain.  The step is therefore
-        // software-pipelined by hand: p, the new d, its store and the deflation test of step i+1
-        // are computed at the top of step i, in the shadow of the 1/sqrt of step i (they need
-        // nothing from it); r is formed as q/r with q = g tb + (d_i - gt) f known before 1/r is;
-        // the operands of step i-1 are loaded at the top of step i; 1/sqrt is the hardware seed
-        // plus two Newton steps, issued before the range test of the rare cases.
-        bool broke = false;
+        // step computes must not stand between two links of that chain, and the step must be ONE
+        // basic block for ptxas to interleave the rest with it.  Hence:
+        //  * the step is software-pipelined by hand: p, the new d, its store and the deflation test
+        //    of step i+1 are computed at the top of step i, in the shadow of the 1/sqrt of step i;
+        //  * r is formed as q/r with q = g tb + (d_i - gt) f, known before 1/r is;
+        //  * the operands of step i-1 are loaded at the top of step i;
+        //  * 1/sqrt is the hardware seed (2^-20) and one third-order step (measured 49 cycles
+        //    against 63 for two Newton steps, same 2.7e-16 error);
+        //  * no branch for the rare cases: an r2 outside [1e-280, 1e280] (underflow to the block
+        //    split of the classic algorithm, overflow, NaN) only sets a flag; the sweep runs on
+        //    garbage in the lane's own shared memory, and the matrix is handed to the slow path
+        //    (flags[b], like a log overflow), whose step treats those cases one by one.
         double2* outp = rot + pos;
         double* pd = d + (i > 0 ? i : 0) * stride;     // &d[i]
         double* pe = e + (i > 0 ? i : 0) * stride;     // &e[i]
         double ei = 0.0, di = 0.0, di1 = 0.0;
         double rp = 0.0, gtp = 0.0, enp = 0.0;         // r, gt and new e of the step before (pending)
+        bool bad = false;
         if (sweeping) { ei = pe[0]; di = pd[0]; di1 = pd[stride]; gtp = pd[2 * stride]; }
         for (int k = 0; k < maxlen; ++k) {
-            if (i >= l) {                              // (i = -1 when not sweeping, l - 1 when done or broken)
+            if (i >= l) {                              // (i = -1 when not sweeping, l - 1 when done)
                 const int nxt = (i > l) ? -stride : 0;
                 const double ein = pe[nxt], din = pd[nxt];
                 const double f = s * ei;
@@ -128,73 +134,55 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
                 const double r2 = fma(f, f, g * g);
                 double rinv;
                 asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(rinv) : "d"(r2));
+                // exponent of r2 in [2^-930, 2^930), on the integer pipe
+                bad |= ((unsigned)__double2hiint(r2) - 0x05d00000u) >= 0x74400000u;
                 // in the shadow: finish step i+1 (s is still its s) ...
                 // (at the first step of a sweep nothing is pending: rp = 0, gtp = the value at d[m+1]
                 // -- or, for m = M-1, at the word that follows the d array -- which is written back)
                 p = s * rp;
                 const double dnew = gtp + p;
                 pd[2 * stride] = dnew;
-                // ... its deflation test, on this sweep's values (d[i+3] = dprev) ...
-                const bool defl = i + 2 < m && fabs(enp) <= fmax(eps * (fabs(dnew) + fabs(dprev)), thr);
+                // ... its deflation test, on this sweep's values (d[i+3] = dprev):
+                // |e| <= max(eps (|d| + |d'|), thr)  <=>  2^53 |e| <= |d| + |d'|  or  |e| <= thr
+                const double es = __hiloint2double(__double2hiint(enp) + (53 << 20), __double2loint(enp));
+                const bool defl = (i + 2 < m) & ((fabs(es) <= fabs(dnew) + fabs(dprev)) | (fabs(enp) <= thr));   // no short circuit: no branch
                 mlow = defl ? i + 2 : mlow;
                 dprev = dnew;
                 // ... and what this step can form without 1/r
                 const double gt = di1 - p;
                 const double q = fma(g, tb, (di - gt) * f);
                 {
-                    const double hx = 0.5 * r2;
-                    double t = fma(-hx * rinv, rinv, 0.5);
-                    rinv = fma(rinv, t, rinv);
-                    t = fma(-hx * rinv, rinv, 0.5);
-                    rinv = fma(rinv, t, rinv);
+                    // (one = 1 + 0 q ties q to the MIDDLE of the 1/sqrt chain: ptxas otherwise sinks
+                    // the five operations of q behind 1/r, where they add 16 cycles to the chain;
+                    // 0 q is not folded because q may be NaN -- when it is, so is the result)
+                    const double one = fma(q, 0.0, 1.0);
+                    const double t = fma(-(0.5 * r2) * rinv, rinv, 0.5);
+                    const double u = fma(1.5, t, one);
+                    rinv = fma(rinv * t, u, rinv);
                 }
-                // (q != q belongs to the test only to make ptxas form q BEFORE the branch, beside
-                // the Newton steps, instead of sinking it into the tail behind 1/r; a NaN q with a
-                // normal r2 merely takes the library rsqrt and continues as it would have)
-                bool ok = true;
-                if (!(r2 > 1e-280 && r2 < 1e280) || q != q) {
-                    if (r2 > 0.0) {
-                        rinv = rsqrt(r2);
-                    } else {                           // underflow / NaN: split the block at i+1
-                        pe[stride] = 0.0;
-                        pd[stride] = gt;
-                        QL_E(m) = 0.0;
-                        broke = true;
-                        ibreak = i;
-                        i = l - 1;
-                        ok = false;
-                    }
-                }
-                if (ok) {
-                    s = f * rinv;
-                    c = g * rinv;
-                    rp = q * rinv;
-                    g = fma(c, rp, -b2);
-                    enp = r2 * rinv;
-                    gtp = gt;
-                    pe[stride] = enp;
-                    *outp++ = make_double2(c, s);
-                    di1 = di; di = din; ei = ein;
-                    pd += nxt; pe += nxt;
-                    --i;
-                }
+                s = f * rinv;
+                c = g * rinv;
+                rp = q * rinv;
+                g = fma(c, rp, -b2);
+                enp = r2 * rinv;
+                gtp = gt;
+                pe[stride] = enp;
+                *outp++ = make_double2(c, s);
+                di1 = di; di = din; ei = ein;
+                pd += nxt; pe += nxt;
+                --i;
             }
         }
-        if (sweeping && !broke) {                      // the last step (i = l) is still pending
-            p = s * rp;
-            const double dnew = gtp + p;
-            QL_D(l + 1) = dnew;
-            if (l + 1 < m && fabs(enp) <= fmax(eps * (fabs(dnew) + fabs(dprev)), thr)) mlow = l + 1;
-            dprev = dnew;
-        }
         if (sweeping) {
-            int lo;
-            if (broke) {
-                lo = ibreak + 1;
-                // the block was split by hand: what is left of it below i+1 is rescanned
-                if (m - lo > 0) { hdr[nsw++] = (uint32_t)lo | ((uint32_t)m << 16); pos += m - lo; }
-                m = scan_end(l);
+            if (bad) {                                 // left to the slow path
+                overflow = 1; done = true;
             } else {
+                // the last step (i = l) is still pending
+                p = s * rp;
+                const double dnew = gtp + p;
+                QL_D(l + 1) = dnew;
+                if (l + 1 < m && fabs(enp) <= fmax(eps * (fabs(dnew) + fabs(dprev)), thr)) mlow = l + 1;
+                dprev = dnew;
                 const double dl = QL_D(l) - p;
                 QL_D(l) = dl;
                 QL_E(l) = g;

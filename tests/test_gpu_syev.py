@@ -166,6 +166,22 @@ def test_nan_input_terminates(lk):
     parity.assert_evd(A[good], w[good], V[good], None, "neighbours of a NaN matrix")
 
 
+@pytest.mark.parametrize("scale", [1e-138, 1e138])
+def test_extreme_scale_takes_the_slow_path(lk, oracle, scale):
+    """Matrices scaled so that r2 = f^2 + g^2 of the QL rotation step leaves [1e-280, 1e280]: the
+    branch-free fast step only flags them (ql_kernel.cuh) and the slow path, whose step handles the
+    rare cases one by one, must redo them -- same tolerances, neighbours untouched.  (Outside the
+    documented range 1e-100 < ||A|| < 1e100, but nowhere near under/overflow of the result.)"""
+    A = wl.letkf_shaped(96, 64, 98, config_index=39)
+    A[1::3] *= scale
+    w, V, info = run_gpu(lk, A)
+    assert ((info & 0xFFFF) == 0).all()
+    slow = (info & lk.INFO_SLOWPATH).astype(bool)
+    assert slow[1::3].all() and not slow[0::3].any() and not slow[2::3].any()
+    wo, _, _, _ = oracle.syev_batched(A)
+    parity.assert_evd(A, w, V, wo, f"scale {scale:g}")
+
+
 def test_headline_full_size(lk, oracle):
     """BASELINE config 3 at full size (M=64, batch=16384, the launch configuration bench.py times):
     residual/orthogonality/ordering on every matrix, oracle parity on a strided sample."""
