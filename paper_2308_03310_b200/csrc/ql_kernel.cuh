@@ -124,8 +124,8 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
         double rp = 0.0, gtp = 0.0, enp = 0.0;         // r, gt and new e of the step before (pending)
         bool bad = false;
         if (sweeping) { ei = pe[0]; di = pd[0]; di1 = pd[stride]; gtp = pd[2 * stride]; }
-        for (int k = 0; k < maxlen; ++k) {
-            if (i >= l) {                              // (i = -1 when not sweeping, l - 1 when done)
+        auto step = [&]() {
+            {
                 const int nxt = (i > l) ? -stride : 0;
                 const double ein = pe[nxt], din = pd[nxt];
                 const double f = s * ei;
@@ -141,7 +141,7 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
                 // -- or, for m = M-1, at the word that follows the d array -- which is written back)
                 p = s * rp;
                 const double dnew = gtp + p;
-                pd[2 * stride] = dnew;
+                if (sweeping) pd[2 * stride] = dnew;
                 // ... its deflation test, on this sweep's values (d[i+3] = dprev):
                 // |e| <= max(eps (|d| + |d'|), thr)  <=>  2^53 |e| <= |d| + |d'|  or  |e| <= thr
                 const double es = __hiloint2double(__double2hiint(enp) + (53 << 20), __double2loint(enp));
@@ -166,13 +166,22 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
                 g = fma(c, rp, -b2);
                 enp = r2 * rinv;
                 gtp = gt;
-                pe[stride] = enp;
-                *outp++ = make_double2(c, s);
+                if (sweeping) { pe[stride] = enp; *outp = make_double2(c, s); }
+                ++outp;
                 di1 = di; di = din; ei = ein;
                 pd += nxt; pe += nxt;
                 --i;
             }
-        }
+        };
+        // the first minlen steps are taken by every sweeping lane: no per-lane guard, hence no
+        // divergence construct around the step (BSSY / BRA / BSYNC and the latency of the
+        // reconvergence cost ~40 of a step's ~200 cycles); lanes that are not sweeping ride along on
+        // their own column with their stores predicated off.  Only the ragged rest is guarded.
+        const int minlen = __reduce_min_sync(FULL, sweeping ? m - l : 0x7fffffff);
+        int k = 0;
+        for (; k < minlen && k < maxlen; ++k) step();
+        for (; k < maxlen; ++k)
+            if (i >= l) step();                        // (i = l - 1 when the lane's sweep is done)
         if (sweeping) {
             if (bad) {                                 // left to the slow path
                 overflow = 1; done = true;
