@@ -210,7 +210,9 @@ int letkf_last_launch_count(void);
  * "ql_tpb" = 32/64/96 matrices per QL CTA (0 = by size); "log_shrink" = k divides the rotation-log
  * capacity by k so that tests can force the log-overflow slow path (default 1); "split" = 1 runs the
  * tridiagonalisation of 48 < M <= 64 as three kernels (pivots down to 33 / trailing 32 x 32 problem /
- * explicit Q; experimental, default 0: measured slower than the single kernel).  Returns 0, or -1 for an unknown name. */
+ * explicit Q; experimental, default 0: measured slower than the single kernel); "sub_chunks" = 1..16
+ * sub-chunks per pass of the calling thread's device calls (default 8; measured flat from 4 to 8).
+ * Returns 0, or -1 for an unknown name. */
 int letkf_set_option(const char* name, int value);
 
 const char* letkf_status_string(int status);

@@ -1065,6 +1065,7 @@ int letkf_set_option(const char* name, int value)
     if (!name) return -1;
     if (strcmp(name, "force_generic") == 0) { g_force_generic = value != 0; return LETKF_OK; }
     if (strcmp(name, "pipeline") == 0) { g_pipeline = value != 0; return LETKF_OK; }
+    if (strcmp(name, "sub_chunks") == 0) { g_max_sub = (value >= 1 && value <= PIPE_MAX_SUB) ? value : 8; return LETKF_OK; }
     if (strcmp(name, "split") == 0) { g_split = value != 0; return LETKF_OK; }
     if (strcmp(name, "log_shrink") == 0) { g_log_shrink = value >= 1 ? value : 1; return LETKF_OK; }
     if (strcmp(name, "ql_tpb") == 0) { g_ql_tpb = (value == 32 || value == 64 || value == 96) ? value : 0; return LETKF_OK; }
