@@ -28,9 +28,9 @@ if ROOT not in sys.path:
 METRIC = "batched fp64 syev matrices/s at M=64 (batch 16384); % of FP64/HBM roofline"
 M_HEAD, BATCH_HEAD, P_HEAD = 64, 16384, 98
 # dram__bytes_read.sum + dram__bytes_write.sum per whole-batch launch (config 3) from the ncu --set full
-# capture kept in profiles/r01d_ncu_key_metrics.txt (bytes; ncu runs are never timed)
-NCU_DRAM_BYTES = {"fast_tridiag_formq": 0.536987e9 + 0.503768e9, "ql_log_kernel": 0.027283e9 + 1.097704e9,
-                  "fast_apply": 1.681378e9 + 0.503778e9}
+# capture kept in profiles/r01e_ncu_key_metrics.txt (bytes; ncu runs are never timed)
+NCU_DRAM_BYTES = {"fast_tridiag_formq": 0.537097e9 + 0.503998e9, "ql_log_kernel": 0.030428e9 + 1.099897e9,
+                  "fast_apply": 1.681331e9 + 0.501880e9}
 SM_COUNT = 148
 DFMA_PER_CLK_SM = 64          # fp64 FMA lanes per SM (4 SMSPs x 16), DESIGN.md section 6
 
@@ -353,7 +353,7 @@ def run_ours(args):
     roofline = {
         "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
         "frac": achieved / peak_tflops, "traffic": NCU_DRAM_BYTES.get(dom),
-        "traffic_unit": "bytes per launch (whole batch), ncu dram read+write, profiles/r01d_ncu_key_metrics.txt",
+        "traffic_unit": "bytes per launch (whole batch), ncu dram read+write, profiles/r01e_ncu_key_metrics.txt",
         "algorithmic_bytes": {"fast_tridiag_formq": 16.0 * M * M * B, "ql_log_kernel": 16.0 * rot_per_matrix * B,
                               "fast_apply": (16.0 * M * M + 16.0 * rot_per_matrix) * B}.get(dom),
         "peak_source": f"derived: {SM_COUNT} SMs x {DFMA_PER_CLK_SM} DFMA/clk x 2 x {sm_max:.0f} MHz (DESIGN.md 6)",
