@@ -286,9 +286,10 @@ static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws,
     }
     if (mid_supported(M) && !g_force_generic) {
         cudaError_t ce;
-        const size_t smem = mid_apply_smem(M, ws.swcap);
+        const int ms = mid_apply_round(M, ws.swcap);
+        const size_t smem = mid_apply_smem(M, ws.swcap, ms);
         if ((ce = allow_smem(mid_apply, smem)) != cudaSuccess) return (int)ce;
-        KLAUNCH("mid_apply", st, mid_apply<<<n, mid_threads(M), smem, st>>>(V, ws, M));
+        KLAUNCH("mid_apply", st, mid_apply<<<n, mid_threads(M), smem, st>>>(V, ws, M, ms));
         KLAUNCH("generic_apply(flagged)", st,
                 generic_apply<<<(n < 296 ? n : 296), GEN_NT, ap_smem, st>>>(V, w, ws, M, n, info, /*only_flagged=*/1, /*q_rowmajor=*/0));
         return 0;

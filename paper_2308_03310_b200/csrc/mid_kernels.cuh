@@ -28,9 +28,16 @@ static inline size_t mid_tridiag_smem(int M)
 {
     return sizeof(double) * ((size_t)M * mid_ld(M) + 3 * ((size_t)mid_ld(M)) + (size_t)MID_TPR * mid_threads(M) + 64 + 8);
 }
-static inline size_t mid_apply_smem(int M, int swcap)
+static inline size_t mid_apply_smem(int M, int swcap, int ms)
 {
-    return sizeof(double) * ((size_t)M * (M + 1) + 4 * (size_t)M) + sizeof(uint32_t) * (size_t)swcap + sizeof(int) * (size_t)M + 32;
+    return sizeof(double) * ((size_t)M * (M + 1) + 4 * (size_t)ms * (size_t)M) + sizeof(uint32_t) * (size_t)swcap + sizeof(int) * (size_t)M + 32;
+}
+// sweeps staged per barrier round of mid_apply: as many (<= 4) as shared memory holds beside the matrix
+static inline int mid_apply_round(int M, int swcap)
+{
+    int ms = 4;
+    while (ms > 1 && mid_apply_smem(M, swcap, ms) > 226 * 1024) ms >>= 1;
+    return ms;
 }
 
 // Block-wide sum for a run-time number of warps (<= 20); ONE barrier: consecutive calls alternate
@@ -196,14 +203,17 @@ mid_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, int M
 }
 
 // a5: thread r owns column r of Q^T (= row r of Q); a rotation (i, i+1) mixes rows i, i+1 of Q^T.
+// The (c, s) of `ms` sweeps are staged per barrier round, double-buffered, straight from the log
+// into shared memory with cp.async (no registers: a thread never waits for the log before it
+// rotates); inside a round the threads do not depend on each other (each rotates its own column).
 __global__ void __launch_bounds__(160)
-mid_apply(double* __restrict__ V_, Workspace ws, int M)
+mid_apply(double* __restrict__ V_, Workspace ws, int M, int ms)
 {
     extern __shared__ __align__(16) double sm[];
     const int LD = M + 1;
     double*   S    = sm;                                                   // [M][LD]  Q^T
-    double2*  cs   = reinterpret_cast<double2*>(sm + (((size_t)M * LD + 1) & ~(size_t)1));   // [2][M]
-    uint32_t* hdr  = reinterpret_cast<uint32_t*>(cs + 2 * M);
+    double2*  cs   = reinterpret_cast<double2*>(sm + (((size_t)M * LD + 1) & ~(size_t)1));   // [2][ms][M]
+    uint32_t* hdr  = reinterpret_cast<uint32_t*>(cs + 2 * ms * M);
     int*      perm = reinterpret_cast<int*>(hdr + ws.swcap);
     const int r = threadIdx.x, nt = blockDim.x;
     const size_t b = blockIdx.x;
@@ -212,52 +222,56 @@ mid_apply(double* __restrict__ V_, Workspace ws, int M)
     const int nsw = ws.nsweeps[b];
     const double2* rot = ws.rot + b * ws.logcap;
 
+    for (int s = r; s < nsw; s += nt) hdr[s] = ws.hdr[b * ws.swcap + s];
     if (r < M) {
         for (int k = 0; k < M; ++k) S[k * LD + r] = V[(size_t)k * M + r];
         perm[r] = ws.perm[b * M + r];
     }
-    for (int s = r; s < nsw; s += nt) hdr[s] = ws.hdr[b * ws.swcap + s];
     __syncthreads();
 
-    // sweeps, (c, s) double-buffered in shared memory: one barrier per sweep
-    int pos = 0;
-    if (nsw > 0) {
-        const uint32_t h = hdr[0];
-        const int lo = h & 0xffff, m = h >> 16;
-        for (int k = r; k < m - lo; k += nt) cs[k] = rot[k];
-    }
+    // stage the sweeps [s0, s0 + ms) of the log, which start at log position p0; returns the
+    // position after them
+    auto stage = [&](int s0, int p0, double2* buf) {
+        for (int t = 0; t < ms && s0 + t < nsw; ++t) {
+            const uint32_t h = hdr[s0 + t];
+            const int n = (int)(h >> 16) - (int)(h & 0xffff);
+            for (int k = r; k < n; k += nt) cp_async16(buf + t * M + k, rot + p0 + k);
+            p0 += n;
+        }
+        return p0;
+    };
+    int pos = stage(0, 0, cs);
+    cp_async_wait_all();
     __syncthreads();
-    for (int s = 0; s < nsw; ++s) {
-        const uint32_t h = hdr[s];
-        const int lo = h & 0xffff, m = h >> 16;
-        pos += m - lo;
-        if (s + 1 < nsw) {
-            const uint32_t h2 = hdr[s + 1];
-            const int n2 = (int)(h2 >> 16) - (int)(h2 & 0xffff);
-            double2* nxt = cs + ((s + 1) & 1) * M;
-            for (int k = r; k < n2; k += nt) nxt[k] = rot[pos + k];
-        }
+    for (int s0 = 0; s0 < nsw; s0 += ms) {
+        const double2* cur0 = cs + ((s0 / ms) & 1) * ms * M;
+        pos = stage(s0 + ms, pos, cs + (((s0 / ms) + 1) & 1) * ms * M);
         if (r < M) {
-            const double2* cur = cs + (s & 1) * M;
             double* col = S + r;
-            double f = col[m * LD];
-            int i = m - 1;
-            for (; i - 3 >= lo; i -= 4) {
-                const double2 q0 = cur[m - 1 - i], q1 = cur[m - i], q2 = cur[m + 1 - i], q3 = cur[m + 2 - i];
-                const double z0 = col[i * LD], z1 = col[(i - 1) * LD], z2 = col[(i - 2) * LD], z3 = col[(i - 3) * LD];
-                col[(i + 1) * LD] = fma(q0.y, z0, q0.x * f);  f = fma(-q0.y, f, q0.x * z0);
-                col[i * LD]       = fma(q1.y, z1, q1.x * f);  f = fma(-q1.y, f, q1.x * z1);
-                col[(i - 1) * LD] = fma(q2.y, z2, q2.x * f);  f = fma(-q2.y, f, q2.x * z2);
-                col[(i - 2) * LD] = fma(q3.y, z3, q3.x * f);  f = fma(-q3.y, f, q3.x * z3);
+            for (int t = 0; t < ms && s0 + t < nsw; ++t) {
+                const uint32_t h = hdr[s0 + t];
+                const int lo = h & 0xffff, m = h >> 16;
+                const double2* cur = cur0 + t * M;
+                double f = col[m * LD];
+                int i = m - 1;
+                for (; i - 3 >= lo; i -= 4) {
+                    const double2 q0 = cur[m - 1 - i], q1 = cur[m - i], q2 = cur[m + 1 - i], q3 = cur[m + 2 - i];
+                    const double z0 = col[i * LD], z1 = col[(i - 1) * LD], z2 = col[(i - 2) * LD], z3 = col[(i - 3) * LD];
+                    col[(i + 1) * LD] = fma(q0.y, z0, q0.x * f);  f = fma(-q0.y, f, q0.x * z0);
+                    col[i * LD]       = fma(q1.y, z1, q1.x * f);  f = fma(-q1.y, f, q1.x * z1);
+                    col[(i - 1) * LD] = fma(q2.y, z2, q2.x * f);  f = fma(-q2.y, f, q2.x * z2);
+                    col[(i - 2) * LD] = fma(q3.y, z3, q3.x * f);  f = fma(-q3.y, f, q3.x * z3);
+                }
+                for (; i >= lo; --i) {
+                    const double2 q = cur[m - 1 - i];
+                    const double zi = col[i * LD];
+                    col[(i + 1) * LD] = fma(q.y, zi, q.x * f);
+                    f = fma(-q.y, f, q.x * zi);
+                }
+                col[lo * LD] = f;
             }
-            for (; i >= lo; --i) {
-                const double2 q = cur[m - 1 - i];
-                const double zi = col[i * LD];
-                col[(i + 1) * LD] = fma(q.y, zi, q.x * f);
-                f = fma(-q.y, f, q.x * zi);
-            }
-            col[lo * LD] = f;
         }
+        cp_async_wait_all();
         __syncthreads();
     }
 
