@@ -14,6 +14,7 @@
 namespace letkf {
 
 constexpr int GEN_NT = 256;
+constexpr int GEN_QK = 4;      // reflectors applied per pass over the rows when Q is formed
 
 // ---------------------------------------------------------------------------------------------
 // a3 + explicit Q.  Reduction order is "from the last row up" (pivot i = M-1 ... 1, reflector
@@ -85,24 +86,46 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
     }
     if (tid == 0) { dws[0] = S[0]; ews[M - 1] = 0.0; }
 
-    // Q^T = H_1 H_2 ... H_{M-1}, grown in place: B_i = diag(B_{i-1}, 1) H_i on the leading i x i
-    for (int i = 1; i <= M - 1; ++i) {
-        for (int c = tid; c < i; c += GEN_NT) v[c] = S[(size_t)i * M + c];
-        const double tau = taus[i];
-        for (int c = tid; c < i - 1; c += GEN_NT) {
-            S[(size_t)(i - 1) * M + c] = 0.0;
-            S[(size_t)c * M + (i - 1)] = 0.0;
-        }
-        if (tid == 0) S[(size_t)(i - 1) * M + (i - 1)] = 1.0;
-        __syncthreads();
-        if (tau != 0.0) {
-            for (int r = warp; r < i; r += NW) {
-                double* br = S + (size_t)r * M;
-                double acc = 0.0;
-                for (int c = lane; c < i; c += 32) acc += br[c] * v[c];
-                acc = warp_sum(acc) * tau;
-                for (int c = lane; c < i; c += 32) br[c] -= acc * v[c];
+    // Q^T = H_1 H_2 ... H_{M-1}, grown in place: B_i = diag(B_{i-1}, 1) H_i on the leading i x i.
+    // The kernel runs at the HBM roof for M > 160 (the resident matrices exceed L2), so GEN_QK
+    // reflectors are applied per pass over the rows: a row is read and written once per GEN_QK
+    // steps, held in registers in between (<= 8 doubles per lane).  The rows and columns the later
+    // reflectors of a group add are set to identity first and every reflector is zero-padded to the
+    // group's width, so H_i leaves the rows >= i alone exactly as the one-at-a-time loop does.
+    double* vk = red + NW;        // [GEN_QK][M]
+    for (int i0 = 1; i0 <= M - 1; i0 += GEN_QK) {
+        const int kk = min(GEN_QK, M - i0);          // reflectors i0 ... i0+kk-1
+        const int nc = i0 + kk - 1;                  // rows and columns of the pass
+        for (int t = 0; t < kk; ++t)
+            for (int c = tid; c < nc; c += GEN_NT) vk[t * M + c] = (c < i0 + t) ? S[(size_t)(i0 + t) * M + c] : 0.0;
+        __syncthreads();                             // the reflectors are copied before their rows are cleared
+        for (int t = 0; t < kk; ++t) {
+            const int idx = i0 + t - 1;
+            for (int c = tid; c < idx; c += GEN_NT) {
+                S[(size_t)idx * M + c] = 0.0;
+                S[(size_t)c * M + idx] = 0.0;
             }
+            if (tid == 0) S[(size_t)idx * M + idx] = 1.0;
+        }
+        __syncthreads();
+        for (int r = warp; r < nc; r += NW) {
+            double* br = S + (size_t)r * M;
+            double x[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) { const int c = lane + 32 * k; x[k] = (c < nc) ? br[c] : 0.0; }
+            for (int t = 0; t < kk; ++t) {
+                const double tau = taus[i0 + t];
+                if (tau == 0.0) continue;
+                const double* vt = vk + t * M;
+                double acc = 0.0;
+#pragma unroll
+                for (int k = 0; k < 8; ++k) { const int c = lane + 32 * k; if (c < nc) acc += x[k] * vt[c]; }
+                acc = warp_sum(acc) * tau;
+#pragma unroll
+                for (int k = 0; k < 8; ++k) { const int c = lane + 32 * k; if (c < nc) x[k] -= acc * vt[c]; }
+            }
+#pragma unroll
+            for (int k = 0; k < 8; ++k) { const int c = lane + 32 * k; if (c < nc) br[c] = x[k]; }
         }
         __syncthreads();
     }

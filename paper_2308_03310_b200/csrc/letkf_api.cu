@@ -237,7 +237,7 @@ static int stage_T(const double* A, int M, int n, double* V, Workspace ws, cudaS
         KLAUNCH("mid_tridiag_formq", st, mid_tridiag_formq<<<n, MID_TPR * mid_threads(M), smem, st>>>(A, V, ws, M));
         return 0;
     }
-    const size_t td_smem = sizeof(double) * (4 * (size_t)M + GEN_NT / 32);
+    const size_t td_smem = sizeof(double) * ((4 + GEN_QK) * (size_t)M + GEN_NT / 32);
     KLAUNCH("generic_tridiag_formq", st, generic_tridiag_formq<<<n, GEN_NT, td_smem, st>>>(A, V, ws, M));
     return 0;
 }
