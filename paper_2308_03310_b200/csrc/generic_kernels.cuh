@@ -14,7 +14,7 @@
 namespace letkf {
 
 constexpr int GEN_NT = 256;
-constexpr int GEN_QK = 4;      // reflectors applied per pass over the rows when Q is formed
+constexpr int GEN_QK = 8;      // reflectors applied per pass over the rows when Q is formed
 
 // ---------------------------------------------------------------------------------------------
 // a3 + explicit Q.  Reduction order is "from the last row up" (pivot i = M-1 ... 1, reflector
@@ -45,8 +45,21 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
         }
     __syncthreads();
 
+    // Pivots i = M-1 ... 1.  The rank-2 update of pivot i+1 and the mat-vec of pivot i share ONE
+    // pass over the rows (the kernel is at the HBM roof for M > 160: a row is read and written once
+    // per pivot instead of read twice and written once): row i is updated first, pivot i's reflector
+    // is formed from it, then every row j < i is updated in registers and dotted with the new v.
+    double* vbuf[2] = {v, red + NW};                 // v of the pending and of the new pivot (vk is free here)
+    double tauP = 0.0;                               // tau of the pending update (0: none)
     for (int i = M - 1; i >= 1; --i) {
         double* rowi = S + (size_t)i * M;
+        const double* vP = vbuf[(i + 1) & 1];        // v, w of pivot i+1 (length i+1)
+        double* vN = vbuf[i & 1];
+        if (tauP != 0.0) {                           // row i: S[i][c] -= v_i w_c + w_i v_c, c <= i
+            const double vi = vP[i], wi = wv[i];
+            for (int c = tid; c <= i; c += GEN_NT) rowi[c] -= vi * wv[c] + wi * vP[c];
+            __syncthreads();
+        }
         double part = 0.0;
         for (int c = tid; c < i - 1; c += GEN_NT) { const double x = rowi[c]; part += x * x; }
         const double sigma = block_sum<GEN_NT>(part, red);
@@ -58,32 +71,45 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
             tau = (beta - alpha) / beta;
             scal = 1.0 / (alpha - beta);
         }
-        for (int c = tid; c < i; c += GEN_NT) v[c] = (c == i - 1) ? 1.0 : rowi[c] * scal;
+        for (int c = tid; c < i; c += GEN_NT) vN[c] = (c == i - 1) ? 1.0 : rowi[c] * scal;
         if (tid == 0) { ews[i - 1] = beta; dws[i] = rowi[i]; taus[i] = tau; }
         __syncthreads();
-        for (int c = tid; c < i; c += GEN_NT) rowi[c] = v[c];            // keep the reflector
-        if (tau != 0.0) {
-            for (int j = warp; j < i; j += NW) {                          // p = tau * S11 v
-                const double* rj = S + (size_t)j * M;
-                double acc = 0.0;
-                for (int c = lane; c < i; c += 32) acc += rj[c] * v[c];
-                acc = warp_sum(acc);
-                if (lane == 0) pv[j] = tau * acc;
-            }
-            __syncthreads();
-            part = 0.0;
-            for (int c = tid; c < i; c += GEN_NT) part += pv[c] * v[c];
-            const double K = 0.5 * tau * block_sum<GEN_NT>(part, red);
-            for (int c = tid; c < i; c += GEN_NT) wv[c] = pv[c] - K * v[c];
-            __syncthreads();
-            for (int j = warp; j < i; j += NW) {                          // S11 -= v w^T + w v^T
+        for (int c = tid; c < i; c += GEN_NT) rowi[c] = vN[c];           // keep the reflector
+        if (tauP != 0.0 || tau != 0.0) {
+            for (int j = warp; j < i; j += NW) {
                 double* rj = S + (size_t)j * M;
-                const double vj = v[j], wj = wv[j];
-                for (int c = lane; c < i; c += 32) rj[c] -= vj * wv[c] + wj * v[c];
+                double x[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) { const int c = lane + 32 * k; x[k] = (c < i) ? rj[c] : 0.0; }
+                if (tauP != 0.0) {                                        // S11 -= v w^T + w v^T (pivot i+1)
+                    const double vj = vP[j], wj = wv[j];
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) {
+                        const int c = lane + 32 * k;
+                        if (c < i) { x[k] -= vj * wv[c] + wj * vP[c]; rj[c] = x[k]; }
+                    }
+                }
+                if (tau != 0.0) {                                         // p = tau * S11 v (pivot i)
+                    double acc = 0.0;
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) { const int c = lane + 32 * k; if (c < i) acc += x[k] * vN[c]; }
+                    acc = warp_sum(acc);
+                    if (lane == 0) pv[j] = tau * acc;
+                }
             }
         }
         __syncthreads();
+        if (tau != 0.0) {
+            part = 0.0;
+            for (int c = tid; c < i; c += GEN_NT) part += pv[c] * vN[c];
+            const double K = 0.5 * tau * block_sum<GEN_NT>(part, red);
+            for (int c = tid; c < i; c += GEN_NT) wv[c] = pv[c] - K * vN[c];
+        }
+        tauP = tau;
+        __syncthreads();
     }
+    if (tauP != 0.0 && tid == 0) S[0] -= 2.0 * vbuf[1][0] * wv[0];       // pending update of pivot 1 (tau_1 = 0 in fact)
+    __syncthreads();
     if (tid == 0) { dws[0] = S[0]; ews[M - 1] = 0.0; }
 
     // Q^T = H_1 H_2 ... H_{M-1}, grown in place: B_i = diag(B_{i-1}, 1) H_i on the leading i x i.
