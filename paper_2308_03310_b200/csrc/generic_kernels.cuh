@@ -204,19 +204,78 @@ generic_apply_one(double* V_, double* __restrict__ w_, const Workspace& ws, int 
         const int nsw = ws.nsweeps[b];
         const uint32_t* hdr = ws.hdr + b * ws.swcap;
         const double2* rot = ws.rot + b * ws.logcap;
+        // The replay streams B from global memory (for M > 160 the resident matrices exceed L2 and
+        // the loop runs at the HBM roof), so two consecutive sweeps share ONE pass over the column
+        // whenever the second lies inside the first (lo2 >= lo, m2 <= m: the usual case, blocks only
+        // shrink): rotation (2, j) on columns (j, j+1) may run as soon as (1, j-1) is done -- the value
+        // (1, i) leaves in column i+1 is final for sweep 1 and goes straight into (2, i+1), whose
+        // carry f2 is column i+2.  One load and one store per element instead of two.
         for (int r = tid; r < M; r += GEN_NT) {
+            double* col = B + r;
             int pos = 0;
-            for (int sidx = 0; sidx < nsw; ++sidx) {
+            for (int sidx = 0; sidx < nsw;) {
                 const uint32_t h = hdr[sidx];
                 const int lo = h & 0xffff, m = h >> 16;
-                double f = B[(size_t)m * M + r];
+                const double2* cur = rot + pos;
+                if (sidx + 1 < nsw) {
+                    const uint32_t h2 = hdr[sidx + 1];
+                    const int lo2 = h2 & 0xffff, m2 = h2 >> 16;
+                    if (lo2 >= lo && m2 <= m) {
+                        const double2* cur2 = cur + (m - lo);
+                        double f1 = col[(size_t)m * M];
+                        int i = m - 1;
+                        for (; i >= m2; --i) {                       // above sweep 2: sweep 1 alone
+                            const double2 q = cur[m - 1 - i];
+                            const double z = col[(size_t)i * M];
+                            col[(size_t)(i + 1) * M] = q.y * z + q.x * f1;
+                            f1 = q.x * z - q.y * f1;
+                        }
+                        double f2;
+                        {                                            // i = m2 - 1: column m2 becomes f2
+                            const double2 q = cur[m - 1 - i];
+                            const double z = col[(size_t)i * M];
+                            f2 = q.y * z + q.x * f1;
+                            f1 = q.x * z - q.y * f1;
+                            --i;
+                        }
+                        const int iend = max(lo2 - 1, lo);
+                        for (; i >= iend; --i) {                     // (1, i) then (2, i + 1)
+                            const double2 q1 = cur[m - 1 - i], q2 = cur2[m2 - 2 - i];
+                            const double z = col[(size_t)i * M];
+                            const double o1 = q1.y * z + q1.x * f1;
+                            f1 = q1.x * z - q1.y * f1;
+                            col[(size_t)(i + 2) * M] = q2.y * o1 + q2.x * f2;
+                            f2 = q2.x * o1 - q2.y * f2;
+                        }
+                        if (lo2 > lo) {                              // below sweep 2: sweep 1 alone
+                            col[(size_t)lo2 * M] = f2;
+                            for (; i >= lo; --i) {
+                                const double2 q = cur[m - 1 - i];
+                                const double z = col[(size_t)i * M];
+                                col[(size_t)(i + 1) * M] = q.y * z + q.x * f1;
+                                f1 = q.x * z - q.y * f1;
+                            }
+                            col[(size_t)lo * M] = f1;
+                        } else {                                     // lo2 == lo: (2, lo) on the final column lo
+                            const double2 q2 = cur2[m2 - 1 - lo];
+                            col[(size_t)(lo + 1) * M] = q2.y * f1 + q2.x * f2;
+                            col[(size_t)lo * M] = q2.x * f1 - q2.y * f2;
+                        }
+                        pos += (m - lo) + (m2 - lo2);
+                        sidx += 2;
+                        continue;
+                    }
+                }
+                double f = col[(size_t)m * M];
                 for (int i = m - 1; i >= lo; --i) {
-                    const double2 q = rot[pos++];
-                    const double zi = B[(size_t)i * M + r];
-                    B[(size_t)(i + 1) * M + r] = q.y * zi + q.x * f;
+                    const double2 q = cur[m - 1 - i];
+                    const double zi = col[(size_t)i * M];
+                    col[(size_t)(i + 1) * M] = q.y * zi + q.x * f;
                     f = q.x * zi - q.y * f;
                 }
-                B[(size_t)lo * M + r] = f;
+                col[(size_t)lo * M] = f;
+                pos += m - lo;
+                sidx += 1;
             }
         }
         for (int k = tid; k < M; k += GEN_NT) permsm[k] = ws.perm[b * M + k];
