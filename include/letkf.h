@@ -211,7 +211,9 @@ int letkf_last_launch_count(void);
  * capacity by k so that tests can force the log-overflow slow path (default 1); "split" = 1 runs the
  * tridiagonalisation of 48 < M <= 64 as three kernels (pivots down to 33 / trailing 32 x 32 problem /
  * explicit Q; experimental, default 0: measured slower than the single kernel); "sub_chunks" = 1..16
- * sub-chunks per pass of the calling thread's device calls (default 8; measured flat from 4 to 8).
+ * sub-chunks per pass of the calling thread's device calls (default 8; measured flat from 4 to 8);
+ * "mid_reg" = 0 / 1 / 2: the reduction of 64 < M <= 160 with the matrix in shared memory / in
+ * registers up to M = 128 and in shared memory above (default) / in registers at every such M.
  * Returns 0, or -1 for an unknown name. */
 int letkf_set_option(const char* name, int value);
 

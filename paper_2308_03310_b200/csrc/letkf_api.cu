@@ -147,6 +147,7 @@ static cudaError_t allow_smem(K kernel, size_t bytes)
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
+static int g_mid_reg = 1;                // letkf_set_option("mid_reg", 0 / 1 / 2): 64 < M <= 160 reduced in shared memory / registers up to M = 128 / registers
 static bool g_force_generic = false;     // letkf_set_option("force_generic", 1): tests only
 
 // a1/a2 inputs when the matrix is to be formed from the LETKF observations instead of read
@@ -233,8 +234,15 @@ static int stage_T(const double* A, int M, int n, double* V, Workspace ws, cudaS
     if (mid_supported(M) && !g_force_generic) {          // matrix resident in shared memory
         cudaError_t ce;
         const size_t smem = mid_tridiag_smem(M);
-        if ((ce = allow_smem(mid_tridiag_formq, smem)) != cudaSuccess) return (int)ce;
-        KLAUNCH("mid_tridiag_formq", st, mid_tridiag_formq<<<n, MID_TPR * mid_threads(M), smem, st>>>(A, V, ws, M));
+        const int mt = mid_threads(M);
+        // registers hold the matrix up to M = 128 (measured, batch 2^26/M^2: M = 96 6.58 -> 5.12 ms, M = 128 9.42 -> 7.57 ms);
+        // at MT = 160 the 80 matrix registers of a thread spill under the 102 a CTA of 640 allows and
+        // the shared-memory form is as fast (10.5 vs 10.9 ms): mid_reg = 1 (default) / 2 (force) / 0 (never)
+        const bool reg = g_mid_reg == 2 || (g_mid_reg == 1 && mt <= 128);
+        auto kern = reg ? (mt == 96 ? mid_tridiag_formq_reg<96> : (mt == 128 ? mid_tridiag_formq_reg<128> : mid_tridiag_formq_reg<160>))
+                        : (mt == 96 ? mid_tridiag_formq<96> : (mt == 128 ? mid_tridiag_formq<128> : mid_tridiag_formq<160>));
+        if ((ce = allow_smem(kern, smem)) != cudaSuccess) return (int)ce;
+        KLAUNCH("mid_tridiag_formq", st, kern<<<n, MID_TPR * mt, smem, st>>>(A, V, ws, M));
         return 0;
     }
     const size_t td_smem = sizeof(double) * ((4 + GEN_QK) * (size_t)M + GEN_NT / 32);
@@ -1067,6 +1075,7 @@ int letkf_set_option(const char* name, int value)
     if (strcmp(name, "force_generic") == 0) { g_force_generic = value != 0; return LETKF_OK; }
     if (strcmp(name, "pipeline") == 0) { g_pipeline = value != 0; return LETKF_OK; }
     if (strcmp(name, "sub_chunks") == 0) { g_max_sub = (value >= 1 && value <= PIPE_MAX_SUB) ? value : 8; return LETKF_OK; }
+    if (strcmp(name, "mid_reg") == 0) { g_mid_reg = (value >= 0 && value <= 2) ? value : 1; return LETKF_OK; }
     if (strcmp(name, "split") == 0) { g_split = value != 0; return LETKF_OK; }
     if (strcmp(name, "log_shrink") == 0) { g_log_shrink = value >= 1 ? value : 1; return LETKF_OK; }
     if (strcmp(name, "ql_tpb") == 0) { g_ql_tpb = (value == 32 || value == 64 || value == 96) ? value : 0; return LETKF_OK; }

@@ -55,16 +55,89 @@ __device__ __forceinline__ double mid_block_sum(double v, double* red, int nwarp
     return t;
 }
 
+// Explicit Q^T = H_1 H_2 ... H_{M-1} (H_i acts on indices 0..i-1) row by row: row j of Q^T is
+// e_j^T H_{j+1} ... H_{M-1}, so the rows do not depend on each other and a row never has to live
+// in shared memory: 8 lanes hold one row in registers (lane h owns the column pairs h, h+8, ...:
+// 16-byte broadcast loads of the reflectors, which stay where the reduction left them: row i of S,
+// zero-padded to a multiple of 16 columns), apply every reflector to it (dot product reduced
+// with three shuffles, no barrier) and store it straight to global memory.  Row j costs
+// sum_{i>j} 4i flops, so a group takes row g and then row M-1-g: all warps stay busy to the end.
+template <int MT, bool KEEPV>
+__device__ __forceinline__ void mid_formq_rows(const double* S, int LD, const double* taus, int M, double* Qt)
+{
+    constexpr int NP = MT / 16;                       // column pairs per lane
+    const int tid = threadIdx.x, h = tid & 7, g = tid >> 3, ngrp = blockDim.x >> 3;
+    const int g0 = g & ~3;                            // first group of this warp
+    const double2* S2 = reinterpret_cast<const double2*>(S);
+    const int LD2 = LD >> 1;
+#pragma unroll 1
+    for (int pass = 0; pass < 2; ++pass) {
+        const int j = pass == 0 ? g : M - 1 - g;
+        const bool valid = pass == 0 ? (j < M) : (j >= ngrp);
+        const int jmin = pass == 0 ? g0 : max(M - 1 - (g0 + 3), 0);    // smallest row of the warp
+        if (pass == 1 && M - 1 - g0 < ngrp) continue;                  // no valid row in this warp
+        double2 x[NP];
+#pragma unroll
+        for (int k = 0; k < NP; ++k) {
+            const int c = 2 * h + 16 * k;
+            x[k] = make_double2((valid && c == j) ? 1.0 : 0.0, (valid && c + 1 == j) ? 1.0 : 0.0);
+        }
+#pragma unroll 1
+        for (int i = jmin + 1; i <= M - 1; ++i) {
+            const double tau = taus[i];
+            if (tau == 0.0) continue;
+            const double2* v2 = S2 + (size_t)i * LD2 + h;
+            double a0 = 0.0, a1 = 0.0;
+            double2 v[NP];
+#pragma unroll
+            for (int k = 0; k < NP; ++k) {
+                if (16 * k < i) {
+                    v[k] = v2[8 * k];
+                    a0 = fma(x[k].x, v[k].x, a0);
+                    a1 = fma(x[k].y, v[k].y, a1);
+                }
+            }
+            double acc = a0 + a1;
+            acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+            acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+            acc += __shfl_xor_sync(0xffffffffu, acc, 4);
+            acc *= -tau;
+#pragma unroll
+            for (int k = 0; k < NP; ++k) {
+                if (16 * k < i) {
+                    const double2 u = KEEPV ? v[k] : v2[8 * k];
+                    x[k].x = fma(acc, u.x, x[k].x);
+                    x[k].y = fma(acc, u.y, x[k].y);
+                }
+            }
+        }
+        if (valid) {
+            double* qrow = Qt + (size_t)j * M;
+#pragma unroll
+            for (int k = 0; k < NP; ++k) {
+                const int c = 2 * h + 16 * k;
+                if ((M & 1) == 0) {
+                    if (c < M) *reinterpret_cast<double2*>(qrow + c) = x[k];
+                } else {
+                    if (c < M) qrow[c] = x[k].x;
+                    if (c + 1 < M) qrow[c + 1] = x[k].y;
+                }
+            }
+        }
+    }
+}
+
 // MID_TPR threads per row: thread (j, h) = (tid % RP, tid / RP), RP = ceil32(M), owns the column
 // pairs p = h, h + TPR, ... of row j (16-byte accesses); the partial products of a row meet in
 // shared memory.  vs / wsm are kept zero at index i (the first dead column) so that a pair that
 // straddles the active range contributes nothing.
-__global__ void __launch_bounds__(160 * MID_TPR)
+template <int MT>
+__global__ void __launch_bounds__(MT * MID_TPR, MT == 96 ? 2 : 1)
 mid_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, int M)
 {
     extern __shared__ __align__(16) double sm[];
     const int LD = mid_ld(M);
-    const int RP = blockDim.x / MID_TPR;
+    constexpr int RP = MT;
     double* S    = sm;                       // [M][LD]
     double* vs   = sm + (size_t)M * LD;      // [LD]
     double* wsm  = vs + LD;                  // [LD]
@@ -146,60 +219,149 @@ mid_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, int M
             }
         }
         if (h == 0 && j < i) S[i * LD + j] = vj;                   // keep the reflector in the dead row i (no
-        if (h == 1 && j == 0) S[i * LD + i] = 0.0;                 // update touches it); (pair overhang)
+        if (h == 1 && j < 16 && i + j < LD) S[i * LD + i + j] = 0.0;  // update touches it), zero-padded for mid_formq_rows
         __syncthreads();
     }
     if (tid == 0) { dws[0] = S[0]; ews[M - 1] = 0.0; }
 
-    // Q^T = H_1 H_2 ... H_{M-1}, grown in place: B_i = diag(B_{i-1}, 1) H_i on the leading i x i
-    for (int i = 1; i <= M - 1; ++i) {
-        if (h == 0) {
-            if (j < i) vs[j] = S[i * LD + j];
-            if (j == i) vs[j] = 0.0;
-        }
-        const double tau = taus[i];
-        __syncthreads();                                           // reflector copied before row i-1 ... are cleared
-        if (h == 0 && j < i - 1) { S[(i - 1) * LD + j] = 0.0; S[j * LD + (i - 1)] = 0.0; }
-        if (h == 1 && j == 0) S[(i - 1) * LD + (i - 1)] = 1.0;
-        __syncthreads();
-        const int npair = (i + 1) >> 1;
-        if (tau != 0.0) {
-            double a0 = 0.0, a1 = 0.0;
-            if (j < i) {
-#pragma unroll 4
-                for (int p = h; p < npair; p += MID_TPR) {
-                    const double2 r = row2[p], v = v2[p];
-                    a0 = fma(r.x, v.x, a0);
-                    a1 = fma(r.y, v.y, a1);
-                }
-            }
-            pd[h * RP + j] = a0 + a1;
-            __syncthreads();
-            if (j < i) {
-                double acc = 0.0;
+    __syncthreads();                                               // taus, reflector rows complete
+    double* Qt = V_ + b * M * M;
+    mid_formq_rows<MT, MT <= 128>(S, LD, taus, M, Qt);
+}
+
+// a3 with the matrix in REGISTERS (the idea of fast_tridiag_formq with four threads per row): the
+// shared-memory copy of A is only the staging area of the load; from then on thread (j, h) =
+// (tid % MT, tid / MT) holds the column pairs h, h+4, ... of row j, and shared memory carries
+// nothing but the vectors every row needs: v_i (written, zero-padded, into row i of S, where the
+// explicit-Q pass finds it) and p.  h is the same in all lanes of a warp, so a 16-byte load of
+// (v_c, v_c+1) is ONE broadcast wavefront that feeds two FMAs in every lane (with the four
+// threads of a row in one warp the same load is four wavefronts and the shared-memory pipe
+// binds: measured, 1.3 / 1.7 k cycles per pivot for the product / the update at M = 96).  Pivot i:
+//   B0  the raw row i (final: its four owners dumped it after pivot i+1's update) is in xs
+//       -> warps of h = 0: sigma, tau, beta, v_i into row i of S
+//   B1  -> partial products sum_c a_jc v_c over the thread's pairs (8-column blocks with 8k < i:
+//          block-uniform bounds, static register indices) into pd[h][j]
+//   B2  -> warps of h = 0: p_j = tau sum_h pd[h][j], the warp's share of p.v
+//   B3  -> a_jc -= v_j p_c + (p_j - tau (p.v) v_j) v_c
+template <int MT>
+__global__ void __launch_bounds__(MT * MID_TPR, MT == 96 ? 2 : 1)
+mid_tridiag_formq_reg(const double* __restrict__ A_, double* V_, Workspace ws, int M)
+{
+    extern __shared__ __align__(16) double sm[];
+    static_assert(MID_TPR == 4, "column pairs are dealt to four threads per row");
+    constexpr int NP = MT / 8;                   // column pairs per thread
+    constexpr int NW0 = MT / 32;                 // warps of h = 0
+    const int LD = mid_ld(M), LD2 = LD >> 1;
+    double* S    = sm;                           // [M][LD]
+    double* xs   = sm + (size_t)M * LD;          // [LD]      raw pivot row
+    double* pb   = xs + LD;                      // [LD]      p
+    double* taus = pb + LD;                      // [LD]
+    double* pd   = taus + LD;                    // [MID_TPR][MT] partial products
+    double* red  = pd + MID_TPR * MT;            // [2][32]
+    const int tid = threadIdx.x, j = tid % MT, h = tid / MT, lane = tid & 31, warp = tid >> 5;
+    const size_t b = blockIdx.x;
+    const double* A = A_ + b * M * M;
+    double* dws = ws.dws + b * M;
+    double* ews = ws.ews + b * M;
+
+    // full symmetric copy of the lower triangle: thread (j, h) copies column j of rows h, h+4, ...
+    if (j < M)
+        for (int r = h; r < M; r += MID_TPR) S[r * LD + j] = (r >= j) ? A[(size_t)r * M + j] : A[(size_t)j * M + r];
+    for (int c = tid; c < LD; c += blockDim.x) pb[c] = 0.0;
+    __syncthreads();
+    double2 a[NP];
+    {
+        const double2* row2 = reinterpret_cast<const double2*>(S + (size_t)min(j, M - 1) * LD);
 #pragma unroll
-                for (int hh = 0; hh < MID_TPR; ++hh) acc += pd[hh * RP + j];
-                acc *= -tau;
-#pragma unroll 4
-                for (int p = h; p < npair; p += MID_TPR) {
-                    double2 r = row2w[p];
-                    const double2 v = v2[p];
-                    r.x = fma(acc, v.x, r.x);
-                    r.y = fma(acc, v.y, r.y);
-                    row2w[p] = r;
+        for (int k = 0; k < NP; ++k) {
+            const int c = 2 * h + 8 * k;
+            double2 t = make_double2(0.0, 0.0);
+            if (j < M && c < M) { t = row2[h + 4 * k]; if (c + 1 >= M) t.y = 0.0; }
+            a[k] = t;
+        }
+    }
+    __syncthreads();                             // S is free: it now collects the reflectors
+    const double2* S2 = reinterpret_cast<const double2*>(S);
+    double2* xs2 = reinterpret_cast<double2*>(xs);
+    auto dump_row = [&]() {                      // the four owners of the next pivot row: raw row -> xs
+#pragma unroll
+        for (int k = 0; k < NP; ++k)
+            if (2 * h + 8 * k < LD) xs2[h + 4 * k] = a[k];
+    };
+    if (j == M - 1) dump_row();
+    for (int i = M - 1; i >= 1; --i) {
+        __syncthreads();                                                     // B0
+        if (h == 0) {
+            double part = 0.0;
+#pragma unroll
+            for (int u = 0; u < MT / 32; ++u) {
+                const int c = lane + 32 * u;
+                const double x = (c < i - 1) ? xs[c] : 0.0;
+                part = fma(x, x, part);
+            }
+            const double sigma = warp_sum(part);                             // each of the NW0 warps, redundantly
+            const double alpha = xs[i - 1];
+            double tau = 0.0, scal = 0.0, beta = alpha;                      // sigma == 0: H_i = I (reading G19)
+            if (sigma != 0.0) {
+                const double nrm2 = fma(alpha, alpha, sigma);
+                const double rinv = rsqrt(nrm2);
+                beta = -copysign(nrm2 * rinv, alpha);
+                tau = fma(fabs(alpha), rinv, 1.0);
+                scal = 1.0 / (alpha - beta);
+            }
+            if (j < LD) S[(size_t)i * LD + j] = (j < i - 1) ? xs[j] * scal : ((j == i - 1) ? 1.0 : 0.0);
+            if (j == 0) { dws[i] = xs[i]; ews[i - 1] = beta; taus[i] = tau; }
+        }
+        __syncthreads();                                                     // B1
+        const double tau = taus[i];
+        if (tau != 0.0) {                                                    // the same in every thread
+            const bool act = (j & ~7) < i;                                   // rows of a dead 8-row block do nothing
+            const double2* v2 = S2 + (size_t)i * LD2 + h;
+            if (act) {
+                double acc[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+                for (int k = 0; k < NP; ++k) {
+                    if (8 * k < i) {
+                        const double2 v = v2[4 * k];
+                        acc[2 * (k & 1)] = fma(a[k].x, v.x, acc[2 * (k & 1)]);
+                        acc[2 * (k & 1) + 1] = fma(a[k].y, v.y, acc[2 * (k & 1) + 1]);
+                    }
+                }
+                pd[h * MT + j] = (acc[0] + acc[1]) + (acc[2] + acc[3]);
+            }
+            __syncthreads();                                                 // B2
+            if (h == 0) {
+                double pj = 0.0;
+                if (act && j < i) pj = tau * ((pd[j] + pd[MT + j]) + (pd[2 * MT + j] + pd[3 * MT + j]));
+                const double vj = (j < i) ? S[(size_t)i * LD + j] : 0.0;
+                const double pvw = warp_sum(pj * vj);
+                if (j < LD) pb[j] = pj;
+                if (lane == 0) red[warp] = pvw;
+            }
+            __syncthreads();                                                 // B3
+            if (act) {
+                const double2* p2 = reinterpret_cast<const double2*>(pb) + h;
+                double ptv = 0.0;
+#pragma unroll
+                for (int w = 0; w < NW0; ++w) ptv += red[w];
+                const double vj = (j < i) ? S[(size_t)i * LD + j] : 0.0;
+                const double pj = (j < i) ? pb[j] : 0.0;
+                const double wj = fma(-tau * ptv, vj, pj);                   // p_j - 2 K v_j, K = tau (p.v) / 2
+#pragma unroll
+                for (int k = 0; k < NP; ++k) {
+                    if (8 * k < i) {
+                        const double2 v = v2[4 * k], p = p2[4 * k];
+                        a[k].x = fma(-vj, p.x, fma(-wj, v.x, a[k].x));
+                        a[k].y = fma(-vj, p.y, fma(-wj, v.y, a[k].y));
+                    }
                 }
             }
         }
-        __syncthreads();
+        if (j == i - 1) dump_row();
     }
-    if (h == 0 && j < M - 1) { S[(M - 1) * LD + j] = 0.0; S[j * LD + (M - 1)] = 0.0; }
-    __syncthreads();
-    if (tid == 0) S[(M - 1) * LD + (M - 1)] = 1.0;
-    __syncthreads();
-    if (j < M) {
-        double* Qt = V_ + b * M * M;
-        for (int r = h; r < M; r += MID_TPR) Qt[(size_t)r * M + j] = S[r * LD + j];
-    }
+    if (tid == 0) { dws[0] = a[0].x; ews[M - 1] = 0.0; }
+    __syncthreads();                                                         // taus, reflector rows complete
+    mid_formq_rows<MT, MT <= 128>(S, LD, taus, M, V_ + b * M * M);
 }
 
 // a5: thread r owns column r of Q^T (= row r of Q); a rotation (i, i+1) mixes rows i, i+1 of Q^T.
