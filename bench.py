@@ -522,7 +522,7 @@ def run_ours(args):
                 tf = syev_model_flops(Ms) * Bs / (sms * 1e-3) / 1e12
                 sweep.append({"M": Ms, "batch": Bs, "ms": round(sms, 4), "matrices_per_s": Bs / (sms * 1e-3),
                               "model_9M3_tflops": round(tf, 3), "frac_of_fp64_peak": round(tf / peak_tflops, 4),
-                              "path": "registers (fast_*)" if Ms <= 64 else ("shared memory (mid_*)" if Ms <= 160 else "global/L2 (generic_*)"),
+                              "path": "registers (fast_*)" if Ms <= 64 else ("registers + shared memory (mid_*)" if Ms <= 160 else "global/L2 (generic_*)"),
                               "info_nonzero": int((infos != 0).sum())})
                 del As, Vs, ws_, wk, infos
             line["sweep"] = sweep

@@ -297,7 +297,18 @@ static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws,
         const int ms = mid_apply_round(M, ws.swcap);
         const size_t smem = mid_apply_smem(M, ws.swcap, ms);
         if ((ce = allow_smem(mid_apply, smem)) != cudaSuccess) return (int)ce;
-        KLAUNCH("mid_apply", st, mid_apply<<<n, mid_threads(M), smem, st>>>(V, ws, M, ms));
+        const int nsplit = mid_apply_split(M), ncol = mid_apply_cols(M);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)n * nsplit);
+        cfg.blockDim = dim3((ncol + 31) / 32 * 32);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = nsplit; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        KLAUNCH("mid_apply", st, cudaLaunchKernelEx(&cfg, mid_apply, V, ws, M, ms, nsplit, ncol));
         KLAUNCH("generic_apply(flagged)", st,
                 generic_apply<<<(n < 296 ? n : 296), GEN_NT, ap_smem, st>>>(V, w, ws, M, n, info, /*only_flagged=*/1, /*q_rowmajor=*/0));
         return 0;

@@ -28,15 +28,21 @@ static inline size_t mid_tridiag_smem(int M)
 {
     return sizeof(double) * ((size_t)M * mid_ld(M) + 3 * ((size_t)mid_ld(M)) + (size_t)MID_TPR * mid_threads(M) + 64 + 8);
 }
+// the columns of a matrix are dealt to this many CTAs (a cluster) in mid_apply
+static inline int mid_apply_split(int M) { return (M > 96 && M <= 128) ? 2 : 1; }
+static inline int mid_apply_cols(int M) { const int ns = mid_apply_split(M); return ((M + ns - 1) / ns + 1) & ~1; }
 static inline size_t mid_apply_smem(int M, int swcap, int ms)
 {
-    return sizeof(double) * ((size_t)M * (M + 1) + 4 * (size_t)ms * (size_t)M) + sizeof(uint32_t) * (size_t)swcap + sizeof(int) * (size_t)M + 32;
+    const int ld = (mid_apply_cols(M) + 1) | 1;
+    return sizeof(double) * ((((size_t)M * ld + 1) & ~(size_t)1) + 4 * (size_t)ms * (size_t)M) + sizeof(uint32_t) * (size_t)swcap + sizeof(int) * (size_t)M + 32;
 }
-// sweeps staged per barrier round of mid_apply: as many (<= 4) as shared memory holds beside the matrix
+// sweeps staged per barrier round of mid_apply: as many (<= 4) as shared memory holds beside the
+// matrix -- beside three CTAs per SM when the columns are split
 static inline int mid_apply_round(int M, int swcap)
 {
+    const size_t cap = mid_apply_split(M) > 1 ? (size_t)(228 * 1024) / 3 - 1024 : (size_t)226 * 1024;
     int ms = 4;
-    while (ms > 1 && mid_apply_smem(M, swcap, ms) > 226 * 1024) ms >>= 1;
+    while (ms > 1 && mid_apply_smem(M, swcap, ms) > cap) ms >>= 1;
     return ms;
 }
 
@@ -364,30 +370,40 @@ mid_tridiag_formq_reg(const double* __restrict__ A_, double* V_, Workspace ws, i
     mid_formq_rows<MT, MT <= 128>(S, LD, taus, M, V_ + b * M * M);
 }
 
-// a5: thread r owns column r of Q^T (= row r of Q); a rotation (i, i+1) mixes rows i, i+1 of Q^T.
-// The (c, s) of `ms` sweeps are staged per barrier round, double-buffered, straight from the log
-// into shared memory with cp.async (no registers: a thread never waits for the log before it
+// a5: thread r owns column c0 + r of Q^T (= a row of Q); a rotation (i, i+1) mixes rows i, i+1 of
+// Q^T.  The (c, s) of `ms` sweeps are staged per barrier round, double-buffered, straight from the
+// log into shared memory with cp.async (no registers: a thread never waits for the log before it
 // rotates); inside a round the threads do not depend on each other (each rotates its own column).
+// The kernel is chain-latency bound and shared memory (M x 8 B per column) caps the warps per SM,
+// so the columns of one matrix may be dealt to the `nsplit` CTAs of a thread-block cluster
+// (nsplit = 2 for 96 < M <= 128: three CTAs of 64 columns per SM instead of one of 128).  The
+// CTAs of a matrix share nothing but the buffer: V is read as Q^T and written as sorted row-major
+// V in place, so every CTA of the cluster must have read its columns before any of them writes
+// its rows -- one cluster barrier after the load.
 __global__ void __launch_bounds__(160)
-mid_apply(double* __restrict__ V_, Workspace ws, int M, int ms)
+mid_apply(double* __restrict__ V_, Workspace ws, int M, int ms, int nsplit, int ncol)
 {
     extern __shared__ __align__(16) double sm[];
-    const int LD = M + 1;
-    double*   S    = sm;                                                   // [M][LD]  Q^T
+    const int LD = (ncol + 1) | 1;
+    double*   S    = sm;                                                   // [M][LD]  columns c0 ... of Q^T
     double2*  cs   = reinterpret_cast<double2*>(sm + (((size_t)M * LD + 1) & ~(size_t)1));   // [2][ms][M]
     uint32_t* hdr  = reinterpret_cast<uint32_t*>(cs + 2 * ms * M);
     int*      perm = reinterpret_cast<int*>(hdr + ws.swcap);
     const int r = threadIdx.x, nt = blockDim.x;
-    const size_t b = blockIdx.x;
-    if (ws.flags[b]) return;                          // finished by generic_apply (slow path)
+    const size_t b = blockIdx.x / nsplit;
+    const int c0 = (int)(blockIdx.x % nsplit) * ncol;
+    const int nc = min(ncol, M - c0);                 // columns of this CTA (<= 0: none)
+    if (ws.flags[b]) return;                          // finished by generic_apply (slow path); the whole cluster leaves
     double* V = V_ + b * M * M;
     const int nsw = ws.nsweeps[b];
     const double2* rot = ws.rot + b * ws.logcap;
 
     for (int s = r; s < nsw; s += nt) hdr[s] = ws.hdr[b * ws.swcap + s];
-    if (r < M) {
-        for (int k = 0; k < M; ++k) S[k * LD + r] = V[(size_t)k * M + r];
-        perm[r] = ws.perm[b * M + r];
+    if (r < nc)
+        for (int k = 0; k < M; ++k) S[k * LD + r] = V[(size_t)k * M + c0 + r];
+    for (int k = r; k < M; k += nt) perm[k] = ws.perm[b * M + k];
+    if (nsplit > 1) {
+        asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
     }
     __syncthreads();
 
@@ -408,7 +424,7 @@ mid_apply(double* __restrict__ V_, Workspace ws, int M, int ms)
     for (int s0 = 0; s0 < nsw; s0 += ms) {
         const double2* cur0 = cs + ((s0 / ms) & 1) * ms * M;
         pos = stage(s0 + ms, pos, cs + (((s0 / ms) + 1) & 1) * ms * M);
-        if (r < M) {
+        if (r < nc) {
             double* col = S + r;
             for (int t = 0; t < ms && s0 + t < nsw; ++t) {
                 const uint32_t h = hdr[s0 + t];
@@ -437,10 +453,10 @@ mid_apply(double* __restrict__ V_, Workspace ws, int M, int ms)
         __syncthreads();
     }
 
-    // V[row][k] = Qt'[perm[k]][row]: one warp per output row, lanes over the sorted columns
+    // V[c0 + row][k] = Qt'[perm[k]][c0 + row]: one warp per output row, lanes over the sorted columns
     const int lane = r & 31, warp = r >> 5, nw = nt >> 5;
-    for (int row = warp; row < M; row += nw)
-        for (int k = lane; k < M; k += 32) V[(size_t)row * M + k] = S[perm[k] * LD + row];
+    for (int row = warp; row < nc; row += nw)
+        for (int k = lane; k < M; k += 32) V[(size_t)(c0 + row) * M + k] = S[perm[k] * LD + row];
 }
 
 }  // namespace letkf
