@@ -321,7 +321,7 @@ mid_tridiag_formq_reg(const double* __restrict__ A_, double* V_, Workspace ws, i
         __syncthreads();                                                     // B1
         const double tau = taus[i];
         if (tau != 0.0) {                                                    // the same in every thread
-            const bool act = (j & ~7) < i;                                   // rows of a dead 8-row block do nothing
+            const bool act = (j & ~31) < i;                                  // warp-uniform: a warp of dead rows does nothing
             const double2* v2 = S2 + (size_t)i * LD2 + h;
             if (act) {
                 double acc[4] = {0.0, 0.0, 0.0, 0.0};
