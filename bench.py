@@ -129,7 +129,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    from paper_2308_03310_b200 import workloads as wl
+    from harness import workloads as wl
     sample = 4096
     A = wl.letkf_shaped(sample, M_HEAD, P_HEAD, config_index=3)
     for _ in range(args.warmup):
@@ -225,7 +225,8 @@ def cusolver_compare(A_dev, steps=2):
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2308_03310_b200 import build as b, letkf, workloads as wl
+    from paper_2308_03310_b200 import build as b, letkf, sharding
+    from harness import workloads as wl
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -248,11 +249,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return sharding.max_over_ranks(x, device="cuda")
 
     M, B, p = M_HEAD, BATCH_HEAD, P_HEAD
     # weak scaling: every rank owns a full config-3 batch (its own seed); no data-path collective

@@ -156,14 +156,6 @@ def toeplitz_tridiagonal(M, a=0.0, b=1.0):
     return A
 
 
-def shard_range(batch, rank, world_size):
-    """Contiguous slice of the grid-point batch owned by ``rank`` (Proc.3 l.5:
-    n_x in [m Nx/M, (m+1) Nx/M)).  Integer arithmetic; covers ragged batches."""
-    lo = (batch * rank) // world_size
-    hi = (batch * (rank + 1)) // world_size
-    return lo, hi
-
-
 def grid_inputs(Ny=128, Nx=128, M=64, V=2, nstate=9, config_index=6, obs_every=1):
     """Grid form of config 4: instead of a materialised Y_loc the
     forecast observations of the whole periodic grid, Yf[V][Ny][Nx][M] ~ 0.05 + N(0, 0.1^2) (NOT

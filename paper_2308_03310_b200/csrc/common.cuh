@@ -17,16 +17,40 @@ struct Workspace {
     double*   ews;      // [chunk][M]
     int*      perm;     // [chunk][M]
     int*      nsweeps;  // [chunk]
-    int*      flags;    // [chunk]   1 = rotation log overflowed, finish on the slow path
+    int*      flags;    // [chunk]   FLAG_REPLAY: replay the log; FLAG_SLOW: log unusable, classic iteration in the apply
+                        //           kernel; FLAG_GETVEC: no log, eigenvectors by twisted factorisation
     uint32_t* hdr;      // [chunk][swcap]
     double2*  rot;      // [chunk][logcap]
+    double*   refl;     // [chunk][reflstride]  M <= 64: the Householder reflectors and their taus (RefLayout)
+    double*   s1;       // [chunk][M]  eigenvalues of the first QL pass by position (classify mode; else unused)
     int       swcap;
     int       logcap;
+    int       reflstride;
     unsigned long long* rot_counter;   // profiling only (NULL otherwise): total rotations logged
 };
 
 __host__ __device__ inline int sweep_capacity(int M) { return 6 * M + 32; }
-__host__ __device__ inline int log_capacity(int M)   { return 2 * M * M + 4 * M + 16; }
+// rotations the log of one matrix holds.  One-pass QL (Wilkinson shifts): measured mean 1.05 M^2, max
+// 1.36 M^2 over the configured workloads -> 2 M^2.  Two-pass QL (second pass shifted by the
+// eigenvalues of the first): mean 0.71 M^2, max 0.81 M^2 -> M^2.  A matrix that needs more is
+// finished by the slow path (flags[b]).
+__host__ __device__ inline int log_capacity(int M, bool two_pass = false)
+{
+    return (two_pass ? 1 : 2) * M * M + 4 * M + 16;
+}
+
+// ---- eigenvectors of T without rotations (fast_apply, M <= 64) -----------------
+// A matrix is "easy" when, inside every unreduced block of T, no two eigenvalues are closer than
+// GV_TINY ||T|| and no more than GV_PH eigenvalues lie within GV_GAP ||T|| above any eigenvalue: its
+// eigenvectors then come from twisted factorisations of T - lambda I (one per thread), and the pairs
+// closer than GV_GAP ||T|| are made orthogonal by a first-order symmetric correction.  Every other
+// matrix has its rotations logged and replayed.  ql_log_kernel (mode 2) classifies, fast_apply
+// follows the flag.
+constexpr double GV_GAP  = 4.0e-3;    // eps C / GV_GAP bounds the loss of orthogonality left uncorrected (C ~ 7 measured)
+constexpr double GV_TINY = 1.0e-8;    // the correction is first order: (eps C / GV_TINY)^2 must stay far below the tolerance
+constexpr int    GV_PH   = 4;         // partners a vector may have on either side
+constexpr int    FLAG_REPLAY = 0, FLAG_SLOW = 1, FLAG_GETVEC = 2, FLAG_PENDING = 3;   // Workspace::flags (PENDING: between
+                                                                                     // the classifying and the logging QL kernel)
 
 __device__ __forceinline__ double warp_sum(double v)
 {
@@ -64,7 +88,8 @@ __device__ __forceinline__ double block_sum(double v, double* red)
 // Returns 1 with (lo, m) set, 0 when all eigenvalues have converged, -1 if the sweep would not
 // fit into sink_cap (nothing is changed in that case).
 // Conventions fixed in DESIGN.md reading G10: Wilkinson shift, deflation when
-// |e_m| <= 2^-53 (|d_m| + |d_m+1|), at most 30 sweeps per eigenvalue (then st.fail is bumped).
+// |e_m| <= 2^-53 max(|d_m| + |d_m+1|, max_i(|d_i| + |e_i|)), at most QL_MAX_SWEEPS sweeps per eigenvalue
+// (then st.fail is bumped).
 struct QLState { int l; int iter; int fail; double thr; };   // thr = 2^-53 max_i(|d_i| + |e_i|), set by ql_threshold
 
 constexpr int QL_MAX_SWEEPS = 60;    // per eigenvalue (reading G10)

@@ -1,18 +1,20 @@
 // fast_kernels.cuh -- register-resident path for M <= 64 (the paper's sizes, Table I,
 // and the headline M = 64).
 //
-// Design: a matrix lives in the REGISTERS of MT threads, one row (or, while
-// Q is formed, one column) per thread, for its whole life inside a kernel.  An SM issues 64 fp64
-// FMAs per clock but shared memory delivers only 16 doubles per clock, so BLAS-2 work fed from
-// shared memory cannot pass 25% of the fp64 peak; here shared memory only carries the
-// broadcast vectors (one LDS.128 feeds two FMAs in every lane).  Register arrays need
-// compile-time indices: the reduction runs in groups of 8 pivots with statically shaped 8-column
-// block loops (pivot_group<G>), the rotation replay in blocks of 4 rotations entered through a
-// switch with fall-through cases (apply_sweep).
+// Design: a matrix lives in the REGISTERS of MT threads, one row (or one
+// column) per thread, for its whole life inside a kernel.  An SM issues 64 fp64 FMAs per clock but
+// shared memory delivers only 16 doubles per clock, so BLAS-2 work fed from shared memory cannot
+// pass 25% of the fp64 peak; here shared memory only carries the broadcast vectors (one LDS.128
+// feeds two FMAs in every lane).  Register arrays need compile-time indices: the reduction runs in
+// groups of 8 pivots with statically shaped 8-column block loops (pivot_group<G>), the rotation
+// replay in blocks of 4 rotations entered through a switch with fall-through cases (apply_sweep).
 //
-//   fast_tridiag_formq<MT>   a3 + explicit Q  : thread j = row j of A, then column r of Q
-//   ql_log_kernel            a4               : ql_kernel.cuh, one thread per matrix
-//   fast_apply<MT>           a5 (+ a6-a9)     : thread r = row r of Q; replays the rotation log
+//   fast_tridiag<MT>   a3 (+ a1, a2)   : thread j = row j of A; leaves (d, e) and the reflectors
+//   ql_log_kernel      a4              : ql_kernel.cuh, one thread per matrix, rotations logged
+//   fast_apply<MT>     a5 (+ a6-a9)    : thread r = row r of Z (from I): replays the log; the matrix
+//                                        is turned through shared memory and thread k applies the
+//                                        reflectors to eigenvector k: V = H_{M-1} ... H_1 Z
+// Q is never formed and the matrix crosses HBM once in (A) and once out (V).
 #pragma once
 #include "common.cuh"
 
@@ -153,7 +155,7 @@ template <int MT> struct RefLayout {
     __device__ static constexpr int len(int G) { return 8 * (G + 1); }
 };
 
-// Explicit Q: reflectors i = 8G+1 ... 8G+8 applied to the column q held by this thread.  The
+// Back-transform: reflectors i = 8G+1 ... 8G+8 applied to the column q held by this thread.  The
 // __syncwarp() after every 8-column block is a scheduling fence: ptxas does not move shared-memory
 // loads across it, and without it the loads of a whole pass are hoisted and the matrix spills.
 template <int MT, int G>
@@ -304,10 +306,18 @@ struct GridArgs {
 __host__ __device__ inline double localisation(int kind, double L, double dist)
 {
     if (kind == 0) return exp(-(dist * dist) / (2.0 * L * L));
-    const double z = dist / L;
-    if (z >= 2.0) return 0.0;
-    if (z <= 1.0) return ((((-0.25 * z + 0.5) * z + 0.625) * z - 5.0 / 3.0) * z) * z + 1.0;
-    return (((((1.0 / 12.0) * z - 0.5) * z + 0.625) * z + 5.0 / 3.0) * z - 5.0) * z + 4.0 - (2.0 / 3.0) / z;
+    // Gaspari-Cohn: near branch is even-odd split in u = z^2, 1 - (5/3) u + (5/8) u z + (1/2) u^2 - (1/4) u^2 z;
+    // far branch 4 - 5 z + (5/3) u + (5/8) u z - (1/2) u^2 + (1/12) u^2 z - 2 / (3 z)
+    const double z = dist / L, u = z * z;
+    if (!(z < 2.0)) return 0.0;
+    if (z <= 1.0) {
+        const double even = fma(u, fma(u, 0.5, -5.0 / 3.0), 1.0);
+        const double odd = u * fma(u, -0.25, 0.625);
+        return fma(odd, z, even);
+    }
+    const double even = fma(u, fma(u, -0.5, 5.0 / 3.0), 4.0);
+    const double odd = fma(u, fma(u, 1.0 / 12.0, 0.625), -5.0);
+    return fma(odd, z, even) - 2.0 / (3.0 * z);
 }
 
 // descriptor of local observation row i of grid point (y, x): index of the observed point in the
@@ -354,20 +364,16 @@ grid_gather(GridArgs g, int M, int p, double* __restrict__ Yb, double* __restric
 }
 
 // ---------------------------------------------------------------------------------------------
-// a3 + explicit Q for one matrix per CTA.  gram == true: the matrix is not read from A but formed
+// a3 for one matrix per CTA.  gram == true: the matrix is not read from A but formed
 // from the LETKF inputs (a1, a2: Eq.17 and the right factor of Eq.14) straight into the registers.
-// Split form of the M in (48, 64] reduction (template SPLIT): this kernel
-// stops after pivot 33; the trailing 32 x 32 problem (fast_tridiag_tail, one warp per matrix, 2.5x
-// the CTAs per SM) and the explicit Q (fast_formq, one warp per 32 columns) are kernels of their
-// own, so that no warp sits idle holding registers while another finishes.  Scratch per matrix
-// (aliased onto the matrix's rotation log, which is not written before the QL kernel): doubles
-//   [0, 2304) reflectors in RefLayout order | [2304, 2368) taus | [2368, 3392) trailing 32 x 32 rows
-//   | [3392, 3456) raw pivot column of pivot 32 | [3456, 3464) sigma partial, -, -, -, alpha
-constexpr int SPLIT_TAUS = 2304, SPLIT_TR = 2368, SPLIT_XS = 3392, SPLIT_RED = 3456, SPLIT_DOUBLES = 3464;
+// Output: (d, e) in ws.dws / ws.ews, and either (QFORM) the explicit Q = H_{M-1} ... H_1, row-major, in
+// Q_, or the reflectors with their taus in ws.refl (RefLayout order, taus behind them) for the
+// back-transform in fast_apply.
+template <int MT> __host__ __device__ constexpr int refl_doubles() { return RefLayout<MT>::TOTAL + FastCfg<MT>::NT; }
 
-template <int MT, bool GRAM, bool SPLIT = false>
+template <int MT, bool GRAM, bool QFORM>
 __global__ void __launch_bounds__(FastCfg<MT>::NT) __maxnreg__((MT == 64) ? LETKF_TRI_REGS64 : (MT == 48 ? 168 : (MT == 32 ? 128 : 80)))
-fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Workspace ws, int M,
+fast_tridiag(const double* __restrict__ A_, double* __restrict__ Q_, Workspace ws, int M,
                    const double* __restrict__ Yb_, const double* __restrict__ d_,
                    const double* __restrict__ r_, int p, double shift, double* __restrict__ gout_,
                    GridArgs grid)
@@ -523,7 +529,7 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
 #pragma unroll
             for (int t = 0; t < 4; ++t)
 #pragma unroll
-                for (int ct = c0 / 8; ct < (c0 + CH) / 8; ++ct)
+                for (int ct = c0 / 8; ct < (c0 + CH) / 8 && ct < CT; ++ct)   // (MT = 48: the last pass is ragged)
                     if (8 * (rt0 + t) < MT)
                         *reinterpret_cast<double2*>(cbuf + (8 * t + (lane >> 2)) * LDC + (8 * ct - c0) + 2 * (lane & 3)) =
                             make_double2(acc[t][ct][0], acc[t][ct][1]);
@@ -532,9 +538,11 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
                 const double2* row2 = reinterpret_cast<const double2*>(cbuf + lane * LDC);
 #pragma unroll
                 for (int q = 0; q < CH / 2; ++q) {
-                    const double2 v = row2[q];
-                    a[c0 + 2 * q] = v.x;
-                    a[c0 + 2 * q + 1] = v.y;
+                    if (c0 + 2 * q + 1 < MT) {                           // MT is even: pairs never straddle the end
+                        const double2 v = row2[q];
+                        a[c0 + 2 * q] = v.x;
+                        a[c0 + 2 * q + 1] = v.y;
+                    }
                 }
             }
         }
@@ -564,110 +572,47 @@ fast_tridiag_formq(const double* __restrict__ A_, double* __restrict__ Q_, Works
     }
     // a warp leaves pivot_groups_down when the rows it holds are done (after the B1 that closes
     // the last pivot it took part in), the others carry on with barriers that no longer count it
-    if constexpr (SPLIT) {
-        static_assert(MT == 64, "the split form is for the MT = 64 bucket");
-        pivot_groups_range<MT, (MT - 2) / 8, 4>(a, sh, M, dws, ews);
-        __syncthreads();
-        double* sc = reinterpret_cast<double*>(ws.rot + b * ws.logcap);
-        for (int k = RefLayout<MT>::base(4) + j; k < RefLayout<MT>::TOTAL; k += C::NT) sc[k] = sh.R[k];
-        sc[SPLIT_TAUS + j] = (j >= 33) ? sh.taus[j] : 0.0;
-        if (j < 32) {
-            double2* tr = reinterpret_cast<double2*>(sc + SPLIT_TR + j * 32);
-#pragma unroll
-            for (int c = 0; c < 32; c += 2) tr[c >> 1] = make_double2(a[c], a[c + 1]);
-            sc[SPLIT_XS + j] = sh.xs[j];
-            if (j < 8) sc[SPLIT_RED + j] = sh.red[j];
-        }
-        return;
-    } else {
     pivot_groups_down<MT, (MT - 2) / 8>(a, sh, M, dws, ews);
-    __syncwarp();
-
-    // ---- explicit Q = H_{M-1} ... H_1: thread r owns column r of Q; no synchronisation needed.
-    // Column r only needs H_i with i > r, and a warp leaves the loop above exactly when all
-    // reflectors with i >= its first row have been stored (barrier 2 of those steps included it),
-    // so the upper warps form their columns of Q while warp 0 is still reducing the last 32 rows.
-    double (&q)[MT] = a;
+    if constexpr (QFORM) {
+        // ---- explicit Q = H_{M-1} ... H_1: thread r owns column r of Q; no synchronisation needed.
+        // Column r only needs H_i with i > r, and a warp leaves the loop above exactly when all
+        // reflectors with i >= its first row have been stored (barrier 2 of those steps included it),
+        // so the upper warps form their columns of Q while warp 0 is still reducing the last 32 rows.
+        __syncwarp();
+        double (&q)[MT] = a;
 #pragma unroll
-    for (int c = 0; c < MT; ++c) q[c] = (c == j) ? 1.0 : 0.0;
-    q_groups_up<MT, 0, (MT - 2) / 8>(q, R, taus, M, warp * 4);
-    if (j < M) {
-        double* Q = Q_ + b * M * M;
+        for (int c = 0; c < MT; ++c) q[c] = (c == j) ? 1.0 : 0.0;
+        q_groups_up<MT, 0, (MT - 2) / 8>(q, R, taus, M, warp * 4);
+        if (j < M) {
+            double* Q = Q_ + b * M * M;
 #pragma unroll
-        for (int c = 0; c < MT; ++c)
-            if (c < M) Q[(size_t)c * M + j] = q[c];
-    }
-    }
-}
-
-// Trailing 32 x 32 problem of the split form: pivots min(M-1, 32) ... 1, one warp per matrix.
-__global__ void __maxnreg__(128)
-fast_tridiag_tail(Workspace ws, int M)
-{
-    extern __shared__ __align__(16) double sm[];
-    TriShared sh;
-    sh.R = sm;                                   // groups 0..3: 640 doubles
-    double* small = sm + 640;
-    sh.xs = small; sh.vbuf = small + 32; sh.pbuf = small + 64; sh.pv = small + 96;
-    sh.taus = small + 128;                       // [40]
-    sh.red = small + 168;                        // [8]
-    const int j = threadIdx.x;
-    const size_t b = blockIdx.x;
-    double* sc = reinterpret_cast<double*>(ws.rot + b * ws.logcap);
-    double a[32];
-    {
-        const double2* tr = reinterpret_cast<const double2*>(sc + SPLIT_TR + j * 32);
-#pragma unroll
-        for (int c = 0; c < 32; c += 2) { const double2 t = tr[c >> 1]; a[c] = t.x; a[c + 1] = t.y; }
-    }
-    sh.xs[j] = sc[SPLIT_XS + j];
-    if (j < 8) sh.red[j] = sc[SPLIT_RED + j];
-    __syncwarp();
-    const int Mt = M < 33 ? M : 33;
-    pivot_groups_down<32, 3>(a, sh, Mt, ws.dws + b * M, ws.ews + b * M);
-    __syncwarp();
-    for (int k = j; k < 640; k += 32) sc[k] = sh.R[k];
-    sc[SPLIT_TAUS + j] = (j >= 1) ? sh.taus[j] : 0.0;
-    if (j == 0) sc[SPLIT_TAUS + 32] = sh.taus[32];
-}
-
-// Explicit Q of the split form: CTA 2b + h forms columns 32h ... 32h+31 of matrix b.
-__global__ void __maxnreg__(168)
-fast_formq(double* __restrict__ Q_, Workspace ws, int M)
-{
-    constexpr int MT = 64;
-    extern __shared__ __align__(16) double sm[];
-    double* R = sm;                              // [2304]
-    double* taus = sm + 2304;                    // [64]
-    const int lane = threadIdx.x, h = blockIdx.x & 1;
-    const size_t b = blockIdx.x >> 1;
-    const int j = 32 * h + lane;
-    const double* sc = reinterpret_cast<const double*>(ws.rot + b * ws.logcap);
-    for (int k = (h ? RefLayout<MT>::base(4) : 0) + lane; k < RefLayout<MT>::TOTAL; k += 32) R[k] = sc[k];
-    taus[lane] = sc[SPLIT_TAUS + lane];
-    taus[lane + 32] = sc[SPLIT_TAUS + 32 + lane];
-    __syncwarp();
-    double q[MT];
-#pragma unroll
-    for (int c = 0; c < MT; ++c) q[c] = (c == j) ? 1.0 : 0.0;
-    q_groups_up<MT, 0, (MT - 2) / 8>(q, R, taus, M, 4 * h);
-    if (j < M) {
-        double* Q = Q_ + b * M * M;
-#pragma unroll
-        for (int c = 0; c < MT; ++c)
-            if (c < M) Q[(size_t)c * M + j] = q[c];
+            for (int c = 0; c < MT; ++c)
+                if (c < M) Q[(size_t)c * M + j] = q[c];
+        }
+    } else {
+        __syncthreads();
+        // reflectors (RefLayout order; H_i with i >= M are never read) and taus for the back-transform
+        double* out = ws.refl + b * ws.reflstride;
+        for (int k = j; k < RefLayout<MT>::TOTAL; k += C::NT) out[k] = R[k];
+        out[RefLayout<MT>::TOTAL + j] = (j >= 1 && j <= M - 1) ? taus[j] : 0.0;
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// a5: V = Q Z by replaying the logged rotations; thread r owns row r of Q in registers.
-// Dynamic shared memory: tile[MT*(MT+1)], cs[2][MT] double2, hdr[swcap] u32, inv[MT] int
+// a5: V = Q Z = H_{M-1} ... H_1 Z.  Z is the product of the logged rotations: thread r replays
+// them on row r of the identity held in registers; the matrix is then turned through shared
+// memory so that thread k holds eigenvector k of T, to which it applies the reflectors (q_group:
+// dot product and update inside the thread, reflectors as 16-byte broadcast loads).
+// Dynamic shared memory: A region [ap_a_doubles], reflectors + taus [refl_doubles], hdr[swcap] u32,
+// inv[MT] int (+ the epilogue's arrays, which alias the reflectors once they are applied).
 constexpr int AP_S = 8;      // sweeps staged per barrier round (measured: 2 / 4 / 8 -> 2.05 / 1.99 / 1.93 ms)
-// tile of fast_apply: HT = min(MT, 32) padded rows (the matrix passes through it 32 rows at a time)
-template <int MT> __host__ __device__ constexpr int ap_tile_doubles()
+// A region of fast_apply: the staged rotations [2][AP_S][MT] double2, later the 32 x 33 tiles of
+// the transposition (one per warp) and of the output pass (HT padded rows)
+template <int MT> __host__ __device__ constexpr int ap_a_doubles()
 {
-    constexpr int tile = (MT < 32 ? MT : 32) * (MT + 1), cs = 4 * AP_S * MT;    // the staged rotations alias the tile
-    return ((tile > cs ? tile : cs) + 3) & ~1;
+    constexpr int cs = 4 * AP_S * MT, tr = FastCfg<MT>::NW * 32 * 33, out = (MT < 32 ? MT : 32) * (MT + 1);
+    constexpr int m1 = cs > tr ? cs : tr, m2 = m1 > out ? m1 : out;
+    return (m2 + 1) & ~1;
 }
 // a6-a9 fused into the tail of fast_apply (the analysis call when W is not wanted): V never
 // goes to HBM.  lam = eigenvalues ascending (output order), g = Yb^T (r o d), Eq.14.
@@ -679,18 +624,31 @@ struct EpiArgs {
     double*       wbar;   // [n][M] or NULL
     int           ns;
 };
-constexpr int EPI_QC = 5;          // right-hand sides accumulated per pass over V
 constexpr int EPI_NS_MAX = 15;     // fused epilogue for nstate <= 15, generic_epilogue beyond
-// extra doubles of dynamic shared memory: Bm[MT][ns+1], Tm[ns+1][MT], xbar[ns], cvec[ns]
-template <int MT> size_t fast_epi_smem(int ns)
+// doubles the epilogue needs: Bm[MT][ns+1 padded to even], Tm[ns+1][MT], xbar[ns], cvec[ns], red[NW][ns]; they alias
+// the reflector region, which is enlarged when they do not fit
+template <int MT> __host__ __device__ inline int fast_epi_doubles(int ns)
 {
-    return sizeof(double) * (2 * (size_t)MT * (ns + 1) + 2 * (size_t)ns + 4);
+    return MT * ((ns + 2) & ~1) + MT * (ns + 1) + 2 * ns + FastCfg<MT>::NW * ns + 4;
+}
+// words of the header region of fast_apply: the sweep headers of the replay, or (eigenvector path)
+// ds[MT], es[MT], lam sorted [MT] as doubles and perm [MT] as bytes
+template <int MT> __host__ __device__ inline int ap_hdr_words(int swcap)
+{
+    const int gv = 6 * MT + MT / 4 + 4;
+    return swcap > gv ? swcap : gv;
 }
 
-template <int MT> size_t fast_apply_smem(int swcap)
+template <int MT> __host__ __device__ inline int fast_apply_rd(int epi_ns, bool qform)
 {
-    static_assert(4 * AP_S * MT <= ap_tile_doubles<MT>(), "the staged rotations alias the tile");
-    return sizeof(double) * (size_t)ap_tile_doubles<MT>() + sizeof(uint32_t) * (size_t)swcap + sizeof(int) * MT + 16;
+    int rd = qform ? 0 : refl_doubles<MT>();
+    if (epi_ns > 0 && fast_epi_doubles<MT>(epi_ns) > rd) rd = (fast_epi_doubles<MT>(epi_ns) + 1) & ~1;
+    return rd;
+}
+template <int MT> size_t fast_apply_smem(int swcap, int epi_ns, bool qform)
+{
+    const int rd = fast_apply_rd<MT>(epi_ns, qform);
+    return sizeof(double) * ((size_t)ap_a_doubles<MT>() + rd) + sizeof(uint32_t) * (size_t)ap_hdr_words<MT>(swcap) + sizeof(int) * MT + 16;
 }
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
@@ -735,82 +693,415 @@ __device__ __forceinline__ void apply_sweep(double (&z)[MT], const double2* cs, 
     }
 }
 
-template <int MT, bool EPI>
-__global__ void __launch_bounds__(FastCfg<MT>::NT, (MT == 64) ? 6 : (MT == 48 ? 8 : 16))
-fast_apply(double* __restrict__ V_, Workspace ws, int M, EpiArgs ep)
+// 32 x 32 block moves of the transposition (compile-time register offsets)
+template <int MT, int C0>
+__device__ __forceinline__ void tr_put(const double (&z)[MT], double* T, int lane)
+{
+#pragma unroll
+    for (int c = 0; c < 32; ++c)
+        if (C0 + c < MT) T[lane * 33 + c] = z[C0 + c];
+}
+template <int MT, int R0>
+__device__ __forceinline__ void tr_get(double (&z)[MT], const double* T, int lane)
+{
+#pragma unroll
+    for (int rr = 0; rr < 32; ++rr)
+        if (R0 + rr < MT) z[R0 + rr] = T[rr * 33 + lane];
+}
+// Thread t holds row t of an MT x MT matrix (threads t >= MT: nothing that matters); afterwards
+// thread t holds column t (an involution: the same call turns it back).  One 32 x 33 tile per warp;
+// with two warps the diagonal blocks turn inside their warp and the two off-diagonal blocks swap
+// through both tiles at once, so a thread never holds more than its MT values.
+template <int MT>
+__device__ __forceinline__ void transpose_regs(double (&z)[MT], double* tiles)
+{
+    constexpr int NW = FastCfg<MT>::NW;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double* T = tiles + warp * (32 * 33);
+    if constexpr (NW == 1) {
+        __syncwarp();
+        tr_put<MT, 0>(z, T, lane);
+        __syncwarp();
+        tr_get<MT, 0>(z, T, lane);
+        __syncwarp();
+    } else {
+        static_assert(NW == 2, "at most two warps per matrix");
+        __syncthreads();                                   // the tiles are free
+        if (warp == 0) tr_put<MT, 0>(z, T, lane); else tr_put<MT, 32>(z, T, lane);
+        __syncwarp();
+        if (warp == 0) tr_get<MT, 0>(z, T, lane); else tr_get<MT, 32>(z, T, lane);
+        __syncwarp();
+        // warp 0 hands block (rows 0..31, columns 32..) to warp 1, warp 1 block (rows 32.., columns 0..31) to warp 0
+        if (warp == 0) tr_put<MT, 32>(z, T, lane); else tr_put<MT, 0>(z, T, lane);
+        __syncthreads();
+        const double* O = tiles + (1 - warp) * (32 * 33);
+        if (warp == 0) tr_get<MT, 32>(z, O, lane); else tr_get<MT, 0>(z, O, lane);
+        __syncthreads();
+    }
+}
+
+// 1/x to about an ulp: hardware seed (2^-23) and two Newton steps; x normal, non-zero
+__device__ __forceinline__ double fast_rcp(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double t = fma(-x, y, 1.0);
+    y = fma(y, t, y);
+    t = fma(-x, y, 1.0);
+    return fma(y, t, y);
+}
+
+// Eigenvector of the symmetric tridiagonal T (diagonal ds, off-diagonal es with the negligible
+// entries set to exactly 0, so T is a direct sum of unreduced blocks) for the eigenvalue lam of
+// the block [lo, hi], by the twisted factorisation of T - lam I (Fernando; Parlett & Dhillon: the
+// "getvec" step of MRRR applied to T itself): with the pivots D+ of L D+ L^T from the top and D- of
+// U D- U^T from the bottom, gamma_i = D+_i + D-_i - (d_i - lam) is the one non-zero residual
+// component of the vector that solves the equations twisted at i, so the twist goes where |gamma|
+// is smallest and  z_r = 1,  z_i = -(e_i / D+_i) z_{i+1} (i < r),  z_{i+1} = -(e_i / D-_{i+1}) z_i (i >= r).
+// One thread per eigenvector, everything in registers with compile-time indices (the loops run
+// over all MT indices: outside the block e = 0 restarts the recurrences and zeroes the vector).
+// z doubles as the store of the reciprocal pivots until each entry is final.  Returns the
+// eigenvector, normalised, and its residual norm ||(T - lam) z||_2.
+template <int MT>
+__device__ __forceinline__ double getvec(double (&z)[MT], const double* ds, const double* es, double lam,
+                                         int lo, int hi, double pivmin)
+{
+    // forward pivots: z[i] = 1 / D+_i
+    {
+        double P = ds[0] - lam;
+#pragma unroll
+        for (int i = 0; i < MT; ++i) {
+            P = (fabs(P) < pivmin) ? -pivmin : P;
+            z[i] = fast_rcp(P);
+            if (i + 1 < MT) { const double ei = es[i]; P = fma(-(ei * ei), z[i], ds[i + 1] - lam); }
+            if ((i & 7) == 7) __syncwarp();        // scheduling fence: ptxas does not hoist shared loads across it
+        }
+    }
+    // backward pivots on the fly: the twist index
+    int r = lo;
+    {
+        double best = 1.7976931348623157e308;
+        double Dm = ds[MT - 1] - lam;
+#pragma unroll
+        for (int i = MT - 1; i >= 0; --i) {
+            Dm = (fabs(Dm) < pivmin) ? -pivmin : Dm;
+            const double di = ds[i] - lam;
+            double Pi = di;
+            if (i > 0) { const double el = es[i - 1]; Pi = fma(-(el * el), z[i - 1], di); }
+            Pi = (fabs(Pi) < pivmin) ? -pivmin : Pi;
+            const double gam = fabs(Pi + Dm - di);
+            if (i >= lo && i <= hi && gam < best) { best = gam; r = i; }
+            if (i > 0) { const double el = es[i - 1]; Dm = fma(-(el * el), fast_rcp(Dm), ds[i - 1] - lam); }
+            if ((i & 7) == 0) __syncwarp();
+        }
+    }
+    // from the bottom down to the twist: 1 / D-_i into z[i] (i > r); below the twist the vector itself
+    {
+        double Dm = ds[MT - 1] - lam, zc = 1.0;
+#pragma unroll
+        for (int i = MT - 1; i >= 0; --i) {
+            if (i > r) {
+                Dm = (fabs(Dm) < pivmin) ? -pivmin : Dm;
+                const double rd = fast_rcp(Dm);
+                z[i] = rd;
+                if (i > 0) { const double el = es[i - 1]; Dm = fma(-(el * el), rd, ds[i - 1] - lam); }
+            } else if (i == r) {
+                z[i] = 1.0;
+            } else {
+                zc = -(es[i] * z[i]) * zc;
+                z[i] = zc;
+            }
+            if ((i & 7) == 0) __syncwarp();
+        }
+    }
+    // from the twist up
+    {
+        double zc = 1.0;
+#pragma unroll
+        for (int i = 0; i + 1 < MT; ++i) {
+            if (i >= r) {
+                zc = -(es[i] * z[i + 1]) * zc;
+                z[i + 1] = zc;
+            }
+            if ((i & 7) == 7) __syncwarp();
+        }
+    }
+    double n0 = 0.0, n1 = 0.0;
+#pragma unroll
+    for (int i = 0; i + 1 < MT; i += 2) { n0 = fma(z[i], z[i], n0); n1 = fma(z[i + 1], z[i + 1], n1); }
+    const double sc = rsqrt(n0 + n1);
+    double r0 = 0.0, r1 = 0.0, zm = 0.0;
+#pragma unroll
+    for (int i = 0; i < MT; ++i) {
+        z[i] *= sc;
+        // residual row i - 1 is complete once z[i] is known
+        if (i > 0) {
+            const double up = (i > 1) ? es[i - 2] * zm : 0.0;
+            const double t = fma(ds[i - 1] - lam, z[i - 1], fma(es[i - 1], z[i], up));
+            if (i & 1) r0 = fma(t, t, r0); else r1 = fma(t, t, r1);
+        }
+        if (i > 0) zm = z[i - 1];
+        if ((i & 7) == 7) __syncwarp();
+    }
+    {
+        const double up = (MT > 1) ? es[MT - 2] * z[MT - 2] : 0.0;
+        const double t = fma(ds[MT - 1] - lam, z[MT - 1], up);
+        r0 = fma(t, t, r0);
+    }
+    return sqrt(r0 + r1);
+}
+
+template <int MT, bool EPI, bool QFORM>
+__global__ void __launch_bounds__(FastCfg<MT>::NT, (MT == 64) ? 6 : (MT == 48 ? 7 : 16))
+fast_apply(double* __restrict__ V_, double* __restrict__ w_, int* __restrict__ info_, Workspace ws, int M, EpiArgs ep)
 {
     using C = FastCfg<MT>;
     extern __shared__ __align__(16) double sm[];
-    double*   tile = sm;
-    double2*  cs   = reinterpret_cast<double2*>(sm);   // [2][AP_S][MT], aliases the tile while rotating
-    uint32_t* hdr  = reinterpret_cast<uint32_t*>(sm + ap_tile_doubles<MT>());
-    int*      inv  = reinterpret_cast<int*>(hdr + ws.swcap);
+    double*   areg = sm;                                   // A region
+    double2*  cs   = reinterpret_cast<double2*>(sm);       // [2][AP_S][MT] while rotating
+    double*   R    = sm + ap_a_doubles<MT>();              // reflectors, RefLayout order
+    double*   taus = R + RefLayout<MT>::TOTAL;
+    const int rd = fast_apply_rd<MT>(EPI ? ep.ns : 0, QFORM);
+    uint32_t* hdr  = reinterpret_cast<uint32_t*>(R + rd);
+    int*      inv  = reinterpret_cast<int*>(hdr + ap_hdr_words<MT>(ws.swcap));
     const int r = threadIdx.x;
     const size_t b = blockIdx.x;
-    if (ws.flags[b]) return;                       // finished by generic_apply (slow path)
-    double* V = V_ + b * M * M;
-    const int nsw = ws.nsweeps[b];
+    const int flag = ws.flags[b];
+    const bool direct = !QFORM && flag == FLAG_GETVEC;     // eigenvectors of T by twisted factorisations
+    bool flagged = flag == FLAG_SLOW;                      // rotation log unusable: classic QL below
+    const int nsw = (flag == FLAG_REPLAY) ? ws.nsweeps[b] : 0;
     const double2* rot = ws.rot + b * ws.logcap;
 
     constexpr int HT = MT < 32 ? MT : 32;          // rows per pass through the tile
+    double* tile = areg;
     for (int s = r; s < nsw; s += C::NT) hdr[s] = ws.hdr[b * ws.swcap + s];
-    if (r < M) inv[ws.perm[b * M + r]] = r;        // output column of QL-order column c
+    if (!flagged && r < M) inv[ws.perm[b * M + r]] = r;    // output column of QL-order column c
     double z[MT];
+    if constexpr (!QFORM) {
+        // the reflectors fly in while the eigenvectors of T are formed
+        const double* src = ws.refl + b * ws.reflstride;
+        for (int k = 2 * r; k < refl_doubles<MT>(); k += 2 * C::NT) cp_async16(R + k, src + k);
+    }
+    bool columns = false;                          // z holds a column of Z (an eigenvector of T) rather than a row
+
+    if (direct) {
+        // ---- eigenvectors of T without a single rotation: thread k = position k, its eigenvalue is
+        // w[inv[k]].
+        double*        ds    = reinterpret_cast<double*>(hdr);         // [MT]
+        double*        es    = ds + MT;                                // [MT] negligible entries are exactly 0
+        double*        wsrt  = es + MT;                                // [MT] eigenvalues ascending
+        unsigned char* perm8 = reinterpret_cast<unsigned char*>(wsrt + MT);   // [MT] position of the k-th smallest
+        unsigned*      cutw  = reinterpret_cast<unsigned*>(perm8 + MT);       // [2] bit i: block boundary behind i
+        if (r < MT) {
+            ds[r] = (r < M) ? ws.dws[b * M + r] : 0.0;
+            es[r] = (r < M - 1) ? ws.ews[b * M + r] : 0.0;
+            wsrt[r] = (r < M) ? w_[b * M + r] : 0.0;
+            perm8[r] = (unsigned char)((r < M) ? ws.perm[b * M + r] : r);
+        }
+        __syncthreads();
+        // the threshold and the split of ql_log_kernel, on the same numbers
+        const double eps = 1.1102230246251565e-16;
+        double nrm = 0.0;
+        for (int i = 0; i < M; ++i) nrm = fmax(nrm, fabs(ds[i]) + (i < M - 1 ? fabs(es[i]) : 0.0));
+        const double thr = eps * nrm;
+        bool cut = true;
+        if (r < M - 1) cut = fabs(es[r]) <= fmax(eps * (fabs(ds[r]) + fabs(ds[r + 1])), thr);
+        __syncthreads();
+        if (r < MT && cut) es[r] = 0.0;
+        const unsigned cw = __ballot_sync(0xffffffffu, cut);
+        if ((r & 31) == 0) cutw[r >> 5] = cw;
+        __syncthreads();
+        int lo = 0, hi = M - 1;
+        double lam = 0.0;
+        if (r < M) {
+            const unsigned long long cuts = (C::NW > 1) ? ((unsigned long long)cutw[1] << 32 | cutw[0]) : (unsigned long long)cutw[0];
+            const unsigned long long below = cuts & ((1ull << r) - 1ull);        // boundaries behind indices < r
+            lo = below ? 64 - __clzll((long long)below) : 0;
+            const unsigned long long above = cuts >> r;                          // bit 0: boundary behind r
+            hi = above ? r + __ffsll((long long)above) - 1 : M - 1;
+            if (hi > M - 1) hi = M - 1;
+            lam = wsrt[inv[r]];
+        }
+        // (every thread runs it -- the fences inside want whole warps; a 1 x 1 block gets its unit vector)
+        const bool own = r < M && lo < hi;
+        double res = getvec<MT>(z, ds, es, lam, lo, hi, fmax(thr * eps, 1e-300));
+        if (!own) {
+            res = 0.0;
 #pragma unroll
-    for (int c = 0; c < MT; ++c) z[c] = 0.0;
-#pragma unroll
-    for (int r0 = 0; r0 < MT; r0 += HT) {
-        if (r0 < M) {
-            load_rows<MT>(tile, V, M, r0, min(HT, M - r0));
-            __syncthreads();
-            if (r >= r0 && r < r0 + HT && r < M) {
-#pragma unroll
-                for (int c = 0; c < MT; ++c) z[c] = (c < M) ? tile[(r - r0) * C::LDT + c] : 0.0;
+            for (int c = 0; c < MT; ++c) z[c] = (c == r) ? 1.0 : 0.0;
+        }
+        // anything suspicious hands the matrix to the classic iteration below
+        const bool bad = !(res <= 64.0 * eps * nrm * sqrt((double)M));
+        if (__syncthreads_or(bad ? 1 : 0)) {
+            flagged = true;
+        } else {
+            columns = true;
+            // eigenvalues closer than GV_GAP ||T|| inside a block: first-order symmetric orthogonalisation,
+            // z_k -= 1/2 (z_q . z_k) z_q for every such partner q (the classifier bounds their number);
+            // the vectors pass through shared memory 32 at a time
+            const double gapabs = GV_GAP * nrm;
+            unsigned long long plist = 0ull;
+            int np = 0;
+            if (own) {
+                const int s0 = inv[r];
+                for (int t = 1; t <= GV_PH && s0 - t >= 0 && lam - wsrt[s0 - t] < gapabs; ++t) {
+                    const int q = perm8[s0 - t];
+                    if (q >= lo && q <= hi) { plist |= (unsigned long long)q << (8 * np); ++np; }
+                }
+                for (int t = 1; t <= GV_PH && s0 + t < M && wsrt[s0 + t] - lam < gapabs; ++t) {
+                    const int q = perm8[s0 + t];
+                    if (q >= lo && q <= hi) { plist |= (unsigned long long)q << (8 * np); ++np; }
+                }
             }
+            if (__syncthreads_or(np)) {
+                constexpr int LDV = MT + 1;
+                const int npw = __reduce_max_sync(0xffffffffu, np);             // whole warps walk the longest list
+#pragma unroll 1
+                for (int ph = 0; ph < C::NW; ++ph) {
+                    if (ph) __syncthreads();
+                    if ((r >> 5) == ph) {
+#pragma unroll
+                        for (int i = 0; i < MT; ++i) areg[(r & 31) * LDV + i] = z[i];
+                    }
+                    __syncthreads();
+#pragma unroll 1
+                    for (int t = 0; t < npw; ++t) {
+                        const int q = (int)((plist >> (8 * t)) & 255ull);
+                        const bool act = t < np && (q >> 5) == ph;
+                        const double* vq = areg + (act ? (q & 31) : 0) * LDV;
+                        double d0 = 0.0, d1 = 0.0;
+#pragma unroll
+                        for (int i = 0; i + 1 < MT; i += 2) {
+                            d0 = fma(z[i], vq[i], d0); d1 = fma(z[i + 1], vq[i + 1], d1);
+                            if ((i & 7) == 6) __syncwarp();
+                        }
+                        const double h = act ? -0.5 * (d0 + d1) : 0.0;
+#pragma unroll
+                        for (int i = 0; i < MT; ++i) {
+                            z[i] = fma(h, vq[i], z[i]);
+                            if ((i & 7) == 7) __syncwarp();
+                        }
+                    }
+                }
+            }
+            cp_async_wait_all();
+            __syncthreads();
+        }
+    } else if (!flagged) {
+        if constexpr (QFORM) {
+            // row r of Q (stored by fast_tridiag in the output buffer) through the tile, HT rows per pass
+            const double* Q = V_ + b * M * M;
+#pragma unroll
+            for (int c = 0; c < MT; ++c) z[c] = 0.0;
+#pragma unroll
+            for (int r0 = 0; r0 < MT; r0 += HT) {
+                if (r0 < M) {
+                    load_rows<MT>(tile, Q, M, r0, min(HT, M - r0));
+                    __syncthreads();
+                    if (r >= r0 && r < r0 + HT && r < M) {
+#pragma unroll
+                        for (int c = 0; c < MT; ++c) z[c] = (c < M) ? tile[(r - r0) * C::LDT + c] : 0.0;
+                    }
+                    __syncthreads();
+                }
+            }
+        } else {
+#pragma unroll
+            for (int c = 0; c < MT; ++c) z[c] = (c == r) ? 1.0 : 0.0;
+            __syncthreads();
+        }
+        // The (c, s) of AP_S sweeps are staged per barrier round, double-buffered: thread r copies the
+        // rotation that acts on columns (r, r+1) of each sweep straight from the log into shared
+        // memory (cp.async, no registers), identity outside [lo, m); the copies of round k+1 fly
+        // while round k is applied.
+        int spos = 0;                                   // log position of the next sweep to stage
+        auto stage = [&](int round) {
+            double2* dst = cs + (round & 1) * AP_S * MT;
+#pragma unroll
+            for (int t = 0; t < AP_S; ++t) {
+                const int s = round * AP_S + t;
+                if (s < nsw) {
+                    const uint32_t h = hdr[s];
+                    const int lo = h & 0xffff, m = h >> 16;
+                    if (r < MT) {
+                        if (r >= lo && r < m) cp_async16(dst + t * MT + r, rot + spos + (m - 1 - r));
+                        else dst[t * MT + r] = make_double2(1.0, 0.0);
+                    }
+                    spos += m - lo;
+                }
+            }
+        };
+        const int nrounds = (nsw + AP_S - 1) / AP_S;
+        if (nrounds > 0) stage(0);
+        cp_async_wait_all();
+        __syncthreads();
+        for (int k = 0; k < nrounds; ++k) {
+            if (k + 1 < nrounds) stage(k + 1);
+            const double2* cur = cs + (k & 1) * AP_S * MT;
+            const int send = min(nsw, (k + 1) * AP_S);
+#pragma unroll 1
+            for (int s = k * AP_S; s < send; ++s) {
+                const uint32_t h = hdr[s];
+                apply_sweep<MT>(z, cur + (s - k * AP_S) * MT, h & 0xffff, h >> 16);
+            }
+            cp_async_wait_all();
             __syncthreads();
         }
     }
-
-    // The (c, s) of AP_S sweeps are staged per barrier round, double-buffered: thread r copies the
-    // rotation that acts on columns (r, r+1) of each sweep straight from the log into shared
-    // memory (cp.async, no registers), identity outside [lo, m); the copies of round k+1 fly
-    // while round k is applied.
-    int spos = 0;                                   // log position of the next sweep to stage
-    auto stage = [&](int round) {
-        double2* dst = cs + (round & 1) * AP_S * MT;
+    if (flagged) {
+        // Slow path (LETKF_INFO_SLOWPATH): the classic iteration, one sweep at a time -- thread 0 runs
+        // the recurrences of ql_next_sweep (which treats underflow, overflow and NaN case by case) on
+        // the tridiagonal form the reduction left, all threads apply the sweep to their rows.
+        double*  dsm  = areg;                                        // [MT]
+        double*  esm  = areg + MT;                                   // [MT]
+        double2* sink = reinterpret_cast<double2*>(areg + 2 * MT);   // [MT] in generation order
+        double2* csb  = sink + MT;                                   // [MT] by column, identity outside [lo, m)
+        int*     ctl  = reinterpret_cast<int*>(csb + MT);            // rc, lo, m, fail
+        __syncthreads();
+        if constexpr (QFORM) {
+            const double* Q = V_ + b * M * M;                        // row r of Q straight from global memory
 #pragma unroll
-        for (int t = 0; t < AP_S; ++t) {
-            const int s = round * AP_S + t;
-            if (s < nsw) {
-                const uint32_t h = hdr[s];
-                const int lo = h & 0xffff, m = h >> 16;
-                if (r < MT) {
-                    if (r >= lo && r < m) cp_async16(dst + t * MT + r, rot + spos + (m - 1 - r));
-                    else dst[t * MT + r] = make_double2(1.0, 0.0);
-                }
-                spos += m - lo;
+            for (int c = 0; c < MT; ++c) z[c] = (r < M && c < M) ? Q[(size_t)r * M + c] : 0.0;
+        } else {
+#pragma unroll
+            for (int c = 0; c < MT; ++c) z[c] = (c == r) ? 1.0 : 0.0;
+        }
+        if (r < M) { dsm[r] = ws.dws[b * M + r]; esm[r] = ws.ews[b * M + r]; }
+        __syncthreads();
+        QLState st{0, 0, 0, 0.0};
+        if (r == 0) { esm[M - 1] = 0.0; st.thr = ql_threshold(dsm, esm, 1, M); }
+        for (;;) {
+            if (r == 0) {
+                int lo = 0, m = 0;
+                ctl[0] = ql_next_sweep(st, dsm, esm, 1, M, sink, M, lo, m);
+                ctl[1] = lo; ctl[2] = m;
             }
+            __syncthreads();
+            if (ctl[0] != 1) break;
+            const int lo = ctl[1], m = ctl[2];
+            if (r < MT) csb[r] = (r >= lo && r < m) ? sink[m - 1 - r] : make_double2(1.0, 0.0);
+            __syncthreads();
+            apply_sweep<MT>(z, csb, lo, m);
+            __syncthreads();
         }
-    };
-    const int nrounds = (nsw + AP_S - 1) / AP_S;
-    if (nrounds > 0) stage(0);                      // every row has left the tile: it now holds cs
-    cp_async_wait_all();
-    __syncthreads();
-    for (int k = 0; k < nrounds; ++k) {
-        if (k + 1 < nrounds) stage(k + 1);
-        const double2* cur = cs + (k & 1) * AP_S * MT;
-        const int send = min(nsw, (k + 1) * AP_S);
-#pragma unroll 1
-        for (int s = k * AP_S; s < send; ++s) {
-            const uint32_t h = hdr[s];
-            apply_sweep<MT>(z, cur + (s - k * AP_S) * MT, h & 0xffff, h >> 16);
-        }
+        int* permsm = reinterpret_cast<int*>(sink);                  // the sink is free now
+        if (r == 0) { sort_eigenvalues(dsm, 1, permsm, 1, M); ctl[3] = st.fail; }
+        __syncthreads();
+        if (r < M) { inv[permsm[r]] = r; w_[b * M + r] = dsm[r]; }
+        if (r == 0 && info_) info_[b] = ctl[3] | 0x40000000;
         cp_async_wait_all();
         __syncthreads();
     }
 
-    if constexpr (!EPI) {
-        // sorted, row-major V through the tile, HT rows per pass
+    if constexpr (!QFORM) {
+        // rows of Z -> eigenvectors of T: thread k holds column k (QL order); then V = H_{M-1} ... H_1 Z
+        if (!columns) transpose_regs<MT>(z, areg);
+        q_groups_up<MT, 0, (MT - 2) / 8>(z, R, taus, M, 0);
+    }
+
+    if constexpr (!EPI && QFORM) {
+        // sorted, row-major V through the tile, HT rows per pass (thread r holds row r)
+        double* V = V_ + b * M * M;
 #pragma unroll
         for (int r0 = 0; r0 < MT; r0 += HT) {
             if (r0 < M) {
@@ -828,20 +1119,44 @@ fast_apply(double* __restrict__ V_, Workspace ws, int M, EpiArgs ep)
                 __syncthreads();
             }
         }
+    } else if constexpr (!EPI) {
+        // sorted, row-major V through the tile, HT rows per pass: thread k scatters its column into
+        // output column inv[k], thread t then writes column t of every row (coalesced)
+        double* V = V_ + b * M * M;
+        const int oc = (r < M) ? inv[r] : 0;
+#pragma unroll
+        for (int r0 = 0; r0 < MT; r0 += HT) {
+            if (r0 < M) {
+                __syncthreads();
+                if (r < M) {
+#pragma unroll
+                    for (int rr = 0; rr < HT; ++rr)
+                        if (r0 + rr < MT) tile[rr * C::LDT + oc] = z[r0 + rr];
+                }
+                __syncthreads();
+                if (r < M) {
+                    const int nr = min(HT, M - r0);
+#pragma unroll 8
+                    for (int rr = 0; rr < nr; ++rr) V[(size_t)(r0 + rr) * M + r] = tile[rr * C::LDT + r];
+                }
+            }
+        }
     } else {
-        // ---- a6-a9 on the V held in registers (row r of V in QL column order; the order of the
-        // columns is irrelevant to sums over k as long as lam_k follows it: lam_k = lam[inv[k]]).
-        //   T[q][k] = sum_r V[r][k] B[r][q],  B = [g | dX^T]               (reduction over rows:
-        //             through the tile, thread k owns column k)
+        if constexpr (QFORM) transpose_regs<MT>(z, areg);                    // rows of V -> eigenvectors
+        // ---- a6-a9 on the V held in registers (thread k = eigenvector k in QL order, its eigenvalue
+        // lam_k = lam[inv[k]]; sums over k do not care about the order).
+        //   T[q][k] = sum_r V[r][k] B[r][q],  B = [g | dX^T]     (inside the thread)
         //   t'_k = T[0][k]/lam_k,  U'[s][k] = sqrt(M-1) T[1+s][k]/sqrt(lam_k)
-        //   c_s = sum_k T[1+s][k] t'_k  (= dX_s . wbar),  wbar_m = sum_k V[m][k] t'_k
-        //   Xa[s][m] = xbar_s + c_s + sum_k U'[s][k] V[m][k]                 (thread m owns row m)
-        const int ns = ep.ns, nq = ns + 1;
-        double* Bm   = reinterpret_cast<double*>(                            // [MT][nq], 16-byte aligned
-            (reinterpret_cast<uintptr_t>(inv + MT) + 15) & ~static_cast<uintptr_t>(15));
-        double* Tm   = Bm + (size_t)MT * nq;                                // [nq][MT]
+        //   c_s = sum_k T[1+s][k] t'_k  (= dX_s . wbar)
+        // then the matrix is turned back (thread m = row m of V) for
+        //   wbar_m = sum_k V[m][k] t'_k,   Xa[s][m] = xbar_s + c_s + sum_k U'[s][k] V[m][k]
+        const int ns = ep.ns, nq = ns + 1, nqp = (nq + 1) & ~1;             // rows of Bm padded to whole pairs
+        __syncthreads();                                                    // the reflectors are dead
+        double* Bm   = R;                                                   // [MT][nqp]
+        double* Tm   = Bm + (size_t)MT * nqp;                               // [nq][MT]
         double* xbar = Tm + (size_t)MT * nq;                                // [ns]
         double* cvec = xbar + ns;                                           // [ns]
+        double* cred = cvec + ns;                                           // [NW][ns]
         const double* Xb = ep.Xb + b * (size_t)ns * M;
         const int lane = r & 31, warp = r >> 5;
         for (int s = warp; s < ns; s += C::NW) {                            // Eq.9-11
@@ -849,65 +1164,50 @@ fast_apply(double* __restrict__ V_, Workspace ws, int M, EpiArgs ep)
             for (int m = lane; m < M; m += 32) acc += Xb[(size_t)s * M + m];
             acc = warp_sum(acc) / (double)M;
             if (lane == 0) xbar[s] = acc;
-            for (int m = lane; m < MT; m += 32) Bm[m * nq + 1 + s] = (m < M) ? Xb[(size_t)s * M + m] - acc : 0.0;
+            for (int m = lane; m < MT; m += 32) Bm[m * nqp + 1 + s] = (m < M) ? Xb[(size_t)s * M + m] - acc : 0.0;
         }
-        if (r < MT) Bm[r * nq] = (r < M) ? ep.g[b * M + r] : 0.0;
-        const double lamk = (r < M) ? ep.lam[b * M + inv[r]] : 1.0;
-        for (int q0 = 0; q0 < nq; q0 += EPI_QC) {
-            double acc[EPI_QC];
-#pragma unroll
-            for (int u = 0; u < EPI_QC; ++u) acc[u] = 0.0;
-#pragma unroll
-            for (int r0 = 0; r0 < MT; r0 += HT) {
-                if (r0 < M) {
-                    __syncthreads();                                        // tile free, Bm visible
-                    if (r >= r0 && r < r0 + HT) {
-#pragma unroll
-                        for (int c = 0; c < MT; ++c) tile[(r - r0) * C::LDT + c] = z[c];
-                    }
-                    __syncthreads();
-                    if (r < MT) {
-                        const int nr = min(HT, M - r0);
-                        for (int rr = 0; rr < nr; ++rr) {
-                            const double v = tile[rr * C::LDT + r];
-                            const double* brow = Bm + (r0 + rr) * nq + q0;
-#pragma unroll
-                            for (int u = 0; u < EPI_QC; ++u)
-                                if (q0 + u < nq) acc[u] = fma(v, brow[u], acc[u]);
-                        }
-                    }
-                }
-            }
-            if (r < MT) {
-#pragma unroll
-                for (int u = 0; u < EPI_QC; ++u)
-                    if (q0 + u < nq) Tm[(q0 + u) * MT + r] = acc[u];            // raw T[q][k]
-            }
-        }
-        __syncthreads();
-        // c_s = sum_k T[1+s][k] T[0][k] / lam_k : thread s sums its row (four partial sums)
-        const double tk = (r < M) ? Tm[r] / lamk : 0.0;
-        const double sk = (r < M) ? sqrt((double)(M - 1)) * rsqrt(lamk) : 0.0;
-        __syncthreads();
         if (r < MT) {
-            Tm[r] = tk;                                                     // t'_k
-            // products for c_s go to the tile (free again), scaled rows stay in Tm
-            for (int s = 0; s < ns; ++s) {
-                const double raw = Tm[(1 + s) * MT + r];
-                tile[s * C::LDT + r] = raw * tk;
-                Tm[(1 + s) * MT + r] = raw * sk;                            // U'[s][k]
+            Bm[r * nqp] = (r < M) ? ep.g[b * M + r] : 0.0;
+            if (nqp > nq) Bm[r * nqp + nq] = 0.0;
+        }
+        const double lamk = (r < M) ? ep.lam[b * M + inv[r]] : 1.0;
+        __syncthreads();
+        const double tk_scale = (r < M) ? 1.0 / lamk : 0.0;
+        const double sk = (r < M) ? sqrt((double)(M - 1)) * rsqrt(lamk) : 0.0;
+        double tk = 0.0;
+        const double2* Bm2 = reinterpret_cast<const double2*>(Bm);
+        const int nqh = nqp >> 1;
+        for (int q = 0; q < nqp; q += 2) {                                  // two right-hand sides per pass over z
+            double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
+            const double2* bq = Bm2 + (q >> 1);
+#pragma unroll
+            for (int c = 0; c + 1 < MT; c += 2) {
+                const double2 t0 = bq[c * nqh], t1 = bq[(c + 1) * nqh];
+                a0 = fma(z[c], t0.x, a0);     b0 = fma(z[c], t0.y, b0);
+                a1 = fma(z[c + 1], t1.x, a1); b1 = fma(z[c + 1], t1.y, b1);
+            }
+            const double raw[2] = {a0 + a1, b0 + b1};
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int qq = q + u;
+                if (qq == 0) {
+                    tk = raw[u] * tk_scale;
+                    if (r < MT) Tm[r] = tk;                                 // t'_k
+                } else if (qq < nq) {
+                    if (r < MT) Tm[qq * MT + r] = raw[u] * sk;              // U'[s][k]
+                    const double part = warp_sum((r < M) ? raw[u] * tk : 0.0);   // c_s, this warp's share
+                    if (lane == 0) cred[warp * ns + (qq - 1)] = part;
+                }
             }
         }
         __syncthreads();
         if (r < ns) {
-            double c0 = 0.0, c1 = 0.0, c2 = 0.0, c3 = 0.0;
-            for (int k = 0; k + 3 < MT; k += 4) {
-                c0 += tile[r * C::LDT + k];     c1 += tile[r * C::LDT + k + 1];
-                c2 += tile[r * C::LDT + k + 2]; c3 += tile[r * C::LDT + k + 3];
-            }
-            cvec[r] = (c0 + c1) + (c2 + c3);
+            double c = 0.0;
+#pragma unroll
+            for (int w = 0; w < C::NW; ++w) c += cred[w * ns + r];
+            cvec[r] = c;
         }
-        __syncthreads();
+        transpose_regs<MT>(z, areg);                                        // (its barriers publish Tm, cvec)
         if (r < M) {
             double* Xa = ep.Xa + b * (size_t)ns * M;
             if (ep.wbar) {
@@ -938,5 +1238,14 @@ fast_apply(double* __restrict__ V_, Workspace ws, int M, EpiArgs ep)
 
 static inline bool fast_supported(int M) { return M >= 2 && M <= 64; }
 static inline int fast_bucket(int M) { return M <= 16 ? 16 : (M <= 32 ? 32 : (M <= 48 ? 48 : 64)); }
+static inline int fast_refl_doubles(int M)
+{
+    switch (fast_bucket(M)) {
+        case 16: return refl_doubles<16>();
+        case 32: return refl_doubles<32>();
+        case 48: return refl_doubles<48>();
+        default: return refl_doubles<64>();
+    }
+}
 
 }  // namespace letkf

@@ -6,6 +6,7 @@
 #include <stdint.h>
 #include <stdio.h>
 #include <string.h>
+#include <mutex>
 #include <vector>
 
 #include "common.cuh"
@@ -69,55 +70,73 @@ static void prof_end(cudaStream_t st)
 
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-// bytes of workspace one matrix needs on the syev path
-static size_t syev_bytes_per_matrix(int M)
-{
-    size_t s = 0;
-    s += 2 * sizeof(double) * (size_t)M;                 // dws, ews
-    s += sizeof(int) * (size_t)M;                        // perm
-    s += 2 * sizeof(int);                                // nsweeps, flags
-    s += sizeof(uint32_t) * (size_t)sweep_capacity(M);   // hdr
-    s += sizeof(double2) * (size_t)log_capacity(M);      // rot
-    return s;
-}
+// ---- options (letkf_set_option) ------------------------------------------------------------------
+// Process-wide settings, written under a mutex.  Every entry point takes ONE snapshot into the
+// calling thread's copy when it starts and reads nothing else, so a letkf_set_option from another
+// host thread can never change the layout or the kernel choice in the middle of a call.
+struct Options {
+    int force_generic = 0;   // 1: every M through the any-M kernels (tests)
+    int pipeline = 1;        // 0: one chunk at a time on the caller's stream
+    int sub_chunk = 0;       // matrices per sub-chunk of the pipeline (0 = by size)
+    int slots = 0;           // sub-chunks in flight = workspace slots (0 = default)
+    int log_slots = 0;       // of which as many may be between the start of their QL and the end of their apply
+                             // kernel (slots of the rotation log, the large part of a slot; 0 = default)
+    int mid_reg = 1;         // 64 < M <= 160 reduced in shared memory (0) / registers up to M = 128 (1) / registers (2)
+    int log_shrink = 1;      // divides the rotation-log capacity (tests force the slow path)
+    int ql_tpb = 0;          // matrices per QL CTA (0 = by size)
+    int two_pass = -1;       // QL with a second, perfectly shifted pass: -1 = by batch size, 0 / 1
+    int host_pass = 0;       // matrices per pass of the host entry points (0 = by arena size; tests)
+    int qform = 0;           // M <= 64: 1 = explicit Q formed by the reduction kernel and replayed on (through the
+                             // output buffer); 0 = reflectors kept, eigenvectors of T formed in the apply kernel,
+                             // which then does the back-transform (nothing but the reflectors crosses HBM in between)
+    int evec = 1;            // M <= 64, qform = 0: 1 = eigenvectors of T by twisted factorisations where the spectrum
+                             // allows (ql_log_kernel classifies), the logged rotations otherwise; 0 = always the log
+};
+static Options g_options;
+static std::mutex g_options_mu;
+static thread_local Options t_opt;
+static thread_local int t_depth = 0;
+struct EntryScope {                      // first thing every entry point constructs
+    EntryScope()
+    {
+        if (t_depth++ == 0) { std::lock_guard<std::mutex> lk(g_options_mu); t_opt = g_options; }
+    }
+    ~EntryScope() { --t_depth; }
+};
 
-// matrices processed per pass.  The workspace (dominated by the rotation log, 16*log_capacity(M)
-// bytes per matrix) is sized for the whole batch up to WORK_CAP: ql_log_kernel costs the serial
-// latency of one matrix's QL iteration whatever the batch (profiles/r01a), so passes are kept as
-// few as the 180 GB of HBM allow.
-static const size_t WORK_CAP = (size_t)8 << 30;
-static int syev_chunk(int M, int batch)
-{
-    const size_t per = syev_bytes_per_matrix(M);
-    size_t c = WORK_CAP / per;
-    if (c < 1024) c = 1024;
-    if (c > (size_t)batch) c = (size_t)batch;
-    if (c < 1) c = 1;
-    return (int)c;
-}
+// ---- workspace -------------------------------------------------------------------------------------
+// The workspace holds `nslot` slots of `per` matrices each; sub-chunk k of a call lives in slot
+// k mod nslot for as long as its three kernels are in flight (Streams).  The
+// rotation log (with its sweep headers: 72 of the 93 KB a matrix of order 64 needs) is only touched
+// from the QL kernel on, so it has slots of its own, `nlog` <= nslot of them: the reductions may run
+// ahead of the eigensolver without holding log space.
+static bool use_fast(int M) { return fast_supported(M) && !t_opt.force_generic; }
+static bool use_mid(int M) { return mid_supported(M) && !t_opt.force_generic; }
+static bool use_getvec(int M) { return use_fast(M) && !t_opt.qform && t_opt.evec; }
 
-static int g_log_shrink = 1;             // letkf_set_option("log_shrink", k): tests force the slow path
-
-static size_t carve(Workspace& ws, void* base, int M, int chunk)
+static size_t carve(Workspace& ws, void* base, int M, int nmat, int nlogmat, bool two_pass)
 {
     char* p = reinterpret_cast<char*>(base);
     size_t off = 0;
     auto take = [&](size_t bytes) { char* q = p ? p + off : nullptr; off = align_up(off + bytes, 256); return q; };
     ws.swcap = sweep_capacity(M);
-    ws.logcap = log_capacity(M) / g_log_shrink;       // (the memory is still sized for the full log)
+    ws.logcap = log_capacity(M, two_pass) / t_opt.log_shrink;      // (the memory is still sized for the full log)
+    ws.reflstride = (use_fast(M) && !t_opt.qform) ? fast_refl_doubles(M) : 0;
     ws.rot_counter = g_prof.on ? g_prof.d_rot : nullptr;
-    ws.dws     = reinterpret_cast<double*>(take(sizeof(double) * (size_t)M * chunk));
-    ws.ews     = reinterpret_cast<double*>(take(sizeof(double) * (size_t)M * chunk));
-    ws.perm    = reinterpret_cast<int*>(take(sizeof(int) * (size_t)M * chunk));
-    ws.nsweeps = reinterpret_cast<int*>(take(sizeof(int) * (size_t)chunk));
-    ws.flags   = reinterpret_cast<int*>(take(sizeof(int) * (size_t)chunk));
-    ws.hdr     = reinterpret_cast<uint32_t*>(take(sizeof(uint32_t) * (size_t)ws.swcap * chunk));
-    ws.rot     = reinterpret_cast<double2*>(take(sizeof(double2) * (size_t)ws.logcap * chunk));
+    ws.dws     = reinterpret_cast<double*>(take(sizeof(double) * (size_t)M * nmat));
+    ws.ews     = reinterpret_cast<double*>(take(sizeof(double) * (size_t)M * nmat));
+    ws.perm    = reinterpret_cast<int*>(take(sizeof(int) * (size_t)M * nmat));
+    ws.nsweeps = reinterpret_cast<int*>(take(sizeof(int) * (size_t)nmat));
+    ws.flags   = reinterpret_cast<int*>(take(sizeof(int) * (size_t)nmat));
+    ws.hdr     = reinterpret_cast<uint32_t*>(take(sizeof(uint32_t) * (size_t)ws.swcap * nlogmat));
+    ws.rot     = reinterpret_cast<double2*>(take(sizeof(double2) * (size_t)log_capacity(M, two_pass) * nlogmat));
+    ws.refl    = reinterpret_cast<double*>(take(sizeof(double) * (size_t)ws.reflstride * nmat));
+    ws.s1      = reinterpret_cast<double*>(take(use_getvec(M) ? sizeof(double) * (size_t)M * nmat : 0));
     return off;
 }
 
-// the records of matrices b0 ... of a carved workspace
-static Workspace ws_slice(const Workspace& w, int M, int b0)
+// the records of a sub-chunk: matrices b0 ... of the small arrays, l0 ... of the log arrays
+static Workspace ws_slice(const Workspace& w, int M, int b0, int l0)
 {
     Workspace s = w;
     s.dws += (size_t)b0 * M;
@@ -125,19 +144,75 @@ static Workspace ws_slice(const Workspace& w, int M, int b0)
     s.perm += (size_t)b0 * M;
     s.nsweeps += b0;
     s.flags += b0;
-    s.hdr += (size_t)b0 * w.swcap;
-    s.rot += (size_t)b0 * w.logcap;
+    s.hdr += (size_t)l0 * w.swcap;
+    s.rot += (size_t)l0 * w.logcap;
+    s.refl += (size_t)b0 * w.reflstride;
+    if (s.s1) s.s1 += (size_t)b0 * M;
     return s;
 }
 
-static inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+// How a call over `batch` matrices is cut up.  Pipelined: nsub sub-chunks of `per` matrices flow
+// tridiag -> QL -> apply over private streams, at most `nslot` of them in flight (a slot of the
+// workspace each).  Not pipelined (small batches, pipeline = 0, kernel-alone profiling): chunks of
+// `per` matrices one after the other on the caller's stream.
+struct Plan { int per, nslot, nlog, nsub; bool pipelined, two_pass; int ql_mode; };
+static const int PIPE_MIN_SUB = 512;     // smallest sub-chunk worth launches of its own
+static const int PIPE_MAX_SUBS = 16;     // sub-chunks per call (bounds the launch count)
+static const int PIPE_SLOTS = 16;        // default number of sub-chunks in flight: all of them
+static const int PIPE_LOG_MATS = 4096;   // default number of matrices that hold a slot of the rotation log
+static const int NQ_STREAMS = 16;
 
-#define LAUNCH_CHECK()                                         \
-    do {                                                       \
-        cudaError_t e_ = cudaGetLastError();                   \
-        if (e_ != cudaSuccess) return (int)e_;                 \
-        ++g_launches;                                          \
-    } while (0)
+static int round_up(int x, int a) { return (x + a - 1) / a * a; }
+
+// bytes of a workspace for nmat matrices in flight (the one formula every size query and every check uses)
+static size_t plan_bytes(int M, size_t nmat, size_t nlogmat, size_t extra, bool two_pass)
+{
+    Workspace tmp;
+    return carve(tmp, nullptr, M, (int)nmat, (int)nlogmat, two_pass) + nmat * extra + 6 * 256;
+}
+
+// extra: bytes per matrix the caller keeps per slot beside the EVD workspace (analysis: Q/V, lam, g, gathered Y_loc);
+// avail: bytes of the workspace at hand (0: plan for the recommended size)
+static Plan make_plan(int M, int batch, size_t extra, size_t avail)
+{
+    Plan pl;
+    pl.two_pass = t_opt.two_pass >= 0 ? t_opt.two_pass != 0 : ((long)batch * M >= (1L << 18));
+    pl.ql_mode = pl.two_pass ? QL_TWO_PASS : QL_ONE_PASS;
+    if (use_getvec(M)) { pl.ql_mode = QL_CLASSIFY; pl.two_pass = true; }   // (a logged pass is always the second one)
+    const bool want_pipe = t_opt.pipeline && (!g_prof.on || g_prof.keep_pipeline) && batch >= 2 * PIPE_MIN_SUB;
+    auto bytes_for = [&](size_t n, size_t nl) { return plan_bytes(M, n, nl, extra, pl.two_pass); };
+    if (want_pipe) {
+        int per = t_opt.sub_chunk > 0 ? t_opt.sub_chunk : round_up((batch + PIPE_MAX_SUBS - 1) / PIPE_MAX_SUBS, 64);
+        if (per < PIPE_MIN_SUB && t_opt.sub_chunk <= 0) per = PIPE_MIN_SUB;
+        if (per > batch) per = batch;
+        int nsub = (batch + per - 1) / per;
+        int nslot = t_opt.slots > 0 ? t_opt.slots : PIPE_SLOTS;
+        if (nslot > nsub) nslot = nsub;
+        int nlog = t_opt.log_slots > 0 ? t_opt.log_slots : (PIPE_LOG_MATS + per - 1) / per;
+        if (nlog < 2) nlog = 2;
+        if (nlog > nslot) nlog = nslot;
+        if (avail) {                       // a smaller workspace: fewer log slots first, then fewer slots
+            while (nlog > 2 && bytes_for((size_t)per * nslot, (size_t)per * nlog) > avail) --nlog;
+            while (nslot > 2 && bytes_for((size_t)per * nslot, (size_t)per * nlog) > avail) { --nslot; if (nlog > nslot) nlog = nslot; }
+        }
+        if (nslot >= 2 && (!avail || bytes_for((size_t)per * nslot, (size_t)per * nlog) <= avail)) {
+            pl.per = per; pl.nslot = nslot; pl.nlog = nlog; pl.nsub = nsub; pl.pipelined = true;
+            return pl;
+        }
+    }
+    // sequential chunks: as large as the workspace allows (recommended: what the pipeline would take)
+    int per = batch;
+    if (avail) {
+        while (per > 1 && bytes_for((size_t)per, (size_t)per) > avail) per = (per + 1) / 2;
+    } else {
+        const int cap = round_up((batch + PIPE_MAX_SUBS - 1) / PIPE_MAX_SUBS, 64) * 4;
+        if (per > cap && cap >= 2 * PIPE_MIN_SUB) per = cap;
+    }
+    pl.per = per; pl.nslot = 1; pl.nlog = 1; pl.nsub = (batch + per - 1) / per; pl.pipelined = false;
+    return pl;
+}
+
+static inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 
 template <typename K>
 static cudaError_t allow_smem(K kernel, size_t bytes)
@@ -147,83 +222,66 @@ static cudaError_t allow_smem(K kernel, size_t bytes)
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
-static int g_mid_reg = 1;                // letkf_set_option("mid_reg", 0 / 1 / 2): 64 < M <= 160 reduced in shared memory / registers up to M = 128 / registers
-static bool g_force_generic = false;     // letkf_set_option("force_generic", 1): tests only
-
 // a1/a2 inputs when the matrix is to be formed from the LETKF observations instead of read
 struct GramArgs { const double* Yb; const double* d; const double* r; int p; double shift; double* gout; GridArgs grid; };
 
-static int g_split = 0;                  // letkf_set_option("split", 1): three-kernel tridiagonalisation for M in (48, 64] (slower so far)
-
-template <int MT>
-static int fast_tridiag_run(const double* A, double* V, Workspace ws, int M, int n, cudaStream_t st,
-                            const GramArgs* gram)
+template <int MT, bool QFORM>
+static int fast_tridiag_run(const double* A, double* V, Workspace ws, int M, int n, cudaStream_t st, const GramArgs* gram)
 {
     const size_t smem = fast_tridiag_smem<MT>();
     cudaError_t ce;
-    if constexpr (MT == 64) {
-        if (g_split && M > 34 && sizeof(double2) * (size_t)ws.logcap >= sizeof(double) * SPLIT_DOUBLES) {
-            if (gram) {
-                if ((ce = allow_smem(fast_tridiag_formq<MT, true, true>, smem)) != cudaSuccess) return (int)ce;
-                KLAUNCH("fast_tridiag_head<gram>", st,
-                        fast_tridiag_formq<MT, true, true><<<n, FastCfg<MT>::NT, smem, st>>>(
-                            nullptr, V, ws, M, gram->Yb, gram->d, gram->r, gram->p, gram->shift, gram->gout, gram->grid));
-            } else {
-                if ((ce = allow_smem(fast_tridiag_formq<MT, false, true>, smem)) != cudaSuccess) return (int)ce;
-                KLAUNCH("fast_tridiag_head", st,
-                        fast_tridiag_formq<MT, false, true><<<n, FastCfg<MT>::NT, smem, st>>>(
-                            A, V, ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{}));
-            }
-            KLAUNCH("fast_tridiag_tail", st, fast_tridiag_tail<<<n, 32, sizeof(double) * (640 + 176), st>>>(ws, M));
-            const size_t qs = sizeof(double) * (2304 + 64);
-            if ((ce = allow_smem(fast_formq, qs)) != cudaSuccess) return (int)ce;
-            KLAUNCH("fast_formq", st, fast_formq<<<2 * n, 32, qs, st>>>(V, ws, M));
-            return 0;
-        }
-    }
     if (gram) {
-        if ((ce = allow_smem(fast_tridiag_formq<MT, true>, smem)) != cudaSuccess) return (int)ce;
-        KLAUNCH("fast_tridiag_formq<gram>", st,
-                fast_tridiag_formq<MT, true><<<n, FastCfg<MT>::NT, smem, st>>>(
+        if ((ce = allow_smem(fast_tridiag<MT, true, QFORM>, smem)) != cudaSuccess) return (int)ce;
+        KLAUNCH("fast_tridiag<gram>", st,
+                fast_tridiag<MT, true, QFORM><<<n, FastCfg<MT>::NT, smem, st>>>(
                     nullptr, V, ws, M, gram->Yb, gram->d, gram->r, gram->p, gram->shift, gram->gout, gram->grid));
     } else {
-        if ((ce = allow_smem(fast_tridiag_formq<MT, false>, smem)) != cudaSuccess) return (int)ce;
-        KLAUNCH("fast_tridiag_formq", st,
-                fast_tridiag_formq<MT, false><<<n, FastCfg<MT>::NT, smem, st>>>(
+        if ((ce = allow_smem(fast_tridiag<MT, false, QFORM>, smem)) != cudaSuccess) return (int)ce;
+        KLAUNCH("fast_tridiag", st,
+                fast_tridiag<MT, false, QFORM><<<n, FastCfg<MT>::NT, smem, st>>>(
                     A, V, ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{}));
     }
     return 0;
 }
 
-template <int MT>
-static int fast_apply_run(double* V, Workspace ws, int M, int n, cudaStream_t st, const EpiArgs* ep)
+template <int MT, bool QFORM>
+static int fast_apply_run(double* V, double* w, int* info, Workspace ws, int M, int n, cudaStream_t st, const EpiArgs* ep)
 {
     cudaError_t ce;
     if (ep) {
-        const size_t smem = fast_apply_smem<MT>(ws.swcap) + fast_epi_smem<MT>(ep->ns);
-        if ((ce = allow_smem(fast_apply<MT, true>, smem)) != cudaSuccess) return (int)ce;
-        KLAUNCH("fast_apply<epilogue>", st, fast_apply<MT, true><<<n, FastCfg<MT>::NT, smem, st>>>(V, ws, M, *ep));
+        const size_t smem = fast_apply_smem<MT>(ws.swcap, ep->ns, QFORM);
+        if ((ce = allow_smem(fast_apply<MT, true, QFORM>, smem)) != cudaSuccess) return (int)ce;
+        KLAUNCH("fast_apply<epilogue>", st, fast_apply<MT, true, QFORM><<<n, FastCfg<MT>::NT, smem, st>>>(V, w, info, ws, M, *ep));
     } else {
-        const size_t smem = fast_apply_smem<MT>(ws.swcap);
-        if ((ce = allow_smem(fast_apply<MT, false>, smem)) != cudaSuccess) return (int)ce;
-        KLAUNCH("fast_apply", st, fast_apply<MT, false><<<n, FastCfg<MT>::NT, smem, st>>>(V, ws, M, EpiArgs{}));
+        const size_t smem = fast_apply_smem<MT>(ws.swcap, 0, QFORM);
+        if ((ce = allow_smem(fast_apply<MT, false, QFORM>, smem)) != cudaSuccess) return (int)ce;
+        KLAUNCH("fast_apply", st, fast_apply<MT, false, QFORM><<<n, FastCfg<MT>::NT, smem, st>>>(V, w, info, ws, M, EpiArgs{}));
     }
     return 0;
 }
 
 // ---------------------------------------------------------------------------------------------
-// The EVD of n matrices as three stages.  stage_T: a3 (+ a1, a2 with `gram`) and the explicit Q;
-// stage_QL: a4, the logged QL iteration; stage_AP: a5, replay of the log on Q, eigenvalue sort.
+// The EVD of n matrices as three stages.  stage_T: a3 (+ a1, a2 with `gram`) -- M <= 64: (d, e) and
+// the reflectors into the workspace; above: (d, e) and the explicit Q^T into V.  stage_QL: a4, the
+// logged QL iteration.  stage_AP: a5, replay of the log (and back-transform), eigenvalue sort.
 // ws is the workspace slice of these n matrices.
 static int stage_T(const double* A, int M, int n, double* V, Workspace ws, cudaStream_t st,
                    const GramArgs* gram)
 {
-    if (fast_supported(M) && !g_force_generic) {
+    if (use_fast(M)) {
+        if (t_opt.qform) {
+            switch (fast_bucket(M)) {
+                case 16: return fast_tridiag_run<16, true>(A, V, ws, M, n, st, gram);
+                case 32: return fast_tridiag_run<32, true>(A, V, ws, M, n, st, gram);
+                case 48: return fast_tridiag_run<48, true>(A, V, ws, M, n, st, gram);
+                default: return fast_tridiag_run<64, true>(A, V, ws, M, n, st, gram);
+            }
+        }
         switch (fast_bucket(M)) {
-            case 16: return fast_tridiag_run<16>(A, V, ws, M, n, st, gram);
-            case 32: return fast_tridiag_run<32>(A, V, ws, M, n, st, gram);
-            case 48: return fast_tridiag_run<48>(A, V, ws, M, n, st, gram);
-            default: return fast_tridiag_run<64>(A, V, ws, M, n, st, gram);
+            case 16: return fast_tridiag_run<16, false>(A, V, ws, M, n, st, gram);
+            case 32: return fast_tridiag_run<32, false>(A, V, ws, M, n, st, gram);
+            case 48: return fast_tridiag_run<48, false>(A, V, ws, M, n, st, gram);
+            default: return fast_tridiag_run<64, false>(A, V, ws, M, n, st, gram);
         }
     }
     if (gram) {
@@ -231,14 +289,14 @@ static int stage_T(const double* A, int M, int n, double* V, Workspace ws, cudaS
                 generic_gram<<<n, 256, 0, st>>>(gram->Yb, gram->d, gram->r, M, gram->p, gram->shift, V, gram->gout));
         A = V;
     }
-    if (mid_supported(M) && !g_force_generic) {          // matrix resident in shared memory
+    if (use_mid(M)) {                                    // matrix resident in shared memory
         cudaError_t ce;
         const size_t smem = mid_tridiag_smem(M);
         const int mt = mid_threads(M);
         // registers hold the matrix up to M = 128 (measured, batch 2^26/M^2: M = 96 6.58 -> 5.12 ms, M = 128 9.42 -> 7.57 ms);
         // at MT = 160 the 80 matrix registers of a thread spill under the 102 a CTA of 640 allows and
         // the shared-memory form is as fast (10.5 vs 10.9 ms): mid_reg = 1 (default) / 2 (force) / 0 (never)
-        const bool reg = g_mid_reg == 2 || (g_mid_reg == 1 && mt <= 128);
+        const bool reg = t_opt.mid_reg == 2 || (t_opt.mid_reg == 1 && mt <= 128);
         auto kern = reg ? (mt == 96 ? mid_tridiag_formq_reg<96> : (mt == 128 ? mid_tridiag_formq_reg<128> : mid_tridiag_formq_reg<160>))
                         : (mt == 96 ? mid_tridiag_formq<96> : (mt == 128 ? mid_tridiag_formq<128> : mid_tridiag_formq<160>));
         if ((ce = allow_smem(kern, smem)) != cudaSuccess) return (int)ce;
@@ -250,49 +308,56 @@ static int stage_T(const double* A, int M, int n, double* V, Workspace ws, cudaS
     return 0;
 }
 
-static int g_ql_tpb = 0;                 // letkf_set_option("ql_tpb", 32/64/96): 0 = by size
-
 template <int TPB>
-static int ql_run(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st)
+static int ql_run(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st, int mode)
 {
     cudaError_t ce;
     const size_t ql_smem = sizeof(double) * 2 * (size_t)M * TPB;
     if ((ce = allow_smem(ql_log_kernel<TPB>, ql_smem)) != cudaSuccess) return (int)ce;
-    const int qblocks = (n + TPB - 1) / TPB;
-    KLAUNCH("ql_log_kernel", st, ql_log_kernel<TPB><<<qblocks, TPB, ql_smem, st>>>(ws, M, n, w, info));
+    const int per_cta = mode == QL_TWO_PASS ? TPB / 2 : TPB;  // two lanes per matrix when the iteration runs twice side by side
+    const int qblocks = (n + per_cta - 1) / per_cta;
+    KLAUNCH("ql_log_kernel", st, ql_log_kernel<TPB><<<qblocks, TPB, ql_smem, st>>>(ws, M, n, w, info, mode));
     return 0;
 }
 
-static int stage_QL(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st)
+static int stage_QL(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st, int mode)
 {
-    int tpb = g_ql_tpb ? g_ql_tpb : (M <= 64 ? 64 : 32);
+    int tpb = t_opt.ql_tpb ? t_opt.ql_tpb : (M <= 64 ? 64 : 32);
     while (tpb > 32 && sizeof(double) * 2 * (size_t)M * tpb > 200 * 1024) tpb -= 32;
     switch (tpb) {
-        case 96: return ql_run<96>(M, n, w, info, ws, st);
-        case 64: return ql_run<64>(M, n, w, info, ws, st);
-        default: return ql_run<32>(M, n, w, info, ws, st);
+        case 96: return ql_run<96>(M, n, w, info, ws, st, mode);
+        case 64: return ql_run<64>(M, n, w, info, ws, st, mode);
+        default: return ql_run<32>(M, n, w, info, ws, st, mode);
     }
+}
+
+// the logging pass of the matrices QL_CLASSIFY left pending (the first kernel to touch the log slot)
+static int stage_QLlog(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st)
+{
+    return stage_QL(M, n, w, info, ws, st, QL_LOGPASS);
 }
 
 static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws, cudaStream_t st,
                     const EpiArgs* ep = nullptr)
 {
     const size_t ap_smem = sizeof(double) * (5 * (size_t)M + 2 * 32 * 33);
-    if (fast_supported(M) && !g_force_generic) {
-        int rc = 0;
-        switch (fast_bucket(M)) {
-            case 16: rc = fast_apply_run<16>(V, ws, M, n, st, ep); break;
-            case 32: rc = fast_apply_run<32>(V, ws, M, n, st, ep); break;
-            case 48: rc = fast_apply_run<48>(V, ws, M, n, st, ep); break;
-            default: rc = fast_apply_run<64>(V, ws, M, n, st, ep); break;
+    if (use_fast(M)) {      // (matrices whose rotation log is unusable are finished inside the kernel)
+        if (t_opt.qform) {
+            switch (fast_bucket(M)) {
+                case 16: return fast_apply_run<16, true>(V, w, info, ws, M, n, st, ep);
+                case 32: return fast_apply_run<32, true>(V, w, info, ws, M, n, st, ep);
+                case 48: return fast_apply_run<48, true>(V, w, info, ws, M, n, st, ep);
+                default: return fast_apply_run<64, true>(V, w, info, ws, M, n, st, ep);
+            }
         }
-        if (rc) return rc;
-        // finisher for matrices whose rotation log overflowed (normally none: exits at once)
-        KLAUNCH("generic_apply(flagged)", st,
-                generic_apply<<<(n < 296 ? n : 296), GEN_NT, ap_smem, st>>>(V, w, ws, M, n, info, /*only_flagged=*/1, /*q_rowmajor=*/1));
-        return 0;
+        switch (fast_bucket(M)) {
+            case 16: return fast_apply_run<16, false>(V, w, info, ws, M, n, st, ep);
+            case 32: return fast_apply_run<32, false>(V, w, info, ws, M, n, st, ep);
+            case 48: return fast_apply_run<48, false>(V, w, info, ws, M, n, st, ep);
+            default: return fast_apply_run<64, false>(V, w, info, ws, M, n, st, ep);
+        }
     }
-    if (mid_supported(M) && !g_force_generic) {
+    if (use_mid(M)) {
         cudaError_t ce;
         const int ms = mid_apply_round(M, ws.swcap);
         const size_t smem = mid_apply_smem(M, ws.swcap, ms);
@@ -309,8 +374,10 @@ static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws,
         cfg.attrs = attr;
         cfg.numAttrs = 1;
         KLAUNCH("mid_apply", st, cudaLaunchKernelEx(&cfg, mid_apply, V, ws, M, ms, nsplit, ncol));
+        // finisher for matrices whose rotation log overflowed (normally none: a few CTAs scan the flags and exit)
         KLAUNCH("generic_apply(flagged)", st,
-                generic_apply<<<(n < 296 ? n : 296), GEN_NT, ap_smem, st>>>(V, w, ws, M, n, info, /*only_flagged=*/1, /*q_rowmajor=*/0));
+                generic_apply<<<(n + GEN_NT - 1) / GEN_NT < 8 ? (n + GEN_NT - 1) / GEN_NT : 8, GEN_NT, ap_smem, st>>>(
+                    V, w, ws, M, n, info, /*only_flagged=*/1, /*q_rowmajor=*/0));
         return 0;
     }
     KLAUNCH("generic_apply", st, generic_apply<<<n, GEN_NT, ap_smem, st>>>(V, w, ws, M, n, info, 0, 0));
@@ -318,128 +385,141 @@ static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws,
 }
 
 // ---------------------------------------------------------------------------------------------
-// Private streams of the calling host thread.  A pass over n matrices is cut into sub-chunks that
+// Private streams of the calling host thread.  A call over n matrices is cut into sub-chunks that
 // flow through three stages on separate streams: ql_log_kernel is bound by the serial latency of
 // one matrix's iteration and keeps one warp per SM sub-partition busy at most, so it runs beside
 // the ALU-bound stage_T / stage_AP kernels of the neighbouring sub-chunks (highest priority, so a
 // ready QL block takes the first free slot).  stage_T outranks stage_AP: every QL kernel should
-// start as early as possible, the apply kernels fill the machine behind them.  Everything is forked from and joined back into the
-// caller's stream with events: the caller sees plain stream order.
+// start as early as possible, the apply kernels fill the machine behind them.  Everything is forked
+// from and joined back into the caller's stream with events: the caller sees plain stream order.
 struct Pipe {
     int dev = -1;
     cudaStream_t sT[2] = {nullptr, nullptr}, sA[4] = {};
-    cudaStream_t sQ[16] = {};          // one per sub-chunk: all QL kernels of a pass run side by side
+    cudaStream_t sQ[NQ_STREAMS] = {};
     std::vector<cudaEvent_t> ev;
     size_t used = 0;
+    void destroy()
+    {
+        for (auto& s : sT) if (s) { cudaStreamDestroy(s); s = nullptr; }
+        for (auto& s : sA) if (s) { cudaStreamDestroy(s); s = nullptr; }
+        for (auto& s : sQ) if (s) { cudaStreamDestroy(s); s = nullptr; }
+        for (auto e : ev) cudaEventDestroy(e);
+        ev.clear();
+        used = 0;
+        dev = -1;
+    }
     int init()
     {
         int d = 0;
         cudaError_t ce = cudaGetDevice(&d);
         if (ce != cudaSuccess) return (int)ce;
         if (d == dev) return 0;
+        if (dev >= 0) {                       // the thread moved to another device: drop the old streams
+            cudaSetDevice(dev);
+            destroy();
+            cudaSetDevice(d);
+        }
         int least = 0, greatest = 0;
         cudaDeviceGetStreamPriorityRange(&least, &greatest);
         const int mid = (greatest < least) ? greatest + 1 : greatest;
-        for (int k = 0; k < 2; ++k) {
+        for (int k = 0; k < 2; ++k)
             if ((ce = cudaStreamCreateWithPriority(&sT[k], cudaStreamNonBlocking, mid)) != cudaSuccess) return (int)ce;
-        }
         for (int k = 0; k < 4; ++k)
             if ((ce = cudaStreamCreateWithPriority(&sA[k], cudaStreamNonBlocking, least)) != cudaSuccess) return (int)ce;
-        for (int k = 0; k < 16; ++k)
+        for (int k = 0; k < NQ_STREAMS; ++k)
             if ((ce = cudaStreamCreateWithPriority(&sQ[k], cudaStreamNonBlocking, greatest)) != cudaSuccess) return (int)ce;
-        ev.clear();
-        used = 0;
         dev = d;
         return 0;
     }
     cudaEvent_t event()
     {
         if (used == ev.size()) {
-            cudaEvent_t e;
+            cudaEvent_t e = nullptr;
             cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
             ev.push_back(e);
         }
         return ev[used++];
     }
     // `to` waits for everything enqueued on `from` so far
-    void link(cudaStream_t from, cudaStream_t to)
+    int link(cudaStream_t from, cudaStream_t to)
     {
         cudaEvent_t e = event();
-        cudaEventRecord(e, from);
-        cudaStreamWaitEvent(to, e, 0);
+        cudaError_t ce;
+        if (!e) return (int)cudaErrorMemoryAllocation;
+        if ((ce = cudaEventRecord(e, from)) != cudaSuccess) return (int)ce;
+        if ((ce = cudaStreamWaitEvent(to, e, 0)) != cudaSuccess) return (int)ce;
+        return 0;
     }
 };
 static thread_local Pipe g_pipe;
 
-static int g_pipeline = 1;               // letkf_set_option("pipeline", 0): one stream, one chunk
-static const int PIPE_MIN_SUB = 1024;    // smallest sub-chunk worth a launch of its own
-static const int PIPE_MAX_SUB = 16;      // = number of QL streams
-static thread_local int g_max_sub = 8;   // sub-chunks per pass: 8 for device calls (measured best), 16 for the
-                                         // host entry points (finer copy/compute overlap: shorter head and tail)
 
-// One pass: n matrices whose workspace records are ws[0..n).  stageT(b0, nk, stream) enqueues the
-// first stage of matrices [b0, b0+nk); post(b0, nk, stream) whatever follows stage_AP (the
-// analysis epilogue) or nothing.
-static EpiArgs epi_slice(const EpiArgs& e, int M, int b0)
+// One call: `batch` matrices, workspace carved for pl.per * pl.nslot matrices.  The callbacks get
+// (b0 = first matrix of the sub-chunk in the batch, nk = its size, s0 = first workspace record of
+// its slot, stream):
+//   stageT  enqueues the first stage (it calls stage_T with ws_slice(ws, M, s0, l0))
+//   stageQA enqueues QL and apply (w / V / info of the sub-chunk are the caller's business: batch-
+//           indexed for the EVD, slot-indexed for the analysis)
+//   post    whatever follows (analysis epilogue, read-back hooks)
+template <class FT, class FQ, class FA, class FP>
+static int run_pipeline(const Plan& pl, int batch, cudaStream_t st, FT stageT, FQ stageQL, FA stageAP, FP post)
 {
-    EpiArgs s = e;
-    s.lam += (size_t)b0 * M;
-    s.g += (size_t)b0 * M;
-    s.Xb += (size_t)b0 * e.ns * M;
-    s.Xa += (size_t)b0 * e.ns * M;
-    if (s.wbar) s.wbar += (size_t)b0 * M;
-    return s;
-}
-
-// Sub-chunks of a pass of n matrices: nsub pieces of `per` matrices (the last one shorter).
-static void pass_partition(int n, int& nsub, int& per)
-{
-    nsub = (g_pipeline && (!g_prof.on || g_prof.keep_pipeline)) ? n / PIPE_MIN_SUB : 1;
-    if (nsub > g_max_sub) nsub = g_max_sub;
-    if (nsub < 1) nsub = 1;
-    per = (n + nsub - 1) / nsub;
-}
-
-// ep0: a6-a9 fused into the apply kernel (pointers of matrix 0 of the pass), or NULL.
-template <class FT, class FP>
-static int run_pass(int M, int n, double* w, double* V, int* info, const Workspace& ws,
-                    cudaStream_t st, FT stageT, FP post, const EpiArgs* ep0 = nullptr)
-{
-    int nsub, per;
-    pass_partition(n, nsub, per);
-    if (nsub < 2) {
-        int rc = stageT(0, n, st);
-        if (rc) return rc;
-        if ((rc = stage_QL(M, n, w, info, ws, st))) return rc;
-        if ((rc = stage_AP(M, n, w, V, info, ws, st, ep0))) return rc;
-        return post(0, n, st);
+    if (!pl.pipelined) {
+        for (int b0 = 0; b0 < batch; b0 += pl.per) {
+            const int nk = (batch - b0 < pl.per) ? batch - b0 : pl.per;
+            int rc;
+            if ((rc = stageT(b0, nk, 0, 0, st))) return rc;
+            if ((rc = stageQL(b0, nk, 0, 0, st, false))) return rc;
+            if (pl.ql_mode == QL_CLASSIFY && (rc = stageQL(b0, nk, 0, 0, st, true))) return rc;
+            if ((rc = stageAP(b0, nk, 0, 0, st))) return rc;
+            if ((rc = post(b0, nk, 0, 0, st))) return rc;
+        }
+        return 0;
     }
     Pipe& P = g_pipe;
     int rc = P.init();
     if (rc) return rc;
     P.used = 0;
-    for (int k = 0; k < 2; ++k) P.link(st, P.sT[k]);
-    for (int k = 0; k < 4; ++k) P.link(st, P.sA[k]);
-    for (int k = 0; k < nsub; ++k) P.link(st, P.sQ[k]);
-    for (int k = 0, b0 = 0; b0 < n; ++k, b0 += per) {
-        const int nk = (n - b0 < per) ? n - b0 : per;
-        const int s = k & 1;
-        const Workspace wk = ws_slice(ws, M, b0);
-        int* infok = info ? info + b0 : nullptr;
-        if ((rc = stageT(b0, nk, P.sT[s]))) return rc;
-        P.link(P.sT[s], P.sQ[k]);
-        if ((rc = stage_QL(M, nk, w + (size_t)b0 * M, infok, wk, P.sQ[k]))) return rc;
-        cudaStream_t sa = P.sA[k & 3];
-        P.link(P.sQ[k], sa);
-        EpiArgs epk;
-        if (ep0) epk = epi_slice(*ep0, M, b0);
-        if ((rc = stage_AP(M, nk, w + (size_t)b0 * M, V + (size_t)b0 * M * M, infok, wk, sa, ep0 ? &epk : nullptr))) return rc;
-        if ((rc = post(b0, nk, sa))) return rc;
+    // every private stream is joined back into `st` on EVERY exit, so that a caller (and the
+    // stream-ordered free of an owned workspace) never runs ahead of work still in flight
+    auto join_all = [&]() {
+        int jr = 0, r2;
+        for (int k = 0; k < 2; ++k) if ((r2 = P.link(P.sT[k], st)) && !jr) jr = r2;
+        for (int k = 0; k < 4; ++k) if ((r2 = P.link(P.sA[k], st)) && !jr) jr = r2;
+        for (int k = 0; k < NQ_STREAMS; ++k) if ((r2 = P.link(P.sQ[k], st)) && !jr) jr = r2;
+        return jr;
+    };
+    for (int k = 0; k < 2 && !rc; ++k) rc = P.link(st, P.sT[k]);
+    for (int k = 0; k < 4 && !rc; ++k) rc = P.link(st, P.sA[k]);
+    for (int k = 0; k < NQ_STREAMS && !rc; ++k) rc = P.link(st, P.sQ[k]);
+    std::vector<cudaEvent_t> done((size_t)pl.nsub, nullptr);
+    for (int k = 0, b0 = 0; b0 < batch && !rc; ++k, b0 += pl.per) {
+        const int nk = (batch - b0 < pl.per) ? batch - b0 : pl.per;
+        const int s0 = (k % pl.nslot) * pl.per, l0 = (k % pl.nlog) * pl.per;
+        cudaStream_t sT = P.sT[k & 1], sQ = P.sQ[k % NQ_STREAMS], sA = P.sA[k & 3];
+        if (k >= pl.nslot) {                       // the slot is free when its previous tenant's last kernel is done
+            cudaError_t ce = cudaStreamWaitEvent(sT, done[k - pl.nslot], 0);
+            if (ce != cudaSuccess) { rc = (int)ce; break; }
+        }
+        if ((rc = stageT(b0, nk, s0, l0, sT))) break;
+        if ((rc = P.link(sT, sQ))) break;
+        // (the classifying QL kernel logs nothing: the log slot is only needed by the kernel behind it)
+        if (pl.ql_mode == QL_CLASSIFY && (rc = stageQL(b0, nk, s0, l0, sQ, false))) break;
+        if (k >= pl.nlog) {                        // ... and so is the log slot
+            cudaError_t ce = cudaStreamWaitEvent(sQ, done[k - pl.nlog], 0);
+            if (ce != cudaSuccess) { rc = (int)ce; break; }
+        }
+        if ((rc = stageQL(b0, nk, s0, l0, sQ, pl.ql_mode == QL_CLASSIFY))) break;
+        if ((rc = P.link(sQ, sA))) break;
+        if ((rc = stageAP(b0, nk, s0, l0, sA))) break;
+        if ((rc = post(b0, nk, s0, l0, sA))) break;
+        done[k] = P.event();
+        if (!done[k]) { rc = (int)cudaErrorMemoryAllocation; break; }
+        cudaError_t ce = cudaEventRecord(done[k], sA);
+        if (ce != cudaSuccess) { rc = (int)ce; break; }
     }
-    for (int k = 0; k < 2; ++k) P.link(P.sT[k], st);
-    for (int k = 0; k < 4; ++k) P.link(P.sA[k], st);
-    for (int k = 0; k < nsub; ++k) P.link(P.sQ[k], st);
-    return 0;
+    const int jr = join_all();
+    return rc ? rc : jr;
 }
 
 struct ScopedWork {
@@ -469,39 +549,51 @@ using namespace letkf;
 
 extern "C" {
 
-size_t letkf_syev_workspace_bytes(int M, int batch)
-{
-    if (M < 1 || M > LETKF_MAX_M || batch < 1) return 0;
-    Workspace ws;
-    return carve(ws, nullptr, M, syev_chunk(M, batch));
-}
-
 // Hooks of the host-buffer entry points: pre(b0, nk, s) is enqueued on the stream of a sub-chunk's
 // first kernel before it (wait for the sub-chunk's inputs), post(b0, nk, s) after its last kernel
-// (start the read-back).  b0 counts from the start of the pass.
+// (start the read-back).  b0 counts from the start of the (device) call.
 struct PassHooks {
     int (*pre)(void* ctx, int b0, int nk, cudaStream_t s);
     int (*post)(void* ctx, int b0, int nk, cudaStream_t s);
     void* ctx;
 };
+static thread_local const PassHooks* t_hooks = nullptr;   // set by the host entry points only
 
-static thread_local const PassHooks* g_analysis_hooks = nullptr;   // set by the host entry point only
+static size_t syev_need(int M, const Plan& pl) { return plan_bytes(M, (size_t)pl.per * pl.nslot, (size_t)pl.per * pl.nlog, 0, pl.two_pass); }
 
-// one pass (n <= syev_chunk matrices, workspace carved for them) of the EVD on device buffers
-static int syev_pass(const double* A, int M, int n, double* w, double* V, int* info, const Workspace& ws,
-                     cudaStream_t st, const PassHooks* hooks)
+size_t letkf_syev_workspace_bytes(int M, int batch)
 {
-    auto stageT = [&](int c0, int nk, cudaStream_t s) {
-        if (hooks) { const int rc = hooks->pre(hooks->ctx, c0, nk, s); if (rc) return rc; }
-        return stage_T(A + (size_t)c0 * M * M, M, nk, V + (size_t)c0 * M * M, ws_slice(ws, M, c0), s, nullptr);
+    EntryScope scope;
+    if (M < 1 || M > LETKF_MAX_M || batch < 1) return 0;
+    return syev_need(M, make_plan(M, batch, 0, 0));
+}
+
+// the EVD of `batch` matrices on device buffers, workspace at `base` (carved per `pl`)
+static int syev_core(const double* A, int M, int batch, double* w, double* V, int* info, void* base,
+                     const Plan& pl, cudaStream_t st)
+{
+    Workspace ws;
+    carve(ws, base, M, pl.per * pl.nslot, pl.per * pl.nlog, pl.two_pass);
+    const PassHooks* hooks = t_hooks;
+    auto stageT = [&](int b0, int nk, int s0, int l0, cudaStream_t s) {
+        if (hooks) { const int rc = hooks->pre(hooks->ctx, b0, nk, s); if (rc) return rc; }
+        return stage_T(A + (size_t)b0 * M * M, M, nk, V + (size_t)b0 * M * M, ws_slice(ws, M, s0, l0), s, nullptr);
     };
-    auto post = [&](int c0, int nk, cudaStream_t s) { return hooks ? hooks->post(hooks->ctx, c0, nk, s) : 0; };
-    return run_pass(M, n, w, V, info, ws, st, stageT, post);
+    auto stageQL = [&](int b0, int nk, int s0, int l0, cudaStream_t s, bool logpass) {
+        if (logpass) return stage_QLlog(M, nk, w + (size_t)b0 * M, info ? info + b0 : nullptr, ws_slice(ws, M, s0, l0), s);
+        return stage_QL(M, nk, w + (size_t)b0 * M, info ? info + b0 : nullptr, ws_slice(ws, M, s0, l0), s, pl.ql_mode);
+    };
+    auto stageAP = [&](int b0, int nk, int s0, int l0, cudaStream_t s) {
+        return stage_AP(M, nk, w + (size_t)b0 * M, V + (size_t)b0 * M * M, info ? info + b0 : nullptr, ws_slice(ws, M, s0, l0), s);
+    };
+    auto post = [&](int b0, int nk, int, int, cudaStream_t s) { return hooks ? hooks->post(hooks->ctx, b0, nk, s) : 0; };
+    return run_pipeline(pl, batch, st, stageT, stageQL, stageAP, post);
 }
 
 int letkf_syev_batched(const double* A, int M, int batch, double* w, double* V, int* info,
                        void* work, size_t work_bytes, void* stream)
 {
+    EntryScope scope;
     g_launches = 0;
     if (M < 1 || M > LETKF_MAX_M) return -2;
     if (batch < 0) return -3;
@@ -511,131 +603,127 @@ int letkf_syev_batched(const double* A, int M, int batch, double* w, double* V, 
     if (!V || misaligned(V)) return -5;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     prof_reset(st);
-
-    const int chunk = syev_chunk(M, batch);
-    Workspace ws;
-    const size_t need = carve(ws, nullptr, M, chunk);
+    const Plan pl = make_plan(M, batch, 0, work ? work_bytes : 0);
     ScopedWork sw;
-    int rc = sw.acquire(work, work_bytes, need, st, 7);
+    int rc = sw.acquire(work, work_bytes, syev_need(M, pl), st, 7);
     if (rc) return rc;
-    carve(ws, sw.ptr, M, chunk);
-
-    for (int b0 = 0; b0 < batch; b0 += chunk) {
-        const int n = (batch - b0 < chunk) ? batch - b0 : chunk;
-        rc = syev_pass(A + (size_t)b0 * M * M, M, n, w + (size_t)b0 * M, V + (size_t)b0 * M * M,
-                       info ? info + b0 : nullptr, ws, st, nullptr);
-        if (rc) return rc;
-    }
-    return LETKF_OK;
+    return syev_core(A, M, batch, w, V, info, sw.ptr, pl, st);
 }
+
+// per-matrix bytes the analysis keeps per slot beside the EVD workspace: Q / V (not on the fused
+// M <= 64 path, where V never leaves the SM), lam, g
+static size_t analysis_extra(int M, bool keepV) { return sizeof(double) * ((keepV ? (size_t)M * M : 0) + 2 * (size_t)M); }
+static bool analysis_fused(int M, int nstate, bool wantW) { return !wantW && use_fast(M) && nstate <= EPI_NS_MAX; }
+// is a Q / V buffer needed per slot?  (not when a6-a9 are fused into fast_apply and Q is never formed)
+static bool analysis_keepV(int M, int nstate, bool wantW) { return !analysis_fused(M, nstate, wantW) || t_opt.qform; }
+static size_t analysis_need(int M, const Plan& pl, size_t extra) { return plan_bytes(M, (size_t)pl.per * pl.nslot, (size_t)pl.per * pl.nlog, extra, pl.two_pass); }
 
 size_t letkf_analysis_workspace_bytes(int M, int p, int nstate, int batch)
 {
+    EntryScope scope;
     (void)p; (void)nstate;
     if (M < 1 || M > LETKF_MAX_M || batch < 1) return 0;
-    const int chunk = syev_chunk(M, batch);
-    Workspace ws;
-    size_t s = carve(ws, nullptr, M, chunk);
-    s += align_up(sizeof(double) * (size_t)M * M * chunk, 256);   // Q / V
-    s += align_up(sizeof(double) * (size_t)M * chunk, 256);       // lam
-    s += align_up(sizeof(double) * (size_t)M * chunk, 256);       // g
-    return s;
+    // sized for the form that needs most (W requested: V is kept per slot)
+    const size_t extra = analysis_extra(M, true);
+    return analysis_need(M, make_plan(M, batch, extra, 0), extra);
 }
 
 // does the grid form run with the gather fused into the tridiagonalisation kernel?
-static bool grid_fused(int M, int nstate) { return fast_supported(M) && !g_force_generic && nstate <= EPI_NS_MAX; }
+static bool grid_fused(int M, int nstate) { return use_fast(M) && nstate <= EPI_NS_MAX; }
+
+static size_t grid_extra(int M, int p, int nstate)
+{
+    size_t e = analysis_extra(M, true);
+    if (!grid_fused(M, nstate)) e += sizeof(double) * ((size_t)p * M + 2 * (size_t)p);      // materialised Y_loc, d, r
+    return e;
+}
 
 size_t letkf_analysis_grid_workspace_bytes(int M, int V, int Ny, int Nx, int hw, int nstate)
 {
+    EntryScope scope;
     if (M < 2 || M > LETKF_MAX_M || V < 1 || Ny < 1 || Nx < 1 || hw < 0 || nstate < 1) return 0;
     const long npts = (long)Ny * Nx;
     if (npts > 0x7fffffffL) return 0;
     const int batch = (int)npts, p = V * (2 * hw + 1) * (2 * hw + 1);
-    size_t s = align_up(letkf_analysis_workspace_bytes(M, p, nstate, batch), 256);
-    s += align_up(sizeof(double) * (size_t)V * npts, 256);                                   // ybar
-    const int chunk = syev_chunk(M, batch);                                                  // materialised Y_loc
-    s += align_up(sizeof(double) * (size_t)p * M * chunk, 256) + 2 * align_up(sizeof(double) * (size_t)p * chunk, 256);
-    return s;
+    const size_t extra = grid_extra(M, p, nstate);
+    return analysis_need(M, make_plan(M, batch, extra, 0), extra) + align_up(sizeof(double) * (size_t)V * npts, 256) + 4 * 256;
 }
 
-// a1-a9 for `batch` grid points.  Either (Yb, d, rinv_loc) or `grid` (then gYb/gd/gr are scratch
-// for the materialised local observations of one pass, used when the gather cannot be fused).
+// a1-a9 for `batch` grid points.  Either (Yb, d, rinv_loc) or `grid` (local observations gathered
+// from the fields: inside the tridiagonalisation kernel when grid_fused(), else materialised per
+// slot in the workspace).  `work` holds analysis_need(M, pl, extra) bytes.
 static int analysis_core(const double* Yb, const double* d, const double* rinv_loc, const GridArgs* grid,
-                         double* gYb, double* gd, double* gr,
                          const double* Xb, int M, int p, int nstate, int batch, double rho,
                          double* Xa, double* W, double* wbar, int* info,
-                         void* work, size_t work_bytes, int work_argpos, cudaStream_t st)
+                         void* work, const Plan& pl, size_t extra, cudaStream_t st)
 {
-    const int chunk = syev_chunk(M, batch);
-    const size_t need = letkf_analysis_workspace_bytes(M, p, nstate, batch);
-    ScopedWork sw;
-    int rc = sw.acquire(work, work_bytes, need, st, work_argpos);
-    if (rc) return rc;
+    (void)extra;
+    const int nrec = pl.per * pl.nslot;
     Workspace ws;
-    size_t off = carve(ws, sw.ptr, M, chunk);
-    char* base = reinterpret_cast<char*>(sw.ptr);
-    double* Vbuf = reinterpret_cast<double*>(base + off); off += align_up(sizeof(double) * (size_t)M * M * chunk, 256);
-    double* lam  = reinterpret_cast<double*>(base + off); off += align_up(sizeof(double) * (size_t)M * chunk, 256);
-    double* gbuf = reinterpret_cast<double*>(base + off);
+    size_t off = carve(ws, work, M, nrec, pl.per * pl.nlog, pl.two_pass);
+    char* base = reinterpret_cast<char*>(work);
+    const bool fused = analysis_fused(M, nstate, W != nullptr);
+    const bool fuse_gather = grid && !W && grid_fused(M, nstate);
+    double* Vbuf = nullptr;
+    if (analysis_keepV(M, nstate, W != nullptr)) { Vbuf = reinterpret_cast<double*>(base + off); off += align_up(sizeof(double) * (size_t)M * M * nrec, 256); }
+    double* lam  = reinterpret_cast<double*>(base + off); off += align_up(sizeof(double) * (size_t)M * nrec, 256);
+    double* gbuf = reinterpret_cast<double*>(base + off); off += align_up(sizeof(double) * (size_t)M * nrec, 256);
+    double *gYb = nullptr, *gd = nullptr, *gr = nullptr;
+    if (grid && !fuse_gather) {
+        gYb = reinterpret_cast<double*>(base + off); off += align_up(sizeof(double) * (size_t)p * M * nrec, 256);
+        gd = reinterpret_cast<double*>(base + off);  off += align_up(sizeof(double) * (size_t)p * nrec, 256);
+        gr = reinterpret_cast<double*>(base + off);  off += align_up(sizeof(double) * (size_t)p * nrec, 256);
+    }
 
     const double shift = (double)(M - 1) / rho;
     cudaError_t ce;
     const size_t ep_smem = sizeof(double) * (2 * (size_t)M + 2 * (size_t)nstate + 2 * (size_t)nstate * M);
     if (ep_smem > 200 * 1024) return -7;
     if ((ce = allow_smem(generic_epilogue, ep_smem)) != cudaSuccess) return (int)ce;
-    const bool fuse_gather = grid && !W && grid_fused(M, nstate);
+    const PassHooks* hooks = t_hooks;
 
-    for (int b0 = 0; b0 < batch; b0 += chunk) {
-        const int n = (batch - b0 < chunk) ? batch - b0 : chunk;
-        // local observations of this pass: the caller's arrays, or the scratch the gather fills
-        const double* Ybc = grid ? gYb : Yb + (size_t)b0 * p * M;
-        const double* dc = grid ? gd : d + (size_t)b0 * p;
-        const double* rc_ = grid ? gr : rinv_loc + (size_t)b0 * p;
-        const double* Xbc = Xb + (size_t)b0 * nstate * M;
-        double* Xac = Xa + (size_t)b0 * nstate * M;
-        double* Wc = W ? W + (size_t)b0 * M * M : nullptr;
-        double* wbc = wbar ? wbar + (size_t)b0 * M : nullptr;
-        int* infoc = info ? info + b0 : nullptr;
-
-        auto stageT = [&](int c0, int nk, cudaStream_t s) {
-            if (g_analysis_hooks) {
-                const int hrc = g_analysis_hooks->pre(g_analysis_hooks->ctx, b0 + c0, nk, s);
-                if (hrc) return hrc;
+    auto stageT = [&](int b0, int nk, int s0, int l0, cudaStream_t s) {
+        if (hooks) { const int hrc = hooks->pre(hooks->ctx, b0, nk, s); if (hrc) return hrc; }
+        GramArgs ga{nullptr, nullptr, nullptr, p, shift, gbuf + (size_t)s0 * M, GridArgs{}};
+        if (grid) {
+            GridArgs gk = *grid;
+            gk.point0 = grid->point0 + b0;
+            if (fuse_gather) {
+                ga.grid = gk;
+            } else {
+                KLAUNCH("grid_gather", s,
+                        grid_gather<<<nk, 256, 0, s>>>(gk, M, p, gYb + (size_t)s0 * p * M, gd + (size_t)s0 * p, gr + (size_t)s0 * p));
+                ga.Yb = gYb + (size_t)s0 * p * M; ga.d = gd + (size_t)s0 * p; ga.r = gr + (size_t)s0 * p;
             }
-            GramArgs ga{Ybc + (size_t)c0 * p * M, dc + (size_t)c0 * p, rc_ + (size_t)c0 * p, p, shift,
-                        gbuf + (size_t)c0 * M, GridArgs{}};
-            if (grid) {
-                GridArgs gk = *grid;
-                gk.point0 = grid->point0 + b0 + c0;
-                if (fuse_gather) {
-                    ga.grid = gk;
-                } else {
-                    KLAUNCH("grid_gather", s,
-                            grid_gather<<<nk, 256, 0, s>>>(gk, M, p, gYb + (size_t)c0 * p * M, gd + (size_t)c0 * p,
-                                                           gr + (size_t)c0 * p));
-                }
-            }
-            double* Vk = Vbuf + (size_t)c0 * M * M;
-            return stage_T(Vk, M, nk, Vk, ws_slice(ws, M, c0), s, &ga);
-        };
-        // a6-a9: fused into fast_apply when W is not wanted (V then never leaves the SM); the
-        // any-M kernel otherwise, and for the grid points the slow path finished.
-        const bool fused = !Wc && fast_supported(M) && !g_force_generic && nstate <= EPI_NS_MAX;
-        auto post = [&](int c0, int nk, cudaStream_t s) -> int {
-            const int gridsz = fused ? (nk < 296 ? nk : 296) : nk;
-            KLAUNCH(fused ? "generic_epilogue(flagged)" : "generic_epilogue", s,
-                    generic_epilogue<<<gridsz, 256, ep_smem, s>>>(
-                        Vbuf + (size_t)c0 * M * M, lam + (size_t)c0 * M, gbuf + (size_t)c0 * M,
-                        Xbc + (size_t)c0 * nstate * M, M, nstate, nk, Xac + (size_t)c0 * nstate * M,
-                        Wc ? Wc + (size_t)c0 * M * M : nullptr, wbc ? wbc + (size_t)c0 * M : nullptr,
-                        fused ? ws.flags + c0 : nullptr));
-            return g_analysis_hooks ? g_analysis_hooks->post(g_analysis_hooks->ctx, b0 + c0, nk, s) : 0;
-        };
-        EpiArgs ep{lam, gbuf, Xbc, Xac, wbc, nstate};
-        rc = run_pass(M, n, lam, Vbuf, infoc, ws, st, stageT, post, fused ? &ep : nullptr);
-        if (rc) return rc;
-    }
-    return LETKF_OK;
+        } else {
+            ga.Yb = Yb + (size_t)b0 * p * M; ga.d = d + (size_t)b0 * p; ga.r = rinv_loc + (size_t)b0 * p;
+        }
+        double* Vk = Vbuf ? Vbuf + (size_t)s0 * M * M : nullptr;
+        return stage_T(Vk, M, nk, Vk, ws_slice(ws, M, s0, l0), s, &ga);
+    };
+    auto stageQL = [&](int b0, int nk, int s0, int l0, cudaStream_t s, bool logpass) {
+        if (logpass) return stage_QLlog(M, nk, lam + (size_t)s0 * M, info ? info + b0 : nullptr, ws_slice(ws, M, s0, l0), s);
+        return stage_QL(M, nk, lam + (size_t)s0 * M, info ? info + b0 : nullptr, ws_slice(ws, M, s0, l0), s, pl.ql_mode);
+    };
+    // a6-a9: fused into fast_apply when W is not wanted (V then never leaves the SM); the any-M
+    // kernel otherwise
+    auto stageAP = [&](int b0, int nk, int s0, int l0, cudaStream_t s) {
+        EpiArgs ep{lam + (size_t)s0 * M, gbuf + (size_t)s0 * M, Xb + (size_t)b0 * nstate * M, Xa + (size_t)b0 * nstate * M,
+                   wbar ? wbar + (size_t)b0 * M : nullptr, nstate};
+        return stage_AP(M, nk, lam + (size_t)s0 * M, Vbuf ? Vbuf + (size_t)s0 * M * M : nullptr, info ? info + b0 : nullptr,
+                        ws_slice(ws, M, s0, l0), s, fused ? &ep : nullptr);
+    };
+    auto post = [&](int b0, int nk, int s0, int l0, cudaStream_t s) -> int {
+        if (!fused) {
+            KLAUNCH("generic_epilogue", s,
+                    generic_epilogue<<<nk, 256, ep_smem, s>>>(
+                        Vbuf + (size_t)s0 * M * M, lam + (size_t)s0 * M, gbuf + (size_t)s0 * M,
+                        Xb + (size_t)b0 * nstate * M, M, nstate, nk, Xa + (size_t)b0 * nstate * M,
+                        W ? W + (size_t)b0 * M * M : nullptr, wbar ? wbar + (size_t)b0 * M : nullptr, nullptr));
+        }
+        return hooks ? hooks->post(hooks->ctx, b0, nk, s) : 0;
+    };
+    return run_pipeline(pl, batch, st, stageT, stageQL, stageAP, post);
 }
 
 int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv_loc,
@@ -643,6 +731,7 @@ int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv
                            double* Xa, double* W, double* wbar, int* info,
                            void* work, size_t work_bytes, void* stream)
 {
+    EntryScope scope;
     g_launches = 0;
     if (M < 2 || M > LETKF_MAX_M) return -5;   // M = 1 has no ensemble spread: Eq.15 is 0/0
     if (p < 0) return -6;
@@ -659,8 +748,12 @@ int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv
     if (wbar && misaligned(wbar)) return -12;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     prof_reset(st);
-    return analysis_core(Yb, d, rinv_loc, nullptr, nullptr, nullptr, nullptr, Xb, M, p, nstate, batch, rho,
-                         Xa, W, wbar, info, work, work_bytes, 14, st);
+    const size_t extra = analysis_extra(M, analysis_keepV(M, nstate, W != nullptr));
+    const Plan pl = make_plan(M, batch, extra, work ? work_bytes : 0);
+    ScopedWork sw;
+    int rc = sw.acquire(work, work_bytes, analysis_need(M, pl, extra), st, 14);
+    if (rc) return rc;
+    return analysis_core(Yb, d, rinv_loc, nullptr, Xb, M, p, nstate, batch, rho, Xa, W, wbar, info, sw.ptr, pl, extra, st);
 }
 
 int letkf_analysis_grid(const double* Yf, const double* yo, const unsigned char* obs_mask, const double* Xb,
@@ -668,6 +761,7 @@ int letkf_analysis_grid(const double* Yf, const double* yo, const unsigned char*
                         double sigma_o, double rho, double* Xa, double* wbar, int* info,
                         void* work, size_t work_bytes, void* stream)
 {
+    EntryScope scope;
     g_launches = 0;
     if (M < 2 || M > LETKF_MAX_M) return -5;
     if (V < 1) return -6;
@@ -687,56 +781,52 @@ int letkf_analysis_grid(const double* Yf, const double* yo, const unsigned char*
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     prof_reset(st);
     const int batch = Ny * Nx, side = 2 * hw + 1, p = V * side * side;
-    const size_t need = letkf_analysis_grid_workspace_bytes(M, V, Ny, Nx, hw, nstate);
+    // carve: [ybar][analysis workspace (with the materialised Y_loc of the slots when the gather is not fused)]
+    const size_t ybytes = align_up(sizeof(double) * (size_t)V * batch, 256);
+    const size_t extra = grid_extra(M, p, nstate) - (analysis_keepV(M, nstate, false) ? 0 : sizeof(double) * (size_t)M * M);
+    const Plan pl = make_plan(M, batch, extra, work ? (work_bytes > ybytes ? work_bytes - ybytes : 1) : 0);
     ScopedWork sw;
-    int rc = sw.acquire(work, work_bytes, need, st, 18);
+    int rc = sw.acquire(work, work_bytes, ybytes + analysis_need(M, pl, extra), st, 18);
     if (rc) return rc;
-    // carve: [analysis workspace][ybar][materialised Y_loc of one pass]
-    const size_t wa = align_up(letkf_analysis_workspace_bytes(M, p, nstate, batch), 256);
     char* base = reinterpret_cast<char*>(sw.ptr);
-    double* ybar = reinterpret_cast<double*>(base + wa);
-    size_t off = wa + align_up(sizeof(double) * (size_t)V * batch, 256);
-    const int chunk = syev_chunk(M, batch);
-    double* gYb = reinterpret_cast<double*>(base + off); off += align_up(sizeof(double) * (size_t)p * M * chunk, 256);
-    double* gd = reinterpret_cast<double*>(base + off);  off += align_up(sizeof(double) * (size_t)p * chunk, 256);
-    double* gr = reinterpret_cast<double*>(base + off);
+    double* ybar = reinterpret_cast<double*>(base);
     const long nobs = (long)V * batch;
     KLAUNCH("grid_obs_mean", st, grid_obs_mean<<<(unsigned)((nobs + 7) / 8), 256, 0, st>>>(Yf, ybar, nobs, M));
     GridArgs g{Yf, ybar, yo, obs_mask, V, Ny, Nx, hw, loc_kind, loc_scale, 1.0 / (sigma_o * sigma_o), 0};
-    rc = analysis_core(nullptr, nullptr, nullptr, &g, gYb, gd, gr, Xb, M, p, nstate, batch, rho,
-                       Xa, nullptr, wbar, info, base, wa, 18, st);
-    return rc;
+    return analysis_core(nullptr, nullptr, nullptr, &g, Xb, M, p, nstate, batch, rho,
+                         Xa, nullptr, wbar, info, base + ybytes, pl, extra, st);
 }
 
 // ---- host-buffer entry points -----------------------------------------------------------------
 // A pass of the batch lives on the device at a time; the sub-chunks of the kernel pipeline are
 // copied in one after the other on a copy-in stream, each sub-chunk's first kernel waits for its
 // own copy only, and its read-back starts on a copy-out stream as soon as its last kernel is done:
-// both copy engines and the SMs overlap (PCIe is full duplex).  The device staging arena is kept by the calling host thread between calls
-// (letkf_host_release() frees it); the call returns after the last byte has reached the host.
+// both copy engines and the SMs overlap (PCIe is full duplex).  The device staging arena is kept by
+// the calling host thread between calls (letkf_host_release() frees it); the call returns after the
+// last byte has reached the host.
 struct HostPipe {
     int dev = -1;
     cudaStream_t s[2] = {nullptr, nullptr};
     cudaStream_t sC = nullptr;    // the stream the kernels of a host call are forked from
     std::vector<cudaEvent_t> ev;
-    void events(size_t n)
+    int events(size_t n)
     {
         while (ev.size() < n) {
             cudaEvent_t e;
-            cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+            cudaError_t ce = cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+            if (ce != cudaSuccess) return (int)ce;
             ev.push_back(e);
         }
+        return 0;
     }
     char* arena = nullptr;        // device staging memory, grown on demand and kept between calls
     size_t arena_bytes = 0;       // (re-allocating > 1 GB per call costs more than the whole EVD)
     int reserve(size_t bytes)
     {
         if (bytes <= arena_bytes) return 0;
-        if (arena) cudaFree(arena);
-        arena = nullptr;
-        arena_bytes = 0;
+        release();
         cudaError_t ce = cudaMalloc(reinterpret_cast<void**>(&arena), bytes);
-        if (ce != cudaSuccess) return (int)ce;
+        if (ce != cudaSuccess) { arena = nullptr; return (int)ce; }
         arena_bytes = bytes;
         return 0;
     }
@@ -752,59 +842,76 @@ struct HostPipe {
         cudaError_t ce = cudaGetDevice(&d);
         if (ce != cudaSuccess) return (int)ce;
         if (d == dev) return 0;
-        arena = nullptr;            // memory of another device is left to that device's context
-        arena_bytes = 0;
+        if (dev >= 0) {                      // the thread moved to another device: free what lives on the old one
+            cudaSetDevice(dev);
+            release();
+            for (auto& x : s) if (x) { cudaStreamDestroy(x); x = nullptr; }
+            if (sC) { cudaStreamDestroy(sC); sC = nullptr; }
+            for (auto e : ev) cudaEventDestroy(e);
+            ev.clear();
+            cudaSetDevice(d);
+        }
         for (int k = 0; k < 2; ++k)
             if ((ce = cudaStreamCreateWithFlags(&s[k], cudaStreamNonBlocking)) != cudaSuccess) return (int)ce;
         if ((ce = cudaStreamCreateWithFlags(&sC, cudaStreamNonBlocking)) != cudaSuccess) return (int)ce;
-        ev.clear();
         dev = d;
         return 0;
+    }
+    // everything of a pass must have left the arena before it is reused or the call returns
+    int drain()
+    {
+        cudaError_t e0 = cudaStreamSynchronize(sC), e1 = cudaStreamSynchronize(s[1]), e2 = cudaStreamSynchronize(s[0]);
+        return (int)(e0 != cudaSuccess ? e0 : (e1 != cudaSuccess ? e1 : e2));
     }
 };
 static thread_local HostPipe g_hpipe;
 
-// the host entry points cut a pass into up to PIPE_MAX_SUB sub-chunks for the duration of the call
-struct HostSubChunks {
-    int old;
-    HostSubChunks() : old(g_max_sub) { g_max_sub = PIPE_MAX_SUB; }
-    ~HostSubChunks() { g_max_sub = old; }
-};
+#define CUDA_TRY(call) do { cudaError_t ce_ = (call); if (ce_ != cudaSuccess) return (int)ce_; } while (0)
 
-// context of the copy hooks of letkf_syev_batched_host
-struct SyevHostCtx {
-    int M, per;                       // sub-chunk size of the pass
-    const double* hA; double* hw; double* hV; int* hinfo;      // host, at the start of the pass
-    double* dV; double* dw; int* dinfo;                          // device, at the start of the pass
-    cudaStream_t sD;                  // read-back stream
-    std::vector<cudaEvent_t>* evH;    // evH[k]: inputs of sub-chunk k are on the device
-    std::vector<cudaEvent_t>* evC;    // evC[k]: outputs of sub-chunk k are final
-};
-static int syev_host_pre(void* c, int b0, int, cudaStream_t s)
+// matrices per pass of a host call: what a staging arena of HOST_ARENA_CAP holds (or the test option)
+static const size_t HOST_ARENA_CAP = (size_t)16 << 30;
+static int host_pass_size(int batch, size_t bytes_per_matrix)
 {
-    SyevHostCtx* x = static_cast<SyevHostCtx*>(c);
-    return (int)cudaStreamWaitEvent(s, (*x->evH)[b0 / x->per], 0);
+    size_t c = t_opt.host_pass > 0 ? (size_t)t_opt.host_pass : HOST_ARENA_CAP / (bytes_per_matrix ? bytes_per_matrix : 1);
+    if (c < 1) c = 1;
+    if (c > (size_t)batch) c = (size_t)batch;
+    return (int)c;
 }
-static int syev_host_post(void* c, int b0, int nk, cudaStream_t s)
+
+// context of the copy hooks: the inputs of sub-chunk k have arrived when evH[k] fires; the outputs
+// listed here (per matrix / grid point: host base, device base, bytes) are read back after its last kernel
+struct HostCtx {
+    int per, nout;
+    char* host[4]; const char* dev[4]; size_t bytes[4];
+    cudaStream_t sD;
+    const cudaEvent_t* evH;
+    const cudaEvent_t* evC;
+    void add(void* h, const void* dv, size_t b) { host[nout] = static_cast<char*>(h); dev[nout] = static_cast<const char*>(dv); bytes[nout] = b; ++nout; }
+};
+static int host_pre(void* c, int b0, int, cudaStream_t s)
 {
-    SyevHostCtx* x = static_cast<SyevHostCtx*>(c);
-    const int M = x->M;
-    cudaEvent_t e = (*x->evC)[b0 / x->per];
-    cudaError_t ce;
-    if ((ce = cudaEventRecord(e, s)) != cudaSuccess) return (int)ce;
-    if ((ce = cudaStreamWaitEvent(x->sD, e, 0)) != cudaSuccess) return (int)ce;
-    if ((ce = cudaMemcpyAsync(x->hV + (size_t)b0 * M * M, x->dV + (size_t)b0 * M * M,
-                              sizeof(double) * (size_t)nk * M * M, cudaMemcpyDeviceToHost, x->sD)) != cudaSuccess) return (int)ce;
-    if ((ce = cudaMemcpyAsync(x->hw + (size_t)b0 * M, x->dw + (size_t)b0 * M,
-                              sizeof(double) * (size_t)nk * M, cudaMemcpyDeviceToHost, x->sD)) != cudaSuccess) return (int)ce;
-    if (x->hinfo &&
-        (ce = cudaMemcpyAsync(x->hinfo + b0, x->dinfo + b0, sizeof(int) * (size_t)nk, cudaMemcpyDeviceToHost, x->sD)) != cudaSuccess)
-        return (int)ce;
+    HostCtx* x = static_cast<HostCtx*>(c);
+    return (int)cudaStreamWaitEvent(s, x->evH[b0 / x->per], 0);
+}
+static int host_post(void* c, int b0, int nk, cudaStream_t s)
+{
+    HostCtx* x = static_cast<HostCtx*>(c);
+    cudaEvent_t e = x->evC[b0 / x->per];
+    CUDA_TRY(cudaEventRecord(e, s));
+    CUDA_TRY(cudaStreamWaitEvent(x->sD, e, 0));
+    for (int q = 0; q < x->nout; ++q)
+        CUDA_TRY(cudaMemcpyAsync(x->host[q] + (size_t)b0 * x->bytes[q], x->dev[q] + (size_t)b0 * x->bytes[q],
+                                 x->bytes[q] * (size_t)nk, cudaMemcpyDeviceToHost, x->sD));
     return 0;
 }
+struct HooksGuard {
+    explicit HooksGuard(const PassHooks* h) { t_hooks = h; }
+    ~HooksGuard() { t_hooks = nullptr; }
+};
 
 int letkf_syev_batched_host(const double* A, int M, int batch, double* w, double* V, int* info)
 {
+    EntryScope scope;
     g_launches = 0;
     if (M < 1 || M > LETKF_MAX_M) return -2;
     if (batch < 0) return -3;
@@ -814,14 +921,10 @@ int letkf_syev_batched_host(const double* A, int M, int batch, double* w, double
     if (!V) return -5;
     int rc = g_hpipe.init();
     if (rc) return rc;
-    // One pass of up to syev_chunk matrices lives on the device at a time.  Its sub-chunks (the
-    // ones the kernel pipeline uses) are copied in one after the other on the copy-in stream; each
-    // sub-chunk's first kernel waits for its own copy only, and its read-back starts on the
-    // copy-out stream as soon as its last kernel is done: both copy engines and the SMs overlap.
-    const int chunk = syev_chunk(M, batch);
     const size_t mat = sizeof(double) * (size_t)M * M, vec = sizeof(double) * (size_t)M;
-    Workspace ws;
-    const size_t wsb = align_up(carve(ws, nullptr, M, chunk), 256);
+    const int chunk = host_pass_size(batch, mat + vec + sizeof(int));
+    const Plan pl = make_plan(M, chunk, 0, 0);
+    const size_t wsb = align_up(syev_need(M, pl), 256);
     const size_t oV = 0, ow = align_up(mat * chunk, 256), oi = ow + align_up(vec * chunk, 256);
     const size_t owk = oi + align_up(sizeof(int) * (size_t)chunk, 256);
     if ((rc = g_hpipe.reserve(owk + wsb))) return rc;
@@ -829,33 +932,34 @@ int letkf_syev_batched_host(const double* A, int M, int batch, double* w, double
     double* dV = reinterpret_cast<double*>(base + oV);
     double* dw = reinterpret_cast<double*>(base + ow);
     int* dinfo = reinterpret_cast<int*>(base + oi);
-    carve(ws, base + owk, M, chunk);
     cudaStream_t sH = g_hpipe.s[0], sD = g_hpipe.s[1], sC = g_hpipe.sC;
     int launches = 0;
-    HostSubChunks max_sub_guard;
     for (int b0 = 0; b0 < batch && rc == 0; b0 += chunk) {
         const int n = (batch - b0 < chunk) ? batch - b0 : chunk;
-        int nsub, per;
+        const Plan pn = (n == chunk) ? pl : make_plan(M, n, 0, wsb);
         prof_reset(sC);
-        pass_partition(n, nsub, per);
-        g_hpipe.events(2 * nsub);
-        std::vector<cudaEvent_t> evH(g_hpipe.ev.begin(), g_hpipe.ev.begin() + nsub);
-        std::vector<cudaEvent_t> evC(g_hpipe.ev.begin() + nsub, g_hpipe.ev.begin() + 2 * nsub);
-        for (int k = 0, c0 = 0; c0 < n; ++k, c0 += per) {
-            const int nk = (n - c0 < per) ? n - c0 : per;
-            cudaMemcpyAsync(dV + (size_t)c0 * M * M, A + (size_t)(b0 + c0) * M * M, mat * nk, cudaMemcpyHostToDevice, sH);
-            cudaEventRecord(evH[k], sH);
+        if ((rc = g_hpipe.events(2 * (size_t)pn.nsub))) break;
+        const cudaEvent_t* evH = g_hpipe.ev.data();
+        const cudaEvent_t* evC = g_hpipe.ev.data() + pn.nsub;
+        for (int k = 0, c0 = 0; c0 < n && rc == 0; ++k, c0 += pn.per) {
+            const int nk = (n - c0 < pn.per) ? n - c0 : pn.per;
+            cudaError_t ce = cudaMemcpyAsync(dV + (size_t)c0 * M * M, A + (size_t)(b0 + c0) * M * M, mat * nk, cudaMemcpyHostToDevice, sH);
+            if (ce == cudaSuccess) ce = cudaEventRecord(evH[k], sH);
+            rc = (int)ce;
         }
-        cudaMemsetAsync(dinfo, 0, sizeof(int) * (size_t)n, sC);
-        SyevHostCtx ctx{M, per, A + (size_t)b0 * M * M, w + (size_t)b0 * M, V + (size_t)b0 * M * M,
-                        info ? info + b0 : nullptr, dV, dw, dinfo, sD, &evH, &evC};
-        PassHooks hooks{syev_host_pre, syev_host_post, &ctx};
-        rc = syev_pass(dV, M, n, dw, dV, dinfo, ws, sC, &hooks);     // in place
-        launches += g_launches;
-        // the arena is reused by the next pass: everything of this one must have left it
-        cudaStreamSynchronize(sC);
-        cudaStreamSynchronize(sD);
-        cudaStreamSynchronize(sH);
+        if (rc == 0) rc = (int)cudaMemsetAsync(dinfo, 0, sizeof(int) * (size_t)n, sC);
+        if (rc == 0) {
+            HostCtx ctx{pn.per, 0, {}, {}, {}, sD, evH, evC};
+            ctx.add(V + (size_t)b0 * M * M, dV, mat);
+            ctx.add(w + (size_t)b0 * M, dw, vec);
+            if (info) ctx.add(info + b0, dinfo, sizeof(int));
+            PassHooks hooks{host_pre, host_post, &ctx};
+            HooksGuard guard(&hooks);
+            rc = syev_core(dV, M, n, dw, dV, dinfo, base + owk, pn, sC);     // in place
+            launches += g_launches;
+        }
+        const int dr = g_hpipe.drain();
+        if (rc == 0) rc = dr;
     }
     cudaError_t ce = cudaGetLastError();
     if (rc == 0 && ce != cudaSuccess) rc = (int)ce;
@@ -863,36 +967,11 @@ int letkf_syev_batched_host(const double* A, int M, int batch, double* w, double
     return rc;
 }
 
-// context of the copy hooks of letkf_analysis_batched_host: up to four output arrays
-struct AnaHostCtx {
-    int per, nout;
-    char* host[4]; const char* dev[4]; size_t bytes[4];       // per grid point, at the start of the pass
-    cudaStream_t sD;
-    std::vector<cudaEvent_t>* evH;
-    std::vector<cudaEvent_t>* evC;
-};
-static int ana_host_pre(void* c, int b0, int, cudaStream_t s)
-{
-    AnaHostCtx* x = static_cast<AnaHostCtx*>(c);
-    return (int)cudaStreamWaitEvent(s, (*x->evH)[b0 / x->per], 0);
-}
-static int ana_host_post(void* c, int b0, int nk, cudaStream_t s)
-{
-    AnaHostCtx* x = static_cast<AnaHostCtx*>(c);
-    cudaEvent_t e = (*x->evC)[b0 / x->per];
-    cudaError_t ce;
-    if ((ce = cudaEventRecord(e, s)) != cudaSuccess) return (int)ce;
-    if ((ce = cudaStreamWaitEvent(x->sD, e, 0)) != cudaSuccess) return (int)ce;
-    for (int q = 0; q < x->nout; ++q)
-        if ((ce = cudaMemcpyAsync(x->host[q] + (size_t)b0 * x->bytes[q], x->dev[q] + (size_t)b0 * x->bytes[q],
-                                  x->bytes[q] * (size_t)nk, cudaMemcpyDeviceToHost, x->sD)) != cudaSuccess) return (int)ce;
-    return 0;
-}
-
 int letkf_analysis_batched_host(const double* Yb, const double* d, const double* rinv_loc,
                                 const double* Xb, int M, int p, int nstate, int batch, double rho,
                                 double* Xa, double* W, double* wbar, int* info)
 {
+    EntryScope scope;
     g_launches = 0;
     if (M < 2 || M > LETKF_MAX_M) return -5;
     if (p < 0) return -6;
@@ -907,14 +986,15 @@ int letkf_analysis_batched_host(const double* Yb, const double* d, const double*
     if (!Xa) return -10;
     int rc = g_hpipe.init();
     if (rc) return rc;
-    HostSubChunks max_sub_guard;
     // as letkf_syev_batched_host: one pass on the device at a time, inputs copied in sub-chunk by
     // sub-chunk, outputs read back as each sub-chunk's last kernel finishes
-    const int chunk = syev_chunk(M, batch);
     const size_t sYb = sizeof(double) * (size_t)p * M, sd = sizeof(double) * (size_t)p;
     const size_t sX = sizeof(double) * (size_t)nstate * M, sW = sizeof(double) * (size_t)M * M;
     const size_t sw = sizeof(double) * (size_t)M;
-    const size_t wsb = align_up(letkf_analysis_workspace_bytes(M, p, nstate, chunk), 256);
+    const int chunk = host_pass_size(batch, sYb + 2 * sd + sX + (W ? sW : 0) + sw + sizeof(int));
+    const size_t extra = analysis_extra(M, analysis_keepV(M, nstate, W != nullptr));
+    const Plan pl = make_plan(M, chunk, extra, 0);
+    const size_t wsb = align_up(analysis_need(M, pl, extra), 256);
     size_t off[8], total = 0;
     const size_t sizes[8] = {sYb * chunk, sd * chunk, sd * chunk, sX * chunk, W ? sW * chunk : 0,
                              wbar ? sw * chunk : 0, sizeof(int) * (size_t)chunk, wsb};
@@ -933,41 +1013,38 @@ int letkf_analysis_batched_host(const double* Yb, const double* d, const double*
     int launches = 0;
     for (int b0 = 0; b0 < batch && rc == 0; b0 += chunk) {
         const int n = (batch - b0 < chunk) ? batch - b0 : chunk;
-        int nsub, per;
-        pass_partition(n, nsub, per);
-        g_hpipe.events(2 * nsub);
-        std::vector<cudaEvent_t> evH(g_hpipe.ev.begin(), g_hpipe.ev.begin() + nsub);
-        std::vector<cudaEvent_t> evC(g_hpipe.ev.begin() + nsub, g_hpipe.ev.begin() + 2 * nsub);
-        for (int k = 0, c0 = 0; c0 < n; ++k, c0 += per) {
-            const int nk = (n - c0 < per) ? n - c0 : per;
+        const Plan pn = (n == chunk) ? pl : make_plan(M, n, extra, wsb);
+        prof_reset(sC);
+        if ((rc = g_hpipe.events(2 * (size_t)pn.nsub))) break;
+        const cudaEvent_t* evH = g_hpipe.ev.data();
+        const cudaEvent_t* evC = g_hpipe.ev.data() + pn.nsub;
+        for (int k = 0, c0 = 0; c0 < n && rc == 0; ++k, c0 += pn.per) {
+            const int nk = (n - c0 < pn.per) ? n - c0 : pn.per;
             const size_t g0 = (size_t)(b0 + c0);
+            cudaError_t ce = cudaSuccess;
             if (p > 0) {
-                cudaMemcpyAsync(dYb + (size_t)c0 * p * M, Yb + g0 * p * M, sYb * nk, cudaMemcpyHostToDevice, sH);
-                cudaMemcpyAsync(dd + (size_t)c0 * p, d + g0 * p, sd * nk, cudaMemcpyHostToDevice, sH);
-                cudaMemcpyAsync(dr + (size_t)c0 * p, rinv_loc + g0 * p, sd * nk, cudaMemcpyHostToDevice, sH);
+                ce = cudaMemcpyAsync(dYb + (size_t)c0 * p * M, Yb + g0 * p * M, sYb * nk, cudaMemcpyHostToDevice, sH);
+                if (ce == cudaSuccess) ce = cudaMemcpyAsync(dd + (size_t)c0 * p, d + g0 * p, sd * nk, cudaMemcpyHostToDevice, sH);
+                if (ce == cudaSuccess) ce = cudaMemcpyAsync(dr + (size_t)c0 * p, rinv_loc + g0 * p, sd * nk, cudaMemcpyHostToDevice, sH);
             }
-            cudaMemcpyAsync(dX + (size_t)c0 * nstate * M, Xb + g0 * nstate * M, sX * nk, cudaMemcpyHostToDevice, sH);
-            cudaEventRecord(evH[k], sH);
+            if (ce == cudaSuccess) ce = cudaMemcpyAsync(dX + (size_t)c0 * nstate * M, Xb + g0 * nstate * M, sX * nk, cudaMemcpyHostToDevice, sH);
+            if (ce == cudaSuccess) ce = cudaEventRecord(evH[k], sH);
+            rc = (int)ce;
         }
-        cudaMemsetAsync(dinfo, 0, sizeof(int) * (size_t)n, sC);
-        AnaHostCtx ctx;
-        ctx.per = per; ctx.sD = sD; ctx.evH = &evH; ctx.evC = &evC; ctx.nout = 0;
-        auto add = [&](void* h, const void* dv, size_t bytes) {
-            ctx.host[ctx.nout] = static_cast<char*>(h); ctx.dev[ctx.nout] = static_cast<const char*>(dv);
-            ctx.bytes[ctx.nout] = bytes; ++ctx.nout;
-        };
-        add(Xa + (size_t)b0 * nstate * M, dX, sX);
-        if (W) add(W + (size_t)b0 * M * M, dW, sW);
-        if (wbar) add(wbar + (size_t)b0 * M, dwb, sw);
-        if (info) add(info + b0, dinfo, sizeof(int));
-        PassHooks hooks{ana_host_pre, ana_host_post, &ctx};
-        g_analysis_hooks = &hooks;
-        rc = letkf_analysis_batched(dYb, dd, dr, dX, M, p, nstate, n, rho, dX, dW, dwb, dinfo, dwork, wsb, sC);
-        g_analysis_hooks = nullptr;
-        launches += g_launches;
-        cudaStreamSynchronize(sC);
-        cudaStreamSynchronize(sD);
-        cudaStreamSynchronize(sH);
+        if (rc == 0) rc = (int)cudaMemsetAsync(dinfo, 0, sizeof(int) * (size_t)n, sC);
+        if (rc == 0) {
+            HostCtx ctx{pn.per, 0, {}, {}, {}, sD, evH, evC};
+            ctx.add(Xa + (size_t)b0 * nstate * M, dX, sX);
+            if (W) ctx.add(W + (size_t)b0 * M * M, dW, sW);
+            if (wbar) ctx.add(wbar + (size_t)b0 * M, dwb, sw);
+            if (info) ctx.add(info + b0, dinfo, sizeof(int));
+            PassHooks hooks{host_pre, host_post, &ctx};
+            HooksGuard guard(&hooks);
+            rc = analysis_core(dYb, dd, dr, nullptr, dX, M, p, nstate, n, rho, dX, dW, dwb, dinfo, dwork, pn, extra, sC);
+            launches += g_launches;
+        }
+        const int dr_ = g_hpipe.drain();
+        if (rc == 0) rc = dr_;
     }
     cudaError_t ce = cudaGetLastError();
     if (rc == 0 && ce != cudaSuccess) rc = (int)ce;
@@ -982,6 +1059,7 @@ int letkf_analysis_grid_host(const double* Yf, const double* yo, const unsigned 
                              int loc_kind, double loc_scale, double sigma_o, double rho,
                              double* Xa, double* wbar, int* info)
 {
+    EntryScope scope;
     g_launches = 0;
     if (M < 2 || M > LETKF_MAX_M) return -5;
     if (V < 1) return -6;
@@ -999,14 +1077,17 @@ int letkf_analysis_grid_host(const double* Yf, const double* yo, const unsigned 
     if (!Xa) return -15;
     int rc = g_hpipe.init();
     if (rc) return rc;
-    HostSubChunks max_sub_guard;
     // The observation fields (V Ny Nx (M+1) doubles: 17 MB at 128 x 128 x 2 x 64) go in first, whole;
     // the background ensemble follows sub-chunk by sub-chunk and the analysis ensemble comes back
-    // the same way (hooks as in letkf_analysis_batched_host).
-    const int batch = Ny * Nx;
+    // the same way (hooks as in letkf_analysis_batched_host).  The whole grid is one pass.
+    const int batch = Ny * Nx, side = 2 * hw + 1, p = V * side * side;
     const size_t nobs = (size_t)V * batch;
     const size_t sX = sizeof(double) * (size_t)nstate * M, sw = sizeof(double) * (size_t)M;
     const size_t wsb = align_up(letkf_analysis_grid_workspace_bytes(M, V, Ny, Nx, hw, nstate), 256);
+    // the sub-chunk size the device call will use with this workspace (same rule, same inputs)
+    const size_t ybytes = align_up(sizeof(double) * nobs, 256);
+    const size_t extra = grid_extra(M, p, nstate) - (analysis_keepV(M, nstate, false) ? 0 : sizeof(double) * (size_t)M * M);
+    const Plan pl = make_plan(M, batch, extra, wsb - ybytes);
     size_t off[7], total = 0;
     const size_t sizes[7] = {sizeof(double) * nobs * M, sizeof(double) * nobs, obs_mask ? (size_t)batch : 0,
                              sX * batch, wbar ? sw * batch : 0, sizeof(int) * (size_t)batch, wsb};
@@ -1021,43 +1102,35 @@ int letkf_analysis_grid_host(const double* Yf, const double* yo, const unsigned 
     int* dinfo = reinterpret_cast<int*>(base + off[5]);
     void* dwork = base + off[6];
     cudaStream_t sH = g_hpipe.s[0], sD = g_hpipe.s[1], sC = g_hpipe.sC;
-    const int chunk = syev_chunk(M, batch);
-    if (chunk < batch) return -8;                      // one pass only (180 GB: > 10^6 points at M = 64)
-    int nsub, per;
-    pass_partition(batch, nsub, per);
-    g_hpipe.events(2 * nsub + 1);
-    std::vector<cudaEvent_t> evH(g_hpipe.ev.begin(), g_hpipe.ev.begin() + nsub);
-    std::vector<cudaEvent_t> evC(g_hpipe.ev.begin() + nsub, g_hpipe.ev.begin() + 2 * nsub);
-    cudaEvent_t evF = g_hpipe.ev[2 * nsub];
-    cudaMemcpyAsync(dYf, Yf, sizes[0], cudaMemcpyHostToDevice, sH);
-    cudaMemcpyAsync(dyo, yo, sizes[1], cudaMemcpyHostToDevice, sH);
-    if (obs_mask) cudaMemcpyAsync(dmask, obs_mask, sizes[2], cudaMemcpyHostToDevice, sH);
-    cudaEventRecord(evF, sH);
-    for (int k = 0, c0 = 0; c0 < batch; ++k, c0 += per) {
-        const int nk = (batch - c0 < per) ? batch - c0 : per;
-        cudaMemcpyAsync(dX + (size_t)c0 * nstate * M, Xb + (size_t)c0 * nstate * M, sX * nk, cudaMemcpyHostToDevice, sH);
-        cudaEventRecord(evH[k], sH);
-    }
-    cudaStreamWaitEvent(sC, evF, 0);                   // the fields before anything is gathered
-    cudaMemsetAsync(dinfo, 0, sizeof(int) * (size_t)batch, sC);
-    AnaHostCtx ctx;
-    ctx.per = per; ctx.sD = sD; ctx.evH = &evH; ctx.evC = &evC; ctx.nout = 0;
-    auto add = [&](void* h, const void* dv, size_t bytes) {
-        ctx.host[ctx.nout] = static_cast<char*>(h); ctx.dev[ctx.nout] = static_cast<const char*>(dv);
-        ctx.bytes[ctx.nout] = bytes; ++ctx.nout;
+    if ((rc = g_hpipe.events(2 * (size_t)pl.nsub + 1))) return rc;
+    const cudaEvent_t* evH = g_hpipe.ev.data();
+    const cudaEvent_t* evC = g_hpipe.ev.data() + pl.nsub;
+    cudaEvent_t evF = g_hpipe.ev[2 * (size_t)pl.nsub];
+    auto enqueue = [&]() -> int {
+        CUDA_TRY(cudaMemcpyAsync(dYf, Yf, sizes[0], cudaMemcpyHostToDevice, sH));
+        CUDA_TRY(cudaMemcpyAsync(dyo, yo, sizes[1], cudaMemcpyHostToDevice, sH));
+        if (obs_mask) CUDA_TRY(cudaMemcpyAsync(dmask, obs_mask, sizes[2], cudaMemcpyHostToDevice, sH));
+        CUDA_TRY(cudaEventRecord(evF, sH));
+        for (int k = 0, c0 = 0; c0 < batch; ++k, c0 += pl.per) {
+            const int nk = (batch - c0 < pl.per) ? batch - c0 : pl.per;
+            CUDA_TRY(cudaMemcpyAsync(dX + (size_t)c0 * nstate * M, Xb + (size_t)c0 * nstate * M, sX * nk, cudaMemcpyHostToDevice, sH));
+            CUDA_TRY(cudaEventRecord(evH[k], sH));
+        }
+        CUDA_TRY(cudaStreamWaitEvent(sC, evF, 0));                   // the fields before anything is gathered
+        CUDA_TRY(cudaMemsetAsync(dinfo, 0, sizeof(int) * (size_t)batch, sC));
+        HostCtx ctx{pl.per, 0, {}, {}, {}, sD, evH, evC};
+        ctx.add(Xa, dX, sX);
+        if (wbar) ctx.add(wbar, dwb, sw);
+        if (info) ctx.add(info, dinfo, sizeof(int));
+        PassHooks hooks{host_pre, host_post, &ctx};
+        HooksGuard guard(&hooks);
+        return letkf_analysis_grid(dYf, dyo, dmask, dX, M, V, Ny, Nx, nstate, hw, loc_kind, loc_scale, sigma_o, rho,
+                                   dX, dwb, dinfo, dwork, wsb, sC);
     };
-    add(Xa, dX, sX);
-    if (wbar) add(wbar, dwb, sw);
-    if (info) add(info, dinfo, sizeof(int));
-    PassHooks hooks{ana_host_pre, ana_host_post, &ctx};
-    g_analysis_hooks = &hooks;
-    rc = letkf_analysis_grid(dYf, dyo, dmask, dX, M, V, Ny, Nx, nstate, hw, loc_kind, loc_scale, sigma_o, rho,
-                             dX, dwb, dinfo, dwork, wsb, sC);
-    g_analysis_hooks = nullptr;
+    rc = enqueue();
     const int launches = g_launches;
-    cudaStreamSynchronize(sC);
-    cudaStreamSynchronize(sD);
-    cudaStreamSynchronize(sH);
+    const int dr = g_hpipe.drain();
+    if (rc == 0) rc = dr;
     cudaError_t ce = cudaGetLastError();
     if (rc == 0 && ce != cudaSuccess) rc = (int)ce;
     g_launches = launches;
@@ -1083,13 +1156,20 @@ int letkf_last_launch_count(void) { return g_launches; }
 int letkf_set_option(const char* name, int value)
 {
     if (!name) return -1;
-    if (strcmp(name, "force_generic") == 0) { g_force_generic = value != 0; return LETKF_OK; }
-    if (strcmp(name, "pipeline") == 0) { g_pipeline = value != 0; return LETKF_OK; }
-    if (strcmp(name, "sub_chunks") == 0) { g_max_sub = (value >= 1 && value <= PIPE_MAX_SUB) ? value : 8; return LETKF_OK; }
-    if (strcmp(name, "mid_reg") == 0) { g_mid_reg = (value >= 0 && value <= 2) ? value : 1; return LETKF_OK; }
-    if (strcmp(name, "split") == 0) { g_split = value != 0; return LETKF_OK; }
-    if (strcmp(name, "log_shrink") == 0) { g_log_shrink = value >= 1 ? value : 1; return LETKF_OK; }
-    if (strcmp(name, "ql_tpb") == 0) { g_ql_tpb = (value == 32 || value == 64 || value == 96) ? value : 0; return LETKF_OK; }
+    std::lock_guard<std::mutex> lk(g_options_mu);
+    Options& o = g_options;
+    if (strcmp(name, "force_generic") == 0) { o.force_generic = value != 0; return LETKF_OK; }
+    if (strcmp(name, "pipeline") == 0) { o.pipeline = value != 0; return LETKF_OK; }
+    if (strcmp(name, "sub_chunk") == 0) { o.sub_chunk = value >= 1 ? value : 0; return LETKF_OK; }
+    if (strcmp(name, "slots") == 0) { o.slots = value >= 2 ? value : 0; return LETKF_OK; }
+    if (strcmp(name, "log_slots") == 0) { o.log_slots = value >= 2 ? value : 0; return LETKF_OK; }
+    if (strcmp(name, "mid_reg") == 0) { o.mid_reg = (value >= 0 && value <= 2) ? value : 1; return LETKF_OK; }
+    if (strcmp(name, "log_shrink") == 0) { o.log_shrink = value >= 1 ? value : 1; return LETKF_OK; }
+    if (strcmp(name, "ql_tpb") == 0) { o.ql_tpb = (value == 32 || value == 64 || value == 96) ? value : 0; return LETKF_OK; }
+    if (strcmp(name, "two_pass") == 0) { o.two_pass = (value == 0 || value == 1) ? value : -1; return LETKF_OK; }
+    if (strcmp(name, "host_pass") == 0) { o.host_pass = value >= 1 ? value : 0; return LETKF_OK; }
+    if (strcmp(name, "qform") == 0) { o.qform = value != 0; return LETKF_OK; }
+    if (strcmp(name, "evec") == 0) { o.evec = value != 0; return LETKF_OK; }
     return -1;
 }
 

@@ -7,7 +7,12 @@ calls raise.  Names and argument order follow the C ABI one to one.
 import ctypes
 import os
 
-import torch
+# The sub-chunk pipeline of a call forks onto up to 22 private streams (2 tridiag, 4 apply, 16 QL);
+# with the default of 8 hardware work queues, streams that share a queue serialise.  Only effective
+# if set before the CUDA context is created, and never overrides the caller's own setting.
+os.environ.setdefault("CUDA_DEVICE_MAX_CONNECTIONS", "32")
+
+import torch  # noqa: E402
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libletkf.so")
@@ -110,6 +115,22 @@ def _dev_f64(t, name):
     return t
 
 
+def _out(t, name, shape, dev, dtype=torch.float64):
+    """A caller-supplied output: right device, dtype, exact shape, contiguous."""
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.device == dev and t.dtype == dtype
+            and t.is_contiguous() and tuple(t.shape) == tuple(shape)):
+        raise LetkfError(f"{name} must be a contiguous {dtype} CUDA tensor of shape {tuple(shape)} on {dev}")
+    return t
+
+
+def _work(work, dev, need):
+    if work is None:
+        return 0
+    if not (isinstance(work, torch.Tensor) and work.is_cuda and work.device == dev and work.is_contiguous()):
+        raise LetkfError(f"work must be a contiguous CUDA tensor on {dev}")
+    return work.numel() * work.element_size()      # (the library checks the size: smaller ones are legal)
+
+
 def version():
     return load().letkf_version()
 
@@ -143,9 +164,10 @@ def syev_batched(A, w=None, V=None, info=None, work=None, stream=None):
         V = torch.empty_like(A)
     if info is None:
         info = torch.zeros((batch,), dtype=torch.int32, device=A.device)
-    _dev_f64(w, "w")
-    _dev_f64(V, "V")
-    wb = work.numel() * work.element_size() if work is not None else 0
+    _out(w, "w", (batch, M), A.device)
+    _out(V, "V", (batch, M, M), A.device)
+    _out(info, "info", (batch,), A.device, torch.int32)
+    wb = _work(work, A.device, lib.letkf_syev_workspace_bytes(M, batch) if batch else 0)
     with torch.cuda.device(A.device):
         st = lib.letkf_syev_batched(_ptr(A), M, batch, _ptr(w), _ptr(V), _ptr(info),
                                     _ptr(work), wb, _stream(stream))
@@ -175,7 +197,13 @@ def analysis_batched(Yb, d, rinv_loc, Xb, rho, Xa=None, want_W=False, want_wbar=
         wbar = torch.empty((batch, M), dtype=torch.float64, device=dev)
     if info is None:
         info = torch.zeros((batch,), dtype=torch.int32, device=dev)
-    wb = work.numel() * work.element_size() if work is not None else 0
+    _out(Xa, "Xa", (batch, nstate, M), dev)
+    if W is not None:
+        _out(W, "W", (batch, M, M), dev)
+    if wbar is not None:
+        _out(wbar, "wbar", (batch, M), dev)
+    _out(info, "info", (batch,), dev, torch.int32)
+    wb = _work(work, dev, lib.letkf_analysis_workspace_bytes(M, p, nstate, batch) if batch else 0)
     with torch.cuda.device(dev):
         st = lib.letkf_analysis_batched(_ptr(Yb), _ptr(d), _ptr(rinv_loc), _ptr(Xb),
                                         M, p, nstate, batch, float(rho),
@@ -206,7 +234,9 @@ def analysis_grid(Yf, yo, Xb, hw, loc_kind, loc_scale, sigma_o, rho, obs_mask=No
     wbar = torch.empty((Ny * Nx, M), dtype=torch.float64, device=dev) if want_wbar else None
     if info is None:
         info = torch.zeros((Ny * Nx,), dtype=torch.int32, device=dev)
-    wb = work.numel() * work.element_size() if work is not None else 0
+    _out(Xa, "Xa", (Ny * Nx, nstate, M), dev)
+    _out(info, "info", (Ny * Nx,), dev, torch.int32)
+    wb = _work(work, dev, lib.letkf_analysis_grid_workspace_bytes(M, V, Ny, Nx, int(hw), nstate))
     with torch.cuda.device(dev):
         st = lib.letkf_analysis_grid(_ptr(Yf), _ptr(yo), _ptr(obs_mask), _ptr(Xb), M, V, Ny, Nx, nstate, int(hw),
                                      int(loc_kind), float(loc_scale), float(sigma_o), float(rho),

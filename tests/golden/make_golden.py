@@ -17,7 +17,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__)
 sys.path.insert(0, ROOT)
 
 import oracle  # noqa: E402
-from paper_2308_03310_b200 import workloads as wl  # noqa: E402
+from harness import workloads as wl  # noqa: E402
 
 
 def main():

@@ -5,7 +5,7 @@ import math
 import numpy as np
 import pytest
 
-from paper_2308_03310_b200 import workloads as wl
+from harness import workloads as wl
 import parity
 
 pytestmark = pytest.mark.gpu
@@ -46,6 +46,37 @@ def test_analysis_vs_oracle(lk, oracle, M, p, ns, batch):
     ref = run_oracle(oracle, inp)
     assert (out["info"] == 0).all()
     parity.assert_analysis(out, ref, inp["Xb"], f"M={M} p={p} ns={ns}")
+
+
+@pytest.mark.parametrize("want_W", [True, False])
+@pytest.mark.parametrize("M,batch", [(128, 4), (160, 3), (192, 3), (256, 2)])
+def test_analysis_large_ensembles(lk, oracle, M, batch, want_W):
+    """LETKF_MAX_M = 256 applies to the analysis call as well: the paths above the register kernels
+    (shared-memory resident up to 160, any-M kernels beyond), with the transform matrix requested
+    and not."""
+    inp = wl.analysis_inputs(batch=batch, M=M, p=98, nstate=9, config_index=430 + M)
+    out = run_gpu(lk, inp, want_W=want_W, want_wbar=True)
+    ref = run_oracle(oracle, inp)
+    assert (out["info"] == 0).all()
+    assert (out["W"] is not None) == want_W
+    parity.assert_analysis(out, ref, inp["Xb"], f"M={M} W={want_W}")
+
+
+@pytest.mark.parametrize("opt", ["qform", "evec"])
+@pytest.mark.parametrize("M,p,ns", [(64, 98, 9), (48, 49, 9), (20, 7, 3), (64, 98, 15)])
+def test_fused_analysis_other_forms(lk, oracle, M, p, ns, opt):
+    """The fused epilogue behind the other forms of the apply kernel: explicit Q (qform = 1) and
+    replayed rotations only (evec = 0); the default is covered by test_fused_epilogue_vs_oracle."""
+    inp = wl.analysis_inputs(batch=70, M=M, p=p, nstate=ns, config_index=450 + M)
+    try:
+        lk.set_option(opt, 1 if opt == "qform" else 0)
+        out = run_gpu(lk, inp, want_W=False, want_wbar=True)
+    finally:
+        lk.set_option("qform", 0)
+        lk.set_option("evec", 1)
+    ref = run_oracle(oracle, inp)
+    assert (out["info"] == 0).all()
+    parity.assert_analysis(out, ref, inp["Xb"], f"{opt} M={M}")
 
 
 def test_without_optional_outputs_and_in_place(lk, oracle):
@@ -165,15 +196,19 @@ def test_fused_epilogue_vs_oracle(lk, oracle, M, p, ns, batch):
     parity.assert_analysis(out, full, inp["Xb"], f"fused vs unfused M={M} p={p} ns={ns}")
 
 
-def test_fused_analysis_on_the_slow_path(lk, oracle):
-    """Log overflow inside the fused analysis: fast_apply<epilogue> skips the flagged points, the
-    finisher completes their EVD and generic_epilogue(flagged) their a6-a9."""
+@pytest.mark.parametrize("opts", [{"evec": 0}, {"qform": 1}])
+def test_fused_analysis_on_the_slow_path(lk, oracle, opts):
+    """A rotation log too short for the matrix inside the fused analysis: fast_apply<epilogue> runs the
+    classic iteration for those points itself (LETKF_INFO_SLOWPATH) and carries on with a6-a9."""
     inp = wl.analysis_inputs(batch=150, M=64, p=98, nstate=9, config_index=45)
     ref = run_oracle(oracle, inp)
     try:
+        for k, v in opts.items():
+            lk.set_option(k, v)
         lk.set_option("log_shrink", 3)
         out = run_gpu(lk, inp, want_W=False, want_wbar=True)
     finally:
-        lk.set_option("log_shrink", 1)
+        for k, v in (("log_shrink", 1), ("evec", 1), ("qform", 0)):
+            lk.set_option(k, v)
     assert ((out["info"] & 0xFFFF) == 0).all() and (out["info"] & lk.INFO_SLOWPATH).astype(bool).all()
     parity.assert_analysis(out, ref, inp["Xb"], "fused analysis, slow path")

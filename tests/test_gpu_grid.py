@@ -3,7 +3,7 @@ and the localisation function fused in front of the local analysis) against the 
 import numpy as np
 import pytest
 
-from paper_2308_03310_b200 import workloads as wl
+from harness import workloads as wl
 import parity
 
 pytestmark = pytest.mark.gpu

@@ -3,7 +3,7 @@ inputs.  PAPER.md:142, 183 (EVD by Householder + QL); tolerances of north_star /
 import numpy as np
 import pytest
 
-from paper_2308_03310_b200 import workloads as wl
+from harness import workloads as wl
 import parity
 
 pytestmark = pytest.mark.gpu
@@ -244,7 +244,7 @@ def test_pipelined_equals_single_stream(lk):
     st.synchronize()
     assert torch.equal(w0, w1) and torch.equal(V0, V1) and torch.equal(i0, i1)
     assert torch.isfinite(s)
-    assert lk.last_launch_count() >= 4 * 4               # >= 4 sub-chunks x 4 kernels
+    assert lk.last_launch_count() >= 4 * 3               # >= 4 sub-chunks x 3 kernels
 
 
 @pytest.mark.parametrize("pinned", [True, False])
@@ -265,14 +265,17 @@ def test_host_entry_point_equals_device_call(lk, pinned):
 @pytest.mark.parametrize("M,batch", [(64, 2100), (48, 300), (100, 12)])
 def test_log_overflow_slow_path(lk, oracle, M, batch):
     """With the rotation log shrunk the QL kernel flags matrices whose log would overflow and the
-    finisher (classic in-kernel QL on the stored Q) completes them: same tolerances, and info
-    carries LETKF_INFO_SLOWPATH for exactly those matrices."""
+    classic iteration completes them (inside the apply kernel for M <= 64, in the finisher on the
+    stored Q above): same tolerances, and info carries LETKF_INFO_SLOWPATH for exactly those
+    matrices."""
     A = wl.letkf_shaped(batch, M, 98 if M >= 64 else 49, config_index=930 + M)
     try:
         lk.set_option("log_shrink", 3)
+        lk.set_option("evec", 0)                          # (M <= 64: every matrix through the log)
         w, V, info = run_gpu(lk, A)
     finally:
         lk.set_option("log_shrink", 1)
+        lk.set_option("evec", 1)
     assert ((info & 0xFFFF) == 0).all()
     assert (info & lk.INFO_SLOWPATH).astype(bool).all(), "every matrix should have taken the slow path"
     wo, _, _, _ = oracle.syev_batched(A[:64])
@@ -337,19 +340,216 @@ def test_mid_tridiagonalisation_both_forms(lk, oracle, M, mode):
     parity.assert_evd(A, w, V, wo, f"mid M={M} mid_reg={mode}")
 
 
-@pytest.mark.parametrize("M", [64, 57, 49])
-def test_split_tridiagonalisation_option(lk, oracle, M):
-    """letkf_set_option("split", 1): pivots down to 33, the trailing 32 x 32 problem and the explicit
-    Q as three kernels (experimental) -- same tolerances."""
-    A = wl.letkf_shaped(300, M, 98, config_index=940 + M)
+VARIANTS = {"direct": {}, "replay": {"evec": 0}, "qform": {"qform": 1}}
+
+
+@pytest.mark.parametrize("variant", sorted(VARIANTS))
+@pytest.mark.parametrize("M,p", [(64, 98), (57, 98), (48, 49), (33, 49), (16, 49), (5, 49), (64, 3), (64, 48), (64, 0)])
+def test_register_path_variants(lk, oracle, M, p, variant):
+    """The three forms of the M <= 64 path.  "direct" (default): the reduction
+    kernel keeps the reflectors, the QL kernel finds the eigenvalues and classifies the matrix, the
+    apply kernel forms the eigenvectors of T by twisted factorisations where the spectrum allows
+    (else it replays the logged rotations on the identity) and does the back-transform
+    V = H_{M-1} ... H_1 Z.  "replay" (evec = 0): always the logged rotations.  "qform" (qform = 1):
+    the explicit Q is formed by the reduction kernel and the rotations are replayed on its rows.
+    Each also with the rotation log shrunk, which sends the replaying matrices to the classic
+    iteration inside the apply kernel."""
+    A = wl.letkf_shaped(150, M, p, config_index=990 + M + p)
     try:
-        lk.set_option("split", 1)
+        for k, v in VARIANTS[variant].items():
+            lk.set_option(k, v)
         w, V, info = run_gpu(lk, A)
+        lk.set_option("log_shrink", 4)
+        w2, V2, info2 = run_gpu(lk, A)
     finally:
-        lk.set_option("split", 0)
+        for k, v in (("qform", 0), ("evec", 1), ("log_shrink", 1)):
+            lk.set_option(k, v)
     assert (info == 0).all()
     wo, _, _, _ = oracle.syev_batched(A)
-    parity.assert_evd(A, w, V, wo, f"split M={M}")
+    parity.assert_evd(A, w, V, wo, f"{variant} M={M}")
+    parity.assert_evd(A, w2, V2, wo, f"{variant}, log shrunk, M={M}")
+    assert ((info2 & 0xFFFF) == 0).all()
+    if p >= M - 1 and M >= 16 and variant != "direct":
+        assert (info2 & lk.INFO_SLOWPATH).astype(bool).all()
+
+
+def test_direct_eigenvectors_are_used_and_fall_back(lk, oracle):
+    """Which matrices take which route: well separated spectra (config 3) need no rotation at all
+    (the profile counts none); a spectrum with eigenvalues closer than 1e-8 ||T|| inside one
+    unreduced block (Wilkinson's W21+, pairs agreeing to 1e-14) has its rotations logged and
+    replayed; both meet the tolerances."""
+    import torch
+    A = wl.letkf_shaped(256, 64, 98, config_index=3)
+    k = 10
+    Wk = np.diag(np.abs(np.arange(21) - k).astype(float)) + np.diag(np.ones(20), 1) + np.diag(np.ones(20), -1)
+    B = np.stack([Wk] * 40)
+    for X, expect_rot in ((A, False), (B, True)):
+        Xt = torch.from_numpy(X).cuda()
+        lk.profile_enable(1)
+        try:
+            w, V, info = lk.syev_batched(Xt)
+            torch.cuda.synchronize()
+            nrot = lk.profile_rotations()
+        finally:
+            lk.profile_enable(0)
+        assert int(info.abs().max()) == 0
+        assert (nrot > 0) == expect_rot
+        wo, _, _, _ = oracle.syev_batched(X)
+        parity.assert_evd(X, w.cpu().numpy(), V.cpu().numpy(), wo, "direct / replay routes")
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("M,p", [(64, 98), (57, 98), (33, 49), (16, 49), (64, 3), (96, 98), (200, 98)])
+def test_ql_one_and_two_pass(lk, oracle, M, p, mode):
+    """letkf_set_option("two_pass", 0 / 1): the QL iteration logged in one pass (Wilkinson shifts) or
+    with a second pass shifted by the eigenvalues of the first: both are
+    orthogonal similarities of the same tridiagonal matrix -- same tolerances.  By default the
+    batch size picks one (large batches: two passes)."""
+    A = wl.letkf_shaped(150 if M <= 64 else 7, M, p, config_index=940 + M + p)
+    try:
+        lk.set_option("two_pass", mode)
+        w, V, info = run_gpu(lk, A)
+    finally:
+        lk.set_option("two_pass", -1)
+    assert (info == 0).all()
+    wo, _, _, _ = oracle.syev_batched(A)
+    parity.assert_evd(A, w, V, wo, f"two_pass={mode} M={M}")
+
+
+@pytest.mark.parametrize("M,batch,sub,slots", [(64, 1000, 64, 2), (32, 777, 128, 3), (100, 150, 32, 2), (64, 4133, 0, 0)])
+def test_workspace_ring(lk, oracle, M, batch, sub, slots):
+    """The sub-chunk pipeline keeps `slots` sub-chunks in flight, each in a slot of the workspace that
+    the next tenant takes over when its last kernel is done (Streams).  With a
+    small sub-chunk and few slots every slot is reused many times: results must equal the
+    one-stream run bitwise (ragged last sub-chunk included)."""
+    import torch
+    A = wl.letkf_shaped(batch, M, 98 if M >= 64 else 49, config_index=970 + M)
+    At = torch.from_numpy(A).cuda()
+    try:
+        lk.set_option("two_pass", 1)
+        lk.set_option("pipeline", 0)
+        w0, V0, i0 = lk.syev_batched(At)
+        torch.cuda.synchronize()
+        lk.set_option("pipeline", 1)
+        lk.set_option("sub_chunk", sub)
+        lk.set_option("slots", slots)
+        work = torch.empty(lk.syev_workspace_bytes(M, batch), dtype=torch.uint8, device="cuda")
+        w1, V1, i1 = lk.syev_batched(At, work=work)
+        w2, V2, i2 = lk.syev_batched(At, work=work)      # back to back on the same workspace
+        torch.cuda.synchronize()
+    finally:
+        for k, v in (("pipeline", 1), ("sub_chunk", 0), ("slots", 0), ("two_pass", -1)):
+            lk.set_option(k, v)
+    assert int(i1.abs().max()) == 0
+    assert torch.equal(w0, w1) and torch.equal(V0, V1) and torch.equal(w0, w2) and torch.equal(V0, V2)
+    sel = slice(0, 48)
+    wo, _, _, _ = oracle.syev_batched(A[sel])
+    parity.assert_evd(A[sel], w1[sel].cpu().numpy(), V1[sel].cpu().numpy(), wo, f"ring M={M}")
+
+
+def test_workspace_smaller_than_recommended(lk):
+    """Any workspace that holds at least one matrix is accepted: the call then keeps fewer
+    sub-chunks in flight, or runs chunk after chunk on the caller's stream; one that holds none is
+    refused (argument 7)."""
+    import torch
+    A = torch.from_numpy(wl.letkf_shaped(3000, 64, 98, config_index=975)).cuda()
+    w0, V0, _ = lk.syev_batched(A)
+    full = lk.syev_workspace_bytes(64, 3000)
+    for frac in (0.5, 0.1):
+        work = torch.empty(int(full * frac), dtype=torch.uint8, device="cuda")
+        lib = lk.load()
+        import ctypes
+        w = torch.empty_like(w0); V = torch.empty_like(V0); info = torch.zeros(3000, dtype=torch.int32, device="cuda")
+        st = lib.letkf_syev_batched(ctypes.c_void_p(A.data_ptr()), 64, 3000, ctypes.c_void_p(w.data_ptr()),
+                                    ctypes.c_void_p(V.data_ptr()), ctypes.c_void_p(info.data_ptr()),
+                                    ctypes.c_void_p(work.data_ptr()), work.numel(),
+                                    ctypes.c_void_p(torch.cuda.current_stream().cuda_stream))
+        assert st == 0
+        torch.cuda.synchronize()
+        assert torch.equal(w, w0) and torch.equal(V, V0)
+    tiny = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    st = lib.letkf_syev_batched(ctypes.c_void_p(A.data_ptr()), 64, 3000, ctypes.c_void_p(w.data_ptr()),
+                                ctypes.c_void_p(V.data_ptr()), ctypes.c_void_p(info.data_ptr()),
+                                ctypes.c_void_p(tiny.data_ptr()), 1024,
+                                ctypes.c_void_p(torch.cuda.current_stream().cuda_stream))
+    assert st == -7
+
+
+def test_host_entry_point_in_passes(lk, oracle):
+    """The host entry points process a batch that exceeds the staging arena in passes
+    (letkf_set_option("host_pass", n) forces small ones): three passes with a ragged last one, arena
+    and workspace reused pass after pass."""
+    import torch
+    A = torch.from_numpy(wl.letkf_shaped(2 * 1100 + 311, 64, 98, config_index=976))
+    try:
+        lk.set_option("host_pass", 1100)
+        lk.set_option("two_pass", 1)
+        w, V, info = lk.syev_batched_host(A.pin_memory())
+        wd, Vd, _ = lk.syev_batched(A.cuda())
+        torch.cuda.synchronize()
+    finally:
+        lk.set_option("host_pass", 0)
+        lk.set_option("two_pass", -1)
+    assert int(info.abs().max()) == 0
+    assert torch.equal(w, wd.cpu()) and torch.equal(V, Vd.cpu())
+
+
+def test_two_host_threads(lk, oracle):
+    """The library keeps its streams, events and staging arena per host thread and snapshots the
+    options once per call: two threads drive it at the same time on streams of their own (one the
+    EVD, one the fused analysis) while the main thread flips an option the calls must not see
+    half-way (a call that changed path between its stages would return garbage)."""
+    import threading
+    import torch
+    A = torch.from_numpy(wl.letkf_shaped(3000, 64, 98, config_index=977)).cuda()
+    inp = wl.analysis_inputs(batch=2500, M=64, p=98, nstate=9, config_index=978)
+    t = {k: torch.from_numpy(inp[k]).cuda() for k in ("Yb", "d", "rinv_loc", "Xb")}
+    w0, V0, _ = lk.syev_batched(A)
+    Xa0 = lk.analysis_batched(t["Yb"], t["d"], t["rinv_loc"], t["Xb"], inp["rho"])["Xa"]
+    torch.cuda.synchronize()
+    out, err = {}, []
+
+    def evd():
+        try:
+            st = torch.cuda.Stream()
+            for _ in range(6):
+                out["evd"] = lk.syev_batched(A, stream=st)
+            st.synchronize()
+        except Exception as ex:      # pragma: no cover
+            err.append(ex)
+
+    def ana():
+        try:
+            st = torch.cuda.Stream()
+            for _ in range(6):
+                out["ana"] = lk.analysis_batched(t["Yb"], t["d"], t["rinv_loc"], t["Xb"], inp["rho"], stream=st)
+            st.synchronize()
+        except Exception as ex:      # pragma: no cover
+            err.append(ex)
+
+    th = [threading.Thread(target=evd), threading.Thread(target=ana)]
+    for x in th:
+        x.start()
+    for k in range(400):                                  # an option that switches the kernel family and the
+        lk.set_option("force_generic", k & 1)             # meaning of the V buffer between the stages
+    for x in th:
+        x.join()
+    lk.set_option("force_generic", 0)
+    assert not err, err
+    # each call ran entirely on one path or the other: valid to tolerance either way
+    w1, V1, i1 = out["evd"]
+    assert int(i1.abs().max()) == 0
+    Af = torch.tril(A) + torch.tril(A, -1).transpose(1, 2)
+    R = torch.matmul(Af, V1) - V1 * w1.unsqueeze(1)
+    assert float((R.flatten(1).norm(dim=1) / Af.flatten(1).norm(dim=1)).max()) <= parity.TOL_RES
+    G = torch.matmul(V1.transpose(1, 2), V1) - torch.eye(64, dtype=torch.float64, device="cuda")
+    assert float(G.abs().max()) <= parity.TOL_ORTH
+    assert float((w1 - w0).abs().max() / w0.abs().max()) <= parity.TOL_W
+    Xa1 = out["ana"]["Xa"]
+    xbar = t["Xb"].mean(dim=2, keepdim=True)
+    num = (Xa1 - Xa0).flatten(1).norm(dim=1)
+    den = (Xa0 - xbar).flatten(1).norm(dim=1)
+    assert float((num / den).max()) <= parity.TOL_ANALYSIS
 
 
 @pytest.mark.parametrize("M", [16, 32, 96, 128, 192, 256])

@@ -4,7 +4,7 @@ Procedure 1 lines 1-2).  CPU only."""
 import numpy as np
 import pytest
 
-from paper_2308_03310_b200 import workloads as wl
+from harness import workloads as wl
 
 
 def gather_numpy(Yf, yo, mask, hw, weight):

@@ -9,7 +9,7 @@ import math
 import numpy as np
 import pytest
 
-from paper_2308_03310_b200 import workloads as wl
+from harness import workloads as wl
 
 EPS = np.finfo(np.float64).eps
 
