@@ -197,10 +197,23 @@ __device__ __forceinline__ int ql_next_sweep(QLState& st, double* d, double* e, 
     }
 }
 
-// Ascending insertion sort of d with the permutation that sorts it (stable).
+// Ascending insertion sort of d with the permutation that sorts it.  The QL iteration tends to
+// leave the eigenvalues in roughly descending order (insertion sort's worst case: it was 28% of the
+// classifying QL kernel), so a sequence with more descents than ascents is reversed first.
 __device__ __forceinline__ void sort_eigenvalues(double* d, int dstride, int* perm, int pstride, int M)
 {
-    for (int k = 0; k < M; ++k) perm[(size_t)k * pstride] = k;
+    int desc = 0;
+    for (int k = 0; k + 1 < M; ++k) desc += d[(size_t)k * dstride] > d[(size_t)(k + 1) * dstride] ? 1 : 0;
+    if (2 * desc > M) {
+        for (int k = 0; k < M / 2; ++k) {
+            const double t = d[(size_t)k * dstride];
+            d[(size_t)k * dstride] = d[(size_t)(M - 1 - k) * dstride];
+            d[(size_t)(M - 1 - k) * dstride] = t;
+        }
+        for (int k = 0; k < M; ++k) perm[(size_t)k * pstride] = M - 1 - k;
+    } else {
+        for (int k = 0; k < M; ++k) perm[(size_t)k * pstride] = k;
+    }
     for (int k = 1; k < M; ++k) {
         const double val = d[(size_t)k * dstride];
         const int pk = perm[(size_t)k * pstride];

@@ -312,7 +312,7 @@ template <int TPB>
 static int ql_run(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st, int mode)
 {
     cudaError_t ce;
-    const size_t ql_smem = sizeof(double) * 2 * (size_t)M * TPB;
+    const size_t ql_smem = sizeof(double) * 2 * (size_t)M * TPB + 24 * (size_t)TPB;   // (d, e) per lane + the sort's bookkeeping
     if ((ce = allow_smem(ql_log_kernel<TPB>, ql_smem)) != cudaSuccess) return (int)ce;
     const int per_cta = mode == QL_TWO_PASS ? TPB / 2 : TPB;  // two lanes per matrix when the iteration runs twice side by side
     const int qblocks = (n + per_cta - 1) / per_cta;
@@ -322,9 +322,12 @@ static int ql_run(int M, int n, double* w, int* info, Workspace ws, cudaStream_t
 
 static int stage_QL(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st, int mode)
 {
-    int tpb = t_opt.ql_tpb ? t_opt.ql_tpb : (M <= 64 ? 64 : 32);
-    while (tpb > 32 && sizeof(double) * 2 * (size_t)M * tpb > 200 * 1024) tpb -= 32;
+    int tpb = t_opt.ql_tpb ? t_opt.ql_tpb : (M <= 64 ? 128 : 32);
+    while (tpb > 32 && (sizeof(double) * 2 * (size_t)M + 24) * tpb > 200 * 1024) tpb -= 32;
+    if (mode == QL_CLASSIFY && tpb < 64) tpb = 64;      // the classifier wants one lane per eigenvalue (M <= 64)
     switch (tpb) {
+        case 192: return ql_run<192>(M, n, w, info, ws, st, mode);
+        case 128: return ql_run<128>(M, n, w, info, ws, st, mode);
         case 96: return ql_run<96>(M, n, w, info, ws, st, mode);
         case 64: return ql_run<64>(M, n, w, info, ws, st, mode);
         default: return ql_run<32>(M, n, w, info, ws, st, mode);
@@ -1165,7 +1168,7 @@ int letkf_set_option(const char* name, int value)
     if (strcmp(name, "log_slots") == 0) { o.log_slots = value >= 2 ? value : 0; return LETKF_OK; }
     if (strcmp(name, "mid_reg") == 0) { o.mid_reg = (value >= 0 && value <= 2) ? value : 1; return LETKF_OK; }
     if (strcmp(name, "log_shrink") == 0) { o.log_shrink = value >= 1 ? value : 1; return LETKF_OK; }
-    if (strcmp(name, "ql_tpb") == 0) { o.ql_tpb = (value == 32 || value == 64 || value == 96) ? value : 0; return LETKF_OK; }
+    if (strcmp(name, "ql_tpb") == 0) { o.ql_tpb = (value == 32 || value == 64 || value == 96 || value == 128 || value == 192) ? value : 0; return LETKF_OK; }
     if (strcmp(name, "two_pass") == 0) { o.two_pass = (value == 0 || value == 1) ? value : -1; return LETKF_OK; }
     if (strcmp(name, "host_pass") == 0) { o.host_pass = value >= 1 ? value : 0; return LETKF_OK; }
     if (strcmp(name, "qform") == 0) { o.qform = value != 0; return LETKF_OK; }

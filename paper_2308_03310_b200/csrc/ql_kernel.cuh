@@ -112,30 +112,6 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
         for (int k = 0; k < M - 1; ++k)
             if (fabs(QL_E(k)) <= fmax(eps * (fabs(QL_D(k)) + fabs(QL_D(k + 1))), thr)) bmask |= 1ull << k;
     }
-    // Classification (end of the first pass; d = eigenvalues by position).  Returns true when the
-    // apply kernel can form the eigenvectors itself; leaves d sorted and the permutation in e.
-    auto classify = [&]() -> bool {
-        for (int k = 0; k < M; ++k) s1g[k] = QL_D(k);
-        sort_eigenvalues(d, QL_TPB, reinterpret_cast<int*>(e), QL_TPB * 2, M);
-        const int* pm = reinterpret_cast<const int*>(e);
-        const double nrm = thr * 9007199254740992.0;                      // max_i(|d_i| + |e_i|)
-        const double tiny = GV_TINY * nrm, gap = GV_GAP * nrm;
-        auto single = [&](int pos_) {                                     // 1 x 1 block: its eigenvector is a unit vector
-            const bool lo_cut = pos_ == 0 || ((bmask >> (pos_ - 1)) & 1ull);
-            const bool hi_cut = pos_ == M - 1 || ((bmask >> pos_) & 1ull);
-            return lo_cut && hi_cut;
-        };
-        bool ok = true;
-        bool sprev = single(pm[0]);
-        for (int k = 0; k + 1 < M; ++k) {
-            const bool snext = single(pm[(k + 1) * stride * 2]);
-            const double dk = QL_D(k);
-            if (QL_D(k + 1) - dk < tiny && !(sprev && snext)) ok = false;
-            if (k + GV_PH + 1 < M && QL_D(k + GV_PH + 1) - dk < gap) ok = false;
-            sprev = snext;
-        }
-        return ok;
-    };
     int l = 0, m = 0, iter = 0, fail = 0;
     int overflow = 0, nsw = 0, pos = 0;
     bool done = !valid;
@@ -150,11 +126,7 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
         while (!done) {
             if (m == l) {                              // eigenvalue l has converged
                 l += 1; iter = 0;
-                if (l >= M) {
-                    if (mode == QL_CLASSIFY) easy = classify();   // (else the logging kernel follows)
-                    done = true;
-                    break;
-                }
+                if (l >= M) { done = true; break; }
                 m = scan_end(l);
                 continue;
             }
@@ -293,27 +265,66 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
     }
 #undef QL_D
 #undef QL_E
+    // ---- the eigenvalues of every matrix of the CTA are sorted by ALL its lanes together (rank of
+    // lambda_k = number of eigenvalues below it: no dependent chain; one lane sorting its own matrix
+    // by insertion was 28% of this kernel), and in QL_CLASSIFY the sorted sequence is classified on
+    // the way (common.cuh, GV_*): easy unless two eigenvalues that are not both 1 x 1 blocks are
+    // closer than GV_TINY ||T||, or more than GV_PH lie within GV_GAP ||T|| above one.
     const bool owner = valid && (!two_pass || (lane & 1));   // the lane that reports the matrix
+    unsigned long long* bm_sh = reinterpret_cast<unsigned long long*>(sm + 2 * (size_t)M * QL_TPB);   // [QL_TPB]
+    double* thr_sh = reinterpret_cast<double*>(bm_sh + QL_TPB);                                        // [QL_TPB]
+    int* sort_sh = reinterpret_cast<int*>(thr_sh + QL_TPB);                                            // [QL_TPB]
+    sort_sh[lane] = (owner && !overflow) ? 1 : 0;
+    bm_sh[lane] = bmask;
+    thr_sh[lane] = thr;
+    __syncthreads();
+    for (int c = 0; c < nb; ++c) {
+        const int col = two_pass ? 2 * c + 1 : c;
+        if (!sort_sh[col]) continue;                          // (uniform)
+        const size_t bc = (size_t)(b0 + c);
+        const double* dc = dsm + col;
+        double* ec = esm + col;
+        int myrank = -1;
+        for (int k = lane; k < M; k += QL_TPB) {
+            const double v = dc[k * stride];
+            int rank = 0;
+            for (int j = 0; j < M; ++j) {
+                const double u = dc[j * stride];
+                rank += (u < v || (u == v && j < k)) ? 1 : 0;
+            }
+            w[bc * M + rank] = v;
+            ws.perm[bc * M + rank] = k;
+            if (mode == QL_CLASSIFY) { ws.s1[bc * M + k] = v; ec[rank * stride] = v; myrank = rank; }
+        }
+        if (mode == QL_CLASSIFY) {                            // (M <= 64 <= QL_TPB: one eigenvalue per lane)
+            __syncthreads();
+            const unsigned long long bmc = bm_sh[col];
+            if (lane < M) {
+                const bool lo_cut = lane == 0 || ((bmc >> (lane - 1)) & 1ull);
+                const bool hi_cut = lane == M - 1 || ((bmc >> lane) & 1ull);
+                dsm[myrank * stride + col] = (lo_cut && hi_cut) ? 1.0 : 0.0;   // 1 x 1 block: its eigenvector is a unit vector
+            }
+            __syncthreads();
+            bool hard = false;
+            if (lane + 1 < M) {
+                const double nrm = thr_sh[col] * 9007199254740992.0;               // max_i(|d_i| + |e_i|)
+                const double dk = ec[lane * stride];
+                const bool both_single = dc[lane * stride] != 0.0 && dc[(lane + 1) * stride] != 0.0;
+                if (ec[(lane + 1) * stride] - dk < GV_TINY * nrm && !both_single) hard = true;
+                if (lane + GV_PH + 1 < M && ec[(lane + GV_PH + 1) * stride] - dk < GV_GAP * nrm) hard = true;
+            }
+            const int anyhard = __syncthreads_or(hard ? 1 : 0);
+            if (lane == col) easy = !anyhard;
+        }
+    }
     if (owner) {
-        if (!overflow && mode != QL_CLASSIFY) sort_eigenvalues(d, QL_TPB, reinterpret_cast<int*>(e), QL_TPB * 2, M);
         ws.nsweeps[b] = nsw;
         ws.flags[b] = overflow ? FLAG_SLOW : (mode == QL_CLASSIFY ? (easy ? FLAG_GETVEC : FLAG_PENDING) : FLAG_REPLAY);
         if (info && !overflow) info[b] = fail;
     }
-    __syncthreads();
     if (ws.rot_counter) {
         const int tot = __reduce_add_sync(FULL, (valid && logging) ? pos : 0);
         if ((lane & 31) == 0) atomicAdd(ws.rot_counter, (unsigned long long)tot);
-    }
-    // coalesced store of w and perm (matrices that overflowed are rewritten by the slow path)
-    const int* psm = reinterpret_cast<const int*>(esm);
-    for (int idx = lane; idx < nmc * M; idx += QL_TPB) {
-        const int bb = idx / M, ii = idx - bb * M;
-        const int col = two_pass ? 2 * bb + 1 : bb;
-        if (bb < nb && (mode != QL_LOGPASS || ws.flags[b0 + bb] == FLAG_REPLAY)) {   // (LOGPASS: only what it redid;
-            w[(size_t)b0 * M + idx] = dsm[ii * QL_TPB + col];                       //  an overflow there keeps the
-            ws.perm[(size_t)b0 * M + idx] = psm[(ii * QL_TPB + col) * 2];           //  classifier's values)
-        }
     }
 }
 
