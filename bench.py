@@ -27,12 +27,25 @@ if ROOT not in sys.path:
 
 METRIC = "batched fp64 syev matrices/s at M=64 (batch 16384); % of FP64/HBM roofline"
 M_HEAD, BATCH_HEAD, P_HEAD = 64, 16384, 98
-# dram__bytes_read.sum + dram__bytes_write.sum per whole-batch launch (config 3) from the ncu --set full
-# capture kept in profiles/r01e_ncu_key_metrics.txt (bytes; ncu runs are never timed)
-NCU_DRAM_BYTES = {"fast_tridiag_formq": 0.537097e9 + 0.503998e9, "ql_log_kernel": 0.030428e9 + 1.099897e9,
-                  "fast_apply": 1.681331e9 + 0.501880e9}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel per launch, from the one ncu --set full
+# capture of this round (profiles/r02_ncu_key_metrics.txt names the command; ncu runs are never timed).  The
+# capture launches the kernel on TRAFFIC_LAUNCH_MATRICES matrices; bench.py scales it to its own launch size.
+NCU_DRAM_BYTES = {}          # filled from profiles/r02_traffic.txt when present ("kernel bytes matrices" per line)
 SM_COUNT = 148
 DFMA_PER_CLK_SM = 64          # fp64 FMA lanes per SM (4 SMSPs x 16), DESIGN.md section 6
+
+
+def ncu_traffic(kernel, matrices):
+    """dram bytes of one launch of `kernel` over `matrices` matrices, scaled from the committed ncu capture."""
+    path = os.path.join(ROOT, "profiles", "r02_traffic.txt")
+    try:
+        for line in open(path):
+            f = line.split()
+            if len(f) >= 3 and not line.startswith("#") and f[0] == kernel:
+                return float(f[1]) * matrices / float(f[2])
+    except OSError:
+        pass
+    return None
 
 
 def host_cores():
@@ -301,34 +314,46 @@ def run_ours(args):
     clocks = sampler.stop()
     ms_total = max_over_ranks(e0.elapsed_time(e1))
     ms_step = ms_total / args.steps
-    # per-kernel durations: 3 more steps with letkf_profile_enable(1) -- one chunk on the caller's
-    # stream, CUDA events around every kernel on that stream, i.e. each kernel timed alone
+    # per-kernel durations: 3 more steps with letkf_profile_enable(1) -- chunk after chunk on the caller's
+    # stream with a workspace that holds the whole batch, i.e. ONE launch per kernel, each timed alone by
+    # CUDA events on that stream
+    work_all = torch.empty(letkf.syev_workspace_bytes(M, 1) * B, dtype=torch.uint8, device="cuda")
     letkf.profile_enable(True)
     nprof = 3
-    rot_total = 0
+    rot_total = direct_total = 0
+    nlaunch = {}
     for _ in range(nprof):
-        step()
+        letkf.syev_batched(A, w=w, V=V, info=info, work=work_all, stream=stream)
         for name, ms in letkf.profile_records():
             kern.setdefault(name, []).append(ms)
+            nlaunch[name] = nlaunch.get(name, 0) + 1
         rot_total = letkf.profile_rotations()
+        direct_total = letkf.profile_direct()
     letkf.profile_enable(False)
+    del work_all
     kern_ms = {k: float(np.sum(v) / nprof) for k, v in kern.items()}
+    launches_alone = {k: v // nprof for k, v in nlaunch.items()}
     rot_per_matrix = rot_total / float(B)
+    direct_frac = direct_total / float(B)
     value = world * B / (ms_step * 1e-3)
 
-    # ---- roofline of the dominant kernel
+    # ---- roofline of the dominant kernel.  Flops per matrix, as the kernels do them:
+    #   fast_tridiag   4/3 M^3                       Householder reduction (the reflectors are kept, no explicit Q)
+    #   ql_log_kernel  30 flops per rotation step    (scalar recurrences; latency bound, not a roofline kernel)
+    #   fast_apply     2 M^3 back-transform + 6 M R  (R logged rotations replayed) + 60 M^2 for a matrix whose
+    #                  eigenvectors come from twisted factorisations (5 passes of ~12 flops per entry)
     sm_max = clocks.get("sm_max_mhz") or 1965.0
-    peak_tflops = SM_COUNT * DFMA_PER_CLK_SM * 2 * sm_max * 1e6 / 1e12
-    flops_by_kernel = {}
+    peak_derived = SM_COUNT * DFMA_PER_CLK_SM * 2 * sm_max * 1e6 / 1e12
+    flops_per_matrix = {}
     for k in kern_ms:
         if "tridiag" in k:
-            flops_by_kernel[k] = (8.0 / 3.0) * M ** 3 * B
+            flops_per_matrix[k] = (4.0 / 3.0) * M ** 3
         elif "apply" in k:
-            flops_by_kernel[k] = 6.0 * M * rot_per_matrix * B
+            flops_per_matrix[k] = 2.0 * M ** 3 + 6.0 * M * rot_per_matrix + 60.0 * M * M * direct_frac
         elif "ql" in k:
-            flops_by_kernel[k] = 30.0 * rot_per_matrix * B
+            flops_per_matrix[k] = 30.0 * 1.05 * M * M
     dom = max(kern_ms, key=kern_ms.get)
-    dom_flops = flops_by_kernel.get(dom, 0.0)
+    dom_flops = flops_per_matrix.get(dom, 0.0) * B
     achieved = dom_flops / (kern_ms[dom] * 1e-3) / 1e12
     peaks = {}
     try:
@@ -337,31 +362,52 @@ def run_ours(args):
         pass
     hbm_peak = peaks.get("hbm_gbs", 6650.0)
 
-    # measured DFMA rate (context for the derived peak)
+    # the fp64 peak, measured in this run: MEASURED_PEAKS.json has no fp64 entry and the profiling guide no
+    # fp64 nominal, so the roofline denominator is the library's own DFMA probe (8 independent FMA chains per
+    # thread, 8 CTAs of 256 threads per SM), timed here with CUDA events
     nfma, _ = letkf.probe_dfma(SM_COUNT * 8, 256, 2048)
     torch.cuda.synchronize()
-    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    p0.record(stream)
-    nfma, _ = letkf.probe_dfma(SM_COUNT * 8, 256, 2048)
-    p1.record(stream)
-    torch.cuda.synchronize()
-    dfma_measured = 2.0 * nfma / (p0.elapsed_time(p1) * 1e-3) / 1e12
+    best = 0.0
+    for _ in range(3):
+        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        p0.record(stream)
+        nfma, _ = letkf.probe_dfma(SM_COUNT * 8, 256, 2048)
+        p1.record(stream)
+        torch.cuda.synchronize()
+        best = max(best, 2.0 * nfma / (p0.elapsed_time(p1) * 1e-3) / 1e12)
+    peak_measured = best
 
+    algorithmic_bytes = {"fast_tridiag": (8.0 * M * M + 8.0 * (M * M / 2 + 3 * M)) * B,        # A in; reflectors, d, e out
+                         "ql_log_kernel": (16.0 * M + 12.0 * M + 16.0 * rot_per_matrix) * B,
+                         "fast_apply": (8.0 * (M * M / 2 + 4 * M) + 16.0 * rot_per_matrix + 8.0 * M * M) * B}
+    step_tflops = syev_model_flops(M) * B / (ms_step * 1e-3) / 1e12
+    counted = (4.0 / 3.0) * M ** 3 + 2.0 * M ** 3 + 6.0 * M * rot_per_matrix + 60.0 * M * M * direct_frac
     roofline = {
-        "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-        "frac": achieved / peak_tflops, "traffic": NCU_DRAM_BYTES.get(dom),
-        "traffic_unit": "bytes per launch (whole batch), ncu dram read+write, profiles/r01e_ncu_key_metrics.txt",
-        "algorithmic_bytes": {"fast_tridiag_formq": 16.0 * M * M * B, "ql_log_kernel": 16.0 * rot_per_matrix * B,
-                              "fast_apply": (16.0 * M * M + 16.0 * rot_per_matrix) * B}.get(dom),
-        "peak_source": f"derived: {SM_COUNT} SMs x {DFMA_PER_CLK_SM} DFMA/clk x 2 x {sm_max:.0f} MHz (DESIGN.md 6)",
-        "dfma_probe_tflops": dfma_measured,
+        "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_measured, "unit": "TFLOP/s",
+        "frac": achieved / peak_measured,
+        "peak_source": "measured in this run: letkf_probe_dfma (fp64 FMA, 148 x 8 CTAs x 256 threads x 8 chains), CUDA events",
+        "peak_derived": peak_derived,
+        "peak_derived_source": f"{SM_COUNT} SMs x {DFMA_PER_CLK_SM} DFMA/clk x 2 x {sm_max:.0f} MHz (DESIGN.md 5)",
+        "frac_of_derived": achieved / peak_derived,
+        "flops_per_launch": dom_flops, "matrices_per_launch": B, "launches_timed_alone": launches_alone.get(dom),
+        "traffic": ncu_traffic(dom, B),
+        "traffic_unit": "bytes per launch (whole batch): ncu dram read+write of profiles/r02_traffic.txt scaled to this launch; null = no capture committed",
+        "algorithmic_bytes": algorithmic_bytes.get(dom),
         "kernel_ms": kern_ms, "kernel_share": {k: v / sum(kern_ms.values()) for k, v in kern_ms.items()},
-        "rotations_per_matrix": rot_per_matrix,
-        "flops_counted_per_matrix": (8.0 / 3.0) * M ** 3 + 6.0 * M * rot_per_matrix,
-        "step_model_9M3": {"achieved": syev_model_flops(M) * B / (ms_step * 1e-3) / 1e12,
-                           "frac": syev_model_flops(M) * B / (ms_step * 1e-3) / 1e12 / peak_tflops},
+        "kernel_flops_per_matrix": flops_per_matrix,
+        "kernel_frac_of_measured_peak": {k: flops_per_matrix[k] * B / (kern_ms[k] * 1e-3) / 1e12 / peak_measured
+                                         for k in kern_ms if k in flops_per_matrix},
+        "rotations_per_matrix": rot_per_matrix, "direct_eigenvector_fraction": direct_frac,
+        "flops_counted_per_matrix": counted,
+        "step_counted": {"achieved": counted * B / (ms_step * 1e-3) / 1e12,
+                         "frac_of_measured": counted * B / (ms_step * 1e-3) / 1e12 / peak_measured},
+        "step_model_9M3": {"achieved": step_tflops, "frac_of_measured": step_tflops / peak_measured,
+                           "frac_of_derived": step_tflops / peak_derived,
+                           "note": "9 M^3 is SURVEY.md 8(d)'s textbook model of Householder + QL with accumulated rotations + back-transform; "
+                                   "the path does flops_counted_per_matrix (no rotation is applied where the eigenvectors of T are formed directly)"},
         "step_hbm": {"achieved_gbs": syev_bytes(M) * B / (ms_step * 1e-3) / 1e9,
                      "peak_gbs": hbm_peak, "frac": syev_bytes(M) * B / (ms_step * 1e-3) / 1e9 / hbm_peak},
+        "workspace_bytes": int(work.numel()),
     }
 
     # ---- end to end through the C ABI with HOST buffers (letkf_syev_batched_host): pinned inputs
@@ -429,11 +475,16 @@ def run_ours(args):
                 "workload": "config4: letkf_analysis_batched fp64 M=64 p=98 nstate=9, 128x128 grid points, W not requested",
                 "value": B / (ams * 1e-3), "unit": "grid points/s", "ms_per_step": ams,
                 "gpu_launches_per_step": letkf.last_launch_count(),
-                "model_tflops": fl * B / (ams * 1e-3) / 1e12, "frac_of_fp64_peak": fl * B / (ams * 1e-3) / 1e12 / peak_tflops,
+                "model_tflops": fl * B / (ams * 1e-3) / 1e12, "frac_of_measured_fp64_peak": fl * B / (ams * 1e-3) / 1e12 / peak_measured,
+                "workspace_bytes": int(awork.numel()),
                 "hbm_gbs": analysis_bytes(M, p, 9) * B / (ams * 1e-3) / 1e9}
             letkf.profile_enable(True)
             astep()
-            line["analysis"]["kernel_ms"] = {k: round(v, 4) for k, v in letkf.profile_records()}
+            akern = {}
+            for k, v in letkf.profile_records():
+                akern[k] = akern.get(k, 0.0) + v
+            line["analysis"]["kernel_ms"] = {k: round(v, 4) for k, v in akern.items()}
+            line["analysis"]["direct_eigenvector_fraction"] = letkf.profile_direct() / float(B)
             letkf.profile_enable(False)
             # end to end through letkf_analysis_batched_host (pinned host buffers, PCIe inside)
             hp = {k: torch.from_numpy(inp[k]).pin_memory() for k in ("Yb", "d", "rinv_loc", "Xb")}
@@ -518,7 +569,8 @@ def run_ours(args):
                 sms = e0.elapsed_time(e1) / nrep
                 tf = syev_model_flops(Ms) * Bs / (sms * 1e-3) / 1e12
                 sweep.append({"M": Ms, "batch": Bs, "ms": round(sms, 4), "matrices_per_s": Bs / (sms * 1e-3),
-                              "model_9M3_tflops": round(tf, 3), "frac_of_fp64_peak": round(tf / peak_tflops, 4),
+                              "model_9M3_tflops": round(tf, 3), "frac_of_measured_fp64_peak": round(tf / peak_measured, 4),
+                              "workspace_bytes": int(wk.numel()),
                               "path": "registers (fast_*)" if Ms <= 64 else ("registers + shared memory (mid_*)" if Ms <= 160 else "global/L2 (generic_*)"),
                               "info_nonzero": int((infos != 0).sum())})
                 del As, Vs, ws_, wk, infos

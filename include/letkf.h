@@ -199,6 +199,9 @@ int letkf_profile_count(void);
 int letkf_profile_record(int idx, const char** name, float* ms);
 int letkf_profile_record_start(int idx, float* ms_from_first);
 long long letkf_profile_rotations(void);
+/* SYNCHRONISES; number of matrices of the last profiled call whose eigenvectors came from twisted
+ * factorisations (no rotation logged or replayed) */
+long long letkf_profile_direct(void);
 
 /* Number of kernels the last compute call on this host thread enqueued (bench.py's
  * gpu_launches claim is counted from this, not guessed). */

@@ -41,8 +41,8 @@ static void prof_reset(cudaStream_t st)
     g_prof.recs.clear();
     g_prof.used = 0;
     if (g_prof.on) {
-        if (!g_prof.d_rot) cudaMalloc(&g_prof.d_rot, sizeof(unsigned long long));
-        cudaMemsetAsync(g_prof.d_rot, 0, sizeof(unsigned long long), st);
+        if (!g_prof.d_rot) cudaMalloc(&g_prof.d_rot, 2 * sizeof(unsigned long long));   // [0] rotations, [1] direct matrices
+        cudaMemsetAsync(g_prof.d_rot, 0, 2 * sizeof(unsigned long long), st);
     }
 }
 static void prof_begin(const char* name, cudaStream_t st)
@@ -159,7 +159,7 @@ struct Plan { int per, nslot, nlog, nsub; bool pipelined, two_pass; int ql_mode;
 static const int PIPE_MIN_SUB = 512;     // smallest sub-chunk worth launches of its own
 static const int PIPE_MAX_SUBS = 16;     // sub-chunks per call (bounds the launch count)
 static const int PIPE_SLOTS = 16;        // default number of sub-chunks in flight: all of them
-static const int PIPE_LOG_MATS = 4096;   // default number of matrices that hold a slot of the rotation log
+static const size_t PIPE_LOG_BYTES = (size_t)288 << 20;   // default size of the log slots together
 static const int NQ_STREAMS = 16;
 
 static int round_up(int x, int a) { return (x + a - 1) / a * a; }
@@ -188,7 +188,8 @@ static Plan make_plan(int M, int batch, size_t extra, size_t avail)
         int nsub = (batch + per - 1) / per;
         int nslot = t_opt.slots > 0 ? t_opt.slots : PIPE_SLOTS;
         if (nslot > nsub) nslot = nsub;
-        int nlog = t_opt.log_slots > 0 ? t_opt.log_slots : (PIPE_LOG_MATS + per - 1) / per;
+        const size_t log_entry = sizeof(double2) * (size_t)log_capacity(M, pl.two_pass) + sizeof(uint32_t) * (size_t)sweep_capacity(M);
+        int nlog = t_opt.log_slots > 0 ? t_opt.log_slots : (int)((PIPE_LOG_BYTES + log_entry * per - 1) / (log_entry * per));
         if (nlog < 2) nlog = 2;
         if (nlog > nslot) nlog = nslot;
         if (avail) {                       // a smaller workspace: fewer log slots first, then fewer slots
@@ -1214,6 +1215,14 @@ long long letkf_profile_rotations(void)
     if (!g_prof.d_rot) return -1;
     unsigned long long v = 0;
     if (cudaMemcpy(&v, g_prof.d_rot, sizeof(v), cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+    return (long long)v;
+}
+
+long long letkf_profile_direct(void)
+{
+    if (!g_prof.d_rot) return -1;
+    unsigned long long v = 0;
+    if (cudaMemcpy(&v, g_prof.d_rot + 1, sizeof(v), cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
     return (long long)v;
 }
 

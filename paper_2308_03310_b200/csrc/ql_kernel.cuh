@@ -325,6 +325,8 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
     if (ws.rot_counter) {
         const int tot = __reduce_add_sync(FULL, (valid && logging) ? pos : 0);
         if ((lane & 31) == 0) atomicAdd(ws.rot_counter, (unsigned long long)tot);
+        const int ne = __reduce_add_sync(FULL, (owner && easy) ? 1 : 0);
+        if ((lane & 31) == 0 && ne) atomicAdd(ws.rot_counter + 1, (unsigned long long)ne);
     }
 }
 

@@ -25,7 +25,7 @@ EXPORTS = (
     "letkf_syev_batched_host", "letkf_analysis_batched_host", "letkf_host_release",
     "letkf_analysis_grid", "letkf_analysis_grid_workspace_bytes", "letkf_analysis_grid_host",
     "letkf_probe_dfma", "letkf_last_launch_count",
-    "letkf_profile_enable", "letkf_profile_count", "letkf_profile_record", "letkf_profile_record_start", "letkf_profile_rotations",
+    "letkf_profile_enable", "letkf_profile_count", "letkf_profile_record", "letkf_profile_record_start", "letkf_profile_rotations", "letkf_profile_direct",
     "letkf_set_option", "letkf_status_string", "letkf_version",
 )
 
@@ -82,6 +82,8 @@ def load():
     lib.letkf_profile_record_start.restype = ci
     lib.letkf_profile_rotations.argtypes = []
     lib.letkf_profile_rotations.restype = ctypes.c_longlong
+    lib.letkf_profile_direct.argtypes = []
+    lib.letkf_profile_direct.restype = ctypes.c_longlong
     lib.letkf_set_option.argtypes = [ctypes.c_char_p, ci]
     lib.letkf_set_option.restype = ci
     lib.letkf_status_string.argtypes = [ci]
@@ -367,6 +369,10 @@ def profile_records():
 
 def profile_rotations():
     return load().letkf_profile_rotations()
+
+
+def profile_direct():
+    return load().letkf_profile_direct()
 
 
 def set_option(name, value):
