@@ -13,6 +13,7 @@
 #include "ql_kernel.cuh"
 #include "generic_kernels.cuh"
 #include "fast_kernels.cuh"
+#include "bisect_kernel.cuh"
 #include "mid_kernels.cuh"
 
 namespace letkf {
@@ -89,6 +90,8 @@ struct Options {
     int qform = 0;           // M <= 64: 1 = explicit Q formed by the reduction kernel and replayed on (through the
                              // output buffer); 0 = reflectors kept, eigenvectors of T formed in the apply kernel,
                              // which then does the back-transform (nothing but the reflectors crosses HBM in between)
+    int bisect = -1;         // M <= 64, evec = 1: eigenvalues by multisection with M threads per matrix instead of the QL
+                             // kernel's one (the latency regime): -1 = for batches up to BISECT_MAX_BATCH, 0 / 1
     int evec = 1;            // M <= 64, qform = 0: 1 = eigenvectors of T by twisted factorisations where the spectrum
                              // allows (ql_log_kernel classifies), the logged rotations otherwise; 0 = always the log
 };
@@ -155,7 +158,8 @@ static Workspace ws_slice(const Workspace& w, int M, int b0, int l0)
 // tridiag -> QL -> apply over private streams, at most `nslot` of them in flight (a slot of the
 // workspace each).  Not pipelined (small batches, pipeline = 0, kernel-alone profiling): chunks of
 // `per` matrices one after the other on the caller's stream.
-struct Plan { int per, nslot, nlog, nsub; bool pipelined, two_pass; int ql_mode; };
+struct Plan { int per, nslot, nlog, nsub; bool pipelined, two_pass; int ql_mode; bool bisect; };
+static const int BISECT_MAX_BATCH = 1024;
 static const int PIPE_MIN_SUB = 512;     // smallest sub-chunk worth launches of its own
 static const int PIPE_MAX_SUBS = 16;     // sub-chunks per call (bounds the launch count)
 static const int PIPE_SLOTS = 16;        // default number of sub-chunks in flight: all of them
@@ -179,6 +183,7 @@ static Plan make_plan(int M, int batch, size_t extra, size_t avail)
     pl.two_pass = t_opt.two_pass >= 0 ? t_opt.two_pass != 0 : ((long)batch * M >= (1L << 18));
     pl.ql_mode = pl.two_pass ? QL_TWO_PASS : QL_ONE_PASS;
     if (use_getvec(M)) { pl.ql_mode = QL_CLASSIFY; pl.two_pass = true; }   // (a logged pass is always the second one)
+    pl.bisect = use_getvec(M) && (t_opt.bisect >= 0 ? t_opt.bisect != 0 : batch <= BISECT_MAX_BATCH);
     const bool want_pipe = t_opt.pipeline && (!g_prof.on || g_prof.keep_pipeline) && batch >= 2 * PIPE_MIN_SUB;
     auto bytes_for = [&](size_t n, size_t nl) { return plan_bytes(M, n, nl, extra, pl.two_pass); };
     if (want_pipe) {
@@ -189,7 +194,10 @@ static Plan make_plan(int M, int batch, size_t extra, size_t avail)
         int nslot = t_opt.slots > 0 ? t_opt.slots : PIPE_SLOTS;
         if (nslot > nsub) nslot = nsub;
         const size_t log_entry = sizeof(double2) * (size_t)log_capacity(M, pl.two_pass) + sizeof(uint32_t) * (size_t)sweep_capacity(M);
-        int nlog = t_opt.log_slots > 0 ? t_opt.log_slots : (int)((PIPE_LOG_BYTES + log_entry * per - 1) / (log_entry * per));
+        // where every matrix logs its rotations (M > 64, or evec = 0) each slot has its log; where most
+        // matrices never do (the eigenvector path of M <= 64) the log slots share a fixed budget
+        int nlog = t_opt.log_slots > 0 ? t_opt.log_slots
+                 : (pl.ql_mode == QL_CLASSIFY ? (int)((PIPE_LOG_BYTES + log_entry * per - 1) / (log_entry * per)) : nslot);
         if (nlog < 2) nlog = 2;
         if (nlog > nslot) nlog = nslot;
         if (avail) {                       // a smaller workspace: fewer log slots first, then fewer slots
@@ -315,7 +323,7 @@ static int ql_run(int M, int n, double* w, int* info, Workspace ws, cudaStream_t
     cudaError_t ce;
     const size_t ql_smem = sizeof(double) * 2 * (size_t)M * TPB + 24 * (size_t)TPB;   // (d, e) per lane + the sort's bookkeeping
     if ((ce = allow_smem(ql_log_kernel<TPB>, ql_smem)) != cudaSuccess) return (int)ce;
-    const int per_cta = mode == QL_TWO_PASS ? TPB / 2 : TPB;  // two lanes per matrix when the iteration runs twice side by side
+    const int per_cta = (mode == QL_TWO_PASS || mode == QL_LOGPASS_PAIRED) ? TPB / 2 : TPB;  // two lanes per matrix when the iteration runs twice side by side
     const int qblocks = (n + per_cta - 1) / per_cta;
     KLAUNCH("ql_log_kernel", st, ql_log_kernel<TPB><<<qblocks, TPB, ql_smem, st>>>(ws, M, n, w, info, mode));
     return 0;
@@ -335,10 +343,23 @@ static int stage_QL(int M, int n, double* w, int* info, Workspace ws, cudaStream
     }
 }
 
-// the logging pass of the matrices QL_CLASSIFY left pending (the first kernel to touch the log slot)
-static int stage_QLlog(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st)
+// a4 for small batches (bisect_kernel.cuh): eigenvalues by multisection, M threads per matrix, then the
+// same classification as QL_CLASSIFY
+static int stage_bisect(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st)
 {
-    return stage_QL(M, n, w, info, ws, st, QL_LOGPASS);
+    switch (fast_bucket(M)) {
+        case 16: KLAUNCH("bisect_classify_kernel", st, bisect_classify_kernel<16><<<n, FastCfg<16>::NT, 0, st>>>(ws, M, w, info)); break;
+        case 32: KLAUNCH("bisect_classify_kernel", st, bisect_classify_kernel<32><<<n, FastCfg<32>::NT, 0, st>>>(ws, M, w, info)); break;
+        case 48: KLAUNCH("bisect_classify_kernel", st, bisect_classify_kernel<48><<<n, FastCfg<48>::NT, 0, st>>>(ws, M, w, info)); break;
+        default: KLAUNCH("bisect_classify_kernel", st, bisect_classify_kernel<64><<<n, FastCfg<64>::NT, 0, st>>>(ws, M, w, info)); break;
+    }
+    return 0;
+}
+
+// the logging pass of the matrices QL_CLASSIFY left pending (the first kernel to touch the log slot)
+static int stage_QLlog(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st, bool paired)
+{
+    return stage_QL(M, n, w, info, ws, st, paired ? QL_LOGPASS_PAIRED : QL_LOGPASS);
 }
 
 static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws, cudaStream_t st,
@@ -584,7 +605,8 @@ static int syev_core(const double* A, int M, int batch, double* w, double* V, in
         return stage_T(A + (size_t)b0 * M * M, M, nk, V + (size_t)b0 * M * M, ws_slice(ws, M, s0, l0), s, nullptr);
     };
     auto stageQL = [&](int b0, int nk, int s0, int l0, cudaStream_t s, bool logpass) {
-        if (logpass) return stage_QLlog(M, nk, w + (size_t)b0 * M, info ? info + b0 : nullptr, ws_slice(ws, M, s0, l0), s);
+        if (logpass) return stage_QLlog(M, nk, w + (size_t)b0 * M, info ? info + b0 : nullptr, ws_slice(ws, M, s0, l0), s, pl.bisect);
+        if (pl.bisect) return stage_bisect(M, nk, w + (size_t)b0 * M, info ? info + b0 : nullptr, ws_slice(ws, M, s0, l0), s);
         return stage_QL(M, nk, w + (size_t)b0 * M, info ? info + b0 : nullptr, ws_slice(ws, M, s0, l0), s, pl.ql_mode);
     };
     auto stageAP = [&](int b0, int nk, int s0, int l0, cudaStream_t s) {
@@ -706,7 +728,8 @@ static int analysis_core(const double* Yb, const double* d, const double* rinv_l
         return stage_T(Vk, M, nk, Vk, ws_slice(ws, M, s0, l0), s, &ga);
     };
     auto stageQL = [&](int b0, int nk, int s0, int l0, cudaStream_t s, bool logpass) {
-        if (logpass) return stage_QLlog(M, nk, lam + (size_t)s0 * M, info ? info + b0 : nullptr, ws_slice(ws, M, s0, l0), s);
+        if (logpass) return stage_QLlog(M, nk, lam + (size_t)s0 * M, info ? info + b0 : nullptr, ws_slice(ws, M, s0, l0), s, pl.bisect);
+        if (pl.bisect) return stage_bisect(M, nk, lam + (size_t)s0 * M, info ? info + b0 : nullptr, ws_slice(ws, M, s0, l0), s);
         return stage_QL(M, nk, lam + (size_t)s0 * M, info ? info + b0 : nullptr, ws_slice(ws, M, s0, l0), s, pl.ql_mode);
     };
     // a6-a9: fused into fast_apply when W is not wanted (V then never leaves the SM); the any-M
@@ -1174,6 +1197,7 @@ int letkf_set_option(const char* name, int value)
     if (strcmp(name, "host_pass") == 0) { o.host_pass = value >= 1 ? value : 0; return LETKF_OK; }
     if (strcmp(name, "qform") == 0) { o.qform = value != 0; return LETKF_OK; }
     if (strcmp(name, "evec") == 0) { o.evec = value != 0; return LETKF_OK; }
+    if (strcmp(name, "bisect") == 0) { o.bisect = (value == 0 || value == 1) ? value : -1; return LETKF_OK; }
     return -1;
 }
 

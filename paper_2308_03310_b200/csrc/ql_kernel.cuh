@@ -36,7 +36,9 @@ namespace letkf {
 // ws.s1 and the matrix is marked FLAG_PENDING.  QL_LOGPASS (a second launch, the first one that needs
 // the matrix's slot of the rotation log) runs the logging pass of the pending matrices, shifted by
 // those eigenvalues (-> FLAG_REPLAY); a CTA without a pending matrix leaves at once.
-constexpr int QL_ONE_PASS = 0, QL_TWO_PASS = 1, QL_CLASSIFY = 2, QL_LOGPASS = 3;
+constexpr int QL_ONE_PASS = 0, QL_TWO_PASS = 1, QL_CLASSIFY = 2, QL_LOGPASS = 3, QL_LOGPASS_PAIRED = 4;
+// (QL_LOGPASS_PAIRED: the pending matrices as in QL_LOGPASS, but by pairs of lanes as in QL_TWO_PASS --
+// behind bisect_kernel.cuh, whose eigenvalues are not in the order in which QL would deflate them)
 
 template <int QL_TPB>
 __global__ void __launch_bounds__(QL_TPB)
@@ -47,7 +49,8 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
     double* esm = sm + (size_t)M * QL_TPB;        // [M][QL_TPB]
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x;              // column of the [M][QL_TPB] arrays
-    const bool two_pass = mode == QL_TWO_PASS;  // (pairs of lanes)
+    const bool two_pass = mode == QL_TWO_PASS || mode == QL_LOGPASS_PAIRED;  // (pairs of lanes)
+    const bool pending_only = mode == QL_LOGPASS || mode == QL_LOGPASS_PAIRED;
     const int nmc = two_pass ? QL_TPB / 2 : QL_TPB;         // matrices per CTA
     const int b0 = blockIdx.x * nmc;
     const int nb = min(nmc, batch - b0);
@@ -73,7 +76,7 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
     const int mloc = two_pass ? lane >> 1 : lane;            // matrix of this lane within the CTA
     const int b = b0 + mloc;
     bool valid = mloc < nb;
-    if (mode == QL_LOGPASS) {                                // only the matrices the classifier left pending
+    if (pending_only) {                                      // only the matrices the classifier left pending
         valid = valid && ws.flags[b] == FLAG_PENDING;
         if (!__syncthreads_or(valid ? 1 : 0)) return;
     }

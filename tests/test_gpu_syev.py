@@ -174,12 +174,19 @@ def test_extreme_scale_takes_the_slow_path(lk, oracle, scale):
     documented range 1e-100 < ||A|| < 1e100, but nowhere near under/overflow of the result.)"""
     A = wl.letkf_shaped(96, 64, 98, config_index=39)
     A[1::3] *= scale
-    w, V, info = run_gpu(lk, A)
+    try:
+        lk.set_option("bisect", 0)                        # (the QL kernel, as large batches use it)
+        w, V, info = run_gpu(lk, A)
+    finally:
+        lk.set_option("bisect", -1)
     assert ((info & 0xFFFF) == 0).all()
     slow = (info & lk.INFO_SLOWPATH).astype(bool)
     assert slow[1::3].all() and not slow[0::3].any() and not slow[2::3].any()
     wo, _, _, _ = oracle.syev_batched(A)
     parity.assert_evd(A, w, V, wo, f"scale {scale:g}")
+    w, V, info = run_gpu(lk, A)                           # small batch: the multisection kernel has no such range
+    assert ((info & 0xFFFF) == 0).all()
+    parity.assert_evd(A, w, V, wo, f"scale {scale:g}, multisection")
 
 
 def test_headline_full_size(lk, oracle):
@@ -373,6 +380,25 @@ def test_register_path_variants(lk, oracle, M, p, variant):
         assert (info2 & lk.INFO_SLOWPATH).astype(bool).all()
 
 
+@pytest.mark.parametrize("force", [0, 1])
+@pytest.mark.parametrize("M,p", [(64, 98), (57, 98), (48, 49), (33, 49), (16, 49), (5, 49), (2, 7), (64, 3), (64, 48), (64, 0)])
+def test_eigenvalues_by_multisection(lk, oracle, M, p, force):
+    """The latency-regime eigenvalue kernel (bisect_kernel.cuh: M threads per matrix,
+    multisection on the Sturm count) against the QL kernel's one thread per matrix: small batches take
+    it by default, letkf_set_option("bisect", 0 / 1) forces either.  Both feed the same classifier
+    and the same apply kernel; clustered spectra (p = 3, 48) go on to the logging QL pass, shifted by
+    the eigenvalues found here."""
+    A = wl.letkf_shaped(130, M, p, config_index=1100 + M + p)
+    try:
+        lk.set_option("bisect", force)
+        w, V, info = run_gpu(lk, A)
+    finally:
+        lk.set_option("bisect", -1)
+    assert (info == 0).all()
+    wo, _, _, _ = oracle.syev_batched(A)
+    parity.assert_evd(A, w, V, wo, f"bisect={force} M={M} p={p}")
+
+
 def test_direct_eigenvectors_are_used_and_fall_back(lk, oracle):
     """Which matrices take which route: well separated spectra (config 3) need no rotation at all
     (the profile counts none); a spectrum with eigenvalues closer than 1e-8 ||T|| inside one
@@ -484,12 +510,14 @@ def test_host_entry_point_in_passes(lk, oracle):
     try:
         lk.set_option("host_pass", 1100)
         lk.set_option("two_pass", 1)
+        lk.set_option("bisect", 0)                        # (the ragged last pass is small: same kernels as the device call)
         w, V, info = lk.syev_batched_host(A.pin_memory())
         wd, Vd, _ = lk.syev_batched(A.cuda())
         torch.cuda.synchronize()
     finally:
         lk.set_option("host_pass", 0)
         lk.set_option("two_pass", -1)
+        lk.set_option("bisect", -1)
     assert int(info.abs().max()) == 0
     assert torch.equal(w, wd.cpu()) and torch.equal(V, Vd.cpu())
 
