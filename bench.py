@@ -596,6 +596,29 @@ def run_ours(args):
                     shapes.append({"M": Ms, "batch": Bs, "ms": round(sms, 4), "matrices_per_s": Bs / (sms * 1e-3)})
                     del As, Vs, ws_, wk
             line["paper_shapes_fp64"] = shapes
+            # the same shapes in the paper's precision (letkf_syev_batched_f32); the
+            # paper's own numbers are FP32 on one A100 (context, another machine)
+            paper_ms = {16: 1.3, 32: 2.4, 48: 7.8, 64: 14.2}
+            shapes32 = []
+            for Ms, ps in ((16, 49), (32, 49), (48, 49), (64, 98)):
+                Bs = 16384
+                As = torch.from_numpy(wl.letkf_shaped(Bs, Ms, ps, config_index=80 + Ms).astype(np.float32)).cuda()
+                ws_ = torch.empty((Bs, Ms), dtype=torch.float32, device="cuda")
+                Vs = torch.empty_like(As)
+                wk = torch.empty(letkf.syev_f32_workspace_bytes(Ms, Bs), dtype=torch.uint8, device="cuda")
+                for _ in range(3):
+                    letkf.syev_batched_f32(As, w=ws_, V=Vs, work=wk, stream=stream)
+                torch.cuda.synchronize()
+                e0.record(stream)
+                for _ in range(10):
+                    letkf.syev_batched_f32(As, w=ws_, V=Vs, work=wk, stream=stream)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                sms = e0.elapsed_time(e1) / 10
+                shapes32.append({"M": Ms, "batch": Bs, "ms": round(sms, 4), "matrices_per_s": Bs / (sms * 1e-3),
+                                 "paper_a100_fp32_ms": paper_ms[Ms]})
+                del As, Vs, ws_, wk
+            line["paper_shapes_fp32"] = shapes32
             A = torch.from_numpy(A_host).cuda()
         # ---- cuSOLVER on the same matrices (comparison only)
         if not args.no_cusolver:

@@ -74,6 +74,22 @@ int letkf_syev_batched(const double* A, int M, int batch, double* w, double* V,
 size_t letkf_syev_workspace_bytes(int M, int batch);
 
 /*
+ * The same decomposition in the paper's precision ("single-precision"; Table I,
+ * M = 16, 32, 48, 64, batch 128^2): A, w, V are fp32.  SURVEY.md section 8(f) N2.
+ * The Householder reduction, the replay of plane rotations and the back-transform run in fp32; the
+ * tridiagonal eigenproblem (O(M^2) of the O(M^3) work) is solved in fp64 on the (d, e) the fp32
+ * reduction produced, so the result is the EVD of a matrix within a few eps32 ||A|| of A:
+ *   max_k |w_k - lambda_k| <~ 50 eps32 ||A||_2,  ||A V - V diag(w)||_F / ||A||_F <~ 100 eps32,
+ *   max |V^T V - I| <~ 100 eps32                                   (eps32 = 2^-24)
+ * 1 <= M <= 64 (the register-resident path); other arguments, info and the workspace as for
+ * letkf_syev_batched (size from letkf_syev_f32_workspace_bytes).  V may alias A.
+ */
+int letkf_syev_batched_f32(const float* A, int M, int batch, float* w, float* V,
+                           int* info, void* work, size_t work_bytes, void* stream);
+
+size_t letkf_syev_f32_workspace_bytes(int M, int batch);
+
+/*
  * Fused LETKF local analysis of `batch` grid points (Eq.13-19;
  * Procedure 1 lines 5-7).  For each point, with dY = Yb (p x M),
  * r = rinv_loc (the diagonal of G o R^-1), dvec = d = y^o - ybar^f:

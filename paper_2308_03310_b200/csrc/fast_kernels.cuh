@@ -30,11 +30,49 @@ namespace letkf {
     X(31) X(30) X(29) X(28) X(27) X(26) X(25) X(24) X(23) X(22) X(21) X(20) X(19) X(18) X(17) X(16) \
     X(15) X(14) X(13) X(12) X(11) X(10) X(9) X(8) X(7) X(6) X(5) X(4) X(3) X(2) X(1) X(0)
 
+// ---- the real type of the register path: double (everything), or float for the reduction, the
+// replay and the back-transform of letkf_syev_batched_f32
+template <typename R> struct Blk8;        // 8 consecutive entries of a broadcast vector in shared memory
+template <> struct Blk8<double> {
+    double2 t0, t1, t2, t3;               // four LDS.128, each feeds two FMAs in every lane
+    __device__ __forceinline__ Blk8(const double* vec, int g)
+    {
+        const double2* v2 = reinterpret_cast<const double2*>(vec);
+        t0 = v2[4 * g]; t1 = v2[4 * g + 1]; t2 = v2[4 * g + 2]; t3 = v2[4 * g + 3];
+    }
+    __device__ __forceinline__ double v0() const { return t0.x; }
+    __device__ __forceinline__ double v1() const { return t0.y; }
+    __device__ __forceinline__ double v2() const { return t1.x; }
+    __device__ __forceinline__ double v3() const { return t1.y; }
+    __device__ __forceinline__ double v4() const { return t2.x; }
+    __device__ __forceinline__ double v5() const { return t2.y; }
+    __device__ __forceinline__ double v6() const { return t3.x; }
+    __device__ __forceinline__ double v7() const { return t3.y; }
+};
+template <> struct Blk8<float> {
+    float4 t0, t1;                        // two LDS.128, each feeds four FMAs
+    __device__ __forceinline__ Blk8(const float* vec, int g)
+    {
+        const float4* v4 = reinterpret_cast<const float4*>(vec);
+        t0 = v4[2 * g]; t1 = v4[2 * g + 1];
+    }
+    __device__ __forceinline__ float v0() const { return t0.x; }
+    __device__ __forceinline__ float v1() const { return t0.y; }
+    __device__ __forceinline__ float v2() const { return t0.z; }
+    __device__ __forceinline__ float v3() const { return t0.w; }
+    __device__ __forceinline__ float v4() const { return t1.x; }
+    __device__ __forceinline__ float v5() const { return t1.y; }
+    __device__ __forceinline__ float v6() const { return t1.z; }
+    __device__ __forceinline__ float v7() const { return t1.w; }
+};
+__device__ __forceinline__ double rsq(double x) { return rsqrt(x); }
+__device__ __forceinline__ float rsq(float x) { return rsqrtf(x); }
+
 // register-array read with a run-time index (jump table; indices stay compile-time constants)
-template <int MT>
-__device__ __forceinline__ double pick(const double (&a)[MT], int i)
+template <int MT, typename R>
+__device__ __forceinline__ R pick(const R (&a)[MT], int i)
 {
-    double x = 0.0;
+    R x = R(0);
     switch (i) {
 #define LETKF_PICK(c) case c: if constexpr (c < MT) x = a[c]; break;
         LETKF_REP64_DESC(LETKF_PICK)
@@ -49,40 +87,38 @@ __device__ __forceinline__ double pick(const double (&a)[MT], int i)
 // free to hoist the shared-memory loads of a whole pass.
 
 // sum_{c < 8(G+1)} a[c] * vec[c]
-template <int MT, int G, bool FENCED = false>
-__device__ __forceinline__ double dot_blocks(const double (&a)[MT], const double* vec)
+template <int MT, int G, bool FENCED = false, typename R>
+__device__ __forceinline__ R dot_blocks(const R (&a)[MT], const R* vec)
 {
-    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0, s4 = 0.0, s5 = 0.0, s6 = 0.0, s7 = 0.0;
-    const double2* v2 = reinterpret_cast<const double2*>(vec);
+    R s0 = R(0), s1 = R(0), s2 = R(0), s3 = R(0), s4 = R(0), s5 = R(0), s6 = R(0), s7 = R(0);
 #pragma unroll
     for (int g = G; g >= 0; --g) {
-        const double2 t0 = v2[4 * g], t1 = v2[4 * g + 1], t2 = v2[4 * g + 2], t3 = v2[4 * g + 3];
-        s0 = fma(a[8 * g],     t0.x, s0); s1 = fma(a[8 * g + 1], t0.y, s1);
-        s2 = fma(a[8 * g + 2], t1.x, s2); s3 = fma(a[8 * g + 3], t1.y, s3);
-        s4 = fma(a[8 * g + 4], t2.x, s4); s5 = fma(a[8 * g + 5], t2.y, s5);
-        s6 = fma(a[8 * g + 6], t3.x, s6); s7 = fma(a[8 * g + 7], t3.y, s7);
+        const Blk8<R> t(vec, g);
+        s0 = fma(a[8 * g],     t.v0(), s0); s1 = fma(a[8 * g + 1], t.v1(), s1);
+        s2 = fma(a[8 * g + 2], t.v2(), s2); s3 = fma(a[8 * g + 3], t.v3(), s3);
+        s4 = fma(a[8 * g + 4], t.v4(), s4); s5 = fma(a[8 * g + 5], t.v5(), s5);
+        s6 = fma(a[8 * g + 6], t.v6(), s6); s7 = fma(a[8 * g + 7], t.v7(), s7);
         if constexpr (FENCED) __syncwarp();     // ptxas does not move shared loads across it
     }
     return ((s0 + s1) + (s2 + s3)) + ((s4 + s5) + (s6 + s7));
 }
 
 // a[c] -= alpha * vec[c] for the 8 columns of block g
-template <int MT>
-__device__ __forceinline__ void axpy_block(double (&a)[MT], const double* vec, double nalpha, int g)
+template <int MT, typename R>
+__device__ __forceinline__ void axpy_block(R (&a)[MT], const R* vec, R nalpha, int g)
 {
-    const double2* v2 = reinterpret_cast<const double2*>(vec);
-    const double2 t0 = v2[4 * g], t1 = v2[4 * g + 1], t2 = v2[4 * g + 2], t3 = v2[4 * g + 3];
-    a[8 * g]     = fma(nalpha, t0.x, a[8 * g]);     a[8 * g + 1] = fma(nalpha, t0.y, a[8 * g + 1]);
-    a[8 * g + 2] = fma(nalpha, t1.x, a[8 * g + 2]); a[8 * g + 3] = fma(nalpha, t1.y, a[8 * g + 3]);
-    a[8 * g + 4] = fma(nalpha, t2.x, a[8 * g + 4]); a[8 * g + 5] = fma(nalpha, t2.y, a[8 * g + 5]);
-    a[8 * g + 6] = fma(nalpha, t3.x, a[8 * g + 6]); a[8 * g + 7] = fma(nalpha, t3.y, a[8 * g + 7]);
+    const Blk8<R> t(vec, g);
+    a[8 * g]     = fma(nalpha, t.v0(), a[8 * g]);     a[8 * g + 1] = fma(nalpha, t.v1(), a[8 * g + 1]);
+    a[8 * g + 2] = fma(nalpha, t.v2(), a[8 * g + 2]); a[8 * g + 3] = fma(nalpha, t.v3(), a[8 * g + 3]);
+    a[8 * g + 4] = fma(nalpha, t.v4(), a[8 * g + 4]); a[8 * g + 5] = fma(nalpha, t.v5(), a[8 * g + 5]);
+    a[8 * g + 6] = fma(nalpha, t.v6(), a[8 * g + 6]); a[8 * g + 7] = fma(nalpha, t.v7(), a[8 * g + 7]);
 }
 
 // a[8G + k], k = 0..7 at run time (select chain; the block is compile-time)
-template <int MT, int G>
-__device__ __forceinline__ double block_pick(const double (&a)[MT], int k)
+template <int MT, int G, typename R>
+__device__ __forceinline__ R block_pick(const R (&a)[MT], int k)
 {
-    double x = a[8 * G];
+    R x = a[8 * G];
 #pragma unroll
     for (int t = 1; t < 8; ++t) x = (k == t) ? a[8 * G + t] : x;
     return x;
@@ -124,17 +160,17 @@ __device__ __forceinline__ void part_barrier(int nwarps)
 // (tile row = matrix row - r0).  Thread t owns column t: no index arithmetic beyond one add per
 // row (a flat index split by a run-time M cost an integer division per element and 17% of the
 // tridiagonalisation kernel, profiles/r01b), 8 loads in flight per thread.
-template <int MT>
-__device__ __forceinline__ void load_rows(double* tile, const double* __restrict__ G, int M, int r0, int nr)
+template <int MT, typename R>
+__device__ __forceinline__ void load_rows(R* tile, const R* __restrict__ G, int M, int r0, int nr)
 {
     using C = FastCfg<MT>;
     const int t = threadIdx.x;
     if (t >= M) return;
-    const double* src = G + (size_t)r0 * M + t;
-    double* dst = tile + t;
+    const R* src = G + (size_t)r0 * M + t;
+    R* dst = tile + t;
     int r = 0;
     for (; r + 8 <= nr; r += 8) {
-        double tmp[8];
+        R tmp[8];
 #pragma unroll
         for (int u = 0; u < 8; ++u) tmp[u] = src[(size_t)(r + u) * M];
 #pragma unroll
@@ -158,44 +194,43 @@ template <int MT> struct RefLayout {
 // Back-transform: reflectors i = 8G+1 ... 8G+8 applied to the column q held by this thread.  The
 // __syncwarp() after every 8-column block is a scheduling fence: ptxas does not move shared-memory
 // loads across it, and without it the loads of a whole pass are hoisted and the matrix spills.
-template <int MT, int G>
-__device__ __forceinline__ void q_group(double (&q)[MT], const double* R, const double* taus, int M)
+template <int MT, int G, typename R>
+__device__ __forceinline__ void q_group(R (&q)[MT], const R* Rf, const R* taus, int M)
 {
 #pragma unroll 1
     for (int i = 8 * G + 1; i <= 8 * G + 8 && i <= M - 1; ++i) {
-        const double tau1 = taus[i];
-        if (tau1 == 0.0) continue;
-        const double* v1 = R + RefLayout<MT>::base(G) + (i - 1 - 8 * G) * RefLayout<MT>::len(G);
-        const double ns1 = -tau1 * dot_blocks<MT, G, true>(q, v1);
+        const R tau1 = taus[i];
+        if (tau1 == R(0)) continue;
+        const R* v1 = Rf + RefLayout<MT>::base(G) + (i - 1 - 8 * G) * RefLayout<MT>::len(G);
+        const R ns1 = -tau1 * dot_blocks<MT, G, true>(q, v1);
 #pragma unroll
         for (int g = G; g >= 0; --g) { axpy_block<MT>(q, v1, ns1, g); __syncwarp(); }
     }
 }
 
-template <int MT, int G, int GMAX>
-__device__ __forceinline__ void q_groups_up(double (&q)[MT], const double* R, const double* taus,
-                                            int M, int gstart)
+template <int MT, int G, int GMAX, typename R>
+__device__ __forceinline__ void q_groups_up(R (&q)[MT], const R* Rf, const R* taus, int M, int gstart)
 {
-    if (G >= gstart) q_group<MT, G>(q, R, taus, M);
-    if constexpr (G < GMAX) q_groups_up<MT, G + 1, GMAX>(q, R, taus, M, gstart);
+    if (G >= gstart) q_group<MT, G>(q, Rf, taus, M);
+    if constexpr (G < GMAX) q_groups_up<MT, G + 1, GMAX>(q, Rf, taus, M, gstart);
 }
 
 // Dynamic shared memory of fast_tridiag_formq<MT>:
 //   region[RefLayout::REGION]  staging of A, 32 padded rows per pass, later the reflectors
 //   xs[NT] raw pivot column;  vbuf[NT] v;  pbuf[NT] p;  pv[NT] p_j v_j;  taus[NT];  red[8]
-template <int MT> constexpr size_t fast_tridiag_smem()
+template <int MT, typename R = double> constexpr size_t fast_tridiag_smem()
 {
-    return sizeof(double) * ((size_t)RefLayout<MT>::REGION + 5 * FastCfg<MT>::NT + 8);
+    return sizeof(R) * ((size_t)RefLayout<MT>::REGION + 5 * FastCfg<MT>::NT + 8);
 }
 
-struct TriShared {
-    double* R;      // reflector storage, RefLayout<MT>
-    double* xs;     // x_c = A[c][i] for c < i-1, zero from i-1 on
-    double* vbuf;   // v_c (v_{i-1} = 1, zero from i on)
-    double* pbuf;   // p_c = tau (A v)_c, zero from i on
-    double* pv;     // p_c v_c
-    double* taus;
-    double* red;    // [0..1] per-warp partial of sigma, [4] alpha
+template <typename R> struct TriShared {
+    R* Rf;      // reflector storage, RefLayout<MT>
+    R* xs;      // x_c = A[c][i] for c < i-1, zero from i-1 on
+    R* vbuf;    // v_c (v_{i-1} = 1, zero from i on)
+    R* pbuf;    // p_c = tau (A v)_c, zero from i on
+    R* pv;      // p_c v_c
+    R* taus;
+    R* red;     // [0..1] per-warp partial of sigma, [4] alpha
 };
 
 // Pivots i = min(8G+8, M-1) ... 8G+1 of the Householder reduction (H_i acts on indices 0..i-1, the
@@ -209,8 +244,8 @@ struct TriShared {
 //       -> pass B  a_jc -= (p_j - tau (p.v) v_j) v_c, top block first: column i-1 is then final, it
 //          is the next pivot's x, whose norm tree overlaps the rest of pass B.
 // Entered and left with B1 done (by the NP warps that hold rows < 8G+8).
-template <int MT, int G>
-__device__ __forceinline__ void pivot_group(double (&a)[MT], const TriShared& sh, int M,
+template <int MT, int G, typename R>
+__device__ __forceinline__ void pivot_group(R (&a)[MT], const TriShared<R>& sh, int M,
                                             double* __restrict__ dws, double* __restrict__ ews)
 {
     using C = FastCfg<MT>;
@@ -222,43 +257,43 @@ __device__ __forceinline__ void pivot_group(double (&a)[MT], const TriShared& sh
     const int ihi = (8 * G + 8 < M - 1) ? 8 * G + 8 : M - 1;
     for (int i = ihi; i >= 8 * G + 1; --i) {
         const int k = i - 1 - 8 * G;
-        double sigma = sh.red[0];
+        R sigma = sh.red[0];
         if constexpr (NP > 1) sigma += sh.red[1];
-        const double alpha = sh.red[4];
-        const double xj = sh.xs[j];
-        const double praw = dot_blocks<MT, G>(a, sh.xs);
-        const double acol = block_pick<MT, G>(a, k);          // A[j][i-1] before the update
-        double tau = 0.0, scal = 0.0, beta = alpha;            // sigma == 0: H_i = I (reading G19)
-        if (sigma != 0.0) {
-            const double nrm2 = fma(alpha, alpha, sigma);
-            const double rinv = rsqrt(nrm2);
+        const R alpha = sh.red[4];
+        const R xj = sh.xs[j];
+        const R praw = dot_blocks<MT, G>(a, sh.xs);
+        const R acol = block_pick<MT, G>(a, k);                // A[j][i-1] before the update
+        R tau = R(0), scal = R(0), beta = alpha;               // sigma == 0: H_i = I (reading G19)
+        if (sigma != R(0)) {
+            const R nrm2 = fma(alpha, alpha, sigma);
+            const R rinv = rsq(nrm2);
             beta = -copysign(nrm2 * rinv, alpha);
-            tau = fma(fabs(alpha), rinv, 1.0);                 // (beta - alpha) / beta
-            scal = 1.0 / (alpha - beta);
+            tau = fma(fabs(alpha), rinv, R(1));                // (beta - alpha) / beta
+            scal = R(1) / (alpha - beta);
         }
-        const double vj = (j < i - 1) ? xj * scal : ((j == i - 1) ? 1.0 : 0.0);
-        const double pj = (j < i) ? tau * fma(scal, praw, acol) : 0.0;
+        const R vj = (j < i - 1) ? xj * scal : ((j == i - 1) ? R(1) : R(0));
+        const R pj = (j < i) ? tau * fma(scal, praw, acol) : R(0);
         sh.vbuf[j] = vj;
         sh.pbuf[j] = pj;
         sh.pv[j] = pj * vj;
-        if (j < RefLayout<MT>::len(G)) sh.R[RefLayout<MT>::base(G) + k * RefLayout<MT>::len(G) + j] = vj;
-        if (j == 0) { ews[i - 1] = beta; sh.taus[i] = tau; }
+        if (j < RefLayout<MT>::len(G)) sh.Rf[RefLayout<MT>::base(G) + k * RefLayout<MT>::len(G) + j] = vj;
+        if (j == 0) { ews[i - 1] = (double)beta; sh.taus[i] = tau; }
         part_barrier(NP);                                      // ---- B2
-        double t = sh.pv[lane];
+        R t = sh.pv[lane];
         if constexpr (NP > 1) t += sh.pv[lane + 32];
-        const double nvj = -vj;
+        const R nvj = -vj;
 #pragma unroll
         for (int step = 0; step < (G + 1 > 5 ? G + 1 : 5); ++step) {
             if (step < 5) t += __shfl_xor_sync(FULL, t, 16 >> step);
             if (step <= G) axpy_block<MT>(a, sh.pbuf, nvj, G - step);
         }
-        const double nwj = fma(tau * t, vj, -pj);              // -(p_j - tau (p.v) v_j)
+        const R nwj = fma(tau * t, vj, -pj);                   // -(p_j - tau (p.v) v_j)
         axpy_block<MT>(a, sh.vbuf, nwj, G);
-        const double xn = block_pick<MT, G>(a, k);             // A[j][i-1], final: next pivot's x_j
-        if (j == i - 1) dws[i - 1] = xn;
-        sh.xs[j] = (j < i - 2) ? xn : 0.0;
+        const R xn = block_pick<MT, G>(a, k);                  // A[j][i-1], final: next pivot's x_j
+        if (j == i - 1) dws[i - 1] = (double)xn;
+        sh.xs[j] = (j < i - 2) ? xn : R(0);
         if (j == i - 2) sh.red[4] = xn;
-        double part = (j < i - 2) ? xn * xn : 0.0;
+        R part = (j < i - 2) ? xn * xn : R(0);
 #pragma unroll
         for (int step = 0; step < (G > 5 ? G : 5); ++step) {
             if (step < 5) part += __shfl_xor_sync(FULL, part, 16 >> step);
@@ -269,17 +304,8 @@ __device__ __forceinline__ void pivot_group(double (&a)[MT], const TriShared& sh
     }
 }
 
-// groups G ... GLO only
-template <int MT, int G, int GLO>
-__device__ __forceinline__ void pivot_groups_range(double (&a)[MT], const TriShared& sh, int M,
-                                                   double* __restrict__ dws, double* __restrict__ ews)
-{
-    pivot_group<MT, G>(a, sh, M, dws, ews);
-    if constexpr (G > GLO) pivot_groups_range<MT, G - 1, GLO>(a, sh, M, dws, ews);
-}
-
-template <int MT, int G>
-__device__ __forceinline__ void pivot_groups_down(double (&a)[MT], const TriShared& sh, int M,
+template <int MT, int G, typename R>
+__device__ __forceinline__ void pivot_groups_down(R (&a)[MT], const TriShared<R>& sh, int M,
                                                   double* __restrict__ dws, double* __restrict__ ews)
 {
     pivot_group<MT, G>(a, sh, M, dws, ews);
@@ -371,35 +397,37 @@ grid_gather(GridArgs g, int M, int p, double* __restrict__ Yb, double* __restric
 // back-transform in fast_apply.
 template <int MT> __host__ __device__ constexpr int refl_doubles() { return RefLayout<MT>::TOTAL + FastCfg<MT>::NT; }
 
-template <int MT, bool GRAM, bool QFORM>
+template <int MT, bool GRAM, bool QFORM, typename R = double>
 __global__ void __launch_bounds__(FastCfg<MT>::NT) __maxnreg__((MT == 64) ? LETKF_TRI_REGS64 : (MT == 48 ? 168 : (MT == 32 ? 128 : 80)))
-fast_tridiag(const double* __restrict__ A_, double* __restrict__ Q_, Workspace ws, int M,
+fast_tridiag(const R* __restrict__ A_, R* __restrict__ Q_, Workspace ws, int M,
                    const double* __restrict__ Yb_, const double* __restrict__ d_,
                    const double* __restrict__ r_, int p, double shift, double* __restrict__ gout_,
                    GridArgs grid)
 {
     using C = FastCfg<MT>;
-    extern __shared__ __align__(16) double sm[];
-    double* tile = sm;
-    double* small = sm + RefLayout<MT>::REGION;
-    TriShared sh;
-    sh.R = tile;
+    static_assert(!GRAM || sizeof(R) == sizeof(double), "the Gram step (DMMA) is fp64");
+    extern __shared__ __align__(16) unsigned char sm_raw[];
+    R* sm = reinterpret_cast<R*>(sm_raw);
+    R* tile = sm;
+    R* small = sm + RefLayout<MT>::REGION;
+    TriShared<R> sh;
+    sh.Rf = tile;
     sh.xs = small;
     sh.vbuf = small + C::NT;
     sh.pbuf = small + 2 * C::NT;
     sh.pv = small + 3 * C::NT;
     sh.taus = small + 4 * C::NT;
     sh.red = small + 5 * C::NT;
-    double* taus = sh.taus;
+    R* taus = sh.taus;
     const int j = threadIdx.x, lane = j & 31, warp = j >> 5;
     const size_t b = blockIdx.x;
-    double a[MT];
+    R a[MT];
 
     if constexpr (!GRAM) {
         // a_j[c] = A[max(j,c)][min(j,c)] (only the lower triangle is read), 32 rows per pass
         constexpr int HT = RefLayout<MT>::HT;
 #pragma unroll
-        for (int c = 0; c < MT; ++c) a[c] = 0.0;
+        for (int c = 0; c < MT; ++c) a[c] = R(0);
 #pragma unroll
         for (int r0 = 0; r0 < MT; r0 += HT) {
             if (r0 < M) {
@@ -554,18 +582,19 @@ fast_tridiag(const double* __restrict__ A_, double* __restrict__ Q_, Workspace w
 
     double* dws = ws.dws + b * M;
     double* ews = ws.ews + b * M;
-    double* R = tile;                              // reflector i at R[i*MT + c]
+    R* Rf = tile;                                  // reflectors, RefLayout order
 
     // ---- a3: Householder tridiagonalisation, pivot i = M-1 ... 1, H_i acts on indices 0..i-1.
     // Prologue = the look-ahead of a fictitious pivot M: publish column M-1 and its partial norms.
     {
         const int i0 = M - 1;
-        const double x = pick<MT>(a, i0);              // x_j = A[j][i0]; for j == i0 this is d_i0
-        if (j == i0) dws[i0] = x;
-        sh.xs[j] = (j < i0 - 1) ? x : 0.0;
+        const R x = pick<MT>(a, i0);                   // x_j = A[j][i0]; for j == i0 this is d_i0
+        if (j == i0) dws[i0] = (double)x;
+        sh.xs[j] = (j < i0 - 1) ? x : R(0);
         if (j == i0 - 1) sh.red[4] = x;
-        double part = (j < i0 - 1) ? x * x : 0.0;
-        part = warp_sum(part);
+        R part = (j < i0 - 1) ? x * x : R(0);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
         if (lane == 0) sh.red[warp] = part;
         if (j == 0) ews[M - 1] = 0.0;
         __syncthreads();
@@ -579,12 +608,12 @@ fast_tridiag(const double* __restrict__ A_, double* __restrict__ Q_, Workspace w
         // reflectors with i >= its first row have been stored (barrier 2 of those steps included it),
         // so the upper warps form their columns of Q while warp 0 is still reducing the last 32 rows.
         __syncwarp();
-        double (&q)[MT] = a;
+        R (&q)[MT] = a;
 #pragma unroll
-        for (int c = 0; c < MT; ++c) q[c] = (c == j) ? 1.0 : 0.0;
-        q_groups_up<MT, 0, (MT - 2) / 8>(q, R, taus, M, warp * 4);
+        for (int c = 0; c < MT; ++c) q[c] = (c == j) ? R(1) : R(0);
+        q_groups_up<MT, 0, (MT - 2) / 8>(q, static_cast<const R*>(Rf), static_cast<const R*>(taus), M, warp * 4);
         if (j < M) {
-            double* Q = Q_ + b * M * M;
+            R* Q = Q_ + b * M * M;
 #pragma unroll
             for (int c = 0; c < MT; ++c)
                 if (c < M) Q[(size_t)c * M + j] = q[c];
@@ -592,9 +621,9 @@ fast_tridiag(const double* __restrict__ A_, double* __restrict__ Q_, Workspace w
     } else {
         __syncthreads();
         // reflectors (RefLayout order; H_i with i >= M are never read) and taus for the back-transform
-        double* out = ws.refl + b * ws.reflstride;
-        for (int k = j; k < RefLayout<MT>::TOTAL; k += C::NT) out[k] = R[k];
-        out[RefLayout<MT>::TOTAL + j] = (j >= 1 && j <= M - 1) ? taus[j] : 0.0;
+        R* out = reinterpret_cast<R*>(ws.refl + b * ws.reflstride);
+        for (int k = j; k < RefLayout<MT>::TOTAL; k += C::NT) out[k] = Rf[k];
+        out[RefLayout<MT>::TOTAL + j] = (j >= 1 && j <= M - 1) ? taus[j] : R(0);
     }
 }
 
@@ -635,7 +664,7 @@ template <int MT> __host__ __device__ inline int fast_epi_doubles(int ns)
 // ds[MT], es[MT], lam sorted [MT] as doubles and perm [MT] as bytes
 template <int MT> __host__ __device__ inline int ap_hdr_words(int swcap)
 {
-    const int gv = 6 * MT + MT / 4 + 4;
+    const int gv = 6 * MT + MT / 4 + 8;
     return swcap > gv ? swcap : gv;
 }
 
@@ -665,16 +694,17 @@ __device__ __forceinline__ void cp_async_wait_all()
 // Blocks of 4 rotations, entered at the block of m-1 and left after the block of lo; cs[] holds
 // the identity (1, 0) outside [lo, m), so the overhang at both ends changes nothing.  The only
 // dependent chain from one rotation to the next is the single FMA that produces z[i].
-template <int MT>
-__device__ __forceinline__ void apply_sweep(double (&z)[MT], const double2* cs, int lo, int m)
+template <int MT, typename R>
+__device__ __forceinline__ void apply_sweep(R (&z)[MT], const double2* cs, int lo, int m)
 {
     switch ((m - 1) >> 2) {
 #define LETKF_ROT1(i, t)                                                      \
         if constexpr ((i) + 1 < MT) {                                         \
-            const double f = z[(i) + 1];                                      \
-            const double zi = z[i];                                           \
-            z[(i) + 1] = fma(t.y, zi, t.x * f);                               \
-            z[i] = fma(-t.y, f, t.x * zi);                                    \
+            const R f = z[(i) + 1];                                           \
+            const R zi = z[i];                                                \
+            const R tc = (R)t.x, ts = (R)t.y;                                 \
+            z[(i) + 1] = fma(ts, zi, tc * f);                                 \
+            z[i] = fma(-ts, f, tc * zi);                                      \
         }
 #define LETKF_ROT(g)                                                          \
     case g:                                                                   \
@@ -694,15 +724,15 @@ __device__ __forceinline__ void apply_sweep(double (&z)[MT], const double2* cs, 
 }
 
 // 32 x 32 block moves of the transposition (compile-time register offsets)
-template <int MT, int C0>
-__device__ __forceinline__ void tr_put(const double (&z)[MT], double* T, int lane)
+template <int MT, int C0, typename R>
+__device__ __forceinline__ void tr_put(const R (&z)[MT], R* T, int lane)
 {
 #pragma unroll
     for (int c = 0; c < 32; ++c)
         if (C0 + c < MT) T[lane * 33 + c] = z[C0 + c];
 }
-template <int MT, int R0>
-__device__ __forceinline__ void tr_get(double (&z)[MT], const double* T, int lane)
+template <int MT, int R0, typename R>
+__device__ __forceinline__ void tr_get(R (&z)[MT], const R* T, int lane)
 {
 #pragma unroll
     for (int rr = 0; rr < 32; ++rr)
@@ -712,12 +742,12 @@ __device__ __forceinline__ void tr_get(double (&z)[MT], const double* T, int lan
 // thread t holds column t (an involution: the same call turns it back).  One 32 x 33 tile per warp;
 // with two warps the diagonal blocks turn inside their warp and the two off-diagonal blocks swap
 // through both tiles at once, so a thread never holds more than its MT values.
-template <int MT>
-__device__ __forceinline__ void transpose_regs(double (&z)[MT], double* tiles)
+template <int MT, typename R>
+__device__ __forceinline__ void transpose_regs(R (&z)[MT], R* tiles)
 {
     constexpr int NW = FastCfg<MT>::NW;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double* T = tiles + warp * (32 * 33);
+    R* T = tiles + warp * (32 * 33);
     if constexpr (NW == 1) {
         __syncwarp();
         tr_put<MT, 0>(z, T, lane);
@@ -734,7 +764,7 @@ __device__ __forceinline__ void transpose_regs(double (&z)[MT], double* tiles)
         // warp 0 hands block (rows 0..31, columns 32..) to warp 1, warp 1 block (rows 32.., columns 0..31) to warp 0
         if (warp == 0) tr_put<MT, 32>(z, T, lane); else tr_put<MT, 0>(z, T, lane);
         __syncthreads();
-        const double* O = tiles + (1 - warp) * (32 * 33);
+        const R* O = tiles + (1 - warp) * (32 * 33);
         if (warp == 0) tr_get<MT, 32>(z, O, lane); else tr_get<MT, 0>(z, O, lane);
         __syncthreads();
     }
@@ -851,6 +881,125 @@ __device__ __forceinline__ double getvec(double (&z)[MT], const double* ds, cons
     return sqrt(r0 + r1);
 }
 
+// The eigenvectors of T of matrix b without a single rotation (route FLAG_GETVEC of fast_apply):
+// thread k = position k, its eigenvalue is w[inv[k]]; on return z holds eigenvector k (a unit vector
+// for a 1 x 1 block).  `scratch` holds ap_hdr_words<MT>() words, `vbuf` 32 (MT + 1) doubles.  Called
+// by all threads of the CTA (barriers inside); returns false when a residual is suspicious and the
+// matrix has to go to the classic iteration.
+template <int MT>
+__device__ __forceinline__ bool direct_eigenvectors(double (&z)[MT], uint32_t* scratch, double* vbuf, const Workspace& ws,
+                                                    const double* __restrict__ w_, size_t b, int M, const int* inv)
+{
+    using C = FastCfg<MT>;
+    const int r = threadIdx.x;
+    bool ok;
+    double*        ds    = reinterpret_cast<double*>(scratch);         // [MT]
+    double*        es    = ds + MT;                                // [MT] negligible entries are exactly 0
+    double*        wsrt  = es + MT;                                // [MT] eigenvalues ascending
+    unsigned char* perm8 = reinterpret_cast<unsigned char*>(wsrt + MT);   // [MT] position of the k-th smallest
+    unsigned*      cutw  = reinterpret_cast<unsigned*>(perm8 + MT);       // [2] bit i: block boundary behind i
+    if (r < MT) {
+        ds[r] = (r < M) ? ws.dws[b * M + r] : 0.0;
+        es[r] = (r < M - 1) ? ws.ews[b * M + r] : 0.0;
+        wsrt[r] = (r < M) ? w_[b * M + r] : 0.0;
+        perm8[r] = (unsigned char)((r < M) ? ws.perm[b * M + r] : r);
+    }
+    __syncthreads();
+    // the threshold and the split of ql_log_kernel, on the same numbers
+    const double eps = 1.1102230246251565e-16;
+    // (max is exact in any order: the same number the QL kernel's serial loop finds)
+    double nrm = (r < M) ? fabs(ds[r]) + (r < M - 1 ? fabs(es[r]) : 0.0) : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) nrm = fmax(nrm, __shfl_xor_sync(0xffffffffu, nrm, o));
+    double* nrmw = reinterpret_cast<double*>(cutw + 2);                      // [2]
+    if ((r & 31) == 0) nrmw[r >> 5] = nrm;
+    __syncthreads();
+    if constexpr (C::NW > 1) nrm = fmax(nrmw[0], nrmw[1]);
+    const double thr = eps * nrm;
+    bool cut = true;
+    if (r < M - 1) cut = fabs(es[r]) <= fmax(eps * (fabs(ds[r]) + fabs(ds[r + 1])), thr);
+    __syncthreads();
+    if (r < MT && cut) es[r] = 0.0;
+    const unsigned cw = __ballot_sync(0xffffffffu, cut);
+    if ((r & 31) == 0) cutw[r >> 5] = cw;
+    __syncthreads();
+    int lo = 0, hi = M - 1;
+    double lam = 0.0;
+    if (r < M) {
+        const unsigned long long cuts = (C::NW > 1) ? ((unsigned long long)cutw[1] << 32 | cutw[0]) : (unsigned long long)cutw[0];
+        const unsigned long long below = cuts & ((1ull << r) - 1ull);        // boundaries behind indices < r
+        lo = below ? 64 - __clzll((long long)below) : 0;
+        const unsigned long long above = cuts >> r;                          // bit 0: boundary behind r
+        hi = above ? r + __ffsll((long long)above) - 1 : M - 1;
+        if (hi > M - 1) hi = M - 1;
+        lam = wsrt[inv[r]];
+    }
+    // (every thread runs it -- the fences inside want whole warps; a 1 x 1 block gets its unit vector)
+    const bool own = r < M && lo < hi;
+    double res = getvec<MT>(z, ds, es, lam, lo, hi, fmax(thr * eps, 1e-300));
+    if (!own) {
+        res = 0.0;
+#pragma unroll
+        for (int c = 0; c < MT; ++c) z[c] = (c == r) ? 1.0 : 0.0;
+    }
+    // anything suspicious hands the matrix to the classic iteration below
+    const bool bad = !(res <= 64.0 * eps * nrm * sqrt((double)M));
+    if (__syncthreads_or(bad ? 1 : 0)) {
+        ok = false;
+    } else {
+        ok = true;
+        // eigenvalues closer than GV_GAP ||T|| inside a block: first-order symmetric orthogonalisation,
+        // z_k -= 1/2 (z_q . z_k) z_q for every such partner q (the classifier bounds their number);
+        // the vectors pass through shared memory 32 at a time
+        const double gapabs = GV_GAP * nrm;
+        unsigned long long plist = 0ull;
+        int np = 0;
+        if (own) {
+            const int s0 = inv[r];
+            for (int t = 1; t <= GV_PH && s0 - t >= 0 && lam - wsrt[s0 - t] < gapabs; ++t) {
+                const int q = perm8[s0 - t];
+                if (q >= lo && q <= hi) { plist |= (unsigned long long)q << (8 * np); ++np; }
+            }
+            for (int t = 1; t <= GV_PH && s0 + t < M && wsrt[s0 + t] - lam < gapabs; ++t) {
+                const int q = perm8[s0 + t];
+                if (q >= lo && q <= hi) { plist |= (unsigned long long)q << (8 * np); ++np; }
+            }
+        }
+        if (__syncthreads_or(np)) {
+            constexpr int LDV = MT + 1;
+            const int npw = __reduce_max_sync(0xffffffffu, np);             // whole warps walk the longest list
+#pragma unroll 1
+            for (int ph = 0; ph < C::NW; ++ph) {
+                if (ph) __syncthreads();
+                if ((r >> 5) == ph) {
+#pragma unroll
+                    for (int i = 0; i < MT; ++i) vbuf[(r & 31) * LDV + i] = z[i];
+                }
+                __syncthreads();
+#pragma unroll 1
+                for (int t = 0; t < npw; ++t) {
+                    const int q = (int)((plist >> (8 * t)) & 255ull);
+                    const bool act = t < np && (q >> 5) == ph;
+                    const double* vq = vbuf + (act ? (q & 31) : 0) * LDV;
+                    double d0 = 0.0, d1 = 0.0;
+#pragma unroll
+                    for (int i = 0; i + 1 < MT; i += 2) {
+                        d0 = fma(z[i], vq[i], d0); d1 = fma(z[i + 1], vq[i + 1], d1);
+                        if ((i & 7) == 6) __syncwarp();
+                    }
+                    const double h = act ? -0.5 * (d0 + d1) : 0.0;
+#pragma unroll
+                    for (int i = 0; i < MT; ++i) {
+                        z[i] = fma(h, vq[i], z[i]);
+                        if ((i & 7) == 7) __syncwarp();
+                    }
+                }
+            }
+        }
+    }
+    return ok;
+}
+
 template <int MT, bool EPI, bool QFORM>
 __global__ void __launch_bounds__(FastCfg<MT>::NT, (MT == 64) ? 6 : (MT == 48 ? 7 : 16))
 fast_apply(double* __restrict__ V_, double* __restrict__ w_, int* __restrict__ info_, Workspace ws, int M, EpiArgs ep)
@@ -885,108 +1034,11 @@ fast_apply(double* __restrict__ V_, double* __restrict__ w_, int* __restrict__ i
     bool columns = false;                          // z holds a column of Z (an eigenvector of T) rather than a row
 
     if (direct) {
-        // ---- eigenvectors of T without a single rotation: thread k = position k, its eigenvalue is
-        // w[inv[k]].
-        double*        ds    = reinterpret_cast<double*>(hdr);         // [MT]
-        double*        es    = ds + MT;                                // [MT] negligible entries are exactly 0
-        double*        wsrt  = es + MT;                                // [MT] eigenvalues ascending
-        unsigned char* perm8 = reinterpret_cast<unsigned char*>(wsrt + MT);   // [MT] position of the k-th smallest
-        unsigned*      cutw  = reinterpret_cast<unsigned*>(perm8 + MT);       // [2] bit i: block boundary behind i
-        if (r < MT) {
-            ds[r] = (r < M) ? ws.dws[b * M + r] : 0.0;
-            es[r] = (r < M - 1) ? ws.ews[b * M + r] : 0.0;
-            wsrt[r] = (r < M) ? w_[b * M + r] : 0.0;
-            perm8[r] = (unsigned char)((r < M) ? ws.perm[b * M + r] : r);
-        }
+        // ---- eigenvectors of T by twisted factorisations (the reflectors keep flying in meanwhile)
+        if (direct_eigenvectors<MT>(z, hdr, areg, ws, w_, b, M, inv)) columns = true;
+        else flagged = true;
+        cp_async_wait_all();
         __syncthreads();
-        // the threshold and the split of ql_log_kernel, on the same numbers
-        const double eps = 1.1102230246251565e-16;
-        double nrm = 0.0;
-        for (int i = 0; i < M; ++i) nrm = fmax(nrm, fabs(ds[i]) + (i < M - 1 ? fabs(es[i]) : 0.0));
-        const double thr = eps * nrm;
-        bool cut = true;
-        if (r < M - 1) cut = fabs(es[r]) <= fmax(eps * (fabs(ds[r]) + fabs(ds[r + 1])), thr);
-        __syncthreads();
-        if (r < MT && cut) es[r] = 0.0;
-        const unsigned cw = __ballot_sync(0xffffffffu, cut);
-        if ((r & 31) == 0) cutw[r >> 5] = cw;
-        __syncthreads();
-        int lo = 0, hi = M - 1;
-        double lam = 0.0;
-        if (r < M) {
-            const unsigned long long cuts = (C::NW > 1) ? ((unsigned long long)cutw[1] << 32 | cutw[0]) : (unsigned long long)cutw[0];
-            const unsigned long long below = cuts & ((1ull << r) - 1ull);        // boundaries behind indices < r
-            lo = below ? 64 - __clzll((long long)below) : 0;
-            const unsigned long long above = cuts >> r;                          // bit 0: boundary behind r
-            hi = above ? r + __ffsll((long long)above) - 1 : M - 1;
-            if (hi > M - 1) hi = M - 1;
-            lam = wsrt[inv[r]];
-        }
-        // (every thread runs it -- the fences inside want whole warps; a 1 x 1 block gets its unit vector)
-        const bool own = r < M && lo < hi;
-        double res = getvec<MT>(z, ds, es, lam, lo, hi, fmax(thr * eps, 1e-300));
-        if (!own) {
-            res = 0.0;
-#pragma unroll
-            for (int c = 0; c < MT; ++c) z[c] = (c == r) ? 1.0 : 0.0;
-        }
-        // anything suspicious hands the matrix to the classic iteration below
-        const bool bad = !(res <= 64.0 * eps * nrm * sqrt((double)M));
-        if (__syncthreads_or(bad ? 1 : 0)) {
-            flagged = true;
-        } else {
-            columns = true;
-            // eigenvalues closer than GV_GAP ||T|| inside a block: first-order symmetric orthogonalisation,
-            // z_k -= 1/2 (z_q . z_k) z_q for every such partner q (the classifier bounds their number);
-            // the vectors pass through shared memory 32 at a time
-            const double gapabs = GV_GAP * nrm;
-            unsigned long long plist = 0ull;
-            int np = 0;
-            if (own) {
-                const int s0 = inv[r];
-                for (int t = 1; t <= GV_PH && s0 - t >= 0 && lam - wsrt[s0 - t] < gapabs; ++t) {
-                    const int q = perm8[s0 - t];
-                    if (q >= lo && q <= hi) { plist |= (unsigned long long)q << (8 * np); ++np; }
-                }
-                for (int t = 1; t <= GV_PH && s0 + t < M && wsrt[s0 + t] - lam < gapabs; ++t) {
-                    const int q = perm8[s0 + t];
-                    if (q >= lo && q <= hi) { plist |= (unsigned long long)q << (8 * np); ++np; }
-                }
-            }
-            if (__syncthreads_or(np)) {
-                constexpr int LDV = MT + 1;
-                const int npw = __reduce_max_sync(0xffffffffu, np);             // whole warps walk the longest list
-#pragma unroll 1
-                for (int ph = 0; ph < C::NW; ++ph) {
-                    if (ph) __syncthreads();
-                    if ((r >> 5) == ph) {
-#pragma unroll
-                        for (int i = 0; i < MT; ++i) areg[(r & 31) * LDV + i] = z[i];
-                    }
-                    __syncthreads();
-#pragma unroll 1
-                    for (int t = 0; t < npw; ++t) {
-                        const int q = (int)((plist >> (8 * t)) & 255ull);
-                        const bool act = t < np && (q >> 5) == ph;
-                        const double* vq = areg + (act ? (q & 31) : 0) * LDV;
-                        double d0 = 0.0, d1 = 0.0;
-#pragma unroll
-                        for (int i = 0; i + 1 < MT; i += 2) {
-                            d0 = fma(z[i], vq[i], d0); d1 = fma(z[i + 1], vq[i + 1], d1);
-                            if ((i & 7) == 6) __syncwarp();
-                        }
-                        const double h = act ? -0.5 * (d0 + d1) : 0.0;
-#pragma unroll
-                        for (int i = 0; i < MT; ++i) {
-                            z[i] = fma(h, vq[i], z[i]);
-                            if ((i & 7) == 7) __syncwarp();
-                        }
-                    }
-                }
-            }
-            cp_async_wait_all();
-            __syncthreads();
-        }
     } else if (!flagged) {
         if constexpr (QFORM) {
             // row r of Q (stored by fast_tridiag in the output buffer) through the tile, HT rows per pass
@@ -1234,6 +1286,165 @@ fast_apply(double* __restrict__ V_, double* __restrict__ w_, int* __restrict__ i
             }
         }
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5 of letkf_syev_batched_f32 (the paper's precision): the
+// reflectors, the replay and the back-transform are fp32, the tridiagonal eigenproblem stays fp64
+// (ql_log_kernel / bisect_classify_kernel on the (d, e) the fp32 reduction left, twisted
+// factorisations in fp64: the orthogonality of Z to 2e-13 costs nothing next to the 2 M^3 fp32
+// flops behind it).  Same three routes as fast_apply; w is written as float on the way.
+template <int MT>
+__global__ void __launch_bounds__(FastCfg<MT>::NT, (MT == 64) ? 6 : (MT == 48 ? 7 : 16))
+fast_apply_f32(float* __restrict__ V_, double* __restrict__ w_, float* __restrict__ wf_, int* __restrict__ info_,
+               Workspace ws, int M)
+{
+    using C = FastCfg<MT>;
+    extern __shared__ __align__(16) double sm[];
+    double*   areg = sm;                                   // A region (ap_a_doubles)
+    float*    aregf = reinterpret_cast<float*>(sm);
+    double2*  cs   = reinterpret_cast<double2*>(sm);       // [2][AP_S][MT] while rotating
+    float*    Rf   = reinterpret_cast<float*>(sm + ap_a_doubles<MT>());   // reflectors, RefLayout order
+    float*    taus = Rf + RefLayout<MT>::TOTAL;
+    uint32_t* hdr  = reinterpret_cast<uint32_t*>(Rf + ((refl_doubles<MT>() + 3) & ~3));
+    int*      inv  = reinterpret_cast<int*>(hdr + ap_hdr_words<MT>(ws.swcap));
+    const int r = threadIdx.x;
+    const size_t b = blockIdx.x;
+    const int flag = ws.flags[b];
+    const bool direct = flag == FLAG_GETVEC;
+    bool flagged = flag == FLAG_SLOW;
+    const int nsw = (flag == FLAG_REPLAY) ? ws.nsweeps[b] : 0;
+    const double2* rot = ws.rot + b * ws.logcap;
+    constexpr int HT = MT < 32 ? MT : 32;
+    for (int s = r; s < nsw; s += C::NT) hdr[s] = ws.hdr[b * ws.swcap + s];
+    if (!flagged && r < M) inv[ws.perm[b * M + r]] = r;
+    {
+        const float* src = reinterpret_cast<const float*>(ws.refl + b * ws.reflstride);
+        for (int k = 4 * r; k < refl_doubles<MT>(); k += 4 * C::NT) cp_async16(Rf + k, src + k);
+    }
+    float z[MT];
+    bool columns = false;
+    if (direct) {
+        double zd[MT];
+        const bool ok = direct_eigenvectors<MT>(zd, hdr, areg, ws, w_, b, M, inv);
+        __syncthreads();
+        if (ok) {
+            columns = true;
+#pragma unroll
+            for (int c = 0; c < MT; ++c) z[c] = (float)zd[c];
+        } else {
+            flagged = true;
+        }
+    } else if (!flagged) {
+#pragma unroll
+        for (int c = 0; c < MT; ++c) z[c] = (c == r) ? 1.0f : 0.0f;
+        __syncthreads();
+        int spos = 0;
+        auto stage = [&](int round) {
+            double2* dst = cs + (round & 1) * AP_S * MT;
+#pragma unroll
+            for (int t = 0; t < AP_S; ++t) {
+                const int s = round * AP_S + t;
+                if (s < nsw) {
+                    const uint32_t h = hdr[s];
+                    const int lo = h & 0xffff, m = h >> 16;
+                    if (r < MT) {
+                        if (r >= lo && r < m) cp_async16(dst + t * MT + r, rot + spos + (m - 1 - r));
+                        else dst[t * MT + r] = make_double2(1.0, 0.0);
+                    }
+                    spos += m - lo;
+                }
+            }
+        };
+        const int nrounds = (nsw + AP_S - 1) / AP_S;
+        if (nrounds > 0) stage(0);
+        cp_async_wait_all();
+        __syncthreads();
+        for (int k = 0; k < nrounds; ++k) {
+            if (k + 1 < nrounds) stage(k + 1);
+            const double2* cur = cs + (k & 1) * AP_S * MT;
+            const int send = min(nsw, (k + 1) * AP_S);
+#pragma unroll 1
+            for (int s = k * AP_S; s < send; ++s) {
+                const uint32_t h = hdr[s];
+                apply_sweep<MT>(z, cur + (s - k * AP_S) * MT, h & 0xffff, h >> 16);
+            }
+            cp_async_wait_all();
+            __syncthreads();
+        }
+    }
+    if (flagged) {
+        double*  dsm  = areg;
+        double*  esm  = areg + MT;
+        double2* sink = reinterpret_cast<double2*>(areg + 2 * MT);
+        double2* csb  = sink + MT;
+        int*     ctl  = reinterpret_cast<int*>(csb + MT);
+        __syncthreads();
+#pragma unroll
+        for (int c = 0; c < MT; ++c) z[c] = (c == r) ? 1.0f : 0.0f;
+        if (r < M) { dsm[r] = ws.dws[b * M + r]; esm[r] = ws.ews[b * M + r]; }
+        __syncthreads();
+        QLState st{0, 0, 0, 0.0};
+        if (r == 0) { esm[M - 1] = 0.0; st.thr = ql_threshold(dsm, esm, 1, M); }
+        for (;;) {
+            if (r == 0) {
+                int lo = 0, m = 0;
+                ctl[0] = ql_next_sweep(st, dsm, esm, 1, M, sink, M, lo, m);
+                ctl[1] = lo; ctl[2] = m;
+            }
+            __syncthreads();
+            if (ctl[0] != 1) break;
+            const int lo = ctl[1], m = ctl[2];
+            if (r < MT) csb[r] = (r >= lo && r < m) ? sink[m - 1 - r] : make_double2(1.0, 0.0);
+            __syncthreads();
+            apply_sweep<MT>(z, csb, lo, m);
+            __syncthreads();
+        }
+        int* permsm = reinterpret_cast<int*>(sink);
+        if (r == 0) { sort_eigenvalues(dsm, 1, permsm, 1, M); ctl[3] = st.fail; }
+        __syncthreads();
+        if (r < M) { inv[permsm[r]] = r; w_[b * M + r] = dsm[r]; }
+        if (r == 0 && info_) info_[b] = ctl[3] | 0x40000000;
+        __syncthreads();
+    }
+    cp_async_wait_all();
+    __syncthreads();
+    if (r < M) wf_[b * M + r] = (float)w_[b * M + r];
+    if (!columns) transpose_regs<MT>(z, aregf);
+    q_groups_up<MT, 0, (MT - 2) / 8>(z, static_cast<const float*>(Rf), static_cast<const float*>(taus), M, 0);
+    // sorted, row-major V through the tile, HT rows per pass
+    float* V = V_ + b * M * M;
+    float* tile = aregf;
+    const int oc = (r < M) ? inv[r] : 0;
+#pragma unroll
+    for (int r0 = 0; r0 < MT; r0 += HT) {
+        if (r0 < M) {
+            __syncthreads();
+            if (r < M) {
+#pragma unroll
+                for (int rr = 0; rr < HT; ++rr)
+                    if (r0 + rr < MT) tile[rr * C::LDT + oc] = z[r0 + rr];
+            }
+            __syncthreads();
+            if (r < M) {
+                const int nr = min(HT, M - r0);
+#pragma unroll 8
+                for (int rr = 0; rr < nr; ++rr) V[(size_t)(r0 + rr) * M + r] = tile[rr * C::LDT + r];
+            }
+        }
+    }
+}
+template <int MT> size_t fast_apply_f32_smem(int swcap)
+{
+    return sizeof(double) * (size_t)ap_a_doubles<MT>() + sizeof(float) * (size_t)((refl_doubles<MT>() + 3) & ~3)
+         + sizeof(uint32_t) * (size_t)ap_hdr_words<MT>(swcap) + sizeof(int) * MT + 16;
+}
+
+// M = 1 of the fp32 entry point
+__global__ void f32_order_one(const float* __restrict__ A, float* __restrict__ w, float* __restrict__ V, int* __restrict__ info, int batch)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < batch) { w[b] = A[b]; V[b] = 1.0f; if (info) info[b] = 0; }
 }
 
 static inline bool fast_supported(int M) { return M >= 2 && M <= 64; }

@@ -243,7 +243,7 @@ static int fast_tridiag_run(const double* A, double* V, Workspace ws, int M, int
         if ((ce = allow_smem(fast_tridiag<MT, true, QFORM>, smem)) != cudaSuccess) return (int)ce;
         KLAUNCH("fast_tridiag<gram>", st,
                 fast_tridiag<MT, true, QFORM><<<n, FastCfg<MT>::NT, smem, st>>>(
-                    nullptr, V, ws, M, gram->Yb, gram->d, gram->r, gram->p, gram->shift, gram->gout, gram->grid));
+                    static_cast<const double*>(nullptr), V, ws, M, gram->Yb, gram->d, gram->r, gram->p, gram->shift, gram->gout, gram->grid));
     } else {
         if ((ce = allow_smem(fast_tridiag<MT, false, QFORM>, smem)) != cudaSuccess) return (int)ce;
         KLAUNCH("fast_tridiag", st,
@@ -568,6 +568,28 @@ struct ScopedWork {
     ~ScopedWork() { if (owned && ptr) cudaFreeAsync(ptr, st); }
 };
 
+// ---- fp32 variant -----------------------------------------------------
+template <int MT>
+static int f32_tridiag_run(const float* A, Workspace ws, int M, int n, cudaStream_t st)
+{
+    const size_t smem = fast_tridiag_smem<MT, float>();
+    cudaError_t ce;
+    if ((ce = allow_smem(fast_tridiag<MT, false, false, float>, smem)) != cudaSuccess) return (int)ce;
+    KLAUNCH("fast_tridiag<f32>", st,
+            fast_tridiag<MT, false, false, float><<<n, FastCfg<MT>::NT, smem, st>>>(
+                A, static_cast<float*>(nullptr), ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{}));
+    return 0;
+}
+template <int MT>
+static int f32_apply_run(float* V, double* wd, float* w, int* info, Workspace ws, int M, int n, cudaStream_t st)
+{
+    const size_t smem = fast_apply_f32_smem<MT>(ws.swcap);
+    cudaError_t ce;
+    if ((ce = allow_smem(fast_apply_f32<MT>, smem)) != cudaSuccess) return (int)ce;
+    KLAUNCH("fast_apply<f32>", st, fast_apply_f32<MT><<<n, FastCfg<MT>::NT, smem, st>>>(V, wd, w, info, ws, M));
+    return 0;
+}
+
 }  // namespace letkf
 
 using namespace letkf;
@@ -634,6 +656,74 @@ int letkf_syev_batched(const double* A, int M, int batch, double* w, double* V, 
     int rc = sw.acquire(work, work_bytes, syev_need(M, pl), st, 7);
     if (rc) return rc;
     return syev_core(A, M, batch, w, V, info, sw.ptr, pl, st);
+}
+
+size_t letkf_syev_f32_workspace_bytes(int M, int batch)
+{
+    EntryScope scope;
+    if (M < 1 || M > 64 || batch < 1) return 0;
+    t_opt.qform = 0; t_opt.force_generic = 0;
+    const size_t extra = sizeof(double) * (size_t)M;
+    const Plan pl = make_plan(M, batch, extra, 0);
+    return plan_bytes(M, (size_t)pl.per * pl.nslot, (size_t)pl.per * pl.nlog, extra, pl.two_pass);
+}
+
+int letkf_syev_batched_f32(const float* A, int M, int batch, float* w, float* V, int* info,
+                           void* work, size_t work_bytes, void* stream)
+{
+    EntryScope scope;
+    g_launches = 0;
+    if (M < 1 || M > 64) return -2;            // the register path only (the paper's Table I sizes)
+    if (batch < 0) return -3;
+    if (batch == 0) return LETKF_OK;
+    if (!A || misaligned(A)) return -1;
+    if (!w || misaligned(w)) return -4;
+    if (!V || misaligned(V)) return -5;
+    t_opt.qform = 0; t_opt.force_generic = 0;  // this entry point has the reflector form only
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    prof_reset(st);
+    const size_t extra = sizeof(double) * (size_t)M;
+    const Plan pl = make_plan(M, batch, extra, work ? work_bytes : 0);
+    ScopedWork sw;
+    int rc = sw.acquire(work, work_bytes, plan_bytes(M, (size_t)pl.per * pl.nslot, (size_t)pl.per * pl.nlog, extra, pl.two_pass), st, 7);
+    if (rc) return rc;
+    Workspace ws;
+    const size_t off = carve(ws, sw.ptr, M, pl.per * pl.nslot, pl.per * pl.nlog, pl.two_pass);
+    double* wd = reinterpret_cast<double*>(reinterpret_cast<char*>(sw.ptr) + off);      // [slot matrices][M] eigenvalues in fp64
+    if (M == 1) {      // nothing to reduce: w = A, V = 1 (the kernels want M >= 2)
+        KLAUNCH("f32_order_one", st, f32_order_one<<<(batch + 255) / 256, 256, 0, st>>>(A, w, V, info, batch));
+        return LETKF_OK;
+    }
+    auto stageT = [&](int b0, int nk, int s0, int l0, cudaStream_t s) {
+        const Workspace wk = ws_slice(ws, M, s0, l0);
+        switch (fast_bucket(M)) {
+            case 16: return f32_tridiag_run<16>(A + (size_t)b0 * M * M, wk, M, nk, s);
+            case 32: return f32_tridiag_run<32>(A + (size_t)b0 * M * M, wk, M, nk, s);
+            case 48: return f32_tridiag_run<48>(A + (size_t)b0 * M * M, wk, M, nk, s);
+            default: return f32_tridiag_run<64>(A + (size_t)b0 * M * M, wk, M, nk, s);
+        }
+    };
+    auto stageQL = [&](int b0, int nk, int s0, int l0, cudaStream_t s, bool logpass) {
+        const Workspace wk = ws_slice(ws, M, s0, l0);
+        int* ik = info ? info + b0 : nullptr;
+        if (logpass) return stage_QLlog(M, nk, wd + (size_t)s0 * M, ik, wk, s, pl.bisect);
+        if (pl.bisect) return stage_bisect(M, nk, wd + (size_t)s0 * M, ik, wk, s);
+        return stage_QL(M, nk, wd + (size_t)s0 * M, ik, wk, s, pl.ql_mode);
+    };
+    auto stageAP = [&](int b0, int nk, int s0, int l0, cudaStream_t s) {
+        const Workspace wk = ws_slice(ws, M, s0, l0);
+        int* ik = info ? info + b0 : nullptr;
+        float* Vk = V + (size_t)b0 * M * M;
+        float* wk_ = w + (size_t)b0 * M;
+        switch (fast_bucket(M)) {
+            case 16: return f32_apply_run<16>(Vk, wd + (size_t)s0 * M, wk_, ik, wk, M, nk, s);
+            case 32: return f32_apply_run<32>(Vk, wd + (size_t)s0 * M, wk_, ik, wk, M, nk, s);
+            case 48: return f32_apply_run<48>(Vk, wd + (size_t)s0 * M, wk_, ik, wk, M, nk, s);
+            default: return f32_apply_run<64>(Vk, wd + (size_t)s0 * M, wk_, ik, wk, M, nk, s);
+        }
+    };
+    auto post = [&](int, int, int, int, cudaStream_t) { return 0; };
+    return run_pipeline(pl, batch, st, stageT, stageQL, stageAP, post);
 }
 
 // per-matrix bytes the analysis keeps per slot beside the EVD workspace: Q / V (not on the fused

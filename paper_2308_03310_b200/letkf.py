@@ -21,6 +21,7 @@ INFO_SLOWPATH = 0x40000000
 
 EXPORTS = (
     "letkf_syev_batched", "letkf_syev_workspace_bytes",
+    "letkf_syev_batched_f32", "letkf_syev_f32_workspace_bytes",
     "letkf_analysis_batched", "letkf_analysis_workspace_bytes",
     "letkf_syev_batched_host", "letkf_analysis_batched_host", "letkf_host_release",
     "letkf_analysis_grid", "letkf_analysis_grid_workspace_bytes", "letkf_analysis_grid_host",
@@ -51,6 +52,10 @@ def load():
     lib.letkf_syev_batched.restype = ci
     lib.letkf_syev_workspace_bytes.argtypes = [ci, ci]
     lib.letkf_syev_workspace_bytes.restype = sz
+    lib.letkf_syev_batched_f32.argtypes = [vp, ci, ci, vp, vp, vp, vp, sz, vp]
+    lib.letkf_syev_batched_f32.restype = ci
+    lib.letkf_syev_f32_workspace_bytes.argtypes = [ci, ci]
+    lib.letkf_syev_f32_workspace_bytes.restype = sz
     lib.letkf_analysis_batched.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, cd,
                                            vp, vp, vp, vp, vp, sz, vp]
     lib.letkf_analysis_batched.restype = ci
@@ -174,6 +179,35 @@ def syev_batched(A, w=None, V=None, info=None, work=None, stream=None):
         st = lib.letkf_syev_batched(_ptr(A), M, batch, _ptr(w), _ptr(V), _ptr(info),
                                     _ptr(work), wb, _stream(stream))
     _check(st, "letkf_syev_batched")
+    return w, V, info
+
+
+def syev_f32_workspace_bytes(M, batch):
+    return load().letkf_syev_f32_workspace_bytes(M, batch)
+
+
+def syev_batched_f32(A, w=None, V=None, info=None, work=None, stream=None):
+    """letkf_syev_batched_f32: the EVD in the paper's precision, A[batch][M][M] float32, M <= 64
+    -> (w, V, info) with w, V float32.  ``V`` may be ``A`` itself."""
+    lib = load()
+    if not (isinstance(A, torch.Tensor) and A.is_cuda and A.dtype == torch.float32 and A.is_contiguous()):
+        raise LetkfError("A must be a contiguous float32 CUDA tensor")
+    batch, M, M2 = A.shape
+    if M != M2:
+        raise LetkfError("A must be [batch][M][M]")
+    if w is None:
+        w = torch.empty((batch, M), dtype=torch.float32, device=A.device)
+    if V is None:
+        V = torch.empty_like(A)
+    if info is None:
+        info = torch.zeros((batch,), dtype=torch.int32, device=A.device)
+    _out(w, "w", (batch, M), A.device, torch.float32)
+    _out(V, "V", (batch, M, M), A.device, torch.float32)
+    _out(info, "info", (batch,), A.device, torch.int32)
+    wb = _work(work, A.device, 0)
+    with torch.cuda.device(A.device):
+        st = lib.letkf_syev_batched_f32(_ptr(A), M, batch, _ptr(w), _ptr(V), _ptr(info), _ptr(work), wb, _stream(stream))
+    _check(st, "letkf_syev_batched_f32")
     return w, V, info
 
 
