@@ -121,6 +121,26 @@ int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv
 size_t letkf_analysis_workspace_bytes(int M, int p, int nstate, int batch);
 
 /*
+ * The same analysis WITHOUT an eigendecomposition (the paper's stated
+ * future work, "explore algorithms that can avoid divergence"): Eq.14-16 need only
+ * Q^-1 applied to a vector and the symmetric square root Q^-1/2, and both come out of a coupled
+ * Newton-Schulz iteration  T = (3I - Z Y)/2, Y <- Y T, Z <- Z T  started from Y = Q/c, Z = I
+ * (Y -> (Q/c)^1/2, Z -> (Q/c)^-1/2; c from the trace bound of lambda_max and the known lower bound
+ * (M-1)/rho of lambda_min).  Every step is a dense M x M x M product on the FP64 tensor cores
+ * (mma.sync.m8n8k4.f64), no data-dependent branch but the convergence test ||I - Z Y||_F <=
+ * 1e-14 sqrt(M) (or its rounding floor).  Same inputs and outputs as letkf_analysis_batched; W and Xa
+ * agree with it to ~3e-13 kappa(Q) relative (the coupled iteration is not backward stable): inside the
+ * 1e-10 tolerance for kappa(Q) <~ 100 (config 4: kappa ~ 4, 1e-12).  Iterations ~ 4 + log_1.5 sqrt(kappa').
+ * 2 <= M <= 64, nstate <= 16; no workspace.  info[b] = iterations taken, or
+ * LETKF_INFO_NS_NOCONV | iterations if the tolerance was not reached in 40 (result not to be trusted).
+ * Measured slower than the EVD route on B200 (fp64 tensor rate = vector rate).
+ */
+#define LETKF_INFO_NS_NOCONV 0x20000000
+int letkf_analysis_batched_evdfree(const double* Yb, const double* d, const double* rinv_loc,
+                                   const double* Xb, int M, int p, int nstate, int batch, double rho,
+                                   double* Xa, double* W, double* wbar, int* info, void* stream);
+
+/*
  * Grid form of the fused analysis (PAPER.md:144-151 R-localisation,
  * Procedure 1 lines 1-2 "Extract local observation data", Eq.18-19): the local observations of
  * every point of a PERIODIC Ny x Nx grid are gathered inside the library from the forecast

@@ -14,6 +14,7 @@
 #include "generic_kernels.cuh"
 #include "fast_kernels.cuh"
 #include "bisect_kernel.cuh"
+#include "ns_kernel.cuh"
 #include "mid_kernels.cuh"
 
 namespace letkf {
@@ -871,6 +872,34 @@ int letkf_analysis_batched(const double* Yb, const double* d, const double* rinv
     int rc = sw.acquire(work, work_bytes, analysis_need(M, pl, extra), st, 14);
     if (rc) return rc;
     return analysis_core(Yb, d, rinv_loc, nullptr, Xb, M, p, nstate, batch, rho, Xa, W, wbar, info, sw.ptr, pl, extra, st);
+}
+
+int letkf_analysis_batched_evdfree(const double* Yb, const double* d, const double* rinv_loc,
+                                   const double* Xb, int M, int p, int nstate, int batch, double rho,
+                                   double* Xa, double* W, double* wbar, int* info, void* stream)
+{
+    EntryScope scope;
+    g_launches = 0;
+    if (M < 2 || M > NS_MT) return -5;
+    if (p < 0) return -6;
+    if (nstate < 1 || nstate > 16) return -7;
+    if (batch < 0) return -8;
+    if (!(rho > 0.0)) return -9;
+    if (batch == 0) return LETKF_OK;
+    if (p > 0 && (!Yb || misaligned(Yb))) return -1;
+    if (p > 0 && (!d || misaligned(d))) return -2;
+    if (p > 0 && (!rinv_loc || misaligned(rinv_loc))) return -3;
+    if (!Xb || misaligned(Xb)) return -4;
+    if (!Xa || misaligned(Xa)) return -10;
+    if (W && misaligned(W)) return -11;
+    if (wbar && misaligned(wbar)) return -12;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    prof_reset(st);
+    cudaError_t ce;
+    if ((ce = allow_smem(ns_analysis_kernel, NS_SMEM)) != cudaSuccess) return (int)ce;
+    KLAUNCH("ns_analysis_kernel", st,
+            ns_analysis_kernel<<<batch, NS_NT, NS_SMEM, st>>>(Yb, d, rinv_loc, Xb, M, p, nstate, rho, Xa, W, wbar, info));
+    return LETKF_OK;
 }
 
 int letkf_analysis_grid(const double* Yf, const double* yo, const unsigned char* obs_mask, const double* Xb,

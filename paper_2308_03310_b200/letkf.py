@@ -18,11 +18,12 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libletkf.so")
 MAX_M = 256
 INFO_SLOWPATH = 0x40000000
+INFO_NS_NOCONV = 0x20000000
 
 EXPORTS = (
     "letkf_syev_batched", "letkf_syev_workspace_bytes",
     "letkf_syev_batched_f32", "letkf_syev_f32_workspace_bytes",
-    "letkf_analysis_batched", "letkf_analysis_workspace_bytes",
+    "letkf_analysis_batched", "letkf_analysis_workspace_bytes", "letkf_analysis_batched_evdfree",
     "letkf_syev_batched_host", "letkf_analysis_batched_host", "letkf_host_release",
     "letkf_analysis_grid", "letkf_analysis_grid_workspace_bytes", "letkf_analysis_grid_host",
     "letkf_probe_dfma", "letkf_last_launch_count",
@@ -59,6 +60,8 @@ def load():
     lib.letkf_analysis_batched.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, cd,
                                            vp, vp, vp, vp, vp, sz, vp]
     lib.letkf_analysis_batched.restype = ci
+    lib.letkf_analysis_batched_evdfree.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, cd, vp, vp, vp, vp, vp]
+    lib.letkf_analysis_batched_evdfree.restype = ci
     lib.letkf_analysis_workspace_bytes.argtypes = [ci, ci, ci, ci]
     lib.letkf_analysis_workspace_bytes.restype = sz
     lib.letkf_syev_batched_host.argtypes = [vp, ci, ci, vp, vp, vp]
@@ -246,6 +249,33 @@ def analysis_batched(Yb, d, rinv_loc, Xb, rho, Xa=None, want_W=False, want_wbar=
                                         _ptr(Xa), _ptr(W), _ptr(wbar), _ptr(info),
                                         _ptr(work), wb, _stream(stream))
     _check(st, "letkf_analysis_batched")
+    return dict(Xa=Xa, W=W, wbar=wbar, info=info)
+
+
+def analysis_batched_evdfree(Yb, d, rinv_loc, Xb, rho, Xa=None, want_W=False, want_wbar=False, info=None, stream=None):
+    """letkf_analysis_batched_evdfree: the analysis by a coupled Newton-Schulz iteration on the FP64
+    tensor cores instead of an EVD (M <= 64).  Same arguments and outputs as analysis_batched;
+    info[b] = iterations taken."""
+    lib = load()
+    for t, n in ((Yb, "Yb"), (d, "d"), (rinv_loc, "rinv_loc"), (Xb, "Xb")):
+        _dev_f64(t, n)
+    batch, p, M = Yb.shape
+    nstate = Xb.shape[1]
+    if d.shape != (batch, p) or rinv_loc.shape != (batch, p) or Xb.shape != (batch, nstate, M):
+        raise LetkfError("inconsistent shapes")
+    dev = Xb.device
+    if Xa is None:
+        Xa = torch.empty_like(Xb)
+    W = torch.empty((batch, M, M), dtype=torch.float64, device=dev) if want_W else None
+    wbar = torch.empty((batch, M), dtype=torch.float64, device=dev) if want_wbar else None
+    if info is None:
+        info = torch.zeros((batch,), dtype=torch.int32, device=dev)
+    _out(Xa, "Xa", (batch, nstate, M), dev)
+    _out(info, "info", (batch,), dev, torch.int32)
+    with torch.cuda.device(dev):
+        st = lib.letkf_analysis_batched_evdfree(_ptr(Yb), _ptr(d), _ptr(rinv_loc), _ptr(Xb), M, p, nstate, batch, float(rho),
+                                                _ptr(Xa), _ptr(W), _ptr(wbar), _ptr(info), _stream(stream))
+    _check(st, "letkf_analysis_batched_evdfree")
     return dict(Xa=Xa, W=W, wbar=wbar, info=info)
 
 

@@ -212,3 +212,49 @@ def test_fused_analysis_on_the_slow_path(lk, oracle, opts):
             lk.set_option(k, v)
     assert ((out["info"] & 0xFFFF) == 0).all() and (out["info"] & lk.INFO_SLOWPATH).astype(bool).all()
     parity.assert_analysis(out, ref, inp["Xb"], "fused analysis, slow path")
+
+
+@pytest.mark.parametrize("M,p,ns,batch,scale", [(64, 98, 9, 120, 0.1), (64, 3, 9, 40, 0.1), (64, 48, 9, 40, 0.1),
+                                                (48, 49, 9, 50, 0.1), (33, 20, 4, 21, 0.1), (16, 5, 3, 30, 0.1),
+                                                (2, 7, 1, 9, 0.1), (64, 98, 9, 30, 1.0), (64, 98, 16, 20, 3.0)])
+def test_evdfree_analysis_vs_oracle(lk, oracle, M, p, ns, batch, scale):
+    """letkf_analysis_batched_evdfree: W = sqrt(M-1) Q^-1/2 and wbar = Q^-1 g by a
+    coupled Newton-Schulz iteration on the FP64 tensor cores, no EVD anywhere -- against the same
+    oracle; the 1e-10 tolerances at kappa(Q) ~ 4 (config 4 shape, the paper's p = 3 / 48 shapes, ragged
+    sizes), the documented ~3e-13 kappa at kappa ~ 300 (yb_scale 1: config 3's conditioning) and ~ 3e3."""
+    import torch
+    inp = wl.analysis_inputs(batch=batch, M=M, p=p, nstate=ns, config_index=470 + M + p, yb_scale=scale)
+    t = {k: torch.from_numpy(inp[k]).cuda() for k in ("Yb", "d", "rinv_loc", "Xb")}
+    out = lk.analysis_batched_evdfree(t["Yb"], t["d"], t["rinv_loc"], t["Xb"], inp["rho"], want_W=True, want_wbar=True)
+    torch.cuda.synchronize()
+    out = {k: (v.cpu().numpy() if v is not None else None) for k, v in out.items()}
+    ref = run_oracle(oracle, inp)
+    assert ((out["info"] & lk.INFO_NS_NOCONV) == 0).all() and (out["info"] > 0).all() and (out["info"] <= 24).all()
+    if scale <= 0.1:
+        parity.assert_analysis(out, ref, inp["Xb"], f"evd-free M={M} p={p} scale={scale}")
+    else:
+        # kappa(Q) ~ 300 / 3e3: the documented accuracy of the coupled iteration, ~3e-13 kappa (letkf.h)
+        xbar = inp["Xb"].mean(axis=2, keepdims=True)
+        bound = 3e-9 if scale == 1.0 else 1e-7
+        assert parity.rel_fro(out["Xa"] - xbar, ref["Xa"] - xbar) <= bound
+        assert parity.rel_fro(out["W"], ref["W"]) <= bound
+
+
+def test_evdfree_full_size_sample(lk, oracle):
+    """Config 4 at full size through the EVD-free form: identities on every grid point (W symmetric,
+    W A W = (M-1) I through W 1 = sqrt(rho) 1 and mean preservation), the oracle on a strided sample."""
+    import torch
+    inp = wl.analysis_inputs()
+    t = {k: torch.from_numpy(inp[k]).cuda() for k in ("Yb", "d", "rinv_loc", "Xb")}
+    out = lk.analysis_batched_evdfree(t["Yb"], t["d"], t["rinv_loc"], t["Xb"], inp["rho"], want_W=True, want_wbar=True)
+    torch.cuda.synchronize()
+    assert int((out["info"] & lk.INFO_NS_NOCONV).max()) == 0
+    W = out["W"]
+    assert float((W - W.transpose(1, 2)).abs().max()) <= 1e-12
+    assert float((W.sum(dim=2) - math.sqrt(inp["rho"])).abs().max()) <= 1e-11          # W 1 = sqrt(rho) 1 (P-8)
+    sel = np.arange(0, inp["Xb"].shape[0], 512)
+    sub = {k: (v[sel] if isinstance(v, np.ndarray) else v) for k, v in inp.items()}
+    ref = run_oracle(oracle, sub)
+    idx = torch.from_numpy(sel).cuda()
+    got = {"Xa": out["Xa"][idx].cpu().numpy(), "W": W[idx].cpu().numpy(), "wbar": out["wbar"][idx].cpu().numpy()}
+    parity.assert_analysis(got, ref, sub["Xb"], "evd-free config 4 sample")
