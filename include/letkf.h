@@ -129,8 +129,8 @@ size_t letkf_analysis_workspace_bytes(int M, int p, int nstate, int batch);
  * (M-1)/rho of lambda_min).  Every step is a dense M x M x M product on the FP64 tensor cores
  * (mma.sync.m8n8k4.f64), no data-dependent branch but the convergence test ||I - Z Y||_F <=
  * 1e-14 sqrt(M) (or its rounding floor).  Same inputs and outputs as letkf_analysis_batched; W and Xa
- * agree with it to ~3e-13 kappa(Q) relative (the coupled iteration is not backward stable): inside the
- * 1e-10 tolerance for kappa(Q) <~ 100 (config 4: kappa ~ 4, 1e-12).  Iterations ~ 4 + log_1.5 sqrt(kappa').
+ * agree with it to ~3e-14 kappa(Q)^2 relative (the coupled iteration is not backward stable): inside the
+ * 1e-10 tolerance for kappa(Q) <~ 50 (config 4: kappa ~ 4, 1e-12; 3e-9 at kappa ~ 300, 2e-7 at 3e3).  Iterations ~ 4 + log_1.5 sqrt(kappa').
  * 2 <= M <= 64, nstate <= 16; no workspace.  info[b] = iterations taken, or
  * LETKF_INFO_NS_NOCONV | iterations if the tolerance was not reached in 40 (result not to be trusted).
  * Measured slower than the EVD route on B200 (fp64 tensor rate = vector rate).

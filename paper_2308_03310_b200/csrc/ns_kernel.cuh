@@ -20,8 +20,8 @@
 // alternative and as an independent route to the same numbers.
 // Accuracy (measured against the oracle): the coupled iteration is not backward stable -- Y_k = B Z_k
 // only holds up to the rounding errors committed so far, which later steps do not repair -- and W, Xa
-// come out within ~3e-13 kappa(Q) of the EVD route's: 1e-12 at config 4 (kappa ~ 4), 1e-10 at
-// kappa ~ 300, 1e-9 at kappa ~ 3e3.  (A final step Z <- Z (3I - Z B Z)/2 against the original B, the
+// come out within ~3e-14 kappa(Q)^2 of the EVD route's: 1e-12 at config 4 (kappa ~ 4), 3e-9 at
+// kappa ~ 300, 2e-7 at kappa ~ 3e3.  (A final step Z <- Z (3I - Z B Z)/2 against the original B, the
 // uncoupled Newton-Schulz step, makes it worse: that iteration is unstable for kappa >> 1; tried.)
 #pragma once
 #include "common.cuh"

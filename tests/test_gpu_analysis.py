@@ -221,7 +221,7 @@ def test_evdfree_analysis_vs_oracle(lk, oracle, M, p, ns, batch, scale):
     """letkf_analysis_batched_evdfree: W = sqrt(M-1) Q^-1/2 and wbar = Q^-1 g by a
     coupled Newton-Schulz iteration on the FP64 tensor cores, no EVD anywhere -- against the same
     oracle; the 1e-10 tolerances at kappa(Q) ~ 4 (config 4 shape, the paper's p = 3 / 48 shapes, ragged
-    sizes), the documented ~3e-13 kappa at kappa ~ 300 (yb_scale 1: config 3's conditioning) and ~ 3e3."""
+    sizes), the documented ~3e-14 kappa^2 at kappa ~ 300 (yb_scale 1: config 3's conditioning) and ~ 3e3."""
     import torch
     inp = wl.analysis_inputs(batch=batch, M=M, p=p, nstate=ns, config_index=470 + M + p, yb_scale=scale)
     t = {k: torch.from_numpy(inp[k]).cuda() for k in ("Yb", "d", "rinv_loc", "Xb")}
@@ -233,9 +233,9 @@ def test_evdfree_analysis_vs_oracle(lk, oracle, M, p, ns, batch, scale):
     if scale <= 0.1:
         parity.assert_analysis(out, ref, inp["Xb"], f"evd-free M={M} p={p} scale={scale}")
     else:
-        # kappa(Q) ~ 300 / 3e3: the documented accuracy of the coupled iteration, ~3e-13 kappa (letkf.h)
+        # kappa(Q) ~ 300 / 3e3: the documented accuracy of the coupled iteration, ~3e-14 kappa^2 (letkf.h)
         xbar = inp["Xb"].mean(axis=2, keepdims=True)
-        bound = 3e-9 if scale == 1.0 else 1e-7
+        bound = 3e-9 if scale == 1.0 else 1e-6
         assert parity.rel_fro(out["Xa"] - xbar, ref["Xa"] - xbar) <= bound
         assert parity.rel_fro(out["W"], ref["W"]) <= bound
 
