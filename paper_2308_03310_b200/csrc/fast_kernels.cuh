@@ -304,6 +304,15 @@ __device__ __forceinline__ void pivot_group(R (&a)[MT], const TriShared<R>& sh, 
     }
 }
 
+// groups G ... GLO only
+template <int MT, int G, int GLO, typename R>
+__device__ __forceinline__ void pivot_groups_range(R (&a)[MT], const TriShared<R>& sh, int M,
+                                                   double* __restrict__ dws, double* __restrict__ ews)
+{
+    pivot_group<MT, G>(a, sh, M, dws, ews);
+    if constexpr (G > GLO) pivot_groups_range<MT, G - 1, GLO>(a, sh, M, dws, ews);
+}
+
 template <int MT, int G, typename R>
 __device__ __forceinline__ void pivot_groups_down(R (&a)[MT], const TriShared<R>& sh, int M,
                                                   double* __restrict__ dws, double* __restrict__ ews)
@@ -397,7 +406,17 @@ grid_gather(GridArgs g, int M, int p, double* __restrict__ Yb, double* __restric
 // back-transform in fast_apply.
 template <int MT> __host__ __device__ constexpr int refl_doubles() { return RefLayout<MT>::TOTAL + FastCfg<MT>::NT; }
 
-template <int MT, bool GRAM, bool QFORM, typename R = double>
+// SPLIT (MT = 64, reflector form): this kernel stops after pivot 33 and hands the trailing 32 x 32
+// block (its lower triangle: 528 entries, parked where the reflectors of pivots 32 ... 1 will go),
+// the raw pivot column of pivot 32 and its norm to fast_tridiag_tail, one warp per matrix -- so that
+// no warp sits at a barrier holding 64 rows' worth of registers while another reduces the last 32
+// pivots (ncu, unsplit: barrier stall 1.4 cycles per issue, profiles/r02_ncu_key_metrics.txt).
+// letkf_set_option("split", 1); OFF by default: measured 1.22 + 0.25 ms against 1.46 ms for the one
+// kernel (config 3) -- the head kernel spills 364 bytes inside the pivot loop where the whole kernel
+// spills 152, whatever shape the hand-over code is given (ptxas), and that eats the gain.
+constexpr int SPLIT_LOW = 528, SPLIT_XS = 528, SPLIT_RED = 560;      // offsets inside the first 640 entries
+
+template <int MT, bool GRAM, bool QFORM, typename R = double, bool SPLIT = false>
 __global__ void __launch_bounds__(FastCfg<MT>::NT) __maxnreg__((MT == 64) ? LETKF_TRI_REGS64 : (MT == 48 ? 168 : (MT == 32 ? 128 : 80)))
 fast_tridiag(const R* __restrict__ A_, R* __restrict__ Q_, Workspace ws, int M,
                    const double* __restrict__ Yb_, const double* __restrict__ d_,
@@ -601,7 +620,26 @@ fast_tridiag(const R* __restrict__ A_, R* __restrict__ Q_, Workspace ws, int M,
     }
     // a warp leaves pivot_groups_down when the rows it holds are done (after the B1 that closes
     // the last pivot it took part in), the others carry on with barriers that no longer count it
-    pivot_groups_down<MT, (MT - 2) / 8>(a, sh, M, dws, ews);
+    if constexpr (SPLIT) {
+        static_assert(MT == 64 && !QFORM, "the split form is for the MT = 64 bucket, reflector form");
+        pivot_groups_range<MT, (MT - 2) / 8, 4>(a, sh, M, dws, ews);
+        __syncthreads();
+        R* out = reinterpret_cast<R*>(ws.refl + b * ws.reflstride);
+        for (int k = RefLayout<MT>::base(4) + j; k < RefLayout<MT>::TOTAL; k += C::NT) out[k] = Rf[k];
+        out[RefLayout<MT>::TOTAL + j] = (j >= 33 && j <= M - 1) ? taus[j] : R(0);
+        if (j < 32) {
+            // row j of the lower triangle at j (j + 1) / 2
+            R* low = out + (j * (j + 1)) / 2;
+#pragma unroll
+            for (int c = 0; c < 32; ++c)
+                if (c <= j) low[c] = a[c];
+            out[SPLIT_XS + j] = sh.xs[j];
+            if (j == 0) { out[SPLIT_RED] = sh.red[0] + sh.red[1]; out[SPLIT_RED + 1] = sh.red[4]; }
+        }
+        return;
+    } else {
+        pivot_groups_down<MT, (MT - 2) / 8>(a, sh, M, dws, ews);
+    }
     if constexpr (QFORM) {
         // ---- explicit Q = H_{M-1} ... H_1: thread r owns column r of Q; no synchronisation needed.
         // Column r only needs H_i with i > r, and a warp leaves the loop above exactly when all
@@ -626,6 +664,42 @@ fast_tridiag(const R* __restrict__ A_, R* __restrict__ Q_, Workspace ws, int M,
         out[RefLayout<MT>::TOTAL + j] = (j >= 1 && j <= M - 1) ? taus[j] : R(0);
     }
 }
+
+// Trailing 32 x 32 problem of the split form: pivots 32 ... 1, one warp per matrix (FastCfg<32>).
+template <typename R>
+__global__ void __maxnreg__(128)
+fast_tridiag_tail(Workspace ws, int M)
+{
+    constexpr int MT = 32;
+    extern __shared__ __align__(16) unsigned char sm_raw[];
+    R* sm = reinterpret_cast<R*>(sm_raw);
+    TriShared<R> sh;
+    sh.Rf = sm;                                  // groups 0..3: 640 entries
+    R* small = sm + 640;
+    sh.xs = small; sh.vbuf = small + 32; sh.pbuf = small + 64; sh.pv = small + 96;
+    sh.taus = small + 128;                       // [40]
+    sh.red = small + 168;                        // [8]
+    const int j = threadIdx.x;
+    const size_t b = blockIdx.x;
+    R* io = reinterpret_cast<R*>(ws.refl + b * ws.reflstride);
+    R a[MT];
+#pragma unroll
+    for (int c = 0; c < MT; ++c) {
+        const int hi = c > j ? c : j, lo = c > j ? j : c;
+        a[c] = io[(hi * (hi + 1)) / 2 + lo];
+    }
+    sh.xs[j] = io[SPLIT_XS + j];
+    if (j == 0) { sh.red[0] = io[SPLIT_RED]; sh.red[4] = io[SPLIT_RED + 1]; }
+    __syncwarp();
+    // as a 33 x 33 problem whose last column is already in xs: pivot 32 takes it from there
+    pivot_groups_down<MT, 3>(a, sh, 33, ws.dws + b * M, ws.ews + b * M);
+    __syncwarp();
+    for (int k = j; k < 640; k += 32) io[k] = sh.Rf[k];
+    constexpr int TOT64 = RefLayout<64>::TOTAL;
+    io[TOT64 + j] = (j >= 1) ? sh.taus[j] : R(0);
+    if (j == 0) io[TOT64 + 32] = sh.taus[32];
+}
+template <typename R> constexpr size_t fast_tridiag_tail_smem() { return sizeof(R) * (640 + 176); }
 
 // ---------------------------------------------------------------------------------------------
 // a5: V = Q Z = H_{M-1} ... H_1 Z.  Z is the product of the logged rotations: thread r replays

@@ -93,6 +93,8 @@ struct Options {
                              // which then does the back-transform (nothing but the reflectors crosses HBM in between)
     int bisect = -1;         // M <= 64, evec = 1: eigenvalues by multisection with M threads per matrix instead of the QL
                              // kernel's one (the latency regime): -1 = for batches up to BISECT_MAX_BATCH, 0 / 1
+    int split = 0;           // 48 < M <= 64, qform = 0: the reduction as two kernels (pivots down to 33 by two warps,
+                             // the trailing 32 x 32 problem by one warp per matrix); measured no faster, off
     int evec = 1;            // M <= 64, qform = 0: 1 = eigenvectors of T by twisted factorisations where the spectrum
                              // allows (ql_log_kernel classifies), the logged rotations otherwise; 0 = always the log
 };
@@ -240,6 +242,23 @@ static int fast_tridiag_run(const double* A, double* V, Workspace ws, int M, int
 {
     const size_t smem = fast_tridiag_smem<MT>();
     cudaError_t ce;
+    if constexpr (MT == 64 && !QFORM) {
+        if (t_opt.split && M > 48) {
+            if (gram) {
+                if ((ce = allow_smem(fast_tridiag<MT, true, false, double, true>, smem)) != cudaSuccess) return (int)ce;
+                KLAUNCH("fast_tridiag_head<gram>", st,
+                        (fast_tridiag<MT, true, false, double, true><<<n, FastCfg<MT>::NT, smem, st>>>(
+                            static_cast<const double*>(nullptr), V, ws, M, gram->Yb, gram->d, gram->r, gram->p, gram->shift, gram->gout, gram->grid)));
+            } else {
+                if ((ce = allow_smem(fast_tridiag<MT, false, false, double, true>, smem)) != cudaSuccess) return (int)ce;
+                KLAUNCH("fast_tridiag_head", st,
+                        (fast_tridiag<MT, false, false, double, true><<<n, FastCfg<MT>::NT, smem, st>>>(
+                            A, V, ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{})));
+            }
+            KLAUNCH("fast_tridiag_tail", st, fast_tridiag_tail<double><<<n, 32, fast_tridiag_tail_smem<double>(), st>>>(ws, M));
+            return 0;
+        }
+    }
     if (gram) {
         if ((ce = allow_smem(fast_tridiag<MT, true, QFORM>, smem)) != cudaSuccess) return (int)ce;
         KLAUNCH("fast_tridiag<gram>", st,
@@ -575,6 +594,16 @@ static int f32_tridiag_run(const float* A, Workspace ws, int M, int n, cudaStrea
 {
     const size_t smem = fast_tridiag_smem<MT, float>();
     cudaError_t ce;
+    if constexpr (MT == 64) {
+        if (t_opt.split && M > 48) {
+            if ((ce = allow_smem(fast_tridiag<MT, false, false, float, true>, smem)) != cudaSuccess) return (int)ce;
+            KLAUNCH("fast_tridiag_head<f32>", st,
+                    (fast_tridiag<MT, false, false, float, true><<<n, FastCfg<MT>::NT, smem, st>>>(
+                        A, static_cast<float*>(nullptr), ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{})));
+            KLAUNCH("fast_tridiag_tail<f32>", st, fast_tridiag_tail<float><<<n, 32, fast_tridiag_tail_smem<float>(), st>>>(ws, M));
+            return 0;
+        }
+    }
     if ((ce = allow_smem(fast_tridiag<MT, false, false, float>, smem)) != cudaSuccess) return (int)ce;
     KLAUNCH("fast_tridiag<f32>", st,
             fast_tridiag<MT, false, false, float><<<n, FastCfg<MT>::NT, smem, st>>>(
@@ -1316,6 +1345,7 @@ int letkf_set_option(const char* name, int value)
     if (strcmp(name, "host_pass") == 0) { o.host_pass = value >= 1 ? value : 0; return LETKF_OK; }
     if (strcmp(name, "qform") == 0) { o.qform = value != 0; return LETKF_OK; }
     if (strcmp(name, "evec") == 0) { o.evec = value != 0; return LETKF_OK; }
+    if (strcmp(name, "split") == 0) { o.split = value != 0; return LETKF_OK; }
     if (strcmp(name, "bisect") == 0) { o.bisect = (value == 0 || value == 1) ? value : -1; return LETKF_OK; }
     return -1;
 }
