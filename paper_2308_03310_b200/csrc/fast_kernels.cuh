@@ -244,15 +244,17 @@ template <typename R> struct TriShared {
 //       -> pass B  a_jc -= (p_j - tau (p.v) v_j) v_c, top block first: column i-1 is then final, it
 //          is the next pivot's x, whose norm tree overlaps the rest of pass B.
 // Entered and left with B1 done (by the NP warps that hold rows < 8G+8).
+// `j` is the row this thread holds (threadIdx.x, or the lane when a second warp reduces a trailing
+// block of its own in the paired kernel).
 template <int MT, int G, typename R>
 __device__ __forceinline__ void pivot_group(R (&a)[MT], const TriShared<R>& sh, int M,
-                                            double* __restrict__ dws, double* __restrict__ ews)
+                                            double* __restrict__ dws, double* __restrict__ ews, const int j)
 {
     using C = FastCfg<MT>;
     constexpr int NPR = (8 * G + 8 + 31) / 32;
     constexpr int NP = NPR < C::NW ? NPR : C::NW;
     constexpr unsigned FULL = 0xffffffffu;
-    const int j = threadIdx.x, lane = j & 31, warp = j >> 5;
+    const int lane = j & 31, warp = j >> 5;
     if (warp >= NP) return;
     const int ihi = (8 * G + 8 < M - 1) ? 8 * G + 8 : M - 1;
     for (int i = ihi; i >= 8 * G + 1; --i) {
@@ -307,18 +309,17 @@ __device__ __forceinline__ void pivot_group(R (&a)[MT], const TriShared<R>& sh, 
 // groups G ... GLO only
 template <int MT, int G, int GLO, typename R>
 __device__ __forceinline__ void pivot_groups_range(R (&a)[MT], const TriShared<R>& sh, int M,
-                                                   double* __restrict__ dws, double* __restrict__ ews)
+                                                   double* __restrict__ dws, double* __restrict__ ews, const int j)
 {
-    pivot_group<MT, G>(a, sh, M, dws, ews);
-    if constexpr (G > GLO) pivot_groups_range<MT, G - 1, GLO>(a, sh, M, dws, ews);
+    pivot_group<MT, G>(a, sh, M, dws, ews, j);
+    if constexpr (G > GLO) pivot_groups_range<MT, G - 1, GLO>(a, sh, M, dws, ews, j);
 }
 
 template <int MT, int G, typename R>
 __device__ __forceinline__ void pivot_groups_down(R (&a)[MT], const TriShared<R>& sh, int M,
                                                   double* __restrict__ dws, double* __restrict__ ews)
 {
-    pivot_group<MT, G>(a, sh, M, dws, ews);
-    if constexpr (G > 0) pivot_groups_down<MT, G - 1>(a, sh, M, dws, ews);
+    pivot_groups_range<MT, G, 0>(a, sh, M, dws, ews, (int)threadIdx.x);
 }
 
 // Grid form of the analysis (Procedure 1 lines 1-2,
@@ -416,15 +417,28 @@ template <int MT> __host__ __device__ constexpr int refl_doubles() { return RefL
 // spills 152, whatever shape the hand-over code is given (ptxas), and that eats the gain.
 constexpr int SPLIT_LOW = 528, SPLIT_XS = 528, SPLIT_RED = 560;      // offsets inside the first 640 entries
 
-template <int MT, bool GRAM, bool QFORM, typename R = double, bool SPLIT = false>
+// PAIR (two-warp buckets, reflector form): a CTA reduces TWO matrices.  Pivots M-1 ... 33 need both
+// warps (rows 0 ... 63), pivots 32 ... 1 only the warp that holds rows 0 ... 31 -- in the one-matrix
+// kernel the other warp then waits at the closing barrier for 36% of the CTA's life (ncu: barrier
+// stall 1.4 cycles per issue).  Here both heads run first (the trailing 32 x 32 block of the first
+// matrix is parked in shared memory meanwhile), then the two tails run side by side, one per warp,
+// each with its own set of broadcast vectors.
+constexpr int PAIR_PARK = 32 * 33;
+template <int MT, typename R = double, bool PAIR = false> constexpr size_t fast_tridiag_smem_pair()
+{
+    return fast_tridiag_smem<MT, R>() + (PAIR ? sizeof(R) * (640 + PAIR_PARK + 5 * FastCfg<MT>::NT + 8) : 0);
+}
+
+template <int MT, bool GRAM, bool QFORM, typename R = double, bool SPLIT = false, bool PAIR = false>
 __global__ void __launch_bounds__(FastCfg<MT>::NT) __maxnreg__((MT == 64) ? LETKF_TRI_REGS64 : (MT == 48 ? 168 : (MT == 32 ? 128 : 80)))
 fast_tridiag(const R* __restrict__ A_, R* __restrict__ Q_, Workspace ws, int M,
                    const double* __restrict__ Yb_, const double* __restrict__ d_,
                    const double* __restrict__ r_, int p, double shift, double* __restrict__ gout_,
-                   GridArgs grid)
+                   GridArgs grid, int nbatch)
 {
     using C = FastCfg<MT>;
     static_assert(!GRAM || sizeof(R) == sizeof(double), "the Gram step (DMMA) is fp64");
+    static_assert(!PAIR || (C::NW == 2 && !QFORM && !SPLIT), "pairs: two-warp buckets, reflector form");
     extern __shared__ __align__(16) unsigned char sm_raw[];
     R* sm = reinterpret_cast<R*>(sm_raw);
     R* tile = sm;
@@ -439,8 +453,15 @@ fast_tridiag(const R* __restrict__ A_, R* __restrict__ Q_, Workspace ws, int M,
     sh.red = small + 5 * C::NT;
     R* taus = sh.taus;
     const int j = threadIdx.x, lane = j & 31, warp = j >> 5;
-    const size_t b = blockIdx.x;
+    const int nmat = PAIR ? min(2, nbatch - 2 * (int)blockIdx.x) : 1;
+    R* Rf2 = small + 5 * C::NT + 8;                // PAIR: reflectors of the second tail, the parked block, its vectors
+    R* park = Rf2 + 640;
+    R* small2 = park + PAIR_PARK;
     R a[MT];
+#pragma unroll 1
+    for (int mi = 0; mi < nmat; ++mi) {
+    const size_t b = PAIR ? 2 * (size_t)blockIdx.x + mi : (size_t)blockIdx.x;
+    if (PAIR && mi) __syncthreads();               // the shared vectors and the staging tile are free again
 
     if constexpr (!GRAM) {
         // a_j[c] = A[max(j,c)][min(j,c)] (only the lower triangle is read), 32 rows per pass
@@ -622,7 +643,7 @@ fast_tridiag(const R* __restrict__ A_, R* __restrict__ Q_, Workspace ws, int M,
     // the last pivot it took part in), the others carry on with barriers that no longer count it
     if constexpr (SPLIT) {
         static_assert(MT == 64 && !QFORM, "the split form is for the MT = 64 bucket, reflector form");
-        pivot_groups_range<MT, (MT - 2) / 8, 4>(a, sh, M, dws, ews);
+        pivot_groups_range<MT, (MT - 2) / 8, 4>(a, sh, M, dws, ews, j);
         __syncthreads();
         R* out = reinterpret_cast<R*>(ws.refl + b * ws.reflstride);
         for (int k = RefLayout<MT>::base(4) + j; k < RefLayout<MT>::TOTAL; k += C::NT) out[k] = Rf[k];
@@ -637,6 +658,21 @@ fast_tridiag(const R* __restrict__ A_, R* __restrict__ Q_, Workspace ws, int M,
             if (j == 0) { out[SPLIT_RED] = sh.red[0] + sh.red[1]; out[SPLIT_RED + 1] = sh.red[4]; }
         }
         return;
+    } else if constexpr (PAIR) {
+        pivot_groups_range<MT, (MT - 2) / 8, 4>(a, sh, M, dws, ews, j);
+        __syncthreads();
+        {   // reflectors of pivots >= 33 and their taus leave now: the region is the next matrix's staging tile
+            R* out = reinterpret_cast<R*>(ws.refl + b * ws.reflstride);
+            for (int k = RefLayout<MT>::base(4) + j; k < RefLayout<MT>::TOTAL; k += C::NT) out[k] = Rf[k];
+            out[RefLayout<MT>::TOTAL + j] = (j >= 33 && j <= M - 1) ? taus[j] : R(0);
+        }
+        if (mi == 0 && nmat == 2 && j < 32) {      // park the trailing block, the raw pivot column and its norm
+#pragma unroll
+            for (int c = 0; c < 32; ++c) park[j * 33 + c] = a[c];
+            small2[j] = sh.xs[j];
+            if (j == 0) { small2[5 * C::NT] = sh.red[0] + sh.red[1]; small2[5 * C::NT + 4] = sh.red[4]; }
+        }
+        continue;
     } else {
         pivot_groups_down<MT, (MT - 2) / 8>(a, sh, M, dws, ews);
     }
@@ -662,6 +698,36 @@ fast_tridiag(const R* __restrict__ A_, R* __restrict__ Q_, Workspace ws, int M,
         R* out = reinterpret_cast<R*>(ws.refl + b * ws.reflstride);
         for (int k = j; k < RefLayout<MT>::TOTAL; k += C::NT) out[k] = Rf[k];
         out[RefLayout<MT>::TOTAL + j] = (j >= 1 && j <= M - 1) ? taus[j] : R(0);
+    }
+    }   // matrices of the CTA
+    if constexpr (PAIR) {
+        // ---- the tails: pivots min(32, M-1) ... 1, one matrix per warp
+        __syncthreads();
+        const size_t b0 = 2 * (size_t)blockIdx.x;
+        size_t bt = b0;
+        TriShared<R> st = sh;
+        if (nmat == 2) {
+            if (warp == 1) {                       // the first matrix: its block comes back from the park
+                st.Rf = Rf2;
+                st.xs = small2; st.vbuf = small2 + C::NT; st.pbuf = small2 + 2 * C::NT; st.pv = small2 + 3 * C::NT;
+                st.taus = small2 + 4 * C::NT; st.red = small2 + 5 * C::NT;
+#pragma unroll
+                for (int c = 0; c < 32; ++c) a[c] = park[lane * 33 + c];
+            } else {
+                bt = b0 + 1;                       // the second matrix is still in warp 0's registers
+                if (lane == 0) st.red[0] += st.red[1];
+            }
+        } else {
+            if (warp == 1) return;
+            if (lane == 0) st.red[0] += st.red[1];
+        }
+        __syncwarp();
+        pivot_groups_range<MT, 3, 0>(a, st, M, ws.dws + bt * M, ws.ews + bt * M, lane);
+        __syncwarp();
+        R* out = reinterpret_cast<R*>(ws.refl + bt * ws.reflstride);
+        for (int k = lane; k < 640; k += 32) out[k] = st.Rf[k];
+        if (lane >= 1) out[RefLayout<MT>::TOTAL + lane] = st.taus[lane];
+        if (lane == 0 && M > 32) out[RefLayout<MT>::TOTAL + 32] = st.taus[32];
     }
 }
 

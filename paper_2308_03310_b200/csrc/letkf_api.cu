@@ -93,6 +93,10 @@ struct Options {
                              // which then does the back-transform (nothing but the reflectors crosses HBM in between)
     int bisect = -1;         // M <= 64, evec = 1: eigenvalues by multisection with M threads per matrix instead of the QL
                              // kernel's one (the latency regime): -1 = for batches up to BISECT_MAX_BATCH, 0 / 1
+    int pair = -1;           // 32 < M <= 64, qform = 0: a CTA reduces two matrices, their trailing 32 x 32 blocks side by
+                             // side on its two warps (0: one matrix per CTA, the second warp idle through the last 32
+                             // pivots).  -1 = where it measured faster: 32 < M <= 48 without the Gram step (config 5,
+                             // M = 48: 1.74 -> 1.51 ms; at M = 64 the paired kernel spills and loses, 1.46 -> 1.65 ms)
     int split = 0;           // 48 < M <= 64, qform = 0: the reduction as two kernels (pivots down to 33 by two warps,
                              // the trailing 32 x 32 problem by one warp per matrix); measured no faster, off
     int evec = 1;            // M <= 64, qform = 0: 1 = eigenvectors of T by twisted factorisations where the spectrum
@@ -248,14 +252,31 @@ static int fast_tridiag_run(const double* A, double* V, Workspace ws, int M, int
                 if ((ce = allow_smem(fast_tridiag<MT, true, false, double, true>, smem)) != cudaSuccess) return (int)ce;
                 KLAUNCH("fast_tridiag_head<gram>", st,
                         (fast_tridiag<MT, true, false, double, true><<<n, FastCfg<MT>::NT, smem, st>>>(
-                            static_cast<const double*>(nullptr), V, ws, M, gram->Yb, gram->d, gram->r, gram->p, gram->shift, gram->gout, gram->grid)));
+                            static_cast<const double*>(nullptr), V, ws, M, gram->Yb, gram->d, gram->r, gram->p, gram->shift, gram->gout, gram->grid, n)));
             } else {
                 if ((ce = allow_smem(fast_tridiag<MT, false, false, double, true>, smem)) != cudaSuccess) return (int)ce;
                 KLAUNCH("fast_tridiag_head", st,
                         (fast_tridiag<MT, false, false, double, true><<<n, FastCfg<MT>::NT, smem, st>>>(
-                            A, V, ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{})));
+                            A, V, ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{}, n)));
             }
             KLAUNCH("fast_tridiag_tail", st, fast_tridiag_tail<double><<<n, 32, fast_tridiag_tail_smem<double>(), st>>>(ws, M));
+            return 0;
+        }
+    }
+    if constexpr ((MT == 64 || MT == 48) && !QFORM) {
+        if (t_opt.pair > 0 || (t_opt.pair < 0 && MT == 48 && !gram)) {
+            const size_t ps = fast_tridiag_smem_pair<MT, double, true>();
+            if (gram) {
+                if ((ce = allow_smem(fast_tridiag<MT, true, false, double, false, true>, ps)) != cudaSuccess) return (int)ce;
+                KLAUNCH("fast_tridiag<gram>", st,
+                        (fast_tridiag<MT, true, false, double, false, true><<<(n + 1) / 2, FastCfg<MT>::NT, ps, st>>>(
+                            static_cast<const double*>(nullptr), V, ws, M, gram->Yb, gram->d, gram->r, gram->p, gram->shift, gram->gout, gram->grid, n)));
+            } else {
+                if ((ce = allow_smem(fast_tridiag<MT, false, false, double, false, true>, ps)) != cudaSuccess) return (int)ce;
+                KLAUNCH("fast_tridiag", st,
+                        (fast_tridiag<MT, false, false, double, false, true><<<(n + 1) / 2, FastCfg<MT>::NT, ps, st>>>(
+                            A, V, ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{}, n)));
+            }
             return 0;
         }
     }
@@ -263,12 +284,12 @@ static int fast_tridiag_run(const double* A, double* V, Workspace ws, int M, int
         if ((ce = allow_smem(fast_tridiag<MT, true, QFORM>, smem)) != cudaSuccess) return (int)ce;
         KLAUNCH("fast_tridiag<gram>", st,
                 fast_tridiag<MT, true, QFORM><<<n, FastCfg<MT>::NT, smem, st>>>(
-                    static_cast<const double*>(nullptr), V, ws, M, gram->Yb, gram->d, gram->r, gram->p, gram->shift, gram->gout, gram->grid));
+                    static_cast<const double*>(nullptr), V, ws, M, gram->Yb, gram->d, gram->r, gram->p, gram->shift, gram->gout, gram->grid, n));
     } else {
         if ((ce = allow_smem(fast_tridiag<MT, false, QFORM>, smem)) != cudaSuccess) return (int)ce;
         KLAUNCH("fast_tridiag", st,
                 fast_tridiag<MT, false, QFORM><<<n, FastCfg<MT>::NT, smem, st>>>(
-                    A, V, ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{}));
+                    A, V, ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{}, n));
     }
     return 0;
 }
@@ -599,15 +620,25 @@ static int f32_tridiag_run(const float* A, Workspace ws, int M, int n, cudaStrea
             if ((ce = allow_smem(fast_tridiag<MT, false, false, float, true>, smem)) != cudaSuccess) return (int)ce;
             KLAUNCH("fast_tridiag_head<f32>", st,
                     (fast_tridiag<MT, false, false, float, true><<<n, FastCfg<MT>::NT, smem, st>>>(
-                        A, static_cast<float*>(nullptr), ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{})));
+                        A, static_cast<float*>(nullptr), ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{}, n)));
             KLAUNCH("fast_tridiag_tail<f32>", st, fast_tridiag_tail<float><<<n, 32, fast_tridiag_tail_smem<float>(), st>>>(ws, M));
+            return 0;
+        }
+    }
+    if constexpr (MT == 64 || MT == 48) {
+        if (t_opt.pair > 0) {
+            const size_t ps = fast_tridiag_smem_pair<MT, float, true>();
+            if ((ce = allow_smem(fast_tridiag<MT, false, false, float, false, true>, ps)) != cudaSuccess) return (int)ce;
+            KLAUNCH("fast_tridiag<f32>", st,
+                    (fast_tridiag<MT, false, false, float, false, true><<<(n + 1) / 2, FastCfg<MT>::NT, ps, st>>>(
+                        A, static_cast<float*>(nullptr), ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{}, n)));
             return 0;
         }
     }
     if ((ce = allow_smem(fast_tridiag<MT, false, false, float>, smem)) != cudaSuccess) return (int)ce;
     KLAUNCH("fast_tridiag<f32>", st,
             fast_tridiag<MT, false, false, float><<<n, FastCfg<MT>::NT, smem, st>>>(
-                A, static_cast<float*>(nullptr), ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{}));
+                A, static_cast<float*>(nullptr), ws, M, nullptr, nullptr, nullptr, 0, 0.0, nullptr, GridArgs{}, n));
     return 0;
 }
 template <int MT>
@@ -1346,6 +1377,7 @@ int letkf_set_option(const char* name, int value)
     if (strcmp(name, "qform") == 0) { o.qform = value != 0; return LETKF_OK; }
     if (strcmp(name, "evec") == 0) { o.evec = value != 0; return LETKF_OK; }
     if (strcmp(name, "split") == 0) { o.split = value != 0; return LETKF_OK; }
+    if (strcmp(name, "pair") == 0) { o.pair = (value == 0 || value == 1) ? value : -1; return LETKF_OK; }
     if (strcmp(name, "bisect") == 0) { o.bisect = (value == 0 || value == 1) ? value : -1; return LETKF_OK; }
     return -1;
 }

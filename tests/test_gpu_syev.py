@@ -347,7 +347,8 @@ def test_mid_tridiagonalisation_both_forms(lk, oracle, M, mode):
     parity.assert_evd(A, w, V, wo, f"mid M={M} mid_reg={mode}")
 
 
-VARIANTS = {"direct": {}, "replay": {"evec": 0}, "qform": {"qform": 1}, "split": {"split": 1}}
+VARIANTS = {"direct": {}, "replay": {"evec": 0}, "qform": {"qform": 1}, "split": {"split": 1}, "pair": {"pair": 1},
+            "nopair": {"pair": 0}}
 
 
 @pytest.mark.parametrize("variant", sorted(VARIANTS))
@@ -359,7 +360,8 @@ def test_register_path_variants(lk, oracle, M, p, variant):
     (else it replays the logged rotations on the identity) and does the back-transform
     V = H_{M-1} ... H_1 Z.  "replay" (evec = 0): always the logged rotations.  "qform" (qform = 1):
     the explicit Q is formed by the reduction kernel and the rotations are replayed on its rows.
-    "split" (split = 1, acts for 48 < M <= 64): the reduction as two kernels.
+    "split" (split = 1, acts for 48 < M <= 64): the reduction as two kernels.  "pair" / "nopair"
+    (32 < M <= 64): two matrices per CTA of the reduction kernel, or one (odd batch: a CTA with one).
     Each also with the rotation log shrunk, which sends the replaying matrices to the classic
     iteration inside the apply kernel."""
     A = wl.letkf_shaped(150, M, p, config_index=990 + M + p)
@@ -370,14 +372,14 @@ def test_register_path_variants(lk, oracle, M, p, variant):
         lk.set_option("log_shrink", 4)
         w2, V2, info2 = run_gpu(lk, A)
     finally:
-        for k, v in (("qform", 0), ("evec", 1), ("log_shrink", 1), ("split", 0)):
+        for k, v in (("qform", 0), ("evec", 1), ("log_shrink", 1), ("split", 0), ("pair", -1)):
             lk.set_option(k, v)
     assert (info == 0).all()
     wo, _, _, _ = oracle.syev_batched(A)
     parity.assert_evd(A, w, V, wo, f"{variant} M={M}")
     parity.assert_evd(A, w2, V2, wo, f"{variant}, log shrunk, M={M}")
     assert ((info2 & 0xFFFF) == 0).all()
-    if p >= M - 1 and M >= 16 and variant not in ("direct", "split"):
+    if p >= M - 1 and M >= 16 and variant in ("replay", "qform"):
         assert (info2 & lk.INFO_SLOWPATH).astype(bool).all()
 
 
