@@ -364,7 +364,7 @@ def test_register_path_variants(lk, oracle, M, p, variant):
     (32 < M <= 64): two matrices per CTA of the reduction kernel, or one (odd batch: a CTA with one).
     Each also with the rotation log shrunk, which sends the replaying matrices to the classic
     iteration inside the apply kernel."""
-    A = wl.letkf_shaped(150, M, p, config_index=990 + M + p)
+    A = wl.letkf_shaped(151, M, p, config_index=990 + M + p)       # (odd: the paired kernel ends on a CTA with one matrix)
     try:
         for k, v in VARIANTS[variant].items():
             lk.set_option(k, v)
