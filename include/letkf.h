@@ -13,8 +13,10 @@
  *     stream) and the call returns without synchronising.  Internally the library may fork
  *     onto private streams that are joined back into `stream` before the call returns, so
  *     stream order is all a caller needs.
- *   - workspace: `work` is a caller-owned device buffer of at least the size returned by
- *     the matching letkf_*_workspace_bytes(); if `work` is NULL the library takes it from
+ *   - workspace: `work` is a caller-owned device buffer; the matching letkf_*_workspace_bytes()
+ *     returns the RECOMMENDED size (all sub-chunks of the call in flight).  Any size that holds one
+ *     matrix's records is accepted -- the call then keeps fewer sub-chunks in flight or runs chunk
+ *     after chunk -- and a smaller one is refused (-k).  If `work` is NULL the library takes it from
  *     the device's default memory pool with cudaMallocAsync / cudaFreeAsync on `stream`
  *     (stream-ordered, no synchronisation).
  *   - return value: 0 = LETKF_OK; -k = the k-th argument (1-based) is invalid (NULL where
@@ -243,16 +245,27 @@ long long letkf_profile_direct(void);
  * gpu_launches claim is counted from this, not guessed). */
 int letkf_last_launch_count(void);
 
-/* Test/diagnostic options.  "force_generic" = 1 routes every M through the any-M kernels
- * (otherwise only M > 64 and overflowed matrices use them); "pipeline" = 0 runs every pass as one
- * chunk on the caller's stream instead of the sub-chunk pipeline over private streams (default 1);
- * "ql_tpb" = 32/64/96 matrices per QL CTA (0 = by size); "log_shrink" = k divides the rotation-log
- * capacity by k so that tests can force the log-overflow slow path (default 1); "split" = 1 runs the
- * tridiagonalisation of 48 < M <= 64 as three kernels (pivots down to 33 / trailing 32 x 32 problem /
- * explicit Q; experimental, default 0: measured slower than the single kernel); "sub_chunks" = 1..16
- * sub-chunks per pass of the calling thread's device calls (default 8; measured flat from 4 to 8);
- * "mid_reg" = 0 / 1 / 2: the reduction of 64 < M <= 160 with the matrix in shared memory / in
- * registers up to M = 128 and in shared memory above (default) / in registers at every such M.
+/* Test / experiment options (process-wide; every entry point takes ONE snapshot of them when it starts, so a
+ * change from another host thread never takes effect in the middle of a call).  value -1 / 0 restores the default
+ * where a default is "by size".
+ *   "force_generic" 1: every M through the any-M kernels (otherwise only M > 160)
+ *   "pipeline"      0: chunk after chunk on the caller's stream instead of the sub-chunk pipeline (default 1)
+ *   "sub_chunk"     matrices per sub-chunk of the pipeline (0 = batch / 16, at least 512)
+ *   "slots"         sub-chunks in flight = workspace slots (0 = all 16); "log_slots": of which as many may hold a
+ *                   slot of the rotation log (0 = a 288 MB budget on the M <= 64 path, every slot elsewhere)
+ *   "ql_tpb"        lanes per QL CTA: 32 / 64 / 96 / 128 / 192 (0 = 128 for M <= 64, 32 above)
+ *   "two_pass"      QL log from a second, perfectly shifted pass: 0 / 1 (-1 = when batch x M >= 2^18)
+ *   "log_shrink"    k divides the rotation-log capacity so that tests can force the in-kernel slow path
+ *   "qform"         M <= 64: 1 = explicit Q formed by the reduction kernel, rotations replayed on its rows (round 1's
+ *                   form); 0 (default) = reflectors kept, back-transform in the apply kernel
+ *   "evec"          M <= 64, qform 0: 1 (default) = eigenvectors of T by twisted factorisations where the classifier
+ *                   allows; 0 = always the logged rotations
+ *   "bisect"        M <= 64, evec 1: eigenvalues by multisection with M threads per matrix: 0 / 1 (-1 = batch <= 1024)
+ *   "pair"          32 < M <= 64: the reduction kernel takes two matrices per CTA: 0 / 1 (-1 = for 32 < M <= 48)
+ *   "split"         48 < M <= 64: the reduction as two kernels (experimental, default 0: measured no faster)
+ *   "mid_reg"       64 < M <= 160: reduction with the matrix in shared memory (0) / in registers up to M = 128 (1,
+ *                   default) / in registers (2)
+ *   "host_pass"     matrices per pass of the host entry points (0 = what a 16 GiB staging arena holds)
  * Returns 0, or -1 for an unknown name. */
 int letkf_set_option(const char* name, int value);
 
