@@ -358,16 +358,27 @@ static int stage_T(const double* A, int M, int n, double* V, Workspace ws, cudaS
     return 0;
 }
 
-template <int TPB>
-static int ql_run(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st, int mode)
+template <int TPB, int MODE>
+static int ql_launch(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st)
 {
     cudaError_t ce;
     const size_t ql_smem = sizeof(double) * 2 * (size_t)M * TPB + 24 * (size_t)TPB;   // (d, e) per lane + the sort's bookkeeping
-    if ((ce = allow_smem(ql_log_kernel<TPB>, ql_smem)) != cudaSuccess) return (int)ce;
-    const int per_cta = (mode == QL_TWO_PASS || mode == QL_LOGPASS_PAIRED) ? TPB / 2 : TPB;  // two lanes per matrix when the iteration runs twice side by side
+    if ((ce = allow_smem(ql_log_kernel<TPB, MODE>, ql_smem)) != cudaSuccess) return (int)ce;
+    const int per_cta = (MODE == QL_TWO_PASS || MODE == QL_LOGPASS_PAIRED) ? TPB / 2 : TPB;  // two lanes per matrix when the iteration runs twice side by side
     const int qblocks = (n + per_cta - 1) / per_cta;
-    KLAUNCH("ql_log_kernel", st, ql_log_kernel<TPB><<<qblocks, TPB, ql_smem, st>>>(ws, M, n, w, info, mode));
+    KLAUNCH("ql_log_kernel", st, (ql_log_kernel<TPB, MODE><<<qblocks, TPB, ql_smem, st>>>(ws, M, n, w, info)));
     return 0;
+}
+template <int TPB>
+static int ql_run(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st, int mode)
+{
+    switch (mode) {
+        case QL_TWO_PASS: return ql_launch<TPB, QL_TWO_PASS>(M, n, w, info, ws, st);
+        case QL_CLASSIFY: return ql_launch<TPB, QL_CLASSIFY>(M, n, w, info, ws, st);
+        case QL_LOGPASS: return ql_launch<TPB, QL_LOGPASS>(M, n, w, info, ws, st);
+        case QL_LOGPASS_PAIRED: return ql_launch<TPB, QL_LOGPASS_PAIRED>(M, n, w, info, ws, st);
+        default: return ql_launch<TPB, QL_ONE_PASS>(M, n, w, info, ws, st);
+    }
 }
 
 static int stage_QL(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st, int mode)

@@ -40,17 +40,19 @@ constexpr int QL_ONE_PASS = 0, QL_TWO_PASS = 1, QL_CLASSIFY = 2, QL_LOGPASS = 3,
 // (QL_LOGPASS_PAIRED: the pending matrices as in QL_LOGPASS, but by pairs of lanes as in QL_TWO_PASS --
 // behind bisect_kernel.cuh, whose eigenvalues are not in the order in which QL would deflate them)
 
-template <int QL_TPB>
+// The mode is a template parameter: in the eigenvalue-only pass the log stores, the shift look-up and the
+// pair bookkeeping are not compiled in at all (as run-time predicates they cost 30% of the rotation step).
+template <int QL_TPB, int mode>
 __global__ void __launch_bounds__(QL_TPB)
-ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __restrict__ info, int mode)
+ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __restrict__ info)
 {
     extern __shared__ double sm[];
     double* dsm = sm;                             // [M][QL_TPB]  one column per LANE
     double* esm = sm + (size_t)M * QL_TPB;        // [M][QL_TPB]
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x;              // column of the [M][QL_TPB] arrays
-    const bool two_pass = mode == QL_TWO_PASS || mode == QL_LOGPASS_PAIRED;  // (pairs of lanes)
-    const bool pending_only = mode == QL_LOGPASS || mode == QL_LOGPASS_PAIRED;
+    constexpr bool two_pass = mode == QL_TWO_PASS || mode == QL_LOGPASS_PAIRED;  // (pairs of lanes)
+    constexpr bool pending_only = mode == QL_LOGPASS || mode == QL_LOGPASS_PAIRED;
     const int nmc = two_pass ? QL_TPB / 2 : QL_TPB;         // matrices per CTA
     const int b0 = blockIdx.x * nmc;
     const int nb = min(nmc, batch - b0);
@@ -82,7 +84,7 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
     }
     const bool logging = mode == QL_ONE_PASS || mode == QL_LOGPASS || (two_pass && (lane & 1));   // rotations recorded
     bool easy = false;                                       // QL_CLASSIFY: FLAG_GETVEC
-    const bool shifted = two_pass || mode == QL_LOGPASS;     // first sweep of a position shifted by a known eigenvalue
+    constexpr bool shifted = two_pass || mode == QL_LOGPASS;     // first sweep of a position shifted by a known eigenvalue
     double* d = dsm + lane;
     double* e = esm + lane;
     constexpr int stride = QL_TPB;
