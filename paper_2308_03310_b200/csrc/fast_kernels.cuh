@@ -124,6 +124,9 @@ __device__ __forceinline__ R block_pick(const R (&a)[MT], int k)
     return x;
 }
 
+#ifndef LETKF_AP48
+#define LETKF_AP48 6      // CTAs per SM of fast_apply<48>: 7 (144 registers) spills 416 B and measured 2.06 ms at config 5, 6 (168) 1.70 ms
+#endif
 #ifndef LETKF_TRI_REGS64
 #define LETKF_TRI_REGS64 168
 #endif
@@ -1141,7 +1144,7 @@ __device__ __forceinline__ bool direct_eigenvectors(double (&z)[MT], uint32_t* s
 }
 
 template <int MT, bool EPI, bool QFORM>
-__global__ void __launch_bounds__(FastCfg<MT>::NT, (MT == 64) ? 6 : (MT == 48 ? 7 : 16))
+__global__ void __launch_bounds__(FastCfg<MT>::NT, (MT == 64) ? 6 : (MT == 48 ? LETKF_AP48 : 16))
 fast_apply(double* __restrict__ V_, double* __restrict__ w_, int* __restrict__ info_, Workspace ws, int M, EpiArgs ep)
 {
     using C = FastCfg<MT>;
@@ -1435,7 +1438,7 @@ fast_apply(double* __restrict__ V_, double* __restrict__ w_, int* __restrict__ i
 // factorisations in fp64: the orthogonality of Z to 2e-13 costs nothing next to the 2 M^3 fp32
 // flops behind it).  Same three routes as fast_apply; w is written as float on the way.
 template <int MT>
-__global__ void __launch_bounds__(FastCfg<MT>::NT, (MT == 64) ? 6 : (MT == 48 ? 7 : 16))
+__global__ void __launch_bounds__(FastCfg<MT>::NT, (MT == 64) ? 6 : (MT == 48 ? LETKF_AP48 : 16))
 fast_apply_f32(float* __restrict__ V_, double* __restrict__ w_, float* __restrict__ wf_, int* __restrict__ info_,
                Workspace ws, int M)
 {
