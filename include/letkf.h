@@ -252,7 +252,7 @@ int letkf_last_launch_count(void);
  *   "pipeline"      0: chunk after chunk on the caller's stream instead of the sub-chunk pipeline (default 1)
  *   "sub_chunk"     matrices per sub-chunk of the pipeline (0 = batch / 16, at least 512)
  *   "slots"         sub-chunks in flight = workspace slots (0 = all 16); "log_slots": of which as many may hold a
- *                   slot of the rotation log (0 = a 288 MB budget on the M <= 64 path, every slot elsewhere)
+ *                   slot of the rotation log (0 = a 256 MB budget on the M <= 64 path, every slot elsewhere)
  *   "ql_tpb"        lanes per QL CTA: 32 / 64 / 96 / 128 / 192 (0 = 128 for M <= 64, 32 above)
  *   "two_pass"      QL log from a second, perfectly shifted pass: 0 / 1 (-1 = when batch x M >= 2^18)
  *   "log_shrink"    k divides the rotation-log capacity so that tests can force the in-kernel slow path

@@ -170,7 +170,7 @@ static const int BISECT_MAX_BATCH = 1024;
 static const int PIPE_MIN_SUB = 512;     // smallest sub-chunk worth launches of its own
 static const int PIPE_MAX_SUBS = 16;     // sub-chunks per call (bounds the launch count)
 static const int PIPE_SLOTS = 16;        // default number of sub-chunks in flight: all of them
-static const size_t PIPE_LOG_BYTES = (size_t)288 << 20;   // default size of the log slots together
+static const size_t PIPE_LOG_BYTES = (size_t)256 << 20;   // default size of the log slots together
 static const int NQ_STREAMS = 16;
 
 static int round_up(int x, int a) { return (x + a - 1) / a * a; }
