@@ -262,7 +262,8 @@ int letkf_last_launch_count(void);
  *                   allows; 0 = always the logged rotations
  *   "bisect"        M <= 64, evec 1: eigenvalues by multisection with M threads per matrix: 0 / 1 (-1 = batch <= 1024)
  *   "pair"          32 < M <= 64: the reduction kernel takes two matrices per CTA: 0 / 1 (-1 = for 32 < M <= 48)
- *   "split"         48 < M <= 64: the reduction as two kernels (experimental, default 0: measured no faster)
+ *   "split"         48 < M <= 64: the reduction as two kernels, pivots M-1 ... 33 by two warps and the trailing
+ *                   32 x 32 problem by one warp per matrix (default 1; 0 = one kernel)
  *   "mid_reg"       64 < M <= 160: reduction with the matrix in shared memory (0) / in registers up to M = 128 (1,
  *                   default) / in registers (2)
  *   "host_pass"     matrices per pass of the host entry points (0 = what a 16 GiB staging arena holds)

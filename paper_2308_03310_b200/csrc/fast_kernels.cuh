@@ -130,6 +130,9 @@ __device__ __forceinline__ R block_pick(const R (&a)[MT], int k)
 #ifndef LETKF_TRI_REGS64
 #define LETKF_TRI_REGS64 168
 #endif
+#ifndef LETKF_TRI_REGS64_HEAD
+#define LETKF_TRI_REGS64_HEAD 200     // the head kernel of the split reduction: 5 CTAs per SM without spills (1.07 ms)
+#endif                                // beats 6 with 364 B of spills inside the pivot loop (1.22 ms)
 template <int MT> struct FastCfg {
     static constexpr int NT = (MT + 31) / 32 * 32;      // threads per matrix = threads per CTA
     static constexpr int NW = NT / 32;
@@ -415,9 +418,10 @@ template <int MT> __host__ __device__ constexpr int refl_doubles() { return RefL
 // the raw pivot column of pivot 32 and its norm to fast_tridiag_tail, one warp per matrix -- so that
 // no warp sits at a barrier holding 64 rows' worth of registers while another reduces the last 32
 // pivots (ncu, unsplit: barrier stall 1.4 cycles per issue, profiles/r02_ncu_key_metrics.txt).
-// letkf_set_option("split", 1); OFF by default: measured 1.22 + 0.25 ms against 1.46 ms for the one
-// kernel (config 3) -- the head kernel spills 364 bytes inside the pivot loop where the whole kernel
-// spills 152, whatever shape the hand-over code is given (ptxas), and that eats the gain.
+// The default for 48 < M <= 64 (letkf_set_option("split", 0) restores the one kernel): measured
+// 1.07 + 0.25 ms against 1.46 ms for the one kernel (config 3).  The head kernel gets 200 registers
+// (LETKF_TRI_REGS64_HEAD, 5 CTAs per SM): at the one kernel's 168 it spills 364 bytes inside the pivot
+// loop, whatever shape the hand-over code is given (ptxas), and measures 1.22 ms.
 constexpr int SPLIT_LOW = 528, SPLIT_XS = 528, SPLIT_RED = 560;      // offsets inside the first 640 entries
 
 // PAIR (two-warp buckets, reflector form): a CTA reduces TWO matrices.  Pivots M-1 ... 33 need both
@@ -433,7 +437,7 @@ template <int MT, typename R = double, bool PAIR = false> constexpr size_t fast_
 }
 
 template <int MT, bool GRAM, bool QFORM, typename R = double, bool SPLIT = false, bool PAIR = false>
-__global__ void __launch_bounds__(FastCfg<MT>::NT) __maxnreg__((MT == 64) ? LETKF_TRI_REGS64 : (MT == 48 ? 168 : (MT == 32 ? 128 : 80)))
+__global__ void __launch_bounds__(FastCfg<MT>::NT) __maxnreg__((MT == 64) ? ((SPLIT && sizeof(R) == 8) ? LETKF_TRI_REGS64_HEAD : LETKF_TRI_REGS64) : (MT == 48 ? 168 : (MT == 32 ? 128 : 80)))
 fast_tridiag(const R* __restrict__ A_, R* __restrict__ Q_, Workspace ws, int M,
                    const double* __restrict__ Yb_, const double* __restrict__ d_,
                    const double* __restrict__ r_, int p, double shift, double* __restrict__ gout_,

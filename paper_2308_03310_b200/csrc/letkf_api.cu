@@ -97,8 +97,8 @@ struct Options {
                              // side on its two warps (0: one matrix per CTA, the second warp idle through the last 32
                              // pivots).  -1 = where it measured faster: 32 < M <= 48 without the Gram step (config 5,
                              // M = 48: 1.74 -> 1.51 ms; at M = 64 the paired kernel spills and loses, 1.46 -> 1.65 ms)
-    int split = 0;           // 48 < M <= 64, qform = 0: the reduction as two kernels (pivots down to 33 by two warps,
-                             // the trailing 32 x 32 problem by one warp per matrix); measured no faster, off
+    int split = 1;           // 48 < M <= 64, qform = 0: the reduction as two kernels (pivots down to 33 by two warps,
+                             // the trailing 32 x 32 problem by one warp per matrix): 1.07 + 0.25 ms against 1.46 ms (config 3)
     int evec = 1;            // M <= 64, qform = 0: 1 = eigenvectors of T by twisted factorisations where the spectrum
                              // allows (ql_log_kernel classifies), the logged rotations otherwise; 0 = always the log
 };
