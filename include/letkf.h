@@ -76,6 +76,33 @@ int letkf_syev_batched(const double* A, int M, int batch, double* w, double* V,
 size_t letkf_syev_workspace_bytes(int M, int batch);
 
 /*
+ * letkf_syev_batched for callers that may not allocate (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): same arguments and results, but there is no
+ * workspace argument and the call makes NO cudaMalloc / cudaFree / cudaMallocAsync, creates no
+ * stream and no event.  The scratch memory of the kernels (reflectors, (d, e), rotation log, flags:
+ * DESIGN.md section 4) is a file-scope `static __device__` array of LETKF_STATIC_WORK_BYTES inside the
+ * library, which every GPU that loads the library holds until the process exits.  All kernels
+ * (reduction, eigenvalues, apply) are launched one after the other on `stream`; the kernels and the
+ * results are those of letkf_syev_batched at the same batch size.
+ *
+ *   batch   must fit the array: batch <= letkf_syev_static_max_batch(M) (paper's latency case, 256
+ *           matrices of M = 64, fits; M = 64: 363, M = 32: 1297, M = 16: 4123, M = 128: 62), else
+ *           the call returns LETKF_ERR_STATIC_CAPACITY and launches nothing.
+ *   Every call on a device shares the one array: two calls whose kernels overlap on the GPU (different
+ *   streams, or different host threads) RACE on it -- keep all calls of a device on one stream or order
+ *   them with events.  The array keeps the last call's contents; the call clears the per-matrix flag
+ *   and sweep-count records it starts from (every other record is written before it is read).
+ *   Profiling records (letkf_profile_enable) are not taken by this entry point.
+ */
+#define LETKF_STATIC_WORK_BYTES (32u << 20)
+#define LETKF_ERR_STATIC_CAPACITY (-100)
+int letkf_syev_batched_static(const double* A, int M, int batch, double* w, double* V,
+                              int* info, void* stream);
+
+/* largest batch letkf_syev_batched_static accepts for order M (0 for an invalid M) */
+int letkf_syev_static_max_batch(int M);
+
+/*
  * The same decomposition in the paper's precision ("single-precision"; Table I,
  * M = 16, 32, 48, 64, batch 128^2): A, w, V are fp32.  SURVEY.md section 8(f) N2.
  * The Householder reduction, the replay of plane rotations and the back-transform run in fp32; the

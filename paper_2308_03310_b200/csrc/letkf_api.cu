@@ -730,6 +730,82 @@ int letkf_syev_batched(const double* A, int M, int batch, double* w, double* V, 
     return syev_core(A, M, batch, w, V, info, sw.ptr, pl, st);
 }
 
+// ---- the entry point that allocates nothing (letkf.h: letkf_syev_batched_static) ---------------------
+// The kernels' scratch memory is this file-scope array: one per GPU that loads the library, held
+// until exit.  In host code `g_static_work` is only a stand-in for the symbol, not a device address:
+// the address is looked up once per device (with that device current) and cached here.
+static __device__ __align__(256) unsigned char g_static_work[LETKF_STATIC_WORK_BYTES];
+static const int STATIC_MAX_DEVICES = 64;
+static void* g_static_ptr[STATIC_MAX_DEVICES] = {};
+static std::mutex g_static_mu;
+
+static int static_work_ptr(void** out)
+{
+    int dev = 0;
+    cudaError_t ce = cudaGetDevice(&dev);
+    if (ce != cudaSuccess) return (int)ce;
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return (int)cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void* p = nullptr;
+        if ((ce = cudaGetSymbolAddress(&p, g_static_work)) != cudaSuccess) return (int)ce;
+        if (!p || misaligned(p)) return (int)cudaErrorInvalidSymbol;
+        g_static_ptr[dev] = p;
+    }
+    *out = g_static_ptr[dev];
+    return 0;
+}
+
+// one chunk of `batch` matrices on the caller's stream: the plan letkf_syev_batched takes when it does not pipeline
+static Plan static_plan(int M, int batch)
+{
+    Plan pl = make_plan(M, batch, 0, 0);
+    pl.per = batch; pl.nslot = 1; pl.nlog = 1; pl.nsub = 1; pl.pipelined = false;
+    return pl;
+}
+
+int letkf_syev_static_max_batch(int M)
+{
+    EntryScope scope;
+    if (M < 1 || M > LETKF_MAX_M) return 0;
+    int lo = 0, hi = 1 << 20;                  // largest batch whose workspace fits (the size grows with the batch wherever it fits)
+    while (lo < hi) {
+        const int mid = lo + (hi - lo + 1) / 2;
+        if (syev_need(M, static_plan(M, mid)) <= (size_t)LETKF_STATIC_WORK_BYTES) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+
+int letkf_syev_batched_static(const double* A, int M, int batch, double* w, double* V, int* info, void* stream)
+{
+    EntryScope scope;
+    g_launches = 0;
+    if (M < 1 || M > LETKF_MAX_M) return -2;
+    if (batch < 0) return -3;
+    if (batch == 0) return LETKF_OK;
+    if (!A || misaligned(A)) return -1;
+    if (!w || misaligned(w)) return -4;
+    if (!V || misaligned(V)) return -5;
+    const Plan pl = static_plan(M, batch);
+    if (syev_need(M, pl) > (size_t)LETKF_STATIC_WORK_BYTES) return LETKF_ERR_STATIC_CAPACITY;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    void* base = nullptr;
+    int rc = static_work_ptr(&base);
+    if (rc) return rc;
+    struct ProfOff {                           // the profiling aid creates events and a counter: not here
+        bool was = g_prof.on;
+        ProfOff() { g_prof.on = false; }
+        ~ProfOff() { g_prof.on = was; }
+    } prof_off;
+    Workspace ws;
+    carve(ws, base, M, batch, batch, pl.two_pass);
+    // the array keeps the last call's contents: the records a matrix starts from are cleared
+    cudaError_t ce;
+    if ((ce = cudaMemsetAsync(ws.flags, 0, sizeof(int) * (size_t)batch, st)) != cudaSuccess) return (int)ce;
+    if ((ce = cudaMemsetAsync(ws.nsweeps, 0, sizeof(int) * (size_t)batch, st)) != cudaSuccess) return (int)ce;
+    return syev_core(A, M, batch, w, V, info, base, pl, st);
+}
+
 size_t letkf_syev_f32_workspace_bytes(int M, int batch)
 {
     EntryScope scope;
@@ -1446,6 +1522,8 @@ const char* letkf_status_string(int status)
 {
     static thread_local char buf[96];
     if (status == 0) return "ok";
+    if (status == LETKF_ERR_STATIC_CAPACITY)
+        return "batch too large for the static scratch array of letkf_syev_batched_static (letkf_syev_static_max_batch)";
     if (status < 0) {
         snprintf(buf, sizeof(buf), "invalid argument %d (1-based position in the call)", -status);
         return buf;

@@ -19,9 +19,12 @@ LIB_PATH = os.path.join(_PKG, "libletkf.so")
 MAX_M = 256
 INFO_SLOWPATH = 0x40000000
 INFO_NS_NOCONV = 0x20000000
+STATIC_WORK_BYTES = 32 << 20
+ERR_STATIC_CAPACITY = -100
 
 EXPORTS = (
     "letkf_syev_batched", "letkf_syev_workspace_bytes",
+    "letkf_syev_batched_static", "letkf_syev_static_max_batch",
     "letkf_syev_batched_f32", "letkf_syev_f32_workspace_bytes",
     "letkf_analysis_batched", "letkf_analysis_workspace_bytes", "letkf_analysis_batched_evdfree",
     "letkf_syev_batched_host", "letkf_analysis_batched_host", "letkf_host_release",
@@ -53,6 +56,10 @@ def load():
     lib.letkf_syev_batched.restype = ci
     lib.letkf_syev_workspace_bytes.argtypes = [ci, ci]
     lib.letkf_syev_workspace_bytes.restype = sz
+    lib.letkf_syev_batched_static.argtypes = [vp, ci, ci, vp, vp, vp, vp]
+    lib.letkf_syev_batched_static.restype = ci
+    lib.letkf_syev_static_max_batch.argtypes = [ci]
+    lib.letkf_syev_static_max_batch.restype = ci
     lib.letkf_syev_batched_f32.argtypes = [vp, ci, ci, vp, vp, vp, vp, sz, vp]
     lib.letkf_syev_batched_f32.restype = ci
     lib.letkf_syev_f32_workspace_bytes.argtypes = [ci, ci]
@@ -182,6 +189,30 @@ def syev_batched(A, w=None, V=None, info=None, work=None, stream=None):
         st = lib.letkf_syev_batched(_ptr(A), M, batch, _ptr(w), _ptr(V), _ptr(info),
                                     _ptr(work), wb, _stream(stream))
     _check(st, "letkf_syev_batched")
+    return w, V, info
+
+
+def syev_static_max_batch(M):
+    return load().letkf_syev_static_max_batch(M)
+
+
+def syev_batched_static(A, w, V, info=None, stream=None):
+    """letkf_syev_batched_static: the EVD with the kernels' scratch memory in the library's static
+    device array -- no allocation on the way, so the outputs ``w`` and ``V`` (``V`` may be ``A``) are
+    the caller's, ``info`` too where wanted.  batch <= syev_static_max_batch(M), else LetkfError
+    (status ERR_STATIC_CAPACITY).  Calls of one device share the array: keep them on one stream."""
+    lib = load()
+    _dev_f64(A, "A")
+    batch, M, M2 = A.shape
+    if M != M2:
+        raise LetkfError("A must be [batch][M][M]")
+    _out(w, "w", (batch, M), A.device)
+    _out(V, "V", (batch, M, M), A.device)
+    if info is not None:
+        _out(info, "info", (batch,), A.device, torch.int32)
+    with torch.cuda.device(A.device):
+        st = lib.letkf_syev_batched_static(_ptr(A), M, batch, _ptr(w), _ptr(V), _ptr(info), _stream(stream))
+    _check(st, "letkf_syev_batched_static")
     return w, V, info
 
 
