@@ -338,16 +338,21 @@ def run_ours(args):
     value = world * B / (ms_step * 1e-3)
 
     # ---- roofline of the dominant kernel.  Flops per matrix, as the kernels do them:
-    #   fast_tridiag   4/3 M^3                       Householder reduction (the reflectors are kept, no explicit Q)
+    #   fast_tridiag   4/3 M^3                       Householder reduction (the reflectors are kept, no explicit Q);
+    #                  48 < M <= 64: fast_tridiag_head 4/3 (M^3 - 32^3) + fast_tridiag_tail 4/3 32^3
     #   ql_log_kernel  30 flops per rotation step    (scalar recurrences; latency bound, not a roofline kernel)
     #   fast_apply     2 M^3 back-transform + 6 M R  (R logged rotations replayed) + 60 M^2 for a matrix whose
     #                  eigenvectors come from twisted factorisations (5 passes of ~12 flops per entry)
     sm_max = clocks.get("sm_max_mhz") or 1965.0
     peak_derived = SM_COUNT * DFMA_PER_CLK_SM * 2 * sm_max * 1e6 / 1e12
     flops_per_matrix = {}
+    split = any("tridiag_tail" in k for k in kern_ms)           # the reduction as two kernels: pivots M-1 ... 33, then 32 ... 1
+    tail_flops = (4.0 / 3.0) * 32 ** 3
     for k in kern_ms:
-        if "tridiag" in k:
-            flops_per_matrix[k] = (4.0 / 3.0) * M ** 3
+        if "tridiag_tail" in k:
+            flops_per_matrix[k] = tail_flops
+        elif "tridiag" in k:
+            flops_per_matrix[k] = (4.0 / 3.0) * M ** 3 - (tail_flops if split else 0.0)
         elif "apply" in k:
             flops_per_matrix[k] = 2.0 * M ** 3 + 6.0 * M * rot_per_matrix + 60.0 * M * M * direct_frac
         elif "ql" in k:
@@ -378,6 +383,9 @@ def run_ours(args):
     peak_measured = best
 
     algorithmic_bytes = {"fast_tridiag": (8.0 * M * M + 8.0 * (M * M / 2 + 3 * M)) * B,        # A in; reflectors, d, e out
+                         # head: A in; reflectors of pivots >= 33, their (d, e), the 640-entry hand-over record out
+                         "fast_tridiag_head": (8.0 * M * M + 8.0 * (M * M / 2 - 528 + 3 * (M - 32) + 640)) * B,
+                         "fast_tridiag_tail": (8.0 * 640 + 8.0 * (528 + 3 * 32)) * B,          # hand-over in; the rest out
                          "ql_log_kernel": (16.0 * M + 12.0 * M + 16.0 * rot_per_matrix) * B,
                          "fast_apply": (8.0 * (M * M / 2 + 4 * M) + 16.0 * rot_per_matrix + 8.0 * M * M) * B}
     step_tflops = syev_model_flops(M) * B / (ms_step * 1e-3) / 1e12

@@ -275,52 +275,64 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
     // by insertion was 28% of this kernel), and in QL_CLASSIFY the sorted sequence is classified on
     // the way (common.cuh, GV_*): easy unless two eigenvalues that are not both 1 x 1 blocks are
     // closer than GV_TINY ||T||, or more than GV_PH lie within GV_GAP ||T|| above one.
+    // The lanes work in groups of GS = 16 / 32 / 64 >= M (M <= 64), one matrix per group and round:
+    // QL_TPB / GS matrices per round (at M = 16 one matrix per round left 112 of 128 lanes idle through
+    // 128 rounds of three barriers each -- more than the iteration itself took).
     const bool owner = valid && (!two_pass || (lane & 1));   // the lane that reports the matrix
     unsigned long long* bm_sh = reinterpret_cast<unsigned long long*>(sm + 2 * (size_t)M * QL_TPB);   // [QL_TPB]
     double* thr_sh = reinterpret_cast<double*>(bm_sh + QL_TPB);                                        // [QL_TPB]
-    int* sort_sh = reinterpret_cast<int*>(thr_sh + QL_TPB);                                            // [QL_TPB]
+    int* sort_sh = reinterpret_cast<int*>(thr_sh + QL_TPB);                                            // [QL_TPB] 1: to sort, 2: and hard
     sort_sh[lane] = (owner && !overflow) ? 1 : 0;
     bm_sh[lane] = bmask;
     thr_sh[lane] = thr;
     __syncthreads();
-    for (int c = 0; c < nb; ++c) {
+    const int gs0 = M <= 16 ? 16 : (M <= 32 ? 32 : 64);
+    const int GS = (M <= 64 && QL_TPB % gs0 == 0) ? gs0 : QL_TPB;      // lanes per matrix
+    const int ng = QL_TPB / GS, grp = lane / GS, kl = lane - grp * GS;
+    for (int c0 = 0; c0 < nb; c0 += ng) {
+        const int c = c0 + grp;
         const int col = two_pass ? 2 * c + 1 : c;
-        if (!sort_sh[col]) continue;                          // (uniform)
+        const bool act = c < nb && sort_sh[col] != 0;
         const size_t bc = (size_t)(b0 + c);
-        const double* dc = dsm + col;
-        double* ec = esm + col;
+        const double* dc = dsm + (act ? col : 0);
+        double* ec = esm + (act ? col : 0);
         int myrank = -1;
-        for (int k = lane; k < M; k += QL_TPB) {
-            const double v = dc[k * stride];
-            int rank = 0;
-            for (int j = 0; j < M; ++j) {
-                const double u = dc[j * stride];
-                rank += (u < v || (u == v && j < k)) ? 1 : 0;
+        if (act) {
+            for (int k = kl; k < M; k += GS) {
+                const double v = dc[k * stride];
+                int rank = 0;
+                for (int j = 0; j < M; ++j) {
+                    const double u = dc[j * stride];
+                    rank += (u < v || (u == v && j < k)) ? 1 : 0;
+                }
+                w[bc * M + rank] = v;
+                ws.perm[bc * M + rank] = k;
+                if (mode == QL_CLASSIFY) { ws.s1[bc * M + k] = v; ec[rank * stride] = v; myrank = rank; }
             }
-            w[bc * M + rank] = v;
-            ws.perm[bc * M + rank] = k;
-            if (mode == QL_CLASSIFY) { ws.s1[bc * M + k] = v; ec[rank * stride] = v; myrank = rank; }
         }
-        if (mode == QL_CLASSIFY) {                            // (M <= 64 <= QL_TPB: one eigenvalue per lane)
+        if (mode == QL_CLASSIFY) {                            // (M <= 64 <= QL_TPB, GS >= M: one eigenvalue per lane)
             __syncthreads();
-            const unsigned long long bmc = bm_sh[col];
-            if (lane < M) {
-                const bool lo_cut = lane == 0 || ((bmc >> (lane - 1)) & 1ull);
-                const bool hi_cut = lane == M - 1 || ((bmc >> lane) & 1ull);
+            if (act && kl < M) {
+                const unsigned long long bmc = bm_sh[col];
+                const bool lo_cut = kl == 0 || ((bmc >> (kl - 1)) & 1ull);
+                const bool hi_cut = kl == M - 1 || ((bmc >> kl) & 1ull);
                 dsm[myrank * stride + col] = (lo_cut && hi_cut) ? 1.0 : 0.0;   // 1 x 1 block: its eigenvector is a unit vector
             }
             __syncthreads();
-            bool hard = false;
-            if (lane + 1 < M) {
+            if (act && kl + 1 < M) {
+                bool hard = false;
                 const double nrm = thr_sh[col] * 9007199254740992.0;               // max_i(|d_i| + |e_i|)
-                const double dk = ec[lane * stride];
-                const bool both_single = dc[lane * stride] != 0.0 && dc[(lane + 1) * stride] != 0.0;
-                if (ec[(lane + 1) * stride] - dk < GV_TINY * nrm && !both_single) hard = true;
-                if (lane + GV_PH + 1 < M && ec[(lane + GV_PH + 1) * stride] - dk < GV_GAP * nrm) hard = true;
+                const double dk = ec[kl * stride];
+                const bool both_single = dc[kl * stride] != 0.0 && dc[(kl + 1) * stride] != 0.0;
+                if (ec[(kl + 1) * stride] - dk < GV_TINY * nrm && !both_single) hard = true;
+                if (kl + GV_PH + 1 < M && ec[(kl + GV_PH + 1) * stride] - dk < GV_GAP * nrm) hard = true;
+                if (hard) sort_sh[col] = 2;                   // (every writer writes the same value)
             }
-            const int anyhard = __syncthreads_or(hard ? 1 : 0);
-            if (lane == col) easy = !anyhard;
         }
+    }
+    if (mode == QL_CLASSIFY) {
+        __syncthreads();
+        easy = sort_sh[lane] == 1;
     }
     if (owner) {
         ws.nsweeps[b] = nsw;
