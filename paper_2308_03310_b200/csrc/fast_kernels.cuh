@@ -260,6 +260,9 @@ __device__ __forceinline__ void pivot_group(R (&a)[MT], const TriShared<R>& sh, 
     constexpr int NPR = (8 * G + 8 + 31) / 32;
     constexpr int NP = NPR < C::NW ? NPR : C::NW;
     constexpr unsigned FULL = 0xffffffffu;
+    // levels of the shuffle trees: 16 rows sit in half a warp (lanes beyond hold zeros), and with four
+    // levels two matrices can share a warp (pack_kernels.cuh)
+    constexpr int NSH = (MT <= 16) ? 4 : 5, SH0 = (MT <= 16) ? 8 : 16;
     const int lane = j & 31, warp = j >> 5;
     if (warp >= NP) return;
     const int ihi = (8 * G + 8 < M - 1) ? 8 * G + 8 : M - 1;
@@ -291,8 +294,8 @@ __device__ __forceinline__ void pivot_group(R (&a)[MT], const TriShared<R>& sh, 
         if constexpr (NP > 1) t += sh.pv[lane + 32];
         const R nvj = -vj;
 #pragma unroll
-        for (int step = 0; step < (G + 1 > 5 ? G + 1 : 5); ++step) {
-            if (step < 5) t += __shfl_xor_sync(FULL, t, 16 >> step);
+        for (int step = 0; step < (G + 1 > NSH ? G + 1 : NSH); ++step) {
+            if (step < NSH) t += __shfl_xor_sync(FULL, t, SH0 >> step);
             if (step <= G) axpy_block<MT>(a, sh.pbuf, nvj, G - step);
         }
         const R nwj = fma(tau * t, vj, -pj);                   // -(p_j - tau (p.v) v_j)
@@ -303,8 +306,8 @@ __device__ __forceinline__ void pivot_group(R (&a)[MT], const TriShared<R>& sh, 
         if (j == i - 2) sh.red[4] = xn;
         R part = (j < i - 2) ? xn * xn : R(0);
 #pragma unroll
-        for (int step = 0; step < (G > 5 ? G : 5); ++step) {
-            if (step < 5) part += __shfl_xor_sync(FULL, part, 16 >> step);
+        for (int step = 0; step < (G > NSH ? G : NSH); ++step) {
+            if (step < NSH) part += __shfl_xor_sync(FULL, part, SH0 >> step);
             if (step < G) axpy_block<MT>(a, sh.vbuf, nwj, G - 1 - step);
         }
         if (lane == 0) sh.red[warp] = part;

@@ -16,6 +16,7 @@
 #include "bisect_kernel.cuh"
 #include "ns_kernel.cuh"
 #include "mid_kernels.cuh"
+#include "pack_kernels.cuh"
 
 namespace letkf {
 
@@ -99,6 +100,8 @@ struct Options {
                              // M = 48: 1.74 -> 1.51 ms; at M = 64 the paired kernel spills and loses, 1.46 -> 1.65 ms)
     int split = 1;           // 48 < M <= 64, qform = 0: the reduction as two kernels (pivots down to 33 by two warps,
                              // the trailing 32 x 32 problem by one warp per matrix): 1.07 + 0.25 ms against 1.46 ms (config 3)
+    int pack = 1;            // M <= 16, qform = 0, EVD calls: two matrices per warp (pack_kernels.cuh): 1 = reduction and
+                             // apply kernel, 2 = reduction only, 3 = apply kernel only, 0 = one matrix per warp
     int evec = 1;            // M <= 64, qform = 0: 1 = eigenvectors of T by twisted factorisations where the spectrum
                              // allows (ql_log_kernel classifies), the logged rotations otherwise; 0 = always the log
 };
@@ -318,6 +321,11 @@ static int fast_apply_run(double* V, double* w, int* info, Workspace ws, int M, 
 static int stage_T(const double* A, int M, int n, double* V, Workspace ws, cudaStream_t st,
                    const GramArgs* gram)
 {
+    if (use_fast(M) && M <= 16 && !gram && !t_opt.qform && (t_opt.pack == 1 || t_opt.pack == 2)) {
+        KLAUNCH("pack16_tridiag", st,
+                (pack16_tridiag<<<(n + 2 * PK_WARPS - 1) / (2 * PK_WARPS), 32 * PK_WARPS, pack16_tridiag_smem(), st>>>(A, ws, M, n)));
+        return 0;
+    }
     if (use_fast(M)) {
         if (t_opt.qform) {
             switch (fast_bucket(M)) {
@@ -418,6 +426,11 @@ static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws,
                     const EpiArgs* ep = nullptr)
 {
     const size_t ap_smem = sizeof(double) * (5 * (size_t)M + 2 * 32 * 33);
+    if (use_fast(M) && M <= 16 && !ep && !t_opt.qform && (t_opt.pack == 1 || t_opt.pack == 3)) {
+        KLAUNCH("pack16_apply", st,
+                (pack16_apply<<<(n + 2 * PK_WARPS - 1) / (2 * PK_WARPS), 32 * PK_WARPS, pack16_apply_smem(), st>>>(V, w, info, ws, M, n)));
+        return 0;
+    }
     if (use_fast(M)) {      // (matrices whose rotation log is unusable are finished inside the kernel)
         if (t_opt.qform) {
             switch (fast_bucket(M)) {
@@ -1464,6 +1477,7 @@ int letkf_set_option(const char* name, int value)
     if (strcmp(name, "qform") == 0) { o.qform = value != 0; return LETKF_OK; }
     if (strcmp(name, "evec") == 0) { o.evec = value != 0; return LETKF_OK; }
     if (strcmp(name, "split") == 0) { o.split = value != 0; return LETKF_OK; }
+    if (strcmp(name, "pack") == 0) { if (value < 0 || value > 3) return -2; o.pack = value; return LETKF_OK; }
     if (strcmp(name, "pair") == 0) { o.pair = (value == 0 || value == 1) ? value : -1; return LETKF_OK; }
     if (strcmp(name, "bisect") == 0) { o.bisect = (value == 0 || value == 1) ? value : -1; return LETKF_OK; }
     return -1;

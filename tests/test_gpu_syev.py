@@ -292,7 +292,7 @@ def test_log_overflow_slow_path(lk, oracle, M, batch):
     assert (info2 == 0).all() and np.abs(w2 - w).max() <= parity.TOL_W * np.abs(w).max()
 
 
-@pytest.mark.parametrize("M", [21, 48, 64, 100, 160, 200])
+@pytest.mark.parametrize("M", [9, 16, 21, 48, 64, 100, 160, 200])
 def test_hard_spectra(lk, oracle, M):
     """Matrices that stress the tridiagonal eigensolver and the deflation logic: Wilkinson W+ (pairs of
     eigenvalues agreeing to ~1e-14), two of them glued by a tiny coupling, graded matrices over
@@ -348,7 +348,8 @@ def test_mid_tridiagonalisation_both_forms(lk, oracle, M, mode):
 
 
 VARIANTS = {"direct": {}, "replay": {"evec": 0}, "qform": {"qform": 1}, "split": {"split": 1}, "pair": {"pair": 1},
-            "nopair": {"pair": 0}}
+            "nopair": {"pair": 0}, "nosplit": {"split": 0}, "nopack": {"pack": 0}, "nopack_replay": {"pack": 0, "evec": 0},
+            "pack_tridiag": {"pack": 2}, "pack_apply": {"pack": 3}}
 
 
 @pytest.mark.parametrize("variant", sorted(VARIANTS))
@@ -372,15 +373,56 @@ def test_register_path_variants(lk, oracle, M, p, variant):
         lk.set_option("log_shrink", 4)
         w2, V2, info2 = run_gpu(lk, A)
     finally:
-        for k, v in (("qform", 0), ("evec", 1), ("log_shrink", 1), ("split", 0), ("pair", -1)):
+        for k, v in (("qform", 0), ("evec", 1), ("log_shrink", 1), ("split", 1), ("pair", -1), ("pack", 1)):
             lk.set_option(k, v)
     assert (info == 0).all()
     wo, _, _, _ = oracle.syev_batched(A)
     parity.assert_evd(A, w, V, wo, f"{variant} M={M}")
     parity.assert_evd(A, w2, V2, wo, f"{variant}, log shrunk, M={M}")
     assert ((info2 & 0xFFFF) == 0).all()
-    if p >= M - 1 and M >= 16 and variant in ("replay", "qform"):
+    if p >= M - 1 and M >= 16 and variant in ("replay", "qform", "nopack_replay"):
         assert (info2 & lk.INFO_SLOWPATH).astype(bool).all()
+
+
+@pytest.mark.parametrize("mode", ["direct", "replay", "slow"])
+@pytest.mark.parametrize("M", [2, 3, 7, 8, 9, 10, 13, 15, 16])
+def test_two_matrices_per_warp(lk, oracle, M, mode):
+    """M <= 16 (pack_kernels.cuh): two matrices share a warp in the reduction and in the
+    apply kernel.  A batch that mixes, matrix by matrix, LETKF-shaped inputs, low-rank ones (repeated
+    eigenvalue, tau = 0 pivots), a diagonal matrix, the Wilkinson matrix and a glued pair of them, a
+    graded matrix and an (M-1)-fold cluster -- so the two halves of a warp take different routes
+    through the apply kernel -- at batch sizes that leave the last half warp, warp and CTA ragged;
+    with the eigenvector route (default), every matrix through the rotation log (evec = 0), and the
+    log shrunk (classic iteration inside the apply kernel).  Same tolerances as everywhere."""
+    rng = np.random.Generator(np.random.Philox(key=5150 + M))
+    k = (M - 1) // 2
+    Wk = np.diag(np.abs(np.arange(M) - k).astype(float)) + np.diag(np.ones(M - 1), 1) + np.diag(np.ones(M - 1), -1)
+    G = Wk.copy()
+    if M >= 4:
+        G[M // 2, M // 2 - 1] = G[M // 2 - 1, M // 2] = 1e-9
+    B = rng.standard_normal((M, M)); B = B + B.T
+    s = 10.0 ** np.linspace(0, 8, M)
+    u = rng.standard_normal(M)
+    special = [Wk, G, np.diag(np.arange(1.0, M + 1)), B * np.outer(s, s) / s[-1] ** 2, np.eye(M) + np.outer(u, u),
+               -(B @ B.T) - np.eye(M), 3.0 * np.eye(M)]
+    for batch in (1, 2, 7, 8, 9, 203):
+        A = wl.letkf_shaped(batch, M, 49, config_index=1200 + M + batch)
+        A[1::5] = wl.letkf_shaped(len(A[1::5]), M, 3, config_index=1300 + M)      # low rank: an (M-3)-fold eigenvalue
+        for i in range(2, batch, 3):
+            A[i] = special[(i // 3) % len(special)]
+        try:
+            if mode != "direct":
+                lk.set_option("evec", 0)
+            if mode == "slow":
+                lk.set_option("log_shrink", 4)
+            w, V, info = run_gpu(lk, A)
+        finally:
+            lk.set_option("evec", 1)
+            lk.set_option("log_shrink", 1)
+        assert ((info & 0xFFFF) == 0).all()
+        wo, _, io, _ = oracle.syev_batched(A)
+        assert (io == 0).all()
+        parity.assert_evd(A, w, V, wo, f"packed M={M} batch={batch} {mode}")
 
 
 @pytest.mark.parametrize("force", [0, 1])
