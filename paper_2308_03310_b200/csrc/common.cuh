@@ -48,7 +48,10 @@ __host__ __device__ inline int log_capacity(int M, bool two_pass = false)
 // follows the flag.
 constexpr double GV_GAP  = 4.0e-3;    // eps C / GV_GAP bounds the loss of orthogonality left uncorrected (C ~ 7 measured)
 constexpr double GV_TINY = 1.0e-8;    // the correction is first order: (eps C / GV_TINY)^2 must stay far below the tolerance
-constexpr int    GV_PH   = 4;         // partners a vector may have on either side
+constexpr int    GV_PH   = 6;         // partners a vector may have on either side (<= 8: the partner lists are two words of
+                                      // 8-bit fields).  4 left 29% of config 5's M = 48 matrices (p = 49: the small eigenvalues
+                                      // of Yb^T R Yb crowd above the shift) to the logging pass, 6 none; the first-order
+                                      // correction's error grows with the partner count: <= 12 (eps C / GV_TINY)^2 ~ 7e-14
 constexpr int    FLAG_REPLAY = 0, FLAG_SLOW = 1, FLAG_GETVEC = 2, FLAG_PENDING = 3;   // Workspace::flags (PENDING: between
                                                                                      // the classifying and the logging QL kernel)
 

@@ -1102,17 +1102,17 @@ __device__ __forceinline__ bool direct_eigenvectors(double (&z)[MT], uint32_t* s
         // z_k -= 1/2 (z_q . z_k) z_q for every such partner q (the classifier bounds their number);
         // the vectors pass through shared memory 32 at a time
         const double gapabs = GV_GAP * nrm;
-        unsigned long long plist = 0ull;
+        unsigned long long pl0 = 0ull, pl1 = 0ull;                      // partners, 8 bits each (GV_PH <= 8 on either side)
         int np = 0;
         if (own) {
             const int s0 = inv[r];
             for (int t = 1; t <= GV_PH && s0 - t >= 0 && lam - wsrt[s0 - t] < gapabs; ++t) {
                 const int q = perm8[s0 - t];
-                if (q >= lo && q <= hi) { plist |= (unsigned long long)q << (8 * np); ++np; }
+                if (q >= lo && q <= hi) { if (np < 8) pl0 |= (unsigned long long)q << (8 * np); else pl1 |= (unsigned long long)q << (8 * (np - 8)); ++np; }
             }
             for (int t = 1; t <= GV_PH && s0 + t < M && wsrt[s0 + t] - lam < gapabs; ++t) {
                 const int q = perm8[s0 + t];
-                if (q >= lo && q <= hi) { plist |= (unsigned long long)q << (8 * np); ++np; }
+                if (q >= lo && q <= hi) { if (np < 8) pl0 |= (unsigned long long)q << (8 * np); else pl1 |= (unsigned long long)q << (8 * (np - 8)); ++np; }
             }
         }
         if (__syncthreads_or(np)) {
@@ -1128,7 +1128,7 @@ __device__ __forceinline__ bool direct_eigenvectors(double (&z)[MT], uint32_t* s
                 __syncthreads();
 #pragma unroll 1
                 for (int t = 0; t < npw; ++t) {
-                    const int q = (int)((plist >> (8 * t)) & 255ull);
+                    const int q = (int)(((t < 8 ? pl0 : pl1) >> (8 * (t & 7))) & 255ull);
                     const bool act = t < np && (q >> 5) == ph;
                     const double* vq = vbuf + (act ? (q & 31) : 0) * LDV;
                     double d0 = 0.0, d1 = 0.0;

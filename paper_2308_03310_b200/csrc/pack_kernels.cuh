@@ -187,17 +187,17 @@ pack16_apply(double* __restrict__ V_, double* __restrict__ w_, int* __restrict__
         if (direct) { columns = ok; slow = !ok; }
         // eigenvalues closer than GV_GAP ||T|| inside a block: first-order symmetric orthogonalisation
         const double gapabs = GV_GAP * nrm;
-        unsigned long long plist = 0ull;
+        unsigned long long pl0 = 0ull, pl1 = 0ull;                      // partners, 8 bits each (GV_PH <= 8 on either side)
         int np = 0;
         if (own && columns) {
             const int s0 = inv[j];
             for (int t = 1; t <= GV_PH && s0 - t >= 0 && lam - wsrt[s0 - t] < gapabs; ++t) {
                 const int q = perm[s0 - t];
-                if (q >= lo && q <= hi) { plist |= (unsigned long long)q << (8 * np); ++np; }
+                if (q >= lo && q <= hi) { if (np < 8) pl0 |= (unsigned long long)q << (8 * np); else pl1 |= (unsigned long long)q << (8 * (np - 8)); ++np; }
             }
             for (int t = 1; t <= GV_PH && s0 + t < M && wsrt[s0 + t] - lam < gapabs; ++t) {
                 const int q = perm[s0 + t];
-                if (q >= lo && q <= hi) { plist |= (unsigned long long)q << (8 * np); ++np; }
+                if (q >= lo && q <= hi) { if (np < 8) pl0 |= (unsigned long long)q << (8 * np); else pl1 |= (unsigned long long)q << (8 * (np - 8)); ++np; }
             }
         }
         const int npw = __reduce_max_sync(FULL, np);                    // the whole warp walks the longest list
@@ -207,7 +207,7 @@ pack16_apply(double* __restrict__ V_, double* __restrict__ w_, int* __restrict__
             __syncwarp();
 #pragma unroll 1
             for (int t = 0; t < npw; ++t) {
-                const int q = (int)((plist >> (8 * t)) & 255ull);
+                const int q = (int)(((t < 8 ? pl0 : pl1) >> (8 * (t & 7))) & 255ull);
                 const bool act = t < np;
                 const double* vq = tile + (act ? q : 0) * PK_LD;
                 double d0 = 0.0, d1 = 0.0;
