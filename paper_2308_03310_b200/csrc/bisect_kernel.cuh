@@ -47,7 +47,7 @@ bisect_classify_kernel(Workspace ws, int M, double* __restrict__ w, int* __restr
 {
     using C = FastCfg<MT>;
     __shared__ double ds[MT], es[MT], e2[MT], lam[MT], wsrt[MT];
-    __shared__ unsigned char single_s[MT];
+    __shared__ short blk_s[MT];                           // block of the k-th smallest eigenvalue (negated: 1 x 1 block)
     __shared__ unsigned cutw[2];
     const int k = threadIdx.x;
     const size_t b = blockIdx.x;
@@ -62,7 +62,7 @@ bisect_classify_kernel(Workspace ws, int M, double* __restrict__ w, int* __restr
     for (int i = 0; i < M; ++i) nrm = fmax(nrm, fabs(ds[i]) + (i < M - 1 ? fabs(es[i]) : 0.0));
     const double thr = eps * nrm;
     bool cut = true;
-    if (k < M - 1) cut = fabs(es[k]) <= fmax(eps * (fabs(ds[k]) + fabs(ds[k + 1])), thr);
+    if (k < M - 1) cut = fabs(es[k]) <= fmax(eps * (fabs(ds[k]) + fabs(ds[k + 1])), GV_SPLIT * thr);
     __syncthreads();
     if (k < MT) { const double ev = cut ? 0.0 : es[k]; es[k] = ev; e2[k] = ev * ev; }
     const unsigned cw = __ballot_sync(0xffffffffu, cut);
@@ -121,16 +121,11 @@ bisect_classify_kernel(Workspace ws, int M, double* __restrict__ w, int* __restr
         ws.perm[b * M + rank] = k;
         ws.s1[b * M + k] = lk;
         wsrt[rank] = lk;
-        single_s[rank] = (lo == hi) ? 1 : 0;
+        blk_s[rank] = (short)((lo == hi) ? -(lo + 1) : (lo + 1));
     }
     __syncthreads();
     bool hard = false;
-    if (k + 1 < M) {
-        const double dk = wsrt[k];
-        const bool both_single = single_s[k] && single_s[k + 1];
-        if (wsrt[k + 1] - dk < GV_TINY * nrm && !both_single) hard = true;
-        if (k + GV_PH + 1 < M && wsrt[k + GV_PH + 1] - dk < GV_GAP * nrm) hard = true;
-    }
+    if (k + 1 < M) hard = gv_hard_at(k, M, nrm, [&](int u) { return wsrt[u]; }, [&](int u) { return (int)blk_s[u]; });
     const int anyhard = __syncthreads_or(hard ? 1 : 0);
     if (k == 0) {
         ws.nsweeps[b] = 0;

@@ -48,10 +48,52 @@ __host__ __device__ inline int log_capacity(int M, bool two_pass = false)
 // follows the flag.
 constexpr double GV_GAP  = 4.0e-3;    // eps C / GV_GAP bounds the loss of orthogonality left uncorrected (C ~ 7 measured)
 constexpr double GV_TINY = 1.0e-8;    // the correction is first order: (eps C / GV_TINY)^2 must stay far below the tolerance
-constexpr int    GV_PH   = 6;         // partners a vector may have on either side (<= 8: the partner lists are two words of
+constexpr int    GV_PH   = 12;        // partners a vector may have on either side (<= 12: the partner lists are three words of
                                       // 8-bit fields).  4 left 29% of config 5's M = 48 matrices (p = 49: the small eigenvalues
-                                      // of Yb^T R Yb crowd above the shift) to the logging pass, 6 none; the first-order
-                                      // correction's error grows with the partner count: <= 12 (eps C / GV_TINY)^2 ~ 7e-14
+                                      // of Yb^T R Yb crowd above the shift) to the logging pass, 6 none; M = 96 with p = 98 has
+                                      // up to 10 in the window.  The first-order correction's error grows with the partner
+                                      // count: <= 24 (eps C / GV_TINY)^2 ~ 1.4e-13
+// Both tests are taken among the eigenvalues of ONE unreduced block of T (the eigenvalue found at position k belongs to the
+// block of k): vectors of different blocks have disjoint supports, and a 1 x 1 block's vector is a unit vector.
+// partner list of one eigenvector: up to 24 positions (< 256), three words of 8-bit fields, selected without indexing
+struct PartnerList {
+    unsigned long long w0 = 0ull, w1 = 0ull, w2 = 0ull;
+    int np = 0;
+    __device__ __forceinline__ void add(int q)
+    {
+        const unsigned long long v = (unsigned long long)q << (8 * (np & 7));
+        if (np < 8) w0 |= v; else if (np < 16) w1 |= v; else if (np < 24) w2 |= v;
+        if (np < 24) ++np;
+    }
+    __device__ __forceinline__ int get(int t) const
+    {
+        const unsigned long long w = t < 8 ? w0 : (t < 16 ? w1 : w2);
+        return (int)((w >> (8 * (t & 7))) & 255ull);
+    }
+};
+// The sorted eigenvalue s (value lam, block id blk > 0, or < 0 for a 1 x 1 block) against the ones above it: returns true
+// when the matrix has to go to the rotation log.  val(s), blkid(s) read the sorted sequence.
+template <class FV, class FB>
+__device__ __forceinline__ bool gv_hard_at(int s, int M, double nrm, FV val, FB blkid)
+{
+    const int blk = blkid(s);
+    if (blk < 0) return false;
+    const double lam = val(s);
+    int cnt = 0;
+    for (int u = s + 1; u < M; ++u) {
+        const double gap = val(u) - lam;
+        if (!(gap < GV_GAP * nrm)) break;
+        if (blkid(u) != blk) continue;
+        if (gap < GV_TINY * nrm) return true;
+        if (++cnt > GV_PH) return true;
+    }
+    return false;
+}
+// Splitting T (reading G24): an off-diagonal |e_i| <= GV_SPLIT 2^-53 ||T|| (or 2^-53 (|d_i| + |d_i+1|)) is set to exactly 0
+// before any solver sees the matrix -- a backward error of GV_SPLIT eps ||T|| per entry, 2 sqrt(2 M) eps ||T|| in all.  The
+// factor is what the rounding of the reduction leaves in the part of T that belongs to a repeated eigenvalue (measured on
+// config 5, M = 128 ... 256 with p = 98: 1e-17 ... 6e-16 ||T||): with it such a cluster falls apart into 1 x 1 blocks.
+constexpr double GV_SPLIT = 8.0;
 constexpr int    FLAG_REPLAY = 0, FLAG_SLOW = 1, FLAG_GETVEC = 2, FLAG_PENDING = 3;   // Workspace::flags (PENDING: between
                                                                                      // the classifying and the logging QL kernel)
 

@@ -1067,7 +1067,7 @@ __device__ __forceinline__ bool direct_eigenvectors(double (&z)[MT], uint32_t* s
     if constexpr (C::NW > 1) nrm = fmax(nrmw[0], nrmw[1]);
     const double thr = eps * nrm;
     bool cut = true;
-    if (r < M - 1) cut = fabs(es[r]) <= fmax(eps * (fabs(ds[r]) + fabs(ds[r + 1])), thr);
+    if (r < M - 1) cut = fabs(es[r]) <= fmax(eps * (fabs(ds[r]) + fabs(ds[r + 1])), GV_SPLIT * thr);
     __syncthreads();
     if (r < MT && cut) es[r] = 0.0;
     const unsigned cw = __ballot_sync(0xffffffffu, cut);
@@ -1102,22 +1102,21 @@ __device__ __forceinline__ bool direct_eigenvectors(double (&z)[MT], uint32_t* s
         // z_k -= 1/2 (z_q . z_k) z_q for every such partner q (the classifier bounds their number);
         // the vectors pass through shared memory 32 at a time
         const double gapabs = GV_GAP * nrm;
-        unsigned long long pl0 = 0ull, pl1 = 0ull;                      // partners, 8 bits each (GV_PH <= 8 on either side)
-        int np = 0;
+        PartnerList pl;                                                 // same-block eigenvalues within GV_GAP ||T|| (the classifier bounds them)
         if (own) {
             const int s0 = inv[r];
-            for (int t = 1; t <= GV_PH && s0 - t >= 0 && lam - wsrt[s0 - t] < gapabs; ++t) {
+            for (int t = 1; s0 - t >= 0 && lam - wsrt[s0 - t] < gapabs; ++t) {
                 const int q = perm8[s0 - t];
-                if (q >= lo && q <= hi) { if (np < 8) pl0 |= (unsigned long long)q << (8 * np); else pl1 |= (unsigned long long)q << (8 * (np - 8)); ++np; }
+                if (q >= lo && q <= hi) pl.add(q);
             }
-            for (int t = 1; t <= GV_PH && s0 + t < M && wsrt[s0 + t] - lam < gapabs; ++t) {
+            for (int t = 1; s0 + t < M && wsrt[s0 + t] - lam < gapabs; ++t) {
                 const int q = perm8[s0 + t];
-                if (q >= lo && q <= hi) { if (np < 8) pl0 |= (unsigned long long)q << (8 * np); else pl1 |= (unsigned long long)q << (8 * (np - 8)); ++np; }
+                if (q >= lo && q <= hi) pl.add(q);
             }
         }
-        if (__syncthreads_or(np)) {
+        if (__syncthreads_or(pl.np)) {
             constexpr int LDV = MT + 1;
-            const int npw = __reduce_max_sync(0xffffffffu, np);             // whole warps walk the longest list
+            const int npw = __reduce_max_sync(0xffffffffu, pl.np);             // whole warps walk the longest list
 #pragma unroll 1
             for (int ph = 0; ph < C::NW; ++ph) {
                 if (ph) __syncthreads();
@@ -1128,8 +1127,8 @@ __device__ __forceinline__ bool direct_eigenvectors(double (&z)[MT], uint32_t* s
                 __syncthreads();
 #pragma unroll 1
                 for (int t = 0; t < npw; ++t) {
-                    const int q = (int)(((t < 8 ? pl0 : pl1) >> (8 * (t & 7))) & 255ull);
-                    const bool act = t < np && (q >> 5) == ph;
+                    const int q = pl.get(t);
+                    const bool act = t < pl.np && (q >> 5) == ph;
                     const double* vq = vbuf + (act ? (q & 31) : 0) * LDV;
                     double d0 = 0.0, d1 = 0.0;
 #pragma unroll

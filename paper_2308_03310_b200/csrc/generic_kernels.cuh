@@ -184,7 +184,9 @@ generic_apply_one(double* V_, double* __restrict__ w_, const Workspace& ws, int 
     __shared__ int sh_rc, sh_lo, sh_m, sh_fail;
 
     const int tid = threadIdx.x;
-    const int flagged = ws.flags[b];
+    const int flag = ws.flags[b];
+    if (flag == FLAG_GETVEC) return;                      // finished by big_getvec + big_gemm (no rotations)
+    const int flagged = flag == FLAG_SLOW;
     if (only_flagged && !flagged) return;
     double* B = V_ + b * M * M;
 
@@ -379,7 +381,7 @@ generic_apply(double* V_, double* __restrict__ w_, Workspace ws, int M, int n, i
     // finisher: scan the flags GEN_NT at a time, work only where one is set (normally nowhere)
     for (size_t base = (size_t)blockIdx.x * GEN_NT; base < (size_t)n; base += (size_t)gridDim.x * GEN_NT) {
         const size_t mine = base + threadIdx.x;
-        const int f = (mine < (size_t)n) ? ws.flags[mine] : 0;
+        const int f = (mine < (size_t)n) ? (ws.flags[mine] == FLAG_SLOW) : 0;
         if (!__syncthreads_or(f)) continue;
         const size_t end = (base + GEN_NT < (size_t)n) ? base + GEN_NT : (size_t)n;
         for (size_t b = base; b < end; ++b) {

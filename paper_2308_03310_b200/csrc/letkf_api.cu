@@ -17,6 +17,7 @@
 #include "ns_kernel.cuh"
 #include "mid_kernels.cuh"
 #include "pack_kernels.cuh"
+#include "big_kernels.cuh"
 
 namespace letkf {
 
@@ -102,6 +103,8 @@ struct Options {
                              // the trailing 32 x 32 problem by one warp per matrix): 1.07 + 0.25 ms against 1.46 ms (config 3)
     int pack = 1;            // M <= 16, qform = 0, EVD calls: two matrices per warp (pack_kernels.cuh): 1 = reduction and
                              // apply kernel, 2 = reduction only, 3 = apply kernel only, 0 = one matrix per warp
+    int bigvec = 1;          // M > 64 (and evec = 1): eigenvectors of T by twisted factorisations and V = Q Z as one product on
+                             // the FP64 tensor cores where the spectrum allows (big_kernels.cuh); 0 = always the rotation log
     int evec = 1;            // M <= 64, qform = 0: 1 = eigenvectors of T by twisted factorisations where the spectrum
                              // allows (ql_log_kernel classifies), the logged rotations otherwise; 0 = always the log
 };
@@ -125,7 +128,9 @@ struct EntryScope {                      // first thing every entry point constr
 // ahead of the eigensolver without holding log space.
 static bool use_fast(int M) { return fast_supported(M) && !t_opt.force_generic; }
 static bool use_mid(int M) { return mid_supported(M) && !t_opt.force_generic; }
-static bool use_getvec(int M) { return use_fast(M) && !t_opt.qform && t_opt.evec; }
+// M > 64: the eigenvector route of big_kernels.cuh (Z in the matrix's record of the rotation log, which must have its full size)
+static bool use_bigvec(int M) { return M > 64 && !use_fast(M) && t_opt.evec && t_opt.bigvec && t_opt.log_shrink == 1; }
+static bool use_getvec(int M) { return (use_fast(M) && !t_opt.qform && t_opt.evec) || use_bigvec(M); }
 
 static size_t carve(Workspace& ws, void* base, int M, int nmat, int nlogmat, bool two_pass)
 {
@@ -193,7 +198,7 @@ static Plan make_plan(int M, int batch, size_t extra, size_t avail)
     pl.two_pass = t_opt.two_pass >= 0 ? t_opt.two_pass != 0 : ((long)batch * M >= (1L << 18));
     pl.ql_mode = pl.two_pass ? QL_TWO_PASS : QL_ONE_PASS;
     if (use_getvec(M)) { pl.ql_mode = QL_CLASSIFY; pl.two_pass = true; }   // (a logged pass is always the second one)
-    pl.bisect = use_getvec(M) && (t_opt.bisect >= 0 ? t_opt.bisect != 0 : batch <= BISECT_MAX_BATCH);
+    pl.bisect = use_getvec(M) && use_fast(M) && (t_opt.bisect >= 0 ? t_opt.bisect != 0 : batch <= BISECT_MAX_BATCH);
     const bool want_pipe = t_opt.pipeline && (!g_prof.on || g_prof.keep_pipeline) && batch >= 2 * PIPE_MIN_SUB;
     auto bytes_for = [&](size_t n, size_t nl) { return plan_bytes(M, n, nl, extra, pl.two_pass); };
     if (want_pipe) {
@@ -207,7 +212,7 @@ static Plan make_plan(int M, int batch, size_t extra, size_t avail)
         // where every matrix logs its rotations (M > 64, or evec = 0) each slot has its log; where most
         // matrices never do (the eigenvector path of M <= 64) the log slots share a fixed budget
         int nlog = t_opt.log_slots > 0 ? t_opt.log_slots
-                 : (pl.ql_mode == QL_CLASSIFY ? (int)((PIPE_LOG_BYTES + log_entry * per - 1) / (log_entry * per)) : nslot);
+                 : ((pl.ql_mode == QL_CLASSIFY && use_fast(M)) ? (int)((PIPE_LOG_BYTES + log_entry * per - 1) / (log_entry * per)) : nslot);
         if (nlog < 2) nlog = 2;
         if (nlog > nslot) nlog = nslot;
         if (avail) {                       // a smaller workspace: fewer log slots first, then fewer slots
@@ -370,7 +375,7 @@ template <int TPB, int MODE>
 static int ql_launch(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st)
 {
     cudaError_t ce;
-    const size_t ql_smem = sizeof(double) * 2 * (size_t)M * TPB + 24 * (size_t)TPB;   // (d, e) per lane + the sort's bookkeeping
+    const size_t ql_smem = sizeof(double) * 2 * (size_t)M * TPB + (8 * (size_t)((M + 63) / 64) + 16) * TPB;   // (d, e) per lane + block boundaries, threshold, sort state
     if ((ce = allow_smem(ql_log_kernel<TPB, MODE>, ql_smem)) != cudaSuccess) return (int)ce;
     const int per_cta = (MODE == QL_TWO_PASS || MODE == QL_LOGPASS_PAIRED) ? TPB / 2 : TPB;  // two lanes per matrix when the iteration runs twice side by side
     const int qblocks = (n + per_cta - 1) / per_cta;
@@ -392,8 +397,7 @@ static int ql_run(int M, int n, double* w, int* info, Workspace ws, cudaStream_t
 static int stage_QL(int M, int n, double* w, int* info, Workspace ws, cudaStream_t st, int mode)
 {
     int tpb = t_opt.ql_tpb ? t_opt.ql_tpb : (M <= 64 ? 128 : 32);
-    while (tpb > 32 && (sizeof(double) * 2 * (size_t)M + 24) * tpb > 200 * 1024) tpb -= 32;
-    if (mode == QL_CLASSIFY && tpb < 64) tpb = 64;      // the classifier wants one lane per eigenvalue (M <= 64)
+    while (tpb > 32 && (sizeof(double) * 2 * (size_t)M + 48) * tpb > 200 * 1024) tpb -= 32;
     switch (tpb) {
         case 192: return ql_run<192>(M, n, w, info, ws, st, mode);
         case 128: return ql_run<128>(M, n, w, info, ws, st, mode);
@@ -446,6 +450,21 @@ static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws,
             case 48: return fast_apply_run<48, false>(V, w, info, ws, M, n, st, ep);
             default: return fast_apply_run<64, false>(V, w, info, ws, M, n, st, ep);
         }
+    }
+    if (use_bigvec(M)) {    // the matrices the classifier left to the eigenvector route (the kernels below skip them)
+        cudaError_t ce;
+        KLAUNCH("big_getvec", st, big_getvec<<<n, (M + 31) / 32 * 32, big_getvec_smem(M), st>>>(ws, w, M));
+#define LETKF_BIG_GEMM(RTW, CT)                                                                               \
+        do {                                                                                                  \
+            if ((ce = allow_smem(big_gemm<RTW, CT>, big_gemm_smem<CT>(M))) != cudaSuccess) return (int)ce;    \
+            KLAUNCH("big_gemm", st, (big_gemm<RTW, CT><<<n, BIG_NT, big_gemm_smem<CT>(M), st>>>(V, ws, M))); \
+        } while (0)
+        if (M <= 96) LETKF_BIG_GEMM(2, 12);
+        else if (M <= 128) LETKF_BIG_GEMM(2, 16);
+        else if (M <= 160) LETKF_BIG_GEMM(3, 10);
+        else if (M <= 192) LETKF_BIG_GEMM(3, 8);
+        else LETKF_BIG_GEMM(4, 8);
+#undef LETKF_BIG_GEMM
     }
     if (use_mid(M)) {
         cudaError_t ce;
@@ -1477,6 +1496,7 @@ int letkf_set_option(const char* name, int value)
     if (strcmp(name, "qform") == 0) { o.qform = value != 0; return LETKF_OK; }
     if (strcmp(name, "evec") == 0) { o.evec = value != 0; return LETKF_OK; }
     if (strcmp(name, "split") == 0) { o.split = value != 0; return LETKF_OK; }
+    if (strcmp(name, "bigvec") == 0) { o.bigvec = value != 0; return LETKF_OK; }
     if (strcmp(name, "pack") == 0) { if (value < 0 || value > 3) return -2; o.pack = value; return LETKF_OK; }
     if (strcmp(name, "pair") == 0) { o.pair = (value == 0 || value == 1) ? value : -1; return LETKF_OK; }
     if (strcmp(name, "bisect") == 0) { o.bisect = (value == 0 || value == 1) ? value : -1; return LETKF_OK; }

@@ -160,7 +160,7 @@ pack16_apply(double* __restrict__ V_, double* __restrict__ w_, int* __restrict__
         for (int o = 8; o > 0; o >>= 1) nrm = fmax(nrm, __shfl_xor_sync(FULL, nrm, o));
         const double thr = eps * nrm;
         bool cut = true;
-        if (j < M - 1) cut = fabs(es[j]) <= fmax(eps * (fabs(ds[j]) + fabs(ds[j + 1])), thr);
+        if (j < M - 1) cut = fabs(es[j]) <= fmax(eps * (fabs(ds[j]) + fabs(ds[j + 1])), GV_SPLIT * thr);
         __syncwarp();
         if (cut) es[j] = 0.0;
         const unsigned cuts = (__ballot_sync(FULL, cut) >> (16 * h)) & 0xffffu;
@@ -187,28 +187,27 @@ pack16_apply(double* __restrict__ V_, double* __restrict__ w_, int* __restrict__
         if (direct) { columns = ok; slow = !ok; }
         // eigenvalues closer than GV_GAP ||T|| inside a block: first-order symmetric orthogonalisation
         const double gapabs = GV_GAP * nrm;
-        unsigned long long pl0 = 0ull, pl1 = 0ull;                      // partners, 8 bits each (GV_PH <= 8 on either side)
-        int np = 0;
+        PartnerList pl;                                                 // same-block eigenvalues within GV_GAP ||T|| (the classifier bounds them)
         if (own && columns) {
             const int s0 = inv[j];
-            for (int t = 1; t <= GV_PH && s0 - t >= 0 && lam - wsrt[s0 - t] < gapabs; ++t) {
+            for (int t = 1; s0 - t >= 0 && lam - wsrt[s0 - t] < gapabs; ++t) {
                 const int q = perm[s0 - t];
-                if (q >= lo && q <= hi) { if (np < 8) pl0 |= (unsigned long long)q << (8 * np); else pl1 |= (unsigned long long)q << (8 * (np - 8)); ++np; }
+                if (q >= lo && q <= hi) pl.add(q);
             }
-            for (int t = 1; t <= GV_PH && s0 + t < M && wsrt[s0 + t] - lam < gapabs; ++t) {
+            for (int t = 1; s0 + t < M && wsrt[s0 + t] - lam < gapabs; ++t) {
                 const int q = perm[s0 + t];
-                if (q >= lo && q <= hi) { if (np < 8) pl0 |= (unsigned long long)q << (8 * np); else pl1 |= (unsigned long long)q << (8 * (np - 8)); ++np; }
+                if (q >= lo && q <= hi) pl.add(q);
             }
         }
-        const int npw = __reduce_max_sync(FULL, np);                    // the whole warp walks the longest list
+        const int npw = __reduce_max_sync(FULL, pl.np);                    // the whole warp walks the longest list
         if (npw > 0) {
 #pragma unroll
             for (int i = 0; i < MT; ++i) tile[j * PK_LD + i] = z[i];
             __syncwarp();
 #pragma unroll 1
             for (int t = 0; t < npw; ++t) {
-                const int q = (int)(((t < 8 ? pl0 : pl1) >> (8 * (t & 7))) & 255ull);
-                const bool act = t < np;
+                const int q = pl.get(t);
+                const bool act = t < pl.np;
                 const double* vq = tile + (act ? q : 0) * PK_LD;
                 double d0 = 0.0, d1 = 0.0;
 #pragma unroll

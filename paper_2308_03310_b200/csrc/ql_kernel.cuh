@@ -111,11 +111,17 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
         QL_E(k) = 0.0;
         return k;
     };
-    // mode 2: boundaries of the unreduced blocks of the ORIGINAL matrix (bit i: e_i negligible)
-    unsigned long long bmask = 0ull;
-    if (mode == QL_CLASSIFY && valid) {
-        for (int k = 0; k < M - 1; ++k)
-            if (fabs(QL_E(k)) <= fmax(eps * (fabs(QL_D(k)) + fabs(QL_D(k + 1))), thr)) bmask |= 1ull << k;
+    // the split of the input (reading G24, common.cuh: GV_SPLIT): negligible off-diagonals are exactly 0 from here on;
+    // mode 2 keeps the boundaries of the unreduced blocks (bit i: e_i = 0), nw64 words per lane behind the (d, e) arrays
+    const int nw64 = (M + 63) >> 6;
+    unsigned long long* bm_sh = reinterpret_cast<unsigned long long*>(sm + 2 * (size_t)M * QL_TPB);   // [nw64][QL_TPB]
+    if (valid) {
+        unsigned long long word = 0ull;
+        for (int k = 0; k < M - 1; ++k) {
+            if (fabs(QL_E(k)) <= fmax(eps * (fabs(QL_D(k)) + fabs(QL_D(k + 1))), GV_SPLIT * thr)) { QL_E(k) = 0.0; word |= 1ull << (k & 63); }
+            if (mode == QL_CLASSIFY && ((k & 63) == 63 || k == M - 2)) { bm_sh[(k >> 6) * QL_TPB + lane] = word; word = 0ull; }
+        }
+        if (mode == QL_CLASSIFY && M == 1) bm_sh[lane] = 0ull;
     }
     int l = 0, m = 0, iter = 0, fail = 0;
     int overflow = 0, nsw = 0, pos = 0;
@@ -279,16 +285,15 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
     // QL_TPB / GS matrices per round (at M = 16 one matrix per round left 112 of 128 lanes idle through
     // 128 rounds of three barriers each -- more than the iteration itself took).
     const bool owner = valid && (!two_pass || (lane & 1));   // the lane that reports the matrix
-    unsigned long long* bm_sh = reinterpret_cast<unsigned long long*>(sm + 2 * (size_t)M * QL_TPB);   // [QL_TPB]
-    double* thr_sh = reinterpret_cast<double*>(bm_sh + QL_TPB);                                        // [QL_TPB]
+    double* thr_sh = reinterpret_cast<double*>(bm_sh + (size_t)nw64 * QL_TPB);                         // [QL_TPB]
     int* sort_sh = reinterpret_cast<int*>(thr_sh + QL_TPB);                                            // [QL_TPB] 1: to sort, 2: and hard
     sort_sh[lane] = (owner && !overflow) ? 1 : 0;
-    bm_sh[lane] = bmask;
     thr_sh[lane] = thr;
     __syncthreads();
     const int gs0 = M <= 16 ? 16 : (M <= 32 ? 32 : 64);
     const int GS = (M <= 64 && QL_TPB % gs0 == 0) ? gs0 : QL_TPB;      // lanes per matrix
     const int ng = QL_TPB / GS, grp = lane / GS, kl = lane - grp * GS;
+    constexpr int KMAX = 8;                                   // eigenvalues per lane: M <= 256 = KMAX * 32
     for (int c0 = 0; c0 < nb; c0 += ng) {
         const int c = c0 + grp;
         const int col = two_pass ? 2 * c + 1 : c;
@@ -296,9 +301,12 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
         const size_t bc = (size_t)(b0 + c);
         const double* dc = dsm + (act ? col : 0);
         double* ec = esm + (act ? col : 0);
-        int myrank = -1;
-        if (act) {
-            for (int k = kl; k < M; k += GS) {
+        int myrank[KMAX];
+#pragma unroll
+        for (int t = 0; t < KMAX; ++t) {
+            const int k = kl + t * GS;
+            myrank[t] = -1;
+            if (act && k < M) {
                 const double v = dc[k * stride];
                 int rank = 0;
                 for (int j = 0; j < M; ++j) {
@@ -307,27 +315,35 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
                 }
                 w[bc * M + rank] = v;
                 ws.perm[bc * M + rank] = k;
-                if (mode == QL_CLASSIFY) { ws.s1[bc * M + k] = v; ec[rank * stride] = v; myrank = rank; }
+                if (mode == QL_CLASSIFY) { ws.s1[bc * M + k] = v; ec[rank * stride] = v; myrank[t] = rank; }
             }
         }
-        if (mode == QL_CLASSIFY) {                            // (M <= 64 <= QL_TPB, GS >= M: one eigenvalue per lane)
+        if (mode == QL_CLASSIFY) {
             __syncthreads();
-            if (act && kl < M) {
-                const unsigned long long bmc = bm_sh[col];
-                const bool lo_cut = kl == 0 || ((bmc >> (kl - 1)) & 1ull);
-                const bool hi_cut = kl == M - 1 || ((bmc >> kl) & 1ull);
-                dsm[myrank * stride + col] = (lo_cut && hi_cut) ? 1.0 : 0.0;   // 1 x 1 block: its eigenvector is a unit vector
+#pragma unroll
+            for (int t = 0; t < KMAX; ++t) {
+                const int k = kl + t * GS;
+                if (act && k < M) {
+                    // block of position k: first position behind the last boundary below k; id > 0, negated for a 1 x 1 block
+                    int lo = 0;
+                    if (k > 0) {
+                        int wq = (k - 1) >> 6;
+                        unsigned long long bits = bm_sh[wq * QL_TPB + col] & (~0ull >> (63 - ((k - 1) & 63)));
+                        while (bits == 0ull && wq > 0) { --wq; bits = bm_sh[wq * QL_TPB + col]; }
+                        if (bits) lo = 64 * wq + (63 - __clzll((long long)bits)) + 1;
+                    }
+                    const bool hi_cut = k == M - 1 || ((bm_sh[(k >> 6) * QL_TPB + col] >> (k & 63)) & 1ull);
+                    dsm[myrank[t] * stride + col] = (lo == k && hi_cut) ? -(double)(lo + 1) : (double)(lo + 1);
+                }
             }
             __syncthreads();
-            if (act && kl + 1 < M) {
-                bool hard = false;
+            bool hard = false;
+            if (act) {
                 const double nrm = thr_sh[col] * 9007199254740992.0;               // max_i(|d_i| + |e_i|)
-                const double dk = ec[kl * stride];
-                const bool both_single = dc[kl * stride] != 0.0 && dc[(kl + 1) * stride] != 0.0;
-                if (ec[(kl + 1) * stride] - dk < GV_TINY * nrm && !both_single) hard = true;
-                if (kl + GV_PH + 1 < M && ec[(kl + GV_PH + 1) * stride] - dk < GV_GAP * nrm) hard = true;
-                if (hard) sort_sh[col] = 2;                   // (every writer writes the same value)
+                for (int k = kl; k + 1 < M && !hard; k += GS)                       // sorted index
+                    hard = gv_hard_at(k, M, nrm, [&](int u) { return ec[u * stride]; }, [&](int u) { return (int)dc[u * stride]; });
             }
+            if (hard) sort_sh[col] = 2;                       // (every writer writes the same value)
         }
     }
     if (mode == QL_CLASSIFY) {

@@ -469,6 +469,40 @@ def test_direct_eigenvectors_are_used_and_fall_back(lk, oracle):
         parity.assert_evd(X, w.cpu().numpy(), V.cpu().numpy(), wo, "direct / replay routes")
 
 
+@pytest.mark.parametrize("bigvec", [1, 0])
+@pytest.mark.parametrize("M,p", [(65, 98), (80, 49), (96, 98), (97, 200), (128, 98), (128, 3), (130, 300), (160, 98), (161, 98),
+                                 (192, 98), (200, 400), (255, 98), (256, 98), (256, 512)])
+def test_eigenvector_route_above_64(lk, oracle, M, p, bigvec):
+    """M > 64 (big_kernels.cuh): where the classifier allows, the eigenvectors of T by twisted
+    factorisations (one thread per eigenvector, the vector in the matrix's record of the rotation
+    log) and V = Q Z as one product on the FP64 tensor cores; letkf_set_option("bigvec", 0) sends
+    every matrix through the rotation log as before.  Shapes: full rank (p >= M - 1: every
+    eigenvalue simple), the sweep's p = 98 < M - 1 (an (M - 98)-fold eigenvalue: T falls apart into
+    1 x 1 blocks there -- reading G24), p = 3, ragged orders at every tile shape of the product;
+    the LETKF-shaped workloads must take the new route (no rotation logged) and the hard spectra of
+    test_hard_spectra (which run with the default) must not."""
+    import torch
+    batch = 21 if M <= 160 else 9
+    A = wl.letkf_shaped(batch, M, p, config_index=1400 + M + p)
+    lk.profile_enable(1)
+    try:
+        lk.set_option("bigvec", bigvec)
+        w, V, info = lk.syev_batched(torch.from_numpy(A).cuda())
+        torch.cuda.synchronize()
+        nrot, ndirect = lk.profile_rotations(), lk.profile_direct()
+    finally:
+        lk.set_option("bigvec", 1)
+        lk.profile_enable(0)
+    w, V, info = w.cpu().numpy(), V.cpu().numpy(), info.cpu().numpy()
+    assert (info == 0).all()
+    if bigvec and p >= M - 1:
+        assert ndirect == batch and nrot == 0, f"{ndirect} of {batch} matrices on the eigenvector route, {nrot} rotations"
+    if not bigvec:
+        assert nrot > 0
+    wo, _, _, _ = oracle.syev_batched(A)
+    parity.assert_evd(A, w, V, wo, f"M={M} p={p} bigvec={bigvec}")
+
+
 @pytest.mark.parametrize("mode", [0, 1])
 @pytest.mark.parametrize("M,p", [(64, 98), (57, 98), (33, 49), (16, 49), (64, 3), (96, 98), (200, 98)])
 def test_ql_one_and_two_pass(lk, oracle, M, p, mode):
@@ -479,9 +513,11 @@ def test_ql_one_and_two_pass(lk, oracle, M, p, mode):
     A = wl.letkf_shaped(150 if M <= 64 else 7, M, p, config_index=940 + M + p)
     try:
         lk.set_option("two_pass", mode)
+        lk.set_option("bigvec", 0)                        # (M > 64: every matrix through the log)
         w, V, info = run_gpu(lk, A)
     finally:
         lk.set_option("two_pass", -1)
+        lk.set_option("bigvec", 1)
     assert (info == 0).all()
     wo, _, _, _ = oracle.syev_batched(A)
     parity.assert_evd(A, w, V, wo, f"two_pass={mode} M={M}")
