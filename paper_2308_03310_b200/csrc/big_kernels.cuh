@@ -22,7 +22,11 @@
 namespace letkf {
 
 constexpr int BIG_NT = 256;
-static inline size_t big_getvec_smem(int M) { return sizeof(double) * 3 * (size_t)M + sizeof(int) * 4 * (size_t)M + 64; }
+static inline size_t big_getvec_smem(int M)
+{
+    // ds, es, wsrt; perm, inv; the tile of the correction [8][M] and its coefficients [2 GV_PH][ceil32(M)]
+    return sizeof(double) * (3 * (size_t)M + 8 * (size_t)M + 2 * GV_PH * (size_t)((M + 31) / 32 * 32)) + sizeof(int) * 4 * (size_t)M + 64;
+}
 
 __device__ __forceinline__ double* big_z(const Workspace& ws, size_t b) { return reinterpret_cast<double*>(ws.rot + b * ws.logcap); }
 
@@ -51,7 +55,6 @@ big_getvec(Workspace ws, const double* __restrict__ w_, int M)
     if (ws.flags[b] != FLAG_GETVEC) return;
     const int k = threadIdx.x, nwarps = blockDim.x >> 5;
     double* Z = big_z(ws, b);
-    double* hcs = Z + (size_t)M * M;                      // [2 GV_PH][M] coefficients of the correction
     const double eps = 1.1102230246251565e-16;
 
     double nrm = 0.0;
@@ -221,46 +224,53 @@ big_getvec(Workspace ws, const double* __restrict__ w_, int M)
         }
     }
     if (!__syncthreads_or(pl.np)) return;
-    const int np = pl.np;
-    for (int t = 0; t < np; ++t) {
-        const int q = pl.get(t);
-        double d0 = 0.0, d1 = 0.0;
-        for (int i0 = lo; i0 <= hi; i0 += BIG_PF) {
-            double bk[BIG_PF], bq[BIG_PF];
-#pragma unroll
-            for (int u = 0; u < BIG_PF; ++u) {
-                const bool in = i0 + u <= hi;
-                bk[u] = in ? Z[(size_t)(i0 + u) * M + k] : 0.0;
-                bq[u] = in ? Z[(size_t)(i0 + u) * M + q] : 0.0;
-            }
-#pragma unroll
-            for (int u = 0; u < BIG_PF; u += 2) { d0 = fma(bk[u], bq[u], d0); d1 = fma(bk[u + 1], bq[u + 1], d1); }
-        }
-        hcs[(size_t)t * M + k] = -0.5 * (d0 + d1);
-    }
-    __syncthreads();
-    for (int i0 = 0; i0 < M; i0 += 4) {
-        double nz[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const int i = i0 + u;
-            nz[u] = 0.0;
-            if (np > 0 && i >= lo && i <= hi) nz[u] = Z[(size_t)i * M + k];
-        }
-        for (int t = 0; t < np; ++t) {
-            const int q = pl.get(t);
-            const double h = hcs[(size_t)t * M + k];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int i = i0 + u;
-                if (i >= lo && i <= hi) nz[u] = fma(h, Z[(size_t)i * M + q], nz[u]);
-            }
+    // Eight rows of Z at a time pass through shared memory (one coalesced copy per tile; the partners'
+    // entries are then random reads of the tile, not of L2): first the coefficients -1/2 z_q . z_k, kept in
+    // shared memory, then z_k += sum_q h_q z_q tile by tile -- the tile holds the uncorrected rows, so the
+    // corrected ones go straight back to Z.
+    const int np = pl.np, NTc = blockDim.x;
+    constexpr int TR = 8;
+    double* tile = reinterpret_cast<double*>(inv + M);                  // [TR][M] (perm and inv: 2 M ints)
+    double* hc = tile + (size_t)TR * M;                                  // [2 GV_PH][NTc]
+    for (int t = 0; t < np; ++t) hc[t * NTc + k] = 0.0;
+    for (int i0 = 0; i0 < M; i0 += TR) {
+        __syncthreads();
+        for (int idx = k; idx < TR * M; idx += NTc) {
+            const int u = idx / M, c = idx - u * M;
+            tile[idx] = (i0 + u < M) ? Z[(size_t)(i0 + u) * M + c] : 0.0;
         }
         __syncthreads();
+        for (int t = 0; t < np; ++t) {
+            const int q = pl.get(t);
+            double d0 = 0.0, d1 = 0.0;
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const int i = i0 + u;
-            if (np > 0 && i >= lo && i <= hi) Z[(size_t)i * M + k] = nz[u];
+            for (int u = 0; u < TR; u += 2) {
+                d0 = fma(tile[u * M + k], tile[u * M + q], d0);
+                d1 = fma(tile[(u + 1) * M + k], tile[(u + 1) * M + q], d1);
+            }
+            hc[t * NTc + k] += d0 + d1;
+        }
+    }
+    for (int i0 = 0; i0 < M; i0 += TR) {
+        __syncthreads();
+        for (int idx = k; idx < TR * M; idx += NTc) {
+            const int u = idx / M, c = idx - u * M;
+            tile[idx] = (i0 + u < M) ? Z[(size_t)(i0 + u) * M + c] : 0.0;
+        }
+        __syncthreads();
+        if (np > 0) {
+            double nz[TR];
+#pragma unroll
+            for (int u = 0; u < TR; ++u) nz[u] = tile[u * M + k];
+            for (int t = 0; t < np; ++t) {
+                const int q = pl.get(t);
+                const double h = -0.5 * hc[t * NTc + k];
+#pragma unroll
+                for (int u = 0; u < TR; ++u) nz[u] = fma(h, tile[u * M + q], nz[u]);
+            }
+#pragma unroll
+            for (int u = 0; u < TR; ++u)
+                if (i0 + u < M) Z[(size_t)(i0 + u) * M + k] = nz[u];
         }
     }
 }

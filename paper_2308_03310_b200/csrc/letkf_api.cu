@@ -197,7 +197,10 @@ static Plan make_plan(int M, int batch, size_t extra, size_t avail)
     Plan pl;
     pl.two_pass = t_opt.two_pass >= 0 ? t_opt.two_pass != 0 : ((long)batch * M >= (1L << 18));
     pl.ql_mode = pl.two_pass ? QL_TWO_PASS : QL_ONE_PASS;
-    if (use_getvec(M)) { pl.ql_mode = QL_CLASSIFY; pl.two_pass = true; }   // (a logged pass is always the second one)
+    // (a logged pass is always the second one.  M > 128: scout and logger side by side and the classification at the end --
+    // measured, config 5 with p = 98, where every matrix of M >= 128 stays on the log: M = 256 27.7 ms against 28.9 ms for
+    // classify-then-log; at M = 96, where none does, 8.5 against 8.0 ms)
+    if (use_getvec(M)) { pl.ql_mode = (use_bigvec(M) && M > 128) ? QL_PAIRED_CLASSIFY : QL_CLASSIFY; pl.two_pass = true; }
     pl.bisect = use_getvec(M) && use_fast(M) && (t_opt.bisect >= 0 ? t_opt.bisect != 0 : batch <= BISECT_MAX_BATCH);
     const bool want_pipe = t_opt.pipeline && (!g_prof.on || g_prof.keep_pipeline) && batch >= 2 * PIPE_MIN_SUB;
     auto bytes_for = [&](size_t n, size_t nl) { return plan_bytes(M, n, nl, extra, pl.two_pass); };
@@ -377,7 +380,7 @@ static int ql_launch(int M, int n, double* w, int* info, Workspace ws, cudaStrea
     cudaError_t ce;
     const size_t ql_smem = sizeof(double) * 2 * (size_t)M * TPB + (8 * (size_t)((M + 63) / 64) + 16) * TPB;   // (d, e) per lane + block boundaries, threshold, sort state
     if ((ce = allow_smem(ql_log_kernel<TPB, MODE>, ql_smem)) != cudaSuccess) return (int)ce;
-    const int per_cta = (MODE == QL_TWO_PASS || MODE == QL_LOGPASS_PAIRED) ? TPB / 2 : TPB;  // two lanes per matrix when the iteration runs twice side by side
+    const int per_cta = (MODE == QL_TWO_PASS || MODE == QL_LOGPASS_PAIRED || MODE == QL_PAIRED_CLASSIFY) ? TPB / 2 : TPB;  // two lanes per matrix when the iteration runs twice side by side
     const int qblocks = (n + per_cta - 1) / per_cta;
     KLAUNCH("ql_log_kernel", st, (ql_log_kernel<TPB, MODE><<<qblocks, TPB, ql_smem, st>>>(ws, M, n, w, info)));
     return 0;
@@ -388,6 +391,7 @@ static int ql_run(int M, int n, double* w, int* info, Workspace ws, cudaStream_t
     switch (mode) {
         case QL_TWO_PASS: return ql_launch<TPB, QL_TWO_PASS>(M, n, w, info, ws, st);
         case QL_CLASSIFY: return ql_launch<TPB, QL_CLASSIFY>(M, n, w, info, ws, st);
+        case QL_PAIRED_CLASSIFY: return ql_launch<TPB, QL_PAIRED_CLASSIFY>(M, n, w, info, ws, st);
         case QL_LOGPASS: return ql_launch<TPB, QL_LOGPASS>(M, n, w, info, ws, st);
         case QL_LOGPASS_PAIRED: return ql_launch<TPB, QL_LOGPASS_PAIRED>(M, n, w, info, ws, st);
         default: return ql_launch<TPB, QL_ONE_PASS>(M, n, w, info, ws, st);
@@ -453,6 +457,7 @@ static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws,
     }
     if (use_bigvec(M)) {    // the matrices the classifier left to the eigenvector route (the kernels below skip them)
         cudaError_t ce;
+        if ((ce = allow_smem(big_getvec, big_getvec_smem(M))) != cudaSuccess) return (int)ce;
         KLAUNCH("big_getvec", st, big_getvec<<<n, (M + 31) / 32 * 32, big_getvec_smem(M), st>>>(ws, w, M));
 #define LETKF_BIG_GEMM(RTW, CT)                                                                               \
         do {                                                                                                  \

@@ -36,9 +36,12 @@ namespace letkf {
 // ws.s1 and the matrix is marked FLAG_PENDING.  QL_LOGPASS (a second launch, the first one that needs
 // the matrix's slot of the rotation log) runs the logging pass of the pending matrices, shifted by
 // those eigenvalues (-> FLAG_REPLAY); a CTA without a pending matrix leaves at once.
-constexpr int QL_ONE_PASS = 0, QL_TWO_PASS = 1, QL_CLASSIFY = 2, QL_LOGPASS = 3, QL_LOGPASS_PAIRED = 4;
+constexpr int QL_ONE_PASS = 0, QL_TWO_PASS = 1, QL_CLASSIFY = 2, QL_LOGPASS = 3, QL_LOGPASS_PAIRED = 4, QL_PAIRED_CLASSIFY = 5;
 // (QL_LOGPASS_PAIRED: the pending matrices as in QL_LOGPASS, but by pairs of lanes as in QL_TWO_PASS --
-// behind bisect_kernel.cuh, whose eigenvalues are not in the order in which QL would deflate them)
+// behind bisect_kernel.cuh, whose eigenvalues are not in the order in which QL would deflate them;
+// QL_PAIRED_CLASSIFY (M > 64, big_kernels.cuh): QL_TWO_PASS, and the matrix is classified at the end -- easy: FLAG_GETVEC, the
+// log is dropped (its record becomes the store of the eigenvectors of T); else FLAG_REPLAY.  One launch and the latency of one
+// pass whatever the spectrum, at the price of log writes nobody reads for the easy matrices)
 
 // The mode is a template parameter: in the eigenvalue-only pass the log stores, the shift look-up and the
 // pair bookkeeping are not compiled in at all (as run-time predicates they cost 30% of the rotation step).
@@ -51,7 +54,8 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
     double* esm = sm + (size_t)M * QL_TPB;        // [M][QL_TPB]
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x;              // column of the [M][QL_TPB] arrays
-    constexpr bool two_pass = mode == QL_TWO_PASS || mode == QL_LOGPASS_PAIRED;  // (pairs of lanes)
+    constexpr bool two_pass = mode == QL_TWO_PASS || mode == QL_LOGPASS_PAIRED || mode == QL_PAIRED_CLASSIFY;  // (pairs of lanes)
+    constexpr bool classify = mode == QL_CLASSIFY || mode == QL_PAIRED_CLASSIFY;
     constexpr bool pending_only = mode == QL_LOGPASS || mode == QL_LOGPASS_PAIRED;
     const int nmc = two_pass ? QL_TPB / 2 : QL_TPB;         // matrices per CTA
     const int b0 = blockIdx.x * nmc;
@@ -119,9 +123,9 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
         unsigned long long word = 0ull;
         for (int k = 0; k < M - 1; ++k) {
             if (fabs(QL_E(k)) <= fmax(eps * (fabs(QL_D(k)) + fabs(QL_D(k + 1))), GV_SPLIT * thr)) { QL_E(k) = 0.0; word |= 1ull << (k & 63); }
-            if (mode == QL_CLASSIFY && ((k & 63) == 63 || k == M - 2)) { bm_sh[(k >> 6) * QL_TPB + lane] = word; word = 0ull; }
+            if (classify && ((k & 63) == 63 || k == M - 2)) { bm_sh[(k >> 6) * QL_TPB + lane] = word; word = 0ull; }
         }
-        if (mode == QL_CLASSIFY && M == 1) bm_sh[lane] = 0ull;
+        if (classify && M == 1) bm_sh[lane] = 0ull;
     }
     int l = 0, m = 0, iter = 0, fail = 0;
     int overflow = 0, nsw = 0, pos = 0;
@@ -315,10 +319,10 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
                 }
                 w[bc * M + rank] = v;
                 ws.perm[bc * M + rank] = k;
-                if (mode == QL_CLASSIFY) { ws.s1[bc * M + k] = v; ec[rank * stride] = v; myrank[t] = rank; }
+                if (classify) { ws.s1[bc * M + k] = v; ec[rank * stride] = v; myrank[t] = rank; }
             }
         }
-        if (mode == QL_CLASSIFY) {
+        if (classify) {
             __syncthreads();
 #pragma unroll
             for (int t = 0; t < KMAX; ++t) {
@@ -346,17 +350,17 @@ ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __res
             if (hard) sort_sh[col] = 2;                       // (every writer writes the same value)
         }
     }
-    if (mode == QL_CLASSIFY) {
+    if (classify) {
         __syncthreads();
         easy = sort_sh[lane] == 1;
     }
     if (owner) {
         ws.nsweeps[b] = nsw;
-        ws.flags[b] = overflow ? FLAG_SLOW : (mode == QL_CLASSIFY ? (easy ? FLAG_GETVEC : FLAG_PENDING) : FLAG_REPLAY);
+        ws.flags[b] = overflow ? FLAG_SLOW : (classify && easy ? FLAG_GETVEC : (mode == QL_CLASSIFY ? FLAG_PENDING : FLAG_REPLAY));
         if (info && !overflow) info[b] = fail;
     }
     if (ws.rot_counter) {
-        const int tot = __reduce_add_sync(FULL, (valid && logging) ? pos : 0);
+        const int tot = __reduce_add_sync(FULL, (valid && logging && !easy) ? pos : 0);   // (a log that is dropped does not count)
         if ((lane & 31) == 0) atomicAdd(ws.rot_counter, (unsigned long long)tot);
         const int ne = __reduce_add_sync(FULL, (owner && easy) ? 1 : 0);
         if ((lane & 31) == 0 && ne) atomicAdd(ws.rot_counter + 1, (unsigned long long)ne);
