@@ -46,7 +46,7 @@ constexpr int QL_ONE_PASS = 0, QL_TWO_PASS = 1, QL_CLASSIFY = 2, QL_LOGPASS = 3,
 // The mode is a template parameter: in the eigenvalue-only pass the log stores, the shift look-up and the
 // pair bookkeeping are not compiled in at all (as run-time predicates they cost 30% of the rotation step).
 template <int QL_TPB, int mode>
-__global__ void __launch_bounds__(QL_TPB)
+__global__ void __launch_bounds__(QL_TPB, 1024 / QL_TPB)     // <= 64 registers: a QL CTA arriving beside tridiag / apply CTAs must stay small
 ql_log_kernel(Workspace ws, int M, int batch, double* __restrict__ w, int* __restrict__ info)
 {
     extern __shared__ double sm[];
