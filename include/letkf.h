@@ -285,8 +285,12 @@ int letkf_last_launch_count(void);
  *   "log_shrink"    k divides the rotation-log capacity so that tests can force the in-kernel slow path
  *   "qform"         M <= 64: 1 = explicit Q formed by the reduction kernel, rotations replayed on its rows (round 1's
  *                   form); 0 (default) = reflectors kept, back-transform in the apply kernel
- *   "evec"          M <= 64, qform 0: 1 (default) = eigenvectors of T by twisted factorisations where the classifier
- *                   allows; 0 = always the logged rotations
+ *   "evec"          1 (default) = eigenvectors of T by twisted factorisations where the classifier allows (M <= 64 with
+ *                   qform 0; M > 64 with bigvec 1); 0 = always the logged rotations
+ *   "bigvec"        M > 64, evec 1: 1 (default) = the eigenvector route above 64 (eigenvectors of T in the matrix's record
+ *                   of the rotation log, V = Q Z on the FP64 tensor cores); 0 = always the logged rotations
+ *   "pack"          M <= 16, qform 0, EVD calls: two matrices per warp in the reduction and the apply kernel (1, default),
+ *                   in the reduction only (2), in the apply kernel only (3), one matrix per warp (0)
  *   "bisect"        M <= 64, evec 1: eigenvalues by multisection with M threads per matrix: 0 / 1 (-1 = batch <= 1024)
  *   "pair"          32 < M <= 64: the reduction kernel takes two matrices per CTA: 0 / 1 (-1 = for 32 < M <= 48)
  *   "split"         48 < M <= 64: the reduction as two kernels, pivots M-1 ... 33 by two warps and the trailing
