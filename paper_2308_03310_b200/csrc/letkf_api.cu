@@ -103,6 +103,8 @@ struct Options {
                              // the trailing 32 x 32 problem by one warp per matrix): 1.07 + 0.25 ms against 1.46 ms (config 3)
     int pack = 1;            // M <= 16, qform = 0, EVD calls: two matrices per warp (pack_kernels.cuh): 1 = reduction and
                              // apply kernel, 2 = reduction only, 3 = apply kernel only, 0 = one matrix per warp
+    int mid_split = 1;       // 64 < M <= 128, mid_reg >= 1: the reduction stops after pivot 64 and the trailing 64 x 64 block goes
+                             // through the register kernels of the M <= 64 path (0 = one kernel down to pivot 1)
     int bigvec = 1;          // M > 64 (and evec = 1): eigenvectors of T by twisted factorisations and V = Q Z as one product on
                              // the FP64 tensor cores where the spectrum allows (big_kernels.cuh); 0 = always the rotation log
     int evec = 1;            // M <= 64, qform = 0: 1 = eigenvectors of T by twisted factorisations where the spectrum
@@ -130,6 +132,11 @@ static bool use_fast(int M) { return fast_supported(M) && !t_opt.force_generic; 
 static bool use_mid(int M) { return mid_supported(M) && !t_opt.force_generic; }
 // M > 64: the eigenvector route of big_kernels.cuh (Z in the matrix's record of the rotation log, which must have its full size)
 static bool use_bigvec(int M) { return M > 64 && !use_fast(M) && t_opt.evec && t_opt.bigvec && t_opt.log_shrink == 1; }
+// 64 < M <= 128: the reduction hands its trailing 64 x 64 block to the register kernels (mid_kernels.cuh, HEAD)
+static bool use_midsplit(int M)
+{
+    return use_mid(M) && mid_threads(M) <= 128 && t_opt.mid_reg >= 1 && t_opt.mid_split && t_opt.log_shrink == 1;
+}
 static bool use_getvec(int M) { return (use_fast(M) && !t_opt.qform && t_opt.evec) || use_bigvec(M); }
 
 static size_t carve(Workspace& ws, void* base, int M, int nmat, int nlogmat, bool two_pass)
@@ -139,7 +146,7 @@ static size_t carve(Workspace& ws, void* base, int M, int nmat, int nlogmat, boo
     auto take = [&](size_t bytes) { char* q = p ? p + off : nullptr; off = align_up(off + bytes, 256); return q; };
     ws.swcap = sweep_capacity(M);
     ws.logcap = log_capacity(M, two_pass) / t_opt.log_shrink;      // (the memory is still sized for the full log)
-    ws.reflstride = (use_fast(M) && !t_opt.qform) ? fast_refl_doubles(M) : 0;
+    ws.reflstride = (use_fast(M) && !t_opt.qform) ? fast_refl_doubles(M) : (use_midsplit(M) ? ((mid_split_refl_doubles(M) + 1) & ~1) : 0);
     ws.rot_counter = g_prof.on ? g_prof.d_rot : nullptr;
     ws.dws     = reinterpret_cast<double*>(take(sizeof(double) * (size_t)M * nmat));
     ws.ews     = reinterpret_cast<double*>(take(sizeof(double) * (size_t)M * nmat));
@@ -363,6 +370,24 @@ static int stage_T(const double* A, int M, int n, double* V, Workspace ws, cudaS
         // at MT = 160 the 80 matrix registers of a thread spill under the 102 a CTA of 640 allows and
         // the shared-memory form is as fast (10.5 vs 10.9 ms): mid_reg = 1 (default) / 2 (force) / 0 (never)
         const bool reg = t_opt.mid_reg == 2 || (t_opt.mid_reg == 1 && mt <= 128);
+        if (use_midsplit(M)) {
+            // pivots M-1 ... 64 here, the trailing 64 x 64 block in the register kernels, then Q^T from both sets of
+            // reflectors.  Scratch (free until the QL kernel): the block, its d and e, flat in the rotation-log area
+            double* blk = reinterpret_cast<double*>(ws.rot);
+            double* d64 = blk + (size_t)n * 4096;
+            double* e64 = d64 + (size_t)n * 64;
+            auto head = mt == 96 ? mid_tridiag_formq_reg<96, true> : mid_tridiag_formq_reg<128, true>;
+            if ((ce = allow_smem(head, smem)) != cudaSuccess) return (int)ce;
+            KLAUNCH("mid_tridiag_head", st, head<<<n, MID_TPR * mt, smem, st>>>(A, V, ws, M));
+            Workspace wsv = ws;
+            wsv.dws = d64; wsv.ews = e64;
+            int rc = fast_tridiag_run<64, false>(blk, nullptr, wsv, 64, n, st, nullptr);
+            if (rc) return rc;
+            auto fq = mt == 96 ? mid_formq_split<96> : mid_formq_split<128>;
+            if ((ce = allow_smem(fq, smem)) != cudaSuccess) return (int)ce;
+            KLAUNCH("mid_formq_split", st, fq<<<n, MID_TPR * mt, smem, st>>>(V, ws, M, d64, e64));
+            return 0;
+        }
         auto kern = reg ? (mt == 96 ? mid_tridiag_formq_reg<96> : (mt == 128 ? mid_tridiag_formq_reg<128> : mid_tridiag_formq_reg<160>))
                         : (mt == 96 ? mid_tridiag_formq<96> : (mt == 128 ? mid_tridiag_formq<128> : mid_tridiag_formq<160>));
         if ((ce = allow_smem(kern, smem)) != cudaSuccess) return (int)ce;
@@ -1502,6 +1527,7 @@ int letkf_set_option(const char* name, int value)
     if (strcmp(name, "evec") == 0) { o.evec = value != 0; return LETKF_OK; }
     if (strcmp(name, "split") == 0) { o.split = value != 0; return LETKF_OK; }
     if (strcmp(name, "bigvec") == 0) { o.bigvec = value != 0; return LETKF_OK; }
+    if (strcmp(name, "mid_split") == 0) { o.mid_split = value != 0; return LETKF_OK; }
     if (strcmp(name, "pack") == 0) { if (value < 0 || value > 3) return -2; o.pack = value; return LETKF_OK; }
     if (strcmp(name, "pair") == 0) { o.pair = (value == 0 || value == 1) ? value : -1; return LETKF_OK; }
     if (strcmp(name, "bisect") == 0) { o.bisect = (value == 0 || value == 1) ? value : -1; return LETKF_OK; }

@@ -249,10 +249,19 @@ mid_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, int M
 //          block-uniform bounds, static register indices) into pd[h][j]
 //   B2  -> warps of h = 0: p_j = tau sum_h pd[h][j], the warp's share of p.v
 //   B3  -> a_jc -= v_j p_c + (p_j - tau (p.v) v_j) v_c
-template <int MT>
+// HEAD (64 < M <= 128, option mid_split): the kernel stops after pivot 64 and hands the trailing 64 x 64
+// block to the register kernels of fast_kernels.cuh (fast_tridiag<64> + fast_tridiag_tail: a pivot there
+// costs ~2400 cycles in 64 threads against ~3300 here in 4 ceil32(M)) -- 63 of the M - 1 pivots.  It leaves
+// the block as a dense 64 x 64 matrix in blk[b], (d_i, e_{i-1}) for i >= 64, and its reflectors (rows
+// 64 ... M-1 of S) and taus behind the RefLayout<64> record of ws.refl; mid_formq_split then gathers both
+// sets of reflectors and forms Q^T as before.
+__host__ __device__ inline int mid_split_fast_doubles() { return 32 * 8 * 9 + 64; }      // RefLayout<64>::TOTAL + 64 taus
+static inline int mid_split_refl_doubles(int M) { return mid_split_fast_doubles() + (M - 64 + 1) * mid_ld(M); }
+template <int MT, bool HEAD = false>
 __global__ void __launch_bounds__(MT * MID_TPR, MT == 96 ? 2 : 1)
 mid_tridiag_formq_reg(const double* __restrict__ A_, double* V_, Workspace ws, int M)
 {
+    double* blk = reinterpret_cast<double*>(ws.rot);      // HEAD: the trailing blocks [n][64][64], flat in the (still unused) log area
     extern __shared__ __align__(16) double sm[];
     static_assert(MID_TPR == 4, "column pairs are dealt to four threads per row");
     constexpr int NP = MT / 8;                   // column pairs per thread
@@ -295,7 +304,7 @@ mid_tridiag_formq_reg(const double* __restrict__ A_, double* V_, Workspace ws, i
             if (2 * h + 8 * k < LD) xs2[h + 4 * k] = a[k];
     };
     if (j == M - 1) dump_row();
-    for (int i = M - 1; i >= 1; --i) {
+    for (int i = M - 1; i >= (HEAD ? 64 : 1); --i) {
         __syncthreads();                                                     // B0
         if (h == 0) {
             double part = 0.0;
@@ -365,8 +374,60 @@ mid_tridiag_formq_reg(const double* __restrict__ A_, double* V_, Workspace ws, i
         }
         if (j == i - 1) dump_row();
     }
+    if constexpr (HEAD) {
+        if (tid == 0) ews[M - 1] = 0.0;
+        __syncthreads();                                                     // taus, reflector rows complete
+        if (j < 64) {                                                        // the trailing block, row j
+            double2* row2 = reinterpret_cast<double2*>(blk + b * 4096 + (size_t)j * 64);
+#pragma unroll
+            for (int k = 0; k < NP; ++k)
+                if (2 * h + 8 * k < 64) row2[h + 4 * k] = a[k];
+        }
+        double* out = ws.refl + b * ws.reflstride + mid_split_fast_doubles();
+        const int nrow = M - 64;
+        for (int idx = tid; idx < nrow * LD; idx += blockDim.x) out[idx] = S[(size_t)64 * LD + idx];
+        for (int c = tid; c < LD; c += blockDim.x) out[(size_t)nrow * LD + c] = (c >= 64 && c <= M - 1) ? taus[c] : 0.0;
+        return;
+    } else {
     if (tid == 0) { dws[0] = a[0].x; ews[M - 1] = 0.0; }
     __syncthreads();                                                         // taus, reflector rows complete
+    mid_formq_rows<MT, MT <= 128>(S, LD, taus, M, V_ + b * M * M);
+    }
+}
+
+// Q^T of the split reduction: the reflectors of pivots M-1 ... 64 (mid_tridiag_formq_reg<MT, true>) and of
+// pivots 63 ... 1 (fast_tridiag<64> / fast_tridiag_tail, RefLayout<64> order) meet in shared memory in the
+// layout mid_formq_rows expects (row i = v of H_i: v_c for c < i-1, 1 at i-1, 0 beyond); (d, e) of the
+// trailing block, which the register kernels left in d64 / e64 [n][64], go to their places in (dws, ews).
+template <int MT>
+__global__ void __launch_bounds__(MT * MID_TPR, MT == 96 ? 2 : 1)
+mid_formq_split(double* V_, Workspace ws, int M, const double* __restrict__ d64, const double* __restrict__ e64)
+{
+    extern __shared__ __align__(16) double sm[];
+    const int LD = mid_ld(M);
+    double* S    = sm;                           // [M][LD]
+    double* taus = sm + (size_t)M * LD + 2 * LD; // (same place as in the reduction kernel)
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const size_t b = blockIdx.x;
+    const double* rec = ws.refl + b * ws.reflstride;
+    const double* mid = rec + mid_split_fast_doubles();
+    const int nrow = M - 64;
+    for (int idx = tid; idx < nrow * LD; idx += nt) S[(size_t)64 * LD + idx] = mid[idx];
+    for (int c = tid; c < LD; c += nt) taus[c] = (c >= 64) ? mid[(size_t)nrow * LD + c] : ((c >= 1) ? rec[32 * 8 * 9 + c] : 0.0);
+    for (int idx = tid; idx < 64 * LD; idx += nt) {
+        const int i = idx / LD, c = idx - i * LD;                             // row i = reflector H_i, 1 <= i <= 63
+        double v = 0.0;
+        if (i >= 1) {
+            const int G = (i - 1) >> 3, k = (i - 1) & 7, len = 8 * (G + 1);
+            if (c < len) v = rec[32 * G * (G + 1) + k * len + c];
+        }
+        S[idx] = v;
+    }
+    if (tid < 64) {
+        ws.dws[b * M + tid] = d64[b * 64 + tid];
+        if (tid < 63) ws.ews[b * M + tid] = e64[b * 64 + tid];
+    }
+    __syncthreads();
     mid_formq_rows<MT, MT <= 128>(S, LD, taus, M, V_ + b * M * M);
 }
 

@@ -328,20 +328,24 @@ def test_hard_spectra(lk, oracle, M):
     parity.assert_evd(A, w, V, wo, f"hard spectra M={M}")
 
 
-@pytest.mark.parametrize("mode", [0, 2])
+@pytest.mark.parametrize("mode", [0, 2, 12])
 @pytest.mark.parametrize("M", [65, 71, 96, 97, 113, 128, 129, 145, 160])
 def test_mid_tridiagonalisation_both_forms(lk, oracle, M, mode):
     """64 < M <= 160 (mid_kernels.cuh): the reduction with the matrix in shared memory
     (mid_reg = 0) and in registers (mid_reg = 2) at every size class (MT = 96 / 128 / 160), ragged
-    orders included; the default picks one of the two by size.  Low-rank inputs (p = 3 < M - 1)
+    orders included; the default picks one of the two by size.  Up to M = 128 the register form hands
+    its trailing 64 x 64 block to the kernels of the M <= 64 path (mid_split = 1, default; mode 12 here
+    is mid_reg = 2 with mid_split = 0: one kernel down to pivot 1).  Low-rank inputs (p = 3 < M - 1)
     exercise the tau = 0 pivots (reading G19) and the eigenvalue cluster."""
     A = np.concatenate([wl.letkf_shaped(9, M, 98, config_index=960 + M),
                         wl.letkf_shaped(4, M, 3, config_index=961 + M)])
     try:
-        lk.set_option("mid_reg", mode)
+        lk.set_option("mid_reg", mode % 10)
+        lk.set_option("mid_split", 0 if mode >= 10 else 1)
         w, V, info = run_gpu(lk, A)
     finally:
         lk.set_option("mid_reg", 1)
+        lk.set_option("mid_split", 1)
     assert (info == 0).all()
     wo, _, _, _ = oracle.syev_batched(A)
     parity.assert_evd(A, w, V, wo, f"mid M={M} mid_reg={mode}")
