@@ -295,6 +295,8 @@ int letkf_last_launch_count(void);
  *   "pair"          32 < M <= 64: the reduction kernel takes two matrices per CTA: 0 / 1 (-1 = for 32 < M <= 48)
  *   "split"         48 < M <= 64: the reduction as two kernels, pivots M-1 ... 33 by two warps and the trailing
  *                   32 x 32 problem by one warp per matrix (default 1; 0 = one kernel)
+ *   "mid_split"     64 < M <= 128: the reduction stops after pivot 64 and its trailing 64 x 64 block goes through the
+ *                   register kernels of the M <= 64 path (1, default; 0 = one kernel down to pivot 1)
  *   "mid_reg"       64 < M <= 160: reduction with the matrix in shared memory (0) / in registers up to M = 128 (1,
  *                   default) / in registers (2)
  *   "host_pass"     matrices per pass of the host entry points (0 = what a 16 GiB staging arena holds)
