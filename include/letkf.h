@@ -86,7 +86,7 @@ size_t letkf_syev_workspace_bytes(int M, int batch);
  * results are those of letkf_syev_batched at the same batch size.
  *
  *   batch   must fit the array: batch <= letkf_syev_static_max_batch(M) (paper's latency case, 256
- *           matrices of M = 64, fits; M = 64: 363, M = 32: 1297, M = 16: 4123, M = 128: 62), else
+ *           matrices of M = 64, fits; M = 64: 363, M = 32: 1297, M = 16: 4123, M = 128: 92, M = 256: 31), else
  *           the call returns LETKF_ERR_STATIC_CAPACITY and launches nothing.
  *   Every call on a device shares the one array: two calls whose kernels overlap on the GPU (different
  *   streams, or different host threads) RACE on it -- keep all calls of a device on one stream or order
