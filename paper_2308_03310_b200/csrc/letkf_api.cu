@@ -187,6 +187,13 @@ static const int PIPE_MAX_SUBS = 16;     // sub-chunks per call (bounds the laun
 static const int PIPE_SLOTS = 16;        // default number of sub-chunks in flight: all of them
 static const size_t PIPE_LOG_BYTES = (size_t)256 << 20;   // default size of the log slots together
 static const int NQ_STREAMS = 16;
+#ifndef LETKF_NT_STREAMS
+#define LETKF_NT_STREAMS 4
+#endif
+#ifndef LETKF_NA_STREAMS
+#define LETKF_NA_STREAMS 4
+#endif
+static const int NT_STREAMS = LETKF_NT_STREAMS, NA_STREAMS = LETKF_NA_STREAMS;
 
 static int round_up(int x, int a) { return (x + a - 1) / a * a; }
 
@@ -533,7 +540,7 @@ static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws,
 // from and joined back into the caller's stream with events: the caller sees plain stream order.
 struct Pipe {
     int dev = -1;
-    cudaStream_t sT[2] = {nullptr, nullptr}, sA[4] = {};
+    cudaStream_t sT[NT_STREAMS] = {}, sA[NA_STREAMS] = {};
     cudaStream_t sQ[NQ_STREAMS] = {};
     std::vector<cudaEvent_t> ev;
     size_t used = 0;
@@ -561,9 +568,9 @@ struct Pipe {
         int least = 0, greatest = 0;
         cudaDeviceGetStreamPriorityRange(&least, &greatest);
         const int mid = (greatest < least) ? greatest + 1 : greatest;
-        for (int k = 0; k < 2; ++k)
+        for (int k = 0; k < NT_STREAMS; ++k)
             if ((ce = cudaStreamCreateWithPriority(&sT[k], cudaStreamNonBlocking, mid)) != cudaSuccess) return (int)ce;
-        for (int k = 0; k < 4; ++k)
+        for (int k = 0; k < NA_STREAMS; ++k)
             if ((ce = cudaStreamCreateWithPriority(&sA[k], cudaStreamNonBlocking, least)) != cudaSuccess) return (int)ce;
         for (int k = 0; k < NQ_STREAMS; ++k)
             if ((ce = cudaStreamCreateWithPriority(&sQ[k], cudaStreamNonBlocking, greatest)) != cudaSuccess) return (int)ce;
@@ -623,19 +630,19 @@ static int run_pipeline(const Plan& pl, int batch, cudaStream_t st, FT stageT, F
     // stream-ordered free of an owned workspace) never runs ahead of work still in flight
     auto join_all = [&]() {
         int jr = 0, r2;
-        for (int k = 0; k < 2; ++k) if ((r2 = P.link(P.sT[k], st)) && !jr) jr = r2;
-        for (int k = 0; k < 4; ++k) if ((r2 = P.link(P.sA[k], st)) && !jr) jr = r2;
+        for (int k = 0; k < NT_STREAMS; ++k) if ((r2 = P.link(P.sT[k], st)) && !jr) jr = r2;
+        for (int k = 0; k < NA_STREAMS; ++k) if ((r2 = P.link(P.sA[k], st)) && !jr) jr = r2;
         for (int k = 0; k < NQ_STREAMS; ++k) if ((r2 = P.link(P.sQ[k], st)) && !jr) jr = r2;
         return jr;
     };
-    for (int k = 0; k < 2 && !rc; ++k) rc = P.link(st, P.sT[k]);
-    for (int k = 0; k < 4 && !rc; ++k) rc = P.link(st, P.sA[k]);
+    for (int k = 0; k < NT_STREAMS && !rc; ++k) rc = P.link(st, P.sT[k]);
+    for (int k = 0; k < NA_STREAMS && !rc; ++k) rc = P.link(st, P.sA[k]);
     for (int k = 0; k < NQ_STREAMS && !rc; ++k) rc = P.link(st, P.sQ[k]);
     std::vector<cudaEvent_t> done((size_t)pl.nsub, nullptr);
     for (int k = 0, b0 = 0; b0 < batch && !rc; ++k, b0 += pl.per) {
         const int nk = (batch - b0 < pl.per) ? batch - b0 : pl.per;
         const int s0 = (k % pl.nslot) * pl.per, l0 = (k % pl.nlog) * pl.per;
-        cudaStream_t sT = P.sT[k & 1], sQ = P.sQ[k % NQ_STREAMS], sA = P.sA[k & 3];
+        cudaStream_t sT = P.sT[k % NT_STREAMS], sQ = P.sQ[k % NQ_STREAMS], sA = P.sA[k % NA_STREAMS];
         if (k >= pl.nslot) {                       // the slot is free when its previous tenant's last kernel is done
             cudaError_t ce = cudaStreamWaitEvent(sT, done[k - pl.nslot], 0);
             if (ce != cudaSuccess) { rc = (int)ce; break; }
