@@ -840,6 +840,32 @@ __device__ __forceinline__ void cp_async_wait_all()
     asm volatile("cp.async.wait_all;" ::: "memory");
 }
 
+// ---- one contiguous record global -> shared by the TMA unit (cp.async.bulk, SASS UBLKCP): one thread arms an
+// mbarrier with the byte count and issues the copy, no thread spends an instruction per 16 bytes; whoever needs the
+// data waits for the barrier's phase.  Addresses and size are multiples of 16 bytes.
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count)
+{
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(a), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_load(void* smem_dst, const void* gmem_src, unsigned bytes, unsigned long long* bar)
+{
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar), d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(a), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(d), "l"(gmem_src), "r"(bytes), "r"(a) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity)
+{
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+    unsigned ok;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    } while (!ok);
+}
+
 // Rotations i = m-1 ... lo on columns (i, i+1):  f = z[i+1]; z[i+1] = s z[i] + c f; z[i] = c z[i] - s f.
 // Blocks of 4 rotations, entered at the block of m-1 and left after the block of lo; cs[] holds
 // the identity (1, 0) outside [lo, m), so the overhang at both ends changes nothing.  The only
@@ -1175,10 +1201,13 @@ fast_apply(double* __restrict__ V_, double* __restrict__ w_, int* __restrict__ i
     for (int s = r; s < nsw; s += C::NT) hdr[s] = ws.hdr[b * ws.swcap + s];
     if (!flagged && r < M) inv[ws.perm[b * M + r]] = r;    // output column of QL-order column c
     double z[MT];
+    __shared__ unsigned long long refl_bar;
     if constexpr (!QFORM) {
-        // the reflectors fly in while the eigenvectors of T are formed
-        const double* src = ws.refl + b * ws.reflstride;
-        for (int k = 2 * r; k < refl_doubles<MT>(); k += 2 * C::NT) cp_async16(R + k, src + k);
+        // the reflectors fly in while the eigenvectors of T are formed: one bulk copy of the record by the TMA unit
+        if (r == 0) {
+            mbar_init(&refl_bar, 1);
+            bulk_load(R, ws.refl + b * ws.reflstride, (unsigned)(sizeof(double) * refl_doubles<MT>()), &refl_bar);
+        }
     }
     bool columns = false;                          // z holds a column of Z (an eigenvector of T) rather than a row
 
@@ -1297,6 +1326,7 @@ fast_apply(double* __restrict__ V_, double* __restrict__ w_, int* __restrict__ i
     if constexpr (!QFORM) {
         // rows of Z -> eigenvectors of T: thread k holds column k (QL order); then V = H_{M-1} ... H_1 Z
         if (!columns) transpose_regs<MT>(z, areg);
+        mbar_wait(&refl_bar, 0);                   // (every path here has passed a block barrier since the copy was issued)
         q_groups_up<MT, 0, (MT - 2) / 8>(z, R, taus, M, 0);
     }
 
