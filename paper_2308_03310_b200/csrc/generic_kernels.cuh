@@ -16,18 +16,72 @@ namespace letkf {
 constexpr int GEN_NT = 256;
 constexpr int GEN_QK = 8;      // reflectors applied per pass over the rows when Q is formed
 
+// One chunk of the reduction's pass: rows j0 ... j0+7, columns c = 32 k + lane, Sc = &S[j0][c].  x <- x - v_j w_c - w_j v_c
+// (vw[.] = (v, w) of the pending pivot), then q[r] += x v_c (row sums, reduced over the lanes by the caller) and
+// acc += x v_j for c < j (this lane's column sum).  _full: every (j, c) of the chunk is strictly below the diagonal and
+// above the pivot row -- no mask anywhere; _masked: the diagonal segment, the ragged last chunk, and the passes with
+// only one of the two operations (H = I, reading G19).
+__device__ __forceinline__ void gen_segment_full(double* __restrict__ Sc, int M, int j0, int c, const double2* __restrict__ vw,
+                                                 const double* __restrict__ vN, double (&q)[8], double& acc)
+{
+    double x[8];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) x[r] = Sc[(size_t)r * M];
+    const double2 t = vw[c];
+    const double vc = vN[c];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const double2 vwj = vw[j0 + r];
+        const double vj = vN[j0 + r];
+        const double xn = fma(-vwj.x, t.y, fma(-vwj.y, t.x, x[r]));
+        Sc[(size_t)r * M] = xn;
+        q[r] = fma(xn, vc, q[r]);
+        acc = fma(xn, vj, acc);
+    }
+}
+__device__ __forceinline__ void gen_segment_masked(double* __restrict__ Sc, int M, int j0, int c, int i, bool upd, bool mv,
+                                                   const double2* __restrict__ vw, const double* __restrict__ vN,
+                                                   double (&q)[8], double& acc)
+{
+    double x[8];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) x[r] = (c <= j0 + r && j0 + r < i) ? Sc[(size_t)r * M] : 0.0;
+    const int cc = min(c, M - 1);
+    if (upd) {
+        const double2 t = vw[cc];
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            const int j = j0 + r;
+            const double2 vwj = vw[min(j, M - 1)];
+            const double xn = fma(-vwj.x, t.y, fma(-vwj.y, t.x, x[r]));
+            const bool m = c <= j && j < i;
+            if (m) Sc[(size_t)r * M] = xn;
+            x[r] = m ? xn : 0.0;
+        }
+    }
+    if (mv) {
+        const double vc = (c < i) ? vN[cc] : 0.0;
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            const int j = j0 + r;
+            const double vj = vN[min(j, M - 1)];
+            q[r] = fma(x[r], vc, q[r]);
+            acc += (c < j && j < i) ? x[r] * vj : 0.0;
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // a3 + explicit Q.  Reduction order is "from the last row up" (pivot i = M-1 ... 1, reflector
 // H_i acts on indices 0..i-1), so Q = H_{M-1} ... H_1 and T = Q^T A Q.
 // A: [batch][M][M] (lower triangle read).  V: [batch][M][M] receives Q^T.  May alias.
-__global__ void __launch_bounds__(GEN_NT)
+// (the reduction at 128 registers, two CTAs per SM: at 80 it spills and measured slower, M = 256: 13.5 against 10.4 ms)
+template <int phase>
+__global__ void __launch_bounds__(GEN_NT, 2)
 generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, int M)
 {
     extern __shared__ double sm[];
-    double* v    = sm;            // [M]
-    double* wv   = sm + M;        // [M]
-    double* pv   = sm + 2 * M;    // [M]
-    double* taus = sm + 3 * M;    // [M]
+    double* taus = sm + 3 * M;    // [M]   (sm ... sm + 3 M: (v, w) pairs and v of the reduction, below)
     double* red  = sm + 4 * M;    // [GEN_NT/32]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = GEN_NT / 32;
@@ -37,27 +91,36 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
     double* dws = ws.dws + b * M;
     double* ews = ws.ews + b * M;
 
-    // full symmetric copy of the lower triangle
+    // phase: bit 0 = the reduction, bit 1 = the formation of Q^T.  The reduction leaves tau_i in S[i][i] (free from pivot
+    // i until Q^T is formed), so the second phase can also follow a reduction done elsewhere (resident_kernels.cuh).
+    if (!(phase & 1)) {
+        for (int i = 1 + tid; i < M; i += GEN_NT) taus[i] = S[(size_t)i * M + i];
+        __syncthreads();
+    }
+    if (phase & 1) {
+    // copy of the lower triangle (the upper one is never read: symmetric half only, below)
     for (int r = warp; r < M; r += NW)
-        for (int c = lane; c < M; c += 32) {
-            const double val = (r >= c) ? A[(size_t)r * M + c] : A[(size_t)c * M + r];
-            S[(size_t)r * M + c] = val;
-        }
+        for (int c = lane; c <= r; c += 32) S[(size_t)r * M + c] = A[(size_t)r * M + c];
     __syncthreads();
 
     // Pivots i = M-1 ... 1.  The rank-2 update of pivot i+1 and the mat-vec of pivot i share ONE
-    // pass over the rows (the kernel is at the HBM roof for M > 160: a row is read and written once
-    // per pivot instead of read twice and written once): row i is updated first, pivot i's reflector
-    // is formed from it, then every row j < i is updated in registers and dotted with the new v.
-    double* vbuf[2] = {v, red + NW};                 // v of the pending and of the new pivot (vk is free here)
+    // pass over the matrix, and the pass touches the LOWER TRIANGLE only (c <= j of row j is read and
+    // written once per pivot): row i is updated first, pivot i's reflector is formed from it, then
+    // the rows j < i go through registers in chunks of eight rows by 32 columns (lane = column, eight
+    // independent loads in flight).  S[j][c] enters p_j with v_c and, for c < j, p_c with v_j: the
+    // second sum accumulates per lane over all the chunks of the warp (summed over the warps through
+    // pT when p is assembled); the eight row sums of a chunk are reduced together by a halving
+    // butterfly (9 shuffles for 8 rows instead of 40) once all its column segments are in.
+    double2* vw = reinterpret_cast<double2*>(sm);    // [M] (v_c, w_c) of the pending pivot i+1 (length i+1)
+    double* vN = sm + 2 * M;                         // [M] v of the new pivot
+    double* pv = red + NW;                           // [M] row sums, then p (row 0 of the vk area, free here)
+    double* pT = red + NW + M;                       // [NW][M] column sums per warp (rows 1 ... NW of the vk area)
     double tauP = 0.0;                               // tau of the pending update (0: none)
     for (int i = M - 1; i >= 1; --i) {
         double* rowi = S + (size_t)i * M;
-        const double* vP = vbuf[(i + 1) & 1];        // v, w of pivot i+1 (length i+1)
-        double* vN = vbuf[i & 1];
         if (tauP != 0.0) {                           // row i: S[i][c] -= v_i w_c + w_i v_c, c <= i
-            const double vi = vP[i], wi = wv[i];
-            for (int c = tid; c <= i; c += GEN_NT) rowi[c] -= vi * wv[c] + wi * vP[c];
+            const double2 vwi = vw[i];
+            for (int c = tid; c <= i; c += GEN_NT) { const double2 t = vw[c]; rowi[c] -= vwi.x * t.y + vwi.y * t.x; }
             __syncthreads();
         }
         double part = 0.0;
@@ -72,45 +135,83 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
             scal = 1.0 / (alpha - beta);
         }
         for (int c = tid; c < i; c += GEN_NT) vN[c] = (c == i - 1) ? 1.0 : rowi[c] * scal;
-        if (tid == 0) { ews[i - 1] = beta; dws[i] = rowi[i]; taus[i] = tau; }
+        if (tid == 0) { ews[i - 1] = beta; dws[i] = rowi[i]; taus[i] = tau; rowi[i] = tau; }
         __syncthreads();
         for (int c = tid; c < i; c += GEN_NT) rowi[c] = vN[c];           // keep the reflector
         if (tauP != 0.0 || tau != 0.0) {
-            for (int j = warp; j < i; j += NW) {
-                double* rj = S + (size_t)j * M;
-                double x[8];
+            double accT[8];
 #pragma unroll
-                for (int k = 0; k < 8; ++k) { const int c = lane + 32 * k; x[k] = (c < i) ? rj[c] : 0.0; }
-                if (tauP != 0.0) {                                        // S11 -= v w^T + w v^T (pivot i+1)
-                    const double vj = vP[j], wj = wv[j];
+            for (int k = 0; k < 8; ++k) accT[k] = 0.0;
+            const bool both = tauP != 0.0 && tau != 0.0;
+            const int nch = (i + 7) >> 3;
+            // chunks in pairs (ch, nch-1-ch): a long and a short one, so that the warps finish together
+            for (int pp = warp; 2 * pp < nch; pp += NW) {
+#pragma unroll 1
+                for (int half = 0; half < 2; ++half) {
+                    const int ch = half ? nch - 1 - pp : pp;
+                    if (half && ch == pp) break;
+                    const int j0 = ch * 8;
+                    const int nseg = (min(j0 + 7, i - 1) >> 5) + 1;       // column segments with some c <= j < i
+                    const int nfull = (both && j0 + 8 <= i) ? (j0 >> 5) : 0;   // of which without a mask: 32 k + 32 <= j0
+                    double q[8];
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) q[r] = 0.0;
+                    double* Sc = S + (size_t)j0 * M + lane;
 #pragma unroll
                     for (int k = 0; k < 8; ++k) {
-                        const int c = lane + 32 * k;
-                        if (c < i) { x[k] -= vj * wv[c] + wj * vP[c]; rj[c] = x[k]; }
+                        if (k < nfull) gen_segment_full(Sc + 32 * k, M, j0, lane + 32 * k, vw, vN, q, accT[k]);
+                        else if (k < nseg) gen_segment_masked(Sc + 32 * k, M, j0, lane + 32 * k, i, tauP != 0.0, tau != 0.0, vw, vN, q, accT[k]);
+                    }
+                    if (tau != 0.0) {                                     // eight row sums over 32 lanes: lane l ends with row l / 4
+                        double a4[4], b2[2];
+#pragma unroll
+                        for (int t = 0; t < 4; ++t) {
+                            const bool hi = lane & 16;
+                            const double keep = hi ? q[t + 4] : q[t], send = hi ? q[t] : q[t + 4];
+                            a4[t] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+                        }
+#pragma unroll
+                        for (int t = 0; t < 2; ++t) {
+                            const bool hi = lane & 8;
+                            const double keep = hi ? a4[t + 2] : a4[t], send = hi ? a4[t] : a4[t + 2];
+                            b2[t] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+                        }
+                        const bool hi = lane & 4;
+                        double s1 = (hi ? b2[1] : b2[0]) + __shfl_xor_sync(0xffffffffu, hi ? b2[0] : b2[1], 4);
+                        s1 += __shfl_xor_sync(0xffffffffu, s1, 2);
+                        s1 += __shfl_xor_sync(0xffffffffu, s1, 1);
+                        const int j = j0 + (lane >> 2);
+                        if ((lane & 3) == 0 && j < i) pv[j] = s1;
                     }
                 }
-                if (tau != 0.0) {                                         // p = tau * S11 v (pivot i)
-                    double acc = 0.0;
+            }
+            if (tau != 0.0) {
 #pragma unroll
-                    for (int k = 0; k < 8; ++k) { const int c = lane + 32 * k; if (c < i) acc += x[k] * vN[c]; }
-                    acc = warp_sum(acc);
-                    if (lane == 0) pv[j] = tau * acc;
-                }
+                for (int k = 0; k < 8; ++k) { const int c = lane + 32 * k; if (c < i) pT[warp * M + c] = accT[k]; }
             }
         }
         __syncthreads();
         if (tau != 0.0) {
             part = 0.0;
-            for (int c = tid; c < i; c += GEN_NT) part += pv[c] * vN[c];
+            for (int c = tid; c < i; c += GEN_NT) {
+                double pc = pv[c];
+#pragma unroll
+                for (int w8 = 0; w8 < NW; ++w8) pc += pT[w8 * M + c];
+                pc *= tau;
+                pv[c] = pc;
+                part += pc * vN[c];
+            }
             const double K = 0.5 * tau * block_sum<GEN_NT>(part, red);
-            for (int c = tid; c < i; c += GEN_NT) wv[c] = pv[c] - K * vN[c];
+            for (int c = tid; c < i; c += GEN_NT) { const double vc = vN[c]; vw[c] = make_double2(vc, pv[c] - K * vc); }
         }
         tauP = tau;
         __syncthreads();
     }
-    if (tauP != 0.0 && tid == 0) S[0] -= 2.0 * vbuf[1][0] * wv[0];       // pending update of pivot 1 (tau_1 = 0 in fact)
+    if (tauP != 0.0 && tid == 0) S[0] -= 2.0 * vw[0].x * vw[0].y;        // pending update of pivot 1 (tau_1 = 0 in fact)
     __syncthreads();
     if (tid == 0) { dws[0] = S[0]; ews[M - 1] = 0.0; }
+    }
+    if (!(phase & 2)) return;
 
     // Q^T = H_1 H_2 ... H_{M-1}, grown in place: B_i = diag(B_{i-1}, 1) H_i on the leading i x i.
     // The kernel runs at the HBM roof for M > 160 (the resident matrices exceed L2), so GEN_QK
@@ -118,7 +219,7 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
     // steps, held in registers in between (<= 8 doubles per lane).  The rows and columns the later
     // reflectors of a group add are set to identity first and every reflector is zero-padded to the
     // group's width, so H_i leaves the rows >= i alone exactly as the one-at-a-time loop does.
-    double* vk = red + NW;        // [GEN_QK][M]
+    double* vk = red + NW;        // [GEN_QK][M] (one more row behind it belongs to pT above)
     for (int i0 = 1; i0 <= M - 1; i0 += GEN_QK) {
         const int kk = min(GEN_QK, M - i0);          // reflectors i0 ... i0+kk-1
         const int nc = i0 + kk - 1;                  // rows and columns of the pass
@@ -134,24 +235,53 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
             if (tid == 0) S[(size_t)idx * M + idx] = 1.0;
         }
         __syncthreads();
-        for (int r = warp; r < nc; r += NW) {
-            double* br = S + (size_t)r * M;
-            double x[8];
+        // four rows per warp and pass: every reflector entry read from shared memory serves four rows (the loop is bound
+        // by shared-memory bandwidth at one row), and the four dot products are reduced together
+        const int nseg = (nc + 31) >> 5;
+        for (int r0 = 4 * warp; r0 < nc; r0 += 4 * NW) {
+            double x[4][8];
 #pragma unroll
-            for (int k = 0; k < 8; ++k) { const int c = lane + 32 * k; x[k] = (c < nc) ? br[c] : 0.0; }
+            for (int rr = 0; rr < 4; ++rr)
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const int c = lane + 32 * k;
+                    x[rr][k] = (k < nseg && c < nc && r0 + rr < nc) ? S[(size_t)(r0 + rr) * M + c] : 0.0;
+                }
             for (int t = 0; t < kk; ++t) {
                 const double tau = taus[i0 + t];
                 if (tau == 0.0) continue;
                 const double* vt = vk + t * M;
-                double acc = 0.0;
+                double v[8], a[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
-                for (int k = 0; k < 8; ++k) { const int c = lane + 32 * k; if (c < nc) acc += x[k] * vt[c]; }
-                acc = warp_sum(acc) * tau;
+                for (int k = 0; k < 8; ++k) {
+                    const int c = lane + 32 * k;
+                    v[k] = (k < nseg && c < nc) ? vt[c] : 0.0;
 #pragma unroll
-                for (int k = 0; k < 8; ++k) { const int c = lane + 32 * k; if (c < nc) x[k] -= acc * vt[c]; }
+                    for (int rr = 0; rr < 4; ++rr) a[rr] = fma(x[rr][k], v[k], a[rr]);
+                }
+                // four sums over 32 lanes: halving butterfly (lane l ends with sum l / 8), then gathered by all lanes
+                const bool h16 = lane & 16, h8 = lane & 8;
+                const double b0 = (h16 ? a[2] : a[0]) + __shfl_xor_sync(0xffffffffu, h16 ? a[0] : a[2], 16);
+                const double b1 = (h16 ? a[3] : a[1]) + __shfl_xor_sync(0xffffffffu, h16 ? a[1] : a[3], 16);
+                double s1 = (h8 ? b1 : b0) + __shfl_xor_sync(0xffffffffu, h8 ? b0 : b1, 8);
+                s1 += __shfl_xor_sync(0xffffffffu, s1, 4);
+                s1 += __shfl_xor_sync(0xffffffffu, s1, 2);
+                s1 += __shfl_xor_sync(0xffffffffu, s1, 1);
+                s1 *= tau;
+#pragma unroll
+                for (int rr = 0; rr < 4; ++rr) {
+                    const double ar = __shfl_sync(0xffffffffu, s1, 8 * rr);
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) x[rr][k] = fma(-ar, v[k], x[rr][k]);
+                }
             }
 #pragma unroll
-            for (int k = 0; k < 8; ++k) { const int c = lane + 32 * k; if (c < nc) br[c] = x[k]; }
+            for (int rr = 0; rr < 4; ++rr)
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const int c = lane + 32 * k;
+                    if (k < nseg && c < nc && r0 + rr < nc) S[(size_t)(r0 + rr) * M + c] = x[rr][k];
+                }
         }
         __syncthreads();
     }
