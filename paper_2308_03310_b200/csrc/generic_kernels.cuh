@@ -16,19 +16,28 @@ namespace letkf {
 constexpr int GEN_NT = 256;
 constexpr int GEN_QK = 8;      // reflectors applied per pass over the rows when Q is formed
 
-// One chunk of the reduction's pass: rows j0 ... j0+7, columns c = 32 k + lane, Sc = &S[j0][c].  x <- x - v_j w_c - w_j v_c
-// (vw[.] = (v, w) of the pending pivot), then q[r] += x v_c (row sums, reduced over the lanes by the caller) and
-// acc += x v_j for c < j (this lane's column sum).  _full: every (j, c) of the chunk is strictly below the diagonal and
-// above the pivot row -- no mask anywhere; _masked: the diagonal segment, the ragged last chunk, and the passes with
-// only one of the two operations (H = I, reading G19).
-__device__ __forceinline__ void gen_segment_full(double* __restrict__ Sc, int M, int j0, int c, const double2* __restrict__ vw,
-                                                 const double* __restrict__ vN, double (&q)[8], double& acc)
+// One segment of the reduction's pass: rows j0 ... j0+7, columns c = 32 k + lane, Sc = &S[j0][c], in two steps so that
+// the loads of the next segment are in flight while this one is worked on.  x <- x - v_j w_c - w_j v_c (vw[.] = (v, w) of
+// the pending pivot), then q[r] += x v_c (row sums, reduced over the lanes by the caller) and acc += x v_j for c < j
+// (this lane's column sum).  _full: every (j, c) of the segment is strictly below the diagonal and above the pivot row --
+// no mask anywhere; _masked: the diagonal segment, the ragged last chunk, and the passes with only one of the two
+// operations (H = I, reading G19).
+__device__ __forceinline__ void gen_load_full(const double* __restrict__ Sc, int M, double (&x)[8])
 {
-    double x[8];
 #pragma unroll
     for (int r = 0; r < 8; ++r) x[r] = Sc[(size_t)r * M];
+}
+__device__ __forceinline__ void gen_load_masked(const double* __restrict__ Sc, int M, int j0, int c, int i, double (&x)[8])
+{
+#pragma unroll
+    for (int r = 0; r < 8; ++r) x[r] = (c <= j0 + r && j0 + r < i) ? Sc[(size_t)r * M] : 0.0;
+}
+__device__ __forceinline__ double gen_segment_full(double* __restrict__ Sc, int M, int j0, int c, const double2* __restrict__ vw,
+                                                   const double* __restrict__ vN, const double (&x)[8], double (&q)[8])
+{
     const double2 t = vw[c];
     const double vc = vN[c];
+    double acc = 0.0;
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
         const double2 vwj = vw[j0 + r];
@@ -38,14 +47,15 @@ __device__ __forceinline__ void gen_segment_full(double* __restrict__ Sc, int M,
         q[r] = fma(xn, vc, q[r]);
         acc = fma(xn, vj, acc);
     }
+    return acc;
 }
-__device__ __forceinline__ void gen_segment_masked(double* __restrict__ Sc, int M, int j0, int c, int i, bool upd, bool mv,
-                                                   const double2* __restrict__ vw, const double* __restrict__ vN,
-                                                   double (&q)[8], double& acc)
+__device__ __forceinline__ double gen_segment_masked(double* __restrict__ Sc, int M, int j0, int c, int i, bool upd, bool mv,
+                                                     const double2* __restrict__ vw, const double* __restrict__ vN,
+                                                     const double (&x)[8], double (&q)[8])
 {
-    double x[8];
+    double y[8];
 #pragma unroll
-    for (int r = 0; r < 8; ++r) x[r] = (c <= j0 + r && j0 + r < i) ? Sc[(size_t)r * M] : 0.0;
+    for (int r = 0; r < 8; ++r) y[r] = x[r];
     const int cc = min(c, M - 1);
     if (upd) {
         const double2 t = vw[cc];
@@ -53,22 +63,24 @@ __device__ __forceinline__ void gen_segment_masked(double* __restrict__ Sc, int 
         for (int r = 0; r < 8; ++r) {
             const int j = j0 + r;
             const double2 vwj = vw[min(j, M - 1)];
-            const double xn = fma(-vwj.x, t.y, fma(-vwj.y, t.x, x[r]));
+            const double xn = fma(-vwj.x, t.y, fma(-vwj.y, t.x, y[r]));
             const bool m = c <= j && j < i;
             if (m) Sc[(size_t)r * M] = xn;
-            x[r] = m ? xn : 0.0;
+            y[r] = m ? xn : 0.0;
         }
     }
+    double acc = 0.0;
     if (mv) {
         const double vc = (c < i) ? vN[cc] : 0.0;
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
             const int j = j0 + r;
             const double vj = vN[min(j, M - 1)];
-            q[r] = fma(x[r], vc, q[r]);
-            acc += (c < j && j < i) ? x[r] * vj : 0.0;
+            q[r] = fma(y[r], vc, q[r]);
+            acc += (c < j && j < i) ? y[r] * vj : 0.0;
         }
     }
+    return acc;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -139,62 +151,78 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
         __syncthreads();
         for (int c = tid; c < i; c += GEN_NT) rowi[c] = vN[c];           // keep the reflector
         if (tauP != 0.0 || tau != 0.0) {
-            double accT[8];
-#pragma unroll
-            for (int k = 0; k < 8; ++k) accT[k] = 0.0;
             const bool both = tauP != 0.0 && tau != 0.0;
             const int nch = (i + 7) >> 3;
-            // chunks in pairs (ch, nch-1-ch): a long and a short one, so that the warps finish together
-            for (int pp = warp; 2 * pp < nch; pp += NW) {
-#pragma unroll 1
-                for (int half = 0; half < 2; ++half) {
-                    const int ch = half ? nch - 1 - pp : pp;
-                    if (half && ch == pp) break;
-                    const int j0 = ch * 8;
-                    const int nseg = (min(j0 + 7, i - 1) >> 5) + 1;       // column segments with some c <= j < i
-                    const int nfull = (both && j0 + 8 <= i) ? (j0 >> 5) : 0;   // of which without a mask: 32 k + 32 <= j0
-                    double q[8];
+            double* pTw = pT + warp * M;                                  // this warp's share of p: row and column sums alike
+            for (int c = lane; c < i; c += 32) pTw[c] = 0.0;
+            __syncwarp();
+            // Work items: (chunk ch of eight rows, column segment k) with 32 k <= 8 ch + 7, segment by segment (k = 0: every
+            // chunk, k = 1: chunks 4 ..., ...), dealt to the warps round robin -- items of one size, so the warps finish
+            // together (whole chunks left a third of the warp time waiting at the barrier).  The loads of a warp's next
+            // item are in flight while it works on the current one.
+            int nitems = 0;
+            for (int k = 0; 4 * k < nch; ++k) nitems += nch - 4 * k;
+            auto decode = [&](int t, int& ch, int& k) { k = 0; while (t >= nch - 4 * k) { t -= nch - 4 * k; ++k; } ch = 4 * k + t; };
+            auto is_full = [&](int ch, int k) { return both && 8 * ch + 8 <= i && 32 * k + 32 <= 8 * ch; };
+            int t = warp, ch = 0, k = 0;
+            double xc[8], xn[8];
 #pragma unroll
-                    for (int r = 0; r < 8; ++r) q[r] = 0.0;
-                    double* Sc = S + (size_t)j0 * M + lane;
-#pragma unroll
-                    for (int k = 0; k < 8; ++k) {
-                        if (k < nfull) gen_segment_full(Sc + 32 * k, M, j0, lane + 32 * k, vw, vN, q, accT[k]);
-                        else if (k < nseg) gen_segment_masked(Sc + 32 * k, M, j0, lane + 32 * k, i, tauP != 0.0, tau != 0.0, vw, vN, q, accT[k]);
-                    }
-                    if (tau != 0.0) {                                     // eight row sums over 32 lanes: lane l ends with row l / 4
-                        double a4[4], b2[2];
-#pragma unroll
-                        for (int t = 0; t < 4; ++t) {
-                            const bool hi = lane & 16;
-                            const double keep = hi ? q[t + 4] : q[t], send = hi ? q[t] : q[t + 4];
-                            a4[t] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-                        }
-#pragma unroll
-                        for (int t = 0; t < 2; ++t) {
-                            const bool hi = lane & 8;
-                            const double keep = hi ? a4[t + 2] : a4[t], send = hi ? a4[t] : a4[t + 2];
-                            b2[t] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-                        }
-                        const bool hi = lane & 4;
-                        double s1 = (hi ? b2[1] : b2[0]) + __shfl_xor_sync(0xffffffffu, hi ? b2[0] : b2[1], 4);
-                        s1 += __shfl_xor_sync(0xffffffffu, s1, 2);
-                        s1 += __shfl_xor_sync(0xffffffffu, s1, 1);
-                        const int j = j0 + (lane >> 2);
-                        if ((lane & 3) == 0 && j < i) pv[j] = s1;
-                    }
-                }
+            for (int r = 0; r < 8; ++r) xn[r] = 0.0;
+            if (t < nitems) {
+                decode(t, ch, k);
+                const double* Sc = S + (size_t)(8 * ch) * M + 32 * k + lane;
+                if (is_full(ch, k)) gen_load_full(Sc, M, xc); else gen_load_masked(Sc, M, 8 * ch, 32 * k + lane, i, xc);
             }
-            if (tau != 0.0) {
+#pragma unroll 1
+            while (t < nitems) {
+                const int tn = t + NW;
+                int chn = 0, kn = 0;
+                if (tn < nitems) {
+                    decode(tn, chn, kn);
+                    const double* Sn = S + (size_t)(8 * chn) * M + 32 * kn + lane;
+                    if (is_full(chn, kn)) gen_load_full(Sn, M, xn); else gen_load_masked(Sn, M, 8 * chn, 32 * kn + lane, i, xn);
+                }
+                const int j0 = 8 * ch, c = 32 * k + lane;
+                double* Sc = S + (size_t)j0 * M + c;
+                double q[8];
 #pragma unroll
-                for (int k = 0; k < 8; ++k) { const int c = lane + 32 * k; if (c < i) pT[warp * M + c] = accT[k]; }
+                for (int r = 0; r < 8; ++r) q[r] = 0.0;
+                const double acc = is_full(ch, k) ? gen_segment_full(Sc, M, j0, c, vw, vN, xc, q)
+                                                  : gen_segment_masked(Sc, M, j0, c, i, tauP != 0.0, tau != 0.0, vw, vN, xc, q);
+                if (tau != 0.0) {                                         // eight row sums over 32 lanes: lane l ends with row l / 4
+                    double a4[4], b2[2];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const bool hi = lane & 16;
+                        const double keep = hi ? q[u + 4] : q[u], send = hi ? q[u] : q[u + 4];
+                        a4[u] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+                    }
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        const bool hi = lane & 8;
+                        const double keep = hi ? a4[u + 2] : a4[u], send = hi ? a4[u] : a4[u + 2];
+                        b2[u] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+                    }
+                    const bool hi = lane & 4;
+                    double s1 = (hi ? b2[1] : b2[0]) + __shfl_xor_sync(0xffffffffu, hi ? b2[0] : b2[1], 4);
+                    s1 += __shfl_xor_sync(0xffffffffu, s1, 2);
+                    s1 += __shfl_xor_sync(0xffffffffu, s1, 1);
+                    if (c < i) pTw[c] += acc;
+                    __syncwarp();
+                    const int j = j0 + (lane >> 2);
+                    if ((lane & 3) == 0 && j < i) pTw[j] += s1;
+                    __syncwarp();
+                }
+#pragma unroll
+                for (int r = 0; r < 8; ++r) xc[r] = xn[r];
+                t = tn; ch = chn; k = kn;
             }
         }
         __syncthreads();
         if (tau != 0.0) {
             part = 0.0;
             for (int c = tid; c < i; c += GEN_NT) {
-                double pc = pv[c];
+                double pc = 0.0;
 #pragma unroll
                 for (int w8 = 0; w8 < NW; ++w8) pc += pT[w8 * M + c];
                 pc *= tau;
