@@ -216,11 +216,13 @@ static Plan make_plan(int M, int batch, size_t extra, size_t avail)
     // classify-then-log; at M = 96, where none does, 8.5 against 8.0 ms)
     if (use_getvec(M)) { pl.ql_mode = (use_bigvec(M) && M > 128) ? QL_PAIRED_CLASSIFY : QL_CLASSIFY; pl.two_pass = true; }
     pl.bisect = use_getvec(M) && use_fast(M) && (t_opt.bisect >= 0 ? t_opt.bisect != 0 : batch <= BISECT_MAX_BATCH);
-    const bool want_pipe = t_opt.pipeline && (!g_prof.on || g_prof.keep_pipeline) && batch >= 2 * PIPE_MIN_SUB;
+    // (M > 160: the kernels of the any-M path hold two CTAs per SM -- sub-chunks of one full wave, measured M = 256: 18.8 -> 17.9 ms)
+    const int min_sub = M > 160 ? 296 : PIPE_MIN_SUB;
+    const bool want_pipe = t_opt.pipeline && (!g_prof.on || g_prof.keep_pipeline) && batch >= 2 * min_sub;
     auto bytes_for = [&](size_t n, size_t nl) { return plan_bytes(M, n, nl, extra, pl.two_pass); };
     if (want_pipe) {
         int per = t_opt.sub_chunk > 0 ? t_opt.sub_chunk : round_up((batch + PIPE_MAX_SUBS - 1) / PIPE_MAX_SUBS, 64);
-        if (per < PIPE_MIN_SUB && t_opt.sub_chunk <= 0) per = PIPE_MIN_SUB;
+        if (per < min_sub && t_opt.sub_chunk <= 0) per = min_sub;
         if (per > batch) per = batch;
         int nsub = (batch + per - 1) / per;
         int nslot = t_opt.slots > 0 ? t_opt.slots : PIPE_SLOTS;
