@@ -531,6 +531,33 @@ def run_ours(args):
                 "d2h_bytes_per_step": int(Xa_pin.numel() * 8 + B * 4), "api": "letkf_analysis_batched_host"}
             del hp, Xa_pin
             letkf.host_release()
+            # ---- the analysis above the register kernels (a1/a2 and a6-a9 are launches of their own there:
+            # generic_gram -> EVD -> generic_epilogue), the sweep's batch sizes
+            line["analysis_large"] = []
+            for Ml in (128, 256):
+                Bl = wl.sweep_batch(Ml)
+                li = wl.analysis_inputs(batch=Bl, M=Ml, p=98, nstate=9, config_index=70)
+                lt = {k: torch.from_numpy(li[k]).cuda() for k in ("Yb", "d", "rinv_loc", "Xb")}
+                lXa = torch.empty_like(lt["Xb"])
+                linfo = torch.zeros((Bl,), dtype=torch.int32, device="cuda")
+                lwork = torch.empty(letkf.analysis_workspace_bytes(Ml, 98, 9, Bl), dtype=torch.uint8, device="cuda")
+                for _ in range(2):
+                    letkf.analysis_batched(lt["Yb"], lt["d"], lt["rinv_loc"], lt["Xb"], li["rho"], Xa=lXa, info=linfo, work=lwork, stream=stream)
+                torch.cuda.synchronize()
+                ks = min(args.steps, 5)
+                e0.record(stream)
+                for _ in range(ks):
+                    letkf.analysis_batched(lt["Yb"], lt["d"], lt["rinv_loc"], lt["Xb"], li["rho"], Xa=lXa, info=linfo, work=lwork, stream=stream)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                lms = e0.elapsed_time(e1) / ks
+                fl = analysis_model_flops(Ml, 98, 9)
+                line["analysis_large"].append({
+                    "workload": f"letkf_analysis_batched fp64 M={Ml} p=98 nstate=9 batch={Bl}, W not requested",
+                    "ms_per_step": round(lms, 4), "value": Bl / (lms * 1e-3), "unit": "grid points/s",
+                    "frac_of_measured_fp64_peak": round(fl * Bl / (lms * 1e-3) / 1e12 / peak_measured, 4),
+                    "info_nonzero": int((linfo != 0).sum())})
+                del lt, lXa, linfo, lwork
             # ---- grid form: same 128 x 128 x 2 x 7x7 problem, the local
             # observations gathered inside the library from the fields (Y_loc never materialised)
             gi = wl.grid_inputs()

@@ -342,6 +342,7 @@ generic_apply_one(double* V_, double* __restrict__ w_, const Workspace& ws, int 
     __shared__ int sh_rc, sh_lo, sh_m, sh_fail;
 
     const int tid = threadIdx.x;
+    const int NT = blockDim.x;                            // (ceil32(M), at least 64: generic_apply; GEN_NT: the finisher)
     const int flag = ws.flags[b];
     if (flag == FLAG_GETVEC) return;                      // finished by big_getvec + big_gemm (no rotations)
     const int flagged = flag == FLAG_SLOW;
@@ -349,7 +350,7 @@ generic_apply_one(double* V_, double* __restrict__ w_, const Workspace& ws, int 
     double* B = V_ + b * M * M;
 
     if (q_rowmajor) {      // bring row-major Q into the Qt layout first (in-place transpose)
-        for (int idx = tid; idx < M * M; idx += GEN_NT) {
+        for (int idx = tid; idx < M * M; idx += NT) {
             const int r = idx / M, c = idx - r * M;
             if (r < c) {
                 const double x = B[(size_t)r * M + c], y = B[(size_t)c * M + r];
@@ -370,7 +371,7 @@ generic_apply_one(double* V_, double* __restrict__ w_, const Workspace& ws, int 
         // shrink): rotation (2, j) on columns (j, j+1) may run as soon as (1, j-1) is done -- the value
         // (1, i) leaves in column i+1 is final for sweep 1 and goes straight into (2, i+1), whose
         // carry f2 is column i+2.  One load and one store per element instead of two.
-        for (int r = tid; r < M; r += GEN_NT) {
+        for (int r = tid; r < M; r += NT) {
             double* col = B + r;
             int pos = 0;
             for (int sidx = 0; sidx < nsw;) {
@@ -399,6 +400,25 @@ generic_apply_one(double* V_, double* __restrict__ w_, const Workspace& ws, int 
                             --i;
                         }
                         const int iend = max(lo2 - 1, lo);
+                        // (the loop is a chain through f1, f2 whose loads do not depend on it: eight steps' worth of
+                        // loads are issued before the chain goes on -- the rows read lie below every row written)
+                        for (; i - 7 >= iend; i -= 8) {
+                            double z[8];
+                            double2 qa[8], qb[8];
+#pragma unroll
+                            for (int u = 0; u < 8; ++u) {
+                                z[u] = col[(size_t)(i - u) * M];
+                                qa[u] = cur[m - 1 - i + u];
+                                qb[u] = cur2[m2 - 2 - i + u];
+                            }
+#pragma unroll
+                            for (int u = 0; u < 8; ++u) {
+                                const double o1 = qa[u].y * z[u] + qa[u].x * f1;
+                                f1 = qa[u].x * z[u] - qa[u].y * f1;
+                                col[(size_t)(i - u + 2) * M] = qb[u].y * o1 + qb[u].x * f2;
+                                f2 = qb[u].x * o1 - qb[u].y * f2;
+                            }
+                        }
                         for (; i >= iend; --i) {                     // (1, i) then (2, i + 1)
                             const double2 q1 = cur[m - 1 - i], q2 = cur2[m2 - 2 - i];
                             const double z = col[(size_t)i * M];
@@ -427,7 +447,19 @@ generic_apply_one(double* V_, double* __restrict__ w_, const Workspace& ws, int 
                     }
                 }
                 double f = col[(size_t)m * M];
-                for (int i = m - 1; i >= lo; --i) {
+                int i = m - 1;
+                for (; i - 3 >= lo; i -= 4) {
+                    double z[4];
+                    double2 qa[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) { z[u] = col[(size_t)(i - u) * M]; qa[u] = cur[m - 1 - i + u]; }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        col[(size_t)(i - u + 1) * M] = qa[u].y * z[u] + qa[u].x * f;
+                        f = qa[u].x * z[u] - qa[u].y * f;
+                    }
+                }
+                for (; i >= lo; --i) {
                     const double2 q = cur[m - 1 - i];
                     const double zi = col[(size_t)i * M];
                     col[(size_t)(i + 1) * M] = q.y * zi + q.x * f;
@@ -438,9 +470,9 @@ generic_apply_one(double* V_, double* __restrict__ w_, const Workspace& ws, int 
                 sidx += 1;
             }
         }
-        for (int k = tid; k < M; k += GEN_NT) permsm[k] = ws.perm[b * M + k];
+        for (int k = tid; k < M; k += NT) permsm[k] = ws.perm[b * M + k];
     } else {
-        for (int k = tid; k < M; k += GEN_NT) { dsm[k] = ws.dws[b * M + k]; esm[k] = ws.ews[b * M + k]; }
+        for (int k = tid; k < M; k += NT) { dsm[k] = ws.dws[b * M + k]; esm[k] = ws.ews[b * M + k]; }
         __syncthreads();
         QLState st{0, 0, 0, 0.0};
         if (tid == 0) { esm[M - 1] = 0.0; st.thr = ql_threshold(dsm, esm, 1, M); }
@@ -453,7 +485,7 @@ generic_apply_one(double* V_, double* __restrict__ w_, const Workspace& ws, int 
             __syncthreads();
             if (sh_rc != 1) break;
             const int lo = sh_lo, m = sh_m;
-            for (int r = tid; r < M; r += GEN_NT) {
+            for (int r = tid; r < M; r += NT) {
                 double f = B[(size_t)m * M + r];
                 for (int i = m - 1; i >= lo; --i) {
                     const double2 q = cs[m - 1 - i];
@@ -470,19 +502,19 @@ generic_apply_one(double* V_, double* __restrict__ w_, const Workspace& ws, int 
             sh_fail = st.fail;
         }
         __syncthreads();
-        for (int k = tid; k < M; k += GEN_NT) w_[b * M + k] = dsm[k];
+        for (int k = tid; k < M; k += NT) w_[b * M + k] = dsm[k];
         if (info && tid == 0) info[b] = sh_fail | 0x40000000;
     }
     __syncthreads();
 
     // sort: new row k of B = old row perm[k]; cycles are followed by every thread for its column
-    for (int k = tid; k < M; k += GEN_NT) {
+    for (int k = tid; k < M; k += NT) {
         int j = permsm[k];
         while (j > k) j = permsm[j];
         leader[k] = (j == k) && (permsm[k] != k);
     }
     __syncthreads();
-    for (int r = tid; r < M; r += GEN_NT) {
+    for (int r = tid; r < M; r += NT) {
         for (int k = 0; k < M; ++k) {
             if (!leader[k]) continue;
             const double first = B[(size_t)k * M + r];
@@ -504,14 +536,14 @@ generic_apply_one(double* V_, double* __restrict__ w_, const Workspace& ws, int 
     const int tx = tid & 31, ty = tid >> 5;       // 32 x 8
     for (int ti = 0; ti < nt; ++ti)
         for (int tj = ti; tj < nt; ++tj) {
-            for (int yy = ty; yy < 32; yy += GEN_NT / 32) {
+            for (int yy = ty; yy < 32; yy += NT / 32) {
                 const int r0 = ti * 32 + yy, c0 = tj * 32 + tx;
                 if (r0 < M && c0 < M) t0[yy * 33 + tx] = B[(size_t)r0 * M + c0];
                 const int r1 = tj * 32 + yy, c1 = ti * 32 + tx;
                 if (r1 < M && c1 < M) t1[yy * 33 + tx] = B[(size_t)r1 * M + c1];
             }
             __syncthreads();
-            for (int yy = ty; yy < 32; yy += GEN_NT / 32) {
+            for (int yy = ty; yy < 32; yy += NT / 32) {
                 const int r1 = tj * 32 + yy, c1 = ti * 32 + tx;       // B[tj-tile] <- t0^T
                 if (r1 < M && c1 < M) B[(size_t)r1 * M + c1] = t0[tx * 33 + yy];
                 if (ti != tj) {

@@ -530,7 +530,8 @@ static int stage_AP(int M, int n, double* w, double* V, int* info, Workspace ws,
                     V, w, ws, M, n, info, /*only_flagged=*/1, /*q_rowmajor=*/0));
         return 0;
     }
-    KLAUNCH("generic_apply", st, generic_apply<<<n, GEN_NT, ap_smem, st>>>(V, w, ws, M, n, info, 0, 0));
+    const int ap_nt = M <= 32 ? 64 : (M + 31) / 32 * 32;          // thread r = column r of Q^T: no idle warps (M = 192: 5.6 -> 4.7 ms)
+    KLAUNCH("generic_apply", st, generic_apply<<<n, ap_nt, ap_smem, st>>>(V, w, ws, M, n, info, 0, 0));
     return 0;
 }
 
