@@ -14,14 +14,15 @@
 namespace letkf {
 
 constexpr int GEN_NT = 256;
-constexpr int GEN_QK = 8;      // reflectors applied per pass over the rows when Q is formed
+constexpr int GEN_QK = 16;     // reflectors applied per pass over the rows when Q is formed
 
 // One segment of the reduction's pass: rows j0 ... j0+7, columns c = 32 k + lane, Sc = &S[j0][c], in two steps so that
 // the loads of the next segment are in flight while this one is worked on.  x <- x - v_j w_c - w_j v_c (vw[.] = (v, w) of
 // the pending pivot), then q[r] += x v_c (row sums, reduced over the lanes by the caller) and acc += x v_j for c < j
-// (this lane's column sum).  _full: every (j, c) of the segment is strictly below the diagonal and above the pivot row --
-// no mask anywhere; _masked: the diagonal segment, the ragged last chunk, and the passes with only one of the two
-// operations (H = I, reading G19).
+// (this lane's column sum).  The 32 x 32 blocks ON the diagonal are kept in full (both triangles, the mirror entries in the
+// otherwise unused upper triangle of S): their segments take the same mask-free path and give row sums only (`diag`: no
+// column sum).  _full: every row and column of the segment lies above the pivot row / left of the pivot column;
+// _masked: the segments that reach row or column i, and the passes with only one of the two operations (H = I, reading G19).
 __device__ __forceinline__ void gen_load_full(const double* __restrict__ Sc, int M, double (&x)[8])
 {
 #pragma unroll
@@ -30,7 +31,7 @@ __device__ __forceinline__ void gen_load_full(const double* __restrict__ Sc, int
 __device__ __forceinline__ void gen_load_masked(const double* __restrict__ Sc, int M, int j0, int c, int i, double (&x)[8])
 {
 #pragma unroll
-    for (int r = 0; r < 8; ++r) x[r] = (c <= j0 + r && j0 + r < i) ? Sc[(size_t)r * M] : 0.0;
+    for (int r = 0; r < 8; ++r) x[r] = (c < i && j0 + r < i) ? Sc[(size_t)r * M] : 0.0;
 }
 __device__ __forceinline__ double gen_segment_full(double* __restrict__ Sc, int M, int j0, int c, const double2* __restrict__ vw,
                                                    const double* __restrict__ vN, const double (&x)[8], double (&q)[8])
@@ -49,7 +50,7 @@ __device__ __forceinline__ double gen_segment_full(double* __restrict__ Sc, int 
     }
     return acc;
 }
-__device__ __forceinline__ double gen_segment_masked(double* __restrict__ Sc, int M, int j0, int c, int i, bool upd, bool mv,
+__device__ __forceinline__ double gen_segment_masked(double* __restrict__ Sc, int M, int j0, int c, int i, bool upd, bool mv, bool diag,
                                                      const double2* __restrict__ vw, const double* __restrict__ vN,
                                                      const double (&x)[8], double (&q)[8])
 {
@@ -64,7 +65,7 @@ __device__ __forceinline__ double gen_segment_masked(double* __restrict__ Sc, in
             const int j = j0 + r;
             const double2 vwj = vw[min(j, M - 1)];
             const double xn = fma(-vwj.x, t.y, fma(-vwj.y, t.x, y[r]));
-            const bool m = c <= j && j < i;
+            const bool m = c < i && j < i;
             if (m) Sc[(size_t)r * M] = xn;
             y[r] = m ? xn : 0.0;
         }
@@ -77,7 +78,7 @@ __device__ __forceinline__ double gen_segment_masked(double* __restrict__ Sc, in
             const int j = j0 + r;
             const double vj = vN[min(j, M - 1)];
             q[r] = fma(y[r], vc, q[r]);
-            acc += (c < j && j < i) ? y[r] * vj : 0.0;
+            acc += (!diag && c < i && j < i) ? y[r] * vj : 0.0;
         }
     }
     return acc;
@@ -111,8 +112,11 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
     }
     if (phase & 1) {
     // copy of the lower triangle (the upper one is never read: symmetric half only, below)
-    for (int r = warp; r < M; r += NW)
-        for (int c = lane; c <= r; c += 32) S[(size_t)r * M + c] = A[(size_t)r * M + c];
+    // (and of the mirror entries inside the 32 x 32 blocks on the diagonal, see gen_segment_*)
+    for (int r = warp; r < M; r += NW) {
+        const int cend = min(M - 1, (r | 31));
+        for (int c = lane; c <= cend; c += 32) S[(size_t)r * M + c] = (c <= r) ? A[(size_t)r * M + c] : A[(size_t)c * M + r];
+    }
     __syncthreads();
 
     // Pivots i = M-1 ... 1.  The rank-2 update of pivot i+1 and the mat-vec of pivot i share ONE
@@ -163,7 +167,8 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
             int nitems = 0;
             for (int k = 0; 4 * k < nch; ++k) nitems += nch - 4 * k;
             auto decode = [&](int t, int& ch, int& k) { k = 0; while (t >= nch - 4 * k) { t -= nch - 4 * k; ++k; } ch = 4 * k + t; };
-            auto is_full = [&](int ch, int k) { return both && 8 * ch + 8 <= i && 32 * k + 32 <= 8 * ch; };
+            auto is_full = [&](int ch, int k) { return both && 8 * ch + 8 <= i && 32 * k + 32 <= i; };   // (k <= block of the chunk)
+            auto is_diag = [&](int ch, int k) { return k == (ch >> 2); };
             int t = warp, ch = 0, k = 0;
             double xc[8], xn[8];
 #pragma unroll
@@ -187,8 +192,10 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
                 double q[8];
 #pragma unroll
                 for (int r = 0; r < 8; ++r) q[r] = 0.0;
-                const double acc = is_full(ch, k) ? gen_segment_full(Sc, M, j0, c, vw, vN, xc, q)
-                                                  : gen_segment_masked(Sc, M, j0, c, i, tauP != 0.0, tau != 0.0, vw, vN, xc, q);
+                const bool diag = is_diag(ch, k);
+                double acc = is_full(ch, k) ? gen_segment_full(Sc, M, j0, c, vw, vN, xc, q)
+                                            : gen_segment_masked(Sc, M, j0, c, i, tauP != 0.0, tau != 0.0, diag, vw, vN, xc, q);
+                if (diag) acc = 0.0;
                 if (tau != 0.0) {                                         // eight row sums over 32 lanes: lane l ends with row l / 4
                     double a4[4], b2[2];
 #pragma unroll
