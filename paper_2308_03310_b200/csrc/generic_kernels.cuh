@@ -131,18 +131,20 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
     double* vN = sm + 2 * M;                         // [M] v of the new pivot
     double* pv = red + NW;                           // [M] row sums, then p (row 0 of the vk area, free here)
     double* pT = red + NW + M;                       // [NW][M] column sums per warp (rows 1 ... NW of the vk area)
+    static_assert(LETKF_MAX_M <= GEN_NT, "one entry of the pivot row per thread");
     double tauP = 0.0;                               // tau of the pending update (0: none)
     for (int i = M - 1; i >= 1; --i) {
         double* rowi = S + (size_t)i * M;
-        if (tauP != 0.0) {                           // row i: S[i][c] -= v_i w_c + w_i v_c, c <= i
-            const double2 vwi = vw[i];
-            for (int c = tid; c <= i; c += GEN_NT) { const double2 t = vw[c]; rowi[c] -= vwi.x * t.y + vwi.y * t.x; }
-            __syncthreads();
+        // row i with the pending update, one entry per thread (M <= GEN_NT), kept in the register through the formation of
+        // the reflector: one read and one write of the row per pivot, no barrier between the update and the norm
+        double xr = 0.0;
+        if (tid <= i) {
+            xr = rowi[tid];
+            if (tauP != 0.0) { const double2 vwi = vw[i], t = vw[tid]; xr -= vwi.x * t.y + vwi.y * t.x; }
         }
-        double part = 0.0;
-        for (int c = tid; c < i - 1; c += GEN_NT) { const double x = rowi[c]; part += x * x; }
-        const double sigma = block_sum<GEN_NT>(part, red);
-        const double alpha = rowi[i - 1];
+        if (tid == i - 1) taus[0] = xr;                                   // alpha (taus[0] is free: reflectors are 1 ... M-1)
+        const double sigma = block_sum<GEN_NT>((tid < i - 1) ? xr * xr : 0.0, red);
+        const double alpha = taus[0];
         double beta, tau, scal;
         if (sigma == 0.0) { tau = 0.0; beta = alpha; scal = 0.0; }       // reading G19: H = I
         else {
@@ -150,10 +152,9 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
             tau = (beta - alpha) / beta;
             scal = 1.0 / (alpha - beta);
         }
-        for (int c = tid; c < i; c += GEN_NT) vN[c] = (c == i - 1) ? 1.0 : rowi[c] * scal;
-        if (tid == 0) { ews[i - 1] = beta; dws[i] = rowi[i]; taus[i] = tau; rowi[i] = tau; }
+        if (tid < i) { const double vc = (tid == i - 1) ? 1.0 : xr * scal; vN[tid] = vc; rowi[tid] = vc; }   // the reflector stays in row i
+        if (tid == i) { ews[i - 1] = beta; dws[i] = xr; taus[i] = tau; rowi[i] = tau; }
         __syncthreads();
-        for (int c = tid; c < i; c += GEN_NT) rowi[c] = vN[c];           // keep the reflector
         if (tauP != 0.0 || tau != 0.0) {
             const bool both = tauP != 0.0 && tau != 0.0;
             const int nch = (i + 7) >> 3;
@@ -227,7 +228,7 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
         }
         __syncthreads();
         if (tau != 0.0) {
-            part = 0.0;
+            double part = 0.0;
             for (int c = tid; c < i; c += GEN_NT) {
                 double pc = 0.0;
 #pragma unroll
