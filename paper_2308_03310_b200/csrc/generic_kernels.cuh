@@ -84,6 +84,21 @@ __device__ __forceinline__ double gen_segment_masked(double* __restrict__ Sc, in
     return acc;
 }
 
+// Block-wide sum with ONE barrier: the caller alternates between scratch rows that are not written again before at
+// least one more barrier has passed.  All threads get the result.
+template <int NT>
+__device__ __forceinline__ double block_sum1(double v, double* red)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    v = warp_sum(v);
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    double t = 0.0;
+#pragma unroll
+    for (int w = 0; w < NT / 32; ++w) t += red[w];
+    return t;
+}
+
 // ---------------------------------------------------------------------------------------------
 // a3 + explicit Q.  Reduction order is "from the last row up" (pivot i = M-1 ... 1, reflector
 // H_i acts on indices 0..i-1), so Q = H_{M-1} ... H_1 and T = Q^T A Q.
@@ -131,6 +146,8 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
     double* vN = sm + 2 * M;                         // [M] v of the new pivot
     double* pv = red + NW;                           // [M] row sums, then p (row 0 of the vk area, free here)
     double* pT = red + NW + M;                       // [NW][M] column sums per warp (rows 1 ... NW of the vk area)
+    double* red1 = red + NW + (NW + 1) * M;          // [NW] second block-sum scratch (row NW+1 of the vk area)
+    static_assert(GEN_QK + 1 >= NW + 2, "the vk area holds p, the per-warp sums and the second scratch row");
     static_assert(LETKF_MAX_M <= GEN_NT, "one entry of the pivot row per thread");
     double tauP = 0.0;                               // tau of the pending update (0: none)
     for (int i = M - 1; i >= 1; --i) {
@@ -143,7 +160,7 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
             if (tauP != 0.0) { const double2 vwi = vw[i], t = vw[tid]; xr -= vwi.x * t.y + vwi.y * t.x; }
         }
         if (tid == i - 1) taus[0] = xr;                                   // alpha (taus[0] is free: reflectors are 1 ... M-1)
-        const double sigma = block_sum<GEN_NT>((tid < i - 1) ? xr * xr : 0.0, red);
+        const double sigma = block_sum1<GEN_NT>((tid < i - 1) ? xr * xr : 0.0, red);    // (red / red1: each written once per pivot)
         const double alpha = taus[0];
         double beta, tau, scal;
         if (sigma == 0.0) { tau = 0.0; beta = alpha; scal = 0.0; }       // reading G19: H = I
@@ -237,7 +254,7 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
                 pv[c] = pc;
                 part += pc * vN[c];
             }
-            const double K = 0.5 * tau * block_sum<GEN_NT>(part, red);
+            const double K = 0.5 * tau * block_sum1<GEN_NT>(part, red1);
             for (int c = tid; c < i; c += GEN_NT) { const double vc = vN[c]; vw[c] = make_double2(vc, pv[c] - K * vc); }
         }
         tauP = tau;
