@@ -666,7 +666,12 @@ generic_gram(const double* __restrict__ Yb_, const double* __restrict__ d_,
 //   W     = sqrt(M-1) V diag(lam^-1/2) V^T                                   Eq.15   (if wanted)
 //   Xa    = xbar 1^T + (dX wbar) 1^T + sqrt(M-1) ((dX V) diag(lam^-1/2)) V^T  Eq.13, without
 //           forming W: dX W = ((dX V) Lam^-1/2) V^T  (same product, associativity only)
-// Dynamic shared memory: t[M], wb[M], xbar[ns], cs[ns], T1[ns][M], dX[ns][M]
+// Dynamic shared memory: t[M], wb[M], xbar[ns], cs[ns], T1[ns][M], gd[1 + ns][M] (g, then dX; dX is later reused for the
+// products that become Xa).
+// V is read twice, each time whole rows by consecutive threads: once by columns (thread k sums V[n][k] against g and
+// the rows of dX over all n: t and T1, no reduction across threads), once by rows (a warp per row m, the 1 + ns dot
+// products of a row reduced eight at a time by a halving butterfly).  c_s = dX[s] . wbar is taken as
+// sum_k (dX V)[s][k] t[k], the same number up to rounding, so that it is known before the second pass.
 __device__ __forceinline__ void
 generic_epilogue_one(const double* __restrict__ V_, const double* __restrict__ lam_,
                      const double* __restrict__ g_, const double* Xb_, int M, int ns,
@@ -678,7 +683,8 @@ generic_epilogue_one(const double* __restrict__ V_, const double* __restrict__ l
     double* xbar = sm + 2 * M;
     double* cs   = xbar + ns;
     double* T1   = cs + ns;
-    double* dX   = T1 + (size_t)ns * M;
+    double* gd   = T1 + (size_t)ns * M;                       // [1 + ns][M]
+    double* dX   = gd + M;
     const double* V = V_ + b * (size_t)M * M;
     const double* lam = lam_ + b * M;
     const double* g = g_ + b * M;
@@ -687,46 +693,95 @@ generic_epilogue_one(const double* __restrict__ V_, const double* __restrict__ l
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const double sq = sqrt((double)(M - 1));
 
-    for (int k = tid; k < M; k += 256) {
-        double acc = 0.0;
-        for (int n = 0; n < M; ++n) acc += V[(size_t)n * M + k] * g[n];
-        t[k] = acc / lam[k];
-    }
+    for (int n = tid; n < M; n += 256) gd[n] = g[n];
     for (int s = warp; s < ns; s += 8) {                      // Eq.9-11
         double acc = 0.0;
         for (int m = lane; m < M; m += 32) acc += Xb[(size_t)s * M + m];
         acc = warp_sum(acc) / (double)M;
-        if (lane == 0) xbar[s] = acc;
+        if (lane == 0) { xbar[s] = acc; cs[s] = 0.0; }
         for (int m = lane; m < M; m += 32) dX[(size_t)s * M + m] = Xb[(size_t)s * M + m] - acc;
     }
     __syncthreads();
-    for (int m = warp; m < M; m += 8) {                       // wbar = V t
-        double acc = 0.0;
-        for (int k = lane; k < M; k += 32) acc += V[(size_t)m * M + k] * t[k];
-        acc = warp_sum(acc);
-        if (lane == 0) { wb[m] = acc; if (wbar_) wbar_[b * M + m] = acc; }
-    }
-    for (int idx = tid; idx < ns * M; idx += 256) {            // T1 = sqrt(M-1) (dX V) Lam^-1/2
-        const int s = idx / M, k = idx - s * M;
-        double acc = 0.0;
-        for (int m = 0; m < M; ++m) acc += dX[(size_t)s * M + m] * V[(size_t)m * M + k];
-        T1[idx] = acc * sq / sqrt(lam[k]);
+    // first pass, by columns: t = Lam^-1 V^T g, T1 = sqrt(M-1) (dX V) Lam^-1/2, eight of the 1 + ns vectors at a time
+    for (int v0 = 0; v0 < 1 + ns; v0 += 8) {
+        const int nv = min(8, 1 + ns - v0);
+        for (int k = tid; k < M; k += 256) {
+            double acc[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) acc[u] = 0.0;
+            const double* gv = gd + (size_t)v0 * M;
+#pragma unroll 4
+            for (int n = 0; n < M; ++n) {
+                const double x = V[(size_t)n * M + k];
+#pragma unroll
+                for (int u = 0; u < 8; ++u)
+                    if (u < nv) acc[u] = fma(x, gv[(size_t)u * M + n], acc[u]);
+            }
+            const double lk = lam[k], rs = sq / sqrt(lk);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                if (u < nv) {
+                    const int idx = v0 + u;
+                    if (idx == 0) t[k] = acc[u] / lk;
+                    else T1[(size_t)(idx - 1) * M + k] = acc[u] * rs;
+                }
+            }
+        }
     }
     __syncthreads();
-    for (int s = warp; s < ns; s += 8) {                      // c_s = dX[s] . wbar
+    for (int s = warp; s < ns; s += 8) {                      // c_s = dX[s] . wbar = sum_k (dX V)[s][k] t[k]
         double acc = 0.0;
-        for (int m = lane; m < M; m += 32) acc += dX[(size_t)s * M + m] * wb[m];
+        for (int k = lane; k < M; k += 32) acc += T1[(size_t)s * M + k] * (sqrt(lam[k]) / sq) * t[k];
         acc = warp_sum(acc);
         if (lane == 0) cs[s] = acc;
     }
-    __syncthreads();
-    for (int m = warp; m < M; m += 8) {                       // Xa[s][m]
-        for (int s = 0; s < ns; ++s) {
-            double acc = 0.0;
-            for (int k = lane; k < M; k += 32) acc += T1[(size_t)s * M + k] * V[(size_t)m * M + k];
-            acc = warp_sum(acc);
-            if (lane == 0) Xa[(size_t)s * M + m] = xbar[s] + cs[s] + acc;
+    __syncthreads();                                          // (dX is dead from here on: its rows receive dX W)
+    // second pass, by rows: wbar[m] = V[m] . t and (dX W)[s][m] = T1[s] . V[m]
+    const int KJ = (M + 31) >> 5;
+    for (int m = warp; m < M; m += 8) {
+        double x[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) { const int k = lane + 32 * j; x[j] = (j < KJ && k < M) ? V[(size_t)m * M + k] : 0.0; }
+        for (int v0 = 0; v0 < 1 + ns; v0 += 8) {
+            const int nv = min(8, 1 + ns - v0);
+            double q[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                q[u] = 0.0;
+                if (u < nv) {
+                    const double* tv = (v0 + u == 0) ? t : T1 + (size_t)(v0 + u - 1) * M;
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) { const int k = lane + 32 * j; if (j < KJ && k < M) q[u] = fma(x[j], tv[k], q[u]); }
+                }
+            }
+            double a4[4], b2[2];                                  // eight sums over 32 lanes: lane l ends with sum l / 4
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const bool hi = lane & 16;
+                const double keep = hi ? q[u + 4] : q[u], send = hi ? q[u] : q[u + 4];
+                a4[u] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const bool hi = lane & 8;
+                const double keep = hi ? a4[u + 2] : a4[u], send = hi ? a4[u] : a4[u + 2];
+                b2[u] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+            }
+            const bool hi = lane & 4;
+            double s1 = (hi ? b2[1] : b2[0]) + __shfl_xor_sync(0xffffffffu, hi ? b2[0] : b2[1], 4);
+            s1 += __shfl_xor_sync(0xffffffffu, s1, 2);
+            s1 += __shfl_xor_sync(0xffffffffu, s1, 1);
+            const int idx = v0 + (lane >> 2);
+            if ((lane & 3) == 0 && (lane >> 2) < nv) {
+                if (idx == 0) { wb[m] = s1; if (wbar_) wbar_[b * M + m] = s1; }
+                else dX[(size_t)(idx - 1) * M + m] = s1;
+            }
         }
+    }
+    __syncthreads();
+    for (int idx = tid; idx < ns * M; idx += 256) {            // Xa = xbar 1^T + c 1^T + dX W   (Eq.13)
+        const int sI = idx / M;
+        Xa[idx] = xbar[sI] + cs[sI] + dX[idx];
     }
     if (W_) {                                                  // Eq.15, 16x16 threads x (4x4)
         double* W = W_ + b * (size_t)M * M;

@@ -1015,7 +1015,7 @@ static int analysis_core(const double* Yb, const double* d, const double* rinv_l
 
     const double shift = (double)(M - 1) / rho;
     cudaError_t ce;
-    const size_t ep_smem = sizeof(double) * (2 * (size_t)M + 2 * (size_t)nstate + 2 * (size_t)nstate * M);
+    const size_t ep_smem = sizeof(double) * (3 * (size_t)M + 2 * (size_t)nstate + 2 * (size_t)nstate * M);
     if (ep_smem > 200 * 1024) return -7;
     if ((ce = allow_smem(generic_epilogue, ep_smem)) != cudaSuccess) return (int)ce;
     const PassHooks* hooks = t_hooks;
