@@ -610,7 +610,8 @@ generic_apply(double* V_, double* __restrict__ w_, Workspace ws, int M, int n, i
 // a1 + a2 (Eq.17 and the right factor of Eq.14), any M, p.
 //   Aout[b][m][n] = ((M-1)/rho) delta_mn + sum_j r_j Yb[j][m] Yb[j][n]
 //   gout[b][m]    = sum_j Yb[j][m] r_j d_j
-// 16 x 16 threads, 4 x 4 outputs each per 64 x 64 output tile.
+// 16 x 16 threads, 4 x 4 outputs each per 64 x 64 output tile; the tiles strictly above the diagonal are not formed
+// (Aout's upper triangle is left as it was, beyond the diagonal tiles).
 __global__ void __launch_bounds__(256)
 generic_gram(const double* __restrict__ Yb_, const double* __restrict__ d_,
              const double* __restrict__ r_, int M, int p, double shift,
@@ -629,7 +630,7 @@ generic_gram(const double* __restrict__ Yb_, const double* __restrict__ d_,
         gout_[b * M + m] = acc;
     }
     for (int m0 = 0; m0 < M; m0 += 64)
-        for (int n0 = 0; n0 < M; n0 += 64) {
+        for (int n0 = 0; n0 <= m0; n0 += 64) {              // (every reduction kernel reads the lower triangle only)
             double acc[4][4];
 #pragma unroll
             for (int a = 0; a < 4; ++a)
