@@ -18,6 +18,7 @@
 #include "mid_kernels.cuh"
 #include "pack_kernels.cuh"
 #include "big_kernels.cuh"
+#include "gram_kernels.cuh"
 
 namespace letkf {
 
@@ -367,6 +368,13 @@ static int stage_T(const double* A, int M, int n, double* V, Workspace ws, cudaS
         }
     }
     if (gram) {
+        if (M > 64) {                                         // the contraction on the FP64 tensor cores (gram_kernels.cuh)
+            cudaError_t ge;
+            const size_t gs = gram_smem(M, gram->p);
+            if ((ge = allow_smem(big_gram, gs)) != cudaSuccess) return (int)ge;
+            KLAUNCH("big_gram", st,
+                    big_gram<<<n, GRAM_NT, gs, st>>>(gram->Yb, gram->d, gram->r, M, gram->p, gram_chunk(M, gram->p), gram->shift, V, gram->gout));
+        } else
         KLAUNCH("generic_gram", st,
                 generic_gram<<<n, 256, 0, st>>>(gram->Yb, gram->d, gram->r, M, gram->p, gram->shift, V, gram->gout));
         A = V;

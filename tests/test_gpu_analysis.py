@@ -48,6 +48,19 @@ def test_analysis_vs_oracle(lk, oracle, M, p, ns, batch):
     parity.assert_analysis(out, ref, inp["Xb"], f"M={M} p={p} ns={ns}")
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("M,p,ns,batch", [(70, 5, 3, 4), (96, 0, 2, 3), (97, 1, 1, 2), (128, 230, 4, 2), (256, 130, 17, 2)])
+def test_analysis_above_64_gram_shapes(lk, oracle, M, p, ns, batch):
+    """The Gram kernel of the orders above 64 (big_gram, FP64 tensor cores): a number of observations that is not a
+    multiple of four, none at all, one, more than one shared-memory chunk holds (M = 128: 212; M = 256: 108), ragged
+    orders; nstate above eight (two rounds of the epilogue's grouped reductions)."""
+    inp = wl.analysis_inputs(batch=batch, M=M, p=p, nstate=ns, config_index=900 + M + p)
+    out = run_gpu(lk, inp, want_wbar=True)
+    ref = run_oracle(oracle, inp)
+    assert (out["info"] == 0).all()
+    parity.assert_analysis(out, ref, inp["Xb"], f"M={M} p={p} ns={ns}")
+
+
 @pytest.mark.parametrize("want_W", [True, False])
 @pytest.mark.parametrize("M,batch", [(128, 4), (160, 3), (192, 3), (256, 2)])
 def test_analysis_large_ensembles(lk, oracle, M, batch, want_W):
