@@ -1,5 +1,5 @@
 // generic_kernels.cuh -- the any-M (1 <= M <= 256) path of libletkf: one CTA per matrix, the
-// matrix held in the caller's V buffer (global memory / L2).  It is the path for M > 64, the
+// matrix held in the caller's V buffer (global memory / L2).  It is the path for M > 160, the
 // finisher for matrices whose rotation log overflowed on the fast path, and the reference point
 // the register-resident kernels of fast_kernels.cuh are measured against.
 //
@@ -267,9 +267,9 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
     if (!(phase & 2)) return;
 
     // Q^T = H_1 H_2 ... H_{M-1}, grown in place: B_i = diag(B_{i-1}, 1) H_i on the leading i x i.
-    // The kernel runs at the HBM roof for M > 160 (the resident matrices exceed L2), so GEN_QK
-    // reflectors are applied per pass over the rows: a row is read and written once per GEN_QK
-    // steps, held in registers in between (<= 8 doubles per lane).  The rows and columns the later
+    // B lives in global memory / L2, so GEN_QK reflectors are applied per pass over the rows: a row is
+    // read and written once per GEN_QK steps, held in registers in between (<= 8 doubles per lane and
+    // row, four rows per warp).  The rows and columns the later
     // reflectors of a group add are set to identity first and every reflector is zero-padded to the
     // group's width, so H_i leaves the rows >= i alone exactly as the one-at-a-time loop does.
     double* vk = red + NW;        // [GEN_QK][M] (one more row behind it belongs to pT above)
@@ -390,8 +390,7 @@ generic_apply_one(double* V_, double* __restrict__ w_, const Workspace& ws, int 
         const int nsw = ws.nsweeps[b];
         const uint32_t* hdr = ws.hdr + b * ws.swcap;
         const double2* rot = ws.rot + b * ws.logcap;
-        // The replay streams B from global memory (for M > 160 the resident matrices exceed L2 and
-        // the loop runs at the HBM roof), so two consecutive sweeps share ONE pass over the column
+        // The replay streams B from global memory / L2, so two consecutive sweeps share ONE pass over the column
         // whenever the second lies inside the first (lo2 >= lo, m2 <= m: the usual case, blocks only
         // shrink): rotation (2, j) on columns (j, j+1) may run as soon as (1, j-1) is done -- the value
         // (1, i) leaves in column i+1 is final for sweep 1 and goes straight into (2, i+1), whose
