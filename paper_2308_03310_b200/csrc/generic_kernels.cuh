@@ -180,30 +180,19 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
             __syncwarp();
             // Work items: (chunk ch of eight rows, column segment k) with 32 k <= 8 ch + 7, segment by segment (k = 0: every
             // chunk, k = 1: chunks 4 ..., ...), dealt to the warps round robin -- items of one size, so the warps finish
-            // together (whole chunks left a third of the warp time waiting at the barrier).  The loads of a warp's next
-            // item are in flight while it works on the current one.
-            int nitems = 0;
-            for (int k = 0; 4 * k < nch; ++k) nitems += nch - 4 * k;
-            auto decode = [&](int t, int& ch, int& k) { k = 0; while (t >= nch - 4 * k) { t -= nch - 4 * k; ++k; } ch = 4 * k + t; };
+            // together (whole chunks left a third of the warp time waiting at the barrier).  (Issuing the loads of a warp's
+            // next item ahead of the current one measured no faster -- two CTAs per SM cover the L2 latency -- and cost 16 moves.)
             auto is_full = [&](int ch, int k) { return both && 8 * ch + 8 <= i && 32 * k + 32 <= i; };   // (k <= block of the chunk)
             auto is_diag = [&](int ch, int k) { return k == (ch >> 2); };
-            int t = warp, ch = 0, k = 0;
-            double xc[8], xn[8];
-#pragma unroll
-            for (int r = 0; r < 8; ++r) xn[r] = 0.0;
-            if (t < nitems) {
-                decode(t, ch, k);
-                const double* Sc = S + (size_t)(8 * ch) * M + 32 * k + lane;
-                if (is_full(ch, k)) gen_load_full(Sc, M, xc); else gen_load_masked(Sc, M, 8 * ch, 32 * k + lane, i, xc);
-            }
+            // (items of a warp: t = warp, warp + 8, ...; within segment k the chunks 4 k ... nch-1, then segment k + 1)
+            int ch = warp, k = 0;
+            while (4 * k < nch && ch >= nch) { ch = ch - nch + 4 * (k + 1); ++k; }
 #pragma unroll 1
-            while (t < nitems) {
-                const int tn = t + NW;
-                int chn = 0, kn = 0;
-                if (tn < nitems) {
-                    decode(tn, chn, kn);
-                    const double* Sn = S + (size_t)(8 * chn) * M + 32 * kn + lane;
-                    if (is_full(chn, kn)) gen_load_full(Sn, M, xn); else gen_load_masked(Sn, M, 8 * chn, 32 * kn + lane, i, xn);
+            while (4 * k < nch) {
+                double xc[8];
+                {
+                    const double* Sl = S + (size_t)(8 * ch) * M + 32 * k + lane;
+                    if (is_full(ch, k)) gen_load_full(Sl, M, xc); else gen_load_masked(Sl, M, 8 * ch, 32 * k + lane, i, xc);
                 }
                 const int j0 = 8 * ch, c = 32 * k + lane;
                 double* Sc = S + (size_t)j0 * M + c;
@@ -238,9 +227,8 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
                     if ((lane & 3) == 0 && j < i) pTw[j] += s1;
                     __syncwarp();
                 }
-#pragma unroll
-                for (int r = 0; r < 8; ++r) xc[r] = xn[r];
-                t = tn; ch = chn; k = kn;
+                ch += NW;                                                 // the warp's next item
+                while (4 * k < nch && ch >= nch) { ch = ch - nch + 4 * (k + 1); ++k; }
             }
         }
         __syncthreads();
