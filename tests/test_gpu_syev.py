@@ -695,3 +695,29 @@ def test_config5_full_sizes(lk, oracle, M):
     wo, _, _, _ = oracle.syev_batched(A[sel])
     wg = w[torch.from_numpy(sel).cuda()].cpu().numpy()
     assert (np.abs(wg - wo).max(axis=1) / np.abs(wo).max(axis=1)).max() <= parity.TOL_W
+
+
+@pytest.mark.parametrize("M,B,p", [(177, 650, 98), (255, 600, 300), (161, 700, 40)])
+def test_any_m_path_pipelined_odd_orders(lk, oracle, M, B, p):
+    """The any-M kernels (M > 160) in the pipelined regime with odd orders and a ragged last sub-chunk
+    (sub-chunks of 296 matrices): the symmetric-half reduction with its full diagonal blocks, the grouped
+    Q formation and the prefetching replay see rows and columns that are no multiple of 8 or 32; p above
+    M - 1 (no repeated eigenvalue), at the sweep's 98 and well below it (most of T falls apart).  Residual,
+    orthogonality and ordering on every matrix, eigenvalues against the oracle on a sample."""
+    import torch
+    A = wl.letkf_shaped(B, M, p, 700 + M)
+    At = torch.from_numpy(A).cuda()
+    w, V, info = lk.syev_batched(At)
+    torch.cuda.synchronize()
+    assert int(info.abs().max()) == 0
+    assert bool((w[:, 1:] >= w[:, :-1]).all())
+    Af = torch.tril(At) + torch.tril(At, -1).transpose(1, 2)
+    R = torch.matmul(Af, V) - V * w.unsqueeze(1)
+    res = float((R.flatten(1).norm(dim=1) / Af.flatten(1).norm(dim=1)).max())
+    G = torch.matmul(V.transpose(1, 2), V) - torch.eye(M, dtype=torch.float64, device="cuda")
+    assert res <= parity.TOL_RES, f"residual {res:.3e}"
+    assert float(G.abs().max()) <= parity.TOL_ORTH, f"orthogonality {float(G.abs().max()):.3e}"
+    sel = np.array([0, 295, 296, B - 1])
+    wo, _, _, _ = oracle.syev_batched(A[sel])
+    wg = w[torch.from_numpy(sel).cuda()].cpu().numpy()
+    assert (np.abs(wg - wo).max(axis=1) / np.abs(wo).max(axis=1)).max() <= parity.TOL_W
