@@ -104,7 +104,8 @@ __device__ __forceinline__ double block_sum1(double v, double* red)
 // H_i acts on indices 0..i-1), so Q = H_{M-1} ... H_1 and T = Q^T A Q.
 // A: [batch][M][M] (lower triangle read).  V: [batch][M][M] receives Q^T.  May alias.
 // (the reduction at 128 registers, two CTAs per SM: at 80 it spills and measured slower, M = 256: 13.5 against 10.4 ms)
-template <int phase>
+// KS: column segments of 32 a row of Q^T may have (ceil(M / 32) <= KS <= 8: the second phase holds rows in registers)
+template <int phase, int KS = 8>
 __global__ void __launch_bounds__(GEN_NT, 2)
 generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, int M)
 {
@@ -280,11 +281,11 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
         // by shared-memory bandwidth at one row), and the four dot products are reduced together
         const int nseg = (nc + 31) >> 5;
         for (int r0 = 4 * warp; r0 < nc; r0 += 4 * NW) {
-            double x[4][8];
+            double x[4][KS];
 #pragma unroll
             for (int rr = 0; rr < 4; ++rr)
 #pragma unroll
-                for (int k = 0; k < 8; ++k) {
+                for (int k = 0; k < KS; ++k) {
                     const int c = lane + 32 * k;
                     x[rr][k] = (k < nseg && c < nc && r0 + rr < nc) ? S[(size_t)(r0 + rr) * M + c] : 0.0;
                 }
@@ -292,9 +293,9 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
                 const double tau = taus[i0 + t];
                 if (tau == 0.0) continue;
                 const double* vt = vk + t * M;
-                double v[8], a[4] = {0.0, 0.0, 0.0, 0.0};
+                double v[KS], a[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
-                for (int k = 0; k < 8; ++k) {
+                for (int k = 0; k < KS; ++k) {
                     const int c = lane + 32 * k;
                     v[k] = (k < nseg && c < nc) ? vt[c] : 0.0;
 #pragma unroll
@@ -313,13 +314,13 @@ generic_tridiag_formq(const double* __restrict__ A_, double* V_, Workspace ws, i
                 for (int rr = 0; rr < 4; ++rr) {
                     const double ar = __shfl_sync(0xffffffffu, s1, 8 * rr);
 #pragma unroll
-                    for (int k = 0; k < 8; ++k) x[rr][k] = fma(-ar, v[k], x[rr][k]);
+                    for (int k = 0; k < KS; ++k) x[rr][k] = fma(-ar, v[k], x[rr][k]);
                 }
             }
 #pragma unroll
             for (int rr = 0; rr < 4; ++rr)
 #pragma unroll
-                for (int k = 0; k < 8; ++k) {
+                for (int k = 0; k < KS; ++k) {
                     const int c = lane + 32 * k;
                     if (k < nseg && c < nc && r0 + rr < nc) S[(size_t)(r0 + rr) * M + c] = x[rr][k];
                 }

@@ -414,7 +414,9 @@ static int stage_T(const double* A, int M, int n, double* V, Workspace ws, cudaS
     const size_t td_smem = sizeof(double) * ((4 + GEN_QK + 1) * (size_t)M + GEN_NT / 32);   // v, w, p, taus; vk[GEN_QK][M] shared with v' + pT[8][M]
     // two launches of one kernel (phase 1: the reduction, phase 2: Q^T from the reflectors), so that each shows in the records
     KLAUNCH("generic_tridiag", st, generic_tridiag_formq<1><<<n, GEN_NT, td_smem, st>>>(A, V, ws, M));
-    KLAUNCH("generic_formq", st, generic_tridiag_formq<2><<<n, GEN_NT, td_smem, st>>>(A, V, ws, M));
+    if (M <= 192) KLAUNCH("generic_formq", st, (generic_tridiag_formq<2, 6><<<n, GEN_NT, td_smem, st>>>(A, V, ws, M)));
+    else if (M <= 224) KLAUNCH("generic_formq", st, (generic_tridiag_formq<2, 7><<<n, GEN_NT, td_smem, st>>>(A, V, ws, M)));
+    else KLAUNCH("generic_formq", st, (generic_tridiag_formq<2, 8><<<n, GEN_NT, td_smem, st>>>(A, V, ws, M)));
     return 0;
 }
 
