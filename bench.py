@@ -532,7 +532,7 @@ def run_ours(args):
             del hp, Xa_pin
             letkf.host_release()
             # ---- the analysis above the register kernels (a1/a2 and a6-a9 are launches of their own there:
-            # generic_gram -> EVD -> generic_epilogue), the sweep's batch sizes
+            # big_gram (FP64 tensor cores) -> EVD -> generic_epilogue), the sweep's batch sizes
             line["analysis_large"] = []
             for Ml in (128, 256):
                 Bl = wl.sweep_batch(Ml)
