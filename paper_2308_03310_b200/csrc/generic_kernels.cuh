@@ -661,6 +661,7 @@ generic_gram(const double* __restrict__ Yb_, const double* __restrict__ d_,
 // the rows of dX over all n: t and T1, no reduction across threads), once by rows (a warp per row m, the 1 + ns dot
 // products of a row reduced eight at a time by a halving butterfly).  c_s = dX[s] . wbar is taken as
 // sum_k (dX V)[s][k] t[k], the same number up to rounding, so that it is known before the second pass.
+template <bool WANTW>
 __device__ __forceinline__ void
 generic_epilogue_one(const double* __restrict__ V_, const double* __restrict__ lam_,
                      const double* __restrict__ g_, const double* Xb_, int M, int ns,
@@ -772,7 +773,7 @@ generic_epilogue_one(const double* __restrict__ V_, const double* __restrict__ l
         const int sI = idx / M;
         Xa[idx] = xbar[sI] + cs[sI] + dX[idx];
     }
-    if (W_) {                                                  // Eq.15, 16x16 threads x (4x4)
+    if (WANTW && W_) {                                         // Eq.15, 16x16 threads x (4x4)
         double* W = W_ + b * (size_t)M * M;
         const int tx = tid & 15, ty = tid >> 4;
         for (int m0 = 0; m0 < M; m0 += 64)
@@ -809,6 +810,8 @@ generic_epilogue_one(const double* __restrict__ V_, const double* __restrict__ l
 
 // Grid-stride over the n grid points of the pass.  flags != NULL: only the points whose EVD was
 // finished by the slow path (the others had a6-a9 fused into fast_apply).
+// (WANTW = false: the common case compiles without the W product and its 16 accumulators)
+template <bool WANTW>
 __global__ void __launch_bounds__(256)
 generic_epilogue(const double* __restrict__ V_, const double* __restrict__ lam_,
                  const double* __restrict__ g_, const double* Xb_, int M, int ns, int n,
@@ -817,7 +820,7 @@ generic_epilogue(const double* __restrict__ V_, const double* __restrict__ lam_,
 {
     if (!flags) {
         for (size_t b = blockIdx.x; b < (size_t)n; b += gridDim.x) {
-            generic_epilogue_one(V_, lam_, g_, Xb_, M, ns, Xa_, W_, wbar_, b);
+            generic_epilogue_one<WANTW>(V_, lam_, g_, Xb_, M, ns, Xa_, W_, wbar_, b);
             __syncthreads();
         }
         return;
@@ -829,7 +832,7 @@ generic_epilogue(const double* __restrict__ V_, const double* __restrict__ lam_,
         const size_t end = (base + 256 < (size_t)n) ? base + 256 : (size_t)n;
         for (size_t b = base; b < end; ++b) {
             if (!flags[b]) continue;
-            generic_epilogue_one(V_, lam_, g_, Xb_, M, ns, Xa_, W_, wbar_, b);
+            generic_epilogue_one<WANTW>(V_, lam_, g_, Xb_, M, ns, Xa_, W_, wbar_, b);
             __syncthreads();
         }
     }
