@@ -661,7 +661,7 @@ generic_gram(const double* __restrict__ Yb_, const double* __restrict__ d_,
 // the rows of dX over all n: t and T1, no reduction across threads), once by rows (a warp per row m, the 1 + ns dot
 // products of a row reduced eight at a time by a halving butterfly).  c_s = dX[s] . wbar is taken as
 // sum_k (dX V)[s][k] t[k], the same number up to rounding, so that it is known before the second pass.
-template <bool WANTW>
+template <bool WANTW, int KS>
 __device__ __forceinline__ void
 generic_epilogue_one(const double* __restrict__ V_, const double* __restrict__ lam_,
                      const double* __restrict__ g_, const double* Xb_, int M, int ns,
@@ -727,21 +727,23 @@ generic_epilogue_one(const double* __restrict__ V_, const double* __restrict__ l
     }
     __syncthreads();                                          // (dX is dead from here on: its rows receive dX W)
     // second pass, by rows: wbar[m] = V[m] . t and (dX W)[s][m] = T1[s] . V[m]
-    const int KJ = (M + 31) >> 5;
-    for (int m = warp; m < M; m += 8) {
-        double x[8];
+    int kidx[KS];                                             // this lane's columns (clamped: x is 0 beyond M)
 #pragma unroll
-        for (int j = 0; j < 8; ++j) { const int k = lane + 32 * j; x[j] = (j < KJ && k < M) ? V[(size_t)m * M + k] : 0.0; }
+    for (int j = 0; j < KS; ++j) kidx[j] = min(lane + 32 * j, M - 1);
+    for (int m = warp; m < M; m += 8) {
+        double x[KS];
+#pragma unroll
+        for (int j = 0; j < KS; ++j) { const int k = lane + 32 * j; x[j] = (k < M) ? V[(size_t)m * M + k] : 0.0; }
         for (int v0 = 0; v0 < 1 + ns; v0 += 8) {
             const int nv = min(8, 1 + ns - v0);
             double q[8];
 #pragma unroll
             for (int u = 0; u < 8; ++u) {
                 q[u] = 0.0;
-                if (u < nv) {
+                if (u < nv) {                                 // warp-uniform
                     const double* tv = (v0 + u == 0) ? t : T1 + (size_t)(v0 + u - 1) * M;
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) { const int k = lane + 32 * j; if (j < KJ && k < M) q[u] = fma(x[j], tv[k], q[u]); }
+                    for (int j = 0; j < KS; ++j) q[u] = fma(x[j], tv[kidx[j]], q[u]);
                 }
             }
             double a4[4], b2[2];                                  // eight sums over 32 lanes: lane l ends with sum l / 4
@@ -810,8 +812,9 @@ generic_epilogue_one(const double* __restrict__ V_, const double* __restrict__ l
 
 // Grid-stride over the n grid points of the pass.  flags != NULL: only the points whose EVD was
 // finished by the slow path (the others had a6-a9 fused into fast_apply).
-// (WANTW = false: the common case compiles without the W product and its 16 accumulators)
-template <bool WANTW>
+// (WANTW = false: the common case compiles without the W product and its 16 accumulators; KS >= ceil(M / 32): the
+// 32-column segments of a row of V a lane holds in the second pass)
+template <bool WANTW, int KS>
 __global__ void __launch_bounds__(256)
 generic_epilogue(const double* __restrict__ V_, const double* __restrict__ lam_,
                  const double* __restrict__ g_, const double* Xb_, int M, int ns, int n,
@@ -820,7 +823,7 @@ generic_epilogue(const double* __restrict__ V_, const double* __restrict__ lam_,
 {
     if (!flags) {
         for (size_t b = blockIdx.x; b < (size_t)n; b += gridDim.x) {
-            generic_epilogue_one<WANTW>(V_, lam_, g_, Xb_, M, ns, Xa_, W_, wbar_, b);
+            generic_epilogue_one<WANTW, KS>(V_, lam_, g_, Xb_, M, ns, Xa_, W_, wbar_, b);
             __syncthreads();
         }
         return;
@@ -832,7 +835,7 @@ generic_epilogue(const double* __restrict__ V_, const double* __restrict__ lam_,
         const size_t end = (base + 256 < (size_t)n) ? base + 256 : (size_t)n;
         for (size_t b = base; b < end; ++b) {
             if (!flags[b]) continue;
-            generic_epilogue_one<WANTW>(V_, lam_, g_, Xb_, M, ns, Xa_, W_, wbar_, b);
+            generic_epilogue_one<WANTW, KS>(V_, lam_, g_, Xb_, M, ns, Xa_, W_, wbar_, b);
             __syncthreads();
         }
     }

@@ -1027,8 +1027,13 @@ static int analysis_core(const double* Yb, const double* d, const double* rinv_l
     cudaError_t ce;
     const size_t ep_smem = sizeof(double) * (3 * (size_t)M + 2 * (size_t)nstate + 2 * (size_t)nstate * M);
     if (ep_smem > 200 * 1024) return -7;
-    if ((ce = allow_smem(generic_epilogue<true>, ep_smem)) != cudaSuccess) return (int)ce;
-    if ((ce = allow_smem(generic_epilogue<false>, ep_smem)) != cudaSuccess) return (int)ce;
+    auto epi_kernel = [&](bool wantW) {
+        const int ks = (M + 31) / 32;
+        if (wantW) return ks <= 2 ? generic_epilogue<true, 2> : (ks <= 4 ? generic_epilogue<true, 4> : (ks <= 6 ? generic_epilogue<true, 6> : generic_epilogue<true, 8>));
+        return ks <= 2 ? generic_epilogue<false, 2> : (ks <= 4 ? generic_epilogue<false, 4> : (ks <= 6 ? generic_epilogue<false, 6> : generic_epilogue<false, 8>));
+    };
+    auto epi = epi_kernel(W != nullptr);
+    if ((ce = allow_smem(epi, ep_smem)) != cudaSuccess) return (int)ce;
     const PassHooks* hooks = t_hooks;
 
     auto stageT = [&](int b0, int nk, int s0, int l0, cudaStream_t s) {
@@ -1066,7 +1071,7 @@ static int analysis_core(const double* Yb, const double* d, const double* rinv_l
     auto post = [&](int b0, int nk, int s0, int l0, cudaStream_t s) -> int {
         if (!fused) {
             KLAUNCH("generic_epilogue", s,
-                    (W ? generic_epilogue<true> : generic_epilogue<false>)<<<nk, 256, ep_smem, s>>>(
+                    epi<<<nk, 256, ep_smem, s>>>(
                         Vbuf + (size_t)s0 * M * M, lam + (size_t)s0 * M, gbuf + (size_t)s0 * M,
                         Xb + (size_t)b0 * nstate * M, M, nstate, nk, Xa + (size_t)b0 * nstate * M,
                         W ? W + (size_t)b0 * M * M : nullptr, wbar ? wbar + (size_t)b0 * M : nullptr, nullptr));
