@@ -297,8 +297,8 @@ int letkf_last_launch_count(void);
  *                   32 x 32 problem by one warp per matrix (default 1; 0 = one kernel)
  *   "mid_split"     64 < M <= 128: the reduction stops after pivot 64 and its trailing 64 x 64 block goes through the
  *                   register kernels of the M <= 64 path (1, default; 0 = one kernel down to pivot 1)
- *   "mid_reg"       64 < M <= 160: reduction with the matrix in shared memory (0) / in registers up to M = 128 (1,
- *                   default) / in registers (2)
+ *   "mid_reg"       64 < M <= 160: reduction with the matrix in shared memory (0) / in registers up to M = 128 and by the
+ *                   any-M kernels above (1, default) / in registers (2)
  *   "host_pass"     matrices per pass of the host entry points (0 = what a 16 GiB staging arena holds)
  * Returns 0, or -1 for an unknown name. */
 int letkf_set_option(const char* name, int value);

@@ -379,7 +379,9 @@ static int stage_T(const double* A, int M, int n, double* V, Workspace ws, cudaS
                 generic_gram<<<n, 256, 0, st>>>(gram->Yb, gram->d, gram->r, M, gram->p, gram->shift, V, gram->gout));
         A = V;
     }
-    if (use_mid(M)) {                                    // matrix resident in shared memory
+    // (128 < M <= 160: the any-M reduction below, 7.1 + 3.0 ms at M = 160 against 10.5 ms for the shared-memory one; the
+    // replay stays mid_apply's)
+    if (use_mid(M) && (M <= 128 || t_opt.mid_reg == 0 || t_opt.mid_reg == 2)) {   // matrix resident in registers / shared memory
         cudaError_t ce;
         const size_t smem = mid_tridiag_smem(M);
         const int mt = mid_threads(M);
